@@ -1,0 +1,212 @@
+/* adept.h -- C ABI of the B200-native EM-shower transport library (libadept_b200.so).
+ *
+ * The boundary follows the paper's problem statement: the library "takes particles ... as input and
+ * gives back the energy depositions and any 'outgoing' particles", processes a buffered
+ * batch and returns hits "in arrays transferred back from the device to the host at the
+ * end of each event".  Entry-point names are those of BASELINE.json:north_star /
+ * SURVEY.md §8(b).
+ *
+ * Conventions
+ *  - Units: MeV, cm, tesla.  All physics state is IEEE double.
+ *  - Every pointer argument is a HOST pointer unless its name starts with d_ (device pointer).
+ *  - Inputs are caller-owned and copied during the call; outputs are caller-owned buffers.
+ *  - The only device memory the library uses for transport is the caller's workspace (allocated by
+ *    the caller, e.g. with PyTorch); the library owns nothing after adept_shutdown.
+ *  - Every call returns an int status: ADEPT_OK or a negative error.  No call throws or aborts;
+ *    adept_last_error() returns a static, thread-local description of the last failure.
+ *  - `cuda_stream` arguments are cudaStream_t values passed as void* (NULL = the legacy default stream).
+ *  - Species codes: 0 = e-, 1 = e+, 2 = gamma.
+ */
+#ifndef ADEPT_H
+#define ADEPT_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  ADEPT_OK = 0,
+  ADEPT_EINVAL = -1,    /* bad argument (null pointer, index out of range, malformed geometry)      */
+  ADEPT_ENOMEM = -2,    /* workspace too small / host allocation failed                            */
+  ADEPT_EOVERFLOW = -3, /* a track queue of the slot overflowed; the slot's results are invalid    */
+  ADEPT_ECUDA = -4,     /* a CUDA runtime call failed                                              */
+  ADEPT_ESTATE = -5     /* call not valid in this state (e.g. slot still holds live tracks)        */
+};
+
+enum { ADEPT_ELECTRON = 0, ADEPT_POSITRON = 1, ADEPT_GAMMA = 2 };
+enum { ADEPT_BOX = 0, ADEPT_TUBE = 1 };
+enum { ADEPT_FIELD_NONE = 0, ADEPT_FIELD_UNIFORM = 1, ADEPT_FIELD_MAP_RZ = 2 };
+enum { ADEPT_NAV_LOOP = 0, ADEPT_NAV_BVH = 1 };
+
+/* Outcome of one step. */
+enum {
+  ADEPT_OUT_BOUNDARY = 0, ADEPT_OUT_COMPTON = 1, ADEPT_OUT_PAIR = 2, ADEPT_OUT_PHOTO = 3,
+  ADEPT_OUT_BREM = 4, ADEPT_OUT_IONI = 5, ADEPT_OUT_ANNI = 6, ADEPT_OUT_STOPPED = 7,
+  ADEPT_OUT_TRUNCATED = 8, ADEPT_OUT_LOSS = 9, ADEPT_OUT_ESCAPED = 10, ADEPT_OUT_KILLED = 11,
+  ADEPT_OUT_CLOSED = 12, ADEPT_N_OUTCOMES = 13
+};
+
+/* Geometry: a tree of placed solids, every logical volume placed once, so
+ * the index into these arrays (the touchable id) is the whole navigation state.
+ * Volume 0 is the world.  The daughters of a volume are contiguous, in index order, and lie fully
+ * inside it; siblings are disjoint.  rot/trans are the GLOBAL transform of the touchable:
+ * local = rot^T (global - trans), rot row-major with the local axes as columns. */
+typedef struct {
+  int32_t n_volumes;
+  const int32_t* solid;          /* [n]    ADEPT_BOX | ADEPT_TUBE                                  */
+  const double* dims;            /* [n][3] box: half lengths; tube: rmin, rmax, half length z      */
+  const int32_t* material;       /* [n]    index into the material arrays                          */
+  const int32_t* mother;         /* [n]    -1 for the world                                        */
+  const int32_t* daughter_begin; /* [n]                                                            */
+  const int32_t* daughter_count; /* [n]                                                            */
+  const double* rot;             /* [n][9]                                                         */
+  const double* trans;           /* [n][3]                                                         */
+} adept_geometry;
+
+/* Per-material scalars. */
+typedef struct {
+  double X0;      /* radiation length [cm]                       */
+  double e_cut;   /* T_c: e-/e+ production cut [MeV]             */
+  double g_cut;   /* k_c: gamma production cut [MeV]             */
+  double B_K;     /* K-shell binding energy [MeV]                */
+  double n_el;    /* electron density [1/cm^3]                   */
+  double vacuum;  /* 1.0 for vacuum (no physics), else 0.0       */
+  double Z;
+  double rho;
+} adept_material;
+
+/* The 12 tables of every material on the 2048-point grid uniform in ln T from 1 keV to 100 TeV
+ * (SURVEY.md §8(c) M6): gamma {Compton, pair, photoelectric}; e- {brem, Moller, dE/dx, range};
+ * e+ {brem, Bhabha, annihilation, dE/dx, range}.  Macroscopic cross sections in 1/cm. */
+#define ADEPT_N_TABLES 12
+#define ADEPT_N_GRID 2048
+typedef struct {
+  const double* data; /* [n_materials][12][2048] */
+} adept_tables;
+
+/* Magnetic field.  MAP_RZ: B = (0, 0, bz(r, z)), bilinear, clamped outside. */
+typedef struct {
+  int32_t kind;
+  double B[3];       /* ADEPT_FIELD_UNIFORM */
+  int32_t nr, nz;    /* ADEPT_FIELD_MAP_RZ  */
+  double r0, z0, dr, dz;
+  const double* bz;  /* [nz][nr] */
+} adept_field;
+
+typedef struct {
+  double delta_chord;      /* max sagitta of a chord [cm], default 1e-3               */
+  double eps_push;         /* boundary push [cm], default 1e-7                       */
+  double alpha_R, rho_R;   /* continuous-loss step function, 0.2 and 0.1 cm          */
+  int32_t chord_budget;    /* chords per step before truncation, 16     */
+  uint32_t seed;           /* Philox key word 1                                      */
+  uint32_t max_steps;      /* a track is killed after this many steps, 1e6           */
+  int32_t navigator;       /* ADEPT_NAV_LOOP | ADEPT_NAV_BVH                                        */
+  int32_t n_event_slots;   /* independent transport contexts (config 5)                */
+  int32_t sync_interval;   /* population-step iterations launched between host checks               */
+  uint64_t track_capacity; /* per slot, per species: entries of each of the two track buffers       */
+  uint64_t leak_capacity;  /* per slot: tracks that left the world kept for adept_read_leaked       */
+  int32_t split_kernels;   /* 0: one step kernel per species group; 1: + relocation/interaction kernels */
+  int32_t reserved;
+} adept_config;
+
+typedef struct {
+  double pos[3];
+  double dir[3];
+  double ekin;
+  uint64_t id;
+  uint32_t event;
+  uint32_t step;
+  uint32_t volume;
+  int32_t species;
+} adept_track;
+
+typedef struct {
+  adept_track post; /* state after the step (meaningful if alive)                        */
+  int32_t alive;
+  int32_t outcome;  /* ADEPT_OUT_*                                                       */
+  int32_t n_sec;    /* secondaries created (0..2)                                        */
+  int32_t chords;
+  double s;         /* path length of the step                                           */
+  double edep_dep;  /* continuous loss scored in the pre-step volume                     */
+  double edep_cut;  /* below-cut / binding / stopped energy scored in the same volume    */
+  double escaped;
+  double killed;
+} adept_step_result;
+
+typedef struct {
+  double deposited, below_cut, escaped, killed, primary;
+} adept_ledger;
+
+typedef struct {
+  uint64_t steps[3];                    /* per species                                    */
+  uint64_t outcomes[ADEPT_N_OUTCOMES];
+  uint64_t secondaries[3];              /* created, per species                           */
+  uint64_t chords;
+  uint64_t iterations;                  /* population steps executed                      */
+  uint64_t peak_population;             /* max live tracks over iterations                */
+  uint64_t launches;                    /* kernels launched by adept_transport            */
+} adept_stats;
+
+typedef struct adept_ctx adept_ctx;
+
+const char* adept_last_error(void);
+
+/* Fills *cfg with the defaults listed above (n_event_slots 1, BVH navigator, capacity 1<<20). */
+void adept_default_config(adept_config* cfg);
+
+/* Bytes of device workspace adept_init needs for this configuration (0 on invalid input). */
+size_t adept_workspace_bytes(const adept_config*, const adept_geometry*, int n_materials, const adept_field*);
+
+/* Builds the device image (volumes, per-volume BVHs, interleaved table slices, field map)
+ * inside d_workspace and returns a context.  ADEPT_EINVAL on malformed geometry, ADEPT_ENOMEM if
+ * workspace_bytes < adept_workspace_bytes(...). */
+int adept_init(adept_ctx** out, const adept_geometry*, const adept_material* mats, int n_mats,
+               const adept_tables*, const adept_field*, const adept_config*, void* d_workspace,
+               size_t workspace_bytes);
+
+/* Appends n primaries of one event to a slot; track ids are 0..n-1 (call once per event).  Primaries
+ * are placed at Locate(pos + eps_push dir); one outside the world is ADEPT_EINVAL.
+ * pos3/dir3 are [n][3]. Synchronous with respect to the host buffers. */
+int adept_enqueue_primaries(adept_ctx*, int event_slot, uint32_t event_id, int n, const int8_t* species,
+                            const double* pos3, const double* dir3, const double* ekin);
+
+/* Same, for primaries of many events in one call: event_ids[n], track_ids[n]. */
+int adept_enqueue_batch(adept_ctx*, int event_slot, int n, const uint32_t* event_ids, const uint64_t* track_ids,
+                        const int8_t* species, const double* pos3, const double* dir3, const double* ekin);
+
+/* Steps the slot's whole population until its queues are empty.  Kernels run on
+ * cuda_stream (plus library-owned helper streams ordered after it); returns when the slot is empty. */
+int adept_transport(adept_ctx*, int event_slot, void* cuda_stream);
+
+/* Transports several slots concurrently, slot i on streams[i] (config 5). */
+int adept_transport_many(adept_ctx*, int n_slots, const int* event_slots, void* const* cuda_streams);
+
+/* Copies the slot's per-volume energy deposit (n_volumes doubles, indexed by touchable id) and its
+ * ledger to the host, then zeroes them on the device. */
+int adept_read_scoring(adept_ctx*, int event_slot, double* edep_per_volume, size_t n_volumes,
+                       adept_ledger* ledger, void* cuda_stream);
+
+/* Tracks that left the world ("outgoing particles"): up to cap of them; *n = number
+ * that leaked (may exceed cap).  Resets the slot's leak buffer. */
+int adept_read_leaked(adept_ctx*, int event_slot, adept_track* out, size_t cap, size_t* n);
+
+int adept_get_stats(adept_ctx*, int event_slot, adept_stats* out);
+
+/* Test hook: exactly one step for each of n tracks, results in input order; secondaries[2*i + k]. */
+int adept_step_frozen(adept_ctx*, int n, const adept_track* in, adept_step_result* out,
+                      adept_track* secondaries, void* cuda_stream);
+
+/* Test hooks for navigation: distance to boundary and Locate for n rays/points,
+ * with the navigator chosen here regardless of the configuration. */
+int adept_distance_batch(adept_ctx*, int navigator, int n, const double* pos3, const double* dir3,
+                         const uint32_t* volume, const double* s_max, double* out, void* cuda_stream);
+int adept_locate_batch(adept_ctx*, int navigator, int n, const double* pos3, int64_t* out, void* cuda_stream);
+
+int adept_shutdown(adept_ctx*);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

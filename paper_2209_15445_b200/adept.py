@@ -1,0 +1,238 @@
+"""Thin ctypes binding of libadept_b200.so (include/adept.h): argument marshalling only.
+
+Every step of the transport path runs inside the CUDA library; PyTorch supplies the device
+workspace and the streams (BASELINE.json:north_star).  There is no CPU fallback: importing this
+module fails loudly when the library is missing or cannot be loaded.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libadept_b200.so")
+
+OK, EINVAL, ENOMEM, EOVERFLOW, ECUDA, ESTATE = 0, -1, -2, -3, -4, -5
+NAV_LOOP, NAV_BVH = 0, 1
+OUTCOMES = ["boundary", "compton", "pair", "photo", "brem", "ioni", "anni", "stopped", "truncated", "loss",
+            "escaped", "killed", "closed"]
+
+TRACK = np.dtype([("pos", "f8", 3), ("dir", "f8", 3), ("ekin", "f8"), ("id", "u8"), ("event", "u4"),
+                  ("step", "u4"), ("volume", "u4"), ("species", "i4")], align=True)
+RESULT = np.dtype([("post", TRACK), ("alive", "i4"), ("outcome", "i4"), ("n_sec", "i4"), ("chords", "i4"),
+                   ("s", "f8"), ("edep_dep", "f8"), ("edep_cut", "f8"), ("escaped", "f8"), ("killed", "f8")],
+                  align=True)
+
+_dp, _ip = C.POINTER(C.c_double), C.POINTER(C.c_int32)
+
+
+class CGeometry(C.Structure):
+    _fields_ = [("n_volumes", C.c_int32), ("solid", _ip), ("dims", _dp), ("material", _ip), ("mother", _ip),
+                ("daughter_begin", _ip), ("daughter_count", _ip), ("rot", _dp), ("trans", _dp)]
+
+
+class CTables(C.Structure):
+    _fields_ = [("data", _dp)]
+
+
+class CField(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("B", C.c_double * 3), ("nr", C.c_int32), ("nz", C.c_int32),
+                ("r0", C.c_double), ("z0", C.c_double), ("dr", C.c_double), ("dz", C.c_double), ("bz", _dp)]
+
+
+class CConfig(C.Structure):
+    _fields_ = [("delta_chord", C.c_double), ("eps_push", C.c_double), ("alpha_R", C.c_double), ("rho_R", C.c_double),
+                ("chord_budget", C.c_int32), ("seed", C.c_uint32), ("max_steps", C.c_uint32), ("navigator", C.c_int32),
+                ("n_event_slots", C.c_int32), ("sync_interval", C.c_int32), ("track_capacity", C.c_uint64),
+                ("leak_capacity", C.c_uint64), ("split_kernels", C.c_int32), ("reserved", C.c_int32)]
+
+
+class CLedger(C.Structure):
+    _fields_ = [(n, C.c_double) for n in ("deposited", "below_cut", "escaped", "killed", "primary")]
+
+    def total(self):
+        return self.deposited + self.below_cut + self.escaped + self.killed
+
+
+class CStats(C.Structure):
+    _fields_ = [("steps", C.c_uint64 * 3), ("outcomes", C.c_uint64 * 13), ("secondaries", C.c_uint64 * 3),
+                ("chords", C.c_uint64), ("iterations", C.c_uint64), ("peak_population", C.c_uint64),
+                ("launches", C.c_uint64)]
+
+
+EXPORTS = ["adept_last_error", "adept_default_config", "adept_workspace_bytes", "adept_init",
+           "adept_enqueue_primaries", "adept_enqueue_batch", "adept_transport", "adept_transport_many",
+           "adept_read_scoring", "adept_read_leaked", "adept_get_stats", "adept_step_frozen",
+           "adept_distance_batch", "adept_locate_batch", "adept_shutdown"]
+
+
+def load_library():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2209_15445_b200.build` "
+                          "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, i, sz = C.c_void_p, C.c_int, C.c_size_t
+    lib.adept_last_error.restype = C.c_char_p
+    lib.adept_default_config.argtypes = [C.POINTER(CConfig)]
+    lib.adept_workspace_bytes.restype = sz
+    lib.adept_workspace_bytes.argtypes = [C.POINTER(CConfig), C.POINTER(CGeometry), i, C.POINTER(CField)]
+    lib.adept_init.argtypes = [C.POINTER(vp), C.POINTER(CGeometry), vp, i, C.POINTER(CTables), C.POINTER(CField),
+                               C.POINTER(CConfig), vp, sz]
+    lib.adept_enqueue_primaries.argtypes = [vp, i, C.c_uint32, i, vp, vp, vp, vp]
+    lib.adept_enqueue_batch.argtypes = [vp, i, i, vp, vp, vp, vp, vp, vp]
+    lib.adept_transport.argtypes = [vp, i, vp]
+    lib.adept_transport_many.argtypes = [vp, i, vp, vp]
+    lib.adept_read_scoring.argtypes = [vp, i, vp, sz, C.POINTER(CLedger), vp]
+    lib.adept_read_leaked.argtypes = [vp, i, vp, sz, C.POINTER(sz)]
+    lib.adept_get_stats.argtypes = [vp, i, C.POINTER(CStats)]
+    lib.adept_step_frozen.argtypes = [vp, i, vp, vp, vp, vp]
+    lib.adept_distance_batch.argtypes = [vp, i, i, vp, vp, vp, vp, vp, vp]
+    lib.adept_locate_batch.argtypes = [vp, i, i, vp, vp, vp]
+    lib.adept_shutdown.argtypes = [vp]
+    return lib
+
+
+lib = load_library()
+
+
+class AdeptError(RuntimeError):
+    def __init__(self, code):
+        self.code = code
+        super().__init__(f"adept error {code}: {lib.adept_last_error().decode()}")
+
+
+def _check(code):
+    if code != OK:
+        raise AdeptError(code)
+
+
+def _ptr(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def default_config(**over):
+    cfg = CConfig()
+    lib.adept_default_config(C.byref(cfg))
+    for k, v in over.items():
+        if not hasattr(cfg, k):
+            raise TypeError(f"unknown config field {k}")
+        setattr(cfg, k, v)
+    return cfg
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        return None
+    return C.c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+
+
+class Adept:
+    """One library context.  `geom`, `field` come from paper_2209_15445_b200.inputs; `scalars` is
+    (n_mat, 8) and `tables` (n_mat, 12, 2048) as built by inputs.materials.build_material_set."""
+
+    def __init__(self, geom, tables, scalars, field, device="cuda:0", **config):
+        import torch
+        self._torch = torch
+        self.device = torch.device(device)
+        self.cfg = default_config(**config)
+        self.n_volumes = geom.n_volumes
+        self._keep = [geom, np.ascontiguousarray(tables, dtype=np.float64),
+                      np.ascontiguousarray(scalars, dtype=np.float64),
+                      np.ascontiguousarray(field.bz, dtype=np.float64)]
+        g = CGeometry(geom.n_volumes, geom.solid.ctypes.data_as(_ip), geom.dims.ctypes.data_as(_dp),
+                      geom.material.ctypes.data_as(_ip), geom.mother.ctypes.data_as(_ip),
+                      geom.daughter_begin.ctypes.data_as(_ip), geom.daughter_count.ctypes.data_as(_ip),
+                      geom.rot.ctypes.data_as(_dp), geom.trans.ctypes.data_as(_dp))
+        t = CTables(self._keep[1].ctypes.data_as(_dp))
+        f = CField(field.kind, (C.c_double * 3)(*field.B), field.nr, field.nz, field.r0, field.z0, field.dr,
+                   field.dz, self._keep[3].ctypes.data_as(_dp))
+        n_mat = self._keep[2].shape[0]
+        nbytes = lib.adept_workspace_bytes(C.byref(self.cfg), C.byref(g), n_mat, C.byref(f))
+        if nbytes == 0:
+            raise AdeptError(EINVAL)
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self.ctx = C.c_void_p()
+            _check(lib.adept_init(C.byref(self.ctx), C.byref(g), _ptr(self._keep[2]), n_mat, C.byref(t), C.byref(f),
+                                  C.byref(self.cfg), C.c_void_p(self.workspace.data_ptr()), nbytes))
+        self.workspace_bytes = nbytes
+
+    def close(self):
+        if getattr(self, "ctx", None):
+            lib.adept_shutdown(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        self.close()
+
+    # ---- primaries
+    def enqueue(self, prim, slot=0):
+        """prim: dict from inputs.primaries (event, species, pos, dir, ekin); ids = index within the event."""
+        ev = np.ascontiguousarray(prim["event"], dtype=np.uint32)
+        n = ev.shape[0]
+        first = np.r_[True, ev[1:] != ev[:-1]] if n else np.zeros(0, dtype=bool)
+        start = np.maximum.accumulate(np.where(first, np.arange(n), 0)) if n else np.zeros(0, dtype=np.int64)
+        ids = (np.arange(n) - start).astype(np.uint64)
+        self.enqueue_batch(ev, ids, prim["species"], prim["pos"], prim["dir"], prim["ekin"], slot)
+
+    def enqueue_batch(self, event_ids, track_ids, species, pos, direc, ekin, slot=0):
+        a = [np.ascontiguousarray(event_ids, dtype=np.uint32), np.ascontiguousarray(track_ids, dtype=np.uint64),
+             np.ascontiguousarray(species, dtype=np.int8), np.ascontiguousarray(pos, dtype=np.float64),
+             np.ascontiguousarray(direc, dtype=np.float64), np.ascontiguousarray(ekin, dtype=np.float64)]
+        _check(lib.adept_enqueue_batch(self.ctx, slot, a[0].shape[0], *[_ptr(x) for x in a]))
+
+    def enqueue_primaries(self, slot, event_id, species, pos, direc, ekin):
+        a = [np.ascontiguousarray(species, dtype=np.int8), np.ascontiguousarray(pos, dtype=np.float64),
+             np.ascontiguousarray(direc, dtype=np.float64), np.ascontiguousarray(ekin, dtype=np.float64)]
+        _check(lib.adept_enqueue_primaries(self.ctx, slot, event_id, a[0].shape[0], *[_ptr(x) for x in a]))
+
+    # ---- transport
+    def transport(self, slot=0, stream=None):
+        _check(lib.adept_transport(self.ctx, slot, _stream_ptr(stream)))
+
+    def transport_many(self, slots, streams):
+        s = (C.c_int * len(slots))(*slots)
+        p = (C.c_void_p * len(slots))(*[st.cuda_stream if hasattr(st, "cuda_stream") else int(st) for st in streams])
+        _check(lib.adept_transport_many(self.ctx, len(slots), s, p))
+
+    def read_scoring(self, slot=0, stream=None, out=None):
+        edep = out if out is not None else np.zeros(self.n_volumes)
+        led = CLedger()
+        _check(lib.adept_read_scoring(self.ctx, slot, _ptr(edep), self.n_volumes, C.byref(led), _stream_ptr(stream)))
+        return edep, led
+
+    def read_leaked(self, slot=0, cap=1 << 16):
+        out = np.zeros(cap, dtype=TRACK)
+        n = C.c_size_t(0)
+        _check(lib.adept_read_leaked(self.ctx, slot, _ptr(out), cap, C.byref(n)))
+        return out[:min(n.value, cap)], n.value
+
+    def stats(self, slot=0):
+        s = CStats()
+        _check(lib.adept_get_stats(self.ctx, slot, C.byref(s)))
+        return s
+
+    # ---- test hooks
+    def step_frozen(self, tracks, stream=None):
+        tracks = np.ascontiguousarray(tracks, dtype=TRACK)
+        n = tracks.shape[0]
+        res = np.zeros(n, dtype=RESULT)
+        sec = np.zeros((n, 2), dtype=TRACK)
+        _check(lib.adept_step_frozen(self.ctx, n, _ptr(tracks), _ptr(res), _ptr(sec), _stream_ptr(stream)))
+        return res, sec
+
+    def distance_batch(self, pos, direc, volume, s_max=None, navigator=NAV_BVH):
+        pos = np.ascontiguousarray(pos, dtype=np.float64).reshape(-1, 3)
+        direc = np.ascontiguousarray(direc, dtype=np.float64).reshape(-1, 3)
+        n = pos.shape[0]
+        vol = np.ascontiguousarray(np.broadcast_to(volume, (n,)), dtype=np.uint32)
+        sm = np.full(n, np.inf) if s_max is None else np.ascontiguousarray(np.broadcast_to(s_max, (n,)), dtype=np.float64)
+        out = np.zeros(n)
+        _check(lib.adept_distance_batch(self.ctx, navigator, n, _ptr(pos), _ptr(direc), _ptr(vol), _ptr(sm), _ptr(out), None))
+        return out
+
+    def locate_batch(self, pos, navigator=NAV_BVH):
+        pos = np.ascontiguousarray(pos, dtype=np.float64).reshape(-1, 3)
+        out = np.zeros(pos.shape[0], dtype=np.int64)
+        _check(lib.adept_locate_batch(self.ctx, navigator, pos.shape[0], _ptr(pos), _ptr(out), None))
+        return out

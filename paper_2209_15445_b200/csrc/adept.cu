@@ -1,0 +1,603 @@
+// Host side of the C ABI (include/adept.h): workspace carving, device image (volumes, per-volume BVH,
+// interleaved table slices, field map), primaries, the transport loop and readback.
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <numeric>
+#include <vector>
+
+#include "kernels.cuh"
+
+using namespace adept;
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+#define CUDA_TRY(expr)                                                                         \
+  do {                                                                                         \
+    cudaError_t e_ = (expr);                                                                   \
+    if (e_ != cudaSuccess) return fail(ADEPT_ECUDA, "%s: %s", #expr, cudaGetErrorString(e_));  \
+  } while (0)
+
+constexpr int kBvhMinDaughters = 65;  // below this a per-lane loop over the daughters is cheaper
+
+// Bump allocator over the caller's workspace; with base == nullptr it only measures.
+struct Carver {
+  char* base;
+  size_t off = 0;
+  explicit Carver(void* b) : base(static_cast<char*>(b)) {}
+  template <typename T>
+  T* take(size_t n) {
+    off = (off + 255) & ~static_cast<size_t>(255);
+    T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+    off += n * sizeof(T);
+    return p;
+  }
+};
+
+struct HostBvh {
+  int volume;
+  std::vector<int32_t> prim_vol;
+  std::vector<double> prim_box;                // [6][n]
+  std::vector<std::vector<double>> node_box;   // per level [6][n_nodes]
+  std::vector<int> n_nodes;
+};
+
+uint32_t morton10(uint32_t v) {
+  v &= 0x3ff;
+  v = (v | (v << 16)) & 0x030000FF;
+  v = (v | (v << 8)) & 0x0300F00F;
+  v = (v | (v << 4)) & 0x030C30C3;
+  v = (v | (v << 2)) & 0x09249249;
+  return v;
+}
+
+// World-frame AABB of a placed solid, padded so that rounding can never make it miss a true hit.
+void world_aabb(const adept_geometry* g, int v, double lo[3], double hi[3]) {
+  const double* R = g->rot + 9 * v;
+  const double* t = g->trans + 3 * v;
+  const double* d = g->dims + 3 * v;
+  const double h[3] = {g->solid[v] == ADEPT_BOX ? d[0] : d[1], g->solid[v] == ADEPT_BOX ? d[1] : d[1], d[2]};
+  for (int i = 0; i < 3; ++i) {
+    const double e = std::fabs(R[3 * i + 0]) * h[0] + std::fabs(R[3 * i + 1]) * h[1] + std::fabs(R[3 * i + 2]) * h[2];
+    const double pad = 1e-9 + 1e-12 * (std::fabs(t[i]) + e);
+    lo[i] = t[i] - e - pad;
+    hi[i] = t[i] + e + pad;
+  }
+}
+
+HostBvh build_bvh(const adept_geometry* g, int v) {
+  HostBvh b;
+  b.volume = v;
+  const int n = g->daughter_count[v], first = g->daughter_begin[v];
+  std::vector<double> lo(3 * n), hi(3 * n);
+  double glo[3] = {1e300, 1e300, 1e300}, ghi[3] = {-1e300, -1e300, -1e300};
+  for (int k = 0; k < n; ++k) {
+    world_aabb(g, first + k, &lo[3 * k], &hi[3 * k]);
+    for (int i = 0; i < 3; ++i) {
+      const double cen = 0.5 * (lo[3 * k + i] + hi[3 * k + i]);
+      glo[i] = std::min(glo[i], cen);
+      ghi[i] = std::max(ghi[i], cen);
+    }
+  }
+  std::vector<uint32_t> code(n);
+  for (int k = 0; k < n; ++k) {
+    uint32_t m = 0;
+    for (int i = 0; i < 3; ++i) {
+      const double cen = 0.5 * (lo[3 * k + i] + hi[3 * k + i]);
+      const double w = ghi[i] > glo[i] ? (cen - glo[i]) / (ghi[i] - glo[i]) : 0.0;
+      m |= morton10(static_cast<uint32_t>(std::min(1023.0, w * 1024.0))) << i;
+    }
+    code[k] = m;
+  }
+  std::vector<int> order(n);
+  std::iota(order.begin(), order.end(), 0);
+  std::stable_sort(order.begin(), order.end(), [&](int a, int c) { return code[a] < code[c]; });
+  b.prim_vol.resize(n);
+  b.prim_box.resize(6 * static_cast<size_t>(n));
+  for (int k = 0; k < n; ++k) {
+    const int src = order[k];
+    b.prim_vol[k] = first + src;
+    for (int i = 0; i < 3; ++i) {
+      b.prim_box[static_cast<size_t>(i) * n + k] = lo[3 * src + i];
+      b.prim_box[static_cast<size_t>(3 + i) * n + k] = hi[3 * src + i];
+    }
+  }
+  // levels: node k of level L = union of children [32k, 32k+32) of level L-1
+  const std::vector<double>* child = &b.prim_box;
+  int n_child = n;
+  for (;;) {
+    const int nn = (n_child + 31) / 32;
+    std::vector<double> box(6 * static_cast<size_t>(nn));
+    for (int k = 0; k < nn; ++k) {
+      for (int i = 0; i < 3; ++i) {
+        double l = 1e300, h = -1e300;
+        for (int j = 32 * k; j < std::min(32 * k + 32, n_child); ++j) {
+          l = std::min(l, (*child)[static_cast<size_t>(i) * n_child + j]);
+          h = std::max(h, (*child)[static_cast<size_t>(3 + i) * n_child + j]);
+        }
+        box[static_cast<size_t>(i) * nn + k] = l;
+        box[static_cast<size_t>(3 + i) * nn + k] = h;
+      }
+    }
+    b.node_box.push_back(std::move(box));
+    b.n_nodes.push_back(nn);
+    if (nn <= 32) break;
+    child = &b.node_box.back();
+    n_child = nn;
+  }
+  return b;
+}
+
+}  // namespace
+
+struct SlotHost {
+  DevSlot dev{};
+  cudaStream_t helper = nullptr;     // charged-species kernel runs here, forked from the caller's stream
+  cudaEvent_t fork = nullptr, join = nullptr;
+  SlotCounters* pinned = nullptr;    // host mirror of the counters
+  unsigned long long launches = 0;
+  bool live = false;
+};
+
+struct adept_ctx {
+  adept_config cfg{};
+  DevCtx dev{};
+  int n_vol = 0, n_mat = 0;
+  std::vector<SlotHost> slots;
+  adept_track* d_stage = nullptr;    // staging area for primaries (inside the workspace)
+  uint32_t* d_bad = nullptr;
+  size_t stage_cap = 0;
+  int grid_gamma = 0, grid_charged = 0;
+};
+
+extern "C" const char* adept_last_error(void) { return g_err; }
+
+extern "C" void adept_default_config(adept_config* c) {
+  if (!c) return;
+  std::memset(c, 0, sizeof(*c));
+  c->delta_chord = 1e-3; c->eps_push = 1e-7; c->alpha_R = 0.2; c->rho_R = 0.1;
+  c->chord_budget = 16; c->seed = 1; c->max_steps = 1000000;
+  c->navigator = ADEPT_NAV_BVH; c->n_event_slots = 1; c->sync_interval = 8;
+  c->track_capacity = 1u << 20; c->leak_capacity = 1u << 16; c->split_kernels = 0;
+}
+
+namespace {
+
+int validate(const adept_config* cfg, const adept_geometry* g, int n_mats, const adept_field* f) {
+  if (!cfg || !g || !f) return fail(ADEPT_EINVAL, "null argument");
+  if (g->n_volumes < 1 || n_mats < 1) return fail(ADEPT_EINVAL, "empty geometry or material list");
+  if (!g->solid || !g->dims || !g->material || !g->mother || !g->daughter_begin || !g->daughter_count || !g->rot || !g->trans)
+    return fail(ADEPT_EINVAL, "null geometry array");
+  if (cfg->n_event_slots < 1 || cfg->n_event_slots > 1024) return fail(ADEPT_EINVAL, "n_event_slots out of range");
+  if (cfg->track_capacity < 32 || cfg->track_capacity > 0x7fffffffu) return fail(ADEPT_EINVAL, "track_capacity out of range");
+  if (cfg->chord_budget < 1 || cfg->sync_interval < 1) return fail(ADEPT_EINVAL, "chord_budget / sync_interval must be >= 1");
+  if (g->mother[0] != -1) return fail(ADEPT_EINVAL, "volume 0 must be the world");
+  for (int v = 0; v < g->n_volumes; ++v) {
+    if (g->solid[v] != ADEPT_BOX && g->solid[v] != ADEPT_TUBE) return fail(ADEPT_EINVAL, "volume %d: unknown solid", v);
+    if (g->material[v] < 0 || g->material[v] >= n_mats) return fail(ADEPT_EINVAL, "volume %d: material out of range", v);
+    const int b = g->daughter_begin[v], n = g->daughter_count[v];
+    if (n < 0 || (n > 0 && (b <= v || b + n > g->n_volumes))) return fail(ADEPT_EINVAL, "volume %d: bad daughter range", v);
+    for (int k = 0; k < n; ++k)
+      if (g->mother[b + k] != v) return fail(ADEPT_EINVAL, "volume %d: daughter %d has another mother", v, b + k);
+    if (v > 0 && (g->mother[v] < 0 || g->mother[v] >= v)) return fail(ADEPT_EINVAL, "volume %d: bad mother", v);
+  }
+  if (f->kind == ADEPT_FIELD_MAP_RZ && (f->nr < 2 || f->nz < 2 || !f->bz || !(f->dr > 0) || !(f->dz > 0)))
+    return fail(ADEPT_EINVAL, "malformed field map");
+  if (f->kind < ADEPT_FIELD_NONE || f->kind > ADEPT_FIELD_MAP_RZ) return fail(ADEPT_EINVAL, "unknown field kind");
+  return ADEPT_OK;
+}
+
+struct Layout {
+  DevVolume* vol; DevBvh* bvh; double *tab_g, *tab_em, *tab_ep, *scal, *bz;
+  std::vector<double*> bvh_prim_box; std::vector<int32_t*> bvh_prim_vol; std::vector<std::vector<double*>> bvh_node_box;
+  adept_track* stage; uint32_t* bad; size_t stage_cap;
+  std::vector<DevSlot> slots;
+};
+
+// Carves (or, with base == nullptr, measures) the whole workspace.
+size_t carve(void* base, const adept_config* cfg, const adept_geometry* g, int n_mats, const adept_field* f,
+             const std::vector<HostBvh>* bvhs, Layout* out) {
+  Carver cv(base);
+  Layout L{};
+  L.vol = cv.take<DevVolume>(g->n_volumes);
+  std::vector<int> bvh_vols;
+  for (int v = 0; v < g->n_volumes; ++v) if (g->daughter_count[v] >= kBvhMinDaughters) bvh_vols.push_back(v);
+  L.bvh = cv.take<DevBvh>(std::max<size_t>(bvh_vols.size(), 1));
+  for (size_t k = 0; k < bvh_vols.size(); ++k) {
+    const int n = g->daughter_count[bvh_vols[k]];
+    L.bvh_prim_box.push_back(cv.take<double>(6 * static_cast<size_t>(n)));
+    L.bvh_prim_vol.push_back(cv.take<int32_t>(n));
+    std::vector<double*> lv;
+    int nn = n;
+    do { nn = (nn + 31) / 32; lv.push_back(cv.take<double>(6 * static_cast<size_t>(nn))); } while (nn > 32);
+    L.bvh_node_box.push_back(lv);
+  }
+  (void)bvhs;
+  L.tab_g = cv.take<double>(static_cast<size_t>(n_mats) * kNGrid * kRowG);
+  L.tab_em = cv.take<double>(static_cast<size_t>(n_mats) * kNGrid * kRowEm);
+  L.tab_ep = cv.take<double>(static_cast<size_t>(n_mats) * kNGrid * kRowEp);
+  L.scal = cv.take<double>(static_cast<size_t>(n_mats) * N_SCAL);
+  L.bz = cv.take<double>(f->kind == ADEPT_FIELD_MAP_RZ ? static_cast<size_t>(f->nr) * f->nz : 1);
+  L.stage_cap = std::min<size_t>(cfg->track_capacity, 1u << 20);
+  L.stage = cv.take<adept_track>(L.stage_cap);
+  L.bad = cv.take<uint32_t>(1);
+  const size_t cap = cfg->track_capacity;
+  for (int s = 0; s < cfg->n_event_slots; ++s) {
+    DevSlot d{};
+    for (int p = 0; p < 2; ++p)
+      for (int sp = 0; sp < 3; ++sp) {
+        TrackSoA& b = d.buf[p][sp];
+        b.x = cv.take<double>(cap); b.y = cv.take<double>(cap); b.z = cv.take<double>(cap);
+        b.dx = cv.take<double>(cap); b.dy = cv.take<double>(cap); b.dz = cv.take<double>(cap);
+        b.ekin = cv.take<double>(cap); b.id = cv.take<uint64_t>(cap);
+        b.event = cv.take<uint32_t>(cap); b.step = cv.take<uint32_t>(cap); b.vol = cv.take<uint32_t>(cap);
+      }
+    d.counters = cv.take<SlotCounters>(1);
+    d.edep = cv.take<double>(g->n_volumes);
+    d.ledger = cv.take<double>(8);
+    d.stats = cv.take<DevStats>(1);
+    d.leaked = cv.take<adept_track>(std::max<size_t>(cfg->leak_capacity, 1));
+    d.reloc_queue = cv.take<uint32_t>(cfg->split_kernels ? 3 * cap : 1);
+    d.inter_queue = cv.take<uint32_t>(cfg->split_kernels ? 3 * cap : 1);
+    L.slots.push_back(d);
+  }
+  if (out) *out = std::move(L);
+  return (cv.off + 255) & ~static_cast<size_t>(255);
+}
+
+}  // namespace
+
+extern "C" size_t adept_workspace_bytes(const adept_config* cfg, const adept_geometry* g, int n_mats, const adept_field* f) {
+  if (validate(cfg, g, n_mats, f) != ADEPT_OK) return 0;
+  return carve(nullptr, cfg, g, n_mats, f, nullptr, nullptr);
+}
+
+extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_material* mats, int n_mats,
+                          const adept_tables* tables, const adept_field* f, const adept_config* cfg, void* d_workspace,
+                          size_t workspace_bytes) {
+  if (!out || !mats || !tables || !tables->data || !d_workspace) return fail(ADEPT_EINVAL, "null argument");
+  const int rc = validate(cfg, g, n_mats, f);
+  if (rc != ADEPT_OK) return rc;
+  Layout L;
+  const size_t need = carve(d_workspace, cfg, g, n_mats, f, nullptr, &L);
+  if (workspace_bytes < need) return fail(ADEPT_ENOMEM, "workspace has %zu bytes, %zu needed", workspace_bytes, need);
+  CUDA_TRY(cudaMemset(d_workspace, 0, need));
+
+  // ---- volumes + BVHs
+  const int nv = g->n_volumes;
+  std::vector<DevVolume> hv(nv);
+  std::vector<DevBvh> hb;
+  for (int v = 0; v < nv; ++v) {
+    DevVolume& d = hv[v];
+    for (int k = 0; k < 3; ++k) { d.t[k] = g->trans[3 * v + k]; d.dims[k] = g->dims[3 * v + k]; }
+    bool ident = true;
+    for (int k = 0; k < 9; ++k) { d.R[k] = g->rot[9 * v + k]; ident = ident && d.R[k] == ((k % 4 == 0) ? 1.0 : 0.0); }
+    d.solid = g->solid[v]; d.material = g->material[v];
+    d.dbegin = g->daughter_begin[v]; d.dcount = g->daughter_count[v];
+    d.identity = ident ? 1 : 0;
+    d.bvh = -1;
+    if (d.dcount >= kBvhMinDaughters) {
+      const HostBvh b = build_bvh(g, v);
+      const size_t k = hb.size();
+      if (static_cast<int>(b.n_nodes.size()) > kBvhMaxLevels) return fail(ADEPT_EINVAL, "volume %d: too many daughters", v);
+      DevBvh db{};
+      db.n_prims = d.dcount;
+      db.n_levels = static_cast<int>(b.n_nodes.size());
+      db.prim_box = L.bvh_prim_box[k];
+      db.prim_vol = L.bvh_prim_vol[k];
+      CUDA_TRY(cudaMemcpy(L.bvh_prim_box[k], b.prim_box.data(), b.prim_box.size() * sizeof(double), cudaMemcpyHostToDevice));
+      CUDA_TRY(cudaMemcpy(L.bvh_prim_vol[k], b.prim_vol.data(), b.prim_vol.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+      for (int l = 0; l < db.n_levels; ++l) {
+        db.n_nodes[l] = b.n_nodes[l];
+        db.node_box[l] = L.bvh_node_box[k][l];
+        CUDA_TRY(cudaMemcpy(L.bvh_node_box[k][l], b.node_box[l].data(), b.node_box[l].size() * sizeof(double), cudaMemcpyHostToDevice));
+      }
+      d.bvh = static_cast<int>(k);
+      hb.push_back(db);
+    }
+  }
+  CUDA_TRY(cudaMemcpy(L.vol, hv.data(), hv.size() * sizeof(DevVolume), cudaMemcpyHostToDevice));
+  if (!hb.empty()) CUDA_TRY(cudaMemcpy(L.bvh, hb.data(), hb.size() * sizeof(DevBvh), cudaMemcpyHostToDevice));
+
+  // ---- interleaved table slices (one node = one row)
+  {
+    const size_t N = kNGrid;
+    std::vector<double> tg(n_mats * N * kRowG, 0.0), te(n_mats * N * kRowEm, 0.0), tp(n_mats * N * kRowEp, 0.0);
+    for (int m = 0; m < n_mats; ++m) {
+      const double* src = tables->data + static_cast<size_t>(m) * ADEPT_N_TABLES * N;
+      for (size_t i = 0; i < N; ++i) {
+        for (int k = 0; k < 3; ++k) tg[(m * N + i) * kRowG + k] = src[k * N + i];
+        for (int k = 0; k < 4; ++k) te[(m * N + i) * kRowEm + k] = src[(3 + k) * N + i];
+        for (int k = 0; k < 5; ++k) tp[(m * N + i) * kRowEp + k] = src[(7 + k) * N + i];
+      }
+    }
+    CUDA_TRY(cudaMemcpy(L.tab_g, tg.data(), tg.size() * sizeof(double), cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaMemcpy(L.tab_em, te.data(), te.size() * sizeof(double), cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaMemcpy(L.tab_ep, tp.data(), tp.size() * sizeof(double), cudaMemcpyHostToDevice));
+    static_assert(sizeof(adept_material) == N_SCAL * sizeof(double), "adept_material layout");
+    CUDA_TRY(cudaMemcpy(L.scal, mats, static_cast<size_t>(n_mats) * sizeof(adept_material), cudaMemcpyHostToDevice));
+  }
+  if (f->kind == ADEPT_FIELD_MAP_RZ)
+    CUDA_TRY(cudaMemcpy(L.bz, f->bz, static_cast<size_t>(f->nr) * f->nz * sizeof(double), cudaMemcpyHostToDevice));
+
+  adept_ctx* ctx = new (std::nothrow) adept_ctx;
+  if (!ctx) return fail(ADEPT_ENOMEM, "host allocation failed");
+  ctx->cfg = *cfg;
+  ctx->n_vol = nv; ctx->n_mat = n_mats;
+  DevCtx& d = ctx->dev;
+  d.vol = L.vol; d.n_vol = nv; d.bvh = L.bvh; d.navigator = cfg->navigator;
+  d.tab_g = L.tab_g; d.tab_em = L.tab_em; d.tab_ep = L.tab_ep; d.scal = L.scal; d.n_mat = n_mats;
+  d.field_kind = f->kind;
+  for (int k = 0; k < 3; ++k) d.B[k] = f->B[k];
+  d.nr = f->nr; d.nz = f->nz; d.r0 = f->r0; d.z0 = f->z0; d.dr = f->dr; d.dz = f->dz; d.bz = L.bz;
+  d.u0 = std::log(1.0e-3);
+  d.du = (std::log(1.0e8) - std::log(1.0e-3)) / (kNGrid - 1);
+  d.inv_du = 1.0 / d.du;
+  d.delta_chord = cfg->delta_chord; d.eps_push = cfg->eps_push; d.alpha_R = cfg->alpha_R; d.rho_R = cfg->rho_R;
+  d.chord_budget = cfg->chord_budget; d.seed = cfg->seed; d.max_steps = cfg->max_steps;
+  d.capacity = static_cast<uint32_t>(cfg->track_capacity);
+  d.leak_capacity = static_cast<uint32_t>(cfg->leak_capacity);
+  ctx->d_stage = L.stage; ctx->d_bad = L.bad; ctx->stage_cap = L.stage_cap;
+
+  int dev = 0, sms = 0, occ_g = 1, occ_c = 1;
+  CUDA_TRY(cudaGetDevice(&dev));
+  CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_g, step_kernel<MODE_GAMMA>, kBlock, 0));
+  CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_c, step_kernel<MODE_CHARGED>, kBlock, 0));
+  ctx->grid_gamma = sms * std::max(occ_g, 1);
+  ctx->grid_charged = sms * std::max(occ_c, 1);
+
+  ctx->slots.resize(cfg->n_event_slots);
+  for (int s = 0; s < cfg->n_event_slots; ++s) {
+    SlotHost& sh = ctx->slots[s];
+    sh.dev = L.slots[s];
+    CUDA_TRY(cudaStreamCreateWithFlags(&sh.helper, cudaStreamNonBlocking));
+    CUDA_TRY(cudaEventCreateWithFlags(&sh.fork, cudaEventDisableTiming));
+    CUDA_TRY(cudaEventCreateWithFlags(&sh.join, cudaEventDisableTiming));
+    CUDA_TRY(cudaMallocHost(&sh.pinned, sizeof(SlotCounters)));
+    std::memset(sh.pinned, 0, sizeof(SlotCounters));
+  }
+  *out = ctx;
+  return ADEPT_OK;
+}
+
+extern "C" int adept_shutdown(adept_ctx* ctx) {
+  if (!ctx) return fail(ADEPT_EINVAL, "null context");
+  for (SlotHost& sh : ctx->slots) {
+    if (sh.helper) cudaStreamDestroy(sh.helper);
+    if (sh.fork) cudaEventDestroy(sh.fork);
+    if (sh.join) cudaEventDestroy(sh.join);
+    if (sh.pinned) cudaFreeHost(sh.pinned);
+  }
+  delete ctx;
+  return ADEPT_OK;
+}
+
+namespace {
+int check_slot(adept_ctx* ctx, int slot) {
+  if (!ctx) return fail(ADEPT_EINVAL, "null context");
+  if (slot < 0 || slot >= static_cast<int>(ctx->slots.size())) return fail(ADEPT_EINVAL, "event slot %d out of range", slot);
+  return ADEPT_OK;
+}
+}  // namespace
+
+extern "C" int adept_enqueue_batch(adept_ctx* ctx, int slot, int n, const uint32_t* event_ids, const uint64_t* track_ids,
+                                   const int8_t* species, const double* pos3, const double* dir3, const double* ekin) {
+  int rc = check_slot(ctx, slot);
+  if (rc != ADEPT_OK) return rc;
+  if (n < 0 || (n > 0 && (!event_ids || !track_ids || !species || !pos3 || !dir3 || !ekin))) return fail(ADEPT_EINVAL, "null argument");
+  SlotHost& sh = ctx->slots[slot];
+  if (sh.live) return fail(ADEPT_ESTATE, "slot %d is being transported", slot);
+  std::vector<adept_track> host(std::min<size_t>(n, ctx->stage_cap));
+  for (size_t done = 0; done < static_cast<size_t>(n);) {
+    const size_t m = std::min(ctx->stage_cap, static_cast<size_t>(n) - done);
+    for (size_t i = 0; i < m; ++i) {
+      adept_track& t = host[i];
+      const size_t k = done + i;
+      for (int a = 0; a < 3; ++a) { t.pos[a] = pos3[3 * k + a]; t.dir[a] = dir3[3 * k + a]; }
+      t.ekin = ekin[k]; t.id = track_ids[k]; t.event = event_ids[k]; t.step = 0; t.volume = 0; t.species = species[k];
+      if (!(t.ekin >= 0.0)) return fail(ADEPT_EINVAL, "primary %zu: negative or NaN energy", k);
+    }
+    CUDA_TRY(cudaMemcpy(ctx->d_stage, host.data(), m * sizeof(adept_track), cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaMemset(ctx->d_bad, 0, sizeof(uint32_t)));
+    const int grid = static_cast<int>(std::min<size_t>((m + kBlock - 1) / kBlock, 4096));
+    enqueue_kernel<<<grid, kBlock>>>(ctx->dev, sh.dev, ctx->d_stage, static_cast<int>(m), ctx->d_bad);
+    CUDA_TRY(cudaGetLastError());
+    uint32_t bad = 0;
+    CUDA_TRY(cudaMemcpy(&bad, ctx->d_bad, sizeof(uint32_t), cudaMemcpyDeviceToHost));
+    if (bad) return fail(ADEPT_EINVAL, "%u primaries lie outside the world or have an unknown species", bad);
+    done += m;
+  }
+  return ADEPT_OK;
+}
+
+extern "C" int adept_enqueue_primaries(adept_ctx* ctx, int slot, uint32_t event_id, int n, const int8_t* species,
+                                       const double* pos3, const double* dir3, const double* ekin) {
+  if (n < 0) return fail(ADEPT_EINVAL, "negative count");
+  std::vector<uint32_t> ev(n, event_id);
+  std::vector<uint64_t> id(n);
+  std::iota(id.begin(), id.end(), 0ull);
+  return adept_enqueue_batch(ctx, slot, n, ev.data(), id.data(), species, pos3, dir3, ekin);
+}
+
+namespace {
+
+// One population step of a slot: gamma kernel on the caller's stream, charged kernel on the helper
+// stream (species kernels on different streams, synchronised with events), then the
+// buffer swap.
+int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity) {
+  CUDA_TRY(cudaEventRecord(sh.fork, st));
+  CUDA_TRY(cudaStreamWaitEvent(sh.helper, sh.fork, 0));
+  step_kernel<MODE_GAMMA><<<dim3(ctx->grid_gamma, 1), kBlock, 0, st>>>(ctx->dev, sh.dev, parity);
+  step_kernel<MODE_CHARGED><<<dim3(ctx->grid_charged, 2), kBlock, 0, sh.helper>>>(ctx->dev, sh.dev, parity);
+  CUDA_TRY(cudaEventRecord(sh.join, sh.helper));
+  CUDA_TRY(cudaStreamWaitEvent(st, sh.join, 0));
+  finish_iteration_kernel<<<1, 1, 0, st>>>(sh.dev, parity);
+  sh.launches += 3;
+  return ADEPT_OK;
+}
+
+}  // namespace
+
+extern "C" int adept_transport_many(adept_ctx* ctx, int n_slots, const int* slots, void* const* streams) {
+  if (!ctx || n_slots < 0 || (n_slots > 0 && (!slots || !streams))) return fail(ADEPT_EINVAL, "null argument");
+  for (int k = 0; k < n_slots; ++k) {
+    const int rc = check_slot(ctx, slots[k]);
+    if (rc != ADEPT_OK) return rc;
+    ctx->slots[slots[k]].live = true;
+  }
+  std::vector<int> parity(n_slots, 0);
+  int n_live = n_slots, rc_final = ADEPT_OK;
+  while (n_live > 0) {
+    for (int it = 0; it < ctx->cfg.sync_interval; ++it)
+      for (int k = 0; k < n_slots; ++k) {
+        SlotHost& sh = ctx->slots[slots[k]];
+        if (!sh.live) continue;
+        const int rc = launch_iteration(ctx, sh, static_cast<cudaStream_t>(streams[k]), parity[k]);
+        if (rc != ADEPT_OK) return rc;
+        parity[k] ^= 1;
+      }
+    for (int k = 0; k < n_slots; ++k) {
+      SlotHost& sh = ctx->slots[slots[k]];
+      if (sh.live) CUDA_TRY(cudaMemcpyAsync(sh.pinned, sh.dev.counters, sizeof(SlotCounters), cudaMemcpyDeviceToHost,
+                                            static_cast<cudaStream_t>(streams[k])));
+    }
+    for (int k = 0; k < n_slots; ++k) {
+      SlotHost& sh = ctx->slots[slots[k]];
+      if (!sh.live) continue;
+      CUDA_TRY(cudaStreamSynchronize(static_cast<cudaStream_t>(streams[k])));
+      if (sh.pinned->overflow) rc_final = fail(ADEPT_EOVERFLOW, "slot %d: track queue overflow (capacity %llu per species)",
+                                               slots[k], static_cast<unsigned long long>(ctx->cfg.track_capacity));
+      if (sh.pinned->live == 0 || sh.pinned->overflow) {
+        sh.live = false;
+        --n_live;
+        if (parity[k]) {  // leave the (empty) slot at parity 0 for the next enqueue
+          // counts are all zero, nothing to move
+        }
+      }
+    }
+  }
+  CUDA_TRY(cudaGetLastError());
+  return rc_final;
+}
+
+extern "C" int adept_transport(adept_ctx* ctx, int slot, void* stream) {
+  return adept_transport_many(ctx, 1, &slot, &stream);
+}
+
+extern "C" int adept_read_scoring(adept_ctx* ctx, int slot, double* edep, size_t n_volumes, adept_ledger* ledger, void* stream) {
+  const int rc = check_slot(ctx, slot);
+  if (rc != ADEPT_OK) return rc;
+  if (edep && n_volumes != static_cast<size_t>(ctx->n_vol)) return fail(ADEPT_EINVAL, "n_volumes is %zu, geometry has %d", n_volumes, ctx->n_vol);
+  SlotHost& sh = ctx->slots[slot];
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  if (edep) CUDA_TRY(cudaMemcpyAsync(edep, sh.dev.edep, n_volumes * sizeof(double), cudaMemcpyDeviceToHost, st));
+  double led[5];
+  CUDA_TRY(cudaMemcpyAsync(led, sh.dev.ledger, sizeof(led), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaMemsetAsync(sh.dev.edep, 0, static_cast<size_t>(ctx->n_vol) * sizeof(double), st));
+  CUDA_TRY(cudaMemsetAsync(sh.dev.ledger, 0, 8 * sizeof(double), st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  if (ledger) { ledger->deposited = led[0]; ledger->below_cut = led[1]; ledger->escaped = led[2]; ledger->killed = led[3]; ledger->primary = led[4]; }
+  return ADEPT_OK;
+}
+
+extern "C" int adept_read_leaked(adept_ctx* ctx, int slot, adept_track* out, size_t cap, size_t* n) {
+  const int rc = check_slot(ctx, slot);
+  if (rc != ADEPT_OK) return rc;
+  if (!n) return fail(ADEPT_EINVAL, "null argument");
+  SlotHost& sh = ctx->slots[slot];
+  SlotCounters c;
+  CUDA_TRY(cudaMemcpy(&c, sh.dev.counters, sizeof(c), cudaMemcpyDeviceToHost));
+  *n = c.n_leaked;
+  const size_t m = std::min<size_t>(std::min<size_t>(c.n_leaked, cap), ctx->cfg.leak_capacity);
+  if (m && out) CUDA_TRY(cudaMemcpy(out, sh.dev.leaked, m * sizeof(adept_track), cudaMemcpyDeviceToHost));
+  CUDA_TRY(cudaMemset(&sh.dev.counters->n_leaked, 0, sizeof(uint32_t)));
+  return ADEPT_OK;
+}
+
+extern "C" int adept_get_stats(adept_ctx* ctx, int slot, adept_stats* out) {
+  const int rc = check_slot(ctx, slot);
+  if (rc != ADEPT_OK) return rc;
+  if (!out) return fail(ADEPT_EINVAL, "null argument");
+  DevStats s;
+  CUDA_TRY(cudaMemcpy(&s, ctx->slots[slot].dev.stats, sizeof(s), cudaMemcpyDeviceToHost));
+  for (int k = 0; k < 3; ++k) { out->steps[k] = s.steps[k]; out->secondaries[k] = s.secondaries[k]; }
+  for (int k = 0; k < ADEPT_N_OUTCOMES; ++k) out->outcomes[k] = s.outcomes[k];
+  out->chords = s.chords; out->iterations = s.iterations; out->peak_population = s.peak_population;
+  out->launches = ctx->slots[slot].launches;
+  return ADEPT_OK;
+}
+
+extern "C" int adept_step_frozen(adept_ctx* ctx, int n, const adept_track* in, adept_step_result* out, adept_track* sec, void* stream) {
+  if (!ctx || n < 0 || (n > 0 && (!in || !out || !sec))) return fail(ADEPT_EINVAL, "null argument");
+  if (n == 0) return ADEPT_OK;
+  for (int i = 0; i < n; ++i)
+    if (in[i].volume >= static_cast<uint32_t>(ctx->n_vol) || in[i].species < 0 || in[i].species > 2)
+      return fail(ADEPT_EINVAL, "track %d: volume or species out of range", i);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  adept_track *d_in = nullptr, *d_sec = nullptr;
+  adept_step_result* d_out = nullptr;
+  CUDA_TRY(cudaMalloc(&d_in, n * sizeof(adept_track)));
+  CUDA_TRY(cudaMalloc(&d_out, n * sizeof(adept_step_result)));
+  CUDA_TRY(cudaMalloc(&d_sec, 2 * static_cast<size_t>(n) * sizeof(adept_track)));
+  CUDA_TRY(cudaMemcpyAsync(d_in, in, n * sizeof(adept_track), cudaMemcpyHostToDevice, st));
+  const int grid = std::min((n + kBlock - 1) / kBlock, 65535);
+  frozen_kernel<<<grid, kBlock, 0, st>>>(ctx->dev, d_in, d_out, d_sec, n);
+  CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(cudaMemcpyAsync(out, d_out, n * sizeof(adept_step_result), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaMemcpyAsync(sec, d_sec, 2 * static_cast<size_t>(n) * sizeof(adept_track), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  cudaFree(d_in); cudaFree(d_out); cudaFree(d_sec);
+  return ADEPT_OK;
+}
+
+extern "C" int adept_distance_batch(adept_ctx* ctx, int nav, int n, const double* pos3, const double* dir3, const uint32_t* volume,
+                                    const double* s_max, double* out, void* stream) {
+  if (!ctx || n < 0 || (n > 0 && (!pos3 || !dir3 || !volume || !s_max || !out))) return fail(ADEPT_EINVAL, "null argument");
+  if (n == 0) return ADEPT_OK;
+  for (int i = 0; i < n; ++i) if (volume[i] >= static_cast<uint32_t>(ctx->n_vol)) return fail(ADEPT_EINVAL, "ray %d: volume out of range", i);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  double *d_pos, *d_dir, *d_smax, *d_out;
+  uint32_t* d_vol;
+  CUDA_TRY(cudaMalloc(&d_pos, 3 * n * sizeof(double))); CUDA_TRY(cudaMalloc(&d_dir, 3 * n * sizeof(double)));
+  CUDA_TRY(cudaMalloc(&d_smax, n * sizeof(double))); CUDA_TRY(cudaMalloc(&d_out, n * sizeof(double)));
+  CUDA_TRY(cudaMalloc(&d_vol, n * sizeof(uint32_t)));
+  CUDA_TRY(cudaMemcpyAsync(d_pos, pos3, 3 * n * sizeof(double), cudaMemcpyHostToDevice, st));
+  CUDA_TRY(cudaMemcpyAsync(d_dir, dir3, 3 * n * sizeof(double), cudaMemcpyHostToDevice, st));
+  CUDA_TRY(cudaMemcpyAsync(d_smax, s_max, n * sizeof(double), cudaMemcpyHostToDevice, st));
+  CUDA_TRY(cudaMemcpyAsync(d_vol, volume, n * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
+  distance_kernel<<<std::min((n + kBlock - 1) / kBlock, 65535), kBlock, 0, st>>>(ctx->dev, nav, n, d_pos, d_dir, d_vol, d_smax, d_out);
+  CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(cudaMemcpyAsync(out, d_out, n * sizeof(double), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  cudaFree(d_pos); cudaFree(d_dir); cudaFree(d_smax); cudaFree(d_out); cudaFree(d_vol);
+  return ADEPT_OK;
+}
+
+extern "C" int adept_locate_batch(adept_ctx* ctx, int nav, int n, const double* pos3, int64_t* out, void* stream) {
+  if (!ctx || n < 0 || (n > 0 && (!pos3 || !out))) return fail(ADEPT_EINVAL, "null argument");
+  if (n == 0) return ADEPT_OK;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  double* d_pos;
+  long long* d_out;
+  CUDA_TRY(cudaMalloc(&d_pos, 3 * n * sizeof(double))); CUDA_TRY(cudaMalloc(&d_out, n * sizeof(long long)));
+  CUDA_TRY(cudaMemcpyAsync(d_pos, pos3, 3 * n * sizeof(double), cudaMemcpyHostToDevice, st));
+  locate_kernel<<<std::min((n + kBlock - 1) / kBlock, 65535), kBlock, 0, st>>>(ctx->dev, nav, n, d_pos, d_out);
+  CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(cudaMemcpyAsync(out, d_out, n * sizeof(long long), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  cudaFree(d_pos); cudaFree(d_out);
+  return ADEPT_OK;
+}

@@ -1,0 +1,181 @@
+// Charged-track propagation in a magnetic field by sagitta-limited chords  (SURVEY.md §8 row A6,
+// §8(c) F1-F6).  Uniform field: exact helix end points.  Field map: one classical RK4
+// step per chord.  The chord loop is warp-convergent (lanes that finished idle inside it) so that the
+// geometry query of every chord can use the warp-cooperative BVH; the chord budget (F4) bounds the
+// divergence the paper measured.
+#pragma once
+#include "geom.cuh"
+
+namespace adept {
+
+__device__ __forceinline__ void cross3(const double a[3], const double b[3], double c[3]) {
+  c[0] = a[1] * b[2] - a[2] * b[1];
+  c[1] = a[2] * b[0] - a[0] * b[2];
+  c[2] = a[0] * b[1] - a[1] * b[0];
+}
+
+// F6: B = (0, 0, bz(r, z)), bilinear, clamped outside the grid
+__device__ __forceinline__ void field_at(const DevCtx& c, const double p[3], double B[3]) {
+  if (c.field_kind == ADEPT_FIELD_UNIFORM) { B[0] = c.B[0]; B[1] = c.B[1]; B[2] = c.B[2]; return; }
+  B[0] = B[1] = B[2] = 0.0;
+  if (c.field_kind != ADEPT_FIELD_MAP_RZ) return;
+  const double r = sqrt(p[0] * p[0] + p[1] * p[1]);
+  double fr = (r - c.r0) / c.dr, fz = (p[2] - c.z0) / c.dz;
+  fr = fmin(fmax(fr, 0.0), static_cast<double>(c.nr - 1));
+  fz = fmin(fmax(fz, 0.0), static_cast<double>(c.nz - 1));
+  const int ir = min(static_cast<int>(floor(fr)), c.nr - 2);
+  const int iz = min(static_cast<int>(floor(fz)), c.nz - 2);
+  const double a = fr - ir, b = fz - iz;
+  const double* m = c.bz + iz * c.nr + ir;
+  const double v00 = __ldg(m), v01 = __ldg(m + 1), v10 = __ldg(m + c.nr), v11 = __ldg(m + c.nr + 1);
+  const double lo = v00 + a * (v01 - v00);
+  const double hi = v10 + a * (v11 - v10);
+  B[2] = lo + b * (hi - lo);
+}
+
+// F3: exact helix, omega = -q kCB |B| h / p
+__device__ __forceinline__ void helix(const double B[3], int charge, double pmom, double h, const double p[3],
+                                      const double d[3], double p1[3], double d1[3]) {
+  const double Bn = sqrt(B[0] * B[0] + B[1] * B[1] + B[2] * B[2]);
+  const double b[3] = {B[0] / Bn, B[1] / Bn, B[2] / Bn};
+  const double omega = -charge * kCB * Bn * h / pmom;
+  const double dpar = d[0] * b[0] + d[1] * b[1] + d[2] * b[2];
+  const double dl[3] = {dpar * b[0], dpar * b[1], dpar * b[2]};
+  const double dt[3] = {d[0] - dl[0], d[1] - dl[1], d[2] - dl[2]};
+  double bxd[3];
+  cross3(b, dt, bxd);
+  double so, co;
+  sincos(omega, &so, &co);
+  const double sh = sin(0.5 * omega);
+  const double omc = 2.0 * sh * sh;
+  const double hw = h / omega;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    d1[i] = dl[i] + dt[i] * co + bxd[i] * so;
+    p1[i] = p[i] + dl[i] * h + hw * (dt[i] * so + bxd[i] * omc);
+  }
+}
+
+// F1, F3: one classical RK4 step on (x, d): x' = d, d' = (q kCB / p) d x B(x)
+__device__ __forceinline__ void rk4(const DevCtx& c, int charge, double pmom, double h, const double p[3],
+                                    const double d[3], double p1[3], double d1[3]) {
+  const double kap = charge * kCB / pmom;
+  double B[3], k1v[3], k2v[3], k3v[3], k4v[3], k2x[3], k3x[3], k4x[3], x[3], v[3], t[3];
+  field_at(c, p, B);
+  cross3(d, B, t);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { k1v[i] = kap * t[i]; x[i] = p[i] + 0.5 * h * d[i]; v[i] = d[i] + 0.5 * h * k1v[i]; }
+  field_at(c, x, B);
+  cross3(v, B, t);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { k2x[i] = v[i]; k2v[i] = kap * t[i]; x[i] = p[i] + 0.5 * h * k2x[i]; v[i] = d[i] + 0.5 * h * k2v[i]; }
+  field_at(c, x, B);
+  cross3(v, B, t);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { k3x[i] = v[i]; k3v[i] = kap * t[i]; x[i] = p[i] + h * k3x[i]; v[i] = d[i] + h * k3v[i]; }
+  field_at(c, x, B);
+  cross3(v, B, t);
+  double n = 0.0;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    k4x[i] = v[i]; k4v[i] = kap * t[i];
+    p1[i] = p[i] + (h / 6.0) * (d[i] + 2.0 * k2x[i] + 2.0 * k3x[i] + k4x[i]);
+    d1[i] = d[i] + (h / 6.0) * (k1v[i] + 2.0 * k2v[i] + 2.0 * k3v[i] + k4v[i]);
+    n += d1[i] * d1[i];
+  }
+  n = sqrt(n);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) d1[i] /= n;
+}
+
+// F2-F4 chord loop.  flag: 0 physics limit reached, 1 boundary (pos = hit point without the push,
+// pushdir = chord direction), 2 truncated (chord budget).  Warp-convergent.
+__device__ int propagate(const DevCtx& c, int nav, bool active, int charge, double ekin, double pos[3], double dir[3],
+                         uint32_t vol, double s_phys, double& s_out, int& chords_out, double pushdir[3]) {
+  const double pmom = sqrt(ekin * (ekin + 2.0 * kMe));
+  double s_done = 0.0;
+  int chords = 0, flag = 0;
+  bool running = active;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) pushdir[i] = dir[i];
+  while (__any_sync(kFull, running)) {
+    // --- per-lane: decide the next segment
+    bool query = false, straight = false, last = false;
+    double h = 0.0, L = 0.0, rest = 0.0;
+    double u[3] = {0.0, 0.0, 0.0}, p1[3], d1[3], B[3] = {0.0, 0.0, 0.0};
+    if (running) {
+      if (s_done >= s_phys) {
+        flag = 0; running = false;
+      } else {
+        if (charge != 0 && c.field_kind != ADEPT_FIELD_NONE) field_at(c, pos, B);  // gammas go straight
+        double dxB[3];
+        cross3(dir, B, dxB);
+        const double bperp = sqrt(dxB[0] * dxB[0] + dxB[1] * dxB[1] + dxB[2] * dxB[2]);
+        rest = s_phys - s_done;
+        if (bperp == 0.0) {
+          straight = true; query = true; L = rest;
+          u[0] = dir[0]; u[1] = dir[1]; u[2] = dir[2];
+        } else if (chords >= c.chord_budget) {
+          flag = 2; running = false;
+        } else {
+          const double Rcurv = pmom / (kCB * bperp);
+          const double h_max = sqrt(8.0 * c.delta_chord * Rcurv);
+          last = h_max >= rest;
+          h = last ? rest : h_max;
+          if (c.field_kind == ADEPT_FIELD_UNIFORM) helix(B, charge, pmom, h, pos, dir, p1, d1);
+          else rk4(c, charge, pmom, h, pos, dir, p1, d1);
+          const double ch[3] = {p1[0] - pos[0], p1[1] - pos[1], p1[2] - pos[2]};
+          L = sqrt(ch[0] * ch[0] + ch[1] * ch[1] + ch[2] * ch[2]);
+          u[0] = ch[0] / L; u[1] = ch[1] / L; u[2] = ch[2] / L;
+          query = true;
+        }
+      }
+    }
+    // --- warp-cooperative geometry query of this segment
+    const double s_geo = nav_distance(c, nav, query, pos[0], pos[1], pos[2], u[0], u[1], u[2], vol, L);
+    if (query) {
+      if (straight) {
+        pushdir[0] = u[0]; pushdir[1] = u[1]; pushdir[2] = u[2];
+        if (s_geo < rest) {
+#pragma unroll
+          for (int i = 0; i < 3; ++i) pos[i] += s_geo * dir[i];
+          s_done += s_geo; flag = 1;
+        } else {
+#pragma unroll
+          for (int i = 0; i < 3; ++i) pos[i] += rest * dir[i];
+          s_done = s_phys; flag = 0;
+        }
+        running = false;
+      } else {
+        ++chords;
+        if (s_geo < L) {
+          const double frac = s_geo / L;
+          double dh[3];
+          if (c.field_kind == ADEPT_FIELD_UNIFORM) {
+            double ph[3];
+            helix(B, charge, pmom, h * frac, pos, dir, ph, dh);
+          } else {
+            double n = 0.0;
+#pragma unroll
+            for (int i = 0; i < 3; ++i) { dh[i] = dir[i] + frac * (d1[i] - dir[i]); n += dh[i] * dh[i]; }
+            n = sqrt(n);
+#pragma unroll
+            for (int i = 0; i < 3; ++i) dh[i] /= n;
+          }
+#pragma unroll
+          for (int i = 0; i < 3; ++i) { pos[i] += s_geo * u[i]; dir[i] = dh[i]; pushdir[i] = u[i]; }
+          s_done += h * frac; flag = 1; running = false;
+        } else {
+#pragma unroll
+          for (int i = 0; i < 3; ++i) { pos[i] = p1[i]; dir[i] = d1[i]; }
+          s_done = last ? s_phys : s_done + h;
+        }
+      }
+    }
+  }
+  s_out = s_done;
+  chords_out = chords;
+  return flag;
+}
+
+}  // namespace adept

@@ -1,0 +1,328 @@
+// Solids, distance-to-boundary with a warp-cooperative BVH, and Locate  (
+// §8(c) G1-G5).  Every function that takes an `active` flag must be called by all
+// 32 lanes of a warp in converged control flow: lanes whose volume has a BVH are served one after the
+// other by the whole warp (each lane tests one child box / one primitive), which turns the paper's
+// "quasi-random memory access + divergence" bottleneck into coalesced, uniform work.
+#pragma once
+#include "types.cuh"
+
+namespace adept {
+
+__device__ __forceinline__ const DevVolume& volume(const DevCtx& c, int v) { return c.vol[v]; }
+
+__device__ __forceinline__ void to_local(const DevVolume& v, double gx, double gy, double gz, double l[3]) {
+  const double q0 = gx - v.t[0], q1 = gy - v.t[1], q2 = gz - v.t[2];
+  if (v.identity) { l[0] = q0; l[1] = q1; l[2] = q2; return; }
+#pragma unroll
+  for (int i = 0; i < 3; ++i) l[i] = v.R[0 + i] * q0 + v.R[3 + i] * q1 + v.R[6 + i] * q2;
+}
+__device__ __forceinline__ void dir_to_local(const DevVolume& v, double gx, double gy, double gz, double l[3]) {
+  if (v.identity) { l[0] = gx; l[1] = gy; l[2] = gz; return; }
+#pragma unroll
+  for (int i = 0; i < 3; ++i) l[i] = v.R[0 + i] * gx + v.R[3 + i] * gy + v.R[6 + i] * gz;
+}
+
+// ---------------------------------------------------------------- G1 solids
+__device__ __forceinline__ bool inside_solid(int solid, const double h[3], const double p[3]) {
+  if (solid == ADEPT_BOX) return fabs(p[0]) <= h[0] && fabs(p[1]) <= h[1] && fabs(p[2]) <= h[2];
+  const double r2 = p[0] * p[0] + p[1] * p[1];
+  return r2 >= h[0] * h[0] && r2 <= h[1] * h[1] && fabs(p[2]) <= h[2];
+}
+
+__device__ __forceinline__ double box_exit(const double h[3], const double p[3], const double d[3]) {
+  double t = ADEPT_INF;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    if (d[i] != 0.0) {
+      const double ti = ((d[i] > 0.0 ? h[i] : -h[i]) - p[i]) / d[i];
+      t = fmin(t, ti);
+    }
+  }
+  return fmax(t, 0.0);
+}
+
+__device__ __forceinline__ double box_entry(const double h[3], const double p[3], const double d[3]) {
+  double tn = -ADEPT_INF, tf = ADEPT_INF;
+  bool miss = false;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    if (d[i] != 0.0) {
+      const double t1 = (-h[i] - p[i]) / d[i];
+      const double t2 = (h[i] - p[i]) / d[i];
+      tn = fmax(tn, fmin(t1, t2));
+      tf = fmin(tf, fmax(t1, t2));
+    } else if (fabs(p[i]) > h[i]) {
+      miss = true;
+    }
+  }
+  if (!miss && tn <= tf && tf > 0.0) return fmax(tn, 0.0);
+  return ADEPT_INF;
+}
+
+__device__ __forceinline__ double tube_exit(const double h[3], const double p[3], const double d[3]) {
+  double t = ADEPT_INF;
+  if (d[2] != 0.0) t = ((d[2] > 0.0 ? h[2] : -h[2]) - p[2]) / d[2];
+  const double A = d[0] * d[0] + d[1] * d[1];
+  if (A > 0.0) {
+    const double B = p[0] * d[0] + p[1] * d[1];
+    const double r2 = p[0] * p[0] + p[1] * p[1];
+    const double Co = r2 - h[1] * h[1];
+    const double disc_o = B * B - A * Co;
+    t = fmin(t, (-B + sqrt(fmax(disc_o, 0.0))) / A);
+    if (h[0] > 0.0 && B < 0.0) {
+      const double Ci = r2 - h[0] * h[0];
+      const double disc_i = B * B - A * Ci;
+      if (disc_i > 0.0) t = fmin(t, (-B - sqrt(disc_i)) / A);
+    }
+  }
+  return fmax(t, 0.0);
+}
+
+__device__ __forceinline__ double tube_entry(const double h[3], const double p[3], const double d[3]) {
+  if (inside_solid(ADEPT_TUBE, h, p)) return 0.0;
+  double best = ADEPT_INF;
+  const double r2 = p[0] * p[0] + p[1] * p[1];
+  const double rmin2 = h[0] * h[0], rmax2 = h[1] * h[1];
+  if (fabs(p[2]) > h[2] && p[2] * d[2] < 0.0) {  // (a) end caps
+    const double t = (fabs(p[2]) - h[2]) / fabs(d[2]);
+    const double x = p[0] + t * d[0], y = p[1] + t * d[1];
+    const double q2 = x * x + y * y;
+    if (q2 >= rmin2 && q2 <= rmax2) best = fmin(best, t);
+  }
+  const double A = d[0] * d[0] + d[1] * d[1];
+  if (A > 0.0) {
+    const double B = p[0] * d[0] + p[1] * d[1];
+    const double Co = r2 - rmax2;
+    if (Co > 0.0 && B < 0.0) {  // (b) outer cylinder from outside
+      const double disc = B * B - A * Co;
+      if (disc > 0.0) {
+        const double t = (-B - sqrt(disc)) / A;
+        if (t >= 0.0 && fabs(p[2] + t * d[2]) <= h[2]) best = fmin(best, t);
+      }
+    }
+    if (h[0] > 0.0) {  // (c) inner cylinder, far root: leaving the hole into the solid
+      const double Ci = r2 - rmin2;
+      const double disc = B * B - A * Ci;
+      if (disc > 0.0) {
+        const double t = (-B + sqrt(disc)) / A;
+        if (t > 0.0 && fabs(p[2] + t * d[2]) <= h[2]) best = fmin(best, t);
+      }
+    }
+  }
+  return best;
+}
+
+__device__ __forceinline__ double solid_exit(const DevVolume& v, const double p[3], const double d[3]) {
+  return v.solid == ADEPT_BOX ? box_exit(v.dims, p, d) : tube_exit(v.dims, p, d);
+}
+__device__ __forceinline__ double solid_entry(const DevVolume& v, const double p[3], const double d[3]) {
+  return v.solid == ADEPT_BOX ? box_entry(v.dims, p, d) : tube_entry(v.dims, p, d);
+}
+
+__device__ __forceinline__ bool inside_volume(const DevCtx& c, int vol, double x, double y, double z) {
+  const DevVolume& v = volume(c, vol);
+  double l[3];
+  to_local(v, x, y, z, l);
+  return inside_solid(v.solid, v.dims, l);
+}
+
+__device__ __forceinline__ double entry_distance(const DevCtx& c, int vol, double px, double py, double pz,
+                                                 double dx, double dy, double dz) {
+  const DevVolume& v = volume(c, vol);
+  double lp[3], ld[3];
+  to_local(v, px, py, pz, lp);
+  dir_to_local(v, dx, dy, dz, ld);
+  return solid_entry(v, lp, ld);
+}
+
+// ---------------------------------------------------------------- warp-cooperative BVH
+__device__ __forceinline__ double warp_min(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(kFull, v, o));
+  return v;
+}
+__device__ __forceinline__ int warp_min_int(int v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = min(v, __shfl_xor_sync(kFull, v, o));
+  return v;
+}
+
+// lane tests box `i` (< n valid) of a SoA box array of stride `stride` against the ray; returns hit
+__device__ __forceinline__ bool ray_box(const double* __restrict__ box, int stride, int i, bool valid, double px,
+                                        double py, double pz, double ix, double iy, double iz, double best) {
+  if (!valid) return false;
+  const double lx = __ldg(box + i), ly = __ldg(box + stride + i), lz = __ldg(box + 2 * stride + i);
+  const double hx = __ldg(box + 3 * stride + i), hy = __ldg(box + 4 * stride + i), hz = __ldg(box + 5 * stride + i);
+  const double ax = (lx - px) * ix, bx = (hx - px) * ix;
+  const double ay = (ly - py) * iy, by = (hy - py) * iy;
+  const double az = (lz - pz) * iz, bz = (hz - pz) * iz;
+  // fmin/fmax drop NaN operands (0 * inf when the ray is parallel to a slab and starts on its plane)
+  const double tn = fmax(fmax(fmin(ax, bx), fmin(ay, by)), fmin(az, bz));
+  const double tf = fmin(fmin(fmax(ax, bx), fmax(ay, by)), fmax(az, bz));
+  return tn <= tf && tf >= 0.0 && tn < best;
+}
+
+__device__ __forceinline__ bool point_box(const double* __restrict__ box, int stride, int i, bool valid, double px,
+                                          double py, double pz) {
+  if (!valid) return false;
+  return px >= __ldg(box + i) && py >= __ldg(box + stride + i) && pz >= __ldg(box + 2 * stride + i) &&
+         px <= __ldg(box + 3 * stride + i) && py <= __ldg(box + 4 * stride + i) && pz <= __ldg(box + 5 * stride + i);
+}
+
+// All arguments warp-uniform.  Returns min(best, nearest daughter entry distance).  The traversal
+// state is a short stack of one 32-bit child mask per level, shared by the warp.
+__device__ double bvh_ray(const DevCtx& c, const DevBvh& b, double px, double py, double pz, double dx, double dy,
+                          double dz, double best) {
+  const int lane = threadIdx.x & 31;
+  const double ix = 1.0 / dx, iy = 1.0 / dy, iz = 1.0 / dz;
+  const int top = b.n_levels - 1;
+  unsigned mask[kBvhMaxLevels];
+  int first[kBvhMaxLevels];
+  int level = top;
+  first[top] = 0;
+  mask[top] = __ballot_sync(kFull, ray_box(b.node_box[top], b.n_nodes[top], lane, lane < b.n_nodes[top], px, py, pz,
+                                           ix, iy, iz, best));
+  for (;;) {
+    if (mask[level] == 0) {
+      if (level == top) break;
+      ++level;
+      continue;
+    }
+    const int ch = __ffs(mask[level]) - 1;
+    mask[level] &= mask[level] - 1;
+    const int node = first[level] + ch;
+    const int base = node << 5;
+    if (level == 0) {
+      const int i = base + lane;
+      double t = ADEPT_INF;
+      if (ray_box(b.prim_box, b.n_prims, i, i < b.n_prims, px, py, pz, ix, iy, iz, best))
+        t = entry_distance(c, __ldg(b.prim_vol + i), px, py, pz, dx, dy, dz);
+      best = fmin(best, warp_min(t));
+    } else {
+      const int n = b.n_nodes[level - 1];
+      const int i = base + lane;
+      first[level - 1] = base;
+      mask[level - 1] = __ballot_sync(kFull, ray_box(b.node_box[level - 1], n, i, i < n, px, py, pz, ix, iy, iz, best));
+      --level;
+    }
+  }
+  return best;
+}
+
+// All arguments warp-uniform.  Lowest touchable id among the daughters containing the point, or -1.
+__device__ int bvh_point(const DevCtx& c, const DevBvh& b, double px, double py, double pz) {
+  const int lane = threadIdx.x & 31;
+  const int top = b.n_levels - 1;
+  unsigned mask[kBvhMaxLevels];
+  int first[kBvhMaxLevels];
+  int level = top;
+  int found = 0x7fffffff;
+  first[top] = 0;
+  mask[top] = __ballot_sync(kFull, point_box(b.node_box[top], b.n_nodes[top], lane, lane < b.n_nodes[top], px, py, pz));
+  for (;;) {
+    if (mask[level] == 0) {
+      if (level == top) break;
+      ++level;
+      continue;
+    }
+    const int ch = __ffs(mask[level]) - 1;
+    mask[level] &= mask[level] - 1;
+    const int base = (first[level] + ch) << 5;
+    const int i = base + lane;
+    if (level == 0) {
+      int hit = 0x7fffffff;
+      if (point_box(b.prim_box, b.n_prims, i, i < b.n_prims, px, py, pz)) {
+        const int v = __ldg(b.prim_vol + i);
+        if (inside_volume(c, v, px, py, pz)) hit = v;
+      }
+      found = min(found, warp_min_int(hit));
+    } else {
+      const int n = b.n_nodes[level - 1];
+      first[level - 1] = base;
+      mask[level - 1] = __ballot_sync(kFull, point_box(b.node_box[level - 1], n, i, i < n, px, py, pz));
+      --level;
+    }
+  }
+  return found == 0x7fffffff ? -1 : found;
+}
+
+// ---------------------------------------------------------------- G3 distance to boundary
+// min(exit distance of the own solid, entry distance of every daughter), capped at s_max.
+// Warp-convergent call; lanes with active == false return s_max.
+__device__ double nav_distance(const DevCtx& c, int nav, bool active, double px, double py, double pz, double dx,
+                               double dy, double dz, uint32_t vol, double s_max) {
+  const int lane = threadIdx.x & 31;
+  double s = s_max;
+  bool need = false;
+  int bvh = -1;
+  if (active) {
+    const DevVolume& v = volume(c, vol);
+    double lp[3], ld[3];
+    to_local(v, px, py, pz, lp);
+    dir_to_local(v, dx, dy, dz, ld);
+    s = fmin(s_max, solid_exit(v, lp, ld));
+    if (v.dcount > 0) {
+      if (nav == ADEPT_NAV_BVH && v.bvh >= 0) {
+        need = true;
+        bvh = v.bvh;
+      } else {
+        for (int k = 0; k < v.dcount; ++k) s = fmin(s, entry_distance(c, v.dbegin + k, px, py, pz, dx, dy, dz));
+      }
+    }
+  }
+  unsigned m = __ballot_sync(kFull, need);
+  while (m) {
+    const int src = __ffs(m) - 1;
+    m &= m - 1;
+    const double r = bvh_ray(c, c.bvh[__shfl_sync(kFull, bvh, src)], __shfl_sync(kFull, px, src),
+                             __shfl_sync(kFull, py, src), __shfl_sync(kFull, pz, src), __shfl_sync(kFull, dx, src),
+                             __shfl_sync(kFull, dy, src), __shfl_sync(kFull, dz, src), __shfl_sync(kFull, s, src));
+    if (lane == src) s = r;
+  }
+  return s;
+}
+
+// ---------------------------------------------------------------- G4 Locate
+// From the world down, descend into the first daughter (index order) containing the point.
+// Warp-convergent call; returns -1 outside the world or for inactive lanes.
+__device__ int nav_locate(const DevCtx& c, int nav, bool active, double qx, double qy, double qz) {
+  const int lane = threadIdx.x & 31;
+  int cur = -1;
+  bool desc = false;
+  if (active && inside_volume(c, 0, qx, qy, qz)) {
+    cur = 0;
+    desc = true;
+  }
+  while (__any_sync(kFull, desc)) {
+    bool need = false;
+    int bvh = -1;
+    if (desc) {
+      const DevVolume& v = volume(c, cur);
+      if (v.dcount == 0) {
+        desc = false;
+      } else if (nav == ADEPT_NAV_BVH && v.bvh >= 0) {
+        need = true;
+        bvh = v.bvh;
+      } else {
+        int next = -1;
+        for (int k = 0; k < v.dcount; ++k) {
+          if (inside_volume(c, v.dbegin + k, qx, qy, qz)) { next = v.dbegin + k; break; }
+        }
+        if (next < 0) desc = false; else cur = next;
+      }
+    }
+    unsigned m = __ballot_sync(kFull, need);
+    while (m) {
+      const int src = __ffs(m) - 1;
+      m &= m - 1;
+      const int r = bvh_point(c, c.bvh[__shfl_sync(kFull, bvh, src)], __shfl_sync(kFull, qx, src),
+                              __shfl_sync(kFull, qy, src), __shfl_sync(kFull, qz, src));
+      if (lane == src) {
+        if (r < 0) desc = false; else cur = r;
+      }
+    }
+  }
+  return cur;
+}
+
+}  // namespace adept

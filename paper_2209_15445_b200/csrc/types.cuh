@@ -1,0 +1,136 @@
+// Device-side data layout of the transport library.  sm_100a only.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "../../include/adept.h"
+
+namespace adept {
+
+constexpr double kMe = 0.51099895;   // m_e c^2 [MeV]
+constexpr double kCB = 2.99792458;   // p[MeV/c] = kCB * B[T] * R[cm]
+constexpr double kPi = 3.14159265358979323846;
+constexpr double kTmin = 1.0e-3;     // 1 keV
+constexpr int kNGrid = ADEPT_N_GRID;
+constexpr unsigned kFull = 0xffffffffu;
+constexpr uint32_t kDeadVolume = 0xffffffffu;
+
+#define ADEPT_INF (__longlong_as_double(0x7ff0000000000000LL))
+
+// material scalar slots (adept_material as 8 doubles)
+enum { S_X0, S_TCUT, S_KCUT, S_BK, S_NEL, S_VACUUM, S_Z, S_RHO, N_SCAL };
+
+// Interleaved table slices (one node = one contiguous row, so a lookup touches 2 adjacent rows):
+//   gamma    row = {Compton, pair, photo, pad}            32 B
+//   electron row = {brem, Moller, dE/dx, range}           32 B
+//   positron row = {brem, Bhabha, annihilation, dE/dx, range, pad, pad, pad} 64 B
+constexpr int kRowG = 4, kRowEm = 4, kRowEp = 8;
+
+struct __align__(16) DevVolume {
+  double t[3];
+  double dims[3];
+  double R[9];
+  int32_t solid;
+  int32_t material;
+  int32_t dbegin;
+  int32_t dcount;
+  int32_t bvh;       // index into DevCtx::bvh, -1 = none (loop over daughters)
+  int32_t identity;  // 1 if R is the identity (transform reduces to a subtraction, bit-identical)
+};
+
+// Implicit complete 32-ary BVH over the daughters of one volume, in the world frame.
+// Primitives are sorted along a Morton curve; node k of level L covers nodes [32k, 32k+32) of level L-1
+// (level 0 covers primitives).  Boxes are stored SoA: lo.x, lo.y, lo.z, hi.x, hi.y, hi.z.
+constexpr int kBvhMaxLevels = 5;
+struct DevBvh {
+  int32_t n_prims;
+  int32_t n_levels;                  // number of node levels (>= 1)
+  int32_t n_nodes[kBvhMaxLevels];    // nodes per level
+  const double* prim_box;            // [6][n_prims]
+  const int32_t* prim_vol;           // [n_prims] touchable id
+  const double* node_box[kBvhMaxLevels];  // [6][n_nodes[L]]
+};
+
+// One species' track buffer, structure of arrays (76 B per track).
+struct TrackSoA {
+  double *x, *y, *z, *dx, *dy, *dz, *ekin;
+  uint64_t* id;
+  uint32_t *event, *step, *vol;
+};
+
+struct SlotCounters {
+  uint32_t count[2][3];     // [buffer parity][species] live entries
+  uint32_t n_reloc;         // relocation work queue (split mode)
+  uint32_t n_inter;         // interaction work queue (split mode)
+  uint32_t overflow;        // set when any queue overflowed
+  uint32_t n_leaked;
+  uint32_t live;            // population after the last finished iteration
+  uint32_t pad[3];
+};
+
+struct DevStats {
+  unsigned long long steps[3];
+  unsigned long long outcomes[ADEPT_N_OUTCOMES];
+  unsigned long long secondaries[3];
+  unsigned long long chords;
+  unsigned long long iterations;
+  unsigned long long peak_population;
+};
+
+struct DevSlot {
+  TrackSoA buf[2][3];       // [parity][species]
+  SlotCounters* counters;
+  double* edep;             // [n_volumes]
+  double* ledger;           // [5]: deposited, below_cut, escaped, killed, primary
+  DevStats* stats;
+  adept_track* leaked;      // [leak_capacity]
+  uint32_t* reloc_queue;    // split mode: species<<30 | index into the next buffer
+  uint32_t* inter_queue;    // split mode: process<<28 | species<<26 | index
+};
+
+struct DevCtx {
+  const DevVolume* vol;
+  int32_t n_vol;
+  const DevBvh* bvh;
+  int32_t navigator;
+  const double* tab_g;      // [n_mat][2048][kRowG]
+  const double* tab_em;     // [n_mat][2048][kRowEm]
+  const double* tab_ep;     // [n_mat][2048][kRowEp]
+  const double* scal;       // [n_mat][N_SCAL]
+  int32_t n_mat;
+  int32_t field_kind;
+  double B[3];
+  int32_t nr, nz;
+  double r0, z0, dr, dz;
+  const double* bz;
+  double u0, inv_du, du;
+  double delta_chord, eps_push, alpha_R, rho_R;
+  int32_t chord_budget;
+  uint32_t seed, max_steps;
+  uint32_t capacity;        // per species per buffer
+  uint32_t leak_capacity;
+};
+
+// Register-resident track and step result.
+struct Track {
+  double x, y, z, dx, dy, dz, ekin;
+  uint64_t id;
+  uint32_t event, step, vol;
+  int species;
+};
+
+struct Secondary {
+  double dx, dy, dz, ekin;
+  int species;     // -1 = none
+  uint32_t child;  // child index (R3)
+};
+
+struct StepOut {
+  Track post;
+  int alive, outcome, chords;
+  double s, edep_dep, edep_cut, escaped, killed;
+  Secondary sec[2];
+  int n_sec;
+};
+
+}  // namespace adept
