@@ -1,0 +1,296 @@
+#!/usr/bin/env python
+"""Benchmark of the EM-shower transport hot path (BASELINE.json: "track steps/s and 10 GeV e- showers/s
+on 1 B200; step-kernel HBM GB/s").
+
+One *step* of this benchmark = one pass of the whole hot path over one batch: `--events` (default
+10 000, BASELINE.json:configs[1]) 10 GeV e- showers in the 50-layer Pb/LAr calorimeter transported
+until every queue is empty.  Inputs are synthetic and seeded.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+`value` is device-timed (CUDA events around adept_transport, primaries already resident in HBM);
+`e2e` goes through the public API with host buffers (enqueue H2D + transport + scoring D2H).
+`--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+BYTES_PER_STEP = 160      # 76 B track read + 76 B survivor write + 8 B scoring atomic
+BYTES_PER_SECONDARY = 76
+E_PRIMARY = 10000.0
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--events", type=int, default=10000, help="showers per batch (config 2: 10000)")
+    ap.add_argument("--field", type=float, default=0.0, help="uniform Bz in tesla (config 3: 1.0)")
+    ap.add_argument("--capacity", type=int, default=0, help="track capacity per species (0 = auto)")
+    ap.add_argument("--sync-interval", type=int, default=8)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--profile", action="store_true",
+                    help="for runs under ncu: take --warmup literally (the timed numbers of such a run are not bench values)")
+    ap.add_argument("--cpu-events-per-core", type=int, default=96)
+    return ap.parse_args()
+
+
+def workload(args, first_event=0):
+    from paper_2209_15445_b200.inputs import field, geometry, materials, primaries
+    g = geometry.calorimeter()
+    mats, tabs, scal = materials.build_material_set(g.material_names)
+    fld = field.uniform_field(0, 0, args.field) if args.field != 0.0 else field.no_field()
+    prim = primaries.beam(args.events, E_PRIMARY, spread=1.0, seed=1, first_event=first_event)
+    return g, tabs, scal, fld, prim
+
+
+# ----------------------------------------------------------------------------- CPU oracle legs
+def _oracle_worker(job):
+    first_event, n_events, field_bz = job
+    from oracle import binding as ob
+    from paper_2209_15445_b200.inputs import field, geometry, materials, primaries
+    g = geometry.calorimeter()
+    _, tabs, scal = materials.build_material_set(g.material_names)
+    fld = field.uniform_field(0, 0, field_bz) if field_bz != 0.0 else field.no_field()
+    o = ob.Oracle(g, tabs, scal, fld)
+    tr = o.make_tracks(primaries.beam(n_events, E_PRIMARY, spread=1.0, seed=1, first_event=first_event))
+    t0 = time.perf_counter()
+    _, _, st = o.run(tr)
+    return sum(st.steps), time.perf_counter() - t0
+
+
+def oracle_throughput(events_per_core, field_bz, cores=None):
+    """Oracle as it stands: one single-threaded process per core over disjoint event ranges."""
+    import multiprocessing as mp
+    from oracle import build as obuild
+    obuild.build()
+    cores = cores or os.cpu_count() or 1
+    jobs = [(c * events_per_core, events_per_core, field_bz) for c in range(cores)]
+    ctx = mp.get_context("spawn")
+    t0 = time.perf_counter()
+    with ctx.Pool(cores) as pool:
+        pool.map(_oracle_worker, [(0, 1, field_bz)] * cores)        # start-up (imports, build) untimed
+        t0 = time.perf_counter()
+        res = pool.map(_oracle_worker, jobs)
+        wall = time.perf_counter() - t0
+    steps = sum(r[0] for r in res)
+    return {"steps": steps, "wall_s": wall, "steps_per_s": steps / wall, "showers_per_s": cores * events_per_core / wall,
+            "cores": cores, "sample": f"{cores * events_per_core} of the workload's 10 GeV e- showers "
+                                      f"({events_per_core} consecutive events per core, one oracle process per core)"}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cores = os.cpu_count() or 1
+    per_core = max(1, min(args.cpu_events_per_core, 32))
+    for _ in range(min(args.warmup, 1)):
+        oracle_throughput(2, args.field, cores)
+    vals = [oracle_throughput(per_core, args.field, cores) for _ in range(args.steps)]
+    best = max(vals, key=lambda v: v["steps_per_s"])
+    total_steps = sum(v["steps"] for v in vals)
+    total_wall = sum(v["wall_s"] for v in vals)
+    v = total_steps / total_wall
+    line = {"impl": "reference", "metric": "track_steps_per_s", "value": v, "unit": "steps/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total_wall / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "config2: 50-layer Pb/LAr calorimeter, 10 GeV e- showers, no field"
+                       if args.field == 0.0 else "config3: same calorimeter, uniform 1 T field", "events_per_step": cores * per_core},
+            "showers_per_s": sum(cores * per_core for _ in vals) / total_wall,
+            "cpu_baseline": {"value": v, "unit": "steps/s", "cores": cores, "kind": "oracle", "sample": best["sample"]},
+            "e2e": {"value": v, "unit": "steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ----------------------------------------------------------------------------- clocks
+class ClockSampler:
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+            "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        reasons = set()
+        for r in self.rows:
+            if len(r) >= 7:
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ----------------------------------------------------------------------------- GPU arm
+def run_ours(args):
+    import torch
+    from paper_2209_15445_b200 import adept
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    torch.cuda.set_device(local)
+    dev = torch.device(f"cuda:{local}")
+
+    # events shard over ranks with no data-path collective: weak scaling
+    g, tabs, scal, fld, prim = workload(args, first_event=rank * args.events)
+    cap = args.capacity or max(1 << 20, 1024 * args.events)
+    a = adept.Adept(g, tabs, scal, fld, device=str(dev), track_capacity=cap, sync_interval=args.sync_interval,
+                    time_kernels=1)
+    stream = torch.cuda.Stream(device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
+    edep_host = np.zeros(g.n_volumes)
+    h2d = sum(prim[k].nbytes for k in ("event", "species", "pos", "dir", "ekin")) + 8 * len(prim["ekin"])
+    d2h = edep_host.nbytes + 40
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def one_pass(timed):
+        """enqueue (H2D) -> transport -> scoring (D2H); returns (device ms of transport, wall s of the whole call)."""
+        flush.zero_()
+        torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        a.enqueue(prim)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(stream):
+            e0.record(stream)
+            a.transport(0, stream)
+            e1.record(stream)
+            a.read_scoring(0, stream, out=edep_host)
+        torch.cuda.synchronize(dev)
+        wall = time.perf_counter() - t0
+        return e0.elapsed_time(e1), wall
+
+    n_warm = args.warmup if args.profile else max(args.warmup, 3)
+    for _ in range(n_warm):
+        one_pass(False)
+    a.kernel_times(0)
+    st0 = a.stats(0)
+    steps0, sec0, launches0 = sum(st0.steps), sum(st0.secondaries), st0.launches
+    gsteps0, gsec0 = st0.steps[2], 0
+
+    clocks = ClockSampler(local)
+    if rank == 0:
+        clocks.start()
+    barrier()
+    t_wall0 = time.perf_counter()
+    dev_ms, wall_s = [], []
+    for _ in range(args.steps):
+        ms, w = one_pass(True)
+        dev_ms.append(ms)
+        wall_s.append(w)
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    clk = clocks.stop() if rank == 0 else None
+
+    st = a.stats(0)
+    kms, kn = a.kernel_times(0)
+    steps = sum(st.steps) - steps0
+    n_sec = sum(st.secondaries) - sec0
+    launches = st.launches - launches0 + args.steps        # + one enqueue kernel per pass
+    t_dev = sum(dev_ms) * 1e-3
+    t_e2e = sum(wall_s)
+    if dist is not None:
+        t = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        t_dev, t_e2e = float(t[0]), float(t[1])
+        c = torch.tensor([steps, launches], dtype=torch.float64, device=dev)
+        dist.all_reduce(c, op=dist.ReduceOp.SUM)
+        steps_all, launches_all = float(c[0]), int(c[1])
+    else:
+        steps_all, launches_all = float(steps), int(launches)
+
+    if rank == 0:
+        peaks = {}
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except Exception:
+            pass
+        peak = float(peaks.get("hbm_gbs", 6650.0))
+        peak_src = "MEASURED_PEAKS.json hbm_gbs (of measured)" if "hbm_gbs" in peaks else "6650 GB/s (of fallback)"
+        # dominant kernel = the step kernel with the larger accumulated device time
+        dom = int(np.argmax(kms))
+        dom_steps = (st.steps[2] - gsteps0) if dom == 0 else (steps - (st.steps[2] - gsteps0))
+        # secondaries are attributed to the kernel that creates them in proportion to its steps
+        dom_bytes = dom_steps * BYTES_PER_STEP + n_sec * BYTES_PER_SECONDARY * (dom_steps / max(steps, 1))
+        achieved = dom_bytes / (kms[dom] * 1e-3) / 1e9 if kms[dom] > 0 else 0.0
+        line = {
+            "metric": "track_steps_per_s", "value": steps_all / t_dev, "unit": "steps/s", "n_gpus": world,
+            "steps": args.steps, "warmup": n_warm, "ms_per_step": 1e3 * t_dev / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": ("config2: 10000 x 10 GeV e- in the 50-layer Pb/LAr calorimeter, no field, 0.7 mm cuts"
+                                    if args.field == 0.0 else f"config3: same calorimeter, uniform {args.field} T field"),
+                       "events_per_step_per_gpu": args.events, "track_capacity": cap, "sync_interval": args.sync_interval,
+                       "l2": "256 MB buffer written between passes (L2 flush); peak live track state also exceeds L2",
+                       "parallelism": f"events sharded over {world} GPU(s), no data-path collective"},
+            "showers_per_s": world * args.events * args.steps / t_dev,
+            "track_steps_per_step": steps_all / args.steps,
+            "e2e": {"value": steps_all / t_e2e, "unit": "steps/s", "showers_per_s": world * args.events * args.steps / t_e2e,
+                    "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
+            "gpu_launches": launches_all,
+            "clocks": clk,
+            "roofline": {"bound": "hbm", "kernel": "step_kernel<gamma>" if dom == 0 else "step_kernel<charged>",
+                         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                         "peak_source": peak_src, "launches": int(kn[dom]), "avg_launch_ms": float(kms[dom] / max(kn[dom], 1)),
+                         "algorithmic_bytes_per_step": BYTES_PER_STEP,
+                         "other_kernel_ms": float(kms[1 - dom]), "dominant_kernel_ms": float(kms[dom]),
+                         "note": "latency/divergence bound fp64 Monte Carlo: see DESIGN.md §5 and profiles/"},
+            "iterations_per_step": (st.iterations - st0.iterations) / args.steps,
+            "peak_population": int(st.peak_population),
+            "wall_s_timed_region": t_wall,
+        }
+        if world == 1 and not args.no_cpu_baseline and not args.profile:
+            ob = oracle_throughput(args.cpu_events_per_core, args.field)
+            line["cpu_baseline"] = {"value": ob["steps_per_s"], "unit": "steps/s", "cores": ob["cores"], "kind": "oracle",
+                                    "sample": ob["sample"], "showers_per_s": ob["showers_per_s"]}
+        print(json.dumps(line))
+    a.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

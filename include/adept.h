@@ -108,7 +108,7 @@ typedef struct {
   uint64_t track_capacity; /* per slot, per species: entries of each of the two track buffers       */
   uint64_t leak_capacity;  /* per slot: tracks that left the world kept for adept_read_leaked       */
   int32_t split_kernels;   /* 0: one step kernel per species group; 1: + relocation/interaction kernels */
-  int32_t reserved;
+  int32_t time_kernels;    /* 1: bracket every step-kernel launch with CUDA events (adept_get_kernel_times) */
 } adept_config;
 
 typedef struct {
@@ -193,6 +193,11 @@ int adept_read_scoring(adept_ctx*, int event_slot, double* edep_per_volume, size
 int adept_read_leaked(adept_ctx*, int event_slot, adept_track* out, size_t cap, size_t* n);
 
 int adept_get_stats(adept_ctx*, int event_slot, adept_stats* out);
+
+/* With config.time_kernels: device time [ms] and launch count of the gamma step kernel [0] and the
+ * charged step kernel [1] of this slot, accumulated since the last call (CUDA events recorded on the
+ * stream each kernel is launched on). */
+int adept_get_kernel_times(adept_ctx*, int event_slot, double ms[2], uint64_t launches[2]);
 
 /* Test hook: exactly one step for each of n tracks, results in input order; secondaries[2*i + k]. */
 int adept_step_frozen(adept_ctx*, int n, const adept_track* in, adept_step_result* out,

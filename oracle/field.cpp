@@ -121,7 +121,13 @@ extern "C" int orc_propagate(const orc_ctx* c, int charge, double ekin, double p
     }
     if (chords >= c->cfg.chord_budget) { flag = 2; break; }
     const double Rcurv = pmom / (kCB * bperp);
-    const double h_max = std::sqrt(8.0 * c->cfg.delta_chord * Rcurv);
+    double h_max = std::sqrt(8.0 * c->cfg.delta_chord * Rcurv);
+    if (c->field.kind == ORC_FIELD_MAP_RZ) {
+      /* F2': an RK4 chord may not turn the direction about B by more than 0.5 rad,
+         or the one-step integrator loses accuracy (local error ~ omega^5/120) and conditioning */
+      const double Bn = std::sqrt(B[0] * B[0] + B[1] * B[1] + B[2] * B[2]);
+      h_max = std::min(h_max, 0.5 * pmom / (kCB * Bn));
+    }
     const bool last = h_max >= rest; /* this chord completes the step */
     const double h = last ? rest : h_max;
     double p1[3], d1[3];

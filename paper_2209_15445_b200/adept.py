@@ -44,7 +44,7 @@ class CConfig(C.Structure):
     _fields_ = [("delta_chord", C.c_double), ("eps_push", C.c_double), ("alpha_R", C.c_double), ("rho_R", C.c_double),
                 ("chord_budget", C.c_int32), ("seed", C.c_uint32), ("max_steps", C.c_uint32), ("navigator", C.c_int32),
                 ("n_event_slots", C.c_int32), ("sync_interval", C.c_int32), ("track_capacity", C.c_uint64),
-                ("leak_capacity", C.c_uint64), ("split_kernels", C.c_int32), ("reserved", C.c_int32)]
+                ("leak_capacity", C.c_uint64), ("split_kernels", C.c_int32), ("time_kernels", C.c_int32)]
 
 
 class CLedger(C.Structure):
@@ -62,7 +62,7 @@ class CStats(C.Structure):
 
 EXPORTS = ["adept_last_error", "adept_default_config", "adept_workspace_bytes", "adept_init",
            "adept_enqueue_primaries", "adept_enqueue_batch", "adept_transport", "adept_transport_many",
-           "adept_read_scoring", "adept_read_leaked", "adept_get_stats", "adept_step_frozen",
+           "adept_read_scoring", "adept_read_leaked", "adept_get_stats", "adept_get_kernel_times", "adept_step_frozen",
            "adept_distance_batch", "adept_locate_batch", "adept_shutdown"]
 
 
@@ -85,6 +85,7 @@ def load_library():
     lib.adept_read_scoring.argtypes = [vp, i, vp, sz, C.POINTER(CLedger), vp]
     lib.adept_read_leaked.argtypes = [vp, i, vp, sz, C.POINTER(sz)]
     lib.adept_get_stats.argtypes = [vp, i, C.POINTER(CStats)]
+    lib.adept_get_kernel_times.argtypes = [vp, i, vp, vp]
     lib.adept_step_frozen.argtypes = [vp, i, vp, vp, vp, vp]
     lib.adept_distance_batch.argtypes = [vp, i, i, vp, vp, vp, vp, vp, vp]
     lib.adept_locate_batch.argtypes = [vp, i, i, vp, vp, vp]
@@ -211,6 +212,13 @@ class Adept:
         s = CStats()
         _check(lib.adept_get_stats(self.ctx, slot, C.byref(s)))
         return s
+
+    def kernel_times(self, slot=0):
+        """(ms[2], launches[2]) of the gamma / charged step kernels since the last call (time_kernels=1)."""
+        ms = np.zeros(2)
+        n = np.zeros(2, dtype=np.uint64)
+        _check(lib.adept_get_kernel_times(self.ctx, slot, _ptr(ms), _ptr(n)))
+        return ms, n
 
     # ---- test hooks
     def step_frozen(self, tracks, stream=None):

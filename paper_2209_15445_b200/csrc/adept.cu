@@ -149,6 +149,11 @@ struct SlotHost {
   SlotCounters* pinned = nullptr;    // host mirror of the counters
   unsigned long long launches = 0;
   bool live = false;
+  // optional per-launch timing (config.time_kernels)
+  std::vector<cudaEvent_t> tev;      // [sync_interval][2 kernels][start, stop]
+  int tev_used = 0;
+  double kernel_ms[2] = {0.0, 0.0};
+  unsigned long long kernel_launches[2] = {0, 0};
 };
 
 struct adept_ctx {
@@ -368,6 +373,10 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
     CUDA_TRY(cudaEventCreateWithFlags(&sh.join, cudaEventDisableTiming));
     CUDA_TRY(cudaMallocHost(&sh.pinned, sizeof(SlotCounters)));
     std::memset(sh.pinned, 0, sizeof(SlotCounters));
+    if (cfg->time_kernels) {
+      sh.tev.resize(static_cast<size_t>(cfg->sync_interval) * 4);
+      for (cudaEvent_t& e : sh.tev) CUDA_TRY(cudaEventCreate(&e));
+    }
   }
   *out = ctx;
   return ADEPT_OK;
@@ -380,6 +389,7 @@ extern "C" int adept_shutdown(adept_ctx* ctx) {
     if (sh.fork) cudaEventDestroy(sh.fork);
     if (sh.join) cudaEventDestroy(sh.join);
     if (sh.pinned) cudaFreeHost(sh.pinned);
+    for (cudaEvent_t e : sh.tev) cudaEventDestroy(e);
   }
   delete ctx;
   return ADEPT_OK;
@@ -440,8 +450,14 @@ namespace {
 int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity) {
   CUDA_TRY(cudaEventRecord(sh.fork, st));
   CUDA_TRY(cudaStreamWaitEvent(sh.helper, sh.fork, 0));
+  const bool timed = !sh.tev.empty() && sh.tev_used + 4 <= static_cast<int>(sh.tev.size());
+  cudaEvent_t* ev = timed ? &sh.tev[sh.tev_used] : nullptr;
+  if (timed) CUDA_TRY(cudaEventRecord(ev[0], st));
   step_kernel<MODE_GAMMA><<<dim3(ctx->grid_gamma, 1), kBlock, 0, st>>>(ctx->dev, sh.dev, parity);
+  if (timed) CUDA_TRY(cudaEventRecord(ev[1], st));
+  if (timed) CUDA_TRY(cudaEventRecord(ev[2], sh.helper));
   step_kernel<MODE_CHARGED><<<dim3(ctx->grid_charged, 2), kBlock, 0, sh.helper>>>(ctx->dev, sh.dev, parity);
+  if (timed) { CUDA_TRY(cudaEventRecord(ev[3], sh.helper)); sh.tev_used += 4; }
   CUDA_TRY(cudaEventRecord(sh.join, sh.helper));
   CUDA_TRY(cudaStreamWaitEvent(st, sh.join, 0));
   finish_iteration_kernel<<<1, 1, 0, st>>>(sh.dev, parity);
@@ -478,6 +494,14 @@ extern "C" int adept_transport_many(adept_ctx* ctx, int n_slots, const int* slot
       SlotHost& sh = ctx->slots[slots[k]];
       if (!sh.live) continue;
       CUDA_TRY(cudaStreamSynchronize(static_cast<cudaStream_t>(streams[k])));
+      for (int e = 0; e + 4 <= sh.tev_used; e += 4)
+        for (int kk = 0; kk < 2; ++kk) {
+          float ms = 0.f;
+          CUDA_TRY(cudaEventElapsedTime(&ms, sh.tev[e + 2 * kk], sh.tev[e + 2 * kk + 1]));
+          sh.kernel_ms[kk] += ms;
+          sh.kernel_launches[kk] += 1;
+        }
+      sh.tev_used = 0;
       if (sh.pinned->overflow) rc_final = fail(ADEPT_EOVERFLOW, "slot %d: track queue overflow (capacity %llu per species)",
                                                slots[k], static_cast<unsigned long long>(ctx->cfg.track_capacity));
       if (sh.pinned->live == 0 || sh.pinned->overflow) {
@@ -537,6 +561,16 @@ extern "C" int adept_get_stats(adept_ctx* ctx, int slot, adept_stats* out) {
   for (int k = 0; k < ADEPT_N_OUTCOMES; ++k) out->outcomes[k] = s.outcomes[k];
   out->chords = s.chords; out->iterations = s.iterations; out->peak_population = s.peak_population;
   out->launches = ctx->slots[slot].launches;
+  return ADEPT_OK;
+}
+
+extern "C" int adept_get_kernel_times(adept_ctx* ctx, int slot, double ms[2], uint64_t launches[2]) {
+  const int rc = check_slot(ctx, slot);
+  if (rc != ADEPT_OK) return rc;
+  if (!ms || !launches) return fail(ADEPT_EINVAL, "null argument");
+  SlotHost& sh = ctx->slots[slot];
+  if (sh.tev.empty()) return fail(ADEPT_ESTATE, "context was not created with time_kernels");
+  for (int k = 0; k < 2; ++k) { ms[k] = sh.kernel_ms[k]; launches[k] = sh.kernel_launches[k]; sh.kernel_ms[k] = 0.0; sh.kernel_launches[k] = 0; }
   return ADEPT_OK;
 }
 

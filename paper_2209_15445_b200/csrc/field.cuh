@@ -119,7 +119,11 @@ __device__ int propagate(const DevCtx& c, int nav, bool active, int charge, doub
           flag = 2; running = false;
         } else {
           const double Rcurv = pmom / (kCB * bperp);
-          const double h_max = sqrt(8.0 * c.delta_chord * Rcurv);
+          double h_max = sqrt(8.0 * c.delta_chord * Rcurv);
+          if (c.field_kind == ADEPT_FIELD_MAP_RZ) {  // F2': at most 0.5 rad of turn per RK4 chord
+            const double Bn = sqrt(B[0] * B[0] + B[1] * B[1] + B[2] * B[2]);
+            h_max = fmin(h_max, 0.5 * pmom / (kCB * Bn));
+          }
           last = h_max >= rest;
           h = last ? rest : h_max;
           if (c.field_kind == ADEPT_FIELD_UNIFORM) helix(B, charge, pmom, h, pos, dir, p1, d1);

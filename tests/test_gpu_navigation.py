@@ -1,0 +1,69 @@
+"""Navigation parity: the warp-cooperative BVH navigator must return exactly what the loop navigator
+returns (a min over the same set), and both must match the oracle (rows A4, A5)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+def _rays(rng, n, r_lo, r_hi, phi_hi, z_half):
+    r, phi, z = rng.uniform(r_lo, r_hi, n), rng.uniform(0, phi_hi, n), rng.uniform(-z_half, z_half, n)
+    pos = np.stack([r * np.cos(phi), r * np.sin(phi), z], axis=1)
+    d = rng.normal(size=(n, 3))
+    return pos, d / np.linalg.norm(d, axis=1, keepdims=True)
+
+
+def test_full_barrel_bvh_equals_loop_bit_for_bit(barrel_full):
+    from paper_2209_15445_b200 import adept
+    from paper_2209_15445_b200.inputs import field
+    g, _, tabs, scal = barrel_full
+    a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=1 << 10)
+    rng = np.random.default_rng(1)
+    n = 4099                                            # several tiles and a ragged tail
+    pos, d = _rays(rng, n, 127.6, 152.9, 2 * np.pi, 289.0)
+    vol_bvh = a.locate_batch(pos, adept.NAV_BVH)
+    vol_loop = a.locate_batch(pos, adept.NAV_LOOP)
+    assert np.array_equal(vol_bvh, vol_loop)
+    assert (vol_bvh >= 12).sum() > 1000 and (vol_bvh == 11).sum() > 200
+    smax = np.where(rng.random(n) < 0.3, rng.uniform(0.01, 5.0, n), np.inf)
+    s_bvh = a.distance_batch(pos, d, vol_bvh, smax, adept.NAV_BVH)
+    s_loop = a.distance_batch(pos, d, vol_bvh, smax, adept.NAV_LOOP)
+    assert np.array_equal(s_bvh, s_loop)               # bit-exact
+    assert np.all(s_bvh <= smax) and np.all(s_bvh >= 0) and np.all(np.isfinite(s_bvh[np.isfinite(smax)]))
+    # rays started in the mother volume (gaps between crystals) exercise the BVH ray query
+    in_gap = vol_bvh == 11
+    assert np.array_equal(s_bvh[in_gap], s_loop[in_gap]) and in_gap.sum() > 100
+    # points outside the world
+    out = a.locate_batch(np.array([[400.0, 0, 0], [0, 0, 301.0]]), adept.NAV_BVH)
+    assert list(out) == [-1, -1]
+    a.close()
+
+
+def test_navigation_matches_oracle(ob, barrel_patch, calo):
+    from paper_2209_15445_b200 import adept
+    from paper_2209_15445_b200.inputs import field
+    rng = np.random.default_rng(2)
+    for geom_set, args in ((barrel_patch, (110.0, 160.0, 0.22, 20.0)), (barrel_patch, (0.0, 120.0, 2 * np.pi, 290.0))):
+        g, _, tabs, scal = geom_set
+        o = ob.Oracle(g, tabs, scal, field.no_field())
+        a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=1 << 10)
+        n = 1500
+        pos, d = _rays(rng, n, *args)
+        vol = a.locate_batch(pos)
+        want = np.array([o.locate(p) for p in pos])
+        assert np.array_equal(vol, want)
+        s = a.distance_batch(pos, d, vol)
+        ws = np.array([o.distance(pos[i], d[i], int(vol[i])) for i in range(n)])
+        np.testing.assert_allclose(s, ws, rtol=0, atol=1e-12 * 300.0)
+        a.close()
+    g, _, tabs, scal = calo
+    o = ob.Oracle(g, tabs, scal, field.no_field())
+    a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=1 << 10)
+    pos = np.stack([rng.uniform(-19, 59, 2000), rng.uniform(-29, 29, 2000), rng.uniform(-29, 29, 2000)], axis=1)
+    d = rng.normal(size=(2000, 3)); d /= np.linalg.norm(d, axis=1, keepdims=True)
+    vol = a.locate_batch(pos)
+    assert np.array_equal(vol, np.array([o.locate(p) for p in pos]))
+    s = a.distance_batch(pos, d, vol)
+    ws = np.array([o.distance(pos[i], d[i], int(vol[i])) for i in range(2000)])
+    np.testing.assert_allclose(s, ws, rtol=0, atol=1e-12 * 60.0)
+    a.close()
