@@ -40,6 +40,7 @@ def parse():
     ap.add_argument("--field", type=float, default=0.0, help="uniform Bz in tesla (config 3: 1.0)")
     ap.add_argument("--capacity", type=int, default=0, help="track capacity per species (0 = auto)")
     ap.add_argument("--sync-interval", type=int, default=8)
+    ap.add_argument("--split", type=int, default=1, help="1: move/relocate/interact kernels; 0: fused step kernels")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--profile", action="store_true",
                     help="for runs under ncu: take --warmup literally (the timed numbers of such a run are not bench values)")
@@ -168,7 +169,7 @@ def run_ours(args):
     g, tabs, scal, fld, prim = workload(args, first_event=rank * args.events)
     cap = args.capacity or max(1 << 20, 1024 * args.events)
     a = adept.Adept(g, tabs, scal, fld, device=str(dev), track_capacity=cap, sync_interval=args.sync_interval,
-                    time_kernels=1)
+                    time_kernels=1, split_kernels=args.split)
     stream = torch.cuda.Stream(device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
     edep_host = np.zeros(g.n_volumes)

@@ -164,7 +164,7 @@ struct adept_ctx {
   adept_track* d_stage = nullptr;    // staging area for primaries (inside the workspace)
   uint32_t* d_bad = nullptr;
   size_t stage_cap = 0;
-  int grid_gamma = 0, grid_charged = 0;
+  int grid_gamma = 0, grid_charged = 0, grid_reloc = 0, grid_inter = 0;
 };
 
 extern "C" const char* adept_last_error(void) { return g_err; }
@@ -186,7 +186,7 @@ int validate(const adept_config* cfg, const adept_geometry* g, int n_mats, const
   if (!g->solid || !g->dims || !g->material || !g->mother || !g->daughter_begin || !g->daughter_count || !g->rot || !g->trans)
     return fail(ADEPT_EINVAL, "null geometry array");
   if (cfg->n_event_slots < 1 || cfg->n_event_slots > 1024) return fail(ADEPT_EINVAL, "n_event_slots out of range");
-  if (cfg->track_capacity < 32 || cfg->track_capacity > 0x7fffffffu) return fail(ADEPT_EINVAL, "track_capacity out of range");
+  if (cfg->track_capacity < 32 || cfg->track_capacity > 0x3fffffffu) return fail(ADEPT_EINVAL, "track_capacity out of range");
   if (cfg->chord_budget < 1 || cfg->sync_interval < 1) return fail(ADEPT_EINVAL, "chord_budget / sync_interval must be >= 1");
   if (g->mother[0] != -1) return fail(ADEPT_EINVAL, "volume 0 must be the world");
   for (int v = 0; v < g->n_volumes; ++v) {
@@ -255,7 +255,7 @@ size_t carve(void* base, const adept_config* cfg, const adept_geometry* g, int n
     d.stats = cv.take<DevStats>(1);
     d.leaked = cv.take<adept_track>(std::max<size_t>(cfg->leak_capacity, 1));
     d.reloc_queue = cv.take<uint32_t>(cfg->split_kernels ? 3 * cap : 1);
-    d.inter_queue = cv.take<uint32_t>(cfg->split_kernels ? 3 * cap : 1);
+    d.inter_queue = cv.take<uint32_t>(cfg->split_kernels ? 7 * cap : 1);
     L.slots.push_back(d);
   }
   if (out) *out = std::move(L);
@@ -361,6 +361,15 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_g, step_kernel<MODE_GAMMA>, kBlock, 0));
   CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_c, step_kernel<MODE_CHARGED>, kBlock, 0));
+  if (cfg->split_kernels) {
+    int occ_r = 1, occ_i = 1;
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_g, move_kernel<MODE_GAMMA>, kBlock, 0));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_c, move_kernel<MODE_CHARGED>, kBlock, 0));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_r, relocate_kernel, kBlock, 0));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_i, interact_kernel, kBlock, 0));
+    ctx->grid_reloc = sms * std::max(occ_r, 1);
+    ctx->grid_inter = sms * std::max(occ_i, 1);
+  }
   ctx->grid_gamma = sms * std::max(occ_g, 1);
   ctx->grid_charged = sms * std::max(occ_c, 1);
 
@@ -452,12 +461,25 @@ int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity) 
   CUDA_TRY(cudaStreamWaitEvent(sh.helper, sh.fork, 0));
   const bool timed = !sh.tev.empty() && sh.tev_used + 4 <= static_cast<int>(sh.tev.size());
   cudaEvent_t* ev = timed ? &sh.tev[sh.tev_used] : nullptr;
+  const bool split = ctx->cfg.split_kernels != 0;
   if (timed) CUDA_TRY(cudaEventRecord(ev[0], st));
-  step_kernel<MODE_GAMMA><<<dim3(ctx->grid_gamma, 1), kBlock, 0, st>>>(ctx->dev, sh.dev, parity);
+  if (split) move_kernel<MODE_GAMMA><<<dim3(ctx->grid_gamma, 1), kBlock, 0, st>>>(ctx->dev, sh.dev, parity);
+  else step_kernel<MODE_GAMMA><<<dim3(ctx->grid_gamma, 1), kBlock, 0, st>>>(ctx->dev, sh.dev, parity);
   if (timed) CUDA_TRY(cudaEventRecord(ev[1], st));
   if (timed) CUDA_TRY(cudaEventRecord(ev[2], sh.helper));
-  step_kernel<MODE_CHARGED><<<dim3(ctx->grid_charged, 2), kBlock, 0, sh.helper>>>(ctx->dev, sh.dev, parity);
+  if (split) move_kernel<MODE_CHARGED><<<dim3(ctx->grid_charged, 2), kBlock, 0, sh.helper>>>(ctx->dev, sh.dev, parity);
+  else step_kernel<MODE_CHARGED><<<dim3(ctx->grid_charged, 2), kBlock, 0, sh.helper>>>(ctx->dev, sh.dev, parity);
   if (timed) { CUDA_TRY(cudaEventRecord(ev[3], sh.helper)); sh.tev_used += 4; }
+  if (split) {
+    // relocation on the caller's stream, interactions on the helper stream: they touch disjoint tracks
+    CUDA_TRY(cudaEventRecord(sh.join, sh.helper));
+    CUDA_TRY(cudaStreamWaitEvent(st, sh.join, 0));
+    CUDA_TRY(cudaEventRecord(sh.fork, st));
+    CUDA_TRY(cudaStreamWaitEvent(sh.helper, sh.fork, 0));
+    relocate_kernel<<<ctx->grid_reloc, kBlock, 0, st>>>(ctx->dev, sh.dev, parity);
+    interact_kernel<<<ctx->grid_inter, kBlock, 0, sh.helper>>>(ctx->dev, sh.dev, parity);
+    sh.launches += 2;
+  }
   CUDA_TRY(cudaEventRecord(sh.join, sh.helper));
   CUDA_TRY(cudaStreamWaitEvent(st, sh.join, 0));
   finish_iteration_kernel<<<1, 1, 0, st>>>(sh.dev, parity);

@@ -126,7 +126,7 @@ __device__ __forceinline__ bool inside_volume(const DevCtx& c, int vol, double x
   return inside_solid(v.solid, v.dims, l);
 }
 
-__device__ __forceinline__ double entry_distance(const DevCtx& c, int vol, double px, double py, double pz,
+__device__ __noinline__ double entry_distance(const DevCtx& c, int vol, double px, double py, double pz,
                                                  double dx, double dy, double dz) {
   const DevVolume& v = volume(c, vol);
   double lp[3], ld[3];
@@ -171,7 +171,7 @@ __device__ __forceinline__ bool point_box(const double* __restrict__ box, int st
 
 // All arguments warp-uniform.  Returns min(best, nearest daughter entry distance).  The traversal
 // state is a short stack of one 32-bit child mask per level, shared by the warp.
-__device__ double bvh_ray(const DevCtx& c, const DevBvh& b, double px, double py, double pz, double dx, double dy,
+__device__ __noinline__ double bvh_ray(const DevCtx& c, const DevBvh& b, double px, double py, double pz, double dx, double dy,
                           double dz, double best) {
   const int lane = threadIdx.x & 31;
   const double ix = 1.0 / dx, iy = 1.0 / dy, iz = 1.0 / dz;
@@ -210,7 +210,7 @@ __device__ double bvh_ray(const DevCtx& c, const DevBvh& b, double px, double py
 }
 
 // All arguments warp-uniform.  Lowest touchable id among the daughters containing the point, or -1.
-__device__ int bvh_point(const DevCtx& c, const DevBvh& b, double px, double py, double pz) {
+__device__ __noinline__ int bvh_point(const DevCtx& c, const DevBvh& b, double px, double py, double pz) {
   const int lane = threadIdx.x & 31;
   const int top = b.n_levels - 1;
   unsigned mask[kBvhMaxLevels];
@@ -249,7 +249,7 @@ __device__ int bvh_point(const DevCtx& c, const DevBvh& b, double px, double py,
 // ---------------------------------------------------------------- G3 distance to boundary
 // min(exit distance of the own solid, entry distance of every daughter), capped at s_max.
 // Warp-convergent call; lanes with active == false return s_max.
-__device__ double nav_distance(const DevCtx& c, int nav, bool active, double px, double py, double pz, double dx,
+__device__ __noinline__ double nav_distance(const DevCtx& c, int nav, bool active, double px, double py, double pz, double dx,
                                double dy, double dz, uint32_t vol, double s_max) {
   const int lane = threadIdx.x & 31;
   double s = s_max;
@@ -285,7 +285,7 @@ __device__ double nav_distance(const DevCtx& c, int nav, bool active, double px,
 // ---------------------------------------------------------------- G4 Locate
 // From the world down, descend into the first daughter (index order) containing the point.
 // Warp-convergent call; returns -1 outside the world or for inactive lanes.
-__device__ int nav_locate(const DevCtx& c, int nav, bool active, double qx, double qy, double qz) {
+__device__ __noinline__ int nav_locate(const DevCtx& c, int nav, bool active, double qx, double qy, double qz) {
   const int lane = threadIdx.x & 31;
   int cur = -1;
   bool desc = false;

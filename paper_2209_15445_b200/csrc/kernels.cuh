@@ -66,9 +66,81 @@ struct BlockTally {
   unsigned long long steps, chords;
   unsigned long long outcomes[ADEPT_N_OUTCOMES];
   unsigned long long secondaries[3];
+  unsigned int touched;
 };
 
-// Steps every track of one species queue once.  grid.y selects the species of a charged launch.
+// per-thread partial sums, folded into the block tally at the end of the kernel
+struct LaneTally {
+  double dep = 0.0, cut = 0.0, esc = 0.0, kill = 0.0;
+  unsigned steps = 0, chords = 0;
+};
+
+__device__ __forceinline__ void flush_tally(BlockTally& tally, const LaneTally& l, const DevSlot& slot, int species) {
+  const int lane = threadIdx.x & 31;
+  const double dep = warp_sum(l.dep), cut = warp_sum(l.cut), esc = warp_sum(l.esc), kill = warp_sum(l.kill);
+  if (lane == 0) {
+    if (dep != 0.0) atomicAdd(&tally.ledger[0], dep);
+    if (cut != 0.0) atomicAdd(&tally.ledger[1], cut);
+    if (esc != 0.0) atomicAdd(&tally.ledger[2], esc);
+    if (kill != 0.0) atomicAdd(&tally.ledger[3], kill);
+  }
+  if (l.steps) {
+    atomicAdd(&tally.steps, static_cast<unsigned long long>(l.steps));
+    atomicAdd(&tally.chords, static_cast<unsigned long long>(l.chords));
+  }
+  __syncthreads();
+  if (threadIdx.x == 0 && tally.touched) {
+    for (int k = 0; k < 4; ++k) if (tally.ledger[k] != 0.0) atomicAdd(slot.ledger + k, tally.ledger[k]);
+    if (tally.steps) atomicAdd(&slot.stats->steps[species], tally.steps);
+    if (tally.chords) atomicAdd(&slot.stats->chords, tally.chords);
+    for (int k = 0; k < ADEPT_N_OUTCOMES; ++k) if (tally.outcomes[k]) atomicAdd(&slot.stats->outcomes[k], tally.outcomes[k]);
+    for (int k = 0; k < 3; ++k) if (tally.secondaries[k]) atomicAdd(&slot.stats->secondaries[k], tally.secondaries[k]);
+  }
+}
+
+// Appends the secondaries of a step to the next buffers: one warp-aggregated atomic per (k, species).
+// Warp-convergent.  `u` is the parent's stream (child ids, R3).
+__device__ __forceinline__ void append_secondaries(const DevCtx& c, const DevSlot& slot, int parity, bool active,
+                                                   uint32_t event, const Stream& u, const StepOut& o, BlockTally& tally) {
+  SlotCounters* cnt = slot.counters;
+#pragma unroll
+  for (int k = 0; k < 2; ++k) {
+    const int ss = (active && k < o.n_sec) ? o.sec[k].species : -1;
+    if (__ballot_sync(kFull, ss >= 0) == 0) continue;
+    const uint64_t cid = ss >= 0 ? u.child_id(o.sec[k].child) : 0;
+#pragma unroll
+    for (int sp = 0; sp < 3; ++sp) {
+      const bool want = ss == sp;
+      const uint32_t j = warp_append(&cnt->count[parity ^ 1][sp], want);
+      if (want) {
+        if (j < c.capacity) {
+          Track s;
+          s.x = o.post.x; s.y = o.post.y; s.z = o.post.z;
+          s.dx = o.sec[k].dx; s.dy = o.sec[k].dy; s.dz = o.sec[k].dz;
+          s.ekin = o.sec[k].ekin; s.id = cid; s.event = event; s.step = 0; s.vol = o.post.vol; s.species = sp;
+          store_track(slot.buf[parity ^ 1][sp], j, s);
+          atomicAdd(&tally.secondaries[sp], 1ull);
+        } else {
+          cnt->overflow = 1;
+        }
+      }
+    }
+  }
+}
+
+__device__ __forceinline__ void record_leak(const DevCtx& c, const DevSlot& slot, const Track& t, int species) {
+  const uint32_t j = atomicAdd(&slot.counters->n_leaked, 1u);
+  if (j < c.leak_capacity) {
+    adept_track& L = slot.leaked[j];
+    L.pos[0] = t.x; L.pos[1] = t.y; L.pos[2] = t.z;
+    L.dir[0] = t.dx; L.dir[1] = t.dy; L.dir[2] = t.dz;
+    L.ekin = t.ekin; L.id = t.id; L.event = t.event; L.step = t.step; L.volume = kDeadVolume;
+    L.species = species;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Fused mode: one kernel per species group does the whole step.  grid.y = species of a charged launch.
 template <int MODE>
 __global__ void __launch_bounds__(kBlock) step_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot,
                                                       int parity) {
@@ -76,99 +148,210 @@ __global__ void __launch_bounds__(kBlock) step_kernel(const __grid_constant__ De
   const TrackSoA& cur = slot.buf[parity][species];
   SlotCounters* cnt = slot.counters;
   const uint32_t n = cnt->count[parity][species];
-  const int lane = threadIdx.x & 31;
 
   __shared__ BlockTally tally;
   if (threadIdx.x == 0) tally = BlockTally{};
   __syncthreads();
-
-  double l_dep = 0.0, l_cut = 0.0, l_esc = 0.0, l_kill = 0.0;
-  unsigned l_steps = 0, l_chords = 0;
+  LaneTally lt;
 
   const uint32_t n_round = (n + 31u) & ~31u;
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += gridDim.x * blockDim.x) {
-    const bool active = i < n;
+    bool active = i < n;
     Track in{};
     if (active) in = load_track(cur, i, species);
     in.species = species;
+    active = active && in.vol != kDeadVolume;
     StepOut o;
     step_track<MODE>(c, c.navigator, active, in, o);
 
-    // scoring (A9) and ledger
     score(slot.edep, in.vol, o.edep_dep + o.edep_cut, active);
     if (active) {
-      l_dep += o.edep_dep; l_cut += o.edep_cut; l_esc += o.escaped; l_kill += o.killed;
-      ++l_steps; l_chords += o.chords;
+      lt.dep += o.edep_dep; lt.cut += o.edep_cut; lt.esc += o.escaped; lt.kill += o.killed;
+      ++lt.steps; lt.chords += o.chords;
       atomicAdd(&tally.outcomes[o.outcome], 1ull);
+      tally.touched = 1;
     }
-    // survivors -> next buffer of the same species
     const bool live = active && o.alive;
-    {
-      const uint32_t j = warp_append(&cnt->count[parity ^ 1][species], live);
-      if (live) {
-        if (j < c.capacity) store_track(slot.buf[parity ^ 1][species], j, o.post);
-        else cnt->overflow = 1;
-      }
+    const uint32_t j = warp_append(&cnt->count[parity ^ 1][species], live);
+    if (live) {
+      if (j < c.capacity) store_track(slot.buf[parity ^ 1][species], j, o.post);
+      else cnt->overflow = 1;
     }
-    // secondaries -> next buffers, one warp-aggregated append per (slot k, species)
-#pragma unroll
-    for (int k = 0; k < 2; ++k) {
-      const int ss = (active && k < o.n_sec) ? o.sec[k].species : -1;
-      if (__ballot_sync(kFull, ss >= 0) == 0) continue;
-      uint64_t cid = 0;
-      if (ss >= 0) {
-        Stream u;
-        u.init(in.event, c.seed, in.id, in.step);
-        cid = u.child_id(o.sec[k].child);
-      }
-#pragma unroll
-      for (int sp = 0; sp < 3; ++sp) {
-        const bool want = ss == sp;
-        const uint32_t j = warp_append(&cnt->count[parity ^ 1][sp], want);
-        if (want) {
-          if (j < c.capacity) {
-            Track s;
-            s.x = o.post.x; s.y = o.post.y; s.z = o.post.z;
-            s.dx = o.sec[k].dx; s.dy = o.sec[k].dy; s.dz = o.sec[k].dz;
-            s.ekin = o.sec[k].ekin; s.id = cid; s.event = in.event; s.step = 0; s.vol = o.post.vol; s.species = sp;
-            store_track(slot.buf[parity ^ 1][sp], j, s);
-            atomicAdd(&tally.secondaries[sp], 1ull);
-          } else {
-            cnt->overflow = 1;
-          }
-        }
-      }
-    }
-    // outgoing particles
-    if (active && o.outcome == ADEPT_OUT_ESCAPED) {
-      const uint32_t j = atomicAdd(&cnt->n_leaked, 1u);
-      if (j < c.leak_capacity) {
-        adept_track& L = slot.leaked[j];
-        L.pos[0] = o.post.x; L.pos[1] = o.post.y; L.pos[2] = o.post.z;
-        L.dir[0] = o.post.dx; L.dir[1] = o.post.dy; L.dir[2] = o.post.dz;
-        L.ekin = o.post.ekin; L.id = in.id; L.event = in.event; L.step = in.step + 1; L.volume = kDeadVolume;
-        L.species = species;
-      }
-    }
+    Stream u;
+    u.init(in.event, c.seed, in.id, in.step);
+    append_secondaries(c, slot, parity, active, in.event, u, o, tally);
+    if (active && o.outcome == ADEPT_OUT_ESCAPED) { o.post.step = in.step + 1; record_leak(c, slot, o.post, species); }
   }
+  flush_tally(tally, lt, slot, species);
+}
 
-  // block-level tallies -> one set of global atomics per block
-  l_dep = warp_sum(l_dep); l_cut = warp_sum(l_cut); l_esc = warp_sum(l_esc); l_kill = warp_sum(l_kill);
-  if (lane == 0) {
-    if (l_dep != 0.0) atomicAdd(&tally.ledger[0], l_dep);
-    if (l_cut != 0.0) atomicAdd(&tally.ledger[1], l_cut);
-    if (l_esc != 0.0) atomicAdd(&tally.ledger[2], l_esc);
-    if (l_kill != 0.0) atomicAdd(&tally.ledger[3], l_kill);
-  }
-  if (l_steps) { atomicAdd(&tally.steps, static_cast<unsigned long long>(l_steps)); atomicAdd(&tally.chords, static_cast<unsigned long long>(l_chords)); }
+// ------------------------------------------------------------------------------------------------
+// Split mode: move kernels leave relocation and interactions to their own kernels.
+//   reloc_queue entry: species << 30 | index into the next buffer of that species
+//   inter_queue[q][k]: same encoding, q = 0 Compton, 1 pair, 2 photoelectric, 3 brems, 4 Moller, 5 annihilation, 6 Bhabha
+constexpr int kNumInterQueues = 7;
+
+__device__ __forceinline__ int inter_queue_index(int process, int species) {
+  return (process == ADEPT_OUT_IONI && species == ADEPT_POSITRON) ? 6 : process - 1;
+}
+__device__ __forceinline__ int inter_queue_process(int q) { return q == 6 ? ADEPT_OUT_IONI : q + 1; }
+
+template <int MODE>
+__global__ void __launch_bounds__(kBlock) move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot,
+                                                      int parity) {
+  const int species = MODE == MODE_GAMMA ? ADEPT_GAMMA : static_cast<int>(blockIdx.y);
+  const TrackSoA& cur = slot.buf[parity][species];
+  SlotCounters* cnt = slot.counters;
+  const uint32_t n = cnt->count[parity][species];
+
+  __shared__ BlockTally tally;
+  if (threadIdx.x == 0) tally = BlockTally{};
   __syncthreads();
-  if (threadIdx.x == 0 && tally.steps) {
-    for (int k = 0; k < 4; ++k) if (tally.ledger[k] != 0.0) atomicAdd(slot.ledger + k, tally.ledger[k]);
-    atomicAdd(&slot.stats->steps[species], tally.steps);
-    atomicAdd(&slot.stats->chords, tally.chords);
-    for (int k = 0; k < ADEPT_N_OUTCOMES; ++k) if (tally.outcomes[k]) atomicAdd(&slot.stats->outcomes[k], tally.outcomes[k]);
-    for (int k = 0; k < 3; ++k) if (tally.secondaries[k]) atomicAdd(&slot.stats->secondaries[k], tally.secondaries[k]);
+  LaneTally lt;
+
+  const uint32_t n_round = (n + 31u) & ~31u;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += gridDim.x * blockDim.x) {
+    bool active = i < n;
+    Track in{};
+    if (active) in = load_track(cur, i, species);
+    in.species = species;
+    active = active && in.vol != kDeadVolume;
+    StepOut o;
+    Stream u;
+    int process, mat;
+    const int next = step_move<MODE>(c, c.navigator, active, in, o, u, process, mat);
+
+    score(slot.edep, in.vol, o.edep_dep + o.edep_cut, active);
+    if (active) {
+      lt.dep += o.edep_dep; lt.cut += o.edep_cut; lt.kill += o.killed;
+      ++lt.steps; lt.chords += o.chords;
+      if (next == NEXT_NONE) atomicAdd(&tally.outcomes[o.outcome], 1ull);
+      tally.touched = 1;
+    }
+    const bool live = active && o.alive;
+    const uint32_t j = warp_append(&cnt->count[parity ^ 1][species], live);
+    const bool stored = live && j < c.capacity;
+    if (live) {
+      o.post.step = in.step + 1;
+      if (stored) store_track(slot.buf[parity ^ 1][species], j, o.post);
+      else cnt->overflow = 1;
+    }
+    const uint32_t entry = (static_cast<uint32_t>(species) << 30) | j;
+    {
+      const bool want = stored && next == NEXT_RELOCATE;
+      const uint32_t k = warp_append(&cnt->n_reloc, want);
+      if (want) slot.reloc_queue[k] = entry;
+    }
+    const int q = (stored && next == NEXT_INTERACT) ? inter_queue_index(process, species) : -1;
+#pragma unroll
+    for (int qq = 0; qq < kNumInterQueues; ++qq) {
+      const bool mine = MODE == MODE_GAMMA ? qq < 3 : qq >= 3;   // queues this kernel can feed
+      if (!mine) continue;
+      const bool want = q == qq;
+      const uint32_t k = warp_append(&cnt->n_inter[qq], want);
+      if (want) slot.inter_queue[static_cast<size_t>(qq) * c.capacity + k] = entry;
+    }
+    append_secondaries(c, slot, parity, active, in.event, u, o, tally);   // at-rest annihilation photons
   }
+  flush_tally(tally, lt, slot, species);
+}
+
+__global__ void __launch_bounds__(kBlock) relocate_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot,
+                                                          int parity) {
+  SlotCounters* cnt = slot.counters;
+  const uint32_t n = cnt->n_reloc;
+  __shared__ BlockTally tally;
+  if (threadIdx.x == 0) tally = BlockTally{};
+  __syncthreads();
+  LaneTally lt;
+  const uint32_t n_round = (n + 31u) & ~31u;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += gridDim.x * blockDim.x) {
+    const bool active = i < n;
+    uint32_t entry = 0;
+    if (active) entry = slot.reloc_queue[i];
+    const int species = entry >> 30;
+    const uint32_t j = entry & 0x3fffffffu;
+    const TrackSoA& b = slot.buf[parity ^ 1][species];
+    double x = 0.0, y = 0.0, z = 0.0;
+    if (active) { x = b.x[j]; y = b.y[j]; z = b.z[j]; }
+    const int nv = nav_locate(c, c.navigator, active, x, y, z);
+    if (!active) continue;
+    tally.touched = 1;
+    if (nv >= 0) {
+      b.vol[j] = static_cast<uint32_t>(nv);
+      atomicAdd(&tally.outcomes[ADEPT_OUT_BOUNDARY], 1ull);
+    } else {
+      Track t = load_track(b, j, species);
+      b.vol[j] = kDeadVolume;
+      lt.esc += carried_energy(species, t.ekin);
+      record_leak(c, slot, t, species);
+      atomicAdd(&tally.outcomes[ADEPT_OUT_ESCAPED], 1ull);
+    }
+  }
+  {
+    const int lane = threadIdx.x & 31;
+    const double esc = warp_sum(lt.esc);
+    if (lane == 0 && esc != 0.0) atomicAdd(&tally.ledger[2], esc);
+    __syncthreads();
+    if (threadIdx.x == 0 && tally.touched) {
+      if (tally.ledger[2] != 0.0) atomicAdd(slot.ledger + 2, tally.ledger[2]);
+      if (tally.outcomes[ADEPT_OUT_BOUNDARY]) atomicAdd(&slot.stats->outcomes[ADEPT_OUT_BOUNDARY], tally.outcomes[ADEPT_OUT_BOUNDARY]);
+      if (tally.outcomes[ADEPT_OUT_ESCAPED]) atomicAdd(&slot.stats->outcomes[ADEPT_OUT_ESCAPED], tally.outcomes[ADEPT_OUT_ESCAPED]);
+    }
+  }
+}
+
+// Every warp works on one process queue at a time, so the rejection loops of different processes never
+// share a warp (PAPER.md:101 names divergence between processes as a main cost).
+__global__ void __launch_bounds__(kBlock) interact_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot,
+                                                          int parity) {
+  SlotCounters* cnt = slot.counters;
+  __shared__ BlockTally tally;
+  __shared__ uint32_t warp_begin[kNumInterQueues + 1];   // prefix of 32-lane groups per queue
+  if (threadIdx.x == 0) {
+    tally = BlockTally{};
+    uint32_t acc = 0;
+    for (int q = 0; q < kNumInterQueues; ++q) { warp_begin[q] = acc; acc += (cnt->n_inter[q] + 31u) >> 5; }
+    warp_begin[kNumInterQueues] = acc;
+  }
+  __syncthreads();
+  LaneTally lt;
+  const int lane = threadIdx.x & 31;
+  const uint32_t warps_per_grid = gridDim.x * (blockDim.x >> 5);
+  const uint32_t total = warp_begin[kNumInterQueues];
+  for (uint32_t w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); w < total; w += warps_per_grid) {
+    int q = 0;
+    while (w >= warp_begin[q + 1]) ++q;
+    const uint32_t i = ((w - warp_begin[q]) << 5) + lane;
+    const bool active = i < cnt->n_inter[q];
+    StepOut o;
+    Stream u;
+    Track t{};
+    uint32_t j = 0;
+    int species = 0;
+    if (active) {
+      const uint32_t entry = slot.inter_queue[static_cast<size_t>(q) * c.capacity + i];
+      species = entry >> 30;
+      j = entry & 0x3fffffffu;
+      t = load_track(slot.buf[parity ^ 1][species], j, species);
+      init_out(o, t, true);
+      u.init(t.event, c.seed, t.id, t.step - 1);          // the stream of the step that chose the process
+      const int mat = volume(c, t.vol).material;
+      run_process(c, inter_queue_process(q), species, mat, o, u);
+      const TrackSoA& b = slot.buf[parity ^ 1][species];
+      if (o.alive) { b.dx[j] = o.post.dx; b.dy[j] = o.post.dy; b.dz[j] = o.post.dz; b.ekin[j] = o.post.ekin; }
+      else b.vol[j] = kDeadVolume;
+      lt.cut += o.edep_cut;
+      atomicAdd(&tally.outcomes[o.outcome], 1ull);
+      tally.touched = 1;
+    } else {
+      init_out(o, t, false);
+      u.init(0, 0, 0, 0);
+    }
+    score(slot.edep, t.vol, o.edep_cut, active);
+    append_secondaries(c, slot, parity, active, t.event, u, o, tally);
+  }
+  flush_tally(tally, lt, slot, 0);
 }
 
 // End of one population step: the just-consumed buffers become the next step's output buffers.
@@ -178,6 +361,8 @@ __global__ void finish_iteration_kernel(const __grid_constant__ DevSlot slot, in
   cnt->count[parity][0] = cnt->count[parity][1] = cnt->count[parity][2] = 0;
   const uint32_t live = cnt->count[parity ^ 1][0] + cnt->count[parity ^ 1][1] + cnt->count[parity ^ 1][2];
   cnt->live = live;
+  cnt->n_reloc = 0;
+  for (int q = 0; q < 8; ++q) cnt->n_inter[q] = 0;
   if (before) {
     slot.stats->iterations += 1;
     if (before > slot.stats->peak_population) slot.stats->peak_population = before;

@@ -24,7 +24,7 @@ __device__ __forceinline__ double interp(const double* __restrict__ tab, int row
 
 // M7 inverse range: cell j with R_j <= r < R_{j+1}, found by galloping down from the cell of the
 // pre-step energy (any search returns the same j).  Returns 0 when r < R_0 (the track stops).
-__device__ __forceinline__ double inverse_range(const DevCtx& c, const double* __restrict__ tab, int row, int col,
+__device__ __noinline__ double inverse_range(const DevCtx& c, const double* __restrict__ tab, int row, int col,
                                                 int i_start, double r) {
   if (r < __ldg(tab + col)) return 0.0;
   int hi = min(i_start + 1, kNGrid - 1);  // R[hi] > r is guaranteed by r < R(T) <= R[i_start+1]
@@ -43,7 +43,7 @@ __device__ __forceinline__ double inverse_range(const DevCtx& c, const double* _
 }
 
 // P10 rotation of d by polar (cos_t, sin_t) and azimuth phi
-__device__ __forceinline__ void rotate(const double d[3], double cos_t, double sin_t, double phi, double out[3]) {
+__device__ __noinline__ void rotate(const double d[3], double cos_t, double sin_t, double phi, double out[3]) {
   const double rho2 = d[0] * d[0] + d[1] * d[1];
   const double rho = sqrt(rho2);
   double e1[3], e2[3];
@@ -83,7 +83,7 @@ __device__ __forceinline__ void emit(const DevCtx& c, int mat, StepOut& o, int s
 }
 
 // ---- P1 Klein-Nishina Compton
-__device__ void compton(const DevCtx& c, int mat, StepOut& o, Stream& u) {
+__device__ __noinline__ void compton(const DevCtx& c, int mat, StepOut& o, Stream& u) {
   Track& g = o.post;
   const double k = g.ekin, kap = k / kMe;
   const double e0 = 1.0 / (1.0 + 2.0 * kap);
@@ -117,7 +117,7 @@ __device__ void compton(const DevCtx& c, int mat, StepOut& o, Stream& u) {
 }
 
 // ---- P2 Bethe-Heitler pair, complete screening
-__device__ void pair_production(const DevCtx& c, int mat, StepOut& o, Stream& u) {
+__device__ __noinline__ void pair_production(const DevCtx& c, int mat, StepOut& o, Stream& u) {
   Track& g = o.post;
   const double k = g.ekin, a = kMe / k;
   const double fmax_ = 1.0 - (4.0 / 3.0) * a * (1.0 - a);
@@ -157,7 +157,7 @@ __device__ void photoelectric(const DevCtx& c, int mat, StepOut& o) {
 }
 
 // ---- P4 bremsstrahlung; false when kinematically closed
-__device__ bool bremsstrahlung(const DevCtx& c, int mat, StepOut& o, Stream& u) {
+__device__ __noinline__ bool bremsstrahlung(const DevCtx& c, int mat, StepOut& o, Stream& u) {
   Track& e = o.post;
   const double T = e.ekin, kc = mat_scalar(c, mat, S_KCUT);
   if (!(T > kc)) return false;
@@ -198,7 +198,7 @@ __device__ __forceinline__ void delta_ray(const DevCtx& c, int mat, StepOut& o, 
 }
 
 // ---- P5 Moller
-__device__ bool moller(const DevCtx& c, int mat, StepOut& o, Stream& u) {
+__device__ __noinline__ bool moller(const DevCtx& c, int mat, StepOut& o, Stream& u) {
   const double T = o.post.ekin, Tc = mat_scalar(c, mat, S_TCUT);
   if (!(T > 2.0 * Tc)) return false;
   const double g = 1.0 + T / kMe, g2 = g * g;
@@ -218,7 +218,7 @@ __device__ bool moller(const DevCtx& c, int mat, StepOut& o, Stream& u) {
 }
 
 // ---- P6 Bhabha
-__device__ bool bhabha(const DevCtx& c, int mat, StepOut& o, Stream& u) {
+__device__ __noinline__ bool bhabha(const DevCtx& c, int mat, StepOut& o, Stream& u) {
   const double T = o.post.ekin, Tc = mat_scalar(c, mat, S_TCUT);
   if (!(T > Tc)) return false;
   const double g = 1.0 + T / kMe;
@@ -240,7 +240,7 @@ __device__ bool bhabha(const DevCtx& c, int mat, StepOut& o, Stream& u) {
 }
 
 // ---- P8 annihilation in flight (Heitler)
-__device__ void annihilation(const DevCtx& c, int mat, StepOut& o, Stream& u) {
+__device__ __noinline__ void annihilation(const DevCtx& c, int mat, StepOut& o, Stream& u) {
   Track& e = o.post;
   const double T = e.ekin, g = 1.0 + T / kMe;
   const double root = sqrt((g - 1.0) / (g + 1.0));
@@ -270,7 +270,7 @@ __device__ void annihilation(const DevCtx& c, int mat, StepOut& o, Stream& u) {
 }
 
 // ---- P8 at rest: two photons of energy m back to back, cos(theta) = 2 U4 - 1, phi = 2 pi U5
-__device__ __forceinline__ void annihilation_at_rest(const DevCtx& c, int mat, StepOut& o, Stream& u) {
+__device__ __noinline__ void annihilation_at_rest(const DevCtx& c, int mat, StepOut& o, Stream& u) {
   const double u4 = u.uniform(4), u5 = u.uniform(5);
   const double cos_t = 2.0 * u4 - 1.0, sin_t = sqrt(fmax(0.0, 1.0 - cos_t * cos_t));
   double sp, cp;

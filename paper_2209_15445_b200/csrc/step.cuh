@@ -1,6 +1,11 @@
-// One transport step of one track per lane  (rows A2-A8).  Warp-convergent:
-// every lane of the warp calls step_track (inactive lanes pass active = false) because propagation
-// and relocation use the warp-cooperative navigator.
+// One transport step of one track per lane  (rows A2-A8), in three phases that
+// the kernels either chain (frozen-step hook, fused mode) or run as separate kernels with work queues
+// in between (split mode, "a separate kernel ... to improve load balancing"):
+//   move      step-start rules, physics step limit, propagation, continuous loss, MSC, process choice
+//   relocate  push past the boundary and Locate (A5)
+//   interact  sample the discrete process, create secondaries (A8)
+// move and relocate are warp-convergent: every lane of the warp must call them (inactive lanes pass
+// active = false) because propagation and Locate use the warp-cooperative navigator.
 #pragma once
 #include "field.cuh"
 #include "physics.cuh"
@@ -9,26 +14,36 @@ namespace adept {
 
 enum { MODE_ANY = 0, MODE_GAMMA = 1, MODE_CHARGED = 2 };
 
+// what the move phase leaves to do
+enum { NEXT_NONE = 0, NEXT_RELOCATE = 1, NEXT_INTERACT = 2 };
+
 __device__ __forceinline__ double carried_energy(int species, double ekin) {
   return species == ADEPT_POSITRON ? ekin + 2.0 * kMe : ekin;
 }
 
-template <int MODE>
-__device__ void step_track(const DevCtx& c, int nav, bool active, const Track& in, StepOut& o) {
+__device__ __forceinline__ void init_out(StepOut& o, const Track& in, bool active) {
   o.post = in;
   o.alive = active ? 1 : 0;
   o.outcome = ADEPT_OUT_BOUNDARY;
   o.chords = 0; o.n_sec = 0;
   o.s = 0.0; o.edep_dep = 0.0; o.edep_cut = 0.0; o.escaped = 0.0; o.killed = 0.0;
   o.sec[0].species = -1; o.sec[1].species = -1;
+}
 
+// Phase 1.  On return o.post holds the moved state (position already pushed past the boundary when
+// the result is NEXT_RELOCATE), `process` the chosen discrete process for NEXT_INTERACT, and `mat`
+// the material of the pre-step volume.  o.post.step is NOT yet incremented.
+template <int MODE>
+__device__ int step_move(const DevCtx& c, int nav, bool active, const Track& in, StepOut& o, Stream& u, int& process,
+                         int& mat) {
+  init_out(o, in, active);
   const bool is_gamma = MODE == MODE_GAMMA || (MODE == MODE_ANY && in.species == ADEPT_GAMMA);
   const bool positron = !is_gamma && in.species == ADEPT_POSITRON;
-  Stream u;
   u.init(in.event, c.seed, in.id, in.step);
+  process = 0;
+  mat = 0;
 
   bool go = active;
-  int mat = 0;
   bool vacuum = true, lim_disc = false, range_out = false;
   double s_phys = 0.0, stot = 0.0, x0 = 0.0, x1 = 0.0, S = 0.0, R = ADEPT_INF;
   GridPos gp{0, 0.0};
@@ -43,8 +58,8 @@ __device__ void step_track(const DevCtx& c, int nav, bool active, const Track& i
     } else if (T0 < kTmin) {
       o.edep_cut += T0; o.alive = 0; o.outcome = ADEPT_OUT_STOPPED; go = false;
       mat = volume(c, in.vol).material;
-      if (positron) { o.post.ekin = 0.0; annihilation_at_rest(c, mat, o, u); }
       if (!is_gamma) o.post.ekin = 0.0;
+      if (positron) annihilation_at_rest(c, mat, o, u);
     } else {
       mat = volume(c, in.vol).material;
       vacuum = mat_scalar(c, mat, S_VACUUM) != 0.0;
@@ -88,83 +103,87 @@ __device__ void step_track(const DevCtx& c, int nav, bool active, const Track& i
   int chords = 0;
   const int charge = is_gamma ? 0 : (positron ? +1 : -1);
   const int flag = propagate(c, nav, go, charge, T0, pos, dir, in.vol, s_phys, s, chords, pushdir);
+  if (!go) return NEXT_NONE;
 
   // ---- along-step actions (A7)
-  bool cross = false;
-  if (go) {
-    o.s = s; o.chords = chords;
-    if (is_gamma) {
-      cross = flag == 1;
-    } else {
-      double dE = 0.0;
-      if (!vacuum) {
-        if (flag == 0 && !lim_disc && range_out) dE = T0;
-        else if (s <= 0.01 * R) dE = S * s;
-        else dE = T0 - inverse_range(c, tab, row, positron ? 4 : 3, gp.i, R - s);
-        dE = fmin(fmax(dE, 0.0), T0);
-      }
-      o.edep_dep += dE;
-      o.post.ekin = T0 - dE;
-      if (o.post.ekin < kTmin) {
-        o.edep_cut += o.post.ekin; o.post.ekin = 0.0;
-        o.post.x = pos[0]; o.post.y = pos[1]; o.post.z = pos[2];
-        o.post.dx = dir[0]; o.post.dy = dir[1]; o.post.dz = dir[2];
-        if (positron) annihilation_at_rest(c, mat, o, u);
-        o.alive = 0; o.outcome = ADEPT_OUT_STOPPED; go = false;
-      } else {
-        if (!vacuum && s > 0.0) {  // P9 Highland MSC at the pre-step energy
-          const double X0 = mat_scalar(c, mat, S_X0);
-          const double pbeta = T0 * (T0 + 2.0 * kMe) / (T0 + kMe);
-          const double beta2 = T0 * (T0 + 2.0 * kMe) / ((T0 + kMe) * (T0 + kMe));
-          const double corr = fmax(0.0, 1.0 + 0.038 * log(s / (X0 * beta2)));
-          const double th0 = (13.6 / pbeta) * sqrt(s / X0) * corr;
-          const double u2 = u.uniform(2), u3 = u.uniform(3);
-          const double th = th0 * sqrt(-2.0 * log(u2));
-          double sn, cs, dn[3];
-          sincos(th, &sn, &cs);
-          rotate(dir, cs, sn, 2.0 * kPi * u3, dn);
-          dir[0] = dn[0]; dir[1] = dn[1]; dir[2] = dn[2];
-        }
-        cross = flag == 1;
-      }
+  o.s = s; o.chords = chords;
+  if (!is_gamma) {
+    double dE = 0.0;
+    if (!vacuum) {
+      if (flag == 0 && !lim_disc && range_out) dE = T0;
+      else if (s <= 0.01 * R) dE = S * s;
+      else dE = T0 - inverse_range(c, tab, row, positron ? 4 : 3, gp.i, R - s);
+      dE = fmin(fmax(dE, 0.0), T0);
+    }
+    o.edep_dep += dE;
+    o.post.ekin = T0 - dE;
+    if (o.post.ekin < kTmin) {
+      o.edep_cut += o.post.ekin; o.post.ekin = 0.0;
+      o.post.x = pos[0]; o.post.y = pos[1]; o.post.z = pos[2];
+      o.post.dx = dir[0]; o.post.dy = dir[1]; o.post.dz = dir[2];
+      if (positron) annihilation_at_rest(c, mat, o, u);
+      o.alive = 0; o.outcome = ADEPT_OUT_STOPPED;
+      return NEXT_NONE;
+    }
+    if (!vacuum && s > 0.0) {  // P9 Highland MSC at the pre-step energy
+      const double X0 = mat_scalar(c, mat, S_X0);
+      const double pbeta = T0 * (T0 + 2.0 * kMe) / (T0 + kMe);
+      const double beta2 = T0 * (T0 + 2.0 * kMe) / ((T0 + kMe) * (T0 + kMe));
+      const double corr = fmax(0.0, 1.0 + 0.038 * log(s / (X0 * beta2)));
+      const double th0 = (13.6 / pbeta) * sqrt(s / X0) * corr;
+      const double u2 = u.uniform(2), u3 = u.uniform(3);
+      const double th = th0 * sqrt(-2.0 * log(u2));
+      double sn, cs, dn[3];
+      sincos(th, &sn, &cs);
+      rotate(dir, cs, sn, 2.0 * kPi * u3, dn);
+      dir[0] = dn[0]; dir[1] = dn[1]; dir[2] = dn[2];
     }
   }
+  o.post.dx = dir[0]; o.post.dy = dir[1]; o.post.dz = dir[2];
+  if (flag == 1) {  // G5: push past the boundary; the new volume is found by the relocate phase
+    o.post.x = pos[0] + c.eps_push * pushdir[0];
+    o.post.y = pos[1] + c.eps_push * pushdir[1];
+    o.post.z = pos[2] + c.eps_push * pushdir[2];
+    return NEXT_RELOCATE;
+  }
+  o.post.x = pos[0]; o.post.y = pos[1]; o.post.z = pos[2];
+  if (flag == 2) { o.outcome = ADEPT_OUT_TRUNCATED; return NEXT_NONE; }
+  if (!is_gamma && !lim_disc) { o.outcome = ADEPT_OUT_LOSS; return NEXT_NONE; }
+  // ---- choice of the discrete process (U1)
+  const double u1 = u.uniform(1);
+  if (is_gamma) {
+    process = ADEPT_OUT_PHOTO;
+    if (u1 * stot < x0) process = ADEPT_OUT_COMPTON;
+    else if (u1 * stot < x0 + x1) process = ADEPT_OUT_PAIR;
+  } else {
+    process = ADEPT_OUT_BREM;
+    if (u1 * stot < x0) process = ADEPT_OUT_BREM;
+    else if (!positron || u1 * stot < x0 + x1) process = ADEPT_OUT_IONI;
+    else process = ADEPT_OUT_ANNI;
+  }
+  return NEXT_INTERACT;
+}
 
-  // ---- relocation (A5, G5): push past the boundary and Locate
+// Phase 2 (A5).  `cross` lanes hold the pushed position in o.post; the others idle.  Warp-convergent.
+__device__ __forceinline__ void step_relocate(const DevCtx& c, int nav, bool cross, int species, StepOut& o) {
+  const int nv = nav_locate(c, nav, cross, o.post.x, o.post.y, o.post.z);
   if (cross) {
-    pos[0] += c.eps_push * pushdir[0]; pos[1] += c.eps_push * pushdir[1]; pos[2] += c.eps_push * pushdir[2];
-  }
-  const int nv = nav_locate(c, nav, cross, pos[0], pos[1], pos[2]);
-  if (go) {
-    o.post.x = pos[0]; o.post.y = pos[1]; o.post.z = pos[2];
-    o.post.dx = dir[0]; o.post.dy = dir[1]; o.post.dz = dir[2];
-    if (cross) {
-      if (nv < 0) {
-        o.escaped += carried_energy(in.species, o.post.ekin); o.alive = 0; o.outcome = ADEPT_OUT_ESCAPED;
-      } else {
-        o.post.vol = static_cast<uint32_t>(nv); o.outcome = ADEPT_OUT_BOUNDARY;
-      }
-    } else if (flag == 2) {
-      o.outcome = ADEPT_OUT_TRUNCATED;
-    } else if (!is_gamma && !lim_disc) {
-      o.outcome = ADEPT_OUT_LOSS;
+    if (nv < 0) {
+      o.escaped += carried_energy(species, o.post.ekin); o.alive = 0; o.outcome = ADEPT_OUT_ESCAPED;
     } else {
-      // ---- discrete interaction (A8)
-      const double u1 = u.uniform(1);
-      int process;
-      if (is_gamma) {
-        process = ADEPT_OUT_PHOTO;
-        if (u1 * stot < x0) process = ADEPT_OUT_COMPTON;
-        else if (u1 * stot < x0 + x1) process = ADEPT_OUT_PAIR;
-      } else {
-        process = ADEPT_OUT_BREM;
-        if (u1 * stot < x0) process = ADEPT_OUT_BREM;
-        else if (!positron || u1 * stot < x0 + x1) process = ADEPT_OUT_IONI;
-        else process = ADEPT_OUT_ANNI;
-      }
-      run_process(c, process, in.species, mat, o, u);
+      o.post.vol = static_cast<uint32_t>(nv); o.outcome = ADEPT_OUT_BOUNDARY;
     }
   }
+}
+
+// The whole step in one call (frozen-step hook and fused kernels).
+template <int MODE>
+__device__ void step_track(const DevCtx& c, int nav, bool active, const Track& in, StepOut& o) {
+  Stream u;
+  int process, mat;
+  const int next = step_move<MODE>(c, nav, active, in, o, u, process, mat);
+  step_relocate(c, nav, next == NEXT_RELOCATE, in.species, o);
+  if (next == NEXT_INTERACT) run_process(c, process, in.species, mat, o, u);
   if (o.alive) o.post.step = in.step + 1;
 }
 

@@ -61,11 +61,11 @@ struct TrackSoA {
 struct SlotCounters {
   uint32_t count[2][3];     // [buffer parity][species] live entries
   uint32_t n_reloc;         // relocation work queue (split mode)
-  uint32_t n_inter;         // interaction work queue (split mode)
+  uint32_t n_inter[8];      // interaction work queues, one per process (split mode)
   uint32_t overflow;        // set when any queue overflowed
   uint32_t n_leaked;
   uint32_t live;            // population after the last finished iteration
-  uint32_t pad[3];
+  uint32_t pad[2];
 };
 
 struct DevStats {
