@@ -107,12 +107,15 @@ __device__ int propagate(const DevCtx& c, int nav, bool active, int charge, doub
       if (s_done >= s_phys) {
         flag = 0; running = false;
       } else {
-        if (charge != 0 && c.field_kind != ADEPT_FIELD_NONE) field_at(c, pos, B);  // gammas go straight
-        double dxB[3];
-        cross3(dir, B, dxB);
-        const double bperp = sqrt(dxB[0] * dxB[0] + dxB[1] * dxB[1] + dxB[2] * dxB[2]);
+        double bperp = 0.0;
+        if (charge != 0 && c.field_kind != ADEPT_FIELD_NONE) {  // gammas go straight
+          field_at(c, pos, B);
+          double dxB[3];
+          cross3(dir, B, dxB);
+          bperp = sqrt(dxB[0] * dxB[0] + dxB[1] * dxB[1] + dxB[2] * dxB[2]);
+        }
         rest = s_phys - s_done;
-        if (bperp == 0.0) {
+        if (charge == 0 || bperp == 0.0) {
           straight = true; query = true; L = rest;
           u[0] = dir[0]; u[1] = dir[1]; u[2] = dir[2];
         } else if (chords >= c.chord_budget) {

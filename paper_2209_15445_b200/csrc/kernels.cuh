@@ -49,7 +49,9 @@ __device__ __forceinline__ double warp_sum(double v) {
 // group leader issues one fp64 atomic; with 100 scoring slabs most warps issue 1-3 atomics.
 __device__ __forceinline__ void score(double* edep, uint32_t vol, double e, bool active) {
   const bool has = active && e != 0.0;
-  const unsigned peers = __match_any_sync(kFull, has ? vol : kDeadVolume);
+  const unsigned hm = __ballot_sync(kFull, has);
+  if (hm == 0 || !has) return;                      // lanes without a deposit take no part
+  const unsigned peers = __match_any_sync(hm, vol);
   const int lane = threadIdx.x & 31;
   double sum = 0.0;
   unsigned m = peers;
@@ -58,7 +60,7 @@ __device__ __forceinline__ void score(double* edep, uint32_t vol, double e, bool
     m &= m - 1;
     sum += __shfl_sync(peers, e, src);
   }
-  if (has && lane == __ffs(peers) - 1) atomicAdd(edep + vol, sum);
+  if (lane == __ffs(peers) - 1) atomicAdd(edep + vol, sum);
 }
 
 struct BlockTally {
@@ -197,7 +199,7 @@ __device__ __forceinline__ int inter_queue_index(int process, int species) {
 __device__ __forceinline__ int inter_queue_process(int q) { return q == 6 ? ADEPT_OUT_IONI : q + 1; }
 
 template <int MODE>
-__global__ void __launch_bounds__(kBlock) move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot,
+__global__ void __launch_bounds__(kBlock, MODE == MODE_GAMMA ? 4 : 3) move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot,
                                                       int parity) {
   const int species = MODE == MODE_GAMMA ? ADEPT_GAMMA : static_cast<int>(blockIdx.y);
   const TrackSoA& cur = slot.buf[parity][species];
