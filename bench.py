@@ -48,6 +48,24 @@ def parse():
     return ap.parse_args()
 
 
+def shard_first_event(rank, events_per_rank):
+    """Events shard over ranks with no data-path collective: rank r owns the event ids
+    [r * E, (r + 1) * E).  Event ids key the Philox streams, so shards never share random numbers."""
+    return rank * events_per_rank
+
+
+def reduce_over_ranks(dist, dev, t_max, c_sum):
+    """max over ranks of the timings, sum over ranks of the counters (the only collectives of the run)."""
+    import torch
+    if dist is None:
+        return list(t_max), list(c_sum)
+    t = torch.tensor(list(t_max), dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    c = torch.tensor(list(c_sum), dtype=torch.float64, device=dev)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return t.tolist(), c.tolist()
+
+
 def workload(args, first_event=0):
     from paper_2209_15445_b200.inputs import field, geometry, materials, primaries
     g = geometry.calorimeter()
@@ -166,7 +184,7 @@ def run_ours(args):
     dev = torch.device(f"cuda:{local}")
 
     # events shard over ranks with no data-path collective: weak scaling
-    g, tabs, scal, fld, prim = workload(args, first_event=rank * args.events)
+    g, tabs, scal, fld, prim = workload(args, first_event=shard_first_event(rank, args.events))
     cap = args.capacity or max(1 << 20, 1024 * args.events)
     a = adept.Adept(g, tabs, scal, fld, device=str(dev), track_capacity=cap, sync_interval=args.sync_interval,
                     time_kernels=1, split_kernels=args.split)
@@ -226,15 +244,8 @@ def run_ours(args):
     launches = st.launches - launches0 + args.steps        # + one enqueue kernel per pass
     t_dev = sum(dev_ms) * 1e-3
     t_e2e = sum(wall_s)
-    if dist is not None:
-        t = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        t_dev, t_e2e = float(t[0]), float(t[1])
-        c = torch.tensor([steps, launches], dtype=torch.float64, device=dev)
-        dist.all_reduce(c, op=dist.ReduceOp.SUM)
-        steps_all, launches_all = float(c[0]), int(c[1])
-    else:
-        steps_all, launches_all = float(steps), int(launches)
+    (t_dev, t_e2e), (steps_all, launches_all) = reduce_over_ranks(dist, dev, [t_dev, t_e2e], [steps, launches])
+    launches_all = int(launches_all)
 
     if rank == 0:
         peaks = {}

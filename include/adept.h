@@ -153,7 +153,7 @@ typedef struct adept_ctx adept_ctx;
 
 const char* adept_last_error(void);
 
-/* Fills *cfg with the defaults listed above (n_event_slots 1, BVH navigator, capacity 1<<20). */
+/* Fills *cfg with the defaults listed above (n_event_slots 1, BVH navigator, capacity 1<<20, split kernels). */
 void adept_default_config(adept_config* cfg);
 
 /* Bytes of device workspace adept_init needs for this configuration (0 on invalid input). */

@@ -27,7 +27,8 @@ def _check_layers(gpu_mean, o_mean, o_err):
     assert not bad.any(), (np.where(bad)[0], gpu_mean[bad], o_mean[bad], tol[bad])
 
 
-def test_config1_calorimeter_256_electrons(ob, calo):
+@pytest.mark.parametrize("split", [1, 0])
+def test_config1_calorimeter_256_electrons(ob, calo, split):
     """BASELINE.json:configs[0]: 256 e- at 1 GeV, seed 1, edep per layer; one slot per group of events so the
     per-event ledgers are checked too."""
     import torch
@@ -39,7 +40,7 @@ def test_config1_calorimeter_256_electrons(ob, calo):
     tr = o.make_tracks(prim)
     o_ev, o_led = _oracle_events(o, tr, g.n_volumes)
     o_mean, o_err = layer_stats(o_ev)
-    a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=1 << 18, n_event_slots=2)
+    a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=1 << 18, n_event_slots=2, split_kernels=split)
     # slot 0: all 256 events in one population; slot 1: single events, ledger per event
     a.enqueue(prim, slot=0)
     a.transport(0, torch.cuda.current_stream())
@@ -90,7 +91,8 @@ def test_config3_uniform_field(ob, calo, species):
     assert st.chords > 0
 
 
-def test_config5_concurrent_events_on_streams(ob, barrel_patch):
+@pytest.mark.parametrize("split", [1, 0])
+def test_config5_concurrent_events_on_streams(ob, barrel_patch, split):
     """BASELINE.json:configs[4] on the crystal patch: 16 events on 16 CUDA streams, per-event per-volume hits
     copied back to the host and checked against the oracle event by event."""
     import torch
@@ -107,7 +109,7 @@ def test_config5_concurrent_events_on_streams(ob, barrel_patch):
     o = ob.Oracle(g, tabs, scal, fld)
     tr = o.make_tracks(prim)
     o_ev, o_led = _oracle_events(o, tr, g.n_volumes)
-    a = adept.Adept(g, tabs, scal, fld, track_capacity=1 << 16, n_event_slots=n_ev, sync_interval=4)
+    a = adept.Adept(g, tabs, scal, fld, track_capacity=1 << 16, n_event_slots=n_ev, sync_interval=4, split_kernels=split)
     streams = [torch.cuda.Stream() for _ in range(n_ev)]
     for e in range(n_ev):
         sel = prim["event"] == e
