@@ -10,7 +10,7 @@ import os
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libadept_b200.so")
+LIB_PATH = os.environ.get("ADEPT_B200_LIB", os.path.join(HERE, "libadept_b200.so"))
 
 OK, EINVAL, ENOMEM, EOVERFLOW, ECUDA, ESTATE = 0, -1, -2, -3, -4, -5
 NAV_LOOP, NAV_BVH = 0, 1

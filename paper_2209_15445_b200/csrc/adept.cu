@@ -165,6 +165,9 @@ struct adept_ctx {
   uint32_t* d_bad = nullptr;
   size_t stage_cap = 0;
   int grid_gamma = 0, grid_charged = 0, grid_reloc = 0, grid_inter = 0;
+  // split-mode kernels specialised for this context's field kind and for geometries without BVH volumes
+  using Kernel = void (*)(DevCtx, DevSlot, int);
+  Kernel k_move_gamma = nullptr, k_move_charged = nullptr, k_relocate = nullptr;
 };
 
 extern "C" const char* adept_last_error(void) { return g_err; }
@@ -363,9 +366,20 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_c, step_kernel<MODE_CHARGED>, kBlock, 0));
   if (cfg->split_kernels) {
     int occ_r = 1, occ_i = 1;
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_g, move_kernel<MODE_GAMMA>, kBlock, 0));
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_c, move_kernel<MODE_CHARGED>, kBlock, 0));
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_r, relocate_kernel, kBlock, 0));
+    const bool bvh = cfg->navigator == ADEPT_NAV_BVH && !hb.empty();
+    ctx->k_move_gamma = bvh ? move_kernel<MODE_GAMMA, ADEPT_FIELD_NONE, true> : move_kernel<MODE_GAMMA, ADEPT_FIELD_NONE, false>;
+    ctx->k_relocate = bvh ? relocate_kernel<true> : relocate_kernel<false>;
+    switch (f->kind) {
+      case ADEPT_FIELD_NONE:
+        ctx->k_move_charged = bvh ? move_kernel<MODE_CHARGED, ADEPT_FIELD_NONE, true> : move_kernel<MODE_CHARGED, ADEPT_FIELD_NONE, false>; break;
+      case ADEPT_FIELD_UNIFORM:
+        ctx->k_move_charged = bvh ? move_kernel<MODE_CHARGED, ADEPT_FIELD_UNIFORM, true> : move_kernel<MODE_CHARGED, ADEPT_FIELD_UNIFORM, false>; break;
+      default:
+        ctx->k_move_charged = bvh ? move_kernel<MODE_CHARGED, ADEPT_FIELD_MAP_RZ, true> : move_kernel<MODE_CHARGED, ADEPT_FIELD_MAP_RZ, false>; break;
+    }
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_g, ctx->k_move_gamma, kBlock, 0));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_c, ctx->k_move_charged, kBlock, 0));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_r, ctx->k_relocate, kBlock, 0));
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_i, interact_kernel, kBlock, 0));
     ctx->grid_reloc = sms * std::max(occ_r, 1);
     ctx->grid_inter = sms * std::max(occ_i, 1);
@@ -463,11 +477,11 @@ int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity) 
   cudaEvent_t* ev = timed ? &sh.tev[sh.tev_used] : nullptr;
   const bool split = ctx->cfg.split_kernels != 0;
   if (timed) CUDA_TRY(cudaEventRecord(ev[0], st));
-  if (split) move_kernel<MODE_GAMMA><<<dim3(ctx->grid_gamma, 1), kBlock, 0, st>>>(ctx->dev, sh.dev, parity);
+  if (split) ctx->k_move_gamma<<<dim3(ctx->grid_gamma, 1), kBlock, 0, st>>>(ctx->dev, sh.dev, parity);
   else step_kernel<MODE_GAMMA><<<dim3(ctx->grid_gamma, 1), kBlock, 0, st>>>(ctx->dev, sh.dev, parity);
   if (timed) CUDA_TRY(cudaEventRecord(ev[1], st));
   if (timed) CUDA_TRY(cudaEventRecord(ev[2], sh.helper));
-  if (split) move_kernel<MODE_CHARGED><<<dim3(ctx->grid_charged, 2), kBlock, 0, sh.helper>>>(ctx->dev, sh.dev, parity);
+  if (split) ctx->k_move_charged<<<dim3(ctx->grid_charged, 2), kBlock, 0, sh.helper>>>(ctx->dev, sh.dev, parity);
   else step_kernel<MODE_CHARGED><<<dim3(ctx->grid_charged, 2), kBlock, 0, sh.helper>>>(ctx->dev, sh.dev, parity);
   if (timed) { CUDA_TRY(cudaEventRecord(ev[3], sh.helper)); sh.tev_used += 4; }
   if (split) {
@@ -476,7 +490,7 @@ int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity) 
     CUDA_TRY(cudaStreamWaitEvent(st, sh.join, 0));
     CUDA_TRY(cudaEventRecord(sh.fork, st));
     CUDA_TRY(cudaStreamWaitEvent(sh.helper, sh.fork, 0));
-    relocate_kernel<<<ctx->grid_reloc, kBlock, 0, st>>>(ctx->dev, sh.dev, parity);
+    ctx->k_relocate<<<ctx->grid_reloc, kBlock, 0, st>>>(ctx->dev, sh.dev, parity);
     interact_kernel<<<ctx->grid_inter, kBlock, 0, sh.helper>>>(ctx->dev, sh.dev, parity);
     sh.launches += 2;
   }

@@ -90,8 +90,11 @@ __device__ __noinline__ void rk4(const DevCtx& c, int charge, double pmom, doubl
 
 // F2-F4 chord loop.  flag: 0 physics limit reached, 1 boundary (pos = hit point without the push,
 // pushdir = chord direction), 2 truncated (chord budget).  Warp-convergent.
+// FIELD >= 0 fixes the field kind at compile time (no helix / RK4 code where it cannot run); -1 = runtime.
+template <int FIELD = -1, bool BVH = true>
 __device__ int propagate(const DevCtx& c, int nav, bool active, int charge, double ekin, double pos[3], double dir[3],
                          uint32_t vol, double s_phys, double& s_out, int& chords_out, double pushdir[3]) {
+  const int field_kind = FIELD >= 0 ? FIELD : c.field_kind;
   const double pmom = sqrt(ekin * (ekin + 2.0 * kMe));
   double s_done = 0.0;
   int chords = 0, flag = 0;
@@ -108,7 +111,7 @@ __device__ int propagate(const DevCtx& c, int nav, bool active, int charge, doub
         flag = 0; running = false;
       } else {
         double bperp = 0.0;
-        if (charge != 0 && c.field_kind != ADEPT_FIELD_NONE) {  // gammas go straight
+        if (charge != 0 && field_kind != ADEPT_FIELD_NONE) {  // gammas go straight
           field_at(c, pos, B);
           double dxB[3];
           cross3(dir, B, dxB);
@@ -123,13 +126,13 @@ __device__ int propagate(const DevCtx& c, int nav, bool active, int charge, doub
         } else {
           const double Rcurv = pmom / (kCB * bperp);
           double h_max = sqrt(8.0 * c.delta_chord * Rcurv);
-          if (c.field_kind == ADEPT_FIELD_MAP_RZ) {  // F2': at most 0.5 rad of turn per RK4 chord
+          if (field_kind == ADEPT_FIELD_MAP_RZ) {  // F2': at most 0.5 rad of turn per RK4 chord
             const double Bn = sqrt(B[0] * B[0] + B[1] * B[1] + B[2] * B[2]);
             h_max = fmin(h_max, 0.5 * pmom / (kCB * Bn));
           }
           last = h_max >= rest;
           h = last ? rest : h_max;
-          if (c.field_kind == ADEPT_FIELD_UNIFORM) helix(B, charge, pmom, h, pos, dir, p1, d1);
+          if (field_kind == ADEPT_FIELD_UNIFORM) helix(B, charge, pmom, h, pos, dir, p1, d1);
           else rk4(c, charge, pmom, h, pos, dir, p1, d1);
           const double ch[3] = {p1[0] - pos[0], p1[1] - pos[1], p1[2] - pos[2]};
           L = sqrt(ch[0] * ch[0] + ch[1] * ch[1] + ch[2] * ch[2]);
@@ -139,7 +142,7 @@ __device__ int propagate(const DevCtx& c, int nav, bool active, int charge, doub
       }
     }
     // --- warp-cooperative geometry query of this segment
-    const double s_geo = nav_distance(c, nav, query, pos[0], pos[1], pos[2], u[0], u[1], u[2], vol, L);
+    const double s_geo = nav_distance<BVH>(c, nav, query, pos[0], pos[1], pos[2], u[0], u[1], u[2], vol, L);
     if (query) {
       if (straight) {
         pushdir[0] = u[0]; pushdir[1] = u[1]; pushdir[2] = u[2];
@@ -158,7 +161,7 @@ __device__ int propagate(const DevCtx& c, int nav, bool active, int charge, doub
         if (s_geo < L) {
           const double frac = s_geo / L;
           double dh[3];
-          if (c.field_kind == ADEPT_FIELD_UNIFORM) {
+          if (field_kind == ADEPT_FIELD_UNIFORM) {
             double ph[3];
             helix(B, charge, pmom, h * frac, pos, dir, ph, dh);
           } else {

@@ -249,6 +249,8 @@ __device__ __noinline__ int bvh_point(const DevCtx& c, const DevBvh& b, double p
 // ---------------------------------------------------------------- G3 distance to boundary
 // min(exit distance of the own solid, entry distance of every daughter), capped at s_max.
 // Warp-convergent call; lanes with active == false return s_max.
+// BVH = false instantiates the pure loop navigator (geometries without a BVH volume): no cooperative code.
+template <bool BVH = true>
 __device__ __noinline__ double nav_distance(const DevCtx& c, int nav, bool active, double px, double py, double pz, double dx,
                                double dy, double dz, uint32_t vol, double s_max) {
   const int lane = threadIdx.x & 31;
@@ -262,7 +264,7 @@ __device__ __noinline__ double nav_distance(const DevCtx& c, int nav, bool activ
     dir_to_local(v, dx, dy, dz, ld);
     s = fmin(s_max, solid_exit(v, lp, ld));
     if (v.dcount > 0) {
-      if (nav == ADEPT_NAV_BVH && v.bvh >= 0) {
+      if (BVH && nav == ADEPT_NAV_BVH && v.bvh >= 0) {
         need = true;
         bvh = v.bvh;
       } else {
@@ -270,6 +272,7 @@ __device__ __noinline__ double nav_distance(const DevCtx& c, int nav, bool activ
       }
     }
   }
+  if (!BVH) return s;
   unsigned m = __ballot_sync(kFull, need);
   while (m) {
     const int src = __ffs(m) - 1;
@@ -285,6 +288,7 @@ __device__ __noinline__ double nav_distance(const DevCtx& c, int nav, bool activ
 // ---------------------------------------------------------------- G4 Locate
 // From the world down, descend into the first daughter (index order) containing the point.
 // Warp-convergent call; returns -1 outside the world or for inactive lanes.
+template <bool BVH = true>
 __device__ __noinline__ int nav_locate(const DevCtx& c, int nav, bool active, double qx, double qy, double qz) {
   const int lane = threadIdx.x & 31;
   int cur = -1;
@@ -292,6 +296,17 @@ __device__ __noinline__ int nav_locate(const DevCtx& c, int nav, bool active, do
   if (active && inside_volume(c, 0, qx, qy, qz)) {
     cur = 0;
     desc = true;
+  }
+  if (!BVH) {  // lane-local descent, no warp cooperation needed
+    while (desc) {
+      const DevVolume& v = volume(c, cur);
+      int next = -1;
+      for (int k = 0; k < v.dcount; ++k) {
+        if (inside_volume(c, v.dbegin + k, qx, qy, qz)) { next = v.dbegin + k; break; }
+      }
+      if (next < 0) desc = false; else cur = next;
+    }
+    return cur;
   }
   while (__any_sync(kFull, desc)) {
     bool need = false;

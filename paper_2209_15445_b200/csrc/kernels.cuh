@@ -9,6 +9,16 @@
 namespace adept {
 
 constexpr int kBlock = 128;
+// minimum resident blocks per SM asked of the compiler (register caps chosen from measurement)
+#ifndef ADEPT_MINB_G
+#define ADEPT_MINB_G 4
+#endif
+#ifndef ADEPT_MINB_C
+#define ADEPT_MINB_C 3
+#endif
+#ifndef ADEPT_MINB_I
+#define ADEPT_MINB_I 6
+#endif
 
 __device__ __forceinline__ Track load_track(const TrackSoA& b, uint32_t i, int species) {
   Track t;
@@ -100,32 +110,41 @@ __device__ __forceinline__ void flush_tally(BlockTally& tally, const LaneTally& 
   }
 }
 
-// Appends the secondaries of a step to the next buffers: one warp-aggregated atomic per (k, species).
-// Warp-convergent.  `u` is the parent's stream (child ids, R3).
+// Appends the secondaries of a step to the next buffers.  All six (k, species) groups of the warp are
+// reserved in ONE round of atomics (lane sp adds the warp's total for species sp), so a warp waits for
+// a single atomic latency.  Warp-convergent.  `u` is the parent's stream (child ids, R3).
 __device__ __forceinline__ void append_secondaries(const DevCtx& c, const DevSlot& slot, int parity, bool active,
                                                    uint32_t event, const Stream& u, const StepOut& o, BlockTally& tally) {
   SlotCounters* cnt = slot.counters;
+  const int s0 = (active && o.n_sec > 0) ? o.sec[0].species : -1;
+  const int s1 = (active && o.n_sec > 1) ? o.sec[1].species : -1;
+  if (__ballot_sync(kFull, s0 >= 0) == 0) return;        // sec[1] exists only with sec[0]
+  const int lane = threadIdx.x & 31;
+  const unsigned lt = (1u << lane) - 1u;
+  unsigned m0[3], m1[3];
+#pragma unroll
+  for (int sp = 0; sp < 3; ++sp) { m0[sp] = __ballot_sync(kFull, s0 == sp); m1[sp] = __ballot_sync(kFull, s1 == sp); }
+  uint32_t mine = 0;
+  if (lane < 3) {
+    const unsigned n = __popc(lane == 0 ? m0[0] : lane == 1 ? m0[1] : m0[2]) + __popc(lane == 0 ? m1[0] : lane == 1 ? m1[1] : m1[2]);
+    if (n) { mine = atomicAdd(&cnt->count[parity ^ 1][lane], n); atomicAdd(&tally.secondaries[lane], static_cast<unsigned long long>(n)); }
+  }
+  uint32_t base[3];
+#pragma unroll
+  for (int sp = 0; sp < 3; ++sp) base[sp] = __shfl_sync(kFull, mine, sp);
 #pragma unroll
   for (int k = 0; k < 2; ++k) {
-    const int ss = (active && k < o.n_sec) ? o.sec[k].species : -1;
-    if (__ballot_sync(kFull, ss >= 0) == 0) continue;
-    const uint64_t cid = ss >= 0 ? u.child_id(o.sec[k].child) : 0;
-#pragma unroll
-    for (int sp = 0; sp < 3; ++sp) {
-      const bool want = ss == sp;
-      const uint32_t j = warp_append(&cnt->count[parity ^ 1][sp], want);
-      if (want) {
-        if (j < c.capacity) {
-          Track s;
-          s.x = o.post.x; s.y = o.post.y; s.z = o.post.z;
-          s.dx = o.sec[k].dx; s.dy = o.sec[k].dy; s.dz = o.sec[k].dz;
-          s.ekin = o.sec[k].ekin; s.id = cid; s.event = event; s.step = 0; s.vol = o.post.vol; s.species = sp;
-          store_track(slot.buf[parity ^ 1][sp], j, s);
-          atomicAdd(&tally.secondaries[sp], 1ull);
-        } else {
-          cnt->overflow = 1;
-        }
-      }
+    const int ss = k == 0 ? s0 : s1;
+    if (ss < 0) continue;
+    const uint32_t j = k == 0 ? base[ss] + __popc(m0[ss] & lt) : base[ss] + __popc(m0[ss]) + __popc(m1[ss] & lt);
+    if (j < c.capacity) {
+      Track s;
+      s.x = o.post.x; s.y = o.post.y; s.z = o.post.z;
+      s.dx = o.sec[k].dx; s.dy = o.sec[k].dy; s.dz = o.sec[k].dz;
+      s.ekin = o.sec[k].ekin; s.id = u.child_id(o.sec[k].child); s.event = event; s.step = 0; s.vol = o.post.vol; s.species = ss;
+      store_track(slot.buf[parity ^ 1][ss], j, s);
+    } else {
+      cnt->overflow = 1;
     }
   }
 }
@@ -198,8 +217,8 @@ __device__ __forceinline__ int inter_queue_index(int process, int species) {
 }
 __device__ __forceinline__ int inter_queue_process(int q) { return q == 6 ? ADEPT_OUT_IONI : q + 1; }
 
-template <int MODE>
-__global__ void __launch_bounds__(kBlock, MODE == MODE_GAMMA ? 4 : 3) move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot,
+template <int MODE, int FIELD, bool BVH>
+__global__ void __launch_bounds__(kBlock, MODE == MODE_GAMMA ? ADEPT_MINB_G : ADEPT_MINB_C) move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot,
                                                       int parity) {
   const int species = MODE == MODE_GAMMA ? ADEPT_GAMMA : static_cast<int>(blockIdx.y);
   const TrackSoA& cur = slot.buf[parity][species];
@@ -221,7 +240,7 @@ __global__ void __launch_bounds__(kBlock, MODE == MODE_GAMMA ? 4 : 3) move_kerne
     StepOut o;
     Stream u;
     int process, mat;
-    const int next = step_move<MODE>(c, c.navigator, active, in, o, u, process, mat);
+    const int next = step_move<MODE, FIELD, BVH>(c, c.navigator, active, in, o, u, process, mat);
 
     score(slot.edep, in.vol, o.edep_dep + o.edep_cut, active);
     if (active) {
@@ -230,34 +249,52 @@ __global__ void __launch_bounds__(kBlock, MODE == MODE_GAMMA ? 4 : 3) move_kerne
       if (next == NEXT_NONE) atomicAdd(&tally.outcomes[o.outcome], 1ull);
       tally.touched = 1;
     }
+    // One round of atomics reserves everything this warp appends: lane 0 the survivor slots, lane 1 the
+    // relocation-queue entries, lanes 2.. the entries of the process queues this kernel feeds.
     const bool live = active && o.alive;
-    const uint32_t j = warp_append(&cnt->count[parity ^ 1][species], live);
-    const bool stored = live && j < c.capacity;
+    constexpr int kQ0 = MODE == MODE_GAMMA ? 0 : 3, kNQ = MODE == MODE_GAMMA ? 3 : 4;
+    const int q = (live && next == NEXT_INTERACT) ? inter_queue_index(process, species) - kQ0 : -1;
+    const int lane = threadIdx.x & 31;
+    const unsigned lt = (1u << lane) - 1u;
+    const unsigned m_live = __ballot_sync(kFull, live);
+    const unsigned m_rel = __ballot_sync(kFull, live && next == NEXT_RELOCATE);
+    unsigned m_q[kNQ];
+#pragma unroll
+    for (int qq = 0; qq < kNQ; ++qq) m_q[qq] = __ballot_sync(kFull, q == qq);
+    uint32_t mine = 0;
+    if (lane == 0) { if (m_live) mine = atomicAdd(&cnt->count[parity ^ 1][species], __popc(m_live)); }
+    else if (lane == 1) { if (m_rel) mine = atomicAdd(&cnt->n_reloc, __popc(m_rel)); }
+    else if (lane < 2 + kNQ) {
+      unsigned mq = 0;
+#pragma unroll
+      for (int qq = 0; qq < kNQ; ++qq) if (lane == 2 + qq) mq = m_q[qq];
+      if (mq) mine = atomicAdd(&cnt->n_inter[kQ0 + lane - 2], __popc(mq));
+    }
+    const uint32_t j = __shfl_sync(kFull, mine, 0) + __popc(m_live & lt);
+    const uint32_t k_rel = __shfl_sync(kFull, mine, 1) + __popc(m_rel & lt);
+    uint32_t k_q = 0;
+#pragma unroll
+    for (int qq = 0; qq < kNQ; ++qq) {
+      const uint32_t bq = __shfl_sync(kFull, mine, 2 + qq);
+      if (q == qq) k_q = bq + __popc(m_q[qq] & lt);
+    }
     if (live) {
       o.post.step = in.step + 1;
-      if (stored) store_track(slot.buf[parity ^ 1][species], j, o.post);
-      else cnt->overflow = 1;
-    }
-    const uint32_t entry = (static_cast<uint32_t>(species) << 30) | j;
-    {
-      const bool want = stored && next == NEXT_RELOCATE;
-      const uint32_t k = warp_append(&cnt->n_reloc, want);
-      if (want) slot.reloc_queue[k] = entry;
-    }
-    const int q = (stored && next == NEXT_INTERACT) ? inter_queue_index(process, species) : -1;
-#pragma unroll
-    for (int qq = 0; qq < kNumInterQueues; ++qq) {
-      const bool mine = MODE == MODE_GAMMA ? qq < 3 : qq >= 3;   // queues this kernel can feed
-      if (!mine) continue;
-      const bool want = q == qq;
-      const uint32_t k = warp_append(&cnt->n_inter[qq], want);
-      if (want) slot.inter_queue[static_cast<size_t>(qq) * c.capacity + k] = entry;
+      if (j < c.capacity) {
+        store_track(slot.buf[parity ^ 1][species], j, o.post);
+        const uint32_t entry = (static_cast<uint32_t>(species) << 30) | j;
+        if (next == NEXT_RELOCATE) slot.reloc_queue[k_rel] = entry;
+        else if (q >= 0) slot.inter_queue[static_cast<size_t>(kQ0 + q) * c.capacity + k_q] = entry;
+      } else {
+        cnt->overflow = 1;
+      }
     }
     append_secondaries(c, slot, parity, active, in.event, u, o, tally);   // at-rest annihilation photons
   }
   flush_tally(tally, lt, slot, species);
 }
 
+template <bool BVH>
 __global__ void __launch_bounds__(kBlock) relocate_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot,
                                                           int parity) {
   SlotCounters* cnt = slot.counters;
@@ -276,7 +313,7 @@ __global__ void __launch_bounds__(kBlock) relocate_kernel(const __grid_constant_
     const TrackSoA& b = slot.buf[parity ^ 1][species];
     double x = 0.0, y = 0.0, z = 0.0;
     if (active) { x = b.x[j]; y = b.y[j]; z = b.z[j]; }
-    const int nv = nav_locate(c, c.navigator, active, x, y, z);
+    const int nv = nav_locate<BVH>(c, c.navigator, active, x, y, z);
     if (!active) continue;
     tally.touched = 1;
     if (nv >= 0) {
@@ -305,7 +342,7 @@ __global__ void __launch_bounds__(kBlock) relocate_kernel(const __grid_constant_
 
 // Every warp works on one process queue at a time, so the rejection loops of different processes never
 // share a warp (PAPER.md:101 names divergence between processes as a main cost).
-__global__ void __launch_bounds__(kBlock) interact_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot,
+__global__ void __launch_bounds__(kBlock, ADEPT_MINB_I) interact_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot,
                                                           int parity) {
   SlotCounters* cnt = slot.counters;
   __shared__ BlockTally tally;

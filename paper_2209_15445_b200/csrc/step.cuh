@@ -33,7 +33,7 @@ __device__ __forceinline__ void init_out(StepOut& o, const Track& in, bool activ
 // Phase 1.  On return o.post holds the moved state (position already pushed past the boundary when
 // the result is NEXT_RELOCATE), `process` the chosen discrete process for NEXT_INTERACT, and `mat`
 // the material of the pre-step volume.  o.post.step is NOT yet incremented.
-template <int MODE>
+template <int MODE, int FIELD = -1, bool BVH = true>
 __device__ int step_move(const DevCtx& c, int nav, bool active, const Track& in, StepOut& o, Stream& u, int& process,
                          int& mat) {
   init_out(o, in, active);
@@ -102,7 +102,7 @@ __device__ int step_move(const DevCtx& c, int nav, bool active, const Track& in,
   double s = 0.0;
   int chords = 0;
   const int charge = is_gamma ? 0 : (positron ? +1 : -1);
-  const int flag = propagate(c, nav, go, charge, T0, pos, dir, in.vol, s_phys, s, chords, pushdir);
+  const int flag = propagate<FIELD, BVH>(c, nav, go, charge, T0, pos, dir, in.vol, s_phys, s, chords, pushdir);
   if (!go) return NEXT_NONE;
 
   // ---- along-step actions (A7)
@@ -165,8 +165,9 @@ __device__ int step_move(const DevCtx& c, int nav, bool active, const Track& in,
 }
 
 // Phase 2 (A5).  `cross` lanes hold the pushed position in o.post; the others idle.  Warp-convergent.
+template <bool BVH = true>
 __device__ __forceinline__ void step_relocate(const DevCtx& c, int nav, bool cross, int species, StepOut& o) {
-  const int nv = nav_locate(c, nav, cross, o.post.x, o.post.y, o.post.z);
+  const int nv = nav_locate<BVH>(c, nav, cross, o.post.x, o.post.y, o.post.z);
   if (cross) {
     if (nv < 0) {
       o.escaped += carried_energy(species, o.post.ekin); o.alive = 0; o.outcome = ADEPT_OUT_ESCAPED;
