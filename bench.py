@@ -40,7 +40,6 @@ def parse():
     ap.add_argument("--field", type=float, default=0.0, help="uniform Bz in tesla (config 3: 1.0)")
     ap.add_argument("--capacity", type=int, default=0, help="track capacity per species (0 = auto)")
     ap.add_argument("--sync-interval", type=int, default=8)
-    ap.add_argument("--split", type=int, default=1, help="1: move/relocate/interact kernels; 0: fused step kernels")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--profile", action="store_true",
                     help="for runs under ncu: take --warmup literally (the timed numbers of such a run are not bench values)")
@@ -187,7 +186,7 @@ def run_ours(args):
     g, tabs, scal, fld, prim = workload(args, first_event=shard_first_event(rank, args.events))
     cap = args.capacity or max(1 << 20, 1024 * args.events)
     a = adept.Adept(g, tabs, scal, fld, device=str(dev), track_capacity=cap, sync_interval=args.sync_interval,
-                    time_kernels=1, split_kernels=args.split)
+                    time_kernels=1)
     stream = torch.cuda.Stream(device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
     edep_host = np.zeros(g.n_volumes)
@@ -256,7 +255,7 @@ def run_ours(args):
         peak = float(peaks.get("hbm_gbs", 6650.0))
         peak_src = "MEASURED_PEAKS.json hbm_gbs (of measured)" if "hbm_gbs" in peaks else "6650 GB/s (of fallback)"
         # dominant kernel = the step kernel with the larger accumulated device time
-        dom = int(np.argmax(kms))
+        dom = int(np.argmax(kms[:2]))
         dom_steps = (st.steps[2] - gsteps0) if dom == 0 else (steps - (st.steps[2] - gsteps0))
         # secondaries are attributed to the kernel that creates them in proportion to its steps
         dom_bytes = dom_steps * BYTES_PER_STEP + n_sec * BYTES_PER_SECONDARY * (dom_steps / max(steps, 1))
@@ -276,11 +275,12 @@ def run_ours(args):
                     "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
             "gpu_launches": launches_all,
             "clocks": clk,
-            "roofline": {"bound": "hbm", "kernel": "step_kernel<gamma>" if dom == 0 else "step_kernel<charged>",
+            "roofline": {"bound": "hbm", "kernel": "move_kernel<gamma>" if dom == 0 else "move_kernel<charged>",
                          "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
                          "peak_source": peak_src, "launches": int(kn[dom]), "avg_launch_ms": float(kms[dom] / max(kn[dom], 1)),
                          "algorithmic_bytes_per_step": BYTES_PER_STEP,
-                         "other_kernel_ms": float(kms[1 - dom]), "dominant_kernel_ms": float(kms[dom]),
+                         "other_move_kernel_ms": float(kms[1 - dom]), "dominant_kernel_ms": float(kms[dom]),
+                         "interact_kernel_ms": float(kms[2]),
                          "note": "latency/divergence bound fp64 Monte Carlo: see DESIGN.md §5 and profiles/"},
             "iterations_per_step": (st.iterations - st0.iterations) / args.steps,
             "peak_population": int(st.peak_population),

@@ -107,7 +107,8 @@ typedef struct {
   int32_t sync_interval;   /* population-step iterations launched between host checks               */
   uint64_t track_capacity; /* per slot, per species: entries of each of the two track buffers       */
   uint64_t leak_capacity;  /* per slot: tracks that left the world kept for adept_read_leaked       */
-  int32_t split_kernels;   /* 0: one step kernel per species group; 1: + relocation/interaction kernels */
+  uint64_t stage_capacity; /* per slot, per interaction queue: tracks staged for their discrete
+                              interaction in one population step (0 = track_capacity)               */
   int32_t time_kernels;    /* 1: bracket every step-kernel launch with CUDA events (adept_get_kernel_times) */
 } adept_config;
 
@@ -153,7 +154,7 @@ typedef struct adept_ctx adept_ctx;
 
 const char* adept_last_error(void);
 
-/* Fills *cfg with the defaults listed above (n_event_slots 1, BVH navigator, capacity 1<<20, split kernels). */
+/* Fills *cfg with the defaults listed above (n_event_slots 1, BVH navigator, capacity 1<<20). */
 void adept_default_config(adept_config* cfg);
 
 /* Bytes of device workspace adept_init needs for this configuration (0 on invalid input). */
@@ -194,10 +195,12 @@ int adept_read_leaked(adept_ctx*, int event_slot, adept_track* out, size_t cap, 
 
 int adept_get_stats(adept_ctx*, int event_slot, adept_stats* out);
 
-/* With config.time_kernels: device time [ms] and launch count of the gamma step kernel [0] and the
- * charged step kernel [1] of this slot, accumulated since the last call (CUDA events recorded on the
- * stream each kernel is launched on). */
-int adept_get_kernel_times(adept_ctx*, int event_slot, double ms[2], uint64_t launches[2]);
+/* With config.time_kernels: device time [ms] and launch count of the gamma move kernel [0], the
+ * charged move kernel [1] and the interaction kernel [2] of this slot, accumulated since the last call
+ * (CUDA events recorded on the stream each kernel is launched on; [0] and [1] run concurrently). */
+#define ADEPT_N_TIMED_KERNELS 3
+int adept_get_kernel_times(adept_ctx*, int event_slot, double ms[ADEPT_N_TIMED_KERNELS],
+                           uint64_t launches[ADEPT_N_TIMED_KERNELS]);
 
 /* Test hook: exactly one step for each of n tracks, results in input order; secondaries[2*i + k]. */
 int adept_step_frozen(adept_ctx*, int n, const adept_track* in, adept_step_result* out,
@@ -208,6 +211,10 @@ int adept_step_frozen(adept_ctx*, int n, const adept_track* in, adept_step_resul
 int adept_distance_batch(adept_ctx*, int navigator, int n, const double* pos3, const double* dir3,
                          const uint32_t* volume, const double* s_max, double* out, void* cuda_stream);
 int adept_locate_batch(adept_ctx*, int navigator, int n, const double* pos3, int64_t* out, void* cuda_stream);
+/* Relocation as the move kernel does it after a boundary (climb from volume from[i] until the point is
+ * inside, then descend): must equal adept_locate_batch for every starting volume. */
+int adept_relocate_batch(adept_ctx*, int navigator, int n, const double* pos3, const uint32_t* from, int64_t* out,
+                         void* cuda_stream);
 
 int adept_shutdown(adept_ctx*);
 

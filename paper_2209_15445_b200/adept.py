@@ -44,7 +44,7 @@ class CConfig(C.Structure):
     _fields_ = [("delta_chord", C.c_double), ("eps_push", C.c_double), ("alpha_R", C.c_double), ("rho_R", C.c_double),
                 ("chord_budget", C.c_int32), ("seed", C.c_uint32), ("max_steps", C.c_uint32), ("navigator", C.c_int32),
                 ("n_event_slots", C.c_int32), ("sync_interval", C.c_int32), ("track_capacity", C.c_uint64),
-                ("leak_capacity", C.c_uint64), ("split_kernels", C.c_int32), ("time_kernels", C.c_int32)]
+                ("leak_capacity", C.c_uint64), ("stage_capacity", C.c_uint64), ("time_kernels", C.c_int32)]
 
 
 class CLedger(C.Structure):
@@ -63,7 +63,7 @@ class CStats(C.Structure):
 EXPORTS = ["adept_last_error", "adept_default_config", "adept_workspace_bytes", "adept_init",
            "adept_enqueue_primaries", "adept_enqueue_batch", "adept_transport", "adept_transport_many",
            "adept_read_scoring", "adept_read_leaked", "adept_get_stats", "adept_get_kernel_times", "adept_step_frozen",
-           "adept_distance_batch", "adept_locate_batch", "adept_shutdown"]
+           "adept_distance_batch", "adept_locate_batch", "adept_relocate_batch", "adept_shutdown"]
 
 
 def load_library():
@@ -89,6 +89,7 @@ def load_library():
     lib.adept_step_frozen.argtypes = [vp, i, vp, vp, vp, vp]
     lib.adept_distance_batch.argtypes = [vp, i, i, vp, vp, vp, vp, vp, vp]
     lib.adept_locate_batch.argtypes = [vp, i, i, vp, vp, vp]
+    lib.adept_relocate_batch.argtypes = [vp, i, i, vp, vp, vp, vp]
     lib.adept_shutdown.argtypes = [vp]
     return lib
 
@@ -214,9 +215,10 @@ class Adept:
         return s
 
     def kernel_times(self, slot=0):
-        """(ms[2], launches[2]) of the gamma / charged step kernels since the last call (time_kernels=1)."""
-        ms = np.zeros(2)
-        n = np.zeros(2, dtype=np.uint64)
+        """(ms[3], launches[3]) of the gamma move / charged move / interaction kernels since the last call
+        (time_kernels=1)."""
+        ms = np.zeros(3)
+        n = np.zeros(3, dtype=np.uint64)
         _check(lib.adept_get_kernel_times(self.ctx, slot, _ptr(ms), _ptr(n)))
         return ms, n
 
@@ -243,4 +245,11 @@ class Adept:
         pos = np.ascontiguousarray(pos, dtype=np.float64).reshape(-1, 3)
         out = np.zeros(pos.shape[0], dtype=np.int64)
         _check(lib.adept_locate_batch(self.ctx, navigator, pos.shape[0], _ptr(pos), _ptr(out), None))
+        return out
+
+    def relocate_batch(self, pos, from_volume, navigator=NAV_BVH):
+        pos = np.ascontiguousarray(pos, dtype=np.float64).reshape(-1, 3)
+        frm = np.ascontiguousarray(np.broadcast_to(from_volume, (pos.shape[0],)), dtype=np.uint32)
+        out = np.zeros(pos.shape[0], dtype=np.int64)
+        _check(lib.adept_relocate_batch(self.ctx, navigator, pos.shape[0], _ptr(pos), _ptr(frm), _ptr(out), None))
         return out

@@ -150,10 +150,10 @@ struct SlotHost {
   unsigned long long launches = 0;
   bool live = false;
   // optional per-launch timing (config.time_kernels)
-  std::vector<cudaEvent_t> tev;      // [sync_interval][2 kernels][start, stop]
+  std::vector<cudaEvent_t> tev;      // [sync_interval][kTimed kernels][start, stop]
   int tev_used = 0;
-  double kernel_ms[2] = {0.0, 0.0};
-  unsigned long long kernel_launches[2] = {0, 0};
+  double kernel_ms[ADEPT_N_TIMED_KERNELS] = {};
+  unsigned long long kernel_launches[ADEPT_N_TIMED_KERNELS] = {};
 };
 
 struct adept_ctx {
@@ -164,10 +164,10 @@ struct adept_ctx {
   adept_track* d_stage = nullptr;    // staging area for primaries (inside the workspace)
   uint32_t* d_bad = nullptr;
   size_t stage_cap = 0;
-  int grid_gamma = 0, grid_charged = 0, grid_reloc = 0, grid_inter = 0;
-  // split-mode kernels specialised for this context's field kind and for geometries without BVH volumes
+  int grid_gamma = 0, grid_charged = 0, grid_inter = 0;
+  // move kernels specialised for this context's field kind and for geometries without BVH volumes
   using Kernel = void (*)(DevCtx, DevSlot, int);
-  Kernel k_move_gamma = nullptr, k_move_charged = nullptr, k_relocate = nullptr;
+  Kernel k_move_gamma = nullptr, k_move_charged = nullptr;
 };
 
 extern "C" const char* adept_last_error(void) { return g_err; }
@@ -178,7 +178,7 @@ extern "C" void adept_default_config(adept_config* c) {
   c->delta_chord = 1e-3; c->eps_push = 1e-7; c->alpha_R = 0.2; c->rho_R = 0.1;
   c->chord_budget = 16; c->seed = 1; c->max_steps = 1000000;
   c->navigator = ADEPT_NAV_BVH; c->n_event_slots = 1; c->sync_interval = 8;
-  c->track_capacity = 1u << 20; c->leak_capacity = 1u << 16; c->split_kernels = 1;
+  c->track_capacity = 1u << 20; c->leak_capacity = 1u << 16; c->stage_capacity = 0;
 }
 
 namespace {
@@ -190,6 +190,7 @@ int validate(const adept_config* cfg, const adept_geometry* g, int n_mats, const
     return fail(ADEPT_EINVAL, "null geometry array");
   if (cfg->n_event_slots < 1 || cfg->n_event_slots > 1024) return fail(ADEPT_EINVAL, "n_event_slots out of range");
   if (cfg->track_capacity < 32 || cfg->track_capacity > 0x3fffffffu) return fail(ADEPT_EINVAL, "track_capacity out of range");
+  if (cfg->stage_capacity != 0 && (cfg->stage_capacity < 32 || cfg->stage_capacity > 0x3fffffffu)) return fail(ADEPT_EINVAL, "stage_capacity out of range");
   if (cfg->chord_budget < 1 || cfg->sync_interval < 1) return fail(ADEPT_EINVAL, "chord_budget / sync_interval must be >= 1");
   if (g->mother[0] != -1) return fail(ADEPT_EINVAL, "volume 0 must be the world");
   for (int v = 0; v < g->n_volumes; ++v) {
@@ -208,7 +209,7 @@ int validate(const adept_config* cfg, const adept_geometry* g, int n_mats, const
 }
 
 struct Layout {
-  DevVolume* vol; DevBvh* bvh; double *tab_g, *tab_em, *tab_ep, *scal, *bz;
+  DevVolume* vol; double* rot; DevBvh* bvh; double *tab_g, *tab_em, *tab_ep, *scal, *bz;
   std::vector<double*> bvh_prim_box; std::vector<int32_t*> bvh_prim_vol; std::vector<std::vector<double*>> bvh_node_box;
   adept_track* stage; uint32_t* bad; size_t stage_cap;
   std::vector<DevSlot> slots;
@@ -220,6 +221,7 @@ size_t carve(void* base, const adept_config* cfg, const adept_geometry* g, int n
   Carver cv(base);
   Layout L{};
   L.vol = cv.take<DevVolume>(g->n_volumes);
+  L.rot = cv.take<double>(9 * static_cast<size_t>(g->n_volumes));
   std::vector<int> bvh_vols;
   for (int v = 0; v < g->n_volumes; ++v) if (g->daughter_count[v] >= kBvhMinDaughters) bvh_vols.push_back(v);
   L.bvh = cv.take<DevBvh>(std::max<size_t>(bvh_vols.size(), 1));
@@ -242,23 +244,23 @@ size_t carve(void* base, const adept_config* cfg, const adept_geometry* g, int n
   L.stage = cv.take<adept_track>(L.stage_cap);
   L.bad = cv.take<uint32_t>(1);
   const size_t cap = cfg->track_capacity;
+  const size_t scap = cfg->stage_capacity ? cfg->stage_capacity : cap;
+  auto take_soa = [&cv](TrackSoA& b, size_t n) {
+    b.x = cv.take<double>(n); b.y = cv.take<double>(n); b.z = cv.take<double>(n);
+    b.dx = cv.take<double>(n); b.dy = cv.take<double>(n); b.dz = cv.take<double>(n);
+    b.ekin = cv.take<double>(n); b.id = cv.take<uint64_t>(n);
+    b.event = cv.take<uint32_t>(n); b.step = cv.take<uint32_t>(n); b.vol = cv.take<uint32_t>(n);
+  };
   for (int s = 0; s < cfg->n_event_slots; ++s) {
     DevSlot d{};
     for (int p = 0; p < 2; ++p)
-      for (int sp = 0; sp < 3; ++sp) {
-        TrackSoA& b = d.buf[p][sp];
-        b.x = cv.take<double>(cap); b.y = cv.take<double>(cap); b.z = cv.take<double>(cap);
-        b.dx = cv.take<double>(cap); b.dy = cv.take<double>(cap); b.dz = cv.take<double>(cap);
-        b.ekin = cv.take<double>(cap); b.id = cv.take<uint64_t>(cap);
-        b.event = cv.take<uint32_t>(cap); b.step = cv.take<uint32_t>(cap); b.vol = cv.take<uint32_t>(cap);
-      }
+      for (int sp = 0; sp < 3; ++sp) take_soa(d.buf[p][sp], cap);
+    for (int q = 0; q < kNumStage; ++q) take_soa(d.stage[q], scap);
     d.counters = cv.take<SlotCounters>(1);
     d.edep = cv.take<double>(g->n_volumes);
     d.ledger = cv.take<double>(8);
     d.stats = cv.take<DevStats>(1);
     d.leaked = cv.take<adept_track>(std::max<size_t>(cfg->leak_capacity, 1));
-    d.reloc_queue = cv.take<uint32_t>(cfg->split_kernels ? 3 * cap : 1);
-    d.inter_queue = cv.take<uint32_t>(cfg->split_kernels ? 7 * cap : 1);
     L.slots.push_back(d);
   }
   if (out) *out = std::move(L);
@@ -291,10 +293,11 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
     DevVolume& d = hv[v];
     for (int k = 0; k < 3; ++k) { d.t[k] = g->trans[3 * v + k]; d.dims[k] = g->dims[3 * v + k]; }
     bool ident = true;
-    for (int k = 0; k < 9; ++k) { d.R[k] = g->rot[9 * v + k]; ident = ident && d.R[k] == ((k % 4 == 0) ? 1.0 : 0.0); }
+    for (int k = 0; k < 9; ++k) ident = ident && g->rot[9 * v + k] == ((k % 4 == 0) ? 1.0 : 0.0);
     d.solid = g->solid[v]; d.material = g->material[v];
     d.dbegin = g->daughter_begin[v]; d.dcount = g->daughter_count[v];
     d.identity = ident ? 1 : 0;
+    d.mother = g->mother[v]; d.pad = 0;
     d.bvh = -1;
     if (d.dcount >= kBvhMinDaughters) {
       const HostBvh b = build_bvh(g, v);
@@ -317,6 +320,7 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
     }
   }
   CUDA_TRY(cudaMemcpy(L.vol, hv.data(), hv.size() * sizeof(DevVolume), cudaMemcpyHostToDevice));
+  CUDA_TRY(cudaMemcpy(L.rot, g->rot, 9 * static_cast<size_t>(nv) * sizeof(double), cudaMemcpyHostToDevice));
   if (!hb.empty()) CUDA_TRY(cudaMemcpy(L.bvh, hb.data(), hb.size() * sizeof(DevBvh), cudaMemcpyHostToDevice));
 
   // ---- interleaved table slices (one node = one row)
@@ -345,7 +349,7 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   ctx->cfg = *cfg;
   ctx->n_vol = nv; ctx->n_mat = n_mats;
   DevCtx& d = ctx->dev;
-  d.vol = L.vol; d.n_vol = nv; d.bvh = L.bvh; d.navigator = cfg->navigator;
+  d.vol = L.vol; d.rot = L.rot; d.n_vol = nv; d.bvh = L.bvh; d.navigator = cfg->navigator;
   d.tab_g = L.tab_g; d.tab_em = L.tab_em; d.tab_ep = L.tab_ep; d.scal = L.scal; d.n_mat = n_mats;
   d.field_kind = f->kind;
   for (int k = 0; k < 3; ++k) d.B[k] = f->B[k];
@@ -356,19 +360,16 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   d.delta_chord = cfg->delta_chord; d.eps_push = cfg->eps_push; d.alpha_R = cfg->alpha_R; d.rho_R = cfg->rho_R;
   d.chord_budget = cfg->chord_budget; d.seed = cfg->seed; d.max_steps = cfg->max_steps;
   d.capacity = static_cast<uint32_t>(cfg->track_capacity);
+  d.stage_capacity = static_cast<uint32_t>(cfg->stage_capacity ? cfg->stage_capacity : cfg->track_capacity);
   d.leak_capacity = static_cast<uint32_t>(cfg->leak_capacity);
   ctx->d_stage = L.stage; ctx->d_bad = L.bad; ctx->stage_cap = L.stage_cap;
 
-  int dev = 0, sms = 0, occ_g = 1, occ_c = 1;
+  int dev = 0, sms = 0, occ_g = 1, occ_c = 1, occ_i = 1;
   CUDA_TRY(cudaGetDevice(&dev));
   CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-  CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_g, step_kernel<MODE_GAMMA>, kBlock, 0));
-  CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_c, step_kernel<MODE_CHARGED>, kBlock, 0));
-  if (cfg->split_kernels) {
-    int occ_r = 1, occ_i = 1;
+  {
     const bool bvh = cfg->navigator == ADEPT_NAV_BVH && !hb.empty();
     ctx->k_move_gamma = bvh ? move_kernel<MODE_GAMMA, ADEPT_FIELD_NONE, true> : move_kernel<MODE_GAMMA, ADEPT_FIELD_NONE, false>;
-    ctx->k_relocate = bvh ? relocate_kernel<true> : relocate_kernel<false>;
     switch (f->kind) {
       case ADEPT_FIELD_NONE:
         ctx->k_move_charged = bvh ? move_kernel<MODE_CHARGED, ADEPT_FIELD_NONE, true> : move_kernel<MODE_CHARGED, ADEPT_FIELD_NONE, false>; break;
@@ -379,13 +380,11 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
     }
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_g, ctx->k_move_gamma, kBlock, 0));
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_c, ctx->k_move_charged, kBlock, 0));
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_r, ctx->k_relocate, kBlock, 0));
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_i, interact_kernel, kBlock, 0));
-    ctx->grid_reloc = sms * std::max(occ_r, 1);
-    ctx->grid_inter = sms * std::max(occ_i, 1);
   }
   ctx->grid_gamma = sms * std::max(occ_g, 1);
   ctx->grid_charged = sms * std::max(occ_c, 1);
+  ctx->grid_inter = sms * std::max(occ_i, 1);
 
   ctx->slots.resize(cfg->n_event_slots);
   for (int s = 0; s < cfg->n_event_slots; ++s) {
@@ -397,7 +396,7 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
     CUDA_TRY(cudaMallocHost(&sh.pinned, sizeof(SlotCounters)));
     std::memset(sh.pinned, 0, sizeof(SlotCounters));
     if (cfg->time_kernels) {
-      sh.tev.resize(static_cast<size_t>(cfg->sync_interval) * 4);
+      sh.tev.resize(static_cast<size_t>(cfg->sync_interval) * 2 * ADEPT_N_TIMED_KERNELS);
       for (cudaEvent_t& e : sh.tev) CUDA_TRY(cudaEventCreate(&e));
     }
   }
@@ -467,37 +466,28 @@ extern "C" int adept_enqueue_primaries(adept_ctx* ctx, int slot, uint32_t event_
 
 namespace {
 
-// One population step of a slot: gamma kernel on the caller's stream, charged kernel on the helper
-// stream (species kernels on different streams, synchronised with events), then the
-// buffer swap.
+// One population step of a slot: gamma move kernel on the caller's stream, charged move kernel on the
+// helper stream (species kernels on different streams, synchronised with events), then the
+// interaction kernel over what they staged and the buffer swap.
 int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity) {
+  constexpr int kEv = 2 * ADEPT_N_TIMED_KERNELS;
   CUDA_TRY(cudaEventRecord(sh.fork, st));
   CUDA_TRY(cudaStreamWaitEvent(sh.helper, sh.fork, 0));
-  const bool timed = !sh.tev.empty() && sh.tev_used + 4 <= static_cast<int>(sh.tev.size());
+  const bool timed = !sh.tev.empty() && sh.tev_used + kEv <= static_cast<int>(sh.tev.size());
   cudaEvent_t* ev = timed ? &sh.tev[sh.tev_used] : nullptr;
-  const bool split = ctx->cfg.split_kernels != 0;
   if (timed) CUDA_TRY(cudaEventRecord(ev[0], st));
-  if (split) ctx->k_move_gamma<<<dim3(ctx->grid_gamma, 1), kBlock, 0, st>>>(ctx->dev, sh.dev, parity);
-  else step_kernel<MODE_GAMMA><<<dim3(ctx->grid_gamma, 1), kBlock, 0, st>>>(ctx->dev, sh.dev, parity);
+  ctx->k_move_gamma<<<dim3(ctx->grid_gamma, 1), kBlock, 0, st>>>(ctx->dev, sh.dev, parity);
   if (timed) CUDA_TRY(cudaEventRecord(ev[1], st));
   if (timed) CUDA_TRY(cudaEventRecord(ev[2], sh.helper));
-  if (split) ctx->k_move_charged<<<dim3(ctx->grid_charged, 2), kBlock, 0, sh.helper>>>(ctx->dev, sh.dev, parity);
-  else step_kernel<MODE_CHARGED><<<dim3(ctx->grid_charged, 2), kBlock, 0, sh.helper>>>(ctx->dev, sh.dev, parity);
-  if (timed) { CUDA_TRY(cudaEventRecord(ev[3], sh.helper)); sh.tev_used += 4; }
-  if (split) {
-    // relocation on the caller's stream, interactions on the helper stream: they touch disjoint tracks
-    CUDA_TRY(cudaEventRecord(sh.join, sh.helper));
-    CUDA_TRY(cudaStreamWaitEvent(st, sh.join, 0));
-    CUDA_TRY(cudaEventRecord(sh.fork, st));
-    CUDA_TRY(cudaStreamWaitEvent(sh.helper, sh.fork, 0));
-    ctx->k_relocate<<<ctx->grid_reloc, kBlock, 0, st>>>(ctx->dev, sh.dev, parity);
-    interact_kernel<<<ctx->grid_inter, kBlock, 0, sh.helper>>>(ctx->dev, sh.dev, parity);
-    sh.launches += 2;
-  }
+  ctx->k_move_charged<<<dim3(ctx->grid_charged, 2), kBlock, 0, sh.helper>>>(ctx->dev, sh.dev, parity);
+  if (timed) CUDA_TRY(cudaEventRecord(ev[3], sh.helper));
   CUDA_TRY(cudaEventRecord(sh.join, sh.helper));
   CUDA_TRY(cudaStreamWaitEvent(st, sh.join, 0));
-  finish_iteration_kernel<<<1, 1, 0, st>>>(sh.dev, parity);
-  sh.launches += 3;
+  if (timed) CUDA_TRY(cudaEventRecord(ev[4], st));
+  interact_kernel<<<ctx->grid_inter, kBlock, 0, st>>>(ctx->dev, sh.dev, parity);
+  if (timed) { CUDA_TRY(cudaEventRecord(ev[5], st)); sh.tev_used += kEv; }
+  finish_iteration_kernel<<<1, 32, 0, st>>>(sh.dev, parity);
+  sh.launches += 4;
   return ADEPT_OK;
 }
 
@@ -530,17 +520,17 @@ extern "C" int adept_transport_many(adept_ctx* ctx, int n_slots, const int* slot
       SlotHost& sh = ctx->slots[slots[k]];
       if (!sh.live) continue;
       CUDA_TRY(cudaStreamSynchronize(static_cast<cudaStream_t>(streams[k])));
-      for (int e = 0; e + 4 <= sh.tev_used; e += 4)
-        for (int kk = 0; kk < 2; ++kk) {
+      for (int e = 0; e + 2 * ADEPT_N_TIMED_KERNELS <= sh.tev_used; e += 2 * ADEPT_N_TIMED_KERNELS)
+        for (int kk = 0; kk < ADEPT_N_TIMED_KERNELS; ++kk) {
           float ms = 0.f;
           CUDA_TRY(cudaEventElapsedTime(&ms, sh.tev[e + 2 * kk], sh.tev[e + 2 * kk + 1]));
           sh.kernel_ms[kk] += ms;
           sh.kernel_launches[kk] += 1;
         }
       sh.tev_used = 0;
-      if (sh.pinned->overflow) rc_final = fail(ADEPT_EOVERFLOW, "slot %d: track queue overflow (capacity %llu per species)",
+      if (sh.pinned->overflow.v) rc_final = fail(ADEPT_EOVERFLOW, "slot %d: track queue overflow (capacity %llu per species)",
                                                slots[k], static_cast<unsigned long long>(ctx->cfg.track_capacity));
-      if (sh.pinned->live == 0 || sh.pinned->overflow) {
+      if (sh.pinned->live.v == 0 || sh.pinned->overflow.v) {
         sh.live = false;
         --n_live;
         if (parity[k]) {  // leave the (empty) slot at parity 0 for the next enqueue
@@ -578,12 +568,12 @@ extern "C" int adept_read_leaked(adept_ctx* ctx, int slot, adept_track* out, siz
   if (rc != ADEPT_OK) return rc;
   if (!n) return fail(ADEPT_EINVAL, "null argument");
   SlotHost& sh = ctx->slots[slot];
-  SlotCounters c;
-  CUDA_TRY(cudaMemcpy(&c, sh.dev.counters, sizeof(c), cudaMemcpyDeviceToHost));
-  *n = c.n_leaked;
-  const size_t m = std::min<size_t>(std::min<size_t>(c.n_leaked, cap), ctx->cfg.leak_capacity);
+  uint32_t n_leaked = 0;
+  CUDA_TRY(cudaMemcpy(&n_leaked, &sh.dev.counters->n_leaked.v, sizeof(uint32_t), cudaMemcpyDeviceToHost));
+  *n = n_leaked;
+  const size_t m = std::min<size_t>(std::min<size_t>(n_leaked, cap), ctx->cfg.leak_capacity);
   if (m && out) CUDA_TRY(cudaMemcpy(out, sh.dev.leaked, m * sizeof(adept_track), cudaMemcpyDeviceToHost));
-  CUDA_TRY(cudaMemset(&sh.dev.counters->n_leaked, 0, sizeof(uint32_t)));
+  CUDA_TRY(cudaMemset(&sh.dev.counters->n_leaked.v, 0, sizeof(uint32_t)));
   return ADEPT_OK;
 }
 
@@ -600,13 +590,14 @@ extern "C" int adept_get_stats(adept_ctx* ctx, int slot, adept_stats* out) {
   return ADEPT_OK;
 }
 
-extern "C" int adept_get_kernel_times(adept_ctx* ctx, int slot, double ms[2], uint64_t launches[2]) {
+extern "C" int adept_get_kernel_times(adept_ctx* ctx, int slot, double ms[ADEPT_N_TIMED_KERNELS],
+                                      uint64_t launches[ADEPT_N_TIMED_KERNELS]) {
   const int rc = check_slot(ctx, slot);
   if (rc != ADEPT_OK) return rc;
   if (!ms || !launches) return fail(ADEPT_EINVAL, "null argument");
   SlotHost& sh = ctx->slots[slot];
   if (sh.tev.empty()) return fail(ADEPT_ESTATE, "context was not created with time_kernels");
-  for (int k = 0; k < 2; ++k) { ms[k] = sh.kernel_ms[k]; launches[k] = sh.kernel_launches[k]; sh.kernel_ms[k] = 0.0; sh.kernel_launches[k] = 0; }
+  for (int k = 0; k < ADEPT_N_TIMED_KERNELS; ++k) { ms[k] = sh.kernel_ms[k]; launches[k] = sh.kernel_launches[k]; sh.kernel_ms[k] = 0.0; sh.kernel_launches[k] = 0; }
   return ADEPT_OK;
 }
 
@@ -669,5 +660,26 @@ extern "C" int adept_locate_batch(adept_ctx* ctx, int nav, int n, const double* 
   CUDA_TRY(cudaMemcpyAsync(out, d_out, n * sizeof(long long), cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
   cudaFree(d_pos); cudaFree(d_out);
+  return ADEPT_OK;
+}
+
+extern "C" int adept_relocate_batch(adept_ctx* ctx, int nav, int n, const double* pos3, const uint32_t* from, int64_t* out,
+                                    void* stream) {
+  if (!ctx || n < 0 || (n > 0 && (!pos3 || !from || !out))) return fail(ADEPT_EINVAL, "null argument");
+  if (n == 0) return ADEPT_OK;
+  for (int i = 0; i < n; ++i) if (from[i] >= static_cast<uint32_t>(ctx->n_vol)) return fail(ADEPT_EINVAL, "point %d: volume out of range", i);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  double* d_pos;
+  uint32_t* d_from;
+  long long* d_out;
+  CUDA_TRY(cudaMalloc(&d_pos, 3 * n * sizeof(double))); CUDA_TRY(cudaMalloc(&d_from, n * sizeof(uint32_t)));
+  CUDA_TRY(cudaMalloc(&d_out, n * sizeof(long long)));
+  CUDA_TRY(cudaMemcpyAsync(d_pos, pos3, 3 * n * sizeof(double), cudaMemcpyHostToDevice, st));
+  CUDA_TRY(cudaMemcpyAsync(d_from, from, n * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
+  relocate_kernel<<<std::min((n + kBlock - 1) / kBlock, 65535), kBlock, 0, st>>>(ctx->dev, nav, n, d_pos, d_from, d_out);
+  CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(cudaMemcpyAsync(out, d_out, n * sizeof(long long), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  cudaFree(d_pos); cudaFree(d_from); cudaFree(d_out);
   return ADEPT_OK;
 }

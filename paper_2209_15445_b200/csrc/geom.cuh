@@ -10,16 +10,21 @@ namespace adept {
 
 __device__ __forceinline__ const DevVolume& volume(const DevCtx& c, int v) { return c.vol[v]; }
 
-__device__ __forceinline__ void to_local(const DevVolume& v, double gx, double gy, double gz, double l[3]) {
+// local = R^T (global - t); R (row-major, local axes as columns) is only read for rotated placements
+__device__ __forceinline__ void to_local(const DevCtx& c, int vi, const DevVolume& v, double gx, double gy, double gz,
+                                         double l[3]) {
   const double q0 = gx - v.t[0], q1 = gy - v.t[1], q2 = gz - v.t[2];
   if (v.identity) { l[0] = q0; l[1] = q1; l[2] = q2; return; }
+  const double* __restrict__ R = c.rot + 9 * static_cast<size_t>(vi);
 #pragma unroll
-  for (int i = 0; i < 3; ++i) l[i] = v.R[0 + i] * q0 + v.R[3 + i] * q1 + v.R[6 + i] * q2;
+  for (int i = 0; i < 3; ++i) l[i] = __ldg(R + i) * q0 + __ldg(R + 3 + i) * q1 + __ldg(R + 6 + i) * q2;
 }
-__device__ __forceinline__ void dir_to_local(const DevVolume& v, double gx, double gy, double gz, double l[3]) {
+__device__ __forceinline__ void dir_to_local(const DevCtx& c, int vi, const DevVolume& v, double gx, double gy, double gz,
+                                             double l[3]) {
   if (v.identity) { l[0] = gx; l[1] = gy; l[2] = gz; return; }
+  const double* __restrict__ R = c.rot + 9 * static_cast<size_t>(vi);
 #pragma unroll
-  for (int i = 0; i < 3; ++i) l[i] = v.R[0 + i] * gx + v.R[3 + i] * gy + v.R[6 + i] * gz;
+  for (int i = 0; i < 3; ++i) l[i] = __ldg(R + i) * gx + __ldg(R + 3 + i) * gy + __ldg(R + 6 + i) * gz;
 }
 
 // ---------------------------------------------------------------- G1 solids
@@ -122,7 +127,7 @@ __device__ __forceinline__ double solid_entry(const DevVolume& v, const double p
 __device__ __forceinline__ bool inside_volume(const DevCtx& c, int vol, double x, double y, double z) {
   const DevVolume& v = volume(c, vol);
   double l[3];
-  to_local(v, x, y, z, l);
+  to_local(c, vol, v, x, y, z, l);
   return inside_solid(v.solid, v.dims, l);
 }
 
@@ -130,8 +135,8 @@ __device__ __noinline__ double entry_distance(const DevCtx& c, int vol, double p
                                                  double dx, double dy, double dz) {
   const DevVolume& v = volume(c, vol);
   double lp[3], ld[3];
-  to_local(v, px, py, pz, lp);
-  dir_to_local(v, dx, dy, dz, ld);
+  to_local(c, vol, v, px, py, pz, lp);
+  dir_to_local(c, vol, v, dx, dy, dz, ld);
   return solid_entry(v, lp, ld);
 }
 
@@ -260,8 +265,8 @@ __device__ __noinline__ double nav_distance(const DevCtx& c, int nav, bool activ
   if (active) {
     const DevVolume& v = volume(c, vol);
     double lp[3], ld[3];
-    to_local(v, px, py, pz, lp);
-    dir_to_local(v, dx, dy, dz, ld);
+    to_local(c, vol, v, px, py, pz, lp);
+    dir_to_local(c, vol, v, dx, dy, dz, ld);
     s = fmin(s_max, solid_exit(v, lp, ld));
     if (v.dcount > 0) {
       if (BVH && nav == ADEPT_NAV_BVH && v.bvh >= 0) {
@@ -334,6 +339,69 @@ __device__ __noinline__ int nav_locate(const DevCtx& c, int nav, bool active, do
                               __shfl_sync(kFull, qy, src), __shfl_sync(kFull, qz, src));
       if (lane == src) {
         if (r < 0) desc = false; else cur = r;
+      }
+    }
+  }
+  return cur;
+}
+
+// ---------------------------------------------------------------- A5 relocation after a boundary
+// Same result as nav_locate(q) -- the deepest volume containing q -- found locally: climb from the
+// volume the track was in until q is inside, then descend.  Daughters lie inside their mothers and
+// siblings are disjoint (adept.h), so at most one daughter contains q and the order in which they are
+// tried cannot change the answer: the neighbours (in index order) of the daughter just left are tried
+// first, which makes a crossing between consecutive layers of a stack O(1) instead of O(layers)
+// (relocation cost and "fewer trial steps").  Warp-convergent call when BVH is true.
+// Returns -1 outside the world or for inactive lanes.
+template <bool BVH = true>
+__device__ __noinline__ int nav_relocate(const DevCtx& c, int nav, bool active, uint32_t vol_old, double qx, double qy,
+                                         double qz) {
+  int cur = -1, prev = -1;
+  bool desc = false;
+  if (active) {
+    cur = static_cast<int>(vol_old);
+    while (cur >= 0 && !inside_volume(c, cur, qx, qy, qz)) { prev = cur; cur = volume(c, cur).mother; }
+    desc = cur >= 0;
+  }
+  for (;;) {
+    if (BVH) { if (!__any_sync(kFull, desc)) break; } else if (!desc) break;
+    bool need = false;
+    int bvh = -1;
+    if (desc) {
+      const DevVolume& v = volume(c, cur);
+      if (v.dcount == 0) {
+        desc = false;
+      } else if (BVH && nav == ADEPT_NAV_BVH && v.bvh >= 0) {
+        need = true;
+        bvh = v.bvh;
+      } else {
+        int next = -1;
+        if (prev >= 0) {  // came up from daughter `prev` (q is outside it): try its neighbours first
+          const int k0 = prev - v.dbegin;
+          if (k0 + 1 < v.dcount && inside_volume(c, prev + 1, qx, qy, qz)) next = prev + 1;
+          else if (k0 >= 1 && inside_volume(c, prev - 1, qx, qy, qz)) next = prev - 1;
+        }
+        for (int k = 0; next < 0 && k < v.dcount; ++k) {
+          const int d = v.dbegin + k;
+          if (prev >= 0 && (d == prev || d == prev + 1 || d == prev - 1)) continue;
+          if (inside_volume(c, d, qx, qy, qz)) next = d;
+        }
+        if (next < 0) desc = false; else cur = next;
+        prev = -1;
+      }
+    }
+    if (BVH) {
+      unsigned m = __ballot_sync(kFull, need);
+      const int lane = threadIdx.x & 31;
+      while (m) {
+        const int src = __ffs(m) - 1;
+        m &= m - 1;
+        const int r = bvh_point(c, c.bvh[__shfl_sync(kFull, bvh, src)], __shfl_sync(kFull, qx, src),
+                                __shfl_sync(kFull, qy, src), __shfl_sync(kFull, qz, src));
+        if (lane == src) {
+          if (r < 0) desc = false; else cur = r;
+          prev = -1;
+        }
       }
     }
   }

@@ -2,13 +2,16 @@
 // A9, A10).  Differences from the paper's design: the per-species
 // "current/next" arrays hold the track records themselves (SoA, ping-pong) instead of indices into
 // an append-only store, so every read and write of track state is coalesced and finished slots are
-// reclaimed every step; survivors and secondaries are appended with warp-aggregated atomics.
+// reclaimed every step.  A thread block works on tiles of kBlock consecutive tracks; everything a tile
+// appends (survivors, staged interactions, secondaries) is reserved with ONE global atomic per
+// destination queue and tile, and every queue counter has its own 128 B line.
 #pragma once
 #include "step.cuh"
 
 namespace adept {
 
 constexpr int kBlock = 128;
+constexpr int kWarps = kBlock / 32;
 // minimum resident blocks per SM asked of the compiler (register caps chosen from measurement)
 #ifndef ADEPT_MINB_G
 #define ADEPT_MINB_G 4
@@ -37,22 +40,50 @@ __device__ __forceinline__ void store_track(const TrackSoA& b, uint32_t i, const
   b.event[i] = t.event; b.step[i] = t.step; b.vol[i] = t.vol;
 }
 
-// Warp-aggregated append (A0): lanes with `want` get consecutive slots of `counter`; one atomic per warp.
-__device__ __forceinline__ uint32_t warp_append(uint32_t* counter, bool want) {
-  const unsigned m = __ballot_sync(kFull, want);
-  if (m == 0) return 0;
-  const int lane = threadIdx.x & 31;
-  const int leader = __ffs(m) - 1;
-  uint32_t base = 0;
-  if (lane == leader) base = atomicAdd(counter, __popc(m));
-  base = __shfl_sync(kFull, base, leader);
-  return base + __popc(m & ((1u << lane) - 1u));
-}
-
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
   return v;
+}
+
+// ------------------------------------------------------------------------------------------------
+// A0: block-aggregated append.  Every lane asks for cnt[d] (0..3) consecutive entries of destination
+// queue d; the block adds its total to each queue counter with one atomic and every lane gets the
+// index of its first entry.  Must be called by all threads of the block (two __syncthreads); the
+// caller alternates `phase` between consecutive calls so that a fast warp cannot overwrite the
+// per-warp totals a slow warp still reads.
+template <int ND>
+struct BlockReserve {
+  uint32_t wtot[2][kWarps][ND];
+  uint32_t base[2][ND];
+};
+
+template <int ND, typename CounterOf>
+__device__ __forceinline__ void block_reserve(BlockReserve<ND>& br, int phase, const uint32_t (&cnt)[ND], uint32_t (&first)[ND],
+                                              CounterOf counter_of) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned lt = (1u << lane) - 1u;
+  uint32_t pre[ND];
+#pragma unroll
+  for (int d = 0; d < ND; ++d) {
+    const unsigned b0 = __ballot_sync(kFull, cnt[d] & 1u), b1 = __ballot_sync(kFull, cnt[d] & 2u);
+    pre[d] = __popc(b0 & lt) + 2 * __popc(b1 & lt);
+    if (lane == 0) br.wtot[phase][warp][d] = __popc(b0) + 2 * __popc(b1);
+  }
+  __syncthreads();
+  if (threadIdx.x < ND) {
+    uint32_t tot = 0;
+#pragma unroll
+    for (int w = 0; w < kWarps; ++w) tot += br.wtot[phase][w][threadIdx.x];
+    br.base[phase][threadIdx.x] = tot ? atomicAdd(counter_of(threadIdx.x), tot) : 0u;
+  }
+  __syncthreads();
+#pragma unroll
+  for (int d = 0; d < ND; ++d) {
+    uint32_t f = br.base[phase][d] + pre[d];
+    for (int w = 0; w < warp; ++w) f += br.wtot[phase][w][d];
+    first[d] = f;
+  }
 }
 
 // A9: warp-reduced scoring.  Lanes depositing into the same volume are combined (match_any) and the
@@ -73,84 +104,46 @@ __device__ __forceinline__ void score(double* edep, uint32_t vol, double e, bool
   if (lane == __ffs(peers) - 1) atomicAdd(edep + vol, sum);
 }
 
+// Per-block statistics, folded into the slot's counters once at the end of the kernel.
 struct BlockTally {
   double ledger[4];                       // deposited, below_cut, escaped, killed
-  unsigned long long steps, chords;
-  unsigned long long outcomes[ADEPT_N_OUTCOMES];
-  unsigned long long secondaries[3];
-  unsigned int touched;
+  unsigned long long chords;
+  unsigned int steps;
+  unsigned int outcomes[ADEPT_N_OUTCOMES];
+  unsigned int secondaries[3];
 };
 
-// per-thread partial sums, folded into the block tally at the end of the kernel
-struct LaneTally {
-  double dep = 0.0, cut = 0.0, esc = 0.0, kill = 0.0;
-  unsigned steps = 0, chords = 0;
-};
-
-__device__ __forceinline__ void flush_tally(BlockTally& tally, const LaneTally& l, const DevSlot& slot, int species) {
-  const int lane = threadIdx.x & 31;
-  const double dep = warp_sum(l.dep), cut = warp_sum(l.cut), esc = warp_sum(l.esc), kill = warp_sum(l.kill);
-  if (lane == 0) {
-    if (dep != 0.0) atomicAdd(&tally.ledger[0], dep);
-    if (cut != 0.0) atomicAdd(&tally.ledger[1], cut);
-    if (esc != 0.0) atomicAdd(&tally.ledger[2], esc);
-    if (kill != 0.0) atomicAdd(&tally.ledger[3], kill);
-  }
-  if (l.steps) {
-    atomicAdd(&tally.steps, static_cast<unsigned long long>(l.steps));
-    atomicAdd(&tally.chords, static_cast<unsigned long long>(l.chords));
-  }
+__device__ __forceinline__ void tally_init(BlockTally& t) {
+  if (threadIdx.x == 0) t = BlockTally{};
   __syncthreads();
-  if (threadIdx.x == 0 && tally.touched) {
-    for (int k = 0; k < 4; ++k) if (tally.ledger[k] != 0.0) atomicAdd(slot.ledger + k, tally.ledger[k]);
-    if (tally.steps) atomicAdd(&slot.stats->steps[species], tally.steps);
-    if (tally.chords) atomicAdd(&slot.stats->chords, tally.chords);
-    for (int k = 0; k < ADEPT_N_OUTCOMES; ++k) if (tally.outcomes[k]) atomicAdd(&slot.stats->outcomes[k], tally.outcomes[k]);
-    for (int k = 0; k < 3; ++k) if (tally.secondaries[k]) atomicAdd(&slot.stats->secondaries[k], tally.secondaries[k]);
-  }
 }
 
-// Appends the secondaries of a step to the next buffers.  All six (k, species) groups of the warp are
-// reserved in ONE round of atomics (lane sp adds the warp's total for species sp), so a warp waits for
-// a single atomic latency.  Warp-convergent.  `u` is the parent's stream (child ids, R3).
-__device__ __forceinline__ void append_secondaries(const DevCtx& c, const DevSlot& slot, int parity, bool active,
-                                                   uint32_t event, const Stream& u, const StepOut& o, BlockTally& tally) {
-  SlotCounters* cnt = slot.counters;
-  const int s0 = (active && o.n_sec > 0) ? o.sec[0].species : -1;
-  const int s1 = (active && o.n_sec > 1) ? o.sec[1].species : -1;
-  if (__ballot_sync(kFull, s0 >= 0) == 0) return;        // sec[1] exists only with sec[0]
-  const int lane = threadIdx.x & 31;
-  const unsigned lt = (1u << lane) - 1u;
-  unsigned m0[3], m1[3];
-#pragma unroll
-  for (int sp = 0; sp < 3; ++sp) { m0[sp] = __ballot_sync(kFull, s0 == sp); m1[sp] = __ballot_sync(kFull, s1 == sp); }
-  uint32_t mine = 0;
-  if (lane < 3) {
-    const unsigned n = __popc(lane == 0 ? m0[0] : lane == 1 ? m0[1] : m0[2]) + __popc(lane == 0 ? m1[0] : lane == 1 ? m1[1] : m1[2]);
-    if (n) { mine = atomicAdd(&cnt->count[parity ^ 1][lane], n); atomicAdd(&tally.secondaries[lane], static_cast<unsigned long long>(n)); }
+// warp-aggregated count of the lanes whose outcome is `which`
+__device__ __forceinline__ void tally_outcome(BlockTally& t, bool active, int outcome, int which) {
+  const unsigned m = __ballot_sync(kFull, active && outcome == which);
+  if (m && (threadIdx.x & 31) == 0) atomicAdd(&t.outcomes[which], static_cast<unsigned>(__popc(m)));
+}
+
+__device__ __forceinline__ void tally_flush(BlockTally& t, const DevSlot& slot, int species, double dep, double cut) {
+  dep = warp_sum(dep);
+  cut = warp_sum(cut);
+  if ((threadIdx.x & 31) == 0) {
+    if (dep != 0.0) atomicAdd(&t.ledger[0], dep);
+    if (cut != 0.0) atomicAdd(&t.ledger[1], cut);
   }
-  uint32_t base[3];
-#pragma unroll
-  for (int sp = 0; sp < 3; ++sp) base[sp] = __shfl_sync(kFull, mine, sp);
-#pragma unroll
-  for (int k = 0; k < 2; ++k) {
-    const int ss = k == 0 ? s0 : s1;
-    if (ss < 0) continue;
-    const uint32_t j = k == 0 ? base[ss] + __popc(m0[ss] & lt) : base[ss] + __popc(m0[ss]) + __popc(m1[ss] & lt);
-    if (j < c.capacity) {
-      Track s;
-      s.x = o.post.x; s.y = o.post.y; s.z = o.post.z;
-      s.dx = o.sec[k].dx; s.dy = o.sec[k].dy; s.dz = o.sec[k].dz;
-      s.ekin = o.sec[k].ekin; s.id = u.child_id(o.sec[k].child); s.event = event; s.step = 0; s.vol = o.post.vol; s.species = ss;
-      store_track(slot.buf[parity ^ 1][ss], j, s);
-    } else {
-      cnt->overflow = 1;
-    }
+  __syncthreads();
+  const int k = threadIdx.x;
+  if (k < 4) { if (t.ledger[k] != 0.0) atomicAdd(slot.ledger + k, t.ledger[k]); }
+  else if (k == 4) { if (t.steps) atomicAdd(&slot.stats->steps[species], static_cast<unsigned long long>(t.steps)); }
+  else if (k == 5) { if (t.chords) atomicAdd(&slot.stats->chords, t.chords); }
+  else if (k < 6 + 3) { if (t.secondaries[k - 6]) atomicAdd(&slot.stats->secondaries[k - 6], static_cast<unsigned long long>(t.secondaries[k - 6])); }
+  else if (k >= 32 && k < 32 + ADEPT_N_OUTCOMES) {
+    if (t.outcomes[k - 32]) atomicAdd(&slot.stats->outcomes[k - 32], static_cast<unsigned long long>(t.outcomes[k - 32]));
   }
 }
 
 __device__ __forceinline__ void record_leak(const DevCtx& c, const DevSlot& slot, const Track& t, int species) {
-  const uint32_t j = atomicAdd(&slot.counters->n_leaked, 1u);
+  const uint32_t j = atomicAdd(&slot.counters->n_leaked.v, 1u);
   if (j < c.leak_capacity) {
     adept_track& L = slot.leaked[j];
     L.pos[0] = t.x; L.pos[1] = t.y; L.pos[2] = t.z;
@@ -160,78 +153,58 @@ __device__ __forceinline__ void record_leak(const DevCtx& c, const DevSlot& slot
   }
 }
 
-// ------------------------------------------------------------------------------------------------
-// Fused mode: one kernel per species group does the whole step.  grid.y = species of a charged launch.
-template <int MODE>
-__global__ void __launch_bounds__(kBlock) step_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot,
-                                                      int parity) {
-  const int species = MODE == MODE_GAMMA ? ADEPT_GAMMA : static_cast<int>(blockIdx.y);
-  const TrackSoA& cur = slot.buf[parity][species];
-  SlotCounters* cnt = slot.counters;
-  const uint32_t n = cnt->count[parity][species];
-
-  __shared__ BlockTally tally;
-  if (threadIdx.x == 0) tally = BlockTally{};
-  __syncthreads();
-  LaneTally lt;
-
-  const uint32_t n_round = (n + 31u) & ~31u;
-  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += gridDim.x * blockDim.x) {
-    bool active = i < n;
-    Track in{};
-    if (active) in = load_track(cur, i, species);
-    in.species = species;
-    active = active && in.vol != kDeadVolume;
-    StepOut o;
-    step_track<MODE>(c, c.navigator, active, in, o);
-
-    score(slot.edep, in.vol, o.edep_dep + o.edep_cut, active);
-    if (active) {
-      lt.dep += o.edep_dep; lt.cut += o.edep_cut; lt.esc += o.escaped; lt.kill += o.killed;
-      ++lt.steps; lt.chords += o.chords;
-      atomicAdd(&tally.outcomes[o.outcome], 1ull);
-      tally.touched = 1;
-    }
-    const bool live = active && o.alive;
-    const uint32_t j = warp_append(&cnt->count[parity ^ 1][species], live);
-    if (live) {
-      if (j < c.capacity) store_track(slot.buf[parity ^ 1][species], j, o.post);
-      else cnt->overflow = 1;
-    }
-    Stream u;
-    u.init(in.event, c.seed, in.id, in.step);
-    append_secondaries(c, slot, parity, active, in.event, u, o, tally);
-    if (active && o.outcome == ADEPT_OUT_ESCAPED) { o.post.step = in.step + 1; record_leak(c, slot, o.post, species); }
-  }
-  flush_tally(tally, lt, slot, species);
+__device__ __forceinline__ Track make_secondary(const StepOut& o, int k, uint32_t event, const Stream& u) {
+  Track s;
+  s.x = o.post.x; s.y = o.post.y; s.z = o.post.z;
+  s.dx = o.sec[k].dx; s.dy = o.sec[k].dy; s.dz = o.sec[k].dz;
+  s.ekin = o.sec[k].ekin; s.id = u.child_id(o.sec[k].child); s.event = event; s.step = 0; s.vol = o.post.vol;
+  s.species = o.sec[k].species;
+  return s;
 }
 
 // ------------------------------------------------------------------------------------------------
-// Split mode: move kernels leave relocation and interactions to their own kernels.
-//   reloc_queue entry: species << 30 | index into the next buffer of that species
-//   inter_queue[q][k]: same encoding, q = 0 Compton, 1 pair, 2 photoelectric, 3 brems, 4 Moller, 5 annihilation, 6 Bhabha
-constexpr int kNumInterQueues = 7;
-
-__device__ __forceinline__ int inter_queue_index(int process, int species) {
-  return (process == ADEPT_OUT_IONI && species == ADEPT_POSITRON) ? 6 : process - 1;
+// Interaction staging queues: see kNumStage in types.cuh.
+__device__ __forceinline__ int stage_queue(int process, int species) {
+  if (species == ADEPT_GAMMA) return process - ADEPT_OUT_COMPTON;                       // 0, 1, 2
+  if (species == ADEPT_ELECTRON) return process == ADEPT_OUT_BREM ? 3 : 4;
+  return process == ADEPT_OUT_BREM ? 5 : (process == ADEPT_OUT_IONI ? 6 : 7);
 }
-__device__ __forceinline__ int inter_queue_process(int q) { return q == 6 ? ADEPT_OUT_IONI : q + 1; }
+__device__ __forceinline__ int stage_process(int q) {
+  constexpr int p[kNumStage] = {ADEPT_OUT_COMPTON, ADEPT_OUT_PAIR, ADEPT_OUT_PHOTO, ADEPT_OUT_BREM, ADEPT_OUT_IONI,
+                                ADEPT_OUT_BREM, ADEPT_OUT_IONI, ADEPT_OUT_ANNI};
+  return p[q];
+}
+__device__ __forceinline__ int stage_species(int q) { return q < 3 ? ADEPT_GAMMA : (q < 5 ? ADEPT_ELECTRON : ADEPT_POSITRON); }
 
+// ------------------------------------------------------------------------------------------------
+// Move kernel: one step of every track of a species up to (not including) its discrete interaction.
+// grid.y = species of a charged launch.  Survivors that do not interact go to the next buffer of their
+// species; survivors that interact are staged, whole record, in the queue of their process, so the
+// interaction kernel reads them coalesced; the photons of an e+ annihilating at rest go to the next
+// gamma buffer.
 template <int MODE, int FIELD, bool BVH>
-__global__ void __launch_bounds__(kBlock, MODE == MODE_GAMMA ? ADEPT_MINB_G : ADEPT_MINB_C) move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot,
-                                                      int parity) {
+__global__ void __launch_bounds__(kBlock, MODE == MODE_GAMMA ? ADEPT_MINB_G : ADEPT_MINB_C)
+move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot, int parity) {
   const int species = MODE == MODE_GAMMA ? ADEPT_GAMMA : static_cast<int>(blockIdx.y);
   const TrackSoA& cur = slot.buf[parity][species];
   SlotCounters* cnt = slot.counters;
-  const uint32_t n = cnt->count[parity][species];
+  const uint32_t n = cnt->count[parity][species].v;
 
+  // destinations of this kernel: 0 = next buffer of the species, 1..3 = its staging queues,
+  // 4 = next gamma buffer (at-rest annihilation photons, charged kernel only)
+  constexpr int ND = MODE == MODE_GAMMA ? 4 : 5;
+  const int q0 = species == ADEPT_GAMMA ? 0 : (species == ADEPT_ELECTRON ? 3 : 5);
   __shared__ BlockTally tally;
-  if (threadIdx.x == 0) tally = BlockTally{};
-  __syncthreads();
-  LaneTally lt;
+  __shared__ BlockReserve<ND> br;
+  tally_init(tally);
+  double sum_dep = 0.0, sum_cut = 0.0;
+  unsigned chords = 0;
+  int phase = 0;
+  const int lane = threadIdx.x & 31;
 
-  const uint32_t n_round = (n + 31u) & ~31u;
-  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += gridDim.x * blockDim.x) {
+  const uint32_t n_tiles = (n + kBlock - 1) / kBlock;
+  for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, phase ^= 1) {
+    const uint32_t i = tile * kBlock + threadIdx.x;
     bool active = i < n;
     Track in{};
     if (active) in = load_track(cur, i, species);
@@ -244,167 +217,165 @@ __global__ void __launch_bounds__(kBlock, MODE == MODE_GAMMA ? ADEPT_MINB_G : AD
 
     score(slot.edep, in.vol, o.edep_dep + o.edep_cut, active);
     if (active) {
-      lt.dep += o.edep_dep; lt.cut += o.edep_cut; lt.kill += o.killed;
-      ++lt.steps; lt.chords += o.chords;
-      if (next == NEXT_NONE) atomicAdd(&tally.outcomes[o.outcome], 1ull);
-      tally.touched = 1;
-    }
-    // One round of atomics reserves everything this warp appends: lane 0 the survivor slots, lane 1 the
-    // relocation-queue entries, lanes 2.. the entries of the process queues this kernel feeds.
-    const bool live = active && o.alive;
-    constexpr int kQ0 = MODE == MODE_GAMMA ? 0 : 3, kNQ = MODE == MODE_GAMMA ? 3 : 4;
-    const int q = (live && next == NEXT_INTERACT) ? inter_queue_index(process, species) - kQ0 : -1;
-    const int lane = threadIdx.x & 31;
-    const unsigned lt = (1u << lane) - 1u;
-    const unsigned m_live = __ballot_sync(kFull, live);
-    const unsigned m_rel = __ballot_sync(kFull, live && next == NEXT_RELOCATE);
-    unsigned m_q[kNQ];
-#pragma unroll
-    for (int qq = 0; qq < kNQ; ++qq) m_q[qq] = __ballot_sync(kFull, q == qq);
-    uint32_t mine = 0;
-    if (lane == 0) { if (m_live) mine = atomicAdd(&cnt->count[parity ^ 1][species], __popc(m_live)); }
-    else if (lane == 1) { if (m_rel) mine = atomicAdd(&cnt->n_reloc, __popc(m_rel)); }
-    else if (lane < 2 + kNQ) {
-      unsigned mq = 0;
-#pragma unroll
-      for (int qq = 0; qq < kNQ; ++qq) if (lane == 2 + qq) mq = m_q[qq];
-      if (mq) mine = atomicAdd(&cnt->n_inter[kQ0 + lane - 2], __popc(mq));
-    }
-    const uint32_t j = __shfl_sync(kFull, mine, 0) + __popc(m_live & lt);
-    const uint32_t k_rel = __shfl_sync(kFull, mine, 1) + __popc(m_rel & lt);
-    uint32_t k_q = 0;
-#pragma unroll
-    for (int qq = 0; qq < kNQ; ++qq) {
-      const uint32_t bq = __shfl_sync(kFull, mine, 2 + qq);
-      if (q == qq) k_q = bq + __popc(m_q[qq] & lt);
-    }
-    if (live) {
-      o.post.step = in.step + 1;
-      if (j < c.capacity) {
-        store_track(slot.buf[parity ^ 1][species], j, o.post);
-        const uint32_t entry = (static_cast<uint32_t>(species) << 30) | j;
-        if (next == NEXT_RELOCATE) slot.reloc_queue[k_rel] = entry;
-        else if (q >= 0) slot.inter_queue[static_cast<size_t>(kQ0 + q) * c.capacity + k_q] = entry;
-      } else {
-        cnt->overflow = 1;
+      sum_dep += o.edep_dep; sum_cut += o.edep_cut; chords += o.chords;
+      if (o.killed != 0.0) atomicAdd(&tally.ledger[3], o.killed);
+      if (next == NEXT_NONE && o.outcome == ADEPT_OUT_ESCAPED) {
+        atomicAdd(&tally.ledger[2], o.escaped);
+        o.post.step = in.step + 1;
+        record_leak(c, slot, o.post, species);
       }
     }
-    append_secondaries(c, slot, parity, active, in.event, u, o, tally);   // at-rest annihilation photons
-  }
-  flush_tally(tally, lt, slot, species);
-}
+    {
+      const unsigned ma = __ballot_sync(kFull, active);
+      if (lane == 0 && ma) atomicAdd(&tally.steps, static_cast<unsigned>(__popc(ma)));
+    }
+    const bool none = active && next == NEXT_NONE;
+    tally_outcome(tally, none, o.outcome, ADEPT_OUT_BOUNDARY);
+    tally_outcome(tally, none, o.outcome, ADEPT_OUT_ESCAPED);
+    tally_outcome(tally, none, o.outcome, ADEPT_OUT_STOPPED);
+    tally_outcome(tally, none, o.outcome, ADEPT_OUT_KILLED);
+    if (MODE != MODE_GAMMA) {
+      tally_outcome(tally, none, o.outcome, ADEPT_OUT_LOSS);
+      tally_outcome(tally, none, o.outcome, ADEPT_OUT_TRUNCATED);
+    }
 
-template <bool BVH>
-__global__ void __launch_bounds__(kBlock) relocate_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot,
-                                                          int parity) {
-  SlotCounters* cnt = slot.counters;
-  const uint32_t n = cnt->n_reloc;
-  __shared__ BlockTally tally;
-  if (threadIdx.x == 0) tally = BlockTally{};
-  __syncthreads();
-  LaneTally lt;
-  const uint32_t n_round = (n + 31u) & ~31u;
-  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += gridDim.x * blockDim.x) {
-    const bool active = i < n;
-    uint32_t entry = 0;
-    if (active) entry = slot.reloc_queue[i];
-    const int species = entry >> 30;
-    const uint32_t j = entry & 0x3fffffffu;
-    const TrackSoA& b = slot.buf[parity ^ 1][species];
-    double x = 0.0, y = 0.0, z = 0.0;
-    if (active) { x = b.x[j]; y = b.y[j]; z = b.z[j]; }
-    const int nv = nav_locate<BVH>(c, c.navigator, active, x, y, z);
-    if (!active) continue;
-    tally.touched = 1;
-    if (nv >= 0) {
-      b.vol[j] = static_cast<uint32_t>(nv);
-      atomicAdd(&tally.outcomes[ADEPT_OUT_BOUNDARY], 1ull);
-    } else {
-      Track t = load_track(b, j, species);
-      b.vol[j] = kDeadVolume;
-      lt.esc += carried_energy(species, t.ekin);
-      record_leak(c, slot, t, species);
-      atomicAdd(&tally.outcomes[ADEPT_OUT_ESCAPED], 1ull);
+    const bool live = active && o.alive;
+    const int dest = !live ? -1 : (next == NEXT_INTERACT ? 1 + stage_queue(process, species) - q0 : 0);
+    uint32_t want[ND], first[ND];
+#pragma unroll
+    for (int d = 0; d < 4; ++d) want[d] = dest == d ? 1u : 0u;
+    if (MODE != MODE_GAMMA) want[4] = active ? static_cast<uint32_t>(o.n_sec) : 0u;
+    block_reserve<ND>(br, phase, want, first, [&](int d) -> uint32_t* {
+      if (d == 0) return &cnt->count[parity ^ 1][species].v;
+      if (d == 4) return &cnt->count[parity ^ 1][ADEPT_GAMMA].v;
+      return &cnt->n_stage[q0 + d - 1].v;
+    });
+    if (live) {
+      o.post.step = in.step + 1;
+      uint32_t j = first[0];
+      bool ok = j < c.capacity;
+      const TrackSoA* dst = &slot.buf[parity ^ 1][species];
+#pragma unroll
+      for (int d = 1; d < 4; ++d)
+        if (dest == d) { j = first[d]; ok = j < c.stage_capacity; dst = &slot.stage[q0 + d - 1]; }
+      if (ok) store_track(*dst, j, o.post);
+      else cnt->overflow.v = 1;
+    }
+    if (MODE != MODE_GAMMA) {
+      if (active && o.n_sec > 0) {  // at-rest annihilation photons
+        for (int k = 0; k < o.n_sec; ++k) {
+          const uint32_t j = first[4] + k;
+          if (j < c.capacity) store_track(slot.buf[parity ^ 1][ADEPT_GAMMA], j, make_secondary(o, k, in.event, u));
+          else cnt->overflow.v = 1;
+        }
+      }
+      const unsigned ns = __reduce_add_sync(kFull, want[4]);
+      if (lane == 0 && ns) atomicAdd(&tally.secondaries[ADEPT_GAMMA], ns);
     }
   }
   {
-    const int lane = threadIdx.x & 31;
-    const double esc = warp_sum(lt.esc);
-    if (lane == 0 && esc != 0.0) atomicAdd(&tally.ledger[2], esc);
-    __syncthreads();
-    if (threadIdx.x == 0 && tally.touched) {
-      if (tally.ledger[2] != 0.0) atomicAdd(slot.ledger + 2, tally.ledger[2]);
-      if (tally.outcomes[ADEPT_OUT_BOUNDARY]) atomicAdd(&slot.stats->outcomes[ADEPT_OUT_BOUNDARY], tally.outcomes[ADEPT_OUT_BOUNDARY]);
-      if (tally.outcomes[ADEPT_OUT_ESCAPED]) atomicAdd(&slot.stats->outcomes[ADEPT_OUT_ESCAPED], tally.outcomes[ADEPT_OUT_ESCAPED]);
-    }
+    const unsigned long long ch = __reduce_add_sync(kFull, chords);
+    if (lane == 0 && ch) atomicAdd(&tally.chords, ch);
   }
+  tally_flush(tally, slot, species, sum_dep, sum_cut);
 }
 
-// Every warp works on one process queue at a time, so the rejection loops of different processes never
-// share a warp (PAPER.md:101 names divergence between processes as a main cost).
-__global__ void __launch_bounds__(kBlock, ADEPT_MINB_I) interact_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot,
-                                                          int parity) {
+// ------------------------------------------------------------------------------------------------
+// Interaction kernel: a tile is kBlock staged tracks of ONE queue, so a whole block runs the rejection
+// loop of one process (PAPER.md:101 names divergence between processes as a main cost).  The updated
+// parent and the secondaries are appended to the next buffers.
+__global__ void __launch_bounds__(kBlock, ADEPT_MINB_I)
+interact_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot, int parity) {
   SlotCounters* cnt = slot.counters;
   __shared__ BlockTally tally;
-  __shared__ uint32_t warp_begin[kNumInterQueues + 1];   // prefix of 32-lane groups per queue
+  __shared__ BlockReserve<3> br;
+  __shared__ uint32_t tile_begin[kNumStage + 1];   // prefix of tiles per queue
+  __shared__ uint32_t n_staged[kNumStage];
   if (threadIdx.x == 0) {
-    tally = BlockTally{};
     uint32_t acc = 0;
-    for (int q = 0; q < kNumInterQueues; ++q) { warp_begin[q] = acc; acc += (cnt->n_inter[q] + 31u) >> 5; }
-    warp_begin[kNumInterQueues] = acc;
+    for (int q = 0; q < kNumStage; ++q) {
+      const uint32_t nq = min(cnt->n_stage[q].v, c.stage_capacity);
+      n_staged[q] = nq;
+      tile_begin[q] = acc;
+      acc += (nq + kBlock - 1) / kBlock;
+    }
+    tile_begin[kNumStage] = acc;
   }
-  __syncthreads();
-  LaneTally lt;
+  tally_init(tally);
+  double sum_cut = 0.0;
+  int phase = 0;
   const int lane = threadIdx.x & 31;
-  const uint32_t warps_per_grid = gridDim.x * (blockDim.x >> 5);
-  const uint32_t total = warp_begin[kNumInterQueues];
-  for (uint32_t w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); w < total; w += warps_per_grid) {
+  const uint32_t total = tile_begin[kNumStage];
+  for (uint32_t tile = blockIdx.x; tile < total; tile += gridDim.x, phase ^= 1) {
     int q = 0;
-    while (w >= warp_begin[q + 1]) ++q;
-    const uint32_t i = ((w - warp_begin[q]) << 5) + lane;
-    const bool active = i < cnt->n_inter[q];
+    while (tile >= tile_begin[q + 1]) ++q;
+    const uint32_t i = (tile - tile_begin[q]) * kBlock + threadIdx.x;
+    const bool active = i < n_staged[q];
+    const int species = stage_species(q);
     StepOut o;
     Stream u;
     Track t{};
-    uint32_t j = 0;
-    int species = 0;
     if (active) {
-      const uint32_t entry = slot.inter_queue[static_cast<size_t>(q) * c.capacity + i];
-      species = entry >> 30;
-      j = entry & 0x3fffffffu;
-      t = load_track(slot.buf[parity ^ 1][species], j, species);
+      t = load_track(slot.stage[q], i, species);
       init_out(o, t, true);
       u.init(t.event, c.seed, t.id, t.step - 1);          // the stream of the step that chose the process
       const int mat = volume(c, t.vol).material;
-      run_process(c, inter_queue_process(q), species, mat, o, u);
-      const TrackSoA& b = slot.buf[parity ^ 1][species];
-      if (o.alive) { b.dx[j] = o.post.dx; b.dy[j] = o.post.dy; b.dz[j] = o.post.dz; b.ekin[j] = o.post.ekin; }
-      else b.vol[j] = kDeadVolume;
-      lt.cut += o.edep_cut;
-      atomicAdd(&tally.outcomes[o.outcome], 1ull);
-      tally.touched = 1;
+      run_process(c, stage_process(q), species, mat, o, u);
+      sum_cut += o.edep_cut;
     } else {
       init_out(o, t, false);
       u.init(0, 0, 0, 0);
     }
     score(slot.edep, t.vol, o.edep_cut, active);
-    append_secondaries(c, slot, parity, active, t.event, u, o, tally);
+#pragma unroll
+    for (int w = ADEPT_OUT_COMPTON; w <= ADEPT_OUT_ANNI; ++w) tally_outcome(tally, active, o.outcome, w);
+    tally_outcome(tally, active, o.outcome, ADEPT_OUT_CLOSED);
+
+    const int s0 = (active && o.n_sec > 0) ? o.sec[0].species : -1;
+    const int s1 = (active && o.n_sec > 1) ? o.sec[1].species : -1;
+    const bool live = active && o.alive;
+    uint32_t want[3], first[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      want[d] = (live && species == d ? 1u : 0u) + (s0 == d ? 1u : 0u) + (s1 == d ? 1u : 0u);
+      const unsigned m = __ballot_sync(kFull, s0 == d), m1 = __ballot_sync(kFull, s1 == d);
+      if (lane == 0 && (m | m1)) atomicAdd(&tally.secondaries[d], static_cast<unsigned>(__popc(m) + __popc(m1)));
+    }
+    block_reserve<3>(br, phase, want, first, [&](int d) -> uint32_t* { return &cnt->count[parity ^ 1][d].v; });
+    // within a destination the lane's entries are ordered: surviving parent, secondary 0, secondary 1
+    const auto sel = [&](int d) { return d == 0 ? first[0] : (d == 1 ? first[1] : first[2]); };
+    if (live) {
+      const uint32_t j = sel(species);
+      if (j < c.capacity) store_track(slot.buf[parity ^ 1][species], j, o.post);
+      else cnt->overflow.v = 1;
+    }
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      const int ss = k == 0 ? s0 : s1;
+      if (ss < 0) continue;
+      const uint32_t j = sel(ss) + ((live && species == ss) ? 1u : 0u) + ((k == 1 && s0 == ss) ? 1u : 0u);
+      if (j < c.capacity) store_track(slot.buf[parity ^ 1][ss], j, make_secondary(o, k, t.event, u));
+      else cnt->overflow.v = 1;
+    }
   }
-  flush_tally(tally, lt, slot, 0);
+  tally_flush(tally, slot, 0, 0.0, sum_cut);
 }
 
 // End of one population step: the just-consumed buffers become the next step's output buffers.
 __global__ void finish_iteration_kernel(const __grid_constant__ DevSlot slot, int parity) {
   SlotCounters* cnt = slot.counters;
-  const uint32_t before = cnt->count[parity][0] + cnt->count[parity][1] + cnt->count[parity][2];
-  cnt->count[parity][0] = cnt->count[parity][1] = cnt->count[parity][2] = 0;
-  const uint32_t live = cnt->count[parity ^ 1][0] + cnt->count[parity ^ 1][1] + cnt->count[parity ^ 1][2];
-  cnt->live = live;
-  cnt->n_reloc = 0;
-  for (int q = 0; q < 8; ++q) cnt->n_inter[q] = 0;
-  if (before) {
-    slot.stats->iterations += 1;
-    if (before > slot.stats->peak_population) slot.stats->peak_population = before;
+  const int k = threadIdx.x;
+  uint32_t before = 0, live = 0;
+  for (int sp = 0; sp < 3; ++sp) { before += cnt->count[parity][sp].v; live += cnt->count[parity ^ 1][sp].v; }
+  __syncthreads();
+  if (k < 3) cnt->count[parity][k].v = 0;
+  else if (k < 3 + kNumStage) cnt->n_stage[k - 3].v = 0;
+  else if (k == 3 + kNumStage) {
+    cnt->live.v = live;
+    if (before) {
+      slot.stats->iterations += 1;
+      if (before > slot.stats->peak_population) slot.stats->peak_population = before;
+    }
   }
 }
 
@@ -420,14 +391,14 @@ __global__ void __launch_bounds__(kBlock) enqueue_kernel(const __grid_constant__
                              p.pos[2] + c.eps_push * p.dir[2]);
     if (active && (v < 0 || p.species < 0 || p.species > 2)) { atomicAdd(bad, 1u); continue; }
     if (!active) continue;
-    const uint32_t j = atomicAdd(&slot.counters->count[0][p.species], 1u);
-    if (j >= c.capacity) { slot.counters->overflow = 1; continue; }
+    const uint32_t j = atomicAdd(&slot.counters->count[0][p.species].v, 1u);
+    if (j >= c.capacity) { slot.counters->overflow.v = 1; continue; }
     Track t;
     t.x = p.pos[0]; t.y = p.pos[1]; t.z = p.pos[2]; t.dx = p.dir[0]; t.dy = p.dir[1]; t.dz = p.dir[2];
     t.ekin = p.ekin; t.id = p.id; t.event = p.event; t.step = 0; t.vol = static_cast<uint32_t>(v); t.species = p.species;
     store_track(slot.buf[0][p.species], j, t);
     atomicAdd(slot.ledger + 4, carried_energy(p.species, p.ekin));
-    atomicAdd(&slot.counters->live, 1u);
+    atomicAdd(&slot.counters->live.v, 1u);
   }
 }
 
@@ -489,6 +460,18 @@ __global__ void __launch_bounds__(kBlock) locate_kernel(const __grid_constant__ 
     const bool a = i < n;
     const int k = a ? i : 0;
     const int r = nav_locate(c, nav, a, pos[3 * k], pos[3 * k + 1], pos[3 * k + 2]);
+    if (a) out[i] = r;
+  }
+}
+
+// Test hook for A5: relocation of point i starting from volume from[i] (any volume of the tree).
+__global__ void __launch_bounds__(kBlock) relocate_kernel(const __grid_constant__ DevCtx c, int nav, int n, const double* pos,
+                                                          const uint32_t* from, long long* out) {
+  const int n_round = (n + 31) & ~31;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += gridDim.x * blockDim.x) {
+    const bool a = i < n;
+    const int k = a ? i : 0;
+    const int r = nav_relocate(c, nav, a, from[k], pos[3 * k], pos[3 * k + 1], pos[3 * k + 2]);
     if (a) out[i] = r;
   }
 }

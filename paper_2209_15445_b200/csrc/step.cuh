@@ -1,11 +1,11 @@
-// One transport step of one track per lane  (rows A2-A8), in three phases that
-// the kernels either chain (frozen-step hook, fused mode) or run as separate kernels with work queues
-// in between (split mode, "a separate kernel ... to improve load balancing"):
-//   move      step-start rules, physics step limit, propagation, continuous loss, MSC, process choice
-//   relocate  push past the boundary and Locate (A5)
+// One transport step of one track per lane  (rows A2-A8), in two phases that the
+// frozen-step hook chains and the transport kernels run as separate kernels with per-process staging
+// queues in between:
+//   move      step-start rules, physics step limit, propagation, continuous loss, MSC, push past the
+//             boundary + relocation (A5), process choice
 //   interact  sample the discrete process, create secondaries (A8)
-// move and relocate are warp-convergent: every lane of the warp must call them (inactive lanes pass
-// active = false) because propagation and Locate use the warp-cooperative navigator.
+// move is warp-convergent: every lane of the warp must call it (inactive lanes pass active = false)
+// because propagation and relocation use the warp-cooperative navigator.
 #pragma once
 #include "field.cuh"
 #include "physics.cuh"
@@ -15,7 +15,7 @@ namespace adept {
 enum { MODE_ANY = 0, MODE_GAMMA = 1, MODE_CHARGED = 2 };
 
 // what the move phase leaves to do
-enum { NEXT_NONE = 0, NEXT_RELOCATE = 1, NEXT_INTERACT = 2 };
+enum { NEXT_NONE = 0, NEXT_INTERACT = 2 };
 
 __device__ __forceinline__ double carried_energy(int species, double ekin) {
   return species == ADEPT_POSITRON ? ekin + 2.0 * kMe : ekin;
@@ -30,9 +30,9 @@ __device__ __forceinline__ void init_out(StepOut& o, const Track& in, bool activ
   o.sec[0].species = -1; o.sec[1].species = -1;
 }
 
-// Phase 1.  On return o.post holds the moved state (position already pushed past the boundary when
-// the result is NEXT_RELOCATE), `process` the chosen discrete process for NEXT_INTERACT, and `mat`
-// the material of the pre-step volume.  o.post.step is NOT yet incremented.
+// Phase 1.  On return o.post holds the moved (and, after a boundary, relocated) state, `process` the
+// chosen discrete process for NEXT_INTERACT, and `mat` the material of the pre-step volume.
+// o.post.step is NOT yet incremented.
 template <int MODE, int FIELD = -1, bool BVH = true>
 __device__ int step_move(const DevCtx& c, int nav, bool active, const Track& in, StepOut& o, Stream& u, int& process,
                          int& mat) {
@@ -103,11 +103,11 @@ __device__ int step_move(const DevCtx& c, int nav, bool active, const Track& in,
   int chords = 0;
   const int charge = is_gamma ? 0 : (positron ? +1 : -1);
   const int flag = propagate<FIELD, BVH>(c, nav, go, charge, T0, pos, dir, in.vol, s_phys, s, chords, pushdir);
-  if (!go) return NEXT_NONE;
 
   // ---- along-step actions (A7)
   o.s = s; o.chords = chords;
-  if (!is_gamma) {
+  bool cross = go && flag == 1;
+  if (go && !is_gamma) {
     double dE = 0.0;
     if (!vacuum) {
       if (flag == 0 && !lim_disc && range_out) dE = T0;
@@ -123,9 +123,9 @@ __device__ int step_move(const DevCtx& c, int nav, bool active, const Track& in,
       o.post.dx = dir[0]; o.post.dy = dir[1]; o.post.dz = dir[2];
       if (positron) annihilation_at_rest(c, mat, o, u);
       o.alive = 0; o.outcome = ADEPT_OUT_STOPPED;
-      return NEXT_NONE;
+      go = false; cross = false;
     }
-    if (!vacuum && s > 0.0) {  // P9 Highland MSC at the pre-step energy
+    if (go && !vacuum && s > 0.0) {  // P9 Highland MSC at the pre-step energy
       const double X0 = mat_scalar(c, mat, S_X0);
       const double pbeta = T0 * (T0 + 2.0 * kMe) / (T0 + kMe);
       const double beta2 = T0 * (T0 + 2.0 * kMe) / ((T0 + kMe) * (T0 + kMe));
@@ -139,14 +139,24 @@ __device__ int step_move(const DevCtx& c, int nav, bool active, const Track& in,
       dir[0] = dn[0]; dir[1] = dn[1]; dir[2] = dn[2];
     }
   }
-  o.post.dx = dir[0]; o.post.dy = dir[1]; o.post.dz = dir[2];
-  if (flag == 1) {  // G5: push past the boundary; the new volume is found by the relocate phase
-    o.post.x = pos[0] + c.eps_push * pushdir[0];
-    o.post.y = pos[1] + c.eps_push * pushdir[1];
-    o.post.z = pos[2] + c.eps_push * pushdir[2];
-    return NEXT_RELOCATE;
+  if (go) {
+    o.post.dx = dir[0]; o.post.dy = dir[1]; o.post.dz = dir[2];
+    if (cross) {  // G5: push past the boundary
+      pos[0] += c.eps_push * pushdir[0]; pos[1] += c.eps_push * pushdir[1]; pos[2] += c.eps_push * pushdir[2];
+    }
+    o.post.x = pos[0]; o.post.y = pos[1]; o.post.z = pos[2];
   }
-  o.post.x = pos[0]; o.post.y = pos[1]; o.post.z = pos[2];
+  // ---- relocation (A5), warp-convergent
+  const int nv = nav_relocate<BVH>(c, nav, cross, in.vol, pos[0], pos[1], pos[2]);
+  if (!go) return NEXT_NONE;
+  if (cross) {
+    if (nv < 0) {
+      o.escaped += carried_energy(in.species, o.post.ekin); o.alive = 0; o.outcome = ADEPT_OUT_ESCAPED;
+    } else {
+      o.post.vol = static_cast<uint32_t>(nv); o.outcome = ADEPT_OUT_BOUNDARY;
+    }
+    return NEXT_NONE;
+  }
   if (flag == 2) { o.outcome = ADEPT_OUT_TRUNCATED; return NEXT_NONE; }
   if (!is_gamma && !lim_disc) { o.outcome = ADEPT_OUT_LOSS; return NEXT_NONE; }
   // ---- choice of the discrete process (U1)
@@ -164,26 +174,12 @@ __device__ int step_move(const DevCtx& c, int nav, bool active, const Track& in,
   return NEXT_INTERACT;
 }
 
-// Phase 2 (A5).  `cross` lanes hold the pushed position in o.post; the others idle.  Warp-convergent.
-template <bool BVH = true>
-__device__ __forceinline__ void step_relocate(const DevCtx& c, int nav, bool cross, int species, StepOut& o) {
-  const int nv = nav_locate<BVH>(c, nav, cross, o.post.x, o.post.y, o.post.z);
-  if (cross) {
-    if (nv < 0) {
-      o.escaped += carried_energy(species, o.post.ekin); o.alive = 0; o.outcome = ADEPT_OUT_ESCAPED;
-    } else {
-      o.post.vol = static_cast<uint32_t>(nv); o.outcome = ADEPT_OUT_BOUNDARY;
-    }
-  }
-}
-
-// The whole step in one call (frozen-step hook and fused kernels).
+// The whole step in one call (frozen-step hook).
 template <int MODE>
 __device__ void step_track(const DevCtx& c, int nav, bool active, const Track& in, StepOut& o) {
   Stream u;
   int process, mat;
   const int next = step_move<MODE>(c, nav, active, in, o, u, process, mat);
-  step_relocate(c, nav, next == NEXT_RELOCATE, in.species, o);
   if (next == NEXT_INTERACT) run_process(c, process, in.species, mat, o, u);
   if (o.alive) o.post.step = in.step + 1;
 }

@@ -26,16 +26,19 @@ enum { S_X0, S_TCUT, S_KCUT, S_BK, S_NEL, S_VACUUM, S_Z, S_RHO, N_SCAL };
 //   positron row = {brem, Bhabha, annihilation, dE/dx, range, pad, pad, pad} 64 B
 constexpr int kRowG = 4, kRowEm = 4, kRowEp = 8;
 
+// Hot part of a touchable (80 B); the 3x3 rotation lives in DevCtx::rot and is only read for rotated
+// placements, so the 152 volumes of the calorimeter stay L1-resident (12 KB).
 struct __align__(16) DevVolume {
   double t[3];
   double dims[3];
-  double R[9];
   int32_t solid;
   int32_t material;
   int32_t dbegin;
   int32_t dcount;
   int32_t bvh;       // index into DevCtx::bvh, -1 = none (loop over daughters)
-  int32_t identity;  // 1 if R is the identity (transform reduces to a subtraction, bit-identical)
+  int32_t identity;  // 1 if the rotation is the identity (transform reduces to a subtraction, bit-identical)
+  int32_t mother;    // -1 for the world
+  int32_t pad;
 };
 
 // Implicit complete 32-ary BVH over the daughters of one volume, in the world frame.
@@ -58,14 +61,23 @@ struct TrackSoA {
   uint32_t *event, *step, *vol;
 };
 
+// Interaction staging queues (one per process and species, so a queue is species-uniform):
+//   0 Compton, 1 pair, 2 photoelectric (gamma); 3 brems, 4 Moller (e-); 5 brems, 6 Bhabha, 7 annihilation (e+)
+constexpr int kNumStage = 8;
+
+// Every hot counter sits in its own 128 B line: appends to different queues never serialise on one
+// L2 atomic unit (measured: with all counters in one line the append atomics were 24 % of the stall
+// samples of the gamma move kernel, profiles/r1_summary.md).
+struct alignas(128) PaddedCounter {
+  uint32_t v;
+  uint32_t pad[31];
+};
 struct SlotCounters {
-  uint32_t count[2][3];     // [buffer parity][species] live entries
-  uint32_t n_reloc;         // relocation work queue (split mode)
-  uint32_t n_inter[8];      // interaction work queues, one per process (split mode)
-  uint32_t overflow;        // set when any queue overflowed
-  uint32_t n_leaked;
-  uint32_t live;            // population after the last finished iteration
-  uint32_t pad[2];
+  PaddedCounter count[2][3];        // [buffer parity][species] live entries
+  PaddedCounter n_stage[kNumStage]; // staged tracks per interaction queue
+  PaddedCounter n_leaked;
+  PaddedCounter overflow;           // set when any queue overflowed
+  PaddedCounter live;               // population after the last finished iteration
 };
 
 struct DevStats {
@@ -84,12 +96,12 @@ struct DevSlot {
   double* ledger;           // [5]: deposited, below_cut, escaped, killed, primary
   DevStats* stats;
   adept_track* leaked;      // [leak_capacity]
-  uint32_t* reloc_queue;    // split mode: species<<30 | index into the next buffer
-  uint32_t* inter_queue;    // split mode: process<<28 | species<<26 | index
+  TrackSoA stage[kNumStage];  // tracks waiting for their discrete interaction (stage_capacity entries each)
 };
 
 struct DevCtx {
   const DevVolume* vol;
+  const double* rot;        // [n_vol][9]
   int32_t n_vol;
   const DevBvh* bvh;
   int32_t navigator;
@@ -108,6 +120,7 @@ struct DevCtx {
   int32_t chord_budget;
   uint32_t seed, max_steps;
   uint32_t capacity;        // per species per buffer
+  uint32_t stage_capacity;  // per interaction queue
   uint32_t leak_capacity;
 };
 

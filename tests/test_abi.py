@@ -29,7 +29,19 @@ def test_library_exports_every_declared_symbol():
 
 def test_binding_structs_match_the_header_layout():
     from paper_2209_15445_b200 import adept
-    assert C.sizeof(adept.CConfig) == 80 and C.sizeof(adept.CStats) == 184 and C.sizeof(adept.CLedger) == 40
+    # sizes as a C compiler sees include/adept.h
+    import subprocess
+    import tempfile
+    with tempfile.TemporaryDirectory() as tmp:
+        src = os.path.join(tmp, "sz.c")
+        open(src, "w").write('#include <stdio.h>\n#include "adept.h"\nint main(void){printf("%zu %zu %zu %zu %zu %zu %zu\\n",'
+                             'sizeof(adept_config),sizeof(adept_stats),sizeof(adept_ledger),sizeof(adept_track),'
+                             'sizeof(adept_step_result),sizeof(adept_geometry),sizeof(adept_field));return 0;}\n')
+        subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), "-o", os.path.join(tmp, "sz"), src])
+        sizes = [int(x) for x in subprocess.check_output([os.path.join(tmp, "sz")]).split()]
+    assert sizes == [C.sizeof(adept.CConfig), C.sizeof(adept.CStats), C.sizeof(adept.CLedger), adept.TRACK.itemsize,
+                     adept.RESULT.itemsize, C.sizeof(adept.CGeometry), C.sizeof(adept.CField)]
+    assert C.sizeof(adept.CConfig) == 88 and C.sizeof(adept.CStats) == 184 and C.sizeof(adept.CLedger) == 40
     assert adept.TRACK.itemsize == 80 and adept.RESULT.itemsize == 136
     cfg = adept.default_config()
     assert cfg.delta_chord == 1e-3 and cfg.eps_push == 1e-7 and cfg.chord_budget == 16 and cfg.navigator == adept.NAV_BVH

@@ -67,3 +67,43 @@ def test_navigation_matches_oracle(ob, barrel_patch, calo):
     ws = np.array([o.distance(pos[i], d[i], int(vol[i])) for i in range(2000)])
     np.testing.assert_allclose(s, ws, rtol=0, atol=1e-12 * 60.0)
     a.close()
+
+
+@pytest.mark.parametrize("navigator", [1, 0])
+def test_relocation_from_any_volume_equals_locate(ob, barrel_full, calo, navigator):
+    """A5: the move kernel relocates locally (climb from the old volume, then descend, neighbours of the
+    daughter just left first).  Whatever volume the climb starts from, the answer must be Locate(q) from
+    the world down, which is the oracle's only relocation routine."""
+    from paper_2209_15445_b200 import adept
+    from paper_2209_15445_b200.inputs import field
+    rng = np.random.default_rng(7)
+    # calorimeter: points anywhere in the world, starts in every kind of volume (world, box, layer, slab)
+    g, _, tabs, scal = calo
+    o = ob.Oracle(g, tabs, scal, field.no_field())
+    a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=1 << 10, navigator=navigator)
+    n = 4099
+    pos = np.stack([rng.uniform(-21, 61, n), rng.uniform(-31, 31, n), rng.uniform(-31, 31, n)], axis=1)
+    # half the points sit a push (1e-7 cm) past a slab face, where real relocations happen
+    k = rng.integers(0, 50, n // 2)
+    pos[: n // 2, 0] = 0.8 * k + rng.choice([0.0, 0.23], n // 2) + rng.choice([-1e-7, 1e-7], n // 2)
+    pos[: n // 2, 1:] = rng.uniform(-19.9, 19.9, (n // 2, 2))
+    frm = rng.integers(0, g.n_volumes, n)
+    want = a.locate_batch(pos, navigator)
+    assert np.array_equal(want[:600], np.array([o.locate(p) for p in pos[:600]]))
+    assert np.array_equal(a.relocate_batch(pos, frm, navigator), want)
+    # neighbouring start volumes (the common case): slab of the previous / next layer
+    near = np.clip(want + rng.choice([-2, -1, 1, 2], n), 52, g.n_volumes - 1)
+    assert np.array_equal(a.relocate_batch(pos, near, navigator), want)
+    assert (want < 0).sum() > 10 and (want >= 52).sum() > 1000
+    a.close()
+    # barrel: crystals (BVH mother), gaps, shells, outside
+    g, _, tabs, scal = barrel_full
+    a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=1 << 10, navigator=navigator)
+    n = 3001 if navigator == 1 else 257
+    pos, _ = _rays(rng, n, 0.0, 305.0, 2 * np.pi, 305.0)
+    pos[: n // 2], _ = _rays(rng, n // 2, 127.6, 152.9, 2 * np.pi, 289.0)
+    frm = rng.integers(0, g.n_volumes, n)
+    want = a.locate_batch(pos, navigator)
+    assert np.array_equal(a.relocate_batch(pos, frm, navigator), want)
+    assert np.array_equal(a.relocate_batch(pos, np.maximum(want, 0), navigator), want)
+    a.close()

@@ -27,8 +27,8 @@ def _check_layers(gpu_mean, o_mean, o_err):
     assert not bad.any(), (np.where(bad)[0], gpu_mean[bad], o_mean[bad], tol[bad])
 
 
-@pytest.mark.parametrize("split", [1, 0])
-def test_config1_calorimeter_256_electrons(ob, calo, split):
+@pytest.mark.parametrize("sync_interval", [8, 1])
+def test_config1_calorimeter_256_electrons(ob, calo, sync_interval):
     """BASELINE.json:configs[0]: 256 e- at 1 GeV, seed 1, edep per layer; one slot per group of events so the
     per-event ledgers are checked too."""
     import torch
@@ -40,7 +40,8 @@ def test_config1_calorimeter_256_electrons(ob, calo, split):
     tr = o.make_tracks(prim)
     o_ev, o_led = _oracle_events(o, tr, g.n_volumes)
     o_mean, o_err = layer_stats(o_ev)
-    a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=1 << 18, n_event_slots=2, split_kernels=split)
+    a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=1 << 18, n_event_slots=2, sync_interval=sync_interval,
+                    stage_capacity=(1 << 17 if sync_interval == 1 else 0))
     # slot 0: all 256 events in one population; slot 1: single events, ledger per event
     a.enqueue(prim, slot=0)
     a.transport(0, torch.cuda.current_stream())
@@ -91,8 +92,8 @@ def test_config3_uniform_field(ob, calo, species):
     assert st.chords > 0
 
 
-@pytest.mark.parametrize("split", [1, 0])
-def test_config5_concurrent_events_on_streams(ob, barrel_patch, split):
+@pytest.mark.parametrize("navigator", [1, 0])
+def test_config5_concurrent_events_on_streams(ob, barrel_patch, navigator):
     """BASELINE.json:configs[4] on the crystal patch: 16 events on 16 CUDA streams, per-event per-volume hits
     copied back to the host and checked against the oracle event by event."""
     import torch
@@ -109,7 +110,7 @@ def test_config5_concurrent_events_on_streams(ob, barrel_patch, split):
     o = ob.Oracle(g, tabs, scal, fld)
     tr = o.make_tracks(prim)
     o_ev, o_led = _oracle_events(o, tr, g.n_volumes)
-    a = adept.Adept(g, tabs, scal, fld, track_capacity=1 << 16, n_event_slots=n_ev, sync_interval=4, split_kernels=split)
+    a = adept.Adept(g, tabs, scal, fld, track_capacity=1 << 16, n_event_slots=n_ev, sync_interval=4, navigator=navigator)
     streams = [torch.cuda.Stream() for _ in range(n_ev)]
     for e in range(n_ev):
         sel = prim["event"] == e
