@@ -41,6 +41,8 @@ def parse():
     ap.add_argument("--capacity", type=int, default=0, help="track capacity per species (0 = auto)")
     ap.add_argument("--sync-interval", type=int, default=8)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-kernel-timing", action="store_true",
+                    help="experiments only: no per-kernel CUDA events (the roofline object is then empty)")
     ap.add_argument("--profile", action="store_true",
                     help="for runs under ncu: take --warmup literally (the timed numbers of such a run are not bench values)")
     ap.add_argument("--cpu-events-per-core", type=int, default=96)
@@ -186,7 +188,7 @@ def run_ours(args):
     g, tabs, scal, fld, prim = workload(args, first_event=shard_first_event(rank, args.events))
     cap = args.capacity or max(1 << 20, 1024 * args.events)
     a = adept.Adept(g, tabs, scal, fld, device=str(dev), track_capacity=cap, sync_interval=args.sync_interval,
-                    time_kernels=1)
+                    time_kernels=0 if args.no_kernel_timing else 1)
     stream = torch.cuda.Stream(device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
     edep_host = np.zeros(g.n_volumes)
@@ -217,7 +219,8 @@ def run_ours(args):
     n_warm = args.warmup if args.profile else max(args.warmup, 3)
     for _ in range(n_warm):
         one_pass(False)
-    a.kernel_times(0)
+    if not args.no_kernel_timing:
+        a.kernel_times(0)
     st0 = a.stats(0)
     steps0, sec0, launches0 = sum(st0.steps), sum(st0.secondaries), st0.launches
     gsteps0, gsec0 = st0.steps[2], 0
@@ -237,7 +240,7 @@ def run_ours(args):
     clk = clocks.stop() if rank == 0 else None
 
     st = a.stats(0)
-    kms, kn = a.kernel_times(0)
+    kms, kn = a.kernel_times(0) if not args.no_kernel_timing else (np.zeros(3), np.zeros(3))
     steps = sum(st.steps) - steps0
     n_sec = sum(st.secondaries) - sec0
     launches = st.launches - launches0 + args.steps        # + one enqueue kernel per pass

@@ -209,7 +209,7 @@ int validate(const adept_config* cfg, const adept_geometry* g, int n_mats, const
 }
 
 struct Layout {
-  DevVolume* vol; double* rot; DevBvh* bvh; double *tab_g, *tab_em, *tab_ep, *scal, *bz;
+  DevVolume* vol; double* rot; int32_t* rhint; DevBvh* bvh; double *tab_g, *tab_em, *tab_ep, *scal, *bz;
   std::vector<double*> bvh_prim_box; std::vector<int32_t*> bvh_prim_vol; std::vector<std::vector<double*>> bvh_node_box;
   adept_track* stage; uint32_t* bad; size_t stage_cap;
   std::vector<DevSlot> slots;
@@ -239,6 +239,7 @@ size_t carve(void* base, const adept_config* cfg, const adept_geometry* g, int n
   L.tab_em = cv.take<double>(static_cast<size_t>(n_mats) * kNGrid * kRowEm);
   L.tab_ep = cv.take<double>(static_cast<size_t>(n_mats) * kNGrid * kRowEp);
   L.scal = cv.take<double>(static_cast<size_t>(n_mats) * N_SCAL);
+  L.rhint = cv.take<int32_t>(static_cast<size_t>(n_mats) * 2 * kHintStride);
   L.bz = cv.take<double>(f->kind == ADEPT_FIELD_MAP_RZ ? static_cast<size_t>(f->nr) * f->nz : 1);
   L.stage_cap = std::min<size_t>(cfg->track_capacity, 1u << 20);
   L.stage = cv.take<adept_track>(L.stage_cap);
@@ -338,6 +339,26 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
     CUDA_TRY(cudaMemcpy(L.tab_g, tg.data(), tg.size() * sizeof(double), cudaMemcpyHostToDevice));
     CUDA_TRY(cudaMemcpy(L.tab_em, te.data(), te.size() * sizeof(double), cudaMemcpyHostToDevice));
     CUDA_TRY(cudaMemcpy(L.tab_ep, tp.data(), tp.size() * sizeof(double), cudaMemcpyHostToDevice));
+    // inverse-range search hints (physics.cuh inverse_range): for key cell k, the largest node j whose
+    // range R_j does not exceed the smallest r of the cell
+    std::vector<int32_t> hint(static_cast<size_t>(n_mats) * 2 * kHintStride, 0);
+    for (int m = 0; m < n_mats; ++m)
+      for (int sp = 0; sp < 2; ++sp) {
+        const double* R = tables->data + (static_cast<size_t>(m) * ADEPT_N_TABLES + (sp == 0 ? 6 : 11)) * N;
+        int32_t* h = hint.data() + (static_cast<size_t>(m) * 2 + sp) * kHintStride;
+        auto key = [](double r) { int64_t b; std::memcpy(&b, &r, 8); return static_cast<int32_t>(b >> 47); };
+        const int32_t key0 = R[0] > 0.0 ? key(R[0]) : 0;
+        h[0] = key0;
+        size_t j = 0;
+        for (int k = 0; k < kHintN; ++k) {
+          const int64_t bits = static_cast<int64_t>(key0 + k) << 47;   // smallest double of the key cell
+          double r_lo;
+          std::memcpy(&r_lo, &bits, 8);
+          while (j + 2 < N && R[j + 1] <= r_lo) ++j;
+          h[1 + k] = static_cast<int32_t>(j);
+        }
+      }
+    CUDA_TRY(cudaMemcpy(L.rhint, hint.data(), hint.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
     static_assert(sizeof(adept_material) == N_SCAL * sizeof(double), "adept_material layout");
     CUDA_TRY(cudaMemcpy(L.scal, mats, static_cast<size_t>(n_mats) * sizeof(adept_material), cudaMemcpyHostToDevice));
   }
@@ -350,7 +371,7 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   ctx->n_vol = nv; ctx->n_mat = n_mats;
   DevCtx& d = ctx->dev;
   d.vol = L.vol; d.rot = L.rot; d.n_vol = nv; d.bvh = L.bvh; d.navigator = cfg->navigator;
-  d.tab_g = L.tab_g; d.tab_em = L.tab_em; d.tab_ep = L.tab_ep; d.scal = L.scal; d.n_mat = n_mats;
+  d.tab_g = L.tab_g; d.tab_em = L.tab_em; d.tab_ep = L.tab_ep; d.scal = L.scal; d.rhint = L.rhint; d.n_mat = n_mats;
   d.field_kind = f->kind;
   for (int k = 0; k < 3; ++k) d.B[k] = f->B[k];
   d.nr = f->nr; d.nz = f->nz; d.r0 = f->r0; d.z0 = f->z0; d.dr = f->dr; d.dz = f->dz; d.bz = L.bz;

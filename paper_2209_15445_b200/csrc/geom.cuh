@@ -34,16 +34,18 @@ __device__ __forceinline__ bool inside_solid(int solid, const double h[3], const
   return r2 >= h[0] * h[0] && r2 <= h[1] * h[1] && fabs(p[2]) <= h[2];
 }
 
+// min_i (sgn(d_i) h_i - p_i) / d_i over d_i != 0.  The three quotients n_i / |d_i| are compared by
+// cross-multiplication and only the smallest is divided (one division instead of three; when two are
+// within rounding of each other either is the minimum to 1 ulp).
 __device__ __forceinline__ double box_exit(const double h[3], const double p[3], const double d[3]) {
-  double t = ADEPT_INF;
+  double num = 1.0, den = 0.0;   // +inf as 1/0
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
-    if (d[i] != 0.0) {
-      const double ti = ((d[i] > 0.0 ? h[i] : -h[i]) - p[i]) / d[i];
-      t = fmin(t, ti);
-    }
+    const double ad = fabs(d[i]);
+    const double ni = h[i] - (d[i] > 0.0 ? p[i] : -p[i]);   // distance to the exit plane along the axis
+    if (ad != 0.0 && ni * den <= num * ad) { num = ni; den = ad; }
   }
-  return fmax(t, 0.0);
+  return den != 0.0 ? fmax(num / den, 0.0) : ADEPT_INF;
 }
 
 __device__ __forceinline__ double box_entry(const double h[3], const double p[3], const double d[3]) {

@@ -1,6 +1,7 @@
 // Table lookup and the discrete-interaction samplers  (§8(c) M7, P1-P10).
 // All functions take scalar arguments and keep no thread-local state.
 #pragma once
+#include "fastmath.cuh"
 #include "rng.cuh"
 #include "types.cuh"
 
@@ -11,7 +12,7 @@ __device__ __forceinline__ double mat_scalar(const DevCtx& c, int mat, int s) { 
 // M7: cell index and fraction of ln T on the grid
 struct GridPos { int i; double f; };
 __device__ __forceinline__ GridPos grid_pos(const DevCtx& c, double ekin) {
-  const double x = (log(ekin) - c.u0) / c.du;
+  const double x = (log_pos(ekin) - c.u0) * c.inv_du;
   int i = static_cast<int>(floor(x));
   i = min(max(i, 0), kNGrid - 2);
   return GridPos{i, x - i};
@@ -22,54 +23,59 @@ __device__ __forceinline__ double interp(const double* __restrict__ tab, int row
   return y0 + g.f * (y1 - y0);
 }
 
-// M7 inverse range: cell j with R_j <= r < R_{j+1}, found by galloping down from the cell of the
-// pre-step energy (any search returns the same j).  Returns 0 when r < R_0 (the track stops).
-__device__ __noinline__ double inverse_range(const DevCtx& c, const double* __restrict__ tab, int row, int col,
-                                                int i_start, double r) {
+// M7 inverse range: cell j with R_j <= r < R_{j+1}, then ln T linear in r.  Any search returns the same
+// j; this one starts from a hint table indexed by the exponent and top 5 mantissa bits of r (a
+// monotone pseudo-logarithm, built by adept_init: hint[k] = largest j with R_j <= lower edge of key
+// cell k) and walks up, typically 0-2 nodes, instead of ~10 dependent loads of a binary search.
+// Returns 0 when r < R_0 (the track stops).
+constexpr int kHintN = 2048;           // key cells per table: 64 octaves of range
+constexpr int kHintStride = kHintN + 2;  // [0] = key of R_0, [1..kHintN] = hints, [last] pad
+__device__ __forceinline__ int range_key(double r) { return __double2hiint(r) >> 15; }
+
+__device__ __forceinline__ double inverse_range(const DevCtx& c, const double* __restrict__ tab, int row, int col,
+                                                const int32_t* __restrict__ hint, double r) {
   if (r < __ldg(tab + col)) return 0.0;
-  int hi = min(i_start + 1, kNGrid - 1);  // R[hi] > r is guaranteed by r < R(T) <= R[i_start+1]
-  int lo = hi, stride = 1;
-  do {                                   // gallop: find lo with R[lo] <= r
-    lo = max(lo - stride, 0);
-    stride <<= 1;
-  } while (__ldg(tab + lo * row + col) > r);
-  while (hi - lo > 1) {
-    const int mid = (lo + hi) >> 1;
-    if (__ldg(tab + mid * row + col) <= r) lo = mid; else hi = mid;
+  const int k = min(max(range_key(r) - __ldg(hint), 0), kHintN - 1);
+  int lo = __ldg(hint + 1 + k);
+  double R0 = __ldg(tab + lo * row + col), R1 = __ldg(tab + (lo + 1) * row + col);
+  while (R1 <= r && lo < kNGrid - 2) {
+    ++lo;
+    R0 = R1;
+    R1 = __ldg(tab + (lo + 1) * row + col);
   }
-  const double R0 = __ldg(tab + lo * row + col), R1 = __ldg(tab + (lo + 1) * row + col);
   const double lnT = c.u0 + c.du * lo + c.du * (r - R0) / (R1 - R0);
   return exp(lnT);
 }
 
-// P10 rotation of d by polar (cos_t, sin_t) and azimuth phi
-__device__ __noinline__ void rotate(const double d[3], double cos_t, double sin_t, double phi, double out[3]) {
+// P10 rotation of d by polar (cos_t, sin_t) and azimuth phi = pi * phi_over_pi (sincospi reduces the
+// argument exactly).  One reciprocal each for 1/rho and the renormalisation.
+__device__ __noinline__ void rotate(const double d[3], double cos_t, double sin_t, double phi_over_pi, double out[3]) {
   const double rho2 = d[0] * d[0] + d[1] * d[1];
-  const double rho = sqrt(rho2);
   double e1[3], e2[3];
-  if (rho > 0.0) {
-    e1[0] = d[0] * d[2] / rho; e1[1] = d[1] * d[2] / rho; e1[2] = -rho2 / rho;
-    e2[0] = -d[1] / rho; e2[1] = d[0] / rho; e2[2] = 0.0;
+  if (rho2 > 0.0) {
+    const double ir = rsqrt(rho2);
+    e1[0] = d[0] * d[2] * ir; e1[1] = d[1] * d[2] * ir; e1[2] = -rho2 * ir;
+    e2[0] = -d[1] * ir; e2[1] = d[0] * ir; e2[2] = 0.0;
   } else {
     e1[0] = d[2] >= 0.0 ? 1.0 : -1.0; e1[1] = 0.0; e1[2] = 0.0;
     e2[0] = 0.0; e2[1] = 1.0; e2[2] = 0.0;
   }
   double sp, cp;
-  sincos(phi, &sp, &cp);
+  sincospi(phi_over_pi, &sp, &cp);
   const double a = sin_t * cp, b = sin_t * sp;
   double n = 0.0;
 #pragma unroll
   for (int i = 0; i < 3; ++i) { out[i] = a * e1[i] + b * e2[i] + cos_t * d[i]; n += out[i] * out[i]; }
-  n = sqrt(n);
+  n = rsqrt(n);
 #pragma unroll
-  for (int i = 0; i < 3; ++i) out[i] /= n;
+  for (int i = 0; i < 3; ++i) out[i] *= n;
 }
 
 __device__ __forceinline__ double momentum(double T) { return sqrt(T * (T + 2.0 * kMe)); }
 
 __device__ __forceinline__ void normalise(double v[3]) {
-  const double n = sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
-  v[0] /= n; v[1] /= n; v[2] /= n;
+  const double n = rsqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+  v[0] *= n; v[1] *= n; v[2] *= n;
 }
 
 // M5: an e- below T_c or a gamma below k_c is not created (energy deposited locally); e+ always are.
@@ -87,7 +93,7 @@ __device__ __noinline__ void compton(const DevCtx& c, int mat, StepOut& o, Strea
   Track& g = o.post;
   const double k = g.ekin, kap = k / kMe;
   const double e0 = 1.0 / (1.0 + 2.0 * kap);
-  const double a1 = -log(e0), a2 = 0.5 * (1.0 - e0 * e0);
+  const double a1 = -log_pos(e0), a2 = 0.5 * (1.0 - e0 * e0);
   double eps = 1.0, t = 0.0, sin2 = 0.0;
   for (int it = 0; it < 1000; ++it) {
     const double r1 = u.draw(), r2 = u.draw(), r3 = u.draw();
@@ -97,7 +103,7 @@ __device__ __noinline__ void compton(const DevCtx& c, int mat, StepOut& o, Strea
     sin2 = t * (2.0 - t);
     if (1.0 - eps * sin2 / (1.0 + eps * eps) >= r3) break;
   }
-  const double phi = 2.0 * kPi * u.draw();
+  const double phi = 2.0 * u.draw();   // azimuth in units of pi
   const double cos_t = 1.0 - t, sin_t = sqrt(fmax(sin2, 0.0));
   const double d0[3] = {g.dx, g.dy, g.dz};
   double d1[3];
@@ -127,7 +133,7 @@ __device__ __noinline__ void pair_production(const DevCtx& c, int mat, StepOut& 
     eps = a + (1.0 - 2.0 * a) * r1;
     if (1.0 - (4.0 / 3.0) * eps * (1.0 - eps) >= r2 * fmax_) break;
   }
-  const double phi = 2.0 * kPi * u.draw();
+  const double phi = 2.0 * u.draw();   // azimuth in units of pi
   const double Ep = eps * k, Em = (1.0 - eps) * k;
   const double Tp = fmax(Ep - kMe, 0.0), Tm = fmax(Em - kMe, 0.0);
   const double thm = kMe / Em, thp = kMe / Ep;
@@ -136,7 +142,7 @@ __device__ __noinline__ void pair_production(const DevCtx& c, int mat, StepOut& 
   sincos(thm, &sn, &cs);
   rotate(d0, cs, sn, phi, dm);
   sincos(thp, &sn, &cs);
-  rotate(d0, cs, sn, phi + kPi, dp);
+  rotate(d0, cs, sn, phi + 1.0, dp);
   emit(c, mat, o, ADEPT_ELECTRON, dm, Tm, 0);
   emit(c, mat, o, ADEPT_POSITRON, dp, Tp, 1);
   o.alive = 0;
@@ -161,7 +167,7 @@ __device__ __noinline__ bool bremsstrahlung(const DevCtx& c, int mat, StepOut& o
   Track& e = o.post;
   const double T = e.ekin, kc = mat_scalar(c, mat, S_KCUT);
   if (!(T > kc)) return false;
-  const double E = T + kMe, lr = log(T / kc);
+  const double E = T + kMe, lr = log_pos(T / kc);
   double k = kc;
   for (int it = 0; it < 1000; ++it) {
     const double r1 = u.draw(), r2 = u.draw();
@@ -170,7 +176,7 @@ __device__ __noinline__ bool bremsstrahlung(const DevCtx& c, int mat, StepOut& o
     if (4.0 / 3.0 - 4.0 * y / 3.0 + y * y >= (4.0 / 3.0) * r2) break;
   }
   k = fmin(k, T);
-  const double phi = 2.0 * kPi * u.draw();
+  const double phi = 2.0 * u.draw();   // azimuth in units of pi
   const double th = kMe / E;
   const double d0[3] = {e.dx, e.dy, e.dz};
   double dg[3], sn, cs;
@@ -212,7 +218,7 @@ __device__ __noinline__ bool moller(const DevCtx& c, int mat, StepOut& o, Stream
     const double h = eps * eps * (c0 + ie * (ie - b) + i1 * (i1 - b));
     if (h >= r2 * hmax) break;
   }
-  const double phi = 2.0 * kPi * u.draw();
+  const double phi = 2.0 * u.draw();   // azimuth in units of pi
   delta_ray(c, mat, o, T, eps * T, phi);
   return true;
 }
@@ -234,7 +240,7 @@ __device__ __noinline__ bool bhabha(const DevCtx& c, int mat, StepOut& o, Stream
     if (h >= r2) break;
   }
   eps = fmin(eps, 1.0);
-  const double phi = 2.0 * kPi * u.draw();
+  const double phi = 2.0 * u.draw();   // azimuth in units of pi
   delta_ray(c, mat, o, T, eps * T, phi);
   return true;
 }
@@ -245,14 +251,14 @@ __device__ __noinline__ void annihilation(const DevCtx& c, int mat, StepOut& o, 
   const double T = e.ekin, g = 1.0 + T / kMe;
   const double root = sqrt((g - 1.0) / (g + 1.0));
   const double emin = 0.5 - 0.5 * root, emax = 0.5 + 0.5 * root;
-  const double lr = log(emax / emin), gp1sq = (g + 1.0) * (g + 1.0);
+  const double lr = log_pos(emax / emin), gp1sq = (g + 1.0) * (g + 1.0);
   double eps = 0.5;
   for (int it = 0; it < 1000; ++it) {
     const double r1 = u.draw(), r2 = u.draw();
     eps = emin * exp(r1 * lr);
     if (1.0 - eps + (2.0 * g * eps - 1.0) / (eps * gp1sq) >= r2) break;
   }
-  const double phi = 2.0 * kPi * u.draw();
+  const double phi = 2.0 * u.draw();   // azimuth in units of pi
   const double Etot = T + 2.0 * kMe;
   const double k1 = eps * Etot, k2 = Etot - k1;
   double cos_t = (eps * (g + 1.0) - 1.0) / (eps * sqrt(g * g - 1.0));
@@ -274,7 +280,7 @@ __device__ __noinline__ void annihilation_at_rest(const DevCtx& c, int mat, Step
   const double u4 = u.uniform(4), u5 = u.uniform(5);
   const double cos_t = 2.0 * u4 - 1.0, sin_t = sqrt(fmax(0.0, 1.0 - cos_t * cos_t));
   double sp, cp;
-  sincos(2.0 * kPi * u5, &sp, &cp);
+  sincospi(2.0 * u5, &sp, &cp);
   const double d1[3] = {sin_t * cp, sin_t * sp, cos_t};
   const double d2[3] = {-d1[0], -d1[1], -d1[2]};
   emit(c, mat, o, ADEPT_GAMMA, d1, kMe, 0);

@@ -73,7 +73,7 @@ __device__ int step_move(const DevCtx& c, int nav, bool active, const Track& in,
           se = interp(tab, row, 2, gp);                                   // photoelectric
         }
         stot = x0 + x1 + se;
-        s_phys = stot > 0.0 ? -log(u.uniform(0)) / stot : ADEPT_INF;
+        s_phys = stot > 0.0 ? div_pos(-log_pos(u.uniform(0)), stot) : ADEPT_INF;
       } else {
         double sa = 0.0;
         if (!vacuum) {
@@ -88,7 +88,7 @@ __device__ int step_move(const DevCtx& c, int nav, bool active, const Track& in,
           }
         }
         stot = x0 + x1 + sa;
-        const double s_disc = stot > 0.0 ? -log(u.uniform(0)) / stot : ADEPT_INF;
+        const double s_disc = stot > 0.0 ? div_pos(-log_pos(u.uniform(0)), stot) : ADEPT_INF;
         range_out = R <= c.rho_R;
         const double s_loss = range_out ? R : c.alpha_R * R + c.rho_R * (1.0 - c.alpha_R) * (2.0 - c.rho_R / R);
         lim_disc = s_disc < s_loss;
@@ -112,7 +112,7 @@ __device__ int step_move(const DevCtx& c, int nav, bool active, const Track& in,
     if (!vacuum) {
       if (flag == 0 && !lim_disc && range_out) dE = T0;
       else if (s <= 0.01 * R) dE = S * s;
-      else dE = T0 - inverse_range(c, tab, row, positron ? 4 : 3, gp.i, R - s);
+      else dE = T0 - inverse_range(c, tab, row, positron ? 4 : 3, c.rhint + (2 * mat + (positron ? 1 : 0)) * kHintStride, R - s);
       dE = fmin(fmax(dE, 0.0), T0);
     }
     o.edep_dep += dE;
@@ -129,13 +129,13 @@ __device__ int step_move(const DevCtx& c, int nav, bool active, const Track& in,
       const double X0 = mat_scalar(c, mat, S_X0);
       const double pbeta = T0 * (T0 + 2.0 * kMe) / (T0 + kMe);
       const double beta2 = T0 * (T0 + 2.0 * kMe) / ((T0 + kMe) * (T0 + kMe));
-      const double corr = fmax(0.0, 1.0 + 0.038 * log(s / (X0 * beta2)));
+      const double corr = fmax(0.0, 1.0 + 0.038 * log_pos(s / (X0 * beta2)));
       const double th0 = (13.6 / pbeta) * sqrt(s / X0) * corr;
       const double u2 = u.uniform(2), u3 = u.uniform(3);
-      const double th = th0 * sqrt(-2.0 * log(u2));
+      const double th = th0 * sqrt(-2.0 * log_pos(u2));
       double sn, cs, dn[3];
       sincos(th, &sn, &cs);
-      rotate(dir, cs, sn, 2.0 * kPi * u3, dn);
+      rotate(dir, cs, sn, 2.0 * u3, dn);
       dir[0] = dn[0]; dir[1] = dn[1]; dir[2] = dn[2];
     }
   }

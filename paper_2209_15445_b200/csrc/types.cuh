@@ -109,6 +109,7 @@ struct DevCtx {
   const double* tab_em;     // [n_mat][2048][kRowEm]
   const double* tab_ep;     // [n_mat][2048][kRowEp]
   const double* scal;       // [n_mat][N_SCAL]
+  const int32_t* rhint;     // [n_mat][2 (e-, e+)][kHintStride] inverse-range search hints (physics.cuh)
   int32_t n_mat;
   int32_t field_kind;
   double B[3];
