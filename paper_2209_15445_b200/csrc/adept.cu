@@ -247,6 +247,7 @@ size_t carve(void* base, const adept_config* cfg, const adept_geometry* g, int n
   const size_t cap = cfg->track_capacity;
   const size_t scap = cfg->stage_capacity ? cfg->stage_capacity : cap;
   auto take_soa = [&cv](TrackSoA& b, size_t n) {
+    n = (n + kBlock - 1) / kBlock * kBlock;   // whole tiles: the kernels fetch a buffer tile by tile (TMA bulk copies)
     b.x = cv.take<double>(n); b.y = cv.take<double>(n); b.z = cv.take<double>(n);
     b.dx = cv.take<double>(n); b.dy = cv.take<double>(n); b.dz = cv.take<double>(n);
     b.ekin = cv.take<double>(n); b.id = cv.take<uint64_t>(n);

@@ -47,6 +47,78 @@ __device__ __forceinline__ double warp_sum(double v) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// A0: tile loads.  A tile is kBlock consecutive entries of a species buffer (or staging queue): eleven
+// contiguous SoA slices, fetched by ONE thread with eleven TMA bulk copies (cp.async.bulk, SASS UBLKCP)
+// into a double-buffered shared-memory tile that completes on an mbarrier.  The copy of tile k+1 is in
+// flight while the block computes tile k, so the HBM latency of the track state is hidden without
+// spending registers or occupancy on it.  Buffers are allocated in multiples of kBlock entries, so a
+// full tile can always be read (entries past the live count are ignored).
+struct alignas(128) TrackTile {
+  double d[7][kBlock];      // x, y, z, dx, dy, dz, ekin
+  uint64_t id[kBlock];
+  uint32_t u[3][kBlock];    // event, step, vol
+};
+constexpr uint32_t kTileBytes = 8u * kBlock * 8u + 3u * kBlock * 4u;
+static_assert(sizeof(TrackTile) % 128 == 0 && sizeof(TrackTile) >= kTileBytes, "TrackTile layout");
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra WAIT_DONE;\n"
+      "bra WAIT_LOOP;\n"
+      "WAIT_DONE:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_load(void* smem_dst, const void* gmem_src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)),
+               "l"(gmem_src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+
+// issued by one thread: tile `tile` of buffer b -> shared tile t, completion on bar
+__device__ __forceinline__ void tile_issue(TrackTile& t, const TrackSoA& b, uint32_t tile, uint64_t* bar) {
+  const size_t base = static_cast<size_t>(tile) * kBlock;
+  mbar_expect_tx(bar, kTileBytes);
+  bulk_load(t.d[0], b.x + base, kBlock * 8, bar); bulk_load(t.d[1], b.y + base, kBlock * 8, bar);
+  bulk_load(t.d[2], b.z + base, kBlock * 8, bar); bulk_load(t.d[3], b.dx + base, kBlock * 8, bar);
+  bulk_load(t.d[4], b.dy + base, kBlock * 8, bar); bulk_load(t.d[5], b.dz + base, kBlock * 8, bar);
+  bulk_load(t.d[6], b.ekin + base, kBlock * 8, bar); bulk_load(t.id, b.id + base, kBlock * 8, bar);
+  bulk_load(t.u[0], b.event + base, kBlock * 4, bar); bulk_load(t.u[1], b.step + base, kBlock * 4, bar);
+  bulk_load(t.u[2], b.vol + base, kBlock * 4, bar);
+}
+
+__device__ __forceinline__ Track tile_read(const TrackTile& t, int k, int species) {
+  Track r;
+  r.x = t.d[0][k]; r.y = t.d[1][k]; r.z = t.d[2][k];
+  r.dx = t.d[3][k]; r.dy = t.d[4][k]; r.dz = t.d[5][k];
+  r.ekin = t.d[6][k]; r.id = t.id[k];
+  r.event = t.u[0][k]; r.step = t.u[1][k]; r.vol = t.u[2][k];
+  r.species = species;
+  return r;
+}
+
+struct TilePipe {
+  TrackTile tile[2];
+  uint64_t bar[2];
+};
+__device__ __forceinline__ void pipe_init(TilePipe& p) {
+  if (threadIdx.x == 0) { mbar_init(&p.bar[0], 1); mbar_init(&p.bar[1], 1); mbar_fence_init(); }
+  __syncthreads();
+}
+
+// ------------------------------------------------------------------------------------------------
 // A0: block-aggregated append.  Every lane asks for cnt[d] (0..3) consecutive entries of destination
 // queue d; the block adds its total to each queue counter with one atomic and every lane gets the
 // index of its first entry.  Must be called by all threads of the block (two __syncthreads); the
@@ -55,8 +127,24 @@ __device__ __forceinline__ double warp_sum(double v) {
 template <int ND>
 struct BlockReserve {
   uint32_t wtot[2][kWarps][ND];
-  uint32_t base[2][ND];
+  uint32_t wbase[2][kWarps][ND];   // first entry of each warp's share
 };
+
+// second half: one thread per destination turns the per-warp totals into per-warp bases
+template <int ND, typename CounterOf>
+__device__ __forceinline__ void block_reserve_commit(BlockReserve<ND>& br, int phase, CounterOf counter_of) {
+  __syncthreads();
+  if (threadIdx.x < ND) {
+    const int d = threadIdx.x;
+    uint32_t w[kWarps], tot = 0;
+#pragma unroll
+    for (int k = 0; k < kWarps; ++k) { w[k] = br.wtot[phase][k][d]; tot += w[k]; }
+    uint32_t base = tot ? atomicAdd(counter_of(d), tot) : 0u;
+#pragma unroll
+    for (int k = 0; k < kWarps; ++k) { br.wbase[phase][k][d] = base; base += w[k]; }
+  }
+  __syncthreads();
+}
 
 template <int ND, typename CounterOf>
 __device__ __forceinline__ void block_reserve(BlockReserve<ND>& br, int phase, const uint32_t (&cnt)[ND], uint32_t (&first)[ND],
@@ -70,20 +158,9 @@ __device__ __forceinline__ void block_reserve(BlockReserve<ND>& br, int phase, c
     pre[d] = __popc(b0 & lt) + 2 * __popc(b1 & lt);
     if (lane == 0) br.wtot[phase][warp][d] = __popc(b0) + 2 * __popc(b1);
   }
-  __syncthreads();
-  if (threadIdx.x < ND) {
-    uint32_t tot = 0;
+  block_reserve_commit<ND>(br, phase, counter_of);
 #pragma unroll
-    for (int w = 0; w < kWarps; ++w) tot += br.wtot[phase][w][threadIdx.x];
-    br.base[phase][threadIdx.x] = tot ? atomicAdd(counter_of(threadIdx.x), tot) : 0u;
-  }
-  __syncthreads();
-#pragma unroll
-  for (int d = 0; d < ND; ++d) {
-    uint32_t f = br.base[phase][d] + pre[d];
-    for (int w = 0; w < warp; ++w) f += br.wtot[phase][w][d];
-    first[d] = f;
-  }
+  for (int d = 0; d < ND; ++d) first[d] = br.wbase[phase][warp][d] + pre[d];
 }
 
 // A9: warp-reduced scoring.  Lanes depositing into the same volume are combined (match_any) and the
@@ -196,20 +273,26 @@ move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot sl
   const int q0 = species == ADEPT_GAMMA ? 0 : (species == ADEPT_ELECTRON ? 3 : 5);
   __shared__ BlockTally tally;
   __shared__ BlockReserve<ND> br;
+  __shared__ TilePipe pipe;
   tally_init(tally);
+  pipe_init(pipe);
   double sum_dep = 0.0, sum_cut = 0.0;
   unsigned chords = 0;
-  int phase = 0;
-  const int lane = threadIdx.x & 31;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned lt = (1u << lane) - 1u;
 
   const uint32_t n_tiles = (n + kBlock - 1) / kBlock;
-  for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, phase ^= 1) {
+  if (threadIdx.x == 0 && blockIdx.x < n_tiles) tile_issue(pipe.tile[0], cur, blockIdx.x, &pipe.bar[0]);
+  uint32_t k = 0;
+  for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++k) {
+    const int phase = k & 1;
+    // prefetch the block's next tile; its buffer was last read one iteration ago, before the barriers
+    // of that iteration's reservation
+    if (threadIdx.x == 0 && tile + gridDim.x < n_tiles) tile_issue(pipe.tile[phase ^ 1], cur, tile + gridDim.x, &pipe.bar[phase ^ 1]);
+    mbar_wait(&pipe.bar[phase], (k >> 1) & 1);
     const uint32_t i = tile * kBlock + threadIdx.x;
-    bool active = i < n;
-    Track in{};
-    if (active) in = load_track(cur, i, species);
-    in.species = species;
-    active = active && in.vol != kDeadVolume;
+    Track in = tile_read(pipe.tile[phase], threadIdx.x, species);
+    const bool active = i < n && in.vol != kDeadVolume;
     StepOut o;
     Stream u;
     int process, mat;
@@ -239,38 +322,45 @@ move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot sl
       tally_outcome(tally, none, o.outcome, ADEPT_OUT_TRUNCATED);
     }
 
+    // reservation: a lane appends at most one survivor (to one of four destinations) and, in the charged
+    // kernel, the photons of an annihilation at rest
     const bool live = active && o.alive;
     const int dest = !live ? -1 : (next == NEXT_INTERACT ? 1 + stage_queue(process, species) - q0 : 0);
-    uint32_t want[ND], first[ND];
+    uint32_t pre = 0, pre_ph = 0;
 #pragma unroll
-    for (int d = 0; d < 4; ++d) want[d] = dest == d ? 1u : 0u;
-    if (MODE != MODE_GAMMA) want[4] = active ? static_cast<uint32_t>(o.n_sec) : 0u;
-    block_reserve<ND>(br, phase, want, first, [&](int d) -> uint32_t* {
+    for (int d = 0; d < 4; ++d) {
+      const unsigned b = __ballot_sync(kFull, dest == d);
+      if (dest == d) pre = __popc(b & lt);
+      if (lane == 0) br.wtot[phase][warp][d] = __popc(b);
+    }
+    const uint32_t n_ph = (MODE != MODE_GAMMA && active) ? static_cast<uint32_t>(o.n_sec) : 0u;
+    if (MODE != MODE_GAMMA) {
+      const unsigned b0 = __ballot_sync(kFull, n_ph & 1u), b1 = __ballot_sync(kFull, n_ph & 2u);
+      pre_ph = __popc(b0 & lt) + 2 * __popc(b1 & lt);
+      const uint32_t tot = __popc(b0) + 2 * __popc(b1);
+      if (lane == 0) { br.wtot[phase][warp][4] = tot; if (tot) atomicAdd(&tally.secondaries[ADEPT_GAMMA], tot); }
+    }
+    block_reserve_commit<ND>(br, phase, [&](int d) -> uint32_t* {
       if (d == 0) return &cnt->count[parity ^ 1][species].v;
       if (d == 4) return &cnt->count[parity ^ 1][ADEPT_GAMMA].v;
       return &cnt->n_stage[q0 + d - 1].v;
     });
     if (live) {
       o.post.step = in.step + 1;
-      uint32_t j = first[0];
-      bool ok = j < c.capacity;
-      const TrackSoA* dst = &slot.buf[parity ^ 1][species];
-#pragma unroll
-      for (int d = 1; d < 4; ++d)
-        if (dest == d) { j = first[d]; ok = j < c.stage_capacity; dst = &slot.stage[q0 + d - 1]; }
-      if (ok) store_track(*dst, j, o.post);
+      const uint32_t j = br.wbase[phase][warp][dest] + pre;
+      const bool staged = dest != 0;
+      const TrackSoA& dst = staged ? slot.stage[q0 + dest - 1] : slot.buf[parity ^ 1][species];
+      if (j < (staged ? c.stage_capacity : c.capacity)) store_track(dst, j, o.post);
       else cnt->overflow.v = 1;
     }
     if (MODE != MODE_GAMMA) {
-      if (active && o.n_sec > 0) {  // at-rest annihilation photons
-        for (int k = 0; k < o.n_sec; ++k) {
-          const uint32_t j = first[4] + k;
-          if (j < c.capacity) store_track(slot.buf[parity ^ 1][ADEPT_GAMMA], j, make_secondary(o, k, in.event, u));
+      if (n_ph) {  // at-rest annihilation photons
+        const uint32_t j0 = br.wbase[phase][warp][4] + pre_ph;
+        for (uint32_t kk = 0; kk < n_ph; ++kk) {
+          if (j0 + kk < c.capacity) store_track(slot.buf[parity ^ 1][ADEPT_GAMMA], j0 + kk, make_secondary(o, kk, in.event, u));
           else cnt->overflow.v = 1;
         }
       }
-      const unsigned ns = __reduce_add_sync(kFull, want[4]);
-      if (lane == 0 && ns) atomicAdd(&tally.secondaries[ADEPT_GAMMA], ns);
     }
   }
   {
@@ -289,6 +379,7 @@ interact_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlo
   SlotCounters* cnt = slot.counters;
   __shared__ BlockTally tally;
   __shared__ BlockReserve<3> br;
+  __shared__ TilePipe pipe;
   __shared__ uint32_t tile_begin[kNumStage + 1];   // prefix of tiles per queue
   __shared__ uint32_t n_staged[kNumStage];
   if (threadIdx.x == 0) {
@@ -302,27 +393,38 @@ interact_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlo
     tile_begin[kNumStage] = acc;
   }
   tally_init(tally);
+  pipe_init(pipe);
   double sum_cut = 0.0;
-  int phase = 0;
   const int lane = threadIdx.x & 31;
   const uint32_t total = tile_begin[kNumStage];
-  for (uint32_t tile = blockIdx.x; tile < total; tile += gridDim.x, phase ^= 1) {
-    int q = 0;
-    while (tile >= tile_begin[q + 1]) ++q;
+  const auto queue_of = [&](uint32_t tile) { int q = 0; while (tile >= tile_begin[q + 1]) ++q; return q; };
+  if (threadIdx.x == 0 && blockIdx.x < total) {
+    const int q = queue_of(blockIdx.x);
+    tile_issue(pipe.tile[0], slot.stage[q], blockIdx.x - tile_begin[q], &pipe.bar[0]);
+  }
+  uint32_t k = 0;
+  for (uint32_t tile = blockIdx.x; tile < total; tile += gridDim.x, ++k) {
+    const int phase = k & 1;
+    if (threadIdx.x == 0 && tile + gridDim.x < total) {
+      const int qn = queue_of(tile + gridDim.x);
+      tile_issue(pipe.tile[phase ^ 1], slot.stage[qn], tile + gridDim.x - tile_begin[qn], &pipe.bar[phase ^ 1]);
+    }
+    const int q = queue_of(tile);
     const uint32_t i = (tile - tile_begin[q]) * kBlock + threadIdx.x;
     const bool active = i < n_staged[q];
     const int species = stage_species(q);
+    mbar_wait(&pipe.bar[phase], (k >> 1) & 1);
     StepOut o;
     Stream u;
-    Track t{};
+    Track t = tile_read(pipe.tile[phase], threadIdx.x, species);
     if (active) {
-      t = load_track(slot.stage[q], i, species);
       init_out(o, t, true);
       u.init(t.event, c.seed, t.id, t.step - 1);          // the stream of the step that chose the process
       const int mat = volume(c, t.vol).material;
       run_process(c, stage_process(q), species, mat, o, u);
       sum_cut += o.edep_cut;
     } else {
+      t = Track{};
       init_out(o, t, false);
       u.init(0, 0, 0, 0);
     }
