@@ -267,9 +267,11 @@ move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot sl
   SlotCounters* cnt = slot.counters;
   const uint32_t n = cnt->count[parity][species].v;
 
-  // destinations of this kernel: 0 = next buffer of the species, 1..3 = its staging queues,
-  // 4 = next gamma buffer (at-rest annihilation photons, charged kernel only)
-  constexpr int ND = MODE == MODE_GAMMA ? 4 : 5;
+  // destinations of this kernel: 0 = next buffer of the species, 1..3 = its staging queues, 4 = next
+  // buffer of the secondaries a move can create: photoelectrons (gamma kernel) or the photons of an
+  // annihilation at rest (charged kernel)
+  constexpr int ND = 5;
+  constexpr int kSecSpecies = MODE == MODE_GAMMA ? ADEPT_ELECTRON : ADEPT_GAMMA;
   const int q0 = species == ADEPT_GAMMA ? 0 : (species == ADEPT_ELECTRON ? 3 : 5);
   __shared__ BlockTally tally;
   __shared__ BlockReserve<ND> br;
@@ -320,10 +322,12 @@ move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot sl
     if (MODE != MODE_GAMMA) {
       tally_outcome(tally, none, o.outcome, ADEPT_OUT_LOSS);
       tally_outcome(tally, none, o.outcome, ADEPT_OUT_TRUNCATED);
+    } else {
+      tally_outcome(tally, none, o.outcome, ADEPT_OUT_PHOTO);
     }
 
-    // reservation: a lane appends at most one survivor (to one of four destinations) and, in the charged
-    // kernel, the photons of an annihilation at rest
+    // reservation: a lane appends at most one survivor (to one of four destinations) and the secondaries
+    // of a photoelectric absorption or an annihilation at rest
     const bool live = active && o.alive;
     const int dest = !live ? -1 : (next == NEXT_INTERACT ? 1 + stage_queue(process, species) - q0 : 0);
     uint32_t pre = 0, pre_ph = 0;
@@ -333,16 +337,17 @@ move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot sl
       if (dest == d) pre = __popc(b & lt);
       if (lane == 0) br.wtot[phase][warp][d] = __popc(b);
     }
-    const uint32_t n_ph = (MODE != MODE_GAMMA && active) ? static_cast<uint32_t>(o.n_sec) : 0u;
-    if (MODE != MODE_GAMMA) {
-      const unsigned b0 = __ballot_sync(kFull, n_ph & 1u), b1 = __ballot_sync(kFull, n_ph & 2u);
+    const uint32_t n_ph = active ? static_cast<uint32_t>(o.n_sec) : 0u;
+    const bool ph0 = n_ph && o.sec[0].species >= 0, ph1 = MODE != MODE_GAMMA && n_ph && o.sec[1].species >= 0;
+    {
+      const unsigned b0 = __ballot_sync(kFull, n_ph & 1u), b1 = MODE != MODE_GAMMA ? __ballot_sync(kFull, n_ph & 2u) : 0u;
       pre_ph = __popc(b0 & lt) + 2 * __popc(b1 & lt);
       const uint32_t tot = __popc(b0) + 2 * __popc(b1);
-      if (lane == 0) { br.wtot[phase][warp][4] = tot; if (tot) atomicAdd(&tally.secondaries[ADEPT_GAMMA], tot); }
+      if (lane == 0) { br.wtot[phase][warp][4] = tot; if (tot) atomicAdd(&tally.secondaries[kSecSpecies], tot); }
     }
     block_reserve_commit<ND>(br, phase, [&](int d) -> uint32_t* {
       if (d == 0) return &cnt->count[parity ^ 1][species].v;
-      if (d == 4) return &cnt->count[parity ^ 1][ADEPT_GAMMA].v;
+      if (d == 4) return &cnt->count[parity ^ 1][kSecSpecies].v;
       return &cnt->n_stage[q0 + d - 1].v;
     });
     if (live) {
@@ -353,13 +358,14 @@ move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot sl
       if (j < (staged ? c.stage_capacity : c.capacity)) store_track(dst, j, o.post);
       else cnt->overflow.v = 1;
     }
-    if (MODE != MODE_GAMMA) {
-      if (n_ph) {  // at-rest annihilation photons
-        const uint32_t j0 = br.wbase[phase][warp][4] + pre_ph;
-        for (uint32_t kk = 0; kk < n_ph; ++kk) {
-          if (j0 + kk < c.capacity) store_track(slot.buf[parity ^ 1][ADEPT_GAMMA], j0 + kk, make_secondary(o, kk, in.event, u));
-          else cnt->overflow.v = 1;
-        }
+    if (n_ph) {  // photoelectron / at-rest annihilation photons
+      const uint32_t j0 = br.wbase[phase][warp][4] + pre_ph;
+#pragma unroll
+      for (int kk = 0; kk < (MODE == MODE_GAMMA ? 1 : 2); ++kk) {
+        if (!(kk == 0 ? ph0 : ph1)) continue;
+        const uint32_t j = j0 + ((kk == 1 && ph0) ? 1u : 0u);
+        if (j < c.capacity) store_track(slot.buf[parity ^ 1][kSecSpecies], j, make_secondary(o, kk, in.event, u));
+        else cnt->overflow.v = 1;
       }
     }
   }
@@ -433,8 +439,8 @@ interact_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlo
     for (int w = ADEPT_OUT_COMPTON; w <= ADEPT_OUT_ANNI; ++w) tally_outcome(tally, active, o.outcome, w);
     tally_outcome(tally, active, o.outcome, ADEPT_OUT_CLOSED);
 
-    const int s0 = (active && o.n_sec > 0) ? o.sec[0].species : -1;
-    const int s1 = (active && o.n_sec > 1) ? o.sec[1].species : -1;
+    const int s0 = active ? o.sec[0].species : -1;
+    const int s1 = active ? o.sec[1].species : -1;
     const bool live = active && o.alive;
     uint32_t want[3], first[3];
 #pragma unroll
@@ -529,15 +535,17 @@ __global__ void __launch_bounds__(kBlock) frozen_kernel(const __grid_constant__ 
     r.s = o.s; r.edep_dep = o.edep_dep; r.edep_cut = o.edep_cut; r.escaped = o.escaped; r.killed = o.killed;
     Stream u;
     u.init(t.event, c.seed, t.id, t.step);
-    for (int k = 0; k < 2; ++k) {
-      adept_track& s = sec[2 * i + k];
-      s = adept_track{};
-      if (k < o.n_sec) {
-        s.pos[0] = o.post.x; s.pos[1] = o.post.y; s.pos[2] = o.post.z;
-        s.dir[0] = o.sec[k].dx; s.dir[1] = o.sec[k].dy; s.dir[2] = o.sec[k].dz;
-        s.ekin = o.sec[k].ekin; s.id = u.child_id(o.sec[k].child); s.event = t.event; s.step = 0;
-        s.volume = o.post.vol; s.species = o.sec[k].species;
-      }
+    sec[2 * i] = adept_track{};
+    sec[2 * i + 1] = adept_track{};
+    int n_out = 0;
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {      // created secondaries, in child order, packed at the front
+      if (o.sec[k].species < 0) continue;
+      adept_track& s = sec[2 * i + n_out++];
+      s.pos[0] = o.post.x; s.pos[1] = o.post.y; s.pos[2] = o.post.z;
+      s.dir[0] = o.sec[k].dx; s.dir[1] = o.sec[k].dy; s.dir[2] = o.sec[k].dz;
+      s.ekin = o.sec[k].ekin; s.id = u.child_id(o.sec[k].child); s.event = t.event; s.step = 0;
+      s.volume = o.post.vol; s.species = o.sec[k].species;
     }
   }
 }

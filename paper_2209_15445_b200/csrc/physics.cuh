@@ -49,7 +49,7 @@ __device__ __forceinline__ double inverse_range(const DevCtx& c, const double* _
 
 // P10 rotation of d by polar (cos_t, sin_t) and azimuth phi = pi * phi_over_pi (sincospi reduces the
 // argument exactly).  One reciprocal each for 1/rho and the renormalisation.
-__device__ __noinline__ void rotate(const double d[3], double cos_t, double sin_t, double phi_over_pi, double out[3]) {
+__device__ __forceinline__ void rotate(const double d[3], double cos_t, double sin_t, double phi_over_pi, double out[3]) {
   const double rho2 = d[0] * d[0] + d[1] * d[1];
   double e1[3], e2[3];
   if (rho2 > 0.0) {
@@ -79,17 +79,20 @@ __device__ __forceinline__ void normalise(double v[3]) {
 }
 
 // M5: an e- below T_c or a gamma below k_c is not created (energy deposited locally); e+ always are.
-__device__ __forceinline__ void emit(const DevCtx& c, int mat, StepOut& o, int species, const double dir[3], double ekin,
-                                     uint32_t child) {
+// Child k of a process lives in the fixed slot o.sec[k] (species -1 = not created), so that StepOut is
+// only ever indexed statically and stays in registers.
+template <int CHILD>
+__device__ __forceinline__ void emit(const DevCtx& c, int mat, StepOut& o, int species, const double dir[3], double ekin) {
   const double cut = species == ADEPT_GAMMA ? mat_scalar(c, mat, S_KCUT) : mat_scalar(c, mat, S_TCUT);
   if (species != ADEPT_POSITRON && ekin < cut) { o.edep_cut += ekin; return; }
-  Secondary& s = o.sec[o.n_sec++];
+  Secondary& s = o.sec[CHILD];
   s.dx = dir[0]; s.dy = dir[1]; s.dz = dir[2];
-  s.ekin = ekin; s.species = species; s.child = child;
+  s.ekin = ekin; s.species = species; s.child = CHILD;
+  o.n_sec += 1;
 }
 
 // ---- P1 Klein-Nishina Compton
-__device__ __noinline__ void compton(const DevCtx& c, int mat, StepOut& o, Stream& u) {
+__device__ __forceinline__ void compton(const DevCtx& c, int mat, StepOut& o, Stream& u) {
   Track& g = o.post;
   const double k = g.ekin, kap = k / kMe;
   const double e0 = 1.0 / (1.0 + 2.0 * kap);
@@ -113,7 +116,7 @@ __device__ __noinline__ void compton(const DevCtx& c, int mat, StepOut& o, Strea
   if (Te >= mat_scalar(c, mat, S_TCUT)) {
     double de[3] = {k * d0[0] - k1 * d1[0], k * d0[1] - k1 * d1[1], k * d0[2] - k1 * d1[2]};
     normalise(de);
-    emit(c, mat, o, ADEPT_ELECTRON, de, Te, 0);
+    emit<0>(c, mat, o, ADEPT_ELECTRON, de, Te);
   } else {
     o.edep_cut += Te;
   }
@@ -123,7 +126,7 @@ __device__ __noinline__ void compton(const DevCtx& c, int mat, StepOut& o, Strea
 }
 
 // ---- P2 Bethe-Heitler pair, complete screening
-__device__ __noinline__ void pair_production(const DevCtx& c, int mat, StepOut& o, Stream& u) {
+__device__ __forceinline__ void pair_production(const DevCtx& c, int mat, StepOut& o, Stream& u) {
   Track& g = o.post;
   const double k = g.ekin, a = kMe / k;
   const double fmax_ = 1.0 - (4.0 / 3.0) * a * (1.0 - a);
@@ -143,8 +146,8 @@ __device__ __noinline__ void pair_production(const DevCtx& c, int mat, StepOut& 
   rotate(d0, cs, sn, phi, dm);
   sincos(thp, &sn, &cs);
   rotate(d0, cs, sn, phi + 1.0, dp);
-  emit(c, mat, o, ADEPT_ELECTRON, dm, Tm, 0);
-  emit(c, mat, o, ADEPT_POSITRON, dp, Tp, 1);
+  emit<0>(c, mat, o, ADEPT_ELECTRON, dm, Tm);
+  emit<1>(c, mat, o, ADEPT_POSITRON, dp, Tp);
   o.alive = 0;
 }
 
@@ -155,7 +158,7 @@ __device__ void photoelectric(const DevCtx& c, int mat, StepOut& o) {
   if (k > BK) {
     o.edep_cut += BK;
     const double d0[3] = {g.dx, g.dy, g.dz};
-    emit(c, mat, o, ADEPT_ELECTRON, d0, k - BK, 0);
+    emit<0>(c, mat, o, ADEPT_ELECTRON, d0, k - BK);
   } else {
     o.edep_cut += k;
   }
@@ -163,7 +166,7 @@ __device__ void photoelectric(const DevCtx& c, int mat, StepOut& o) {
 }
 
 // ---- P4 bremsstrahlung; false when kinematically closed
-__device__ __noinline__ bool bremsstrahlung(const DevCtx& c, int mat, StepOut& o, Stream& u) {
+__device__ __forceinline__ bool bremsstrahlung(const DevCtx& c, int mat, StepOut& o, Stream& u) {
   Track& e = o.post;
   const double T = e.ekin, kc = mat_scalar(c, mat, S_KCUT);
   if (!(T > kc)) return false;
@@ -182,7 +185,7 @@ __device__ __noinline__ bool bremsstrahlung(const DevCtx& c, int mat, StepOut& o
   double dg[3], sn, cs;
   sincos(th, &sn, &cs);
   rotate(d0, cs, sn, phi, dg);
-  emit(c, mat, o, ADEPT_GAMMA, dg, k, 0);
+  emit<0>(c, mat, o, ADEPT_GAMMA, dg, k);
   e.ekin = T - k;
   return true;
 }
@@ -198,13 +201,13 @@ __device__ __forceinline__ void delta_ray(const DevCtx& c, int mat, StepOut& o, 
   const double p = momentum(T), pd = momentum(Td);
   double dn[3] = {p * d0[0] - pd * dd[0], p * d0[1] - pd * dd[1], p * d0[2] - pd * dd[2]};
   normalise(dn);
-  emit(c, mat, o, ADEPT_ELECTRON, dd, Td, 0);
+  emit<0>(c, mat, o, ADEPT_ELECTRON, dd, Td);
   e.dx = dn[0]; e.dy = dn[1]; e.dz = dn[2];
   e.ekin = T - Td;
 }
 
 // ---- P5 Moller
-__device__ __noinline__ bool moller(const DevCtx& c, int mat, StepOut& o, Stream& u) {
+__device__ __forceinline__ bool moller(const DevCtx& c, int mat, StepOut& o, Stream& u) {
   const double T = o.post.ekin, Tc = mat_scalar(c, mat, S_TCUT);
   if (!(T > 2.0 * Tc)) return false;
   const double g = 1.0 + T / kMe, g2 = g * g;
@@ -224,7 +227,7 @@ __device__ __noinline__ bool moller(const DevCtx& c, int mat, StepOut& o, Stream
 }
 
 // ---- P6 Bhabha
-__device__ __noinline__ bool bhabha(const DevCtx& c, int mat, StepOut& o, Stream& u) {
+__device__ __forceinline__ bool bhabha(const DevCtx& c, int mat, StepOut& o, Stream& u) {
   const double T = o.post.ekin, Tc = mat_scalar(c, mat, S_TCUT);
   if (!(T > Tc)) return false;
   const double g = 1.0 + T / kMe;
@@ -246,7 +249,7 @@ __device__ __noinline__ bool bhabha(const DevCtx& c, int mat, StepOut& o, Stream
 }
 
 // ---- P8 annihilation in flight (Heitler)
-__device__ __noinline__ void annihilation(const DevCtx& c, int mat, StepOut& o, Stream& u) {
+__device__ __forceinline__ void annihilation(const DevCtx& c, int mat, StepOut& o, Stream& u) {
   Track& e = o.post;
   const double T = e.ekin, g = 1.0 + T / kMe;
   const double root = sqrt((g - 1.0) / (g + 1.0));
@@ -270,21 +273,21 @@ __device__ __noinline__ void annihilation(const DevCtx& c, int mat, StepOut& o, 
   const double p = momentum(T);
   double d2[3] = {p * d0[0] - k1 * d1[0], p * d0[1] - k1 * d1[1], p * d0[2] - k1 * d1[2]};
   normalise(d2);
-  emit(c, mat, o, ADEPT_GAMMA, d1, k1, 0);
-  emit(c, mat, o, ADEPT_GAMMA, d2, k2, 1);
+  emit<0>(c, mat, o, ADEPT_GAMMA, d1, k1);
+  emit<1>(c, mat, o, ADEPT_GAMMA, d2, k2);
   o.alive = 0;
 }
 
 // ---- P8 at rest: two photons of energy m back to back, cos(theta) = 2 U4 - 1, phi = 2 pi U5
-__device__ __noinline__ void annihilation_at_rest(const DevCtx& c, int mat, StepOut& o, Stream& u) {
+__device__ __forceinline__ void annihilation_at_rest(const DevCtx& c, int mat, StepOut& o, Stream& u) {
   const double u4 = u.uniform(4), u5 = u.uniform(5);
   const double cos_t = 2.0 * u4 - 1.0, sin_t = sqrt(fmax(0.0, 1.0 - cos_t * cos_t));
   double sp, cp;
   sincospi(2.0 * u5, &sp, &cp);
   const double d1[3] = {sin_t * cp, sin_t * sp, cos_t};
   const double d2[3] = {-d1[0], -d1[1], -d1[2]};
-  emit(c, mat, o, ADEPT_GAMMA, d1, kMe, 0);
-  emit(c, mat, o, ADEPT_GAMMA, d2, kMe, 1);
+  emit<0>(c, mat, o, ADEPT_GAMMA, d1, kMe);
+  emit<1>(c, mat, o, ADEPT_GAMMA, d2, kMe);
 }
 
 // Runs one discrete process on the state in o.post with uniforms U8.. of the parent's stream.

@@ -165,6 +165,11 @@ __device__ int step_move(const DevCtx& c, int nav, bool active, const Track& in,
     process = ADEPT_OUT_PHOTO;
     if (u1 * stot < x0) process = ADEPT_OUT_COMPTON;
     else if (u1 * stot < x0 + x1) process = ADEPT_OUT_PAIR;
+    if (process == ADEPT_OUT_PHOTO) {  // no sampling involved: done here rather than staged (12 % of all steps)
+      photoelectric(c, mat, o);
+      o.outcome = ADEPT_OUT_PHOTO;
+      return NEXT_NONE;
+    }
   } else {
     process = ADEPT_OUT_BREM;
     if (u1 * stot < x0) process = ADEPT_OUT_BREM;
