@@ -9,6 +9,7 @@
 #include <vector>
 
 #include "kernels.cuh"
+#include "gamma.cuh"
 
 using namespace adept;
 
@@ -391,7 +392,11 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   {
     const bool bvh = cfg->navigator == ADEPT_NAV_BVH && !hb.empty();
+#ifdef ADEPT_GAMMA_GENERIC   // the generic move kernel (step_move<MODE_GAMMA>), kept for A/B measurements
     ctx->k_move_gamma = bvh ? move_kernel<MODE_GAMMA, ADEPT_FIELD_NONE, true> : move_kernel<MODE_GAMMA, ADEPT_FIELD_NONE, false>;
+#else
+    ctx->k_move_gamma = bvh ? gamma_move_kernel<true> : gamma_move_kernel<false>;
+#endif
     switch (f->kind) {
       case ADEPT_FIELD_NONE:
         ctx->k_move_charged = bvh ? move_kernel<MODE_CHARGED, ADEPT_FIELD_NONE, true> : move_kernel<MODE_CHARGED, ADEPT_FIELD_NONE, false>; break;

@@ -1,0 +1,207 @@
+// Gamma move kernel, hand-specialised (§8(c) S1).
+//
+// Same arithmetic, in the same order, as step_move<MODE_GAMMA> (step.cuh), which stays the reference
+// implementation behind the frozen-step hook.  What differs is where the track lives: the step kernels
+// are bound by instruction latency at 4 resident warps per scheduler (profiles/r1b_summary.md), and the
+// resident warps are set by registers.  Here a lane's track stays in its slot of the shared-memory tile
+// the TMA pipeline filled and every phase reads only the fields it needs, at the point of use; the two
+// navigator calls (not inlined) are the fences between phases, so nothing but the position, the step
+// length and three flags is live across them.  The discrete process is chosen (U1) before the
+// propagation -- it depends on nothing the propagation computes -- so neither the cross sections nor
+// the Philox state survive phase A.
+#pragma once
+#include "kernels.cuh"
+
+namespace adept {
+
+#ifndef ADEPT_MINB_G2
+#define ADEPT_MINB_G2 5
+#endif
+
+// per-thread outcome counters, 10 bits per field, folded into the block tally every 1023 tiles
+enum { GC_STEPS = 0, GC_BOUNDARY, GC_ESCAPED, GC_STOPPED, GC_KILLED, GC_PHOTO, GC_N };
+
+__device__ __forceinline__ void gamma_counts_flush(BlockTally& t, unsigned long long& packed) {
+  constexpr int which[GC_N] = {-1, ADEPT_OUT_BOUNDARY, ADEPT_OUT_ESCAPED, ADEPT_OUT_STOPPED, ADEPT_OUT_KILLED, ADEPT_OUT_PHOTO};
+#pragma unroll
+  for (int f = 0; f < GC_N; ++f) {
+    const unsigned v = __reduce_add_sync(kFull, static_cast<unsigned>((packed >> (10 * f)) & 1023ull));
+    if ((threadIdx.x & 31) == 0 && v) {
+      if (f == GC_STEPS) atomicAdd(&t.steps, v);
+      else atomicAdd(&t.outcomes[which[f]], v);
+    }
+  }
+  packed = 0;
+}
+
+template <bool BVH>
+__global__ void __launch_bounds__(kBlock, ADEPT_MINB_G2)
+gamma_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot, int parity) {
+  constexpr int species = ADEPT_GAMMA;
+  enum { FATE_NONE = 0, FATE_KILLED, FATE_STOPPED, FATE_GO };
+  const TrackSoA& cur = slot.buf[parity][species];
+  SlotCounters* cnt = slot.counters;
+  const uint32_t n = cnt->count[parity][species].v;
+
+  // destinations: 0 = next gamma buffer, 1..3 = Compton / pair / (unused) staging queues, 4 = next
+  // electron buffer (photoelectrons)
+  constexpr int ND = 5;
+  __shared__ BlockTally tally;
+  __shared__ BlockReserve<ND> br;
+  __shared__ TilePipe pipe;
+  tally_init(tally);
+  pipe_init(pipe);
+  double sum_cut = 0.0;
+  unsigned long long packed = 0;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned lt = (1u << lane) - 1u;
+  const int t = threadIdx.x;
+
+  const uint32_t n_tiles = (n + kBlock - 1) / kBlock;
+  if (t == 0 && blockIdx.x < n_tiles) tile_issue(pipe.tile[0], cur, blockIdx.x, &pipe.bar[0]);
+  uint32_t k = 0;
+  for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++k) {
+    const int phase = k & 1;
+    if (t == 0 && tile + gridDim.x < n_tiles) tile_issue(pipe.tile[phase ^ 1], cur, tile + gridDim.x, &pipe.bar[phase ^ 1]);
+    mbar_wait(&pipe.bar[phase], (k >> 1) & 1);
+    const TrackTile& T = pipe.tile[phase];
+    const uint32_t vol = T.u[2][t];
+    const bool active = tile * kBlock + t < n && vol != kDeadVolume;
+
+    // ---- phase A: step-start rules, physics step limit, process choice (S1, A2)
+    int fate = FATE_NONE, process = 0, mat = 0;
+    double s_phys = ADEPT_INF;
+    if (active) {
+      const uint32_t step = T.u[1][t];
+      const double T0 = T.d[6][t];
+      if (step >= c.max_steps) {
+        fate = FATE_KILLED;
+      } else if (T0 < kTmin) {
+        fate = FATE_STOPPED;
+      } else {
+        fate = FATE_GO;
+        mat = volume(c, vol).material;
+        if (mat_scalar(c, mat, S_VACUUM) == 0.0) {
+          const GridPos gp = grid_pos(c, T0);
+          const double* tab = c.tab_g + static_cast<size_t>(mat) * kNGrid * kRowG;
+          const double x0 = interp(tab, kRowG, 0, gp);                                 // Compton
+          const double x1 = T0 > 2.0 * kMe ? interp(tab, kRowG, 1, gp) : 0.0;          // pair, exact threshold (P2)
+          const double se = interp(tab, kRowG, 2, gp);                                 // photoelectric
+          const double stot = x0 + x1 + se;
+          if (stot > 0.0) {
+            Stream u;
+            u.init(T.u[0][t], c.seed, T.id[t], step);
+            s_phys = div_pos(-log_pos(u.uniform(0)), stot);
+            const double u1 = u.uniform(1);
+            process = ADEPT_OUT_PHOTO;
+            if (u1 * stot < x0) process = ADEPT_OUT_COMPTON;
+            else if (u1 * stot < x0 + x1) process = ADEPT_OUT_PAIR;
+          }
+        }
+      }
+    }
+    const bool go = fate == FATE_GO;
+
+    // ---- phase B: straight-line propagation to min(s_phys, boundary) (A4), push (G5)
+    double px = T.d[0][t], py = T.d[1][t], pz = T.d[2][t];
+    bool cross = false;
+    {
+      const double dx = T.d[3][t], dy = T.d[4][t], dz = T.d[5][t];
+      const double s_geo = nav_distance<BVH>(c, c.navigator, go, px, py, pz, dx, dy, dz, vol, s_phys);
+      if (go) {
+        cross = s_geo < s_phys;
+        const double s = cross ? s_geo : s_phys;
+        px += s * dx; py += s * dy; pz += s * dz;
+        if (cross) { px += c.eps_push * dx; py += c.eps_push * dy; pz += c.eps_push * dz; }
+      }
+    }
+    // ---- phase C: relocation (A5)
+    const int nv = nav_relocate<BVH>(c, c.navigator, cross, vol, px, py, pz);
+
+    // ---- outcome.  Everything still needed of the track is read from the tile here, before the
+    // reservation barriers: after them thread 0 may already refill this tile buffer.
+    Track post;
+    post.x = px; post.y = py; post.z = pz;
+    post.dx = T.d[3][t]; post.dy = T.d[4][t]; post.dz = T.d[5][t];
+    post.ekin = T.d[6][t]; post.id = T.id[t];
+    post.event = T.u[0][t]; post.step = T.u[1][t] + 1; post.vol = vol; post.species = species;
+    double edep = 0.0, T_pe = 0.0;
+    bool live = false, has_pe = false;
+    int dest = -1;
+    if (active) {
+      packed += 1ull << (10 * GC_STEPS);
+      if (fate == FATE_KILLED) {
+        atomicAdd(&tally.ledger[3], post.ekin);
+        packed += 1ull << (10 * GC_KILLED);
+      } else if (fate == FATE_STOPPED) {
+        edep = post.ekin;
+        packed += 1ull << (10 * GC_STOPPED);
+      } else if (cross) {
+        if (nv < 0) {
+          atomicAdd(&tally.ledger[2], post.ekin);
+          record_leak(c, slot, post, species);
+          packed += 1ull << (10 * GC_ESCAPED);
+        } else {
+          post.vol = static_cast<uint32_t>(nv);
+          live = true; dest = 0;
+          packed += 1ull << (10 * GC_BOUNDARY);
+        }
+      } else if (process == ADEPT_OUT_PHOTO) {   // P3: no sampling involved, done here rather than staged
+        const double BK = mat_scalar(c, mat, S_BK);
+        if (post.ekin > BK) {
+          edep = BK;
+          T_pe = post.ekin - BK;
+          if (T_pe < mat_scalar(c, mat, S_TCUT)) edep += T_pe;   // M5: below the production cut
+          else has_pe = true;
+        } else {
+          edep = post.ekin;
+        }
+        packed += 1ull << (10 * GC_PHOTO);
+      } else {                                   // Compton / pair: staged for the interaction kernel
+        live = true; dest = 1 + process - ADEPT_OUT_COMPTON;
+      }
+    }
+    score(slot.edep, vol, edep, active);
+    sum_cut += edep;
+
+    // ---- reservation and stores (A0)
+    uint32_t pre = 0;
+#pragma unroll
+    for (int d = 0; d < 4; ++d) {
+      const unsigned b = __ballot_sync(kFull, dest == d);
+      if (dest == d) pre = __popc(b & lt);
+      if (lane == 0) br.wtot[phase][warp][d] = __popc(b);
+    }
+    const unsigned bpe = __ballot_sync(kFull, has_pe);
+    const uint32_t pre_pe = __popc(bpe & lt);
+    if (lane == 0) {
+      br.wtot[phase][warp][4] = __popc(bpe);
+      if (bpe) atomicAdd(&tally.secondaries[ADEPT_ELECTRON], static_cast<unsigned>(__popc(bpe)));
+    }
+    block_reserve_commit<ND>(br, phase, [&](int d) -> uint32_t* {
+      if (d == 0) return &cnt->count[parity ^ 1][species].v;
+      if (d == 4) return &cnt->count[parity ^ 1][ADEPT_ELECTRON].v;
+      return &cnt->n_stage[d - 1].v;
+    });
+    if (live) {
+      const uint32_t j = br.wbase[phase][warp][dest] + pre;
+      const bool staged = dest != 0;
+      const TrackSoA& dst = staged ? slot.stage[dest - 1] : slot.buf[parity ^ 1][species];
+      if (j < (staged ? c.stage_capacity : c.capacity)) store_track(dst, j, post);
+      else cnt->overflow.v = 1;
+    }
+    if (has_pe) {   // photoelectron along the photon direction, child 0 of this step's stream (R3)
+      const uint32_t j = br.wbase[phase][warp][4] + pre_pe;
+      Stream u;
+      u.init(post.event, c.seed, post.id, post.step - 1);
+      post.ekin = T_pe; post.id = u.child_id(0); post.step = 0; post.species = ADEPT_ELECTRON;
+      if (j < c.capacity) store_track(slot.buf[parity ^ 1][ADEPT_ELECTRON], j, post);
+      else cnt->overflow.v = 1;
+    }
+    if ((k & 1023u) == 1022u) gamma_counts_flush(tally, packed);
+  }
+  gamma_counts_flush(tally, packed);
+  tally_flush(tally, slot, species, 0.0, sum_cut);
+}
+
+}  // namespace adept

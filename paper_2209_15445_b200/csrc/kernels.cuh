@@ -10,7 +10,10 @@
 
 namespace adept {
 
-constexpr int kBlock = 128;
+#ifndef ADEPT_BLOCK
+#define ADEPT_BLOCK 128
+#endif
+constexpr int kBlock = ADEPT_BLOCK;
 constexpr int kWarps = kBlock / 32;
 // minimum resident blocks per SM asked of the compiler (register caps chosen from measurement)
 #ifndef ADEPT_MINB_G

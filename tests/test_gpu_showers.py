@@ -92,6 +92,53 @@ def test_config3_uniform_field(ob, calo, species):
     assert st.chords > 0
 
 
+def test_config4_full_barrel_showers(ob, barrel_full):
+    """BASELINE.json:configs[3] on the FULL barrel (61 200 crystals, 10 Si shells, solenoid map, RK4, BVH
+    navigator) at reduced energies so the loop-navigator oracle finishes in seconds: 3 events of 4 e-/gamma
+    primaries, 0.2-2 GeV log-uniform, isotropic in phi, |eta| < 1.4.  Identical Philox streams: every event
+    must reproduce the oracle's per-volume deposits, step counts and leaked energy."""
+    import torch
+    from paper_2209_15445_b200 import adept
+    from paper_2209_15445_b200.inputs import field, primaries
+    g, _, tabs, scal = barrel_full
+    fld = field.solenoid_map()
+    n_ev, n_per = 3, 4
+    prim = primaries.barrel_events(n_ev, n_per, 200.0, 2000.0, mode="cfg4")
+    o = ob.Oracle(g, tabs, scal, fld)
+    tr = o.make_tracks(prim)
+    o_ev, o_led, o_steps, o_outcomes = np.zeros((n_ev, g.n_volumes)), [], np.zeros(3, dtype=np.int64), None
+    for e in range(n_ev):
+        _, led_e, st_e = o.run(tr[tr["event"] == e], o_ev[e])
+        o_led.append(led_e)
+        o_steps += np.array(list(st_e.steps), dtype=np.int64)
+        o_outcomes = np.array(list(st_e.outcomes), dtype=np.int64) + (0 if o_outcomes is None else o_outcomes)
+    a = adept.Adept(g, tabs, scal, fld, track_capacity=1 << 16, n_event_slots=n_ev + 1, sync_interval=8)
+    same = 0
+    for e in range(n_ev):
+        sel = prim["event"] == e
+        a.enqueue_primaries(e, e, prim["species"][sel], prim["pos"][sel], prim["dir"][sel], prim["ekin"][sel])
+        a.transport(e, torch.cuda.current_stream())
+        hits, led = a.read_scoring(e)
+        assert abs(led.total() - led.primary) <= 1e-9 * led.primary
+        assert led.primary == pytest.approx(o_led[e].primary, rel=1e-14)
+        if np.allclose(hits, o_ev[e], rtol=1e-8, atol=1e-8):
+            same += 1
+            assert led.escaped == pytest.approx(o_led[e].escaped, rel=1e-9, abs=1e-9)
+        else:    # a threshold flip: the shower legitimately diverges, totals stay statistically close
+            assert hits.sum() == pytest.approx(o_ev[e].sum(), rel=0.05)
+    assert same >= n_ev - 1
+    # all events in one population: counts of every outcome equal the oracle's
+    a.enqueue(prim, slot=n_ev)
+    a.transport(n_ev, torch.cuda.current_stream())
+    hits, led = a.read_scoring(n_ev)
+    st = a.stats(n_ev)
+    a.close()
+    if same == n_ev:
+        assert list(st.steps) == list(o_steps) and list(st.outcomes) == list(o_outcomes)
+        np.testing.assert_allclose(hits, o_ev.sum(axis=0), rtol=1e-8, atol=1e-8)
+    assert st.chords > 0 and hits[12:].sum() > 0          # RK4 chords ran, crystals were hit
+
+
 @pytest.mark.parametrize("navigator", [1, 0])
 def test_config5_concurrent_events_on_streams(ob, barrel_patch, navigator):
     """BASELINE.json:configs[4] on the crystal patch: 16 events on 16 CUDA streams, per-event per-volume hits
