@@ -260,7 +260,14 @@ size_t carve(void* base, const adept_config* cfg, const adept_geometry* g, int n
       for (int sp = 0; sp < 3; ++sp) take_soa(d.buf[p][sp], cap);
     for (int q = 0; q < kNumStage; ++q) take_soa(d.stage[q], scap);
     d.counters = cv.take<SlotCounters>(1);
-    d.edep = cv.take<double>(g->n_volumes);
+    {  // replicated scoring arrays (kernels.cuh: score): up to 64 replicas within 2 MiB per slot
+      const uint32_t stride = (static_cast<uint32_t>(g->n_volumes) + 15u) & ~15u;
+      uint32_t rep = 64;
+      while (rep > 1 && static_cast<size_t>(rep) * stride * sizeof(double) > (2u << 20)) rep >>= 1;
+      d.edep = cv.take<double>(static_cast<size_t>(rep) * stride);
+      d.edep_stride = stride;
+      d.edep_mask = rep - 1;
+    }
     d.ledger = cv.take<double>(8);
     d.stats = cv.take<DevStats>(1);
     d.leaked = cv.take<adept_track>(std::max<size_t>(cfg->leak_capacity, 1));
@@ -580,6 +587,7 @@ extern "C" int adept_read_scoring(adept_ctx* ctx, int slot, double* edep, size_t
   if (edep && n_volumes != static_cast<size_t>(ctx->n_vol)) return fail(ADEPT_EINVAL, "n_volumes is %zu, geometry has %d", n_volumes, ctx->n_vol);
   SlotHost& sh = ctx->slots[slot];
   cudaStream_t st = static_cast<cudaStream_t>(stream);
+  fold_edep_kernel<<<(ctx->n_vol + 255) / 256, 256, 0, st>>>(sh.dev, ctx->n_vol);
   if (edep) CUDA_TRY(cudaMemcpyAsync(edep, sh.dev.edep, n_volumes * sizeof(double), cudaMemcpyDeviceToHost, st));
   double led[5];
   CUDA_TRY(cudaMemcpyAsync(led, sh.dev.ledger, sizeof(led), cudaMemcpyDeviceToHost, st));

@@ -34,39 +34,24 @@ __device__ __forceinline__ void gamma_counts_flush(BlockTally& t, unsigned long 
   packed = 0;
 }
 
-template <bool BVH>
-__global__ void __launch_bounds__(kBlock, ADEPT_MINB_G2)
-gamma_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot, int parity) {
+// One gamma step of lane `t` of a tile (phases A-C and the outcome); warp-convergent.  On return `post`
+// is the state to store if `live` (dest 0 = next gamma buffer, 1.. = staging queue of the process), and
+// (has_pe, T_pe) describe the photoelectron.
+struct GammaLane {
+  Track post;
+  double edep, T_pe;
+  bool active, live, has_pe;
+  int dest;
+  uint32_t vol;   // pre-step volume (scoring)
+};
+
+template <bool BVH, int N>
+__device__ __forceinline__ void gamma_lane(const DevCtx& c, const DevSlot& slot, BlockTally& tally, const TrackTileT<N>& T, int t,
+                                           bool in_range, unsigned long long& packed, GammaLane& r) {
   constexpr int species = ADEPT_GAMMA;
   enum { FATE_NONE = 0, FATE_KILLED, FATE_STOPPED, FATE_GO };
-  const TrackSoA& cur = slot.buf[parity][species];
-  SlotCounters* cnt = slot.counters;
-  const uint32_t n = cnt->count[parity][species].v;
-
-  // destinations: 0 = next gamma buffer, 1..3 = Compton / pair / (unused) staging queues, 4 = next
-  // electron buffer (photoelectrons)
-  constexpr int ND = 5;
-  __shared__ BlockTally tally;
-  __shared__ BlockReserve<ND> br;
-  __shared__ TilePipe pipe;
-  tally_init(tally);
-  pipe_init(pipe);
-  double sum_cut = 0.0;
-  unsigned long long packed = 0;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const unsigned lt = (1u << lane) - 1u;
-  const int t = threadIdx.x;
-
-  const uint32_t n_tiles = (n + kBlock - 1) / kBlock;
-  if (t == 0 && blockIdx.x < n_tiles) tile_issue(pipe.tile[0], cur, blockIdx.x, &pipe.bar[0]);
-  uint32_t k = 0;
-  for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++k) {
-    const int phase = k & 1;
-    if (t == 0 && tile + gridDim.x < n_tiles) tile_issue(pipe.tile[phase ^ 1], cur, tile + gridDim.x, &pipe.bar[phase ^ 1]);
-    mbar_wait(&pipe.bar[phase], (k >> 1) & 1);
-    const TrackTile& T = pipe.tile[phase];
     const uint32_t vol = T.u[2][t];
-    const bool active = tile * kBlock + t < n && vol != kDeadVolume;
+    const bool active = in_range && vol != kDeadVolume;
 
     // ---- phase A: step-start rules, physics step limit, process choice (S1, A2)
     int fate = FATE_NONE, process = 0, mat = 0;
@@ -161,7 +146,46 @@ gamma_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevS
         live = true; dest = 1 + process - ADEPT_OUT_COMPTON;
       }
     }
-    score(slot.edep, vol, edep, active);
+    r.post = post; r.edep = edep; r.T_pe = T_pe; r.active = active; r.live = live; r.has_pe = has_pe; r.dest = dest; r.vol = vol;
+}
+
+template <bool BVH>
+__global__ void __launch_bounds__(kBlock, ADEPT_MINB_G2)
+gamma_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot, int parity) {
+  constexpr int species = ADEPT_GAMMA;
+  const TrackSoA& cur = slot.buf[parity][species];
+  SlotCounters* cnt = slot.counters;
+  const uint32_t n = cnt->count[parity][species].v;
+
+  // destinations: 0 = next gamma buffer, 1..3 = Compton / pair / (unused) staging queues, 4 = next
+  // electron buffer (photoelectrons)
+  constexpr int ND = 5;
+  __shared__ BlockTally tally;
+  __shared__ BlockReserve<ND> br;
+  __shared__ TilePipe pipe;
+  tally_init(tally);
+  pipe_init(pipe);
+  double sum_cut = 0.0;
+  unsigned long long packed = 0;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned lt = (1u << lane) - 1u;
+  const int t = threadIdx.x;
+
+  const uint32_t n_tiles = (n + kBlock - 1) / kBlock;
+  if (t == 0 && blockIdx.x < n_tiles) tile_issue(pipe.tile[0], cur, blockIdx.x, &pipe.bar[0]);
+  uint32_t k = 0;
+  for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++k) {
+    const int phase = k & 1;
+    if (t == 0 && tile + gridDim.x < n_tiles) tile_issue(pipe.tile[phase ^ 1], cur, tile + gridDim.x, &pipe.bar[phase ^ 1]);
+    mbar_wait(&pipe.bar[phase], (k >> 1) & 1);
+    GammaLane r;
+    gamma_lane<BVH>(c, slot, tally, pipe.tile[phase], t, tile * kBlock + t < n, packed, r);
+    Track post = r.post;
+    const double edep = r.edep, T_pe = r.T_pe;
+    const bool active = r.active, live = r.live, has_pe = r.has_pe;
+    const int dest = r.dest;
+    const uint32_t vol = r.vol;
+    score(slot, vol, edep, active);
     sum_cut += edep;
 
     // ---- reservation and stores (A0)

@@ -56,13 +56,17 @@ __device__ __forceinline__ double warp_sum(double v) {
 // flight while the block computes tile k, so the HBM latency of the track state is hidden without
 // spending registers or occupancy on it.  Buffers are allocated in multiples of kBlock entries, so a
 // full tile can always be read (entries past the live count are ignored).
-struct alignas(128) TrackTile {
-  double d[7][kBlock];      // x, y, z, dx, dy, dz, ekin
-  uint64_t id[kBlock];
-  uint32_t u[3][kBlock];    // event, step, vol
+template <int N>
+struct alignas(128) TrackTileT {
+  double d[7][N];      // x, y, z, dx, dy, dz, ekin
+  uint64_t id[N];
+  uint32_t u[3][N];    // event, step, vol
+  static constexpr uint32_t kBytes = 8u * N * 8u + 3u * N * 4u;
 };
-constexpr uint32_t kTileBytes = 8u * kBlock * 8u + 3u * kBlock * 4u;
+using TrackTile = TrackTileT<kBlock>;
+constexpr uint32_t kTileBytes = TrackTile::kBytes;
 static_assert(sizeof(TrackTile) % 128 == 0 && sizeof(TrackTile) >= kTileBytes, "TrackTile layout");
+static_assert(sizeof(TrackTileT<32>) % 128 == 0 && sizeof(TrackTileT<32>) >= TrackTileT<32>::kBytes, "warp tile layout");
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
 
@@ -90,16 +94,17 @@ __device__ __forceinline__ void bulk_load(void* smem_dst, const void* gmem_src, 
                : "memory");
 }
 
-// issued by one thread: tile `tile` of buffer b -> shared tile t, completion on bar
-__device__ __forceinline__ void tile_issue(TrackTile& t, const TrackSoA& b, uint32_t tile, uint64_t* bar) {
-  const size_t base = static_cast<size_t>(tile) * kBlock;
-  mbar_expect_tx(bar, kTileBytes);
-  bulk_load(t.d[0], b.x + base, kBlock * 8, bar); bulk_load(t.d[1], b.y + base, kBlock * 8, bar);
-  bulk_load(t.d[2], b.z + base, kBlock * 8, bar); bulk_load(t.d[3], b.dx + base, kBlock * 8, bar);
-  bulk_load(t.d[4], b.dy + base, kBlock * 8, bar); bulk_load(t.d[5], b.dz + base, kBlock * 8, bar);
-  bulk_load(t.d[6], b.ekin + base, kBlock * 8, bar); bulk_load(t.id, b.id + base, kBlock * 8, bar);
-  bulk_load(t.u[0], b.event + base, kBlock * 4, bar); bulk_load(t.u[1], b.step + base, kBlock * 4, bar);
-  bulk_load(t.u[2], b.vol + base, kBlock * 4, bar);
+// issued by one thread: tile `tile` (N entries) of buffer b -> shared tile t, completion on bar
+template <int N>
+__device__ __forceinline__ void tile_issue(TrackTileT<N>& t, const TrackSoA& b, uint32_t tile, uint64_t* bar) {
+  const size_t base = static_cast<size_t>(tile) * N;
+  mbar_expect_tx(bar, TrackTileT<N>::kBytes);
+  bulk_load(t.d[0], b.x + base, N * 8, bar); bulk_load(t.d[1], b.y + base, N * 8, bar);
+  bulk_load(t.d[2], b.z + base, N * 8, bar); bulk_load(t.d[3], b.dx + base, N * 8, bar);
+  bulk_load(t.d[4], b.dy + base, N * 8, bar); bulk_load(t.d[5], b.dz + base, N * 8, bar);
+  bulk_load(t.d[6], b.ekin + base, N * 8, bar); bulk_load(t.id, b.id + base, N * 8, bar);
+  bulk_load(t.u[0], b.event + base, N * 4, bar); bulk_load(t.u[1], b.step + base, N * 4, bar);
+  bulk_load(t.u[2], b.vol + base, N * 4, bar);
 }
 
 __device__ __forceinline__ Track tile_read(const TrackTile& t, int k, int species) {
@@ -167,8 +172,14 @@ __device__ __forceinline__ void block_reserve(BlockReserve<ND>& br, int phase, c
 }
 
 // A9: warp-reduced scoring.  Lanes depositing into the same volume are combined (match_any) and the
-// group leader issues one fp64 atomic; with 100 scoring slabs most warps issue 1-3 atomics.
-__device__ __forceinline__ void score(double* edep, uint32_t vol, double e, bool active) {
+// group leader issues one fp64 atomic.  With 100 scoring slabs all deposits of a calorimeter fall on
+// seven 128 B lines, two or three of them hot at the shower maximum, and one L2 slice retires an fp64
+// atomic on one line every ~3.5 cycles: measured, the atomic unit of the hottest slice was busy 60 %
+// (gamma move) and 86 % (charged move) of the kernel time (profiles/r1c_summary.md) -- the two
+// concurrent step kernels were serialised by it.  The deposits therefore go to one of several replicas
+// of the array, chosen per warp, which spreads them over as many L2 slices; adept_read_scoring folds the
+// replicas in a fixed order.
+__device__ __forceinline__ void score(const DevSlot& slot, uint32_t vol, double e, bool active) {
   const bool has = active && e != 0.0;
   const unsigned hm = __ballot_sync(kFull, has);
   if (hm == 0 || !has) return;                      // lanes without a deposit take no part
@@ -181,7 +192,24 @@ __device__ __forceinline__ void score(double* edep, uint32_t vol, double e, bool
     m &= m - 1;
     sum += __shfl_sync(peers, e, src);
   }
-  if (lane == __ffs(peers) - 1) atomicAdd(edep + vol, sum);
+  if (lane == __ffs(peers) - 1) {
+    const uint32_t rep = (blockIdx.x * kWarps + (threadIdx.x >> 5)) & slot.edep_mask;
+    atomicAdd(slot.edep + static_cast<size_t>(rep) * slot.edep_stride + vol, sum);
+  }
+}
+
+// Folds the replicas into replica 0 (fixed order, so the result does not depend on scheduling) and
+// clears the others.
+__global__ void fold_edep_kernel(const __grid_constant__ DevSlot slot, int n_vol) {
+  const int v = blockIdx.x * blockDim.x + threadIdx.x;
+  if (v >= n_vol) return;
+  double s = slot.edep[v];
+  for (uint32_t r = 1; r <= slot.edep_mask; ++r) {
+    double* p = slot.edep + static_cast<size_t>(r) * slot.edep_stride + v;
+    s += *p;
+    *p = 0.0;
+  }
+  slot.edep[v] = s;
 }
 
 // Per-block statistics, folded into the slot's counters once at the end of the kernel.
@@ -303,7 +331,7 @@ move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot sl
     int process, mat;
     const int next = step_move<MODE, FIELD, BVH>(c, c.navigator, active, in, o, u, process, mat);
 
-    score(slot.edep, in.vol, o.edep_dep + o.edep_cut, active);
+    score(slot, in.vol, o.edep_dep + o.edep_cut, active);
     if (active) {
       sum_dep += o.edep_dep; sum_cut += o.edep_cut; chords += o.chords;
       if (o.killed != 0.0) atomicAdd(&tally.ledger[3], o.killed);
@@ -437,7 +465,7 @@ interact_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlo
       init_out(o, t, false);
       u.init(0, 0, 0, 0);
     }
-    score(slot.edep, t.vol, o.edep_cut, active);
+    score(slot, t.vol, o.edep_cut, active);
 #pragma unroll
     for (int w = ADEPT_OUT_COMPTON; w <= ADEPT_OUT_ANNI; ++w) tally_outcome(tally, active, o.outcome, w);
     tally_outcome(tally, active, o.outcome, ADEPT_OUT_CLOSED);

@@ -92,7 +92,9 @@ struct DevStats {
 struct DevSlot {
   TrackSoA buf[2][3];       // [parity][species]
   SlotCounters* counters;
-  double* edep;             // [n_volumes]
+  double* edep;             // [edep_replicas][edep_stride]: replicated per-volume deposits, folded by adept_read_scoring
+  uint32_t edep_stride;     // doubles per replica (n_volumes rounded up to a 128 B multiple)
+  uint32_t edep_mask;       // replicas - 1 (power of two)
   double* ledger;           // [5]: deposited, below_cut, escaped, killed, primary
   DevStats* stats;
   adept_track* leaked;      // [leak_capacity]
