@@ -211,10 +211,12 @@ int adept_step_frozen(adept_ctx*, int n, const adept_track* in, adept_step_resul
 int adept_distance_batch(adept_ctx*, int navigator, int n, const double* pos3, const double* dir3,
                          const uint32_t* volume, const double* s_max, double* out, void* cuda_stream);
 int adept_locate_batch(adept_ctx*, int navigator, int n, const double* pos3, int64_t* out, void* cuda_stream);
-/* Relocation as the move kernel does it after a boundary (climb from volume from[i] until the point is
- * inside, then descend): must equal adept_locate_batch for every starting volume. */
-int adept_relocate_batch(adept_ctx*, int navigator, int n, const double* pos3, const uint32_t* from, int64_t* out,
-                         void* cuda_stream);
+/* Relocation as the move kernel does it after a boundary (the hinted neighbour beyond exit face face[i]
+ * of box volume from[i] first -- face = 2 * axis + (direction > 0) in the volume's frame, -1 or a null
+ * array = no hint -- else climb from from[i] until the point is inside, then descend): must equal
+ * adept_locate_batch for every starting volume and every face, right or wrong. */
+int adept_relocate_batch(adept_ctx*, int navigator, int n, const double* pos3, const uint32_t* from,
+                         const int32_t* face, int64_t* out, void* cuda_stream);
 
 int adept_shutdown(adept_ctx*);
 

@@ -89,7 +89,7 @@ def load_library():
     lib.adept_step_frozen.argtypes = [vp, i, vp, vp, vp, vp]
     lib.adept_distance_batch.argtypes = [vp, i, i, vp, vp, vp, vp, vp, vp]
     lib.adept_locate_batch.argtypes = [vp, i, i, vp, vp, vp]
-    lib.adept_relocate_batch.argtypes = [vp, i, i, vp, vp, vp, vp]
+    lib.adept_relocate_batch.argtypes = [vp, i, i, vp, vp, vp, vp, vp]
     lib.adept_shutdown.argtypes = [vp]
     return lib
 
@@ -247,9 +247,11 @@ class Adept:
         _check(lib.adept_locate_batch(self.ctx, navigator, pos.shape[0], _ptr(pos), _ptr(out), None))
         return out
 
-    def relocate_batch(self, pos, from_volume, navigator=NAV_BVH):
+    def relocate_batch(self, pos, from_volume, navigator=NAV_BVH, face=None):
         pos = np.ascontiguousarray(pos, dtype=np.float64).reshape(-1, 3)
         frm = np.ascontiguousarray(np.broadcast_to(from_volume, (pos.shape[0],)), dtype=np.uint32)
+        fc = None if face is None else np.ascontiguousarray(np.broadcast_to(face, (pos.shape[0],)), dtype=np.int32)
         out = np.zeros(pos.shape[0], dtype=np.int64)
-        _check(lib.adept_relocate_batch(self.ctx, navigator, pos.shape[0], _ptr(pos), _ptr(frm), _ptr(out), None))
+        _check(lib.adept_relocate_batch(self.ctx, navigator, pos.shape[0], _ptr(pos), _ptr(frm),
+                                        None if fc is None else _ptr(fc), _ptr(out), None))
         return out

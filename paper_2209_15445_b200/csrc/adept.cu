@@ -210,7 +210,7 @@ int validate(const adept_config* cfg, const adept_geometry* g, int n_mats, const
 }
 
 struct Layout {
-  DevVolume* vol; double* rot; int32_t* rhint; DevBvh* bvh; double *tab_g, *tab_em, *tab_ep, *scal, *bz;
+  DevVolume* vol; double* rot; int32_t* nbr; int32_t* rhint; DevBvh* bvh; double *tab_g, *tab_em, *tab_ep, *scal, *bz;
   std::vector<double*> bvh_prim_box; std::vector<int32_t*> bvh_prim_vol; std::vector<std::vector<double*>> bvh_node_box;
   adept_track* stage; uint32_t* bad; size_t stage_cap;
   std::vector<DevSlot> slots;
@@ -223,6 +223,7 @@ size_t carve(void* base, const adept_config* cfg, const adept_geometry* g, int n
   Layout L{};
   L.vol = cv.take<DevVolume>(g->n_volumes);
   L.rot = cv.take<double>(9 * static_cast<size_t>(g->n_volumes));
+  L.nbr = cv.take<int32_t>(6 * static_cast<size_t>(g->n_volumes));
   std::vector<int> bvh_vols;
   for (int v = 0; v < g->n_volumes; ++v) if (g->daughter_count[v] >= kBvhMinDaughters) bvh_vols.push_back(v);
   L.bvh = cv.take<DevBvh>(std::max<size_t>(bvh_vols.size(), 1));
@@ -379,7 +380,7 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   ctx->cfg = *cfg;
   ctx->n_vol = nv; ctx->n_mat = n_mats;
   DevCtx& d = ctx->dev;
-  d.vol = L.vol; d.rot = L.rot; d.n_vol = nv; d.bvh = L.bvh; d.navigator = cfg->navigator;
+  d.vol = L.vol; d.rot = L.rot; d.nbr = L.nbr; d.n_vol = nv; d.bvh = L.bvh; d.navigator = cfg->navigator;
   d.tab_g = L.tab_g; d.tab_em = L.tab_em; d.tab_ep = L.tab_ep; d.scal = L.scal; d.rhint = L.rhint; d.n_mat = n_mats;
   d.field_kind = f->kind;
   for (int k = 0; k < 3; ++k) d.B[k] = f->B[k];
@@ -393,6 +394,11 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   d.stage_capacity = static_cast<uint32_t>(cfg->stage_capacity ? cfg->stage_capacity : cfg->track_capacity);
   d.leak_capacity = static_cast<uint32_t>(cfg->leak_capacity);
   ctx->d_stage = L.stage; ctx->d_bad = L.bad; ctx->stage_cap = L.stage_cap;
+
+  // ---- relocation hints: the volume beyond each face of each box (kernels.cuh hint_kernel)
+  hint_kernel<<<std::min((6 * nv + kBlock - 1) / kBlock, 4096), kBlock>>>(d, L.nbr);
+  CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(cudaDeviceSynchronize());
 
   int dev = 0, sms = 0, occ_g = 1, occ_c = 1, occ_i = 1;
   CUDA_TRY(cudaGetDevice(&dev));
@@ -698,23 +704,32 @@ extern "C" int adept_locate_batch(adept_ctx* ctx, int nav, int n, const double* 
   return ADEPT_OK;
 }
 
-extern "C" int adept_relocate_batch(adept_ctx* ctx, int nav, int n, const double* pos3, const uint32_t* from, int64_t* out,
-                                    void* stream) {
+extern "C" int adept_relocate_batch(adept_ctx* ctx, int nav, int n, const double* pos3, const uint32_t* from, const int32_t* face,
+                                    int64_t* out, void* stream) {
   if (!ctx || n < 0 || (n > 0 && (!pos3 || !from || !out))) return fail(ADEPT_EINVAL, "null argument");
   if (n == 0) return ADEPT_OK;
-  for (int i = 0; i < n; ++i) if (from[i] >= static_cast<uint32_t>(ctx->n_vol)) return fail(ADEPT_EINVAL, "point %d: volume out of range", i);
+  for (int i = 0; i < n; ++i) {
+    if (from[i] >= static_cast<uint32_t>(ctx->n_vol)) return fail(ADEPT_EINVAL, "point %d: volume out of range", i);
+    if (face && (face[i] < -1 || face[i] > 5)) return fail(ADEPT_EINVAL, "point %d: face out of range", i);
+  }
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   double* d_pos;
   uint32_t* d_from;
+  int32_t* d_face = nullptr;
   long long* d_out;
   CUDA_TRY(cudaMalloc(&d_pos, 3 * n * sizeof(double))); CUDA_TRY(cudaMalloc(&d_from, n * sizeof(uint32_t)));
   CUDA_TRY(cudaMalloc(&d_out, n * sizeof(long long)));
   CUDA_TRY(cudaMemcpyAsync(d_pos, pos3, 3 * n * sizeof(double), cudaMemcpyHostToDevice, st));
   CUDA_TRY(cudaMemcpyAsync(d_from, from, n * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
-  relocate_kernel<<<std::min((n + kBlock - 1) / kBlock, 65535), kBlock, 0, st>>>(ctx->dev, nav, n, d_pos, d_from, d_out);
+  if (face) {
+    CUDA_TRY(cudaMalloc(&d_face, n * sizeof(int32_t)));
+    CUDA_TRY(cudaMemcpyAsync(d_face, face, n * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  }
+  relocate_kernel<<<std::min((n + kBlock - 1) / kBlock, 65535), kBlock, 0, st>>>(ctx->dev, nav, n, d_pos, d_from, d_face, d_out);
   CUDA_TRY(cudaGetLastError());
   CUDA_TRY(cudaMemcpyAsync(out, d_out, n * sizeof(long long), cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
+  if (d_face) cudaFree(d_face);
   cudaFree(d_pos); cudaFree(d_from); cudaFree(d_out);
   return ADEPT_OK;
 }

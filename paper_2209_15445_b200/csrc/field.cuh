@@ -93,11 +93,11 @@ __device__ __noinline__ void rk4(const DevCtx& c, int charge, double pmom, doubl
 // FIELD >= 0 fixes the field kind at compile time (no helix / RK4 code where it cannot run); -1 = runtime.
 template <int FIELD = -1, bool BVH = true>
 __device__ int propagate(const DevCtx& c, int nav, bool active, int charge, double ekin, double pos[3], double dir[3],
-                         uint32_t vol, double s_phys, double& s_out, int& chords_out, double pushdir[3]) {
+                         uint32_t vol, double s_phys, double& s_out, int& chords_out, double pushdir[3], int& face_out) {
   const int field_kind = FIELD >= 0 ? FIELD : c.field_kind;
   const double pmom = sqrt(ekin * (ekin + 2.0 * kMe));
   double s_done = 0.0;
-  int chords = 0, flag = 0;
+  int chords = 0, flag = 0, face_hit = -1;
   bool running = active;
 #pragma unroll
   for (int i = 0; i < 3; ++i) pushdir[i] = dir[i];
@@ -142,8 +142,10 @@ __device__ int propagate(const DevCtx& c, int nav, bool active, int charge, doub
       }
     }
     // --- warp-cooperative geometry query of this segment
-    const double s_geo = nav_distance<BVH>(c, nav, query, pos[0], pos[1], pos[2], u[0], u[1], u[2], vol, L);
+    int face;
+    const double s_geo = nav_distance<BVH>(c, nav, query, pos[0], pos[1], pos[2], u[0], u[1], u[2], vol, L, face);
     if (query) {
+      face_hit = face;   // only meaningful when this segment ends on the boundary (flag 1), which ends the loop
       if (straight) {
         pushdir[0] = u[0]; pushdir[1] = u[1]; pushdir[2] = u[2];
         if (s_geo < rest) {
@@ -185,6 +187,7 @@ __device__ int propagate(const DevCtx& c, int nav, bool active, int charge, doub
   }
   s_out = s_done;
   chords_out = chords;
+  face_out = flag == 1 ? face_hit : -1;
   return flag;
 }
 

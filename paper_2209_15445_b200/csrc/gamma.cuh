@@ -90,9 +90,10 @@ __device__ __forceinline__ void gamma_lane(const DevCtx& c, const DevSlot& slot,
     // ---- phase B: straight-line propagation to min(s_phys, boundary) (A4), push (G5)
     double px = T.d[0][t], py = T.d[1][t], pz = T.d[2][t];
     bool cross = false;
+    int face = -1;
     {
       const double dx = T.d[3][t], dy = T.d[4][t], dz = T.d[5][t];
-      const double s_geo = nav_distance<BVH>(c, c.navigator, go, px, py, pz, dx, dy, dz, vol, s_phys);
+      const double s_geo = nav_distance<BVH>(c, c.navigator, go, px, py, pz, dx, dy, dz, vol, s_phys, face);
       if (go) {
         cross = s_geo < s_phys;
         const double s = cross ? s_geo : s_phys;
@@ -101,7 +102,7 @@ __device__ __forceinline__ void gamma_lane(const DevCtx& c, const DevSlot& slot,
       }
     }
     // ---- phase C: relocation (A5)
-    const int nv = nav_relocate<BVH>(c, c.navigator, cross, vol, px, py, pz);
+    const int nv = nav_relocate<BVH>(c, c.navigator, cross, vol, px, py, pz, face);
 
     // ---- outcome.  Everything still needed of the track is read from the tile here, before the
     // reservation barriers: after them thread 0 may already refill this tile buffer.

@@ -27,6 +27,14 @@ __device__ __forceinline__ void dir_to_local(const DevCtx& c, int vi, const DevV
   for (int i = 0; i < 3; ++i) l[i] = __ldg(R + i) * gx + __ldg(R + 3 + i) * gy + __ldg(R + 6 + i) * gz;
 }
 
+// global = t + R local (inverse of to_local)
+__device__ __forceinline__ void to_global(const DevCtx& c, int vi, const DevVolume& v, const double l[3], double g[3]) {
+  if (v.identity) { g[0] = v.t[0] + l[0]; g[1] = v.t[1] + l[1]; g[2] = v.t[2] + l[2]; return; }
+  const double* __restrict__ R = c.rot + 9 * static_cast<size_t>(vi);
+#pragma unroll
+  for (int j = 0; j < 3; ++j) g[j] = v.t[j] + __ldg(R + 3 * j) * l[0] + __ldg(R + 3 * j + 1) * l[1] + __ldg(R + 3 * j + 2) * l[2];
+}
+
 // ---------------------------------------------------------------- G1 solids
 __device__ __forceinline__ bool inside_solid(int solid, const double h[3], const double p[3]) {
   if (solid == ADEPT_BOX) return fabs(p[0]) <= h[0] && fabs(p[1]) <= h[1] && fabs(p[2]) <= h[2];
@@ -37,13 +45,15 @@ __device__ __forceinline__ bool inside_solid(int solid, const double h[3], const
 // min_i (sgn(d_i) h_i - p_i) / d_i over d_i != 0.  The three quotients n_i / |d_i| are compared by
 // cross-multiplication and only the smallest is divided (one division instead of three; when two are
 // within rounding of each other either is the minimum to 1 ulp).
-__device__ __forceinline__ double box_exit(const double h[3], const double p[3], const double d[3]) {
+// `face` receives the exit face, 2 * axis + (d[axis] > 0), or -1.
+__device__ __forceinline__ double box_exit(const double h[3], const double p[3], const double d[3], int& face) {
   double num = 1.0, den = 0.0;   // +inf as 1/0
+  face = -1;
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
     const double ad = fabs(d[i]);
     const double ni = h[i] - (d[i] > 0.0 ? p[i] : -p[i]);   // distance to the exit plane along the axis
-    if (ad != 0.0 && ni * den <= num * ad) { num = ni; den = ad; }
+    if (ad != 0.0 && ni * den <= num * ad) { num = ni; den = ad; face = 2 * i + (d[i] > 0.0 ? 1 : 0); }
   }
   return den != 0.0 ? fmax(num / den, 0.0) : ADEPT_INF;
 }
@@ -119,8 +129,10 @@ __device__ __forceinline__ double tube_entry(const double h[3], const double p[3
   return best;
 }
 
-__device__ __forceinline__ double solid_exit(const DevVolume& v, const double p[3], const double d[3]) {
-  return v.solid == ADEPT_BOX ? box_exit(v.dims, p, d) : tube_exit(v.dims, p, d);
+__device__ __forceinline__ double solid_exit(const DevVolume& v, const double p[3], const double d[3], int& face) {
+  if (v.solid == ADEPT_BOX) return box_exit(v.dims, p, d, face);
+  face = -1;
+  return tube_exit(v.dims, p, d);
 }
 __device__ __forceinline__ double solid_entry(const DevVolume& v, const double p[3], const double d[3]) {
   return v.solid == ADEPT_BOX ? box_entry(v.dims, p, d) : tube_entry(v.dims, p, d);
@@ -257,25 +269,34 @@ __device__ __noinline__ int bvh_point(const DevCtx& c, const DevBvh& b, double p
 // min(exit distance of the own solid, entry distance of every daughter), capped at s_max.
 // Warp-convergent call; lanes with active == false return s_max.
 // BVH = false instantiates the pure loop navigator (geometries without a BVH volume): no cooperative code.
+// `face` (out): when the returned distance is the exit of the volume's own box through one face and no
+// daughter is entered first, the face index 2 * axis + (direction > 0) in the volume's frame -- the key of
+// the relocation hint table (nav_relocate); -1 otherwise.
 template <bool BVH = true>
 __device__ __noinline__ double nav_distance(const DevCtx& c, int nav, bool active, double px, double py, double pz, double dx,
-                               double dy, double dz, uint32_t vol, double s_max) {
+                               double dy, double dz, uint32_t vol, double s_max, int& face) {
   const int lane = threadIdx.x & 31;
   double s = s_max;
   bool need = false;
   int bvh = -1;
+  face = -1;
   if (active) {
     const DevVolume& v = volume(c, vol);
     double lp[3], ld[3];
     to_local(c, vol, v, px, py, pz, lp);
     dir_to_local(c, vol, v, dx, dy, dz, ld);
-    s = fmin(s_max, solid_exit(v, lp, ld));
+    int f;
+    const double s_exit = solid_exit(v, lp, ld, f);
+    if (s_exit < s_max) { s = s_exit; face = f; }
     if (v.dcount > 0) {
       if (BVH && nav == ADEPT_NAV_BVH && v.bvh >= 0) {
         need = true;
         bvh = v.bvh;
       } else {
-        for (int k = 0; k < v.dcount; ++k) s = fmin(s, entry_distance(c, v.dbegin + k, px, py, pz, dx, dy, dz));
+        for (int k = 0; k < v.dcount; ++k) {
+          const double e = entry_distance(c, v.dbegin + k, px, py, pz, dx, dy, dz);
+          if (e <= s) { if (e < s) s = e; face = -1; }
+        }
       }
     }
   }
@@ -287,9 +308,15 @@ __device__ __noinline__ double nav_distance(const DevCtx& c, int nav, bool activ
     const double r = bvh_ray(c, c.bvh[__shfl_sync(kFull, bvh, src)], __shfl_sync(kFull, px, src),
                              __shfl_sync(kFull, py, src), __shfl_sync(kFull, pz, src), __shfl_sync(kFull, dx, src),
                              __shfl_sync(kFull, dy, src), __shfl_sync(kFull, dz, src), __shfl_sync(kFull, s, src));
-    if (lane == src) s = r;
+    if (lane == src && r < s) { s = r; face = -1; }
   }
   return s;
+}
+template <bool BVH = true>
+__device__ __forceinline__ double nav_distance(const DevCtx& c, int nav, bool active, double px, double py, double pz, double dx,
+                                               double dy, double dz, uint32_t vol, double s_max) {
+  int face;
+  return nav_distance<BVH>(c, nav, active, px, py, pz, dx, dy, dz, vol, s_max, face);
 }
 
 // ---------------------------------------------------------------- G4 Locate
@@ -355,14 +382,25 @@ __device__ __noinline__ int nav_locate(const DevCtx& c, int nav, bool active, do
 // first, which makes a crossing between consecutive layers of a stack O(1) instead of O(layers)
 // (relocation cost and "fewer trial steps").  Warp-convergent call when BVH is true.
 // Returns -1 outside the world or for inactive lanes.
+//
+// Hint table (DevCtx::nbr, built once by adept_init with hint_kernel): nbr[6 v + f] = Locate of the point
+// just outside the centre of face f of box volume v.  A track that left v through face f (nav_distance
+// reports f) is tested against that one candidate first; if the pushed point is inside it, the descent
+// starts there -- the deepest volume containing q is unique, so the answer is the same as the climb's --
+// and in a stack of slabs a crossing costs one containment test instead of four or five dependent ones.
 template <bool BVH = true>
 __device__ __noinline__ int nav_relocate(const DevCtx& c, int nav, bool active, uint32_t vol_old, double qx, double qy,
-                                         double qz) {
+                                         double qz, int face = -1) {
   int cur = -1, prev = -1;
   bool desc = false;
   if (active) {
-    cur = static_cast<int>(vol_old);
-    while (cur >= 0 && !inside_volume(c, cur, qx, qy, qz)) { prev = cur; cur = volume(c, cur).mother; }
+    const int cand = face >= 0 ? __ldg(c.nbr + 6 * static_cast<size_t>(vol_old) + face) : -1;
+    if (cand >= 0 && inside_volume(c, cand, qx, qy, qz)) {
+      cur = cand;
+    } else {
+      cur = static_cast<int>(vol_old);
+      while (cur >= 0 && !inside_volume(c, cur, qx, qy, qz)) { prev = cur; cur = volume(c, cur).mother; }
+    }
     desc = cur >= 0;
   }
   for (;;) {

@@ -541,6 +541,27 @@ __global__ void __launch_bounds__(kBlock) enqueue_kernel(const __grid_constant__
   }
 }
 
+// Relocation hints (geom.cuh nav_relocate), built once per context: thread (v, f) locates the point
+// eps_push outside the centre of face f of box volume v.  Hints are only ever candidates that the
+// relocation verifies, so a face whose neighbourhood is not uniform costs speed, never correctness.
+__global__ void __launch_bounds__(kBlock) hint_kernel(const __grid_constant__ DevCtx c, int32_t* __restrict__ nbr) {
+  const int n = 6 * c.n_vol, n_round = (n + 31) & ~31;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += gridDim.x * blockDim.x) {
+    const int vi = i / 6, f = i - 6 * vi;
+    bool active = i < n;
+    double g[3] = {0.0, 0.0, 0.0};
+    if (active) {
+      const DevVolume& v = volume(c, vi);
+      active = v.solid == ADEPT_BOX;
+      double l[3] = {0.0, 0.0, 0.0};
+      l[f >> 1] = (f & 1) ? v.dims[f >> 1] + c.eps_push : -(v.dims[f >> 1] + c.eps_push);
+      to_global(c, vi, v, l, g);
+    }
+    const int r = nav_locate(c, c.navigator, active, g[0], g[1], g[2]);
+    if (i < n) nbr[i] = r;   // -1: non-box volume or outside the world
+  }
+}
+
 // Test hook: exactly one step per track, results in input order.
 __global__ void __launch_bounds__(kBlock) frozen_kernel(const __grid_constant__ DevCtx c, const adept_track* __restrict__ in,
                                                         adept_step_result* __restrict__ out, adept_track* __restrict__ sec,
@@ -607,12 +628,12 @@ __global__ void __launch_bounds__(kBlock) locate_kernel(const __grid_constant__ 
 
 // Test hook for A5: relocation of point i starting from volume from[i] (any volume of the tree).
 __global__ void __launch_bounds__(kBlock) relocate_kernel(const __grid_constant__ DevCtx c, int nav, int n, const double* pos,
-                                                          const uint32_t* from, long long* out) {
+                                                          const uint32_t* from, const int32_t* face, long long* out) {
   const int n_round = (n + 31) & ~31;
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += gridDim.x * blockDim.x) {
     const bool a = i < n;
     const int k = a ? i : 0;
-    const int r = nav_relocate(c, nav, a, from[k], pos[3 * k], pos[3 * k + 1], pos[3 * k + 2]);
+    const int r = nav_relocate(c, nav, a, from[k], pos[3 * k], pos[3 * k + 1], pos[3 * k + 2], face ? face[k] : -1);
     if (a) out[i] = r;
   }
 }

@@ -102,7 +102,8 @@ __device__ int step_move(const DevCtx& c, int nav, bool active, const Track& in,
   double s = 0.0;
   int chords = 0;
   const int charge = is_gamma ? 0 : (positron ? +1 : -1);
-  const int flag = propagate<FIELD, BVH>(c, nav, go, charge, T0, pos, dir, in.vol, s_phys, s, chords, pushdir);
+  int face;
+  const int flag = propagate<FIELD, BVH>(c, nav, go, charge, T0, pos, dir, in.vol, s_phys, s, chords, pushdir, face);
 
   // ---- along-step actions (A7)
   o.s = s; o.chords = chords;
@@ -147,7 +148,7 @@ __device__ int step_move(const DevCtx& c, int nav, bool active, const Track& in,
     o.post.x = pos[0]; o.post.y = pos[1]; o.post.z = pos[2];
   }
   // ---- relocation (A5), warp-convergent
-  const int nv = nav_relocate<BVH>(c, nav, cross, in.vol, pos[0], pos[1], pos[2]);
+  const int nv = nav_relocate<BVH>(c, nav, cross, in.vol, pos[0], pos[1], pos[2], face);
   if (!go) return NEXT_NONE;
   if (cross) {
     if (nv < 0) {

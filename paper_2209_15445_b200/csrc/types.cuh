@@ -104,6 +104,7 @@ struct DevSlot {
 struct DevCtx {
   const DevVolume* vol;
   const double* rot;        // [n_vol][9]
+  const int32_t* nbr;       // [n_vol][6] relocation hints: volume beyond each box face, -1 = none (geom.cuh nav_relocate)
   int32_t n_vol;
   const DevBvh* bvh;
   int32_t navigator;

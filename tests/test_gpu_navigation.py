@@ -95,6 +95,17 @@ def test_relocation_from_any_volume_equals_locate(ob, barrel_full, calo, navigat
     near = np.clip(want + rng.choice([-2, -1, 1, 2], n), 52, g.n_volumes - 1)
     assert np.array_equal(a.relocate_batch(pos, near, navigator), want)
     assert (want < 0).sum() > 10 and (want >= 52).sum() > 1000
+    # relocation hints (the volume beyond each box face, built by adept_init) are candidates that are
+    # verified: any face, right or wrong, from any volume gives Locate(q)
+    for f in (0, 1, 2, 5):
+        assert np.array_equal(a.relocate_batch(pos, near, navigator, face=f), want)
+    assert np.array_equal(a.relocate_batch(pos, frm, navigator, face=rng.integers(-1, 6, n)), want)
+    # the right face: a point a push beyond the +x / -x face of slab v is in the next / previous slab
+    slabs = np.arange(52, g.n_volumes - 1)
+    px = np.array([g.trans[v][0] + g.dims[v][0] + 1e-7 for v in slabs])
+    q = np.stack([px, rng.uniform(-19, 19, len(slabs)), rng.uniform(-19, 19, len(slabs))], axis=1)
+    assert np.array_equal(a.relocate_batch(q, slabs, navigator, face=1), slabs + 1)
+    assert np.array_equal(a.locate_batch(q, navigator), slabs + 1)
     a.close()
     # barrel: crystals (BVH mother), gaps, shells, outside
     g, _, tabs, scal = barrel_full
@@ -106,4 +117,5 @@ def test_relocation_from_any_volume_equals_locate(ob, barrel_full, calo, navigat
     want = a.locate_batch(pos, navigator)
     assert np.array_equal(a.relocate_batch(pos, frm, navigator), want)
     assert np.array_equal(a.relocate_batch(pos, np.maximum(want, 0), navigator), want)
+    assert np.array_equal(a.relocate_batch(pos, np.maximum(want, 0), navigator, face=rng.integers(-1, 6, n)), want)
     a.close()
