@@ -340,6 +340,7 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
     std::vector<double> tg(n_mats * N * kRowG, 0.0), te(n_mats * N * kRowEm, 0.0), tp(n_mats * N * kRowEp, 0.0);
     for (int m = 0; m < n_mats; ++m) {
       const double* src = tables->data + static_cast<size_t>(m) * ADEPT_N_TABLES * N;
+      if (mats[m].vacuum != 0.0) continue;   // a vacuum has no physics: its rows stay zero (the gamma kernel relies on it)
       for (size_t i = 0; i < N; ++i) {
         for (int k = 0; k < 3; ++k) tg[(m * N + i) * kRowG + k] = src[k * N + i];
         for (int k = 0; k < 4; ++k) te[(m * N + i) * kRowEm + k] = src[(3 + k) * N + i];

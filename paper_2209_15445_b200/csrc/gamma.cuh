@@ -66,12 +66,13 @@ __device__ __forceinline__ void gamma_lane(const DevCtx& c, const DevSlot& slot,
       } else {
         fate = FATE_GO;
         mat = volume(c, vol).material;
-        if (mat_scalar(c, mat, S_VACUUM) == 0.0) {
+        {  // the rows of a vacuum are zero (adept_init), so no material flag has to be read first
           const GridPos gp = grid_pos(c, T0);
-          const double* tab = c.tab_g + static_cast<size_t>(mat) * kNGrid * kRowG;
-          const double x0 = interp(tab, kRowG, 0, gp);                                 // Compton
-          const double x1 = T0 > 2.0 * kMe ? interp(tab, kRowG, 1, gp) : 0.0;          // pair, exact threshold (P2)
-          const double se = interp(tab, kRowG, 2, gp);                                 // photoelectric
+          const double* tab = c.tab_g + (static_cast<size_t>(mat) * kNGrid + gp.i) * kRowG;
+          const Row4 r0 = load_row4(tab), r1 = load_row4(tab + kRowG);
+          const double x0 = lerp_col(r0, r1, 0, gp.f);                                 // Compton
+          const double x1 = T0 > 2.0 * kMe ? lerp_col(r0, r1, 1, gp.f) : 0.0;          // pair, exact threshold (P2)
+          const double se = lerp_col(r0, r1, 2, gp.f);                                 // photoelectric
           const double stot = x0 + x1 + se;
           if (stot > 0.0) {
             Stream u;

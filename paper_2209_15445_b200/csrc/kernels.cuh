@@ -171,30 +171,20 @@ __device__ __forceinline__ void block_reserve(BlockReserve<ND>& br, int phase, c
   for (int d = 0; d < ND; ++d) first[d] = br.wbase[phase][warp][d] + pre[d];
 }
 
-// A9: warp-reduced scoring.  Lanes depositing into the same volume are combined (match_any) and the
-// group leader issues one fp64 atomic.  With 100 scoring slabs all deposits of a calorimeter fall on
-// seven 128 B lines, two or three of them hot at the shower maximum, and one L2 slice retires an fp64
-// atomic on one line every ~3.5 cycles: measured, the atomic unit of the hottest slice was busy 60 %
-// (gamma move) and 86 % (charged move) of the kernel time (profiles/r1c_summary.md) -- the two
-// concurrent step kernels were serialised by it.  The deposits therefore go to one of several replicas
-// of the array, chosen per warp, which spreads them over as many L2 slices; adept_read_scoring folds the
-// replicas in a fixed order.
+// A9: scoring.  Every depositing lane issues one fp64 reduction (RED.ADD.F64, no return value, so the
+// warp does not wait for it).  With 100 scoring slabs all deposits of a calorimeter fall on seven 128 B
+// lines, two or three of them hot at the shower maximum, and one L2 slice retires an fp64 atomic on one
+// line every ~3.5 cycles: with a single array the atomic unit of the hottest slice was busy 60 % (gamma
+// move) and 86 % (charged move) of the kernel time and serialised the two concurrent step kernels.  The
+// deposits therefore go to one of several replicas of the array, chosen per warp, which spreads them over
+// as many L2 slices; adept_read_scoring folds the replicas in a fixed order.  Combining the lanes of a
+// warp by volume first (match_any + shuffles, one atomic per group) was measured 5 % slower per config-2
+// pass once the replicas had removed the contention: the ~40 instructions per warp cost more than the
+// reductions they save (profiles/r1e_summary.md).
 __device__ __forceinline__ void score(const DevSlot& slot, uint32_t vol, double e, bool active) {
-  const bool has = active && e != 0.0;
-  const unsigned hm = __ballot_sync(kFull, has);
-  if (hm == 0 || !has) return;                      // lanes without a deposit take no part
-  const unsigned peers = __match_any_sync(hm, vol);
-  const int lane = threadIdx.x & 31;
-  double sum = 0.0;
-  unsigned m = peers;
-  while (m) {  // sum over the group (groups are disjoint; every lane walks its own peer mask)
-    const int src = __ffs(m) - 1;
-    m &= m - 1;
-    sum += __shfl_sync(peers, e, src);
-  }
-  if (lane == __ffs(peers) - 1) {
+  if (active && e != 0.0) {
     const uint32_t rep = (blockIdx.x * kWarps + (threadIdx.x >> 5)) & slot.edep_mask;
-    atomicAdd(slot.edep + static_cast<size_t>(rep) * slot.edep_stride + vol, sum);
+    atomicAdd(slot.edep + static_cast<size_t>(rep) * slot.edep_stride + vol, e);
   }
 }
 
@@ -284,6 +274,33 @@ __device__ __forceinline__ int stage_process(int q) {
 }
 __device__ __forceinline__ int stage_species(int q) { return q < 3 ? ADEPT_GAMMA : (q < 5 ? ADEPT_ELECTRON : ADEPT_POSITRON); }
 
+// Outcome counters of the move kernel, packed one byte per field in a per-thread 64-bit word.
+enum { MC_STEPS = 0, MC_BOUNDARY, MC_ESCAPED, MC_STOPPED, MC_KILLED, MC_LOSS, MC_TRUNCATED, MC_PHOTO, MC_N };
+__device__ __forceinline__ int move_count_field(int outcome) {
+  switch (outcome) {
+    case ADEPT_OUT_BOUNDARY: return MC_BOUNDARY;
+    case ADEPT_OUT_ESCAPED: return MC_ESCAPED;
+    case ADEPT_OUT_STOPPED: return MC_STOPPED;
+    case ADEPT_OUT_KILLED: return MC_KILLED;
+    case ADEPT_OUT_LOSS: return MC_LOSS;
+    case ADEPT_OUT_TRUNCATED: return MC_TRUNCATED;
+    default: return MC_PHOTO;
+  }
+}
+__device__ __forceinline__ void move_counts_flush(BlockTally& t, unsigned long long& packed) {
+  constexpr int which[MC_N] = {-1, ADEPT_OUT_BOUNDARY, ADEPT_OUT_ESCAPED, ADEPT_OUT_STOPPED, ADEPT_OUT_KILLED, ADEPT_OUT_LOSS,
+                               ADEPT_OUT_TRUNCATED, ADEPT_OUT_PHOTO};
+#pragma unroll
+  for (int f = 0; f < MC_N; ++f) {
+    const unsigned v = __reduce_add_sync(kFull, static_cast<unsigned>((packed >> (8 * f)) & 255ull));
+    if ((threadIdx.x & 31) == 0 && v) {
+      if (f == MC_STEPS) atomicAdd(&t.steps, v);
+      else atomicAdd(&t.outcomes[which[f]], v);
+    }
+  }
+  packed = 0;
+}
+
 // ------------------------------------------------------------------------------------------------
 // Move kernel: one step of every track of a species up to (not including) its discrete interaction.
 // grid.y = species of a charged launch.  Survivors that do not interact go to the next buffer of their
@@ -311,6 +328,7 @@ move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot sl
   pipe_init(pipe);
   double sum_dep = 0.0, sum_cut = 0.0;
   unsigned chords = 0;
+  unsigned long long packed = 0;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const unsigned lt = (1u << lane) - 1u;
 
@@ -341,20 +359,10 @@ move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot sl
         record_leak(c, slot, o.post, species);
       }
     }
-    {
-      const unsigned ma = __ballot_sync(kFull, active);
-      if (lane == 0 && ma) atomicAdd(&tally.steps, static_cast<unsigned>(__popc(ma)));
-    }
-    const bool none = active && next == NEXT_NONE;
-    tally_outcome(tally, none, o.outcome, ADEPT_OUT_BOUNDARY);
-    tally_outcome(tally, none, o.outcome, ADEPT_OUT_ESCAPED);
-    tally_outcome(tally, none, o.outcome, ADEPT_OUT_STOPPED);
-    tally_outcome(tally, none, o.outcome, ADEPT_OUT_KILLED);
-    if (MODE != MODE_GAMMA) {
-      tally_outcome(tally, none, o.outcome, ADEPT_OUT_LOSS);
-      tally_outcome(tally, none, o.outcome, ADEPT_OUT_TRUNCATED);
-    } else {
-      tally_outcome(tally, none, o.outcome, ADEPT_OUT_PHOTO);
+    // per-thread outcome counters, one byte per field, folded into the block tally every 255 tiles
+    if (active) {
+      packed += 1ull << (8 * MC_STEPS);
+      if (next == NEXT_NONE) packed += 1ull << (8 * move_count_field(o.outcome));
     }
 
     // reservation: a lane appends at most one survivor (to one of four destinations) and the secondaries
@@ -399,7 +407,9 @@ move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot sl
         else cnt->overflow.v = 1;
       }
     }
+    if (k % 255u == 254u) move_counts_flush(tally, packed);
   }
+  move_counts_flush(tally, packed);
   {
     const unsigned long long ch = __reduce_add_sync(kFull, chords);
     if (lane == 0 && ch) atomicAdd(&tally.chords, ch);

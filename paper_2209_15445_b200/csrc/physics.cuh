@@ -23,6 +23,16 @@ __device__ __forceinline__ double interp(const double* __restrict__ tab, int row
   return y0 + g.f * (y1 - y0);
 }
 
+// One 32 B table row (4 columns) in two 16 B loads.
+struct Row4 { double v[4]; };
+__device__ __forceinline__ Row4 load_row4(const double* __restrict__ row) {
+  const double2 a = __ldg(reinterpret_cast<const double2*>(row)), b = __ldg(reinterpret_cast<const double2*>(row) + 1);
+  return Row4{{a.x, a.y, b.x, b.y}};
+}
+__device__ __forceinline__ double lerp_col(const Row4& r0, const Row4& r1, int col, double f) {
+  return r0.v[col] + f * (r1.v[col] - r0.v[col]);
+}
+
 // M7 inverse range: cell j with R_j <= r < R_{j+1}, then ln T linear in r.  Any search returns the same
 // j; this one starts from a hint table indexed by the exponent and top 5 mantissa bits of r (a
 // monotone pseudo-logarithm, built by adept_init: hint[k] = largest j with R_j <= lower edge of key

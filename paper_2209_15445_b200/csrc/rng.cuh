@@ -7,7 +7,9 @@ namespace adept {
 
 struct Philox4 { uint32_t w0, w1, w2, w3; };
 
-__device__ __noinline__ Philox4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+// Inlined: the ten rounds are integer work that the scheduler interleaves with the fp64 chains around
+// them (measured 1.3 % of a config-2 pass over a call).
+__device__ __forceinline__ Philox4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
                                                  uint32_t k0, uint32_t k1) {
 #pragma unroll
   for (int r = 0; r < 10; ++r) {
