@@ -442,7 +442,20 @@ interact_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlo
   tally_init(tally);
   pipe_init(pipe);
   double sum_cut = 0.0;
-  const int lane = threadIdx.x & 31;
+  unsigned long long pk_out = 0, pk_sec = 0;
+  const auto counts_flush = [&]() {
+#pragma unroll
+    for (int f = 0; f < 7; ++f) {
+      const unsigned v = __reduce_add_sync(kFull, static_cast<unsigned>((pk_out >> (8 * f)) & 255ull));
+      if ((threadIdx.x & 31) == 0 && v) atomicAdd(&tally.outcomes[f == 6 ? ADEPT_OUT_CLOSED : ADEPT_OUT_COMPTON + f], v);
+    }
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      const unsigned v = __reduce_add_sync(kFull, static_cast<unsigned>((pk_sec >> (16 * d)) & 65535ull));
+      if ((threadIdx.x & 31) == 0 && v) atomicAdd(&tally.secondaries[d], v);
+    }
+    pk_out = 0; pk_sec = 0;
+  };
   const uint32_t total = tile_begin[kNumStage];
   const auto queue_of = [&](uint32_t tile) { int q = 0; while (tile >= tile_begin[q + 1]) ++q; return q; };
   if (threadIdx.x == 0 && blockIdx.x < total) {
@@ -476,20 +489,19 @@ interact_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlo
       u.init(0, 0, 0, 0);
     }
     score(slot, t.vol, o.edep_cut, active);
-#pragma unroll
-    for (int w = ADEPT_OUT_COMPTON; w <= ADEPT_OUT_ANNI; ++w) tally_outcome(tally, active, o.outcome, w);
-    tally_outcome(tally, active, o.outcome, ADEPT_OUT_CLOSED);
-
     const int s0 = active ? o.sec[0].species : -1;
     const int s1 = active ? o.sec[1].species : -1;
     const bool live = active && o.alive;
+    // per-thread counters: outcomes one byte per field (COMPTON..ANNI -> 0..5, CLOSED -> 6), secondaries
+    // 16 bits per species; folded into the block tally every 127 tiles
+    if (active) {
+      pk_out += 1ull << (8 * (o.outcome == ADEPT_OUT_CLOSED ? 6 : o.outcome - ADEPT_OUT_COMPTON));
+      if (s0 >= 0) pk_sec += 1ull << (16 * s0);
+      if (s1 >= 0) pk_sec += 1ull << (16 * s1);
+    }
     uint32_t want[3], first[3];
 #pragma unroll
-    for (int d = 0; d < 3; ++d) {
-      want[d] = (live && species == d ? 1u : 0u) + (s0 == d ? 1u : 0u) + (s1 == d ? 1u : 0u);
-      const unsigned m = __ballot_sync(kFull, s0 == d), m1 = __ballot_sync(kFull, s1 == d);
-      if (lane == 0 && (m | m1)) atomicAdd(&tally.secondaries[d], static_cast<unsigned>(__popc(m) + __popc(m1)));
-    }
+    for (int d = 0; d < 3; ++d) want[d] = (live && species == d ? 1u : 0u) + (s0 == d ? 1u : 0u) + (s1 == d ? 1u : 0u);
     block_reserve<3>(br, phase, want, first, [&](int d) -> uint32_t* { return &cnt->count[parity ^ 1][d].v; });
     // within a destination the lane's entries are ordered: surviving parent, secondary 0, secondary 1
     const auto sel = [&](int d) { return d == 0 ? first[0] : (d == 1 ? first[1] : first[2]); };
@@ -499,14 +511,16 @@ interact_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlo
       else cnt->overflow.v = 1;
     }
 #pragma unroll
-    for (int k = 0; k < 2; ++k) {
-      const int ss = k == 0 ? s0 : s1;
+    for (int kk = 0; kk < 2; ++kk) {
+      const int ss = kk == 0 ? s0 : s1;
       if (ss < 0) continue;
-      const uint32_t j = sel(ss) + ((live && species == ss) ? 1u : 0u) + ((k == 1 && s0 == ss) ? 1u : 0u);
-      if (j < c.capacity) store_track(slot.buf[parity ^ 1][ss], j, make_secondary(o, k, t.event, u));
+      const uint32_t j = sel(ss) + ((live && species == ss) ? 1u : 0u) + ((kk == 1 && s0 == ss) ? 1u : 0u);
+      if (j < c.capacity) store_track(slot.buf[parity ^ 1][ss], j, make_secondary(o, kk, t.event, u));
       else cnt->overflow.v = 1;
     }
+    if (k % 127u == 126u) counts_flush();
   }
+  counts_flush();
   tally_flush(tally, slot, 0, 0.0, sum_cut);
 }
 
