@@ -10,6 +10,7 @@
 
 #include "kernels.cuh"
 #include "gamma.cuh"
+#include "charged.cuh"
 
 using namespace adept;
 
@@ -411,13 +412,18 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
 #else
     ctx->k_move_gamma = bvh ? gamma_move_kernel<true> : gamma_move_kernel<false>;
 #endif
+#ifdef ADEPT_CHARGED_GENERIC   // the generic move kernel (step_move<MODE_CHARGED>), kept for A/B measurements
+#define ADEPT_CHARGED_KERNEL(F, B) move_kernel<MODE_CHARGED, F, B>
+#else
+#define ADEPT_CHARGED_KERNEL(F, B) charged_move_kernel<F, B>
+#endif
     switch (f->kind) {
       case ADEPT_FIELD_NONE:
-        ctx->k_move_charged = bvh ? move_kernel<MODE_CHARGED, ADEPT_FIELD_NONE, true> : move_kernel<MODE_CHARGED, ADEPT_FIELD_NONE, false>; break;
+        ctx->k_move_charged = bvh ? ADEPT_CHARGED_KERNEL(ADEPT_FIELD_NONE, true) : ADEPT_CHARGED_KERNEL(ADEPT_FIELD_NONE, false); break;
       case ADEPT_FIELD_UNIFORM:
-        ctx->k_move_charged = bvh ? move_kernel<MODE_CHARGED, ADEPT_FIELD_UNIFORM, true> : move_kernel<MODE_CHARGED, ADEPT_FIELD_UNIFORM, false>; break;
+        ctx->k_move_charged = bvh ? ADEPT_CHARGED_KERNEL(ADEPT_FIELD_UNIFORM, true) : ADEPT_CHARGED_KERNEL(ADEPT_FIELD_UNIFORM, false); break;
       default:
-        ctx->k_move_charged = bvh ? move_kernel<MODE_CHARGED, ADEPT_FIELD_MAP_RZ, true> : move_kernel<MODE_CHARGED, ADEPT_FIELD_MAP_RZ, false>; break;
+        ctx->k_move_charged = bvh ? ADEPT_CHARGED_KERNEL(ADEPT_FIELD_MAP_RZ, true) : ADEPT_CHARGED_KERNEL(ADEPT_FIELD_MAP_RZ, false); break;
     }
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_g, ctx->k_move_gamma, kBlock, 0));
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_c, ctx->k_move_charged, kBlock, 0));

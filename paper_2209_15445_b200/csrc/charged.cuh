@@ -1,0 +1,293 @@
+// Charged (e-/e+) move kernel, hand-specialised (§8(c) S1-S4).
+//
+// Same arithmetic, in the same order, as step_move<MODE_CHARGED> (step.cuh), which stays the reference
+// implementation behind the frozen-step hook.  The generic kernel needs 166 registers, i.e. three
+// resident blocks (12 warps) per SM, and at that occupancy it issues 0.39 instructions per cycle and
+// scheduler with `wait` (fixed-latency fp64 dependencies) as its top stall (profiles/r1c_summary.md):
+// throughput is set by the number of resident warps.  As in gamma.cuh the lane's track stays in its
+// slot of the shared-memory tile and is read at the point of use; in addition the lane WRITES its
+// post-step direction and energy back into that slot before the relocation call, so the tile is the
+// lane's spill space and almost nothing is live across the two (not inlined) navigator calls.
+// The discrete process is chosen (U1, same Philox block as U0) before the propagation; the MSC draws
+// (U2, U3) and the at-rest annihilation draws (U4, U5) are regenerated from the key where they are used.
+#pragma once
+#include "kernels.cuh"
+
+namespace adept {
+
+#ifndef ADEPT_MINB_C2
+#define ADEPT_MINB_C2 5
+#endif
+
+// generic-proxy writes to the tile must be ordered before the TMA (async proxy) refill of the same buffer
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+template <int FIELD, bool BVH>
+__global__ void __launch_bounds__(kBlock, ADEPT_MINB_C2)
+charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot, int parity) {
+  const int species = static_cast<int>(blockIdx.y);   // ADEPT_ELECTRON or ADEPT_POSITRON
+  const bool positron = species == ADEPT_POSITRON;
+  const TrackSoA& cur = slot.buf[parity][species];
+  SlotCounters* cnt = slot.counters;
+  const uint32_t n = cnt->count[parity][species].v;
+
+  // destinations: 0 = next buffer of the species, 1..3 = its staging queues, 4 = next gamma buffer (the
+  // photons of an annihilation at rest)
+  constexpr int ND = 5;
+  const int q0 = positron ? 5 : 3;
+  __shared__ BlockTally tally;
+  __shared__ BlockReserve<ND> br;
+  __shared__ TilePipe pipe;
+  tally_init(tally);
+  pipe_init(pipe);
+  double sum_dep = 0.0, sum_cut = 0.0;
+  unsigned chords_sum = 0;
+  unsigned long long packed = 0;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned lt = (1u << lane) - 1u;
+  const int t = threadIdx.x;
+  enum { FATE_NONE = 0, FATE_KILLED, FATE_STOPPED, FATE_GO };
+
+  const uint32_t n_tiles = (n + kBlock - 1) / kBlock;
+  if (t == 0 && blockIdx.x < n_tiles) tile_issue(pipe.tile[0], cur, blockIdx.x, &pipe.bar[0]);
+  uint32_t k = 0;
+  for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++k) {
+    const int phase = k & 1;
+    if (t == 0 && tile + gridDim.x < n_tiles) tile_issue(pipe.tile[phase ^ 1], cur, tile + gridDim.x, &pipe.bar[phase ^ 1]);
+    mbar_wait(&pipe.bar[phase], (k >> 1) & 1);
+    TrackTile& T = pipe.tile[phase];
+    const uint32_t vol = T.u[2][t];
+    const bool active = tile * kBlock + t < n && vol != kDeadVolume;
+
+    // ---- phase A: step-start rules, physics step limit (A3), process choice (U1)
+    int fate = FATE_NONE, process = 0, mat = 0;
+    bool vacuum = true, lim_disc = false, range_out = false;
+    double s_phys = 0.0, S = 0.0, R = ADEPT_INF;
+    if (active) {
+      const uint32_t step = T.u[1][t];
+      const double T0 = T.d[6][t];
+      if (step >= c.max_steps) {
+        fate = FATE_KILLED;
+      } else if (T0 < kTmin) {
+        fate = FATE_STOPPED;
+        mat = volume(c, vol).material;
+      } else {
+        fate = FATE_GO;
+        mat = volume(c, vol).material;
+        vacuum = mat_scalar(c, mat, S_VACUUM) != 0.0;
+        double x0 = 0.0, x1 = 0.0, sa = 0.0;
+        if (!vacuum) {
+          const GridPos gp = grid_pos(c, T0);
+          if (positron) {
+            const double* tab = c.tab_ep + static_cast<size_t>(mat) * kNGrid * kRowEp;
+            x0 = interp(tab, kRowEp, 0, gp); x1 = interp(tab, kRowEp, 1, gp); sa = interp(tab, kRowEp, 2, gp);
+            S = interp(tab, kRowEp, 3, gp); R = interp(tab, kRowEp, 4, gp);
+          } else {
+            const double* tab = c.tab_em + (static_cast<size_t>(mat) * kNGrid + gp.i) * kRowEm;
+            const Row4 r0 = load_row4(tab), r1 = load_row4(tab + kRowEm);
+            x0 = lerp_col(r0, r1, 0, gp.f); x1 = lerp_col(r0, r1, 1, gp.f);
+            S = lerp_col(r0, r1, 2, gp.f); R = lerp_col(r0, r1, 3, gp.f);
+          }
+        }
+        const double stot = x0 + x1 + sa;
+        double s_disc = ADEPT_INF;
+        if (stot > 0.0) {
+          Stream u;
+          u.init(T.u[0][t], c.seed, T.id[t], step);
+          s_disc = div_pos(-log_pos(u.uniform(0)), stot);
+          const double u1 = u.uniform(1);
+          process = ADEPT_OUT_BREM;
+          if (u1 * stot < x0) process = ADEPT_OUT_BREM;
+          else if (!positron || u1 * stot < x0 + x1) process = ADEPT_OUT_IONI;
+          else process = ADEPT_OUT_ANNI;
+        }
+        range_out = R <= c.rho_R;
+        const double s_loss = range_out ? R : c.alpha_R * R + c.rho_R * (1.0 - c.alpha_R) * (2.0 - c.rho_R / R);
+        lim_disc = s_disc < s_loss;
+        s_phys = lim_disc ? s_disc : s_loss;
+      }
+    }
+    bool go = fate == FATE_GO;
+
+    // ---- phase B: propagation (A4, A6)
+    double px = T.d[0][t], py = T.d[1][t], pz = T.d[2][t];
+    double s = 0.0;
+    int flag = 0, face = -1;
+    double pdx, pdy, pdz;   // push direction
+    if (FIELD == ADEPT_FIELD_NONE) {
+      // straight line: one geometry query (what propagate() does when the field vanishes)
+      const double dx = T.d[3][t], dy = T.d[4][t], dz = T.d[5][t];
+      const bool query = go && !(0.0 >= s_phys);
+      int f;
+      const double s_geo = nav_distance<BVH>(c, c.navigator, query, px, py, pz, dx, dy, dz, vol, s_phys, f);
+      if (query) {
+        if (s_geo < s_phys) { px += s_geo * dx; py += s_geo * dy; pz += s_geo * dz; s = s_geo; flag = 1; face = f; }
+        else { px += s_phys * dx; py += s_phys * dy; pz += s_phys * dz; s = s_phys; }
+      }
+      pdx = dx; pdy = dy; pdz = dz;
+    } else {
+      double pos[3] = {px, py, pz}, dir[3] = {T.d[3][t], T.d[4][t], T.d[5][t]}, pushdir[3];
+      int chords = 0;
+      flag = propagate<FIELD, BVH>(c, c.navigator, go, positron ? +1 : -1, T.d[6][t], pos, dir, vol, s_phys, s, chords, pushdir, face);
+      px = pos[0]; py = pos[1]; pz = pos[2];
+      pdx = pushdir[0]; pdy = pushdir[1]; pdz = pushdir[2];
+      if (go) { T.d[3][t] = dir[0]; T.d[4][t] = dir[1]; T.d[5][t] = dir[2]; chords_sum += chords; }
+    }
+
+    // ---- along-step actions (A7): continuous loss, stop test, MSC; the post-step direction and energy
+    // go back into the lane's tile slot
+    bool cross = go && flag == 1;
+    bool ann_rest = false;
+    double edep_dep = 0.0, edep_cut = 0.0;
+    if (fate == FATE_STOPPED) {
+      edep_cut += T.d[6][t];
+      T.d[6][t] = 0.0;
+      ann_rest = positron;
+    }
+    if (go) {
+      const double T0 = T.d[6][t];
+      double dE = 0.0;
+      if (!vacuum) {
+        if (flag == 0 && !lim_disc && range_out) dE = T0;
+        else if (s <= 0.01 * R) dE = S * s;
+        else {
+          const double* tab = positron ? c.tab_ep + static_cast<size_t>(mat) * kNGrid * kRowEp
+                                       : c.tab_em + static_cast<size_t>(mat) * kNGrid * kRowEm;
+          dE = T0 - inverse_range(c, tab, positron ? kRowEp : kRowEm, positron ? 4 : 3,
+                                  c.rhint + (2 * mat + (positron ? 1 : 0)) * kHintStride, R - s);
+        }
+        dE = fmin(fmax(dE, 0.0), T0);
+      }
+      edep_dep += dE;
+      double T1 = T0 - dE;
+      if (T1 < kTmin) {
+        edep_cut += T1; T1 = 0.0;
+        ann_rest = positron;
+        fate = FATE_STOPPED;
+        go = false; cross = false;
+      }
+      T.d[6][t] = T1;
+      if (go && !vacuum && s > 0.0) {  // P9 Highland MSC at the pre-step energy, U2 and U3 of this step
+        const double X0 = mat_scalar(c, mat, S_X0);
+        const double pbeta = T0 * (T0 + 2.0 * kMe) / (T0 + kMe);
+        const double beta2 = T0 * (T0 + 2.0 * kMe) / ((T0 + kMe) * (T0 + kMe));
+        const double corr = fmax(0.0, 1.0 + 0.038 * log_pos(s / (X0 * beta2)));
+        const double th0 = (13.6 / pbeta) * sqrt(s / X0) * corr;
+        Stream u;
+        u.init(T.u[0][t], c.seed, T.id[t], T.u[1][t]);
+        const double u2 = u.uniform(2), u3 = u.uniform(3);
+        const double th = th0 * sqrt(-2.0 * log_pos(u2));
+        double sn, cs, dn[3];
+        sincos(th, &sn, &cs);
+        const double dir[3] = {T.d[3][t], T.d[4][t], T.d[5][t]};
+        rotate(dir, cs, sn, 2.0 * u3, dn);
+        T.d[3][t] = dn[0]; T.d[4][t] = dn[1]; T.d[5][t] = dn[2];
+      }
+      if (cross) { px += c.eps_push * pdx; py += c.eps_push * pdy; pz += c.eps_push * pdz; }   // G5
+    }
+    // at-rest annihilation (P8): both photons carry m; below the gamma cut they are deposited (M5)
+    bool has_ph = false;
+    if (ann_rest) {
+      if (kMe < mat_scalar(c, mat, S_KCUT)) { edep_cut += kMe; edep_cut += kMe; }
+      else has_ph = true;
+    }
+
+    // ---- relocation (A5), warp-convergent
+    const int nv = nav_relocate<BVH>(c, c.navigator, cross, vol, px, py, pz, face);
+
+    // ---- outcome.  Everything still needed of the track is read from the tile here, before the
+    // reservation barriers: after them thread 0 may already refill this tile buffer.
+    Track post;
+    post.x = px; post.y = py; post.z = pz;
+    post.dx = T.d[3][t]; post.dy = T.d[4][t]; post.dz = T.d[5][t];
+    post.ekin = T.d[6][t]; post.id = T.id[t];
+    post.event = T.u[0][t]; post.step = T.u[1][t] + 1; post.vol = vol; post.species = species;
+    bool live = false;
+    int dest = -1;
+    if (active) {
+      packed += 1ull << (8 * MC_STEPS);
+      sum_dep += edep_dep; sum_cut += edep_cut;
+      if (fate == FATE_KILLED) {
+        atomicAdd(&tally.ledger[3], carried_energy(species, post.ekin));
+        packed += 1ull << (8 * MC_KILLED);
+      } else if (fate == FATE_STOPPED) {
+        packed += 1ull << (8 * MC_STOPPED);
+      } else if (cross) {
+        if (nv < 0) {
+          atomicAdd(&tally.ledger[2], carried_energy(species, post.ekin));
+          record_leak(c, slot, post, species);
+          packed += 1ull << (8 * MC_ESCAPED);
+        } else {
+          post.vol = static_cast<uint32_t>(nv);
+          live = true; dest = 0;
+          packed += 1ull << (8 * MC_BOUNDARY);
+        }
+      } else if (flag == 2) {
+        live = true; dest = 0;
+        packed += 1ull << (8 * MC_TRUNCATED);
+      } else if (!lim_disc) {
+        live = true; dest = 0;
+        packed += 1ull << (8 * MC_LOSS);
+      } else {
+        live = true; dest = 1 + stage_queue(process, species) - q0;
+      }
+    }
+    score(slot, vol, edep_dep + edep_cut, active);
+    fence_proxy_async_smem();
+
+    // ---- reservation and stores (A0)
+    uint32_t pre = 0;
+#pragma unroll
+    for (int d = 0; d < 4; ++d) {
+      const unsigned b = __ballot_sync(kFull, dest == d);
+      if (dest == d) pre = __popc(b & lt);
+      if (lane == 0) br.wtot[phase][warp][d] = __popc(b);
+    }
+    const unsigned bph = __ballot_sync(kFull, has_ph);
+    const uint32_t pre_ph = 2 * __popc(bph & lt);
+    if (lane == 0) {
+      br.wtot[phase][warp][4] = 2 * __popc(bph);
+      if (bph) atomicAdd(&tally.secondaries[ADEPT_GAMMA], static_cast<unsigned>(2 * __popc(bph)));
+    }
+    block_reserve_commit<ND>(br, phase, [&](int d) -> uint32_t* {
+      if (d == 0) return &cnt->count[parity ^ 1][species].v;
+      if (d == 4) return &cnt->count[parity ^ 1][ADEPT_GAMMA].v;
+      return &cnt->n_stage[q0 + d - 1].v;
+    });
+    if (live) {
+      const uint32_t j = br.wbase[phase][warp][dest] + pre;
+      const bool staged = dest != 0;
+      const TrackSoA& dst = staged ? slot.stage[q0 + dest - 1] : slot.buf[parity ^ 1][species];
+      if (j < (staged ? c.stage_capacity : c.capacity)) store_track(dst, j, post);
+      else cnt->overflow.v = 1;
+    }
+    if (has_ph) {   // two back-to-back photons: cos(theta) = 2 U4 - 1, phi = 2 pi U5; children 0 and 1 (R3)
+      const uint32_t j = br.wbase[phase][warp][4] + pre_ph;
+      Stream u;
+      u.init(post.event, c.seed, post.id, post.step - 1);
+      const double u4 = u.uniform(4), u5 = u.uniform(5);
+      const double cos_t = 2.0 * u4 - 1.0, sin_t = sqrt(fmax(0.0, 1.0 - cos_t * cos_t));
+      double sp, cp;
+      sincospi(2.0 * u5, &sp, &cp);
+      const uint64_t id0 = u.child_id(0), id1 = u.child_id(1);
+      post.dx = sin_t * cp; post.dy = sin_t * sp; post.dz = cos_t;
+      post.ekin = kMe; post.step = 0; post.species = ADEPT_GAMMA; post.id = id0;
+      if (j + 1 < c.capacity) {
+        store_track(slot.buf[parity ^ 1][ADEPT_GAMMA], j, post);
+        post.dx = -post.dx; post.dy = -post.dy; post.dz = -post.dz; post.id = id1;
+        store_track(slot.buf[parity ^ 1][ADEPT_GAMMA], j + 1, post);
+      } else {
+        cnt->overflow.v = 1;
+      }
+    }
+    if (k % 255u == 254u) move_counts_flush(tally, packed);
+  }
+  move_counts_flush(tally, packed);
+  {
+    const unsigned long long ch = __reduce_add_sync(kFull, chords_sum);
+    if (lane == 0 && ch) atomicAdd(&tally.chords, ch);
+  }
+  tally_flush(tally, slot, species, sum_dep, sum_cut);
+}
+
+}  // namespace adept
