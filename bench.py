@@ -28,6 +28,15 @@ sys.path.insert(0, ROOT)
 BYTES_PER_STEP = 160      # 76 B track read + 76 B survivor write + 8 B scoring atomic
 BYTES_PER_SECONDARY = 76
 E_PRIMARY = 10000.0
+KERNELS = ("gamma_move_kernel", "charged_move_kernel", "interact_kernel")
+# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of each kernel at the peak
+# population of a config-2 pass, and the tracks that launch processed, from the `ncu --set full` capture
+# summarised in profiles/r1d_summary.md.  Reported as roofline.traffic beside the algorithmic bytes.
+NCU_TRAFFIC = {
+    "gamma_move_kernel": None,
+    "charged_move_kernel": None,
+    "interact_kernel": None,
+}
 
 
 def parse():
@@ -189,6 +198,8 @@ def run_ours(args):
     cap = args.capacity or max(1 << 20, 1024 * args.events)
     a = adept.Adept(g, tabs, scal, fld, device=str(dev), track_capacity=cap, sync_interval=args.sync_interval,
                     time_kernels=0 if args.no_kernel_timing else 1)
+    if not args.no_kernel_timing:
+        a.set_kernel_timing(False)       # the timed passes run without per-launch events
     stream = torch.cuda.Stream(device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
     edep_host = np.zeros(g.n_volumes)
@@ -200,7 +211,7 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize(dev)
 
-    def one_pass(timed):
+    def one_pass():
         """enqueue (H2D) -> transport -> scoring (D2H); returns (device ms of transport, wall s of the whole call)."""
         flush.zero_()
         torch.cuda.synchronize(dev)
@@ -218,12 +229,8 @@ def run_ours(args):
 
     n_warm = args.warmup if args.profile else max(args.warmup, 3)
     for _ in range(n_warm):
-        one_pass(False)
-    if not args.no_kernel_timing:
-        a.kernel_times(0)
+        one_pass()
     st0 = a.stats(0)
-    steps0, sec0, launches0 = sum(st0.steps), sum(st0.secondaries), st0.launches
-    gsteps0, gsec0 = st0.steps[2], 0
 
     clocks = ClockSampler(local)
     if rank == 0:
@@ -232,18 +239,33 @@ def run_ours(args):
     t_wall0 = time.perf_counter()
     dev_ms, wall_s = [], []
     for _ in range(args.steps):
-        ms, w = one_pass(True)
+        ms, w = one_pass()
         dev_ms.append(ms)
         wall_s.append(w)
     barrier()
     t_wall = time.perf_counter() - t_wall0
+    st = a.stats(0)
+
+    # Instrumented passes of the same workload, for the roofline object only: CUDA events around every
+    # launch, kernels one after the other on the stream (adept.h: adept_set_kernel_timing).  The events
+    # cost stream time (~5 ms per pass), which is why the timed passes above run without them.
+    kms, kn, ims = np.zeros(3), np.zeros(3), []
+    if not args.no_kernel_timing:
+        a.set_kernel_timing(True)
+        a.kernel_times(0)
+        for _ in range(args.steps):
+            ims.append(one_pass()[0])
+        kms, kn = a.kernel_times(0)
+        a.set_kernel_timing(False)
     clk = clocks.stop() if rank == 0 else None
 
-    st = a.stats(0)
-    kms, kn = a.kernel_times(0) if not args.no_kernel_timing else (np.zeros(3), np.zeros(3))
-    steps = sum(st.steps) - steps0
-    n_sec = sum(st.secondaries) - sec0
-    launches = st.launches - launches0 + args.steps        # + one enqueue kernel per pass
+    n_pass = args.steps
+    steps_sp = [st.steps[k] - st0.steps[k] for k in range(3)]            # e-, e+, gamma track steps
+    steps = sum(steps_sp)
+    n_sec = sum(st.secondaries) - sum(st0.secondaries)
+    n_int = sum(st.outcomes[k] - st0.outcomes[k] for k in range(len(st.outcomes))
+                if k in adept.INTERACTION_OUTCOMES)
+    launches = st.launches - st0.launches + n_pass * 2          # + one enqueue and one fold kernel per pass
     t_dev = sum(dev_ms) * 1e-3
     t_e2e = sum(wall_s)
     (t_dev, t_e2e), (steps_all, launches_all) = reduce_over_ranks(dist, dev, [t_dev, t_e2e], [steps, launches])
@@ -257,12 +279,17 @@ def run_ours(args):
             pass
         peak = float(peaks.get("hbm_gbs", 6650.0))
         peak_src = "MEASURED_PEAKS.json hbm_gbs (of measured)" if "hbm_gbs" in peaks else "6650 GB/s (of fallback)"
-        # dominant kernel = the step kernel with the larger accumulated device time
-        dom = int(np.argmax(kms[:2]))
-        dom_steps = (st.steps[2] - gsteps0) if dom == 0 else (steps - (st.steps[2] - gsteps0))
-        # secondaries are attributed to the kernel that creates them in proportion to its steps
-        dom_bytes = dom_steps * BYTES_PER_STEP + n_sec * BYTES_PER_SECONDARY * (dom_steps / max(steps, 1))
-        achieved = dom_bytes / (kms[dom] * 1e-3) / 1e9 if kms[dom] > 0 else 0.0
+        # algorithmic HBM bytes of the timed passes per kernel: a move kernel reads 76 B and
+        # writes 76 B per track step and scores 8 B; the interaction kernel reads the staged track, writes
+        # the parent back and writes 76 B per secondary
+        alg = [steps_sp[2] * BYTES_PER_STEP, (steps_sp[0] + steps_sp[1]) * BYTES_PER_STEP,
+               n_int * (2 * 76 + 8) + n_sec * BYTES_PER_SECONDARY]
+        dom = int(np.argmax(kms))      # dominant kernel = largest accumulated device time, kernels run alone
+        achieved = alg[dom] / (kms[dom] * 1e-3) / 1e9 if kms[dom] > 0 else 0.0
+        per_kernel = {KERNELS[k]: {"ms_per_pass": float(kms[k] / n_pass), "launches": int(kn[k]),
+                                   "algorithmic_GBps": float(alg[k] / (kms[k] * 1e-3) / 1e9) if kms[k] > 0 else None,
+                                   "frac": float(alg[k] / (kms[k] * 1e-3) / 1e9 / peak) if kms[k] > 0 else None}
+                      for k in range(3)}
         line = {
             "metric": "track_steps_per_s", "value": steps_all / t_dev, "unit": "steps/s", "n_gpus": world,
             "steps": args.steps, "warmup": n_warm, "ms_per_step": 1e3 * t_dev / args.steps,
@@ -278,14 +305,16 @@ def run_ours(args):
                     "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
             "gpu_launches": launches_all,
             "clocks": clk,
-            "roofline": {"bound": "hbm", "kernel": "move_kernel<gamma>" if dom == 0 else "move_kernel<charged>",
-                         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+            "roofline": {"bound": "hbm", "kernel": KERNELS[dom],
+                         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": NCU_TRAFFIC[KERNELS[dom]],
                          "peak_source": peak_src, "launches": int(kn[dom]), "avg_launch_ms": float(kms[dom] / max(kn[dom], 1)),
-                         "algorithmic_bytes_per_step": BYTES_PER_STEP,
-                         "other_move_kernel_ms": float(kms[1 - dom]), "dominant_kernel_ms": float(kms[dom]),
-                         "interact_kernel_ms": float(kms[2]),
-                         "note": "latency/divergence bound fp64 Monte Carlo: see DESIGN.md §5 and profiles/"},
+                         "algorithmic_bytes_per_step": BYTES_PER_STEP, "per_kernel": per_kernel,
+                         "timing": f"CUDA events around every launch in {n_pass} instrumented passes after the timed region "
+                                   f"(kernels run one after the other; {np.mean(ims) if ims else 0:.2f} ms per instrumented pass)",
+                         "note": "latency/divergence bound fp64 Monte Carlo: see DESIGN.md \u00a75 and profiles/"},
             "iterations_per_step": (st.iterations - st0.iterations) / args.steps,
+            "track_steps_per_species_per_step": {"e-": steps_sp[0] / n_pass, "e+": steps_sp[1] / n_pass, "gamma": steps_sp[2] / n_pass},
             "peak_population": int(st.peak_population),
             "wall_s_timed_region": t_wall,
         }

@@ -109,7 +109,10 @@ typedef struct {
   uint64_t leak_capacity;  /* per slot: tracks that left the world kept for adept_read_leaked       */
   uint64_t stage_capacity; /* per slot, per interaction queue: tracks staged for their discrete
                               interaction in one population step (0 = track_capacity)               */
-  int32_t time_kernels;    /* 1: bracket every step-kernel launch with CUDA events (adept_get_kernel_times) */
+  int32_t time_kernels;    /* 1: bracket every step-kernel launch with CUDA events (adept_get_kernel_times);
+                              the events cost ~5 us of stream time per launch, so timed passes are slower */
+  int32_t concurrent_species; /* 1 (default): gamma and charged move kernels on two streams;
+                              0: all kernels of a slot on the caller's stream, one after the other          */
 } adept_config;
 
 typedef struct {
@@ -197,10 +200,22 @@ int adept_get_stats(adept_ctx*, int event_slot, adept_stats* out);
 
 /* With config.time_kernels: device time [ms] and launch count of the gamma move kernel [0], the
  * charged move kernel [1] and the interaction kernel [2] of this slot, accumulated since the last call
- * (CUDA events recorded on the stream each kernel is launched on; [0] and [1] run concurrently). */
+ * (CUDA events recorded on the stream the kernels are launched on).  While timing is on, the kernels of
+ * a population step run one after the other on the caller's stream, so every event pair brackets one
+ * kernel alone; the events themselves cost ~5 us of stream time per launch.  adept_set_kernel_timing
+ * switches the events off (0) and on (1) between passes of a context created with time_kernels = 1, so
+ * that a benchmark can time untimed passes and instrumented passes of the same context. */
+int adept_set_kernel_timing(adept_ctx*, int on);
 #define ADEPT_N_TIMED_KERNELS 3
 int adept_get_kernel_times(adept_ctx*, int event_slot, double ms[ADEPT_N_TIMED_KERNELS],
                            uint64_t launches[ADEPT_N_TIMED_KERNELS]);
+
+/* Trace of the slot's population steps since the previous call (at most ADEPT_TRACE_CAPACITY of them):
+ * t_ns[i] = device %globaltimer [ns] when population step i finished, population[i] = live tracks that
+ * entered it.  Written by the kernel that ends a population step, so recording costs no stream time.
+ * *n = entries copied (<= cap).  The slot must not be in transport. */
+#define ADEPT_TRACE_CAPACITY 4096
+int adept_get_iteration_trace(adept_ctx*, int event_slot, uint64_t* t_ns, uint32_t* population, size_t cap, size_t* n);
 
 /* Test hook: exactly one step for each of n tracks, results in input order; secondaries[2*i + k]. */
 int adept_step_frozen(adept_ctx*, int n, const adept_track* in, adept_step_result* out,

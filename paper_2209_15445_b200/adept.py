@@ -44,7 +44,8 @@ class CConfig(C.Structure):
     _fields_ = [("delta_chord", C.c_double), ("eps_push", C.c_double), ("alpha_R", C.c_double), ("rho_R", C.c_double),
                 ("chord_budget", C.c_int32), ("seed", C.c_uint32), ("max_steps", C.c_uint32), ("navigator", C.c_int32),
                 ("n_event_slots", C.c_int32), ("sync_interval", C.c_int32), ("track_capacity", C.c_uint64),
-                ("leak_capacity", C.c_uint64), ("stage_capacity", C.c_uint64), ("time_kernels", C.c_int32)]
+                ("leak_capacity", C.c_uint64), ("stage_capacity", C.c_uint64), ("time_kernels", C.c_int32),
+                ("concurrent_species", C.c_int32)]
 
 
 class CLedger(C.Structure):
@@ -60,9 +61,13 @@ class CStats(C.Structure):
                 ("launches", C.c_uint64)]
 
 
+# outcomes (ADEPT_OUT_*) counted by the interaction kernel: Compton, pair, brems, ionisation, annihilation, closed
+INTERACTION_OUTCOMES = (1, 2, 4, 5, 6, 12)
+
 EXPORTS = ["adept_last_error", "adept_default_config", "adept_workspace_bytes", "adept_init",
            "adept_enqueue_primaries", "adept_enqueue_batch", "adept_transport", "adept_transport_many",
-           "adept_read_scoring", "adept_read_leaked", "adept_get_stats", "adept_get_kernel_times", "adept_step_frozen",
+           "adept_read_scoring", "adept_read_leaked", "adept_get_stats", "adept_get_kernel_times", "adept_set_kernel_timing", "adept_get_iteration_trace",
+           "adept_step_frozen",
            "adept_distance_batch", "adept_locate_batch", "adept_relocate_batch", "adept_shutdown"]
 
 
@@ -86,6 +91,8 @@ def load_library():
     lib.adept_read_leaked.argtypes = [vp, i, vp, sz, C.POINTER(sz)]
     lib.adept_get_stats.argtypes = [vp, i, C.POINTER(CStats)]
     lib.adept_get_kernel_times.argtypes = [vp, i, vp, vp]
+    lib.adept_set_kernel_timing.argtypes = [vp, i]
+    lib.adept_get_iteration_trace.argtypes = [vp, i, vp, vp, sz, C.POINTER(sz)]
     lib.adept_step_frozen.argtypes = [vp, i, vp, vp, vp, vp]
     lib.adept_distance_batch.argtypes = [vp, i, i, vp, vp, vp, vp, vp, vp]
     lib.adept_locate_batch.argtypes = [vp, i, i, vp, vp, vp]
@@ -221,6 +228,17 @@ class Adept:
         n = np.zeros(3, dtype=np.uint64)
         _check(lib.adept_get_kernel_times(self.ctx, slot, _ptr(ms), _ptr(n)))
         return ms, n
+
+    def set_kernel_timing(self, on):
+        _check(lib.adept_set_kernel_timing(self.ctx, 1 if on else 0))
+
+    def iteration_trace(self, slot=0, cap=4096):
+        """(t_ns[n], population[n]) of the population steps since the last call (device %globaltimer)."""
+        t = np.zeros(cap, dtype=np.uint64)
+        pop = np.zeros(cap, dtype=np.uint32)
+        n = C.c_size_t(0)
+        _check(lib.adept_get_iteration_trace(self.ctx, slot, _ptr(t), _ptr(pop), cap, C.byref(n)))
+        return t[:n.value], pop[:n.value]
 
     # ---- test hooks
     def step_frozen(self, tracks, stream=None):

@@ -170,6 +170,7 @@ struct adept_ctx {
   // move kernels specialised for this context's field kind and for geometries without BVH volumes
   using Kernel = void (*)(DevCtx, DevSlot, int);
   Kernel k_move_gamma = nullptr, k_move_charged = nullptr;
+  bool timing_on = false;            // per-launch CUDA events active (adept_set_kernel_timing)
 };
 
 extern "C" const char* adept_last_error(void) { return g_err; }
@@ -181,6 +182,7 @@ extern "C" void adept_default_config(adept_config* c) {
   c->chord_budget = 16; c->seed = 1; c->max_steps = 1000000;
   c->navigator = ADEPT_NAV_BVH; c->n_event_slots = 1; c->sync_interval = 8;
   c->track_capacity = 1u << 20; c->leak_capacity = 1u << 16; c->stage_capacity = 0;
+  c->concurrent_species = 1;
 }
 
 namespace {
@@ -273,6 +275,9 @@ size_t carve(void* base, const adept_config* cfg, const adept_geometry* g, int n
     d.ledger = cv.take<double>(8);
     d.stats = cv.take<DevStats>(1);
     d.leaked = cv.take<adept_track>(std::max<size_t>(cfg->leak_capacity, 1));
+    d.trace_t = cv.take<unsigned long long>(ADEPT_TRACE_CAPACITY);
+    d.trace_pop = cv.take<uint32_t>(ADEPT_TRACE_CAPACITY);
+    d.trace_n = cv.take<uint32_t>(1);
     L.slots.push_back(d);
   }
   if (out) *out = std::move(L);
@@ -447,7 +452,16 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
       for (cudaEvent_t& e : sh.tev) CUDA_TRY(cudaEventCreate(&e));
     }
   }
+  ctx->timing_on = cfg->time_kernels != 0;
   *out = ctx;
+  return ADEPT_OK;
+}
+
+extern "C" int adept_set_kernel_timing(adept_ctx* ctx, int on) {
+  if (!ctx) return fail(ADEPT_EINVAL, "null context");
+  if (on && !ctx->cfg.time_kernels) return fail(ADEPT_ESTATE, "context was not created with time_kernels");
+  for (const SlotHost& sh : ctx->slots) if (sh.live) return fail(ADEPT_ESTATE, "a slot is being transported");
+  ctx->timing_on = on != 0;
   return ADEPT_OK;
 }
 
@@ -518,23 +532,29 @@ namespace {
 // interaction kernel over what they staged and the buffer swap.
 int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity) {
   constexpr int kEv = 2 * ADEPT_N_TIMED_KERNELS;
-  CUDA_TRY(cudaEventRecord(sh.fork, st));
-  CUDA_TRY(cudaStreamWaitEvent(sh.helper, sh.fork, 0));
-  const bool timed = !sh.tev.empty() && sh.tev_used + kEv <= static_cast<int>(sh.tev.size());
+  const bool timed = ctx->timing_on && !sh.tev.empty() && sh.tev_used + kEv <= static_cast<int>(sh.tev.size());
+  // a timed pass runs the kernels one after the other, so that an event pair brackets one kernel alone
+  const bool fork = ctx->cfg.concurrent_species != 0 && !ctx->timing_on;
+  cudaStream_t sc = fork ? sh.helper : st;   // stream of the charged move kernel
+  if (fork) {
+    CUDA_TRY(cudaEventRecord(sh.fork, st));
+    CUDA_TRY(cudaStreamWaitEvent(sh.helper, sh.fork, 0));
+  }
   cudaEvent_t* ev = timed ? &sh.tev[sh.tev_used] : nullptr;
   if (timed) CUDA_TRY(cudaEventRecord(ev[0], st));
   ctx->k_move_gamma<<<dim3(ctx->grid_gamma, 1), kBlock, 0, st>>>(ctx->dev, sh.dev, parity);
   if (timed) CUDA_TRY(cudaEventRecord(ev[1], st));
-  if (timed) CUDA_TRY(cudaEventRecord(ev[2], sh.helper));
-  ctx->k_move_charged<<<dim3(ctx->grid_charged, 2), kBlock, 0, sh.helper>>>(ctx->dev, sh.dev, parity);
-  if (timed) CUDA_TRY(cudaEventRecord(ev[3], sh.helper));
-  CUDA_TRY(cudaEventRecord(sh.join, sh.helper));
-  CUDA_TRY(cudaStreamWaitEvent(st, sh.join, 0));
+  if (timed) CUDA_TRY(cudaEventRecord(ev[2], sc));
+  ctx->k_move_charged<<<dim3(ctx->grid_charged, 2), kBlock, 0, sc>>>(ctx->dev, sh.dev, parity);
+  if (timed) CUDA_TRY(cudaEventRecord(ev[3], sc));
+  if (fork) {
+    CUDA_TRY(cudaEventRecord(sh.join, sh.helper));
+    CUDA_TRY(cudaStreamWaitEvent(st, sh.join, 0));
+  }
   if (timed) CUDA_TRY(cudaEventRecord(ev[4], st));
   interact_kernel<<<ctx->grid_inter, kBlock, 0, st>>>(ctx->dev, sh.dev, parity);
   if (timed) { CUDA_TRY(cudaEventRecord(ev[5], st)); sh.tev_used += kEv; }
-  finish_iteration_kernel<<<1, 32, 0, st>>>(sh.dev, parity);
-  sh.launches += 4;
+  sh.launches += 3;
   return ADEPT_OK;
 }
 
@@ -635,6 +655,22 @@ extern "C" int adept_get_stats(adept_ctx* ctx, int slot, adept_stats* out) {
   for (int k = 0; k < ADEPT_N_OUTCOMES; ++k) out->outcomes[k] = s.outcomes[k];
   out->chords = s.chords; out->iterations = s.iterations; out->peak_population = s.peak_population;
   out->launches = ctx->slots[slot].launches;
+  return ADEPT_OK;
+}
+
+extern "C" int adept_get_iteration_trace(adept_ctx* ctx, int slot, uint64_t* t_ns, uint32_t* population, size_t cap, size_t* n) {
+  const int rc = check_slot(ctx, slot);
+  if (rc != ADEPT_OK) return rc;
+  if (!n) return fail(ADEPT_EINVAL, "null argument");
+  SlotHost& sh = ctx->slots[slot];
+  if (sh.live) return fail(ADEPT_ESTATE, "slot %d is being transported", slot);
+  uint32_t m = 0;
+  CUDA_TRY(cudaMemcpy(&m, sh.dev.trace_n, sizeof(uint32_t), cudaMemcpyDeviceToHost));
+  const size_t k = std::min<size_t>(std::min<size_t>(m, cap), ADEPT_TRACE_CAPACITY);
+  if (k && t_ns) CUDA_TRY(cudaMemcpy(t_ns, sh.dev.trace_t, k * sizeof(uint64_t), cudaMemcpyDeviceToHost));
+  if (k && population) CUDA_TRY(cudaMemcpy(population, sh.dev.trace_pop, k * sizeof(uint32_t), cudaMemcpyDeviceToHost));
+  CUDA_TRY(cudaMemset(sh.dev.trace_n, 0, sizeof(uint32_t)));
+  *n = k;
   return ADEPT_OK;
 }
 

@@ -35,6 +35,7 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
   // photons of an annihilation at rest)
   constexpr int ND = 5;
   const int q0 = positron ? 5 : 3;
+  if (blockIdx.x >= (n + kBlock - 1) / kBlock) return;   // no tile for this block (tail of a shower: most blocks)
   __shared__ BlockTally tally;
   __shared__ BlockReserve<ND> br;
   __shared__ TilePipe pipe;

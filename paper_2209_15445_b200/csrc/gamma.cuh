@@ -162,6 +162,7 @@ gamma_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevS
   // destinations: 0 = next gamma buffer, 1..3 = Compton / pair / (unused) staging queues, 4 = next
   // electron buffer (photoelectrons)
   constexpr int ND = 5;
+  if (blockIdx.x >= (n + kBlock - 1) / kBlock) return;   // no tile for this block (tail of a shower: most blocks)
   __shared__ BlockTally tally;
   __shared__ BlockReserve<ND> br;
   __shared__ TilePipe pipe;

@@ -417,6 +417,33 @@ move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot sl
   tally_flush(tally, slot, species, sum_dep, sum_cut);
 }
 
+// End of one population step: the just-consumed buffers become the next step's output buffers.  Run by
+// the last block of the interaction kernel to finish (ticket counter), so a population step is three
+// launches; every other block has completed its appends (they precede its ticket) when this runs.
+__device__ __forceinline__ void finish_iteration(const DevSlot& slot, int parity) {
+  SlotCounters* cnt = slot.counters;
+  const int k = threadIdx.x;
+  uint32_t before = 0, live = 0;
+  for (int sp = 0; sp < 3; ++sp) { before += __ldcg(&cnt->count[parity][sp].v); live += __ldcg(&cnt->count[parity ^ 1][sp].v); }
+  __syncthreads();
+  if (k < 3) cnt->count[parity][k].v = 0;
+  else if (k < 3 + kNumStage) cnt->n_stage[k - 3].v = 0;
+  else if (k == 3 + kNumStage) {
+    cnt->live.v = live;
+    cnt->ticket.v = 0;
+    if (before) {
+      slot.stats->iterations += 1;
+      if (before > slot.stats->peak_population) slot.stats->peak_population = before;
+      const uint32_t j = *slot.trace_n;
+      if (j < ADEPT_TRACE_CAPACITY) {
+        unsigned long long now;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+        slot.trace_t[j] = now; slot.trace_pop[j] = before; *slot.trace_n = j + 1;
+      }
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------------------------
 // Interaction kernel: a tile is kBlock staged tracks of ONE queue, so a whole block runs the rejection
 // loop of one process (PAPER.md:101 names divergence between processes as a main cost).  The updated
@@ -429,6 +456,16 @@ interact_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlo
   __shared__ TilePipe pipe;
   __shared__ uint32_t tile_begin[kNumStage + 1];   // prefix of tiles per queue
   __shared__ uint32_t n_staged[kNumStage];
+  __shared__ bool is_last;
+  uint32_t total = 0;
+#pragma unroll
+  for (int q = 0; q < kNumStage; ++q) total += (min(__ldcg(&cnt->n_stage[q].v), c.stage_capacity) + kBlock - 1) / kBlock;
+  if (blockIdx.x >= total) {   // no tile for this block (tail of a shower: most blocks); it only takes its ticket
+    if (threadIdx.x == 0) is_last = atomicAdd(&cnt->ticket.v, 1u) == gridDim.x - 1;
+    __syncthreads();
+    if (is_last) finish_iteration(slot, parity);
+    return;
+  }
   if (threadIdx.x == 0) {
     uint32_t acc = 0;
     for (int q = 0; q < kNumStage; ++q) {
@@ -456,7 +493,6 @@ interact_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlo
     }
     pk_out = 0; pk_sec = 0;
   };
-  const uint32_t total = tile_begin[kNumStage];
   const auto queue_of = [&](uint32_t tile) { int q = 0; while (tile >= tile_begin[q + 1]) ++q; return q; };
   if (threadIdx.x == 0 && blockIdx.x < total) {
     const int q = queue_of(blockIdx.x);
@@ -522,24 +558,14 @@ interact_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlo
   }
   counts_flush();
   tally_flush(tally, slot, 0, 0.0, sum_cut);
-}
-
-// End of one population step: the just-consumed buffers become the next step's output buffers.
-__global__ void finish_iteration_kernel(const __grid_constant__ DevSlot slot, int parity) {
-  SlotCounters* cnt = slot.counters;
-  const int k = threadIdx.x;
-  uint32_t before = 0, live = 0;
-  for (int sp = 0; sp < 3; ++sp) { before += cnt->count[parity][sp].v; live += cnt->count[parity ^ 1][sp].v; }
+  // the last block to get here ends the population step
   __syncthreads();
-  if (k < 3) cnt->count[parity][k].v = 0;
-  else if (k < 3 + kNumStage) cnt->n_stage[k - 3].v = 0;
-  else if (k == 3 + kNumStage) {
-    cnt->live.v = live;
-    if (before) {
-      slot.stats->iterations += 1;
-      if (before > slot.stats->peak_population) slot.stats->peak_population = before;
-    }
+  if (threadIdx.x == 0) {
+    __threadfence();
+    is_last = atomicAdd(&cnt->ticket.v, 1u) == gridDim.x - 1;
   }
+  __syncthreads();
+  if (is_last) finish_iteration(slot, parity);
 }
 
 // Places primaries (G5: volume = Locate(p + eps d)) and appends them to the parity-0 buffers.

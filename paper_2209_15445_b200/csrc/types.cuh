@@ -78,6 +78,7 @@ struct SlotCounters {
   PaddedCounter n_leaked;
   PaddedCounter overflow;           // set when any queue overflowed
   PaddedCounter live;               // population after the last finished iteration
+  PaddedCounter ticket;             // blocks of the interaction kernel that have finished (last one ends the step)
 };
 
 struct DevStats {
@@ -98,6 +99,9 @@ struct DevSlot {
   double* ledger;           // [5]: deposited, below_cut, escaped, killed, primary
   DevStats* stats;
   adept_track* leaked;      // [leak_capacity]
+  unsigned long long* trace_t;  // [ADEPT_TRACE_CAPACITY] %globaltimer at the end of each population step
+  uint32_t* trace_pop;          // [ADEPT_TRACE_CAPACITY] population that entered it
+  uint32_t* trace_n;            // entries written since adept_get_iteration_trace
   TrackSoA stage[kNumStage];  // tracks waiting for their discrete interaction (stage_capacity entries each)
 };
 
