@@ -111,6 +111,12 @@ typedef struct {
                               interaction in one population step (0 = track_capacity)               */
   int32_t time_kernels;    /* 1: bracket every step-kernel launch with CUDA events (adept_get_kernel_times);
                               the events cost ~5 us of stream time per launch, so timed passes are slower */
+  uint64_t inject_chunk;   /* staggered injection: 0 (default) = every enqueued primary
+                              enters the first population step; n > 0 = enqueued primaries wait in a per-slot
+                              pending store and at most n of them enter each population step, in enqueue order,
+                              so that showers overlap at a lower peak population                            */
+  uint64_t pending_capacity; /* per slot: primaries the pending store holds (0 = track_capacity); used only
+                              when inject_chunk > 0                                                          */
   int32_t concurrent_species; /* 1 (default): gamma and charged move kernels on two streams;
                               0: all kernels of a slot on the caller's stream, one after the other          */
 } adept_config;
@@ -211,9 +217,10 @@ int adept_get_kernel_times(adept_ctx*, int event_slot, double ms[ADEPT_N_TIMED_K
                            uint64_t launches[ADEPT_N_TIMED_KERNELS]);
 
 /* Trace of the slot's population steps since the previous call (at most ADEPT_TRACE_CAPACITY of them):
- * t_ns[i] = device %globaltimer [ns] when population step i finished, population[i] = live tracks that
- * entered it.  Written by the kernel that ends a population step, so recording costs no stream time.
- * *n = entries copied (<= cap).  The slot must not be in transport. */
+ * t_ns[i] = device %globaltimer [ns] when population step i finished, population[3 * i + s] = tracks of
+ * species s (0 e-, 1 e+, 2 gamma) that entered it.  Written by the kernel that ends a population step, so
+ * recording costs no stream time.  *n = steps copied (<= cap; population holds 3 * cap entries).  The
+ * slot must not be in transport. */
 #define ADEPT_TRACE_CAPACITY 4096
 int adept_get_iteration_trace(adept_ctx*, int event_slot, uint64_t* t_ns, uint32_t* population, size_t cap, size_t* n);
 

@@ -45,7 +45,7 @@ class CConfig(C.Structure):
                 ("chord_budget", C.c_int32), ("seed", C.c_uint32), ("max_steps", C.c_uint32), ("navigator", C.c_int32),
                 ("n_event_slots", C.c_int32), ("sync_interval", C.c_int32), ("track_capacity", C.c_uint64),
                 ("leak_capacity", C.c_uint64), ("stage_capacity", C.c_uint64), ("time_kernels", C.c_int32),
-                ("concurrent_species", C.c_int32)]
+                ("inject_chunk", C.c_uint64), ("pending_capacity", C.c_uint64), ("concurrent_species", C.c_int32)]
 
 
 class CLedger(C.Structure):
@@ -233,9 +233,10 @@ class Adept:
         _check(lib.adept_set_kernel_timing(self.ctx, 1 if on else 0))
 
     def iteration_trace(self, slot=0, cap=4096):
-        """(t_ns[n], population[n]) of the population steps since the last call (device %globaltimer)."""
+        """(t_ns[n], population[n, 3]) of the population steps since the last call (device %globaltimer;
+        e-, e+, gamma tracks that entered each step)."""
         t = np.zeros(cap, dtype=np.uint64)
-        pop = np.zeros(cap, dtype=np.uint32)
+        pop = np.zeros((cap, 3), dtype=np.uint32)
         n = C.c_size_t(0)
         _check(lib.adept_get_iteration_trace(self.ctx, slot, _ptr(t), _ptr(pop), cap, C.byref(n)))
         return t[:n.value], pop[:n.value]

@@ -151,6 +151,7 @@ struct SlotHost {
   SlotCounters* pinned = nullptr;    // host mirror of the counters
   unsigned long long launches = 0;
   bool live = false;
+  size_t n_pending = 0, n_injected = 0;   // staggered injection: primaries in the pending store / already injected
   // optional per-launch timing (config.time_kernels)
   std::vector<cudaEvent_t> tev;      // [sync_interval][kTimed kernels][start, stop]
   int tev_used = 0;
@@ -275,8 +276,9 @@ size_t carve(void* base, const adept_config* cfg, const adept_geometry* g, int n
     d.ledger = cv.take<double>(8);
     d.stats = cv.take<DevStats>(1);
     d.leaked = cv.take<adept_track>(std::max<size_t>(cfg->leak_capacity, 1));
+    d.pending = cfg->inject_chunk ? cv.take<adept_track>(cfg->pending_capacity ? cfg->pending_capacity : cap) : nullptr;
     d.trace_t = cv.take<unsigned long long>(ADEPT_TRACE_CAPACITY);
-    d.trace_pop = cv.take<uint32_t>(ADEPT_TRACE_CAPACITY);
+    d.trace_pop = cv.take<uint32_t>(3 * ADEPT_TRACE_CAPACITY);
     d.trace_n = cv.take<uint32_t>(1);
     L.slots.push_back(d);
   }
@@ -493,6 +495,10 @@ extern "C" int adept_enqueue_batch(adept_ctx* ctx, int slot, int n, const uint32
   if (n < 0 || (n > 0 && (!event_ids || !track_ids || !species || !pos3 || !dir3 || !ekin))) return fail(ADEPT_EINVAL, "null argument");
   SlotHost& sh = ctx->slots[slot];
   if (sh.live) return fail(ADEPT_ESTATE, "slot %d is being transported", slot);
+  const bool stagger = ctx->cfg.inject_chunk != 0;
+  const size_t pcap = ctx->cfg.pending_capacity ? ctx->cfg.pending_capacity : ctx->cfg.track_capacity;
+  if (stagger && sh.n_pending + static_cast<size_t>(n) > pcap)
+    return fail(ADEPT_EOVERFLOW, "slot %d: pending store full (%zu + %d > %zu primaries)", slot, sh.n_pending, n, pcap);
   std::vector<adept_track> host(std::min<size_t>(n, ctx->stage_cap));
   for (size_t done = 0; done < static_cast<size_t>(n);) {
     const size_t m = std::min(ctx->stage_cap, static_cast<size_t>(n) - done);
@@ -506,11 +512,13 @@ extern "C" int adept_enqueue_batch(adept_ctx* ctx, int slot, int n, const uint32
     CUDA_TRY(cudaMemcpy(ctx->d_stage, host.data(), m * sizeof(adept_track), cudaMemcpyHostToDevice));
     CUDA_TRY(cudaMemset(ctx->d_bad, 0, sizeof(uint32_t)));
     const int grid = static_cast<int>(std::min<size_t>((m + kBlock - 1) / kBlock, 4096));
-    enqueue_kernel<<<grid, kBlock>>>(ctx->dev, sh.dev, ctx->d_stage, static_cast<int>(m), ctx->d_bad);
+    enqueue_kernel<<<grid, kBlock>>>(ctx->dev, sh.dev, ctx->d_stage, static_cast<int>(m), ctx->d_bad,
+                                     stagger ? sh.dev.pending + sh.n_pending : nullptr);
     CUDA_TRY(cudaGetLastError());
     uint32_t bad = 0;
     CUDA_TRY(cudaMemcpy(&bad, ctx->d_bad, sizeof(uint32_t), cudaMemcpyDeviceToHost));
     if (bad) return fail(ADEPT_EINVAL, "%u primaries lie outside the world or have an unknown species", bad);
+    if (stagger) sh.n_pending += m;
     done += m;
   }
   return ADEPT_OK;
@@ -532,6 +540,13 @@ namespace {
 // interaction kernel over what they staged and the buffer swap.
 int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity) {
   constexpr int kEv = 2 * ADEPT_N_TIMED_KERNELS;
+  if (sh.n_injected < sh.n_pending) {   // staggered injection: the next chunk joins the population of this step
+    const size_t m = std::min<size_t>(ctx->cfg.inject_chunk, sh.n_pending - sh.n_injected);
+    inject_kernel<<<static_cast<int>(std::min<size_t>((m + kBlock - 1) / kBlock, 1024)), kBlock, 0, st>>>(
+        ctx->dev, sh.dev, parity, static_cast<uint32_t>(sh.n_injected), static_cast<uint32_t>(m));
+    sh.n_injected += m;
+    sh.launches += 1;
+  }
   const bool timed = ctx->timing_on && !sh.tev.empty() && sh.tev_used + kEv <= static_cast<int>(sh.tev.size());
   // a timed pass runs the kernels one after the other, so that an event pair brackets one kernel alone
   const bool fork = ctx->cfg.concurrent_species != 0 && !ctx->timing_on;
@@ -597,7 +612,8 @@ extern "C" int adept_transport_many(adept_ctx* ctx, int n_slots, const int* slot
       sh.tev_used = 0;
       if (sh.pinned->overflow.v) rc_final = fail(ADEPT_EOVERFLOW, "slot %d: track queue overflow (capacity %llu per species)",
                                                slots[k], static_cast<unsigned long long>(ctx->cfg.track_capacity));
-      if (sh.pinned->live.v == 0 || sh.pinned->overflow.v) {
+      if ((sh.pinned->live.v == 0 && sh.n_injected == sh.n_pending) || sh.pinned->overflow.v) {
+        sh.n_pending = sh.n_injected = 0;
         sh.live = false;
         --n_live;
         if (parity[k]) {  // leave the (empty) slot at parity 0 for the next enqueue
@@ -668,7 +684,7 @@ extern "C" int adept_get_iteration_trace(adept_ctx* ctx, int slot, uint64_t* t_n
   CUDA_TRY(cudaMemcpy(&m, sh.dev.trace_n, sizeof(uint32_t), cudaMemcpyDeviceToHost));
   const size_t k = std::min<size_t>(std::min<size_t>(m, cap), ADEPT_TRACE_CAPACITY);
   if (k && t_ns) CUDA_TRY(cudaMemcpy(t_ns, sh.dev.trace_t, k * sizeof(uint64_t), cudaMemcpyDeviceToHost));
-  if (k && population) CUDA_TRY(cudaMemcpy(population, sh.dev.trace_pop, k * sizeof(uint32_t), cudaMemcpyDeviceToHost));
+  if (k && population) CUDA_TRY(cudaMemcpy(population, sh.dev.trace_pop, 3 * k * sizeof(uint32_t), cudaMemcpyDeviceToHost));
   CUDA_TRY(cudaMemset(sh.dev.trace_n, 0, sizeof(uint32_t)));
   *n = k;
   return ADEPT_OK;

@@ -423,8 +423,8 @@ move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot sl
 __device__ __forceinline__ void finish_iteration(const DevSlot& slot, int parity) {
   SlotCounters* cnt = slot.counters;
   const int k = threadIdx.x;
-  uint32_t before = 0, live = 0;
-  for (int sp = 0; sp < 3; ++sp) { before += __ldcg(&cnt->count[parity][sp].v); live += __ldcg(&cnt->count[parity ^ 1][sp].v); }
+  uint32_t before = 0, live = 0, in_sp[3];
+  for (int sp = 0; sp < 3; ++sp) { in_sp[sp] = __ldcg(&cnt->count[parity][sp].v); before += in_sp[sp]; live += __ldcg(&cnt->count[parity ^ 1][sp].v); }
   __syncthreads();
   if (k < 3) cnt->count[parity][k].v = 0;
   else if (k < 3 + kNumStage) cnt->n_stage[k - 3].v = 0;
@@ -438,7 +438,8 @@ __device__ __forceinline__ void finish_iteration(const DevSlot& slot, int parity
       if (j < ADEPT_TRACE_CAPACITY) {
         unsigned long long now;
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
-        slot.trace_t[j] = now; slot.trace_pop[j] = before; *slot.trace_n = j + 1;
+        slot.trace_t[j] = now; *slot.trace_n = j + 1;
+        for (int sp = 0; sp < 3; ++sp) slot.trace_pop[3 * j + sp] = in_sp[sp];
       }
     }
   }
@@ -568,9 +569,12 @@ interact_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlo
   if (is_last) finish_iteration(slot, parity);
 }
 
-// Places primaries (G5: volume = Locate(p + eps d)) and appends them to the parity-0 buffers.
+// Places primaries (G5: volume = Locate(p + eps d)).  pending == nullptr: appends them to the parity-0
+// buffers.  Otherwise (staggered injection) stores the located primary i at pending[i]; inject_kernel
+// moves it into the population later.
 __global__ void __launch_bounds__(kBlock) enqueue_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot,
-                                                         const adept_track* __restrict__ prim, int n, uint32_t* bad) {
+                                                         const adept_track* __restrict__ prim, int n, uint32_t* bad,
+                                                         adept_track* __restrict__ pending) {
   const int n_round = (n + 31) & ~31;
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += gridDim.x * blockDim.x) {
     const bool active = i < n;
@@ -580,6 +584,12 @@ __global__ void __launch_bounds__(kBlock) enqueue_kernel(const __grid_constant__
                              p.pos[2] + c.eps_push * p.dir[2]);
     if (active && (v < 0 || p.species < 0 || p.species > 2)) { atomicAdd(bad, 1u); continue; }
     if (!active) continue;
+    if (pending) {
+      p.volume = static_cast<uint32_t>(v); p.step = 0;
+      pending[i] = p;
+      atomicAdd(slot.ledger + 4, carried_energy(p.species, p.ekin));
+      continue;
+    }
     const uint32_t j = atomicAdd(&slot.counters->count[0][p.species].v, 1u);
     if (j >= c.capacity) { slot.counters->overflow.v = 1; continue; }
     Track t;
@@ -588,6 +598,38 @@ __global__ void __launch_bounds__(kBlock) enqueue_kernel(const __grid_constant__
     store_track(slot.buf[0][p.species], j, t);
     atomicAdd(slot.ledger + 4, carried_energy(p.species, p.ekin));
     atomicAdd(&slot.counters->live.v, 1u);
+  }
+}
+
+// Staggered injection: appends the pending primaries [first, first + n) to
+// the buffers the population step about to start reads (launched before its move kernels on the same
+// stream).  One atomic per warp and species.
+__global__ void __launch_bounds__(kBlock) inject_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot,
+                                                        int parity, uint32_t first, uint32_t n) {
+  const uint32_t n_round = (n + 31u) & ~31u;
+  const int lane = threadIdx.x & 31;
+  const unsigned lt = (1u << lane) - 1u;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += gridDim.x * blockDim.x) {
+    const bool active = i < n;
+    adept_track p{};
+    if (active) p = slot.pending[first + i];
+    const int sp = active ? p.species : -1;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      const unsigned b = __ballot_sync(kFull, sp == d);
+      if (!b) continue;
+      uint32_t base = 0;
+      if (lane == __ffs(b) - 1) base = atomicAdd(&slot.counters->count[parity][d].v, static_cast<uint32_t>(__popc(b)));
+      base = __shfl_sync(kFull, base, __ffs(b) - 1);
+      if (sp == d) {
+        const uint32_t j = base + __popc(b & lt);
+        if (j >= c.capacity) { slot.counters->overflow.v = 1; continue; }
+        Track t;
+        t.x = p.pos[0]; t.y = p.pos[1]; t.z = p.pos[2]; t.dx = p.dir[0]; t.dy = p.dir[1]; t.dz = p.dir[2];
+        t.ekin = p.ekin; t.id = p.id; t.event = p.event; t.step = 0; t.vol = p.volume; t.species = d;
+        store_track(slot.buf[parity][d], j, t);
+      }
+    }
   }
 }
 

@@ -99,8 +99,9 @@ struct DevSlot {
   double* ledger;           // [5]: deposited, below_cut, escaped, killed, primary
   DevStats* stats;
   adept_track* leaked;      // [leak_capacity]
+  adept_track* pending;         // [pending_capacity] located primaries waiting for injection (inject_chunk > 0)
   unsigned long long* trace_t;  // [ADEPT_TRACE_CAPACITY] %globaltimer at the end of each population step
-  uint32_t* trace_pop;          // [ADEPT_TRACE_CAPACITY] population that entered it
+  uint32_t* trace_pop;          // [ADEPT_TRACE_CAPACITY][3] e-, e+, gamma tracks that entered it
   uint32_t* trace_n;            // entries written since adept_get_iteration_trace
   TrackSoA stage[kNumStage];  // tracks waiting for their discrete interaction (stage_capacity entries each)
 };
