@@ -3,7 +3,7 @@
 // Same arithmetic, in the same order, as step_move<MODE_CHARGED> (step.cuh), which stays the reference
 // implementation behind the frozen-step hook.  The generic kernel needs 166 registers, i.e. three
 // resident blocks (12 warps) per SM, and at that occupancy it issues 0.39 instructions per cycle and
-// scheduler with `wait` (fixed-latency fp64 dependencies) as its top stall (profiles/r1c_summary.md):
+// scheduler with `wait` (fixed-latency fp64 dependencies) as its top stall (profiles/r1d_summary.md):
 // throughput is set by the number of resident warps.  As in gamma.cuh the lane's track stays in its
 // slot of the shared-memory tile and is read at the point of use; in addition the lane WRITES its
 // post-step direction and energy back into that slot before the relocation call, so the tile is the

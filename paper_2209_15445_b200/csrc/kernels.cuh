@@ -180,7 +180,7 @@ __device__ __forceinline__ void block_reserve(BlockReserve<ND>& br, int phase, c
 // as many L2 slices; adept_read_scoring folds the replicas in a fixed order.  Combining the lanes of a
 // warp by volume first (match_any + shuffles, one atomic per group) was measured 5 % slower per config-2
 // pass once the replicas had removed the contention: the ~40 instructions per warp cost more than the
-// reductions they save (profiles/r1e_summary.md).
+// reductions they save.
 __device__ __forceinline__ void score(const DevSlot& slot, uint32_t vol, double e, bool active) {
   if (active && e != 0.0) {
     const uint32_t rep = (blockIdx.x * kWarps + (threadIdx.x >> 5)) & slot.edep_mask;
