@@ -46,8 +46,12 @@ def parse():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--events", type=int, default=10000, help="showers per batch (config 2: 10000)")
-    ap.add_argument("--field", type=float, default=0.0, help="uniform Bz in tesla (config 3: 1.0)")
+    ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4],
+                    help="BASELINE.json config: 2 (default, the bench line), 3 (same + 1 T field), 4 (barrel, BVH, field map; extra)")
+    ap.add_argument("--events", type=int, default=0, help="events per batch (0 = 10000 for configs 2-3, 100 x 50 primaries for config 4)")
+    ap.add_argument("--field", type=float, default=0.0, help="uniform Bz in tesla for configs 2-3 (config 3 sets 1.0)")
+    ap.add_argument("--max-steps", type=int, default=0, help="looper cut S4 (0 = 1e6 for configs 2-3, 4096 for config 4)")
+    ap.add_argument("--inject-chunk", type=int, default=0, help="staggered injection: primaries per population step (0 = all at once)")
     ap.add_argument("--capacity", type=int, default=0, help="track capacity per species (0 = auto)")
     ap.add_argument("--sync-interval", type=int, default=8)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -56,7 +60,21 @@ def parse():
     ap.add_argument("--profile", action="store_true",
                     help="for runs under ncu: take --warmup literally (the timed numbers of such a run are not bench values)")
     ap.add_argument("--cpu-events-per-core", type=int, default=96)
-    return ap.parse_args()
+    a = ap.parse_args()
+    if a.config == 3 and a.field == 0.0:
+        a.field = 1.0
+    a.events = a.events or (100 if a.config == 4 else 10000)
+    a.max_steps = a.max_steps or (4096 if a.config == 4 else 1000000)
+    return a
+
+
+def workload_name(args):
+    if args.config == 4:
+        return (f"config4: barrel of 61200 PbWO4 crystals + 10 Si shells, BVH navigation, solenoid field map (RK4), "
+                f"{args.events} events x 50 e-/gamma of 1-100 GeV, looper cut max_steps={args.max_steps}")
+    if args.field != 0.0:
+        return f"config3: {args.events} x 10 GeV e- in the 50-layer Pb/LAr calorimeter, uniform {args.field} T field, 0.7 mm cuts"
+    return f"config2: {args.events} x 10 GeV e- in the 50-layer Pb/LAr calorimeter, no field, 0.7 mm cuts"
 
 
 def shard_first_event(rank, events_per_rank):
@@ -79,46 +97,61 @@ def reduce_over_ranks(dist, dev, t_max, c_sum):
 
 def workload(args, first_event=0):
     from paper_2209_15445_b200.inputs import field, geometry, materials, primaries
-    g = geometry.calorimeter()
+    if args.config == 4:
+        g = geometry.barrel()
+        fld = field.solenoid_map()
+        prim = primaries.barrel_events(args.events, 50, 1000.0, 100000.0, mode="cfg4", seed=1, first_event=first_event)
+    else:
+        g = geometry.calorimeter()
+        fld = field.uniform_field(0, 0, args.field) if args.field != 0.0 else field.no_field()
+        prim = primaries.beam(args.events, E_PRIMARY, spread=1.0, seed=1, first_event=first_event)
     mats, tabs, scal = materials.build_material_set(g.material_names)
-    fld = field.uniform_field(0, 0, args.field) if args.field != 0.0 else field.no_field()
-    prim = primaries.beam(args.events, E_PRIMARY, spread=1.0, seed=1, first_event=first_event)
     return g, tabs, scal, fld, prim
 
 
 # ----------------------------------------------------------------------------- CPU oracle legs
 def _oracle_worker(job):
-    first_event, n_events, field_bz = job
+    config, first_event, n_events, field_bz, max_steps = job
     from oracle import binding as ob
     from paper_2209_15445_b200.inputs import field, geometry, materials, primaries
-    g = geometry.calorimeter()
+    if config == 4:     # the loop navigator over 61 212 volumes: low-energy primaries of the same generator
+        g = geometry.barrel()
+        fld = field.solenoid_map()
+        prim = primaries.barrel_events(n_events, 2, 200.0, 2000.0, mode="cfg4", seed=1, first_event=first_event)
+    else:
+        g = geometry.calorimeter()
+        fld = field.uniform_field(0, 0, field_bz) if field_bz != 0.0 else field.no_field()
+        prim = primaries.beam(n_events, E_PRIMARY, spread=1.0, seed=1, first_event=first_event)
     _, tabs, scal = materials.build_material_set(g.material_names)
-    fld = field.uniform_field(0, 0, field_bz) if field_bz != 0.0 else field.no_field()
-    o = ob.Oracle(g, tabs, scal, fld)
-    tr = o.make_tracks(primaries.beam(n_events, E_PRIMARY, spread=1.0, seed=1, first_event=first_event))
+    o = ob.Oracle(g, tabs, scal, fld, max_steps=max_steps)
+    tr = o.make_tracks(prim)
     t0 = time.perf_counter()
     _, _, st = o.run(tr)
     return sum(st.steps), time.perf_counter() - t0
 
 
-def oracle_throughput(events_per_core, field_bz, cores=None):
+def oracle_throughput(args, events_per_core, cores=None):
     """Oracle as it stands: one single-threaded process per core over disjoint event ranges."""
     import multiprocessing as mp
     from oracle import build as obuild
     obuild.build()
     cores = cores or os.cpu_count() or 1
-    jobs = [(c * events_per_core, events_per_core, field_bz) for c in range(cores)]
+    if args.config == 4:
+        events_per_core = 1
+    jobs = [(args.config, c * events_per_core, events_per_core, args.field, args.max_steps) for c in range(cores)]
     ctx = mp.get_context("spawn")
-    t0 = time.perf_counter()
     with ctx.Pool(cores) as pool:
-        pool.map(_oracle_worker, [(0, 1, field_bz)] * cores)        # start-up (imports, build) untimed
+        pool.map(_oracle_worker, [(2, 0, 1, 0.0, args.max_steps)] * cores)        # start-up (imports, build) untimed
         t0 = time.perf_counter()
         res = pool.map(_oracle_worker, jobs)
         wall = time.perf_counter() - t0
     steps = sum(r[0] for r in res)
+    sample = (f"{cores} events of 2 e-/gamma primaries of 0.2-2 GeV from config 4's generator in the full barrel (one oracle "
+              f"process per core; the loop navigator makes full-energy events take minutes)" if args.config == 4 else
+              f"{cores * events_per_core} of the workload's 10 GeV e- showers ({events_per_core} consecutive events per core, "
+              f"one oracle process per core)")
     return {"steps": steps, "wall_s": wall, "steps_per_s": steps / wall, "showers_per_s": cores * events_per_core / wall,
-            "cores": cores, "sample": f"{cores * events_per_core} of the workload's 10 GeV e- showers "
-                                      f"({events_per_core} consecutive events per core, one oracle process per core)"}
+            "cores": cores, "sample": sample, "events": cores * events_per_core}
 
 
 def run_reference(args):
@@ -128,8 +161,8 @@ def run_reference(args):
     cores = os.cpu_count() or 1
     per_core = max(1, min(args.cpu_events_per_core, 32))
     for _ in range(min(args.warmup, 1)):
-        oracle_throughput(2, args.field, cores)
-    vals = [oracle_throughput(per_core, args.field, cores) for _ in range(args.steps)]
+        oracle_throughput(args, 2, cores)
+    vals = [oracle_throughput(args, per_core, cores) for _ in range(args.steps)]
     best = max(vals, key=lambda v: v["steps_per_s"])
     total_steps = sum(v["steps"] for v in vals)
     total_wall = sum(v["wall_s"] for v in vals)
@@ -137,9 +170,8 @@ def run_reference(args):
     line = {"impl": "reference", "metric": "track_steps_per_s", "value": v, "unit": "steps/s", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total_wall / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "config2: 50-layer Pb/LAr calorimeter, 10 GeV e- showers, no field"
-                       if args.field == 0.0 else "config3: same calorimeter, uniform 1 T field", "events_per_step": cores * per_core},
-            "showers_per_s": sum(cores * per_core for _ in vals) / total_wall,
+            "config": {"workload": workload_name(args), "events_per_step": best["events"]},
+            "showers_per_s": sum(x["events"] for x in vals) / total_wall,
             "cpu_baseline": {"value": v, "unit": "steps/s", "cores": cores, "kind": "oracle", "sample": best["sample"]},
             "e2e": {"value": v, "unit": "steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -196,8 +228,10 @@ def run_ours(args):
 
     # events shard over ranks with no data-path collective: weak scaling
     g, tabs, scal, fld, prim = workload(args, first_event=shard_first_event(rank, args.events))
-    cap = args.capacity or max(1 << 20, 1024 * args.events)
+    cap = args.capacity or (max(1 << 20, 65536 * args.events) if args.config == 4 else max(1 << 20, 1024 * args.events))
     a = adept.Adept(g, tabs, scal, fld, device=str(dev), track_capacity=cap, sync_interval=args.sync_interval,
+                    stage_capacity=max(1 << 16, cap // 4) if args.config == 4 else 0, max_steps=args.max_steps,
+                    inject_chunk=args.inject_chunk, pending_capacity=len(prim["ekin"]) if args.inject_chunk else 0,
                     time_kernels=0 if args.no_kernel_timing else 1)
     if not args.no_kernel_timing:
         a.set_kernel_timing(False)       # the timed passes run without per-launch events
@@ -295,8 +329,7 @@ def run_ours(args):
             "metric": "track_steps_per_s", "value": steps_all / t_dev, "unit": "steps/s", "n_gpus": world,
             "steps": args.steps, "warmup": n_warm, "ms_per_step": 1e3 * t_dev / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": ("config2: 10000 x 10 GeV e- in the 50-layer Pb/LAr calorimeter, no field, 0.7 mm cuts"
-                                    if args.field == 0.0 else f"config3: same calorimeter, uniform {args.field} T field"),
+            "config": {"workload": workload_name(args), "inject_chunk": args.inject_chunk,
                        "events_per_step_per_gpu": args.events, "track_capacity": cap, "sync_interval": args.sync_interval,
                        "l2": "256 MB buffer written between passes (L2 flush); peak live track state also exceeds L2",
                        "parallelism": f"events sharded over {world} GPU(s), no data-path collective"},
@@ -319,10 +352,12 @@ def run_ours(args):
             "iterations_per_step": (st.iterations - st0.iterations) / args.steps,
             "track_steps_per_species_per_step": {"e-": steps_sp[0] / n_pass, "e+": steps_sp[1] / n_pass, "gamma": steps_sp[2] / n_pass},
             "peak_population": int(st.peak_population),
+            "chords_per_step": (st.chords - st0.chords) / n_pass,
+            "killed_tracks_per_step": (st.outcomes[11] - st0.outcomes[11]) / n_pass,
             "wall_s_timed_region": t_wall,
         }
         if world == 1 and not args.no_cpu_baseline and not args.profile:
-            ob = oracle_throughput(args.cpu_events_per_core, args.field)
+            ob = oracle_throughput(args, args.cpu_events_per_core)
             line["cpu_baseline"] = {"value": ob["steps_per_s"], "unit": "steps/s", "cores": ob["cores"], "kind": "oracle",
                                     "sample": ob["sample"], "showers_per_s": ob["showers_per_s"]}
         print(json.dumps(line))

@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <numeric>
 #include <vector>
@@ -76,6 +77,65 @@ void world_aabb(const adept_geometry* g, int v, double lo[3], double hi[3]) {
     const double pad = 1e-9 + 1e-12 * (std::fabs(t[i]) + e);
     lo[i] = t[i] - e - pad;
     hi[i] = t[i] + e + pad;
+  }
+}
+
+// True if the placed boxes a and b are farther apart than `margin` (separating-axis test on the 15 axes of
+// two oriented boxes; conservative: false when in doubt).  Columns of R are the local axes in the world frame.
+bool boxes_apart(const adept_geometry* g, int a, int b, double margin) {
+  const double *Ra = g->rot + 9 * a, *Rb = g->rot + 9 * b, *ha = g->dims + 3 * a, *hb = g->dims + 3 * b;
+  const double T[3] = {g->trans[3 * b] - g->trans[3 * a], g->trans[3 * b + 1] - g->trans[3 * a + 1], g->trans[3 * b + 2] - g->trans[3 * a + 2]};
+  double A[3][3], B[3][3];
+  for (int j = 0; j < 3; ++j) for (int i = 0; i < 3; ++i) { A[j][i] = Ra[3 * i + j]; B[j][i] = Rb[3 * i + j]; }
+  auto apart_on = [&](const double L[3]) {
+    const double n = std::sqrt(L[0] * L[0] + L[1] * L[1] + L[2] * L[2]);
+    if (n < 1e-9) return false;
+    double ra = 0.0, rb = 0.0;
+    for (int j = 0; j < 3; ++j) {
+      ra += ha[j] * std::fabs(A[j][0] * L[0] + A[j][1] * L[1] + A[j][2] * L[2]);
+      rb += hb[j] * std::fabs(B[j][0] * L[0] + B[j][1] * L[1] + B[j][2] * L[2]);
+    }
+    return std::fabs(T[0] * L[0] + T[1] * L[1] + T[2] * L[2]) > ra + rb + (margin + 1e-9) * n;
+  };
+  for (int j = 0; j < 3; ++j) if (apart_on(A[j]) || apart_on(B[j])) return true;
+  for (int j = 0; j < 3; ++j)
+    for (int k = 0; k < 3; ++k) {
+      const double L[3] = {A[j][1] * B[k][2] - A[j][2] * B[k][1], A[j][2] * B[k][0] - A[j][0] * B[k][2], A[j][0] * B[k][1] - A[j][1] * B[k][0]};
+      if (apart_on(L)) return true;
+    }
+  return false;
+}
+
+// DevVolume::isolated for the daughters of volume m: a box daughter is isolated when every sibling is
+// farther than `margin` from it.  Sweep along the axis on which the daughters spread most; pairs whose
+// padded world boxes overlap are decided by boxes_apart (a tube sibling counts as near).
+void mark_isolated(const adept_geometry* g, int m, double margin, std::vector<int32_t>& isolated) {
+  const int b0 = g->daughter_begin[m], n = g->daughter_count[m];
+  std::vector<double> lo(3 * static_cast<size_t>(n)), hi(3 * static_cast<size_t>(n));
+  double span[3] = {0, 0, 0}, mn[3] = {1e300, 1e300, 1e300}, mx[3] = {-1e300, -1e300, -1e300};
+  for (int k = 0; k < n; ++k) {
+    world_aabb(g, b0 + k, &lo[3 * k], &hi[3 * k]);
+    for (int i = 0; i < 3; ++i) { mn[i] = std::min(mn[i], lo[3 * k + i]); mx[i] = std::max(mx[i], hi[3 * k + i]); }
+    isolated[b0 + k] = g->solid[b0 + k] == ADEPT_BOX ? 1 : 0;
+  }
+  for (int i = 0; i < 3; ++i) span[i] = mx[i] - mn[i];
+  const int ax = span[0] >= span[1] && span[0] >= span[2] ? 0 : (span[1] >= span[2] ? 1 : 2);
+  const int a1 = (ax + 1) % 3, a2 = (ax + 2) % 3;
+  std::vector<int> order(n);
+  std::iota(order.begin(), order.end(), 0);
+  std::sort(order.begin(), order.end(), [&](int p, int q) { return lo[3 * p + ax] < lo[3 * q + ax]; });
+  for (int ii = 0; ii < n; ++ii) {
+    const int p = order[ii];
+    for (int jj = ii + 1; jj < n; ++jj) {
+      const int q = order[jj];
+      if (lo[3 * q + ax] > hi[3 * p + ax] + margin) break;
+      if (lo[3 * q + a1] > hi[3 * p + a1] + margin || lo[3 * p + a1] > hi[3 * q + a1] + margin) continue;
+      if (lo[3 * q + a2] > hi[3 * p + a2] + margin || lo[3 * p + a2] > hi[3 * q + a2] + margin) continue;
+      if (!isolated[b0 + p] && !isolated[b0 + q]) continue;
+      const bool both_boxes = g->solid[b0 + p] == ADEPT_BOX && g->solid[b0 + q] == ADEPT_BOX;
+      if (both_boxes && boxes_apart(g, b0 + p, b0 + q, margin)) continue;
+      isolated[b0 + p] = 0; isolated[b0 + q] = 0;
+    }
   }
 }
 
@@ -308,6 +368,16 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   const int nv = g->n_volumes;
   std::vector<DevVolume> hv(nv);
   std::vector<DevBvh> hb;
+  std::vector<int32_t> isolated(nv, 0);
+  for (int v = 0; v < nv; ++v)
+    if (g->daughter_count[v] >= kBvhMinDaughters) {
+      mark_isolated(g, v, kIsolationMargin, isolated);
+      if (std::getenv("ADEPT_VERBOSE")) {
+        const int b0 = g->daughter_begin[v], n = g->daughter_count[v];
+        std::fprintf(stderr, "adept_init: volume %d: %d of %d daughters isolated (margin %g cm)\n", v,
+                     static_cast<int>(std::count(isolated.begin() + b0, isolated.begin() + b0 + n, 1)), n, kIsolationMargin);
+      }
+    }
   for (int v = 0; v < nv; ++v) {
     DevVolume& d = hv[v];
     for (int k = 0; k < 3; ++k) { d.t[k] = g->trans[3 * v + k]; d.dims[k] = g->dims[3 * v + k]; }
@@ -316,7 +386,7 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
     d.solid = g->solid[v]; d.material = g->material[v];
     d.dbegin = g->daughter_begin[v]; d.dcount = g->daughter_count[v];
     d.identity = ident ? 1 : 0;
-    d.mother = g->mother[v]; d.pad = 0;
+    d.mother = g->mother[v]; d.isolated = isolated[v];
     d.bvh = -1;
     if (d.dcount >= kBvhMinDaughters) {
       const HostBvh b = build_bvh(g, v);

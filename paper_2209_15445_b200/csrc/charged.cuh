@@ -35,7 +35,15 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
   // photons of an annihilation at rest)
   constexpr int ND = 5;
   const int q0 = positron ? 5 : 3;
-  if (blockIdx.x >= (n + kBlock - 1) / kBlock) return;   // no tile for this block (tail of a shower: most blocks)
+  // Tracks per tile.  A population smaller than the grid's lanes is spread over all blocks and warps
+  // (g tracks per tile, one lane in every 128/g): the warp-cooperative BVH serves the queries of a warp
+  // one after the other, so a few hundred loopers packed into a few warps would take 32 x 16 chord queries
+  // in sequence per step (measured 4 ms per population step on config 4), spread out they run in parallel.
+  uint32_t g = kBlock;
+  while (g > 4 && (n + (g >> 1) - 1) / (g >> 1) <= gridDim.x) g >>= 1;
+  const uint32_t lane_stride = kBlock / g;
+  const uint32_t n_tiles = (n + g - 1) / g;
+  if (blockIdx.x >= n_tiles) return;   // no tile for this block
   __shared__ BlockTally tally;
   __shared__ BlockReserve<ND> br;
   __shared__ TilePipe pipe;
@@ -46,19 +54,20 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
   unsigned long long packed = 0;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const unsigned lt = (1u << lane) - 1u;
-  const int t = threadIdx.x;
+  const int t = threadIdx.x / lane_stride;                 // this lane's entry of the tile
+  const bool mine = threadIdx.x % lane_stride == 0;
   enum { FATE_NONE = 0, FATE_KILLED, FATE_STOPPED, FATE_GO };
 
-  const uint32_t n_tiles = (n + kBlock - 1) / kBlock;
-  if (t == 0 && blockIdx.x < n_tiles) tile_issue(pipe.tile[0], cur, blockIdx.x, &pipe.bar[0]);
+  if (threadIdx.x == 0) tile_issue_n(pipe.tile[0], cur, static_cast<size_t>(blockIdx.x) * g, g, &pipe.bar[0]);
   uint32_t k = 0;
   for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++k) {
     const int phase = k & 1;
-    if (t == 0 && tile + gridDim.x < n_tiles) tile_issue(pipe.tile[phase ^ 1], cur, tile + gridDim.x, &pipe.bar[phase ^ 1]);
+    if (threadIdx.x == 0 && tile + gridDim.x < n_tiles)
+      tile_issue_n(pipe.tile[phase ^ 1], cur, static_cast<size_t>(tile + gridDim.x) * g, g, &pipe.bar[phase ^ 1]);
     mbar_wait(&pipe.bar[phase], (k >> 1) & 1);
     TrackTile& T = pipe.tile[phase];
     const uint32_t vol = T.u[2][t];
-    const bool active = tile * kBlock + t < n && vol != kDeadVolume;
+    const bool active = mine && tile * g + t < n && vol != kDeadVolume;
 
     // ---- phase A: step-start rules, physics step limit (A3), process choice (U1)
     int fate = FATE_NONE, process = 0, mat = 0;

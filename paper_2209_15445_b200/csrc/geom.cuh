@@ -190,8 +190,11 @@ __device__ __forceinline__ bool point_box(const double* __restrict__ box, int st
 
 // All arguments warp-uniform.  Returns min(best, nearest daughter entry distance).  The traversal
 // state is a short stack of one 32-bit child mask per level, shared by the warp.
+// `hit` (warp-uniform, out): touchable id of the daughter that gave the returned minimum, -1 if none did
+// or two daughters tie.
 __device__ __noinline__ double bvh_ray(const DevCtx& c, const DevBvh& b, double px, double py, double pz, double dx, double dy,
-                          double dz, double best) {
+                          double dz, double best, int& hit) {
+  hit = -1;
   const int lane = threadIdx.x & 31;
   const double ix = 1.0 / dx, iy = 1.0 / dy, iz = 1.0 / dz;
   const int top = b.n_levels - 1;
@@ -214,9 +217,18 @@ __device__ __noinline__ double bvh_ray(const DevCtx& c, const DevBvh& b, double 
     if (level == 0) {
       const int i = base + lane;
       double t = ADEPT_INF;
-      if (ray_box(b.prim_box, b.n_prims, i, i < b.n_prims, px, py, pz, ix, iy, iz, best))
-        t = entry_distance(c, __ldg(b.prim_vol + i), px, py, pz, dx, dy, dz);
-      best = fmin(best, warp_min(t));
+      int pv = -1;
+      if (ray_box(b.prim_box, b.n_prims, i, i < b.n_prims, px, py, pz, ix, iy, iz, best)) {
+        pv = __ldg(b.prim_vol + i);
+        t = entry_distance(c, pv, px, py, pz, dx, dy, dz);
+      }
+      const double m = warp_min(t);
+      if (m < best) {
+        best = m;
+        const unsigned w = __ballot_sync(kFull, t == m);
+        hit = __shfl_sync(kFull, pv, __ffs(w) - 1);
+        if (w & (w - 1)) hit = -1;
+      }
     } else {
       const int n = b.n_nodes[level - 1];
       const int i = base + lane;
@@ -269,9 +281,10 @@ __device__ __noinline__ int bvh_point(const DevCtx& c, const DevBvh& b, double p
 // min(exit distance of the own solid, entry distance of every daughter), capped at s_max.
 // Warp-convergent call; lanes with active == false return s_max.
 // BVH = false instantiates the pure loop navigator (geometries without a BVH volume): no cooperative code.
-// `face` (out): when the returned distance is the exit of the volume's own box through one face and no
-// daughter is entered first, the face index 2 * axis + (direction > 0) in the volume's frame -- the key of
-// the relocation hint table (nav_relocate); -1 otherwise.
+// `face` (out) is the relocation hint (nav_relocate): when the returned distance is the exit of the volume's
+// own box through one face and no daughter is entered first, the face index 2 * axis + (direction > 0) in
+// the volume's frame -- the key of the hint table; when it is the entry into daughter d, -2 - d; -1 when
+// neither is known (the cap s_max, a tube, a tie).
 template <bool BVH = true>
 __device__ __noinline__ double nav_distance(const DevCtx& c, int nav, bool active, double px, double py, double pz, double dx,
                                double dy, double dz, uint32_t vol, double s_max, int& face) {
@@ -295,7 +308,7 @@ __device__ __noinline__ double nav_distance(const DevCtx& c, int nav, bool activ
       } else {
         for (int k = 0; k < v.dcount; ++k) {
           const double e = entry_distance(c, v.dbegin + k, px, py, pz, dx, dy, dz);
-          if (e <= s) { if (e < s) s = e; face = -1; }
+          if (e <= s) { face = e < s ? -2 - (v.dbegin + k) : -1; s = e; }
         }
       }
     }
@@ -305,10 +318,11 @@ __device__ __noinline__ double nav_distance(const DevCtx& c, int nav, bool activ
   while (m) {
     const int src = __ffs(m) - 1;
     m &= m - 1;
+    int hit;
     const double r = bvh_ray(c, c.bvh[__shfl_sync(kFull, bvh, src)], __shfl_sync(kFull, px, src),
                              __shfl_sync(kFull, py, src), __shfl_sync(kFull, pz, src), __shfl_sync(kFull, dx, src),
-                             __shfl_sync(kFull, dy, src), __shfl_sync(kFull, dz, src), __shfl_sync(kFull, s, src));
-    if (lane == src && r < s) { s = r; face = -1; }
+                             __shfl_sync(kFull, dy, src), __shfl_sync(kFull, dz, src), __shfl_sync(kFull, s, src), hit);
+    if (lane == src && r < s) { s = r; face = hit >= 0 ? -2 - hit : -1; }
   }
   return s;
 }
@@ -383,25 +397,40 @@ __device__ __noinline__ int nav_locate(const DevCtx& c, int nav, bool active, do
 // (relocation cost and "fewer trial steps").  Warp-convergent call when BVH is true.
 // Returns -1 outside the world or for inactive lanes.
 //
-// Hint table (DevCtx::nbr, built once by adept_init with hint_kernel): nbr[6 v + f] = Locate of the point
-// just outside the centre of face f of box volume v.  A track that left v through face f (nav_distance
-// reports f) is tested against that one candidate first; if the pushed point is inside it, the descent
+// Hints (`face`, from nav_distance).  face >= 0: hint table (DevCtx::nbr, built once by adept_init with
+// hint_kernel): nbr[6 v + f] = Locate of the point just outside the centre of face f of box volume v.
+// face <= -2: the daughter -2 - face the step ended on.  Either way that one candidate is tested first; if the pushed point is inside it, the descent
 // starts there -- the deepest volume containing q is unique, so the answer is the same as the climb's --
 // and in a stack of slabs a crossing costs one containment test instead of four or five dependent ones.
 template <bool BVH = true>
 __device__ __noinline__ int nav_relocate(const DevCtx& c, int nav, bool active, uint32_t vol_old, double qx, double qy,
                                          double qz, int face = -1) {
   int cur = -1, prev = -1;
-  bool desc = false;
+  bool desc = false, done = false;
   if (active) {
-    const int cand = face >= 0 ? __ldg(c.nbr + 6 * static_cast<size_t>(vol_old) + face) : -1;
+    const int cand = face >= 0 ? __ldg(c.nbr + 6 * static_cast<size_t>(vol_old) + face) : (face <= -2 ? -2 - face : -1);
     if (cand >= 0 && inside_volume(c, cand, qx, qy, qz)) {
       cur = cand;
+      // Out of an ISOLATED daughter (adept_init: a box with no sibling within kIsolationMargin of it) into
+      // its mother: a point outside the box but within margin / 2 of it along every local axis is nearer
+      // than the margin to the box, so no sibling can contain it and the mother is the answer -- no
+      // descent, i.e. no BVH point query per crystal-to-gap crossing.  Checked here, not assumed, so the
+      // result is Locate(q) for any q and any hint.
+      if (face >= 0) {
+        const DevVolume& vo = volume(c, vol_old);
+        if (vo.isolated && vo.mother == cand) {
+          double l[3];
+          to_local(c, vol_old, vo, qx, qy, qz, l);
+          const double a0 = fabs(l[0]) - vo.dims[0], a1 = fabs(l[1]) - vo.dims[1], a2 = fabs(l[2]) - vo.dims[2];
+          const double out = fmax(a0, fmax(a1, a2));      // > 0: outside the box; <= margin / 2: within reach of no sibling
+          done = out > 0.0 && out <= 0.5 * kIsolationMargin;
+        }
+      }
     } else {
       cur = static_cast<int>(vol_old);
       while (cur >= 0 && !inside_volume(c, cur, qx, qy, qz)) { prev = cur; cur = volume(c, cur).mother; }
     }
-    desc = cur >= 0;
+    desc = cur >= 0 && !done;
   }
   for (;;) {
     if (BVH) { if (!__any_sync(kFull, desc)) break; } else if (!desc) break;

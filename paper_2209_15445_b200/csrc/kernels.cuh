@@ -107,6 +107,18 @@ __device__ __forceinline__ void tile_issue(TrackTileT<N>& t, const TrackSoA& b, 
   bulk_load(t.u[2], b.vol + base, N * 4, bar);
 }
 
+// same for the first g entries of a tile (g a power of two >= 4, so every copy is a multiple of 16 B):
+// sparse tiles of a small population (charged.cuh)
+__device__ __forceinline__ void tile_issue_n(TrackTile& t, const TrackSoA& b, size_t base, uint32_t g, uint64_t* bar) {
+  mbar_expect_tx(bar, g * 76u);
+  bulk_load(t.d[0], b.x + base, g * 8, bar); bulk_load(t.d[1], b.y + base, g * 8, bar);
+  bulk_load(t.d[2], b.z + base, g * 8, bar); bulk_load(t.d[3], b.dx + base, g * 8, bar);
+  bulk_load(t.d[4], b.dy + base, g * 8, bar); bulk_load(t.d[5], b.dz + base, g * 8, bar);
+  bulk_load(t.d[6], b.ekin + base, g * 8, bar); bulk_load(t.id, b.id + base, g * 8, bar);
+  bulk_load(t.u[0], b.event + base, g * 4, bar); bulk_load(t.u[1], b.step + base, g * 4, bar);
+  bulk_load(t.u[2], b.vol + base, g * 4, bar);
+}
+
 __device__ __forceinline__ Track tile_read(const TrackTile& t, int k, int species) {
   Track r;
   r.x = t.d[0][k]; r.y = t.d[1][k]; r.z = t.d[2][k];

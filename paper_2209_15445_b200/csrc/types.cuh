@@ -14,6 +14,7 @@ constexpr double kTmin = 1.0e-3;     // 1 keV
 constexpr int kNGrid = ADEPT_N_GRID;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr uint32_t kDeadVolume = 0xffffffffu;
+constexpr double kIsolationMargin = 1.0e-4;  // [cm] see DevVolume::isolated (1000 x the default boundary push)
 
 #define ADEPT_INF (__longlong_as_double(0x7ff0000000000000LL))
 
@@ -38,7 +39,7 @@ struct __align__(16) DevVolume {
   int32_t bvh;       // index into DevCtx::bvh, -1 = none (loop over daughters)
   int32_t identity;  // 1 if the rotation is the identity (transform reduces to a subtraction, bit-identical)
   int32_t mother;    // -1 for the world
-  int32_t pad;
+  int32_t isolated;  // 1: a box with no sibling within kIsolationMargin (adept_init), see nav_relocate
 };
 
 // Implicit complete 32-ary BVH over the daughters of one volume, in the world frame.
