@@ -224,6 +224,25 @@ int adept_get_kernel_times(adept_ctx*, int event_slot, double ms[ADEPT_N_TIMED_K
 #define ADEPT_TRACE_CAPACITY 4096
 int adept_get_iteration_trace(adept_ctx*, int event_slot, uint64_t* t_ns, uint32_t* population, size_t cap, size_t* n);
 
+/* ---- Hybrid-workflow boundary.  The host simulation hands over, one at
+ * a time, the tracks that enter the GPU region; they are buffered on the host until `threshold` of them
+ * trigger synchronous transport of the batch in `event_slot` on `cuda_stream`; adept_buffer_flush transports
+ * what is left (the paper's Flush, called when the host's own stack is empty).  Deposits of all batches
+ * accumulate per volume; tracks that left the world ("outgoing particles") are collected for the caller to
+ * put back on its stack.  The buffer owns host memory only and must be destroyed before adept_shutdown.
+ * adept_buffer_add / _flush return 1 when a batch was transported, 0 when not, < 0 on error.
+ * adept_buffer_take copies and clears what has accumulated (any of edep / ledger / outgoing may be NULL;
+ * outgoing needs room for *n_outgoing tracks: ask adept_buffer_pending first). */
+typedef struct adept_buffer adept_buffer;
+int adept_buffer_create(adept_buffer** out, adept_ctx*, int event_slot, size_t threshold, void* cuda_stream);
+int adept_buffer_add(adept_buffer*, uint32_t event_id, uint64_t track_id, int species, const double pos[3],
+                     const double dir[3], double ekin);
+int adept_buffer_flush(adept_buffer*);
+int adept_buffer_pending(const adept_buffer*, size_t* n_buffered, size_t* n_outgoing, uint64_t* n_batches);
+int adept_buffer_take(adept_buffer*, double* edep_per_volume, size_t n_volumes, adept_ledger* ledger,
+                      adept_track* outgoing, size_t cap, size_t* n_outgoing);
+int adept_buffer_destroy(adept_buffer*);
+
 /* Test hook: exactly one step for each of n tracks, results in input order; secondaries[2*i + k]. */
 int adept_step_frozen(adept_ctx*, int n, const adept_track* in, adept_step_result* out,
                       adept_track* secondaries, void* cuda_stream);

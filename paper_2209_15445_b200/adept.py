@@ -67,7 +67,8 @@ INTERACTION_OUTCOMES = (1, 2, 4, 5, 6, 12)
 EXPORTS = ["adept_last_error", "adept_default_config", "adept_workspace_bytes", "adept_init",
            "adept_enqueue_primaries", "adept_enqueue_batch", "adept_transport", "adept_transport_many",
            "adept_read_scoring", "adept_read_leaked", "adept_get_stats", "adept_get_kernel_times", "adept_set_kernel_timing", "adept_get_iteration_trace",
-           "adept_step_frozen",
+           "adept_buffer_create", "adept_buffer_add", "adept_buffer_flush", "adept_buffer_pending", "adept_buffer_take",
+           "adept_buffer_destroy", "adept_step_frozen",
            "adept_distance_batch", "adept_locate_batch", "adept_relocate_batch", "adept_shutdown"]
 
 
@@ -98,6 +99,12 @@ def load_library():
     lib.adept_locate_batch.argtypes = [vp, i, i, vp, vp, vp]
     lib.adept_relocate_batch.argtypes = [vp, i, i, vp, vp, vp, vp, vp]
     lib.adept_shutdown.argtypes = [vp]
+    lib.adept_buffer_create.argtypes = [C.POINTER(vp), vp, i, sz, vp]
+    lib.adept_buffer_add.argtypes = [vp, C.c_uint32, C.c_uint64, i, vp, vp, C.c_double]
+    lib.adept_buffer_flush.argtypes = [vp]
+    lib.adept_buffer_pending.argtypes = [vp, C.POINTER(sz), C.POINTER(sz), C.POINTER(C.c_uint64)]
+    lib.adept_buffer_take.argtypes = [vp, vp, sz, C.POINTER(CLedger), vp, sz, C.POINTER(sz)]
+    lib.adept_buffer_destroy.argtypes = [vp]
     return lib
 
 
@@ -274,3 +281,50 @@ class Adept:
         _check(lib.adept_relocate_batch(self.ctx, navigator, pos.shape[0], _ptr(pos), _ptr(frm),
                                         None if fc is None else _ptr(fc), _ptr(out), None))
         return out
+
+
+class HybridBuffer:
+    """Host-side track buffer of the hybrid workflow: add() tracks one at a time, a batch is
+    transported when `threshold` are buffered, flush() transports the rest, take() returns the accumulated
+    deposits, ledger and outgoing (leaked) tracks."""
+
+    def __init__(self, adept_obj, threshold, slot=0, stream=None):
+        self._a = adept_obj
+        self.h = C.c_void_p()
+        _check(lib.adept_buffer_create(C.byref(self.h), adept_obj.ctx, slot, threshold, _stream_ptr(stream)))
+
+    def add(self, event, track_id, species, pos, direc, ekin):
+        p = np.ascontiguousarray(pos, dtype=np.float64)
+        d = np.ascontiguousarray(direc, dtype=np.float64)
+        rc = lib.adept_buffer_add(self.h, int(event), int(track_id), int(species), _ptr(p), _ptr(d), float(ekin))
+        if rc < 0:
+            raise AdeptError(rc)
+        return rc == 1
+
+    def flush(self):
+        rc = lib.adept_buffer_flush(self.h)
+        if rc < 0:
+            raise AdeptError(rc)
+        return rc == 1
+
+    def pending(self):
+        a, b, c = C.c_size_t(0), C.c_size_t(0), C.c_uint64(0)
+        _check(lib.adept_buffer_pending(self.h, C.byref(a), C.byref(b), C.byref(c)))
+        return a.value, b.value, c.value
+
+    def take(self):
+        _, n_out, _ = self.pending()
+        edep = np.zeros(self._a.n_volumes)
+        led = CLedger()
+        out = np.zeros(max(n_out, 1), dtype=TRACK)
+        n = C.c_size_t(0)
+        _check(lib.adept_buffer_take(self.h, _ptr(edep), edep.shape[0], C.byref(led), _ptr(out), out.shape[0], C.byref(n)))
+        return edep, led, out[:n.value]
+
+    def close(self):
+        if getattr(self, "h", None):
+            lib.adept_buffer_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        self.close()

@@ -862,3 +862,103 @@ extern "C" int adept_relocate_batch(adept_ctx* ctx, int nav, int n, const double
   cudaFree(d_pos); cudaFree(d_from); cudaFree(d_out);
   return ADEPT_OK;
 }
+
+// ------------------------------------------------------------------------------------------------
+// Hybrid-workflow boundary: the host simulation hands tracks over one at
+// a time; they are buffered until a threshold triggers synchronous transport of the batch; Flush
+// transports what is left; deposits accumulate per volume and the tracks that left the world ("outgoing
+// particles") are kept for the caller to put back on its own stack.
+struct adept_buffer {
+  adept_ctx* ctx = nullptr;
+  int slot = 0;
+  size_t threshold = 0;
+  cudaStream_t stream = nullptr;
+  std::vector<uint32_t> event;
+  std::vector<uint64_t> id;
+  std::vector<int8_t> species;
+  std::vector<double> pos, dir, ekin;
+  std::vector<double> edep, scratch;       // accumulated per-volume deposits; one batch
+  adept_ledger ledger{};
+  std::vector<adept_track> outgoing;
+  uint64_t batches = 0, tracks_in = 0;
+};
+
+extern "C" int adept_buffer_create(adept_buffer** out, adept_ctx* ctx, int slot, size_t threshold, void* stream) {
+  if (!out) return fail(ADEPT_EINVAL, "null argument");
+  *out = nullptr;
+  const int rc = check_slot(ctx, slot);
+  if (rc != ADEPT_OK) return rc;
+  if (threshold < 1 || threshold > ctx->cfg.track_capacity) return fail(ADEPT_EINVAL, "threshold must be in [1, track_capacity]");
+  adept_buffer* b = new adept_buffer;
+  b->ctx = ctx; b->slot = slot; b->threshold = threshold; b->stream = static_cast<cudaStream_t>(stream);
+  b->edep.assign(ctx->n_vol, 0.0);
+  b->scratch.assign(ctx->n_vol, 0.0);
+  *out = b;
+  return ADEPT_OK;
+}
+
+extern "C" int adept_buffer_flush(adept_buffer* b) {
+  if (!b) return fail(ADEPT_EINVAL, "null buffer");
+  const int n = static_cast<int>(b->ekin.size());
+  if (n == 0) return 0;
+  int rc = adept_enqueue_batch(b->ctx, b->slot, n, b->event.data(), b->id.data(), b->species.data(), b->pos.data(),
+                               b->dir.data(), b->ekin.data());
+  if (rc != ADEPT_OK) return rc;
+  b->event.clear(); b->id.clear(); b->species.clear(); b->pos.clear(); b->dir.clear(); b->ekin.clear();
+  rc = adept_transport(b->ctx, b->slot, b->stream);
+  if (rc != ADEPT_OK) return rc;
+  adept_ledger led{};
+  rc = adept_read_scoring(b->ctx, b->slot, b->scratch.data(), b->scratch.size(), &led, b->stream);
+  if (rc != ADEPT_OK) return rc;
+  for (size_t v = 0; v < b->edep.size(); ++v) b->edep[v] += b->scratch[v];
+  b->ledger.deposited += led.deposited; b->ledger.below_cut += led.below_cut; b->ledger.escaped += led.escaped;
+  b->ledger.killed += led.killed; b->ledger.primary += led.primary;
+  size_t n_leaked = 0;
+  const size_t old = b->outgoing.size();
+  b->outgoing.resize(old + b->ctx->cfg.leak_capacity);
+  rc = adept_read_leaked(b->ctx, b->slot, b->outgoing.data() + old, b->ctx->cfg.leak_capacity, &n_leaked);
+  if (rc != ADEPT_OK) { b->outgoing.resize(old); return rc; }
+  b->outgoing.resize(old + std::min<size_t>(n_leaked, b->ctx->cfg.leak_capacity));
+  if (n_leaked > b->ctx->cfg.leak_capacity) return fail(ADEPT_EOVERFLOW, "%zu outgoing tracks, leak_capacity is %llu", n_leaked,
+                                                        static_cast<unsigned long long>(b->ctx->cfg.leak_capacity));
+  b->batches += 1;
+  return 1;
+}
+
+extern "C" int adept_buffer_add(adept_buffer* b, uint32_t event_id, uint64_t track_id, int species, const double pos[3],
+                                const double dir[3], double ekin) {
+  if (!b || !pos || !dir) return fail(ADEPT_EINVAL, "null argument");
+  if (species < 0 || species > 2) return fail(ADEPT_EINVAL, "unknown species %d", species);
+  if (!(ekin >= 0.0)) return fail(ADEPT_EINVAL, "negative or NaN energy");
+  b->event.push_back(event_id); b->id.push_back(track_id); b->species.push_back(static_cast<int8_t>(species));
+  for (int a = 0; a < 3; ++a) { b->pos.push_back(pos[a]); b->dir.push_back(dir[a]); }
+  b->ekin.push_back(ekin);
+  b->tracks_in += 1;
+  if (b->ekin.size() >= b->threshold) return adept_buffer_flush(b);
+  return 0;
+}
+
+extern "C" int adept_buffer_pending(const adept_buffer* b, size_t* n_buffered, size_t* n_outgoing, uint64_t* n_batches) {
+  if (!b) return fail(ADEPT_EINVAL, "null buffer");
+  if (n_buffered) *n_buffered = b->ekin.size();
+  if (n_outgoing) *n_outgoing = b->outgoing.size();
+  if (n_batches) *n_batches = b->batches;
+  return ADEPT_OK;
+}
+
+extern "C" int adept_buffer_take(adept_buffer* b, double* edep, size_t n_volumes, adept_ledger* ledger, adept_track* outgoing,
+                                 size_t cap, size_t* n_outgoing) {
+  if (!b) return fail(ADEPT_EINVAL, "null buffer");
+  if (edep && n_volumes != b->edep.size()) return fail(ADEPT_EINVAL, "n_volumes is %zu, geometry has %zu", n_volumes, b->edep.size());
+  if (outgoing && b->outgoing.size() > cap) return fail(ADEPT_EINVAL, "%zu outgoing tracks do not fit %zu", b->outgoing.size(), cap);
+  if (edep) { std::memcpy(edep, b->edep.data(), n_volumes * sizeof(double)); std::fill(b->edep.begin(), b->edep.end(), 0.0); }
+  if (ledger) { *ledger = b->ledger; b->ledger = adept_ledger{}; }
+  if (n_outgoing) *n_outgoing = b->outgoing.size();
+  if (outgoing) { std::memcpy(outgoing, b->outgoing.data(), b->outgoing.size() * sizeof(adept_track)); b->outgoing.clear(); }
+  return ADEPT_OK;
+}
+
+extern "C" int adept_buffer_destroy(adept_buffer* b) {
+  delete b;
+  return ADEPT_OK;
+}

@@ -41,7 +41,7 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
   // in sequence per step (measured 4 ms per population step on config 4), spread out they run in parallel.
   uint32_t g = kBlock;
   while (g > 4 && (n + (g >> 1) - 1) / (g >> 1) <= gridDim.x) g >>= 1;
-  const uint32_t lane_stride = kBlock / g;
+  const int lane_shift = __ffs(kBlock / g) - 1;            // every (1 << lane_shift)-th lane takes a track
   const uint32_t n_tiles = (n + g - 1) / g;
   if (blockIdx.x >= n_tiles) return;   // no tile for this block
   __shared__ BlockTally tally;
@@ -54,8 +54,8 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
   unsigned long long packed = 0;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const unsigned lt = (1u << lane) - 1u;
-  const int t = threadIdx.x / lane_stride;                 // this lane's entry of the tile
-  const bool mine = threadIdx.x % lane_stride == 0;
+  const int t = threadIdx.x >> lane_shift;                 // this lane's entry of the tile
+  const bool mine = (threadIdx.x & ((1u << lane_shift) - 1u)) == 0;
   enum { FATE_NONE = 0, FATE_KILLED, FATE_STOPPED, FATE_GO };
 
   if (threadIdx.x == 0) tile_issue_n(pipe.tile[0], cur, static_cast<size_t>(blockIdx.x) * g, g, &pipe.bar[0]);

@@ -290,3 +290,48 @@ def test_staggered_injection_gives_the_same_showers(ob, calo, chunk):
     assert s1.iterations >= s0.iterations
     if chunk < 64:
         assert s1.peak_population < s0.peak_population
+
+
+def test_hybrid_buffer_threshold_and_flush(ob, calo):
+    """tracks handed over one at a time, a batch transported whenever the
+    threshold is reached, Flush for the rest; accumulated deposits and ledger equal one transport of all
+    tracks (and the oracle's), outgoing tracks are the leaked ones."""
+    import torch
+    from paper_2209_15445_b200 import adept
+    from paper_2209_15445_b200.inputs import field, primaries
+    g, _, tabs, scal = calo
+    prim = primaries.beam(50, 300.0, spread=1.0)
+    prim["species"][1::3] = 1
+    prim["species"][2::3] = 2
+    prim["dir"][::7] = [0.0, 1.0, 0.0]            # some tracks start in front of the calorimeter and leave the world
+    prim["pos"][::7, 0] = -5.0                    # sideways: outgoing particles
+    o = ob.Oracle(g, tabs, scal, field.no_field())
+    oe, ol, ost = o.run(o.make_tracks(prim))
+    a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=1 << 16, n_event_slots=2)
+    a.enqueue(prim, slot=1)
+    a.transport(1, torch.cuda.current_stream())
+    e_all, led_all = a.read_scoring(1)
+    leaked_all, _ = a.read_leaked(1)
+    buf = adept.HybridBuffer(a, threshold=16, slot=0, stream=torch.cuda.current_stream())
+    flushed = 0
+    for i in range(50):
+        flushed += buf.add(prim["event"][i], 0, prim["species"][i], prim["pos"][i], prim["dir"][i], prim["ekin"][i])
+    assert flushed == 3 and buf.pending()[0] == 2 and buf.pending()[2] == 3
+    assert buf.flush() and not buf.flush()        # Flush transports the remaining two; nothing left afterwards
+    assert buf.pending()[0] == 0 and buf.pending()[2] == 4
+    e, led, out = buf.take()
+    np.testing.assert_allclose(e, e_all, rtol=1e-9, atol=1e-9)
+    np.testing.assert_allclose(e, oe, rtol=1e-9, atol=1e-9)
+    assert led.primary == pytest.approx(led_all.primary, rel=1e-13)
+    assert abs(led.total() - led.primary) <= 1e-9 * led.primary
+    assert led.escaped == pytest.approx(led_all.escaped, rel=1e-9) and led.escaped == pytest.approx(ol.escaped, rel=1e-9)
+    assert len(out) == len(leaked_all) > 0
+    key = lambda t: (int(t["event"]), int(t["id"]), int(t["step"]))
+    assert sorted(map(key, out)) == sorted(map(key, leaked_all))
+    assert sum(float(t["ekin"]) + (2 * M if t["species"] == 1 else 0.0) for t in out) == pytest.approx(led.escaped, rel=1e-9)
+    e2, led2, out2 = buf.take()                   # taking clears
+    assert e2.sum() == 0.0 and led2.primary == 0.0 and len(out2) == 0
+    with pytest.raises(adept.AdeptError):
+        buf.add(0, 0, 5, prim["pos"][0], prim["dir"][0], 1.0)
+    buf.close()
+    a.close()
