@@ -224,6 +224,14 @@ int adept_get_kernel_times(adept_ctx*, int event_slot, double ms[ADEPT_N_TIMED_K
 #define ADEPT_TRACE_CAPACITY 4096
 int adept_get_iteration_trace(adept_ctx*, int event_slot, uint64_t* t_ns, uint32_t* population, size_t cap, size_t* n);
 
+/* Ray-cast validator of the navigator (PAPER.md:49 and Fig. 1): ray i from pos3[i] along the unit
+ * vector dir3[i] is marched boundary by boundary -- distance to boundary, push, relocation: the calls of a photon
+ * step -- until it leaves the world or has crossed max_crossings boundaries.  column[i] = sum of path length x
+ * density [g/cm^2], crossings[i] = boundaries crossed (-1 if the ray starts outside the world).  Host arrays in
+ * and out; *device_ms (may be NULL) = CUDA-event time of the kernel.  The navigator is chosen here. */
+int adept_raycast_batch(adept_ctx*, int navigator, int n, const double* pos3, const double* dir3, int max_crossings,
+                        double* column, int32_t* crossings, double* device_ms, void* cuda_stream);
+
 /* ---- Hybrid-workflow boundary.  The host simulation hands over, one at
  * a time, the tracks that enter the GPU region; they are buffered on the host until `threshold` of them
  * trigger synchronous transport of the batch in `event_slot` on `cuda_stream`; adept_buffer_flush transports

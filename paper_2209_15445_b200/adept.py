@@ -67,7 +67,7 @@ INTERACTION_OUTCOMES = (1, 2, 4, 5, 6, 12)
 EXPORTS = ["adept_last_error", "adept_default_config", "adept_workspace_bytes", "adept_init",
            "adept_enqueue_primaries", "adept_enqueue_batch", "adept_transport", "adept_transport_many",
            "adept_read_scoring", "adept_read_leaked", "adept_get_stats", "adept_get_kernel_times", "adept_set_kernel_timing", "adept_get_iteration_trace",
-           "adept_buffer_create", "adept_buffer_add", "adept_buffer_flush", "adept_buffer_pending", "adept_buffer_take",
+           "adept_raycast_batch", "adept_buffer_create", "adept_buffer_add", "adept_buffer_flush", "adept_buffer_pending", "adept_buffer_take",
            "adept_buffer_destroy", "adept_step_frozen",
            "adept_distance_batch", "adept_locate_batch", "adept_relocate_batch", "adept_shutdown"]
 
@@ -99,6 +99,7 @@ def load_library():
     lib.adept_locate_batch.argtypes = [vp, i, i, vp, vp, vp]
     lib.adept_relocate_batch.argtypes = [vp, i, i, vp, vp, vp, vp, vp]
     lib.adept_shutdown.argtypes = [vp]
+    lib.adept_raycast_batch.argtypes = [vp, i, i, vp, vp, i, vp, vp, C.POINTER(C.c_double), vp]
     lib.adept_buffer_create.argtypes = [C.POINTER(vp), vp, i, sz, vp]
     lib.adept_buffer_add.argtypes = [vp, C.c_uint32, C.c_uint64, i, vp, vp, C.c_double]
     lib.adept_buffer_flush.argtypes = [vp]
@@ -238,6 +239,19 @@ class Adept:
 
     def set_kernel_timing(self, on):
         _check(lib.adept_set_kernel_timing(self.ctx, 1 if on else 0))
+
+    def raycast(self, pos, direc, navigator=NAV_BVH, max_crossings=100000, stream=None):
+        """(column density [g/cm^2], boundaries crossed, kernel ms) of n rays marched through the geometry."""
+        p = np.ascontiguousarray(pos, dtype=np.float64)
+        d = np.ascontiguousarray(direc, dtype=np.float64)
+        n = p.shape[0]
+        col = np.zeros(n)
+        nx = np.zeros(n, dtype=np.int32)
+        ms = C.c_double(0.0)
+        with self._torch.cuda.device(self.device):
+            _check(lib.adept_raycast_batch(self.ctx, navigator, n, _ptr(p), _ptr(d), max_crossings, _ptr(col), _ptr(nx),
+                                           C.byref(ms), _stream_ptr(stream)))
+        return col, nx, ms.value
 
     def iteration_trace(self, slot=0, cap=4096):
         """(t_ns[n], population[n, 3]) of the population steps since the last call (device %globaltimer;

@@ -817,6 +817,41 @@ extern "C" int adept_distance_batch(adept_ctx* ctx, int nav, int n, const double
   return ADEPT_OK;
 }
 
+extern "C" int adept_raycast_batch(adept_ctx* ctx, int nav, int n, const double* pos3, const double* dir3, int max_crossings,
+                                   double* column, int32_t* crossings, double* device_ms, void* stream) {
+  if (!ctx || n < 0 || (n > 0 && (!pos3 || !dir3 || !column || !crossings))) return fail(ADEPT_EINVAL, "null argument");
+  if (nav != ADEPT_NAV_LOOP && nav != ADEPT_NAV_BVH) return fail(ADEPT_EINVAL, "unknown navigator");
+  if (max_crossings < 1) return fail(ADEPT_EINVAL, "max_crossings must be >= 1");
+  if (n == 0) return ADEPT_OK;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  double *d_pos = nullptr, *d_dir = nullptr, *d_col = nullptr;
+  int32_t* d_nx = nullptr;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  int rc = ADEPT_OK;
+  const size_t nb = static_cast<size_t>(n) * 3 * sizeof(double);
+  do {
+    if (cudaMalloc(&d_pos, nb) != cudaSuccess || cudaMalloc(&d_dir, nb) != cudaSuccess ||
+        cudaMalloc(&d_col, static_cast<size_t>(n) * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&d_nx, static_cast<size_t>(n) * sizeof(int32_t)) != cudaSuccess ||
+        cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { rc = fail(ADEPT_ENOMEM, "ray-cast buffers"); break; }
+    if (cudaMemcpyAsync(d_pos, pos3, nb, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(d_dir, dir3, nb, cudaMemcpyHostToDevice, st) != cudaSuccess) { rc = fail(ADEPT_ECUDA, "ray-cast upload"); break; }
+    cudaEventRecord(e0, st);
+    raycast_kernel<<<std::min((n + kBlock - 1) / kBlock, 65535), kBlock, 0, st>>>(ctx->dev, nav, n, d_pos, d_dir, max_crossings, d_col, d_nx);
+    cudaEventRecord(e1, st);
+    if (cudaMemcpyAsync(column, d_col, static_cast<size_t>(n) * sizeof(double), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaMemcpyAsync(crossings, d_nx, static_cast<size_t>(n) * sizeof(int32_t), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) { rc = fail(ADEPT_ECUDA, "ray-cast kernel"); break; }
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (device_ms) *device_ms = ms;
+  } while (false);
+  cudaFree(d_pos); cudaFree(d_dir); cudaFree(d_col); cudaFree(d_nx);
+  if (e0) cudaEventDestroy(e0);
+  if (e1) cudaEventDestroy(e1);
+  return rc;
+}
+
 extern "C" int adept_locate_batch(adept_ctx* ctx, int nav, int n, const double* pos3, int64_t* out, void* stream) {
   if (!ctx || n < 0 || (n > 0 && (!pos3 || !out))) return fail(ADEPT_EINVAL, "null argument");
   if (n == 0) return ADEPT_OK;

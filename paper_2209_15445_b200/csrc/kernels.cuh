@@ -730,6 +730,42 @@ __global__ void __launch_bounds__(kBlock) locate_kernel(const __grid_constant__ 
   }
 }
 
+// Ray-cast validator of the navigator (Fig. 1): ray i starts at pos[i] along
+// dir[i] and is marched boundary by boundary -- distance to boundary (A4), push, relocation (A5), exactly the
+// calls a photon step makes -- until it leaves the world or has crossed max_crossings boundaries.
+// column[i] = sum of path x density [g/cm^2], crossings[i] = boundaries crossed (-1: start outside the world).
+__global__ void __launch_bounds__(kBlock) raycast_kernel(const __grid_constant__ DevCtx c, int nav, int n, const double* __restrict__ pos,
+                                                         const double* __restrict__ dir, int max_crossings, double* __restrict__ column,
+                                                         int32_t* __restrict__ crossings) {
+  const int n_round = (n + 31) & ~31;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += gridDim.x * blockDim.x) {
+    const bool a = i < n;
+    const int k = a ? i : 0;
+    double px = pos[3 * k], py = pos[3 * k + 1], pz = pos[3 * k + 2];
+    const double dx = dir[3 * k], dy = dir[3 * k + 1], dz = dir[3 * k + 2];
+    int vol = nav_locate(c, nav, a, px, py, pz);
+    bool alive = a && vol >= 0;
+    double col = 0.0;
+    int nx = alive ? 0 : -1;
+    while (__any_sync(kFull, alive)) {
+      int face;
+      const double s = nav_distance(c, nav, alive, px, py, pz, dx, dy, dz, alive ? static_cast<uint32_t>(vol) : 0u, ADEPT_INF, face);
+      if (alive) {
+        col += s * mat_scalar(c, volume(c, vol).material, S_RHO);
+        px += s * dx; py += s * dy; pz += s * dz;
+        px += c.eps_push * dx; py += c.eps_push * dy; pz += c.eps_push * dz;
+      }
+      const int nv = nav_relocate(c, nav, alive, alive ? static_cast<uint32_t>(vol) : 0u, px, py, pz, face);
+      if (alive) {
+        ++nx;
+        vol = nv;
+        if (nv < 0 || nx >= max_crossings) alive = false;
+      }
+    }
+    if (a) { column[i] = col; crossings[i] = nx; }
+  }
+}
+
 // Test hook for A5: relocation of point i starting from volume from[i] (any volume of the tree).
 __global__ void __launch_bounds__(kBlock) relocate_kernel(const __grid_constant__ DevCtx c, int nav, int n, const double* pos,
                                                           const uint32_t* from, const int32_t* face, long long* out) {

@@ -119,3 +119,69 @@ def test_relocation_from_any_volume_equals_locate(ob, barrel_full, calo, navigat
     assert np.array_equal(a.relocate_batch(pos, np.maximum(want, 0), navigator), want)
     assert np.array_equal(a.relocate_batch(pos, np.maximum(want, 0), navigator, face=rng.integers(-1, 6, n)), want)
     a.close()
+
+
+def _oracle_raycast(o, scal, g, pos, direc, max_crossings=10000, eps=1e-7):
+    """The same march with the oracle's Locate and loop-navigator distance (G3-G5), one ray at a time."""
+    col, nx = np.zeros(len(pos)), np.zeros(len(pos), dtype=np.int32)
+    for i, (p, d) in enumerate(zip(pos, direc)):
+        p = p.copy()
+        v = o.locate(p)
+        if v < 0:
+            nx[i] = -1
+            continue
+        while v >= 0 and nx[i] < max_crossings:
+            s = o.distance(p, d, v)
+            col[i] += s * scal[g.material[v]][7]
+            p = p + s * d
+            p = p + eps * d
+            nx[i] += 1
+            v = o.locate(p)
+    return col, nx
+
+
+def test_raycast_validator(ob, barrel_patch, barrel_full, tmp_path):
+    """SURVEY.md 8(f)3 / PAPER.md:49, Fig. 1: a picture of the geometry taken with the navigation calls of the
+    transport path.  Patch: equals the oracle's march (crossings exact, column density to rounding).  Full
+    barrel: the BVH picture equals the loop navigator's picture bit for bit; PPM written headless."""
+    from paper_2209_15445_b200 import adept, raycast
+    from paper_2209_15445_b200.inputs import field
+    g, _, tabs, scal = barrel_patch
+    o = ob.Oracle(g, tabs, scal, field.no_field())
+    a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=1 << 10)
+    rng = np.random.default_rng(11)
+    # rays from the origin into the patch (12 x 12 crystals around eta = 0, phi = 0..12 columns), and a few away from it
+    phi = rng.uniform(-0.02, 0.23, 300)
+    eta = rng.uniform(-0.12, 0.12, 300)
+    th = 2.0 * np.arctan(np.exp(-eta))
+    d = np.stack([np.sin(th) * np.cos(phi), np.sin(th) * np.sin(phi), np.cos(th)], axis=1)
+    d[-20:] = -d[-20:]
+    pos = np.zeros_like(d)
+    pos[-5:] = [400.0, 0.0, 0.0]                       # outside the world
+    col, nx, _ = a.raycast(pos, d, adept.NAV_BVH)
+    ocol, onx = _oracle_raycast(o, scal, g, pos, d)
+    assert np.array_equal(nx, onx) and (nx[-5:] == -1).all() and nx[:280].max() >= 8
+    np.testing.assert_allclose(col, ocol, rtol=1e-12, atol=1e-12)
+    col2, nx2, _ = a.raycast(pos, d, adept.NAV_LOOP)
+    assert np.array_equal(nx2, nx) and np.array_equal(col2, col)
+    a.close()
+    # full barrel: BVH == loop, bit for bit, on an eta-phi picture
+    g, _, tabs, scal = barrel_full
+    a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=1 << 10)
+    w, h = 96, 40
+    p, d = raycast.barrel_rays(w, h)
+    cb, nb, _ = a.raycast(p, d, adept.NAV_BVH)
+    cl, nl, _ = a.raycast(p, d, adept.NAV_LOOP)
+    assert np.array_equal(nb, nl) and np.array_equal(cb, cl)
+    inside = np.abs(-1.45 + (np.arange(h) + 0.5) * 2.9 / h) < 1.3
+    # 10 shells in and out, mother, at least one crystal, mother, world; >= 20 cm of PbWO4 on a line of sight of the
+    # barrel; the crystals point at the origin and cover 97.7 % of the row / column pitch, so about one pixel in
+    # twenty looks straight down a gap between them
+    assert (nb.reshape(h, w)[inside] >= 23).mean() > 0.9
+    assert (cb.reshape(h, w)[inside] > 8.28 * 20.0).mean() > 0.9
+    assert (nb.reshape(h, w)[inside] >= 21).all()      # every line of sight crosses the ten shells and enters the mother
+    out = tmp_path / "barrel.ppm"
+    raycast.write_ppm(str(out), cb, w, h)
+    data = out.read_bytes()
+    assert data.startswith(b"P6\n96 40\n255\n") and len(data) == len(b"P6\n96 40\n255\n") + 3 * w * h
+    a.close()
