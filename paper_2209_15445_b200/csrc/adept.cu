@@ -484,16 +484,8 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   {
     const bool bvh = cfg->navigator == ADEPT_NAV_BVH && !hb.empty();
-#ifdef ADEPT_GAMMA_GENERIC   // the generic move kernel (step_move<MODE_GAMMA>), kept for A/B measurements
-    ctx->k_move_gamma = bvh ? move_kernel<MODE_GAMMA, ADEPT_FIELD_NONE, true> : move_kernel<MODE_GAMMA, ADEPT_FIELD_NONE, false>;
-#else
     ctx->k_move_gamma = bvh ? gamma_move_kernel<true> : gamma_move_kernel<false>;
-#endif
-#ifdef ADEPT_CHARGED_GENERIC   // the generic move kernel (step_move<MODE_CHARGED>), kept for A/B measurements
-#define ADEPT_CHARGED_KERNEL(F, B) move_kernel<MODE_CHARGED, F, B>
-#else
 #define ADEPT_CHARGED_KERNEL(F, B) charged_move_kernel<F, B>
-#endif
     switch (f->kind) {
       case ADEPT_FIELD_NONE:
         ctx->k_move_charged = bvh ? ADEPT_CHARGED_KERNEL(ADEPT_FIELD_NONE, true) : ADEPT_CHARGED_KERNEL(ADEPT_FIELD_NONE, false); break;

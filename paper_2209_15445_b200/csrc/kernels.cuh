@@ -16,12 +16,6 @@ namespace adept {
 constexpr int kBlock = ADEPT_BLOCK;
 constexpr int kWarps = kBlock / 32;
 // minimum resident blocks per SM asked of the compiler (register caps chosen from measurement)
-#ifndef ADEPT_MINB_G
-#define ADEPT_MINB_G 4
-#endif
-#ifndef ADEPT_MINB_C
-#define ADEPT_MINB_C 3
-#endif
 #ifndef ADEPT_MINB_I
 #define ADEPT_MINB_I 6
 #endif
@@ -311,122 +305,6 @@ __device__ __forceinline__ void move_counts_flush(BlockTally& t, unsigned long l
     }
   }
   packed = 0;
-}
-
-// ------------------------------------------------------------------------------------------------
-// Move kernel: one step of every track of a species up to (not including) its discrete interaction.
-// grid.y = species of a charged launch.  Survivors that do not interact go to the next buffer of their
-// species; survivors that interact are staged, whole record, in the queue of their process, so the
-// interaction kernel reads them coalesced; the photons of an e+ annihilating at rest go to the next
-// gamma buffer.
-template <int MODE, int FIELD, bool BVH>
-__global__ void __launch_bounds__(kBlock, MODE == MODE_GAMMA ? ADEPT_MINB_G : ADEPT_MINB_C)
-move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot, int parity) {
-  const int species = MODE == MODE_GAMMA ? ADEPT_GAMMA : static_cast<int>(blockIdx.y);
-  const TrackSoA& cur = slot.buf[parity][species];
-  SlotCounters* cnt = slot.counters;
-  const uint32_t n = cnt->count[parity][species].v;
-
-  // destinations of this kernel: 0 = next buffer of the species, 1..3 = its staging queues, 4 = next
-  // buffer of the secondaries a move can create: photoelectrons (gamma kernel) or the photons of an
-  // annihilation at rest (charged kernel)
-  constexpr int ND = 5;
-  constexpr int kSecSpecies = MODE == MODE_GAMMA ? ADEPT_ELECTRON : ADEPT_GAMMA;
-  const int q0 = species == ADEPT_GAMMA ? 0 : (species == ADEPT_ELECTRON ? 3 : 5);
-  __shared__ BlockTally tally;
-  __shared__ BlockReserve<ND> br;
-  __shared__ TilePipe pipe;
-  tally_init(tally);
-  pipe_init(pipe);
-  double sum_dep = 0.0, sum_cut = 0.0;
-  unsigned chords = 0;
-  unsigned long long packed = 0;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const unsigned lt = (1u << lane) - 1u;
-
-  const uint32_t n_tiles = (n + kBlock - 1) / kBlock;
-  if (threadIdx.x == 0 && blockIdx.x < n_tiles) tile_issue(pipe.tile[0], cur, blockIdx.x, &pipe.bar[0]);
-  uint32_t k = 0;
-  for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++k) {
-    const int phase = k & 1;
-    // prefetch the block's next tile; its buffer was last read one iteration ago, before the barriers
-    // of that iteration's reservation
-    if (threadIdx.x == 0 && tile + gridDim.x < n_tiles) tile_issue(pipe.tile[phase ^ 1], cur, tile + gridDim.x, &pipe.bar[phase ^ 1]);
-    mbar_wait(&pipe.bar[phase], (k >> 1) & 1);
-    const uint32_t i = tile * kBlock + threadIdx.x;
-    Track in = tile_read(pipe.tile[phase], threadIdx.x, species);
-    const bool active = i < n && in.vol != kDeadVolume;
-    StepOut o;
-    Stream u;
-    int process, mat;
-    const int next = step_move<MODE, FIELD, BVH>(c, c.navigator, active, in, o, u, process, mat);
-
-    score(slot, in.vol, o.edep_dep + o.edep_cut, active);
-    if (active) {
-      sum_dep += o.edep_dep; sum_cut += o.edep_cut; chords += o.chords;
-      if (o.killed != 0.0) atomicAdd(&tally.ledger[3], o.killed);
-      if (next == NEXT_NONE && o.outcome == ADEPT_OUT_ESCAPED) {
-        atomicAdd(&tally.ledger[2], o.escaped);
-        o.post.step = in.step + 1;
-        record_leak(c, slot, o.post, species);
-      }
-    }
-    // per-thread outcome counters, one byte per field, folded into the block tally every 255 tiles
-    if (active) {
-      packed += 1ull << (8 * MC_STEPS);
-      if (next == NEXT_NONE) packed += 1ull << (8 * move_count_field(o.outcome));
-    }
-
-    // reservation: a lane appends at most one survivor (to one of four destinations) and the secondaries
-    // of a photoelectric absorption or an annihilation at rest
-    const bool live = active && o.alive;
-    const int dest = !live ? -1 : (next == NEXT_INTERACT ? 1 + stage_queue(process, species) - q0 : 0);
-    uint32_t pre = 0, pre_ph = 0;
-#pragma unroll
-    for (int d = 0; d < 4; ++d) {
-      const unsigned b = __ballot_sync(kFull, dest == d);
-      if (dest == d) pre = __popc(b & lt);
-      if (lane == 0) br.wtot[phase][warp][d] = __popc(b);
-    }
-    const uint32_t n_ph = active ? static_cast<uint32_t>(o.n_sec) : 0u;
-    const bool ph0 = n_ph && o.sec[0].species >= 0, ph1 = MODE != MODE_GAMMA && n_ph && o.sec[1].species >= 0;
-    {
-      const unsigned b0 = __ballot_sync(kFull, n_ph & 1u), b1 = MODE != MODE_GAMMA ? __ballot_sync(kFull, n_ph & 2u) : 0u;
-      pre_ph = __popc(b0 & lt) + 2 * __popc(b1 & lt);
-      const uint32_t tot = __popc(b0) + 2 * __popc(b1);
-      if (lane == 0) { br.wtot[phase][warp][4] = tot; if (tot) atomicAdd(&tally.secondaries[kSecSpecies], tot); }
-    }
-    block_reserve_commit<ND>(br, phase, [&](int d) -> uint32_t* {
-      if (d == 0) return &cnt->count[parity ^ 1][species].v;
-      if (d == 4) return &cnt->count[parity ^ 1][kSecSpecies].v;
-      return &cnt->n_stage[q0 + d - 1].v;
-    });
-    if (live) {
-      o.post.step = in.step + 1;
-      const uint32_t j = br.wbase[phase][warp][dest] + pre;
-      const bool staged = dest != 0;
-      const TrackSoA& dst = staged ? slot.stage[q0 + dest - 1] : slot.buf[parity ^ 1][species];
-      if (j < (staged ? c.stage_capacity : c.capacity)) store_track(dst, j, o.post);
-      else cnt->overflow.v = 1;
-    }
-    if (n_ph) {  // photoelectron / at-rest annihilation photons
-      const uint32_t j0 = br.wbase[phase][warp][4] + pre_ph;
-#pragma unroll
-      for (int kk = 0; kk < (MODE == MODE_GAMMA ? 1 : 2); ++kk) {
-        if (!(kk == 0 ? ph0 : ph1)) continue;
-        const uint32_t j = j0 + ((kk == 1 && ph0) ? 1u : 0u);
-        if (j < c.capacity) store_track(slot.buf[parity ^ 1][kSecSpecies], j, make_secondary(o, kk, in.event, u));
-        else cnt->overflow.v = 1;
-      }
-    }
-    if (k % 255u == 254u) move_counts_flush(tally, packed);
-  }
-  move_counts_flush(tally, packed);
-  {
-    const unsigned long long ch = __reduce_add_sync(kFull, chords);
-    if (lane == 0 && ch) atomicAdd(&tally.chords, ch);
-  }
-  tally_flush(tally, slot, species, sum_dep, sum_cut);
 }
 
 // End of one population step: the just-consumed buffers become the next step's output buffers.  Run by
