@@ -15,15 +15,20 @@
 
 namespace adept {
 
+// resident blocks per SM asked of the compiler: 6 (80 registers) without a field -- measured 1.3 % of a
+// config-2 pass over 5 -- and 5 (96 registers) with the chord loop, which spills already at 96
 #ifndef ADEPT_MINB_C2
-#define ADEPT_MINB_C2 5
+#define ADEPT_MINB_C2 6
+#endif
+#ifndef ADEPT_MINB_C2F
+#define ADEPT_MINB_C2F 5
 #endif
 
 // generic-proxy writes to the tile must be ordered before the TMA (async proxy) refill of the same buffer
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 template <int FIELD, bool BVH>
-__global__ void __launch_bounds__(kBlock, ADEPT_MINB_C2)
+__global__ void __launch_bounds__(kBlock, FIELD == ADEPT_FIELD_NONE ? ADEPT_MINB_C2 : ADEPT_MINB_C2F)
 charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot, int parity) {
   const int species = static_cast<int>(blockIdx.y);   // ADEPT_ELECTRON or ADEPT_POSITRON
   const bool positron = species == ADEPT_POSITRON;
