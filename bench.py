@@ -31,12 +31,12 @@ E_PRIMARY = 10000.0
 KERNELS = ("gamma_move_kernel", "charged_move_kernel", "interact_kernel")
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of each kernel at the peak
 # population of a config-2 pass, and the tracks that launch processed, from the `ncu --set full` capture
-# summarised in profiles/r1e_summary.md.  Reported as roofline.traffic (bytes of that one launch) beside the
+# summarised in profiles/r1f_summary.md.  Reported as roofline.traffic (bytes of that one launch) beside the
 # algorithmic bytes of the same launch (tracks x 160 B).
 NCU_TRAFFIC = {   # bytes of DRAM traffic, tracks processed, kernel time [us] of the captured launch (population step 64)
-    "gamma_move_kernel": {"dram_bytes": 517.7e6, "tracks": 3986758, "time_us": 211.0},
-    "charged_move_kernel": {"dram_bytes": 202.3e6, "tracks": 1698340, "time_us": 184.2},
-    "interact_kernel": {"dram_bytes": 188.7e6, "tracks": None, "time_us": 104.5},
+    "gamma_move_kernel": {"dram_bytes": 516.2e6, "tracks": 3986758, "time_us": 195.0},
+    "charged_move_kernel": {"dram_bytes": 203.8e6, "tracks": 1698340, "time_us": 167.6},
+    "interact_kernel": {"dram_bytes": 188.7e6, "tracks": None, "time_us": 102.6},
 }
 
 
@@ -342,7 +342,7 @@ def run_ours(args):
             "roofline": {"bound": "hbm", "kernel": KERNELS[dom],
                          "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": NCU_TRAFFIC[KERNELS[dom]]["dram_bytes"],
-                         "traffic_launch": dict(NCU_TRAFFIC[KERNELS[dom]], source="ncu --set full, profiles/r1e_summary.md",
+                         "traffic_launch": dict(NCU_TRAFFIC[KERNELS[dom]], source="ncu --set full, profiles/r1f_summary.md",
                                                 algorithmic_bytes=(NCU_TRAFFIC[KERNELS[dom]]["tracks"] or 0) * BYTES_PER_STEP),
                          "peak_source": peak_src, "launches": int(kn[dom]), "avg_launch_ms": float(kms[dom] / max(kn[dom], 1)),
                          "algorithmic_bytes_per_step": BYTES_PER_STEP, "per_kernel": per_kernel,
