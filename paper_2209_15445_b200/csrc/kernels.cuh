@@ -17,7 +17,7 @@ constexpr int kBlock = ADEPT_BLOCK;
 constexpr int kWarps = kBlock / 32;
 // minimum resident blocks per SM asked of the compiler (register caps chosen from measurement)
 #ifndef ADEPT_MINB_I
-#define ADEPT_MINB_I 6
+#define ADEPT_MINB_I 4   // 128 registers: measured 9.75 ms per config-2 pass against 9.9 (5 blocks) and 10.1 (6, spills)
 #endif
 
 __device__ __forceinline__ Track load_track(const TrackSoA& b, uint32_t i, int species) {
