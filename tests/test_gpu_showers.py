@@ -335,3 +335,47 @@ def test_hybrid_buffer_threshold_and_flush(ob, calo):
         buf.add(0, 0, 5, prim["pos"][0], prim["dir"][0], 1.0)
     buf.close()
     a.close()
+
+
+def test_measurement_modes_do_not_change_the_showers(ob, calo):
+    """The measurement switches of the C ABI -- species kernels on one stream or two, CUDA events around every
+    launch, the iteration trace -- change the schedule, never the result."""
+    import torch
+    from paper_2209_15445_b200 import adept
+    from paper_2209_15445_b200.inputs import field, primaries
+    g, _, tabs, scal = calo
+    prim = primaries.beam(40, 400.0, spread=1.0)
+    prim["species"][1::2] = 2
+    ref = None
+    for conc, timed in ((1, 0), (0, 0), (1, 1)):
+        a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=1 << 16, concurrent_species=conc, time_kernels=timed)
+        if not timed:
+            with pytest.raises(adept.AdeptError):
+                a.set_kernel_timing(True)           # context was not created with time_kernels
+        a.enqueue(prim)
+        a.iteration_trace()
+        a.transport(0, torch.cuda.current_stream())
+        e, led = a.read_scoring(0)
+        st = a.stats(0)
+        t, pop = a.iteration_trace()
+        assert len(t) == st.iterations and list(pop[0]) == [20, 0, 20]
+        assert (np.diff(t.astype(np.int64)) > 0).all() and pop.sum(axis=1).max() == st.peak_population
+        assert len(a.iteration_trace()[0]) == 0     # reading clears
+        if timed:
+            ms, n = a.kernel_times(0)
+            assert (n == st.iterations).all() or (n >= st.iterations).all()
+            assert (ms > 0).all()
+            a.set_kernel_timing(False)
+            a.enqueue(prim)
+            a.transport(0, torch.cuda.current_stream())
+            e2, _ = a.read_scoring(0)
+            assert (a.kernel_times(0)[1] == 0).all()
+            np.testing.assert_allclose(e2, e, rtol=1e-9, atol=1e-9)
+        key = (list(st.steps), list(st.outcomes), list(st.secondaries), st.iterations)
+        if ref is None:
+            ref = (key, e, led.total())
+        else:
+            assert key == ref[0]
+            np.testing.assert_allclose(e, ref[1], rtol=1e-9, atol=1e-9)
+            assert led.total() == pytest.approx(ref[2], rel=1e-12)
+        a.close()
