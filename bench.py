@@ -46,8 +46,9 @@ def parse():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4],
-                    help="BASELINE.json config: 2 (default, the bench line), 3 (same + 1 T field), 4 (barrel, BVH, field map; extra)")
+    ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4, 5],
+                    help="BASELINE.json config: 2 (default, the bench line), 3 (same + 1 T field), 4 (barrel, BVH, field map; extra), "
+                         "5 (16 barrel events on 16 streams; extra, 1 GPU)")
     ap.add_argument("--events", type=int, default=0, help="events per batch (0 = 10000 for configs 2-3, 100 x 50 primaries for config 4)")
     ap.add_argument("--field", type=float, default=0.0, help="uniform Bz in tesla for configs 2-3 (config 3 sets 1.0)")
     ap.add_argument("--max-steps", type=int, default=0, help="looper cut S4 (0 = 1e6 for configs 2-3, 4096 for config 4)")
@@ -63,8 +64,8 @@ def parse():
     a = ap.parse_args()
     if a.config == 3 and a.field == 0.0:
         a.field = 1.0
-    a.events = a.events or (100 if a.config == 4 else 10000)
-    a.max_steps = a.max_steps or (4096 if a.config == 4 else 1000000)
+    a.events = a.events or (100 if a.config == 4 else (16 if a.config == 5 else 10000))
+    a.max_steps = a.max_steps or (4096 if a.config in (4, 5) else 1000000)
     return a
 
 
@@ -366,10 +367,84 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_config5(args):
+    """BASELINE.json:configs[4]: `--events` (16) events of 200 primaries (e-, e+, gamma 2:1:2, 0.1-50 GeV) in the barrel
+    of config 4, one event slot and one CUDA stream per event, per-event hits (61 212 doubles) copied back per event.
+    Times adept_transport_many (all slots interleaved) against the same slots transported one after the other."""
+    import torch
+    from paper_2209_15445_b200 import adept
+    from paper_2209_15445_b200.inputs import field, geometry, materials, primaries
+    dev = torch.device("cuda:0")
+    torch.cuda.set_device(dev)
+    g = geometry.barrel()
+    _, tabs, scal = materials.build_material_set(g.material_names)
+    n_ev = args.events
+    prim = primaries.barrel_events(n_ev, 200, 100.0, 50000.0, mode="cfg5", seed=1)
+    cap = args.capacity or (1 << 20)
+    a = adept.Adept(g, tabs, scal, field.solenoid_map(), device=str(dev), track_capacity=cap, stage_capacity=cap // 4,
+                    n_event_slots=n_ev, sync_interval=args.sync_interval, max_steps=args.max_steps)
+    streams = [torch.cuda.Stream(device=dev) for _ in range(n_ev)]
+    hits = np.zeros((n_ev, g.n_volumes))
+    sel = [prim["event"] == e for e in range(n_ev)]
+
+    def one_pass(concurrent):
+        torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        for e in range(n_ev):
+            a.enqueue_primaries(e, e, prim["species"][sel[e]], prim["pos"][sel[e]], prim["dir"][sel[e]], prim["ekin"][sel[e]])
+        t1 = time.perf_counter()
+        if concurrent:
+            a.transport_many(list(range(n_ev)), streams)
+        else:
+            for e in range(n_ev):
+                a.transport(e, streams[e])
+        torch.cuda.synchronize(dev)
+        t2 = time.perf_counter()
+        leds = [a.read_scoring(e, streams[e], out=hits[e])[1] for e in range(n_ev)]
+        torch.cuda.synchronize(dev)
+        return t2 - t1, time.perf_counter() - t0, leds
+
+    def steps_now():
+        return sum(sum(a.stats(e).steps) for e in range(n_ev))
+
+    res = {}
+    clocks = ClockSampler(0)
+    clocks.start()
+    for name, conc in (("concurrent", True), ("sequential", False)):
+        for _ in range(max(args.warmup, 1)):
+            one_pass(conc)
+        s0 = steps_now()
+        tt, te, leds = zip(*[one_pass(conc) for _ in range(args.steps)])
+        res[name] = {"transport_s": sum(tt), "e2e_s": sum(te), "steps": steps_now() - s0,
+                     "ledger_closes": max(abs(l.total() - l.primary) / l.primary for l in leds[-1])}
+    clk = clocks.stop()
+    c, q = res["concurrent"], res["sequential"]
+    launches = sum(a.stats(e).launches for e in range(n_ev))
+    line = {"metric": "track_steps_per_s", "value": c["steps"] / c["transport_s"], "unit": "steps/s", "n_gpus": 1,
+            "steps": args.steps, "warmup": max(args.warmup, 1), "ms_per_step": 1e3 * c["transport_s"] / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"config5: {n_ev} events x 200 primaries (e-, e+, gamma 2:1:2, 0.1-50 GeV) in the barrel of config 4, "
+                                   f"one slot and one CUDA stream per event, looper cut max_steps={args.max_steps}",
+                       "track_capacity_per_slot": cap, "sync_interval": args.sync_interval,
+                       "l2": "track state of 16 slots (17 GB workspace) exceeds L2"},
+            "events_per_s": n_ev * args.steps / c["transport_s"],
+            "sequential": {"value": q["steps"] / q["transport_s"], "ms_per_step": 1e3 * q["transport_s"] / args.steps,
+                           "events_per_s": n_ev * args.steps / q["transport_s"]},
+            "speedup_concurrent_over_sequential": q["transport_s"] / c["transport_s"],
+            "e2e": {"value": c["steps"] / c["e2e_s"], "unit": "steps/s", "events_per_s": n_ev * args.steps / c["e2e_s"],
+                    "h2d_bytes_per_step": int(len(prim["ekin"]) * 80), "d2h_bytes_per_step": int(hits.nbytes + 40 * n_ev)},
+            "gpu_launches": int(launches), "clocks": clk, "ledger_closes": c["ledger_closes"],
+            "roofline": None, "cpu_baseline": None}
+    print(json.dumps(line))
+    a.close()
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         run_reference(args)
+    elif args.config == 5:
+        run_config5(args)
     else:
         run_ours(args)
 

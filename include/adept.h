@@ -119,6 +119,9 @@ typedef struct {
                               when inject_chunk > 0                                                          */
   int32_t concurrent_species; /* 1 (default): gamma and charged move kernels on two streams;
                               0: all kernels of a slot on the caller's stream, one after the other          */
+  int32_t use_graphs;      /* 1 (default): a host round of sync_interval population steps is replayed as one CUDA
+                              graph per slot (needs an even sync_interval; off while per-launch timing is on or
+                              primaries wait for injection); 0: every kernel is launched individually           */
 } adept_config;
 
 typedef struct {

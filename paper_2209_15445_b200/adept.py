@@ -45,7 +45,7 @@ class CConfig(C.Structure):
                 ("chord_budget", C.c_int32), ("seed", C.c_uint32), ("max_steps", C.c_uint32), ("navigator", C.c_int32),
                 ("n_event_slots", C.c_int32), ("sync_interval", C.c_int32), ("track_capacity", C.c_uint64),
                 ("leak_capacity", C.c_uint64), ("stage_capacity", C.c_uint64), ("time_kernels", C.c_int32),
-                ("inject_chunk", C.c_uint64), ("pending_capacity", C.c_uint64), ("concurrent_species", C.c_int32)]
+                ("inject_chunk", C.c_uint64), ("pending_capacity", C.c_uint64), ("concurrent_species", C.c_int32), ("use_graphs", C.c_int32)]
 
 
 class CLedger(C.Structure):

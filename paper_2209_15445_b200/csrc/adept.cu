@@ -212,6 +212,10 @@ struct SlotHost {
   unsigned long long launches = 0;
   bool live = false;
   size_t n_pending = 0, n_injected = 0;   // staggered injection: primaries in the pending store / already injected
+  // CUDA graph of one host round (sync_interval population steps), captured once on `cap` and replayed
+  cudaStream_t cap = nullptr;
+  cudaGraphExec_t gexec = nullptr;
+  bool graph_failed = false;
   // optional per-launch timing (config.time_kernels)
   std::vector<cudaEvent_t> tev;      // [sync_interval][kTimed kernels][start, stop]
   int tev_used = 0;
@@ -244,6 +248,7 @@ extern "C" void adept_default_config(adept_config* c) {
   c->navigator = ADEPT_NAV_BVH; c->n_event_slots = 1; c->sync_interval = 8;
   c->track_capacity = 1u << 20; c->leak_capacity = 1u << 16; c->stage_capacity = 0;
   c->concurrent_species = 1;
+  c->use_graphs = 1;
 }
 
 namespace {
@@ -532,6 +537,8 @@ extern "C" int adept_set_kernel_timing(adept_ctx* ctx, int on) {
 extern "C" int adept_shutdown(adept_ctx* ctx) {
   if (!ctx) return fail(ADEPT_EINVAL, "null context");
   for (SlotHost& sh : ctx->slots) {
+    if (sh.gexec) cudaGraphExecDestroy(sh.gexec);
+    if (sh.cap) cudaStreamDestroy(sh.cap);
     if (sh.helper) cudaStreamDestroy(sh.helper);
     if (sh.fork) cudaEventDestroy(sh.fork);
     if (sh.join) cudaEventDestroy(sh.join);
@@ -635,6 +642,29 @@ int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity) 
   return ADEPT_OK;
 }
 
+// One host round -- sync_interval population steps, starting at parity 0 -- as a CUDA graph: the slot's
+// kernels, forks and joins are captured once on a library-owned stream and replayed with one launch per
+// round.  A small event (config 5: 200 primaries, thousands of nearly empty population steps on each of 16
+// streams) is otherwise bound by the host issuing ~10 API calls per step.  Needs an even sync_interval (every
+// round then starts at parity 0), no per-launch timing and no pending injection; returns false to fall back.
+bool round_graph(adept_ctx* ctx, SlotHost& sh) {
+  if (sh.gexec) return true;
+  if (sh.graph_failed || !ctx->cfg.use_graphs || (ctx->cfg.sync_interval & 1)) return false;
+  if (!sh.cap && cudaStreamCreateWithFlags(&sh.cap, cudaStreamNonBlocking) != cudaSuccess) { sh.graph_failed = true; return false; }
+  const unsigned long long launches = sh.launches;
+  cudaGraph_t graph = nullptr;
+  bool ok = cudaStreamBeginCapture(sh.cap, cudaStreamCaptureModeRelaxed) == cudaSuccess;
+  if (ok) {
+    for (int it = 0; it < ctx->cfg.sync_interval && ok; ++it) ok = launch_iteration(ctx, sh, sh.cap, it & 1) == ADEPT_OK;
+    ok = (cudaStreamEndCapture(sh.cap, &graph) == cudaSuccess) && ok && graph;
+  }
+  if (ok) ok = cudaGraphInstantiate(&sh.gexec, graph, 0) == cudaSuccess;
+  if (graph) cudaGraphDestroy(graph);
+  sh.launches = launches;
+  if (!ok) { cudaGetLastError(); sh.gexec = nullptr; sh.graph_failed = true; }
+  return ok;
+}
+
 }  // namespace
 
 extern "C" int adept_transport_many(adept_ctx* ctx, int n_slots, const int* slots, void* const* streams) {
@@ -647,10 +677,19 @@ extern "C" int adept_transport_many(adept_ctx* ctx, int n_slots, const int* slot
   std::vector<int> parity(n_slots, 0);
   int n_live = n_slots, rc_final = ADEPT_OK;
   while (n_live > 0) {
+    // slots whose round is a graph: one launch each
+    std::vector<char> graphed(n_slots, 0);
+    for (int k = 0; k < n_slots; ++k) {
+      SlotHost& sh = ctx->slots[slots[k]];
+      if (!sh.live || parity[k] != 0 || ctx->timing_on || sh.n_injected < sh.n_pending || !round_graph(ctx, sh)) continue;
+      CUDA_TRY(cudaGraphLaunch(sh.gexec, static_cast<cudaStream_t>(streams[k])));
+      sh.launches += 3ull * ctx->cfg.sync_interval;
+      graphed[k] = 1;
+    }
     for (int it = 0; it < ctx->cfg.sync_interval; ++it)
       for (int k = 0; k < n_slots; ++k) {
         SlotHost& sh = ctx->slots[slots[k]];
-        if (!sh.live) continue;
+        if (!sh.live || graphed[k]) continue;
         const int rc = launch_iteration(ctx, sh, static_cast<cudaStream_t>(streams[k]), parity[k]);
         if (rc != ADEPT_OK) return rc;
         parity[k] ^= 1;
