@@ -54,7 +54,7 @@ def parse():
     ap.add_argument("--max-steps", type=int, default=0, help="looper cut S4 (0 = 1e6 for configs 2-3, 4096 for config 4)")
     ap.add_argument("--inject-chunk", type=int, default=0, help="staggered injection: primaries per population step (0 = all at once)")
     ap.add_argument("--capacity", type=int, default=0, help="track capacity per species (0 = auto)")
-    ap.add_argument("--sync-interval", type=int, default=8)
+    ap.add_argument("--sync-interval", type=int, default=16)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-kernel-timing", action="store_true",
                     help="experiments only: no per-kernel CUDA events (the roofline object is then empty)")

@@ -104,7 +104,7 @@ typedef struct {
   uint32_t max_steps;      /* a track is killed after this many steps, 1e6           */
   int32_t navigator;       /* ADEPT_NAV_LOOP | ADEPT_NAV_BVH                                        */
   int32_t n_event_slots;   /* independent transport contexts (config 5)                */
-  int32_t sync_interval;   /* population-step iterations launched between host checks               */
+  int32_t sync_interval;   /* population-step iterations launched between host checks, default 16    */
   uint64_t track_capacity; /* per slot, per species: entries of each of the two track buffers       */
   uint64_t leak_capacity;  /* per slot: tracks that left the world kept for adept_read_leaked       */
   uint64_t stage_capacity; /* per slot, per interaction queue: tracks staged for their discrete

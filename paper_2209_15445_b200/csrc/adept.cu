@@ -245,7 +245,7 @@ extern "C" void adept_default_config(adept_config* c) {
   std::memset(c, 0, sizeof(*c));
   c->delta_chord = 1e-3; c->eps_push = 1e-7; c->alpha_R = 0.2; c->rho_R = 0.1;
   c->chord_budget = 16; c->seed = 1; c->max_steps = 1000000;
-  c->navigator = ADEPT_NAV_BVH; c->n_event_slots = 1; c->sync_interval = 8;
+  c->navigator = ADEPT_NAV_BVH; c->n_event_slots = 1; c->sync_interval = 16;
   c->track_capacity = 1u << 20; c->leak_capacity = 1u << 16; c->stage_capacity = 0;
   c->concurrent_species = 1;
   c->use_graphs = 1;
