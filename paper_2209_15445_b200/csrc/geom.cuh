@@ -145,7 +145,7 @@ __device__ __forceinline__ bool inside_volume(const DevCtx& c, int vol, double x
   return inside_solid(v.solid, v.dims, l);
 }
 
-__device__ __noinline__ double entry_distance(const DevCtx& c, int vol, double px, double py, double pz,
+__device__ __forceinline__ double entry_distance(const DevCtx& c, int vol, double px, double py, double pz,
                                                  double dx, double dy, double dz) {
   const DevVolume& v = volume(c, vol);
   double lp[3], ld[3];
