@@ -192,7 +192,7 @@ __device__ __forceinline__ bool point_box(const double* __restrict__ box, int st
 // state is a short stack of one 32-bit child mask per level, shared by the warp.
 // `hit` (warp-uniform, out): touchable id of the daughter that gave the returned minimum, -1 if none did
 // or two daughters tie.
-__device__ __noinline__ double bvh_ray(const DevCtx& c, const DevBvh& b, double px, double py, double pz, double dx, double dy,
+__device__ __forceinline__ double bvh_ray(const DevCtx& c, const DevBvh& b, double px, double py, double pz, double dx, double dy,
                           double dz, double best, int& hit) {
   hit = -1;
   const int lane = threadIdx.x & 31;
@@ -241,7 +241,7 @@ __device__ __noinline__ double bvh_ray(const DevCtx& c, const DevBvh& b, double 
 }
 
 // All arguments warp-uniform.  Lowest touchable id among the daughters containing the point, or -1.
-__device__ __noinline__ int bvh_point(const DevCtx& c, const DevBvh& b, double px, double py, double pz) {
+__device__ __forceinline__ int bvh_point(const DevCtx& c, const DevBvh& b, double px, double py, double pz) {
   const int lane = threadIdx.x & 31;
   const int top = b.n_levels - 1;
   unsigned mask[kBvhMaxLevels];
@@ -285,9 +285,9 @@ __device__ __noinline__ int bvh_point(const DevCtx& c, const DevBvh& b, double p
 // own box through one face and no daughter is entered first, the face index 2 * axis + (direction > 0) in
 // the volume's frame -- the key of the hint table; when it is the entry into daughter d, -2 - d; -1 when
 // neither is known (the cap s_max, a tube, a tie).
-// The BVH instantiation is a call (its cooperative code is large and the call bounds what is live across
-// it); the loop-navigator instantiation is inlined into the step kernels (3.7 % of a config-2 pass: no
-// argument moves, and the compiler schedules the box test into the surrounding phase).
+// Inlined into the step kernels (3.7 % of a config-2 pass, 5 % of a config-4 pass, 20 % of the ray-cast over
+// calls: no argument moves, and the compiler schedules the box test into the surrounding phase), and so are
+// the cooperative traversals bvh_ray / bvh_point (another 5 % of a config-4 pass).
 template <bool BVH>
 __device__ __forceinline__ double nav_distance_body(const DevCtx& c, int nav, bool active, double px, double py, double pz, double dx,
                                double dy, double dz, uint32_t vol, double s_max, int& face) {
@@ -329,16 +329,10 @@ __device__ __forceinline__ double nav_distance_body(const DevCtx& c, int nav, bo
   }
   return s;
 }
-template <bool BVH>
-__device__ __noinline__ double nav_distance_call(const DevCtx& c, int nav, bool active, double px, double py, double pz, double dx,
-                                                 double dy, double dz, uint32_t vol, double s_max, int& face) {
-  return nav_distance_body<BVH>(c, nav, active, px, py, pz, dx, dy, dz, vol, s_max, face);
-}
 template <bool BVH = true>
 __device__ __forceinline__ double nav_distance(const DevCtx& c, int nav, bool active, double px, double py, double pz, double dx,
                                                double dy, double dz, uint32_t vol, double s_max, int& face) {
-  if constexpr (BVH) return nav_distance_call<true>(c, nav, active, px, py, pz, dx, dy, dz, vol, s_max, face);
-  else return nav_distance_body<false>(c, nav, active, px, py, pz, dx, dy, dz, vol, s_max, face);
+  return nav_distance_body<BVH>(c, nav, active, px, py, pz, dx, dy, dz, vol, s_max, face);
 }
 template <bool BVH = true>
 __device__ __forceinline__ double nav_distance(const DevCtx& c, int nav, bool active, double px, double py, double pz, double dx,
@@ -490,16 +484,10 @@ __device__ __forceinline__ int nav_relocate_body(const DevCtx& c, int nav, bool 
   }
   return cur;
 }
-template <bool BVH>
-__device__ __noinline__ int nav_relocate_call(const DevCtx& c, int nav, bool active, uint32_t vol_old, double qx, double qy, double qz,
-                                              int face) {
-  return nav_relocate_body<BVH>(c, nav, active, vol_old, qx, qy, qz, face);
-}
 template <bool BVH = true>
 __device__ __forceinline__ int nav_relocate(const DevCtx& c, int nav, bool active, uint32_t vol_old, double qx, double qy, double qz,
                                             int face = -1) {
-  if constexpr (BVH) return nav_relocate_call<true>(c, nav, active, vol_old, qx, qy, qz, face);
-  else return nav_relocate_body<false>(c, nav, active, vol_old, qx, qy, qz, face);
+  return nav_relocate_body<BVH>(c, nav, active, vol_old, qx, qy, qz, face);
 }
 
 }  // namespace adept
