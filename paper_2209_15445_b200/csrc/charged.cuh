@@ -16,12 +16,13 @@
 namespace adept {
 
 // resident blocks per SM asked of the compiler: 6 (80 registers) without a field -- measured 1.3 % of a
-// config-2 pass over 5 -- and 5 (96 registers) with the chord loop, which spills already at 96
+// config-2 pass over 5 -- and 4 (128 registers) with the chord loop, which spills 700 B at 96 registers
+// (config 4: 3.92 -> 3.72 s per pass over 5 blocks; 3 blocks, no spills at all, are no faster)
 #ifndef ADEPT_MINB_C2
 #define ADEPT_MINB_C2 6
 #endif
 #ifndef ADEPT_MINB_C2F
-#define ADEPT_MINB_C2F 5
+#define ADEPT_MINB_C2F 4
 #endif
 
 // generic-proxy writes to the tile must be ordered before the TMA (async proxy) refill of the same buffer

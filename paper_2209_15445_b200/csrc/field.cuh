@@ -93,7 +93,7 @@ __device__ __forceinline__ void rk4(const DevCtx& c, int charge, double pmom, do
 // pushdir = chord direction), 2 truncated (chord budget).  Warp-convergent.
 // FIELD >= 0 fixes the field kind at compile time (no helix / RK4 code where it cannot run); -1 = runtime.
 template <int FIELD = -1, bool BVH = true>
-__device__ int propagate(const DevCtx& c, int nav, bool active, int charge, double ekin, double pos[3], double dir[3],
+__device__ __forceinline__ int propagate(const DevCtx& c, int nav, bool active, int charge, double ekin, double pos[3], double dir[3],
                          uint32_t vol, double s_phys, double& s_out, int& chords_out, double pushdir[3], int& face_out) {
   const int field_kind = FIELD >= 0 ? FIELD : c.field_kind;
   const double pmom = sqrt(ekin * (ekin + 2.0 * kMe));
