@@ -4,9 +4,9 @@
 // implementation behind the frozen-step hook.  What differs is where the track lives: the step kernels
 // are bound by instruction latency at 4 resident warps per scheduler (profiles/r1b_summary.md), and the
 // resident warps are set by registers.  Here a lane's track stays in its slot of the shared-memory tile
-// the TMA pipeline filled and every phase reads only the fields it needs, at the point of use; the two
-// navigator calls (not inlined) are the fences between phases, so nothing but the position, the step
-// length and three flags is live across them.  The discrete process is chosen (U1) before the
+// the TMA pipeline filled and every phase reads only the fields it needs, at the point of use, so nothing
+// but the position, the step length and three flags is live across the two navigator phases (which are
+// inlined: as calls they cost 4 % of a config-2 pass).  The discrete process is chosen (U1) before the
 // propagation -- it depends on nothing the propagation computes -- so neither the cross sections nor
 // the Philox state survive phase A.
 #pragma once
