@@ -4,7 +4,12 @@
  * sagitta stays below delta_chord, with a chord budget per step (F4).
  * Uniform field: exact helix endpoints.  Field map: one classical RK4 step per chord.
  * Pinned by tests/test_oracle_field.py: helix vs the analytic circle and the return to the start
- * after one turn, RK4 in a uniform map vs the helix with the h^5 error law, |d| = 1.
+ * after one turn, RK4 in a uniform map vs the helix with the h^5 error law, |d| = 1; the chord loop of
+ * the ORC_FIELD_MAP_RZ branch by its chord count (sagitta limit, and the F2' clamp as the number
+ * ceil(s / (0.5 p / (2.998 |B|)))), its end point vs the exact helix within the RK4 bound, a boundary
+ * hit (point within delta_chord of the analytic circle, unit interpolated tangent within (h/R)^2 of
+ * the exact one, push direction = unit chord) and an adaptive DOP853 integration of F1 in the real,
+ * non-uniform solenoid map; tests/test_oracle_stepper.py closes the per-event ledger through it.
  */
 #include <algorithm>
 

@@ -44,6 +44,30 @@ def test_energy_ledger_closes_per_event(ob, calo, fld):
         assert led.killed == 0.0 and led.escaped < 0.2 * carried
 
 
+def test_energy_ledger_closes_per_event_in_the_field_map(ob, barrel_patch):
+    """Same invariant through the ORC_FIELD_MAP_RZ branch of the chord loop (RK4, F2' clamp, boundary hits with
+    interpolated tangents): tubes, rotated crystals and the solenoid map of configs 4-5, one event at a time."""
+    g, _, tabs, scal = barrel_patch
+    o = ob.Oracle(g, tabs, scal, field.solenoid_map())
+    prim = primaries.barrel_events(5, 5, 500.0, 3000.0, mode="cfg5")     # e-, e-, e+, gamma, gamma per event
+    d = np.array([np.cos(0.1), np.sin(0.1), 0.01])
+    prim["dir"][:] = d / np.linalg.norm(d)                      # into the 12 x 12 crystal patch
+    tr = o.make_tracks(prim)
+    chords, in_crystals, photons = 0, 0.0, 0.0
+    for e in range(5):
+        sel = tr[tr["event"] == e]
+        edep, led, st = o.run(sel)
+        carried = float(sum(t["ekin"] + (2 * M if t["species"] == 1 else 0.0) for t in sel))
+        assert led.primary == pytest.approx(carried, rel=1e-15)
+        assert abs(led.total() - carried) <= 1e-9 * carried
+        assert edep.sum() == pytest.approx(led.deposited + led.below_cut, rel=1e-12)
+        in_crystals += edep[12:].sum()
+        photons += float(sel["ekin"][sel["species"] == 2].sum())
+        chords += st.chords
+    # the photons fly straight into the crystals and shower there; the e+- spiral through the tracker shells
+    assert in_crystals > 0.5 * photons and chords > 1000
+
+
 def test_unscattered_photon_fraction(ob, calo):
     """G pins: fraction of photons crossing the first 5 layers without interacting = exp(-sum Sigma t)."""
     g, _, tabs, scal = calo
