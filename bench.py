@@ -55,6 +55,8 @@ def parse():
     ap.add_argument("--inject-chunk", type=int, default=0, help="staggered injection: primaries per population step (0 = all at once)")
     ap.add_argument("--capacity", type=int, default=0, help="track capacity per species (0 = auto)")
     ap.add_argument("--sync-interval", type=int, default=16)
+    ap.add_argument("--steps-per-launch", type=int, default=0,
+                    help="adept_config.steps_per_launch: 0 = chosen per launch from the population (default), n = at most n")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-kernel-timing", action="store_true",
                     help="experiments only: no per-kernel CUDA events (the roofline object is then empty)")
@@ -233,7 +235,7 @@ def run_ours(args):
     a = adept.Adept(g, tabs, scal, fld, device=str(dev), track_capacity=cap, sync_interval=args.sync_interval,
                     stage_capacity=max(1 << 16, cap // 4) if args.config == 4 else 0, max_steps=args.max_steps,
                     inject_chunk=args.inject_chunk, pending_capacity=len(prim["ekin"]) if args.inject_chunk else 0,
-                    time_kernels=0 if args.no_kernel_timing else 1)
+                    time_kernels=0 if args.no_kernel_timing else 1, steps_per_launch=args.steps_per_launch)
     if not args.no_kernel_timing:
         a.set_kernel_timing(False)       # the timed passes run without per-launch events
     stream = torch.cuda.Stream(device=dev)
@@ -332,6 +334,7 @@ def run_ours(args):
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(args), "inject_chunk": args.inject_chunk,
                        "events_per_step_per_gpu": args.events, "track_capacity": cap, "sync_interval": args.sync_interval,
+                       "steps_per_launch": args.steps_per_launch,
                        "l2": "256 MB buffer written between passes (L2 flush); peak live track state also exceeds L2",
                        "parallelism": f"events sharded over {world} GPU(s), no data-path collective"},
             "showers_per_s": world * args.events * args.steps / t_dev,
@@ -382,7 +385,8 @@ def run_config5(args):
     prim = primaries.barrel_events(n_ev, 200, 100.0, 50000.0, mode="cfg5", seed=1)
     cap = args.capacity or (1 << 20)
     a = adept.Adept(g, tabs, scal, field.solenoid_map(), device=str(dev), track_capacity=cap, stage_capacity=cap // 4,
-                    n_event_slots=n_ev, sync_interval=args.sync_interval, max_steps=args.max_steps)
+                    n_event_slots=n_ev, sync_interval=args.sync_interval, max_steps=args.max_steps,
+                    steps_per_launch=args.steps_per_launch)
     streams = [torch.cuda.Stream(device=dev) for _ in range(n_ev)]
     hits = np.zeros((n_ev, g.n_volumes))
     sel = [prim["event"] == e for e in range(n_ev)]

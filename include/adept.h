@@ -30,7 +30,8 @@ enum {
   ADEPT_OK = 0,
   ADEPT_EINVAL = -1,    /* bad argument (null pointer, index out of range, malformed geometry)      */
   ADEPT_ENOMEM = -2,    /* workspace too small / host allocation failed                            */
-  ADEPT_EOVERFLOW = -3, /* a track queue of the slot overflowed; the slot's results are invalid    */
+  ADEPT_EOVERFLOW = -3, /* a track queue of the slot overflowed: the slot's results are invalid and
+                           the slot has been reset (empty, scoring zeroed), ready for reuse        */
   ADEPT_ECUDA = -4,     /* a CUDA runtime call failed                                              */
   ADEPT_ESTATE = -5     /* call not valid in this state (e.g. slot still holds live tracks)        */
 };
@@ -119,6 +120,11 @@ typedef struct {
                               when inject_chunk > 0                                                          */
   int32_t concurrent_species; /* 1 (default): gamma and charged move kernels on two streams;
                               0: all kernels of a slot on the caller's stream, one after the other          */
+  int32_t steps_per_launch; /* steps a lane may take of its own track inside one move-kernel launch while the outcome
+                              keeps the track in its species buffer (boundary, continuous-loss limit, chord budget):
+                              0 (default) = chosen per launch from the population (1 for a full GPU, more for the
+                              tails), n > 0 = at most n.  Random numbers are keyed by (event, track, step), so the
+                              showers are identical whatever the value                                          */
   int32_t use_graphs;      /* 1 (default): a host round of sync_interval population steps is replayed as one CUDA
                               graph per slot (needs an even sync_interval; off while per-launch timing is on or
                               primaries wait for injection); 0: every kernel is launched individually           */
@@ -190,11 +196,18 @@ int adept_enqueue_batch(adept_ctx*, int event_slot, int n, const uint32_t* event
                         const int8_t* species, const double* pos3, const double* dir3, const double* ekin);
 
 /* Steps the slot's whole population until its queues are empty.  Kernels run on
- * cuda_stream (plus library-owned helper streams ordered after it); returns when the slot is empty. */
+ * cuda_stream (plus library-owned helper streams ordered after it); returns when the slot is empty.
+ * ADEPT_EOVERFLOW: a queue of the slot was too small (track_capacity / stage_capacity); the pass is
+ * abandoned and the slot reset as by adept_reset_slot, so the caller may enqueue a smaller batch. */
 int adept_transport(adept_ctx*, int event_slot, void* cuda_stream);
 
-/* Transports several slots concurrently, slot i on streams[i] (config 5). */
+/* Transports several slots concurrently, slot i on streams[i] (config 5).  A slot listed
+ * twice, or one already in transport, is ADEPT_EINVAL.  On any error no listed slot stays marked live. */
 int adept_transport_many(adept_ctx*, int n_slots, const int* event_slots, void* const* cuda_streams);
+
+/* Empties a slot: drops its tracks, pending primaries and leaked tracks and zeroes its scoring arrays,
+ * ledger and iteration trace (the cumulative counters of adept_get_stats stay).  Synchronous. */
+int adept_reset_slot(adept_ctx*, int event_slot);
 
 /* Copies the slot's per-volume energy deposit (n_volumes doubles, indexed by touchable id) and its
  * ledger to the host, then zeroes them on the device. */
@@ -254,7 +267,19 @@ int adept_buffer_take(adept_buffer*, double* edep_per_volume, size_t n_volumes, 
                       adept_track* outgoing, size_t cap, size_t* n_outgoing);
 int adept_buffer_destroy(adept_buffer*);
 
-/* Test hook: exactly one step for each of n tracks, results in input order; secondaries[2*i + k]. */
+/* Test hook for the kernels adept_transport runs.  Loads n tracks -- any species, step, id and volume, taken
+ * as given (no Locate, steps not reset) -- into the EMPTY slot, runs EXACTLY ONE population step
+ * with the very kernels and launch configuration of adept_transport (gamma move, charged move, interaction;
+ * one step per track whatever config.steps_per_launch says) and copies the tracks of the next population --
+ * survivors and secondaries of all species, in no particular order -- to out[0 .. *n_out) (*n_out may exceed
+ * out_cap; only out_cap are copied).  The slot is empty again afterwards; deposits, the ledger (primary = energy
+ * carried by the n tracks), leaked tracks and the counters are read with the usual calls.  Allocates its
+ * transfer buffers with cudaMalloc, outside the workspace (test hooks do; transport never does). */
+int adept_step_population(adept_ctx*, int event_slot, int n, const adept_track* in, adept_track* out, size_t out_cap,
+                          size_t* n_out, void* cuda_stream);
+
+/* Test hook of the generic per-lane step (csrc/step.cuh), the form the persistent tail kernel runs: exactly one
+ * step for each of n tracks, results in input order; secondaries[2*i + k]. */
 int adept_step_frozen(adept_ctx*, int n, const adept_track* in, adept_step_result* out,
                       adept_track* secondaries, void* cuda_stream);
 

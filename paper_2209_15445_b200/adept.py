@@ -45,7 +45,8 @@ class CConfig(C.Structure):
                 ("chord_budget", C.c_int32), ("seed", C.c_uint32), ("max_steps", C.c_uint32), ("navigator", C.c_int32),
                 ("n_event_slots", C.c_int32), ("sync_interval", C.c_int32), ("track_capacity", C.c_uint64),
                 ("leak_capacity", C.c_uint64), ("stage_capacity", C.c_uint64), ("time_kernels", C.c_int32),
-                ("inject_chunk", C.c_uint64), ("pending_capacity", C.c_uint64), ("concurrent_species", C.c_int32), ("use_graphs", C.c_int32)]
+                ("inject_chunk", C.c_uint64), ("pending_capacity", C.c_uint64), ("concurrent_species", C.c_int32), ("steps_per_launch", C.c_int32),
+                ("use_graphs", C.c_int32)]
 
 
 class CLedger(C.Structure):
@@ -68,7 +69,7 @@ EXPORTS = ["adept_last_error", "adept_default_config", "adept_workspace_bytes", 
            "adept_enqueue_primaries", "adept_enqueue_batch", "adept_transport", "adept_transport_many",
            "adept_read_scoring", "adept_read_leaked", "adept_get_stats", "adept_get_kernel_times", "adept_set_kernel_timing", "adept_get_iteration_trace",
            "adept_raycast_batch", "adept_buffer_create", "adept_buffer_add", "adept_buffer_flush", "adept_buffer_pending", "adept_buffer_take",
-           "adept_buffer_destroy", "adept_step_frozen",
+           "adept_buffer_destroy", "adept_step_frozen", "adept_step_population", "adept_reset_slot",
            "adept_distance_batch", "adept_locate_batch", "adept_relocate_batch", "adept_shutdown"]
 
 
@@ -95,6 +96,8 @@ def load_library():
     lib.adept_set_kernel_timing.argtypes = [vp, i]
     lib.adept_get_iteration_trace.argtypes = [vp, i, vp, vp, sz, C.POINTER(sz)]
     lib.adept_step_frozen.argtypes = [vp, i, vp, vp, vp, vp]
+    lib.adept_step_population.argtypes = [vp, i, i, vp, vp, sz, C.POINTER(sz), vp]
+    lib.adept_reset_slot.argtypes = [vp, i]
     lib.adept_distance_batch.argtypes = [vp, i, i, vp, vp, vp, vp, vp, vp]
     lib.adept_locate_batch.argtypes = [vp, i, i, vp, vp, vp]
     lib.adept_relocate_batch.argtypes = [vp, i, i, vp, vp, vp, vp, vp]
@@ -147,10 +150,12 @@ class Adept:
     """One library context.  `geom`, `field` come from paper_2209_15445_b200.inputs; `scalars` is
     (n_mat, 8) and `tables` (n_mat, 12, 2048) as built by inputs.materials.build_material_set."""
 
-    def __init__(self, geom, tables, scalars, field, device="cuda:0", **config):
+    def __init__(self, geom, tables, scalars, field, device="cuda:0", _workspace_bytes=None, **config):
+        """_workspace_bytes (tests): size of the workspace handed to adept_init instead of adept_workspace_bytes()."""
         import torch
         self._torch = torch
         self.device = torch.device(device)
+        self.ctx = None
         self.cfg = default_config(**config)
         self.n_volumes = geom.n_volumes
         self._keep = [geom, np.ascontiguousarray(tables, dtype=np.float64),
@@ -167,12 +172,15 @@ class Adept:
         nbytes = lib.adept_workspace_bytes(C.byref(self.cfg), C.byref(g), n_mat, C.byref(f))
         if nbytes == 0:
             raise AdeptError(EINVAL)
+        self.workspace_bytes = nbytes
+        if _workspace_bytes is not None:
+            nbytes = _workspace_bytes
         with torch.cuda.device(self.device):
             self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
-            self.ctx = C.c_void_p()
-            _check(lib.adept_init(C.byref(self.ctx), C.byref(g), _ptr(self._keep[2]), n_mat, C.byref(t), C.byref(f),
+            ctx = C.c_void_p()
+            _check(lib.adept_init(C.byref(ctx), C.byref(g), _ptr(self._keep[2]), n_mat, C.byref(t), C.byref(f),
                                   C.byref(self.cfg), C.c_void_p(self.workspace.data_ptr()), nbytes))
-        self.workspace_bytes = nbytes
+            self.ctx = ctx
 
     def close(self):
         if getattr(self, "ctx", None):
@@ -262,7 +270,22 @@ class Adept:
         _check(lib.adept_get_iteration_trace(self.ctx, slot, _ptr(t), _ptr(pop), cap, C.byref(n)))
         return t[:n.value], pop[:n.value]
 
+    def reset_slot(self, slot=0):
+        _check(lib.adept_reset_slot(self.ctx, slot))
+
     # ---- test hooks
+    def step_population(self, tracks, slot=0, stream=None):
+        """Exactly one population step of the transport kernels on `tracks` (TRACK array, taken as given) in the
+        empty slot -> TRACK array of the next population (survivors and secondaries, no particular order)."""
+        tracks = np.ascontiguousarray(tracks, dtype=TRACK)
+        n = tracks.shape[0]
+        cap = 3 * n + 16
+        out = np.zeros(cap, dtype=TRACK)
+        n_out = C.c_size_t(0)
+        _check(lib.adept_step_population(self.ctx, slot, n, _ptr(tracks), _ptr(out), cap, C.byref(n_out), _stream_ptr(stream)))
+        assert n_out.value <= cap
+        return out[:n_out.value]
+
     def step_frozen(self, tracks, stream=None):
         tracks = np.ascontiguousarray(tracks, dtype=TRACK)
         n = tracks.shape[0]

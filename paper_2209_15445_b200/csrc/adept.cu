@@ -27,11 +27,37 @@ int fail(int code, const char* fmt, ...) {
   return code;
 }
 
+#define ADEPT_ON_DEVICE(ctx)                                                         \
+  DeviceGuard device_guard_((ctx)->device);                                          \
+  if (!device_guard_.ok) return fail(ADEPT_ECUDA, "cannot make device %d current", (ctx)->device)
+
 #define CUDA_TRY(expr)                                                                         \
   do {                                                                                         \
     cudaError_t e_ = (expr);                                                                   \
     if (e_ != cudaSuccess) return fail(ADEPT_ECUDA, "%s: %s", #expr, cudaGetErrorString(e_));  \
   } while (0)
+
+// Makes the context's device current for the duration of an ABI call and restores the caller's.
+struct DeviceGuard {
+  int prev = -1;
+  bool ok = true;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+    if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+    if (prev == dev) prev = -1;
+  }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+// Device scratch of the test hooks (they allocate outside the caller's workspace; transport never does):
+// freed on every exit path.
+template <typename T>
+struct DevBuf {
+  T* p = nullptr;
+  ~DevBuf() { if (p) cudaFree(p); }
+  cudaError_t alloc(size_t n) { return cudaMalloc(&p, std::max<size_t>(n, 1) * sizeof(T)); }
+  operator T*() const { return p; }
+};
 
 constexpr int kBvhMinDaughters = 65;  // below this a per-lane loop over the daughters is cheaper
 
@@ -226,6 +252,7 @@ struct SlotHost {
 struct adept_ctx {
   adept_config cfg{};
   DevCtx dev{};
+  int device = 0;                    // CUDA device of the workspace: made current at every ABI entry
   int n_vol = 0, n_mat = 0;
   std::vector<SlotHost> slots;
   adept_track* d_stage = nullptr;    // staging area for primaries (inside the workspace)
@@ -238,6 +265,21 @@ struct adept_ctx {
   bool timing_on = false;            // per-launch CUDA events active (adept_set_kernel_timing)
 };
 
+namespace {
+void destroy_ctx(adept_ctx* ctx) {
+  for (SlotHost& sh : ctx->slots) {
+    if (sh.gexec) cudaGraphExecDestroy(sh.gexec);
+    if (sh.cap) cudaStreamDestroy(sh.cap);
+    if (sh.helper) cudaStreamDestroy(sh.helper);
+    if (sh.fork) cudaEventDestroy(sh.fork);
+    if (sh.join) cudaEventDestroy(sh.join);
+    if (sh.pinned) cudaFreeHost(sh.pinned);
+    for (cudaEvent_t e : sh.tev) if (e) cudaEventDestroy(e);
+  }
+  delete ctx;
+}
+}  // namespace
+
 extern "C" const char* adept_last_error(void) { return g_err; }
 
 extern "C" void adept_default_config(adept_config* c) {
@@ -248,6 +290,7 @@ extern "C" void adept_default_config(adept_config* c) {
   c->navigator = ADEPT_NAV_BVH; c->n_event_slots = 1; c->sync_interval = 16;
   c->track_capacity = 1u << 20; c->leak_capacity = 1u << 16; c->stage_capacity = 0;
   c->concurrent_species = 1;
+  c->steps_per_launch = 0;
   c->use_graphs = 1;
 }
 
@@ -262,6 +305,7 @@ int validate(const adept_config* cfg, const adept_geometry* g, int n_mats, const
   if (cfg->track_capacity < 32 || cfg->track_capacity > 0x3fffffffu) return fail(ADEPT_EINVAL, "track_capacity out of range");
   if (cfg->stage_capacity != 0 && (cfg->stage_capacity < 32 || cfg->stage_capacity > 0x3fffffffu)) return fail(ADEPT_EINVAL, "stage_capacity out of range");
   if (cfg->chord_budget < 1 || cfg->sync_interval < 1) return fail(ADEPT_EINVAL, "chord_budget / sync_interval must be >= 1");
+  if (cfg->steps_per_launch < 0 || cfg->steps_per_launch > 4096) return fail(ADEPT_EINVAL, "steps_per_launch out of range");
   if (g->mother[0] != -1) return fail(ADEPT_EINVAL, "volume 0 must be the world");
   for (int v = 0; v < g->n_volumes; ++v) {
     if (g->solid[v] != ADEPT_BOX && g->solid[v] != ADEPT_TUBE) return fail(ADEPT_EINVAL, "volume %d: unknown solid", v);
@@ -367,6 +411,14 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   Layout L;
   const size_t need = carve(d_workspace, cfg, g, n_mats, f, nullptr, &L);
   if (workspace_bytes < need) return fail(ADEPT_ENOMEM, "workspace has %zu bytes, %zu needed", workspace_bytes, need);
+  // the context lives on the device that owns the workspace, whatever device is current in later calls
+  cudaPointerAttributes attr{};
+  if (cudaPointerGetAttributes(&attr, d_workspace) != cudaSuccess || attr.type != cudaMemoryTypeDevice) {
+    cudaGetLastError();
+    return fail(ADEPT_EINVAL, "d_workspace is not device memory");
+  }
+  DeviceGuard device_guard_(attr.device);
+  if (!device_guard_.ok) return fail(ADEPT_ECUDA, "cannot make device %d current", attr.device);
   CUDA_TRY(cudaMemset(d_workspace, 0, need));
 
   // ---- volumes + BVHs
@@ -461,7 +513,9 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
 
   adept_ctx* ctx = new (std::nothrow) adept_ctx;
   if (!ctx) return fail(ADEPT_ENOMEM, "host allocation failed");
+  struct Holder { adept_ctx* c; ~Holder() { if (c) destroy_ctx(c); } } holder{ctx};   // freed on every error return below
   ctx->cfg = *cfg;
+  ctx->device = attr.device;
   ctx->n_vol = nv; ctx->n_mat = n_mats;
   DevCtx& d = ctx->dev;
   d.vol = L.vol; d.rot = L.rot; d.nbr = L.nbr; d.n_vol = nv; d.bvh = L.bvh; d.navigator = cfg->navigator;
@@ -474,6 +528,7 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   d.inv_du = 1.0 / d.du;
   d.delta_chord = cfg->delta_chord; d.eps_push = cfg->eps_push; d.alpha_R = cfg->alpha_R; d.rho_R = cfg->rho_R;
   d.chord_budget = cfg->chord_budget; d.seed = cfg->seed; d.max_steps = cfg->max_steps;
+  d.steps_per_launch = cfg->steps_per_launch;
   d.capacity = static_cast<uint32_t>(cfg->track_capacity);
   d.stage_capacity = static_cast<uint32_t>(cfg->stage_capacity ? cfg->stage_capacity : cfg->track_capacity);
   d.leak_capacity = static_cast<uint32_t>(cfg->leak_capacity);
@@ -484,9 +539,8 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   CUDA_TRY(cudaGetLastError());
   CUDA_TRY(cudaDeviceSynchronize());
 
-  int dev = 0, sms = 0, occ_g = 1, occ_c = 1, occ_i = 1;
-  CUDA_TRY(cudaGetDevice(&dev));
-  CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  int sms = 0, occ_g = 1, occ_c = 1, occ_i = 1;
+  CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->device));
   {
     const bool bvh = cfg->navigator == ADEPT_NAV_BVH && !hb.empty();
     ctx->k_move_gamma = bvh ? gamma_move_kernel<true> : gamma_move_kernel<false>;
@@ -522,12 +576,14 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
     }
   }
   ctx->timing_on = cfg->time_kernels != 0;
+  holder.c = nullptr;
   *out = ctx;
   return ADEPT_OK;
 }
 
 extern "C" int adept_set_kernel_timing(adept_ctx* ctx, int on) {
   if (!ctx) return fail(ADEPT_EINVAL, "null context");
+  ADEPT_ON_DEVICE(ctx);
   if (on && !ctx->cfg.time_kernels) return fail(ADEPT_ESTATE, "context was not created with time_kernels");
   for (const SlotHost& sh : ctx->slots) if (sh.live) return fail(ADEPT_ESTATE, "a slot is being transported");
   ctx->timing_on = on != 0;
@@ -536,16 +592,8 @@ extern "C" int adept_set_kernel_timing(adept_ctx* ctx, int on) {
 
 extern "C" int adept_shutdown(adept_ctx* ctx) {
   if (!ctx) return fail(ADEPT_EINVAL, "null context");
-  for (SlotHost& sh : ctx->slots) {
-    if (sh.gexec) cudaGraphExecDestroy(sh.gexec);
-    if (sh.cap) cudaStreamDestroy(sh.cap);
-    if (sh.helper) cudaStreamDestroy(sh.helper);
-    if (sh.fork) cudaEventDestroy(sh.fork);
-    if (sh.join) cudaEventDestroy(sh.join);
-    if (sh.pinned) cudaFreeHost(sh.pinned);
-    for (cudaEvent_t e : sh.tev) cudaEventDestroy(e);
-  }
-  delete ctx;
+  ADEPT_ON_DEVICE(ctx);
+  destroy_ctx(ctx);
   return ADEPT_OK;
 }
 
@@ -555,13 +603,41 @@ int check_slot(adept_ctx* ctx, int slot) {
   if (slot < 0 || slot >= static_cast<int>(ctx->slots.size())) return fail(ADEPT_EINVAL, "event slot %d out of range", slot);
   return ADEPT_OK;
 }
+
+// Empties a slot on `st`: counters (populations, staging queues, leaked tracks, overflow flag), every replica
+// of the scoring array, the ledger and the iteration trace.  The cumulative DevStats stay.
+int reset_slot_async(adept_ctx* ctx, SlotHost& sh, cudaStream_t st) {
+  CUDA_TRY(cudaMemsetAsync(sh.dev.counters, 0, sizeof(SlotCounters), st));
+  CUDA_TRY(cudaMemsetAsync(sh.dev.edep, 0, static_cast<size_t>(sh.dev.edep_mask + 1) * sh.dev.edep_stride * sizeof(double), st));
+  CUDA_TRY(cudaMemsetAsync(sh.dev.ledger, 0, 8 * sizeof(double), st));
+  CUDA_TRY(cudaMemsetAsync(sh.dev.trace_n, 0, sizeof(uint32_t), st));
+  sh.n_pending = sh.n_injected = 0;
+  (void)ctx;
+  return ADEPT_OK;
+}
 }  // namespace
+
+extern "C" int adept_reset_slot(adept_ctx* ctx, int slot) {
+  const int rc = check_slot(ctx, slot);
+  if (rc != ADEPT_OK) return rc;
+  ADEPT_ON_DEVICE(ctx);
+  SlotHost& sh = ctx->slots[slot];
+  if (sh.live) return fail(ADEPT_ESTATE, "slot %d is being transported", slot);
+  CUDA_TRY(cudaDeviceSynchronize());
+  const int r2 = reset_slot_async(ctx, sh, nullptr);
+  if (r2 != ADEPT_OK) return r2;
+  CUDA_TRY(cudaDeviceSynchronize());
+  return ADEPT_OK;
+}
 
 extern "C" int adept_enqueue_batch(adept_ctx* ctx, int slot, int n, const uint32_t* event_ids, const uint64_t* track_ids,
                                    const int8_t* species, const double* pos3, const double* dir3, const double* ekin) {
   int rc = check_slot(ctx, slot);
   if (rc != ADEPT_OK) return rc;
   if (n < 0 || (n > 0 && (!event_ids || !track_ids || !species || !pos3 || !dir3 || !ekin))) return fail(ADEPT_EINVAL, "null argument");
+  ADEPT_ON_DEVICE(ctx);
+  // Runs on the legacy default stream and ends with a blocking copy of the error counter: the primaries are in
+  // the slot when the call returns, whatever stream the transport then uses.
   SlotHost& sh = ctx->slots[slot];
   if (sh.live) return fail(ADEPT_ESTATE, "slot %d is being transported", slot);
   const bool stagger = ctx->cfg.inject_chunk != 0;
@@ -607,12 +683,12 @@ namespace {
 // One population step of a slot: gamma move kernel on the caller's stream, charged move kernel on the
 // helper stream (species kernels on different streams, synchronised with events), then the
 // interaction kernel over what they staged and the buffer swap.
-int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity) {
+int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity, const DevCtx& dc) {
   constexpr int kEv = 2 * ADEPT_N_TIMED_KERNELS;
   if (sh.n_injected < sh.n_pending) {   // staggered injection: the next chunk joins the population of this step
     const size_t m = std::min<size_t>(ctx->cfg.inject_chunk, sh.n_pending - sh.n_injected);
     inject_kernel<<<static_cast<int>(std::min<size_t>((m + kBlock - 1) / kBlock, 1024)), kBlock, 0, st>>>(
-        ctx->dev, sh.dev, parity, static_cast<uint32_t>(sh.n_injected), static_cast<uint32_t>(m));
+        dc, sh.dev, parity, static_cast<uint32_t>(sh.n_injected), static_cast<uint32_t>(m));
     sh.n_injected += m;
     sh.launches += 1;
   }
@@ -626,17 +702,17 @@ int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity) 
   }
   cudaEvent_t* ev = timed ? &sh.tev[sh.tev_used] : nullptr;
   if (timed) CUDA_TRY(cudaEventRecord(ev[0], st));
-  ctx->k_move_gamma<<<dim3(ctx->grid_gamma, 1), kBlock, 0, st>>>(ctx->dev, sh.dev, parity);
+  ctx->k_move_gamma<<<dim3(ctx->grid_gamma, 1), kBlock, 0, st>>>(dc, sh.dev, parity);
   if (timed) CUDA_TRY(cudaEventRecord(ev[1], st));
   if (timed) CUDA_TRY(cudaEventRecord(ev[2], sc));
-  ctx->k_move_charged<<<dim3(ctx->grid_charged, 2), kBlock, 0, sc>>>(ctx->dev, sh.dev, parity);
+  ctx->k_move_charged<<<dim3(ctx->grid_charged, 2), kBlock, 0, sc>>>(dc, sh.dev, parity);
   if (timed) CUDA_TRY(cudaEventRecord(ev[3], sc));
   if (fork) {
     CUDA_TRY(cudaEventRecord(sh.join, sh.helper));
     CUDA_TRY(cudaStreamWaitEvent(st, sh.join, 0));
   }
   if (timed) CUDA_TRY(cudaEventRecord(ev[4], st));
-  interact_kernel<<<ctx->grid_inter, kBlock, 0, st>>>(ctx->dev, sh.dev, parity);
+  interact_kernel<<<ctx->grid_inter, kBlock, 0, st>>>(dc, sh.dev, parity);
   if (timed) { CUDA_TRY(cudaEventRecord(ev[5], st)); sh.tev_used += kEv; }
   sh.launches += 3;
   return ADEPT_OK;
@@ -655,7 +731,7 @@ bool round_graph(adept_ctx* ctx, SlotHost& sh) {
   cudaGraph_t graph = nullptr;
   bool ok = cudaStreamBeginCapture(sh.cap, cudaStreamCaptureModeRelaxed) == cudaSuccess;
   if (ok) {
-    for (int it = 0; it < ctx->cfg.sync_interval && ok; ++it) ok = launch_iteration(ctx, sh, sh.cap, it & 1) == ADEPT_OK;
+    for (int it = 0; it < ctx->cfg.sync_interval && ok; ++it) ok = launch_iteration(ctx, sh, sh.cap, it & 1, ctx->dev) == ADEPT_OK;
     ok = (cudaStreamEndCapture(sh.cap, &graph) == cudaSuccess) && ok && graph;
   }
   if (ok) ok = cudaGraphInstantiate(&sh.gexec, graph, 0) == cudaSuccess;
@@ -669,10 +745,21 @@ bool round_graph(adept_ctx* ctx, SlotHost& sh) {
 
 extern "C" int adept_transport_many(adept_ctx* ctx, int n_slots, const int* slots, void* const* streams) {
   if (!ctx || n_slots < 0 || (n_slots > 0 && (!slots || !streams))) return fail(ADEPT_EINVAL, "null argument");
+  ADEPT_ON_DEVICE(ctx);
   for (int k = 0; k < n_slots; ++k) {
     const int rc = check_slot(ctx, slots[k]);
     if (rc != ADEPT_OK) return rc;
-    ctx->slots[slots[k]].live = true;
+  }
+  // Marks the listed slots live; whatever way this call ends, none of them stays marked.
+  struct LiveMarks {
+    adept_ctx* ctx; const int* slots; int n = 0;
+    ~LiveMarks() { for (int k = 0; k < n; ++k) ctx->slots[slots[k]].live = false; }
+  } marks{ctx, slots};
+  for (int k = 0; k < n_slots; ++k) {
+    SlotHost& sh = ctx->slots[slots[k]];
+    if (sh.live) return fail(ADEPT_EINVAL, "event slot %d is listed twice or already in transport", slots[k]);
+    sh.live = true;
+    marks.n = k + 1;
   }
   std::vector<int> parity(n_slots, 0);
   int n_live = n_slots, rc_final = ADEPT_OK;
@@ -690,7 +777,7 @@ extern "C" int adept_transport_many(adept_ctx* ctx, int n_slots, const int* slot
       for (int k = 0; k < n_slots; ++k) {
         SlotHost& sh = ctx->slots[slots[k]];
         if (!sh.live || graphed[k]) continue;
-        const int rc = launch_iteration(ctx, sh, static_cast<cudaStream_t>(streams[k]), parity[k]);
+        const int rc = launch_iteration(ctx, sh, static_cast<cudaStream_t>(streams[k]), parity[k], ctx->dev);
         if (rc != ADEPT_OK) return rc;
         parity[k] ^= 1;
       }
@@ -702,7 +789,8 @@ extern "C" int adept_transport_many(adept_ctx* ctx, int n_slots, const int* slot
     for (int k = 0; k < n_slots; ++k) {
       SlotHost& sh = ctx->slots[slots[k]];
       if (!sh.live) continue;
-      CUDA_TRY(cudaStreamSynchronize(static_cast<cudaStream_t>(streams[k])));
+      cudaStream_t st = static_cast<cudaStream_t>(streams[k]);
+      CUDA_TRY(cudaStreamSynchronize(st));
       for (int e = 0; e + 2 * ADEPT_N_TIMED_KERNELS <= sh.tev_used; e += 2 * ADEPT_N_TIMED_KERNELS)
         for (int kk = 0; kk < ADEPT_N_TIMED_KERNELS; ++kk) {
           float ms = 0.f;
@@ -711,19 +799,27 @@ extern "C" int adept_transport_many(adept_ctx* ctx, int n_slots, const int* slot
           sh.kernel_launches[kk] += 1;
         }
       sh.tev_used = 0;
-      if (sh.pinned->overflow.v) rc_final = fail(ADEPT_EOVERFLOW, "slot %d: track queue overflow (capacity %llu per species)",
-                                               slots[k], static_cast<unsigned long long>(ctx->cfg.track_capacity));
-      if ((sh.pinned->live.v == 0 && sh.n_injected == sh.n_pending) || sh.pinned->overflow.v) {
+      const bool overflow = sh.pinned->overflow.v != 0;
+      if (overflow) {
+        // The pass is abandoned: the slot is emptied (tracks, staging queues, scoring, ledger, leaked tracks) so
+        // that the caller can enqueue a smaller batch into it.
+        rc_final = fail(ADEPT_EOVERFLOW, "slot %d: track queue overflow (capacity %llu per species, %llu per staging queue); slot reset",
+                        slots[k], static_cast<unsigned long long>(ctx->dev.capacity), static_cast<unsigned long long>(ctx->dev.stage_capacity));
+        const int rr = reset_slot_async(ctx, sh, st);
+        if (rr != ADEPT_OK) return rr;
+        CUDA_TRY(cudaStreamSynchronize(st));
+      }
+      if ((sh.pinned->live.v == 0 && sh.n_injected == sh.n_pending) || overflow) {
         sh.n_pending = sh.n_injected = 0;
         sh.live = false;
         --n_live;
-        if (parity[k]) {  // leave the (empty) slot at parity 0 for the next enqueue
-          // counts are all zero, nothing to move
-        }
+        // counts are all zero: the (empty) slot is at parity 0 for the next enqueue whatever parity[k] is
       }
     }
   }
   CUDA_TRY(cudaGetLastError());
+  if (rc_final != ADEPT_OK) fail(rc_final, "a slot's track queue overflowed (track_capacity %llu, stage_capacity %llu); the slot was reset",
+                                 static_cast<unsigned long long>(ctx->dev.capacity), static_cast<unsigned long long>(ctx->dev.stage_capacity));
   return rc_final;
 }
 
@@ -734,6 +830,7 @@ extern "C" int adept_transport(adept_ctx* ctx, int slot, void* stream) {
 extern "C" int adept_read_scoring(adept_ctx* ctx, int slot, double* edep, size_t n_volumes, adept_ledger* ledger, void* stream) {
   const int rc = check_slot(ctx, slot);
   if (rc != ADEPT_OK) return rc;
+  ADEPT_ON_DEVICE(ctx);
   if (edep && n_volumes != static_cast<size_t>(ctx->n_vol)) return fail(ADEPT_EINVAL, "n_volumes is %zu, geometry has %d", n_volumes, ctx->n_vol);
   SlotHost& sh = ctx->slots[slot];
   cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -751,6 +848,7 @@ extern "C" int adept_read_scoring(adept_ctx* ctx, int slot, double* edep, size_t
 extern "C" int adept_read_leaked(adept_ctx* ctx, int slot, adept_track* out, size_t cap, size_t* n) {
   const int rc = check_slot(ctx, slot);
   if (rc != ADEPT_OK) return rc;
+  ADEPT_ON_DEVICE(ctx);
   if (!n) return fail(ADEPT_EINVAL, "null argument");
   SlotHost& sh = ctx->slots[slot];
   uint32_t n_leaked = 0;
@@ -765,6 +863,7 @@ extern "C" int adept_read_leaked(adept_ctx* ctx, int slot, adept_track* out, siz
 extern "C" int adept_get_stats(adept_ctx* ctx, int slot, adept_stats* out) {
   const int rc = check_slot(ctx, slot);
   if (rc != ADEPT_OK) return rc;
+  ADEPT_ON_DEVICE(ctx);
   if (!out) return fail(ADEPT_EINVAL, "null argument");
   DevStats s;
   CUDA_TRY(cudaMemcpy(&s, ctx->slots[slot].dev.stats, sizeof(s), cudaMemcpyDeviceToHost));
@@ -778,6 +877,7 @@ extern "C" int adept_get_stats(adept_ctx* ctx, int slot, adept_stats* out) {
 extern "C" int adept_get_iteration_trace(adept_ctx* ctx, int slot, uint64_t* t_ns, uint32_t* population, size_t cap, size_t* n) {
   const int rc = check_slot(ctx, slot);
   if (rc != ADEPT_OK) return rc;
+  ADEPT_ON_DEVICE(ctx);
   if (!n) return fail(ADEPT_EINVAL, "null argument");
   SlotHost& sh = ctx->slots[slot];
   if (sh.live) return fail(ADEPT_ESTATE, "slot %d is being transported", slot);
@@ -808,12 +908,11 @@ extern "C" int adept_step_frozen(adept_ctx* ctx, int n, const adept_track* in, a
   for (int i = 0; i < n; ++i)
     if (in[i].volume >= static_cast<uint32_t>(ctx->n_vol) || in[i].species < 0 || in[i].species > 2)
       return fail(ADEPT_EINVAL, "track %d: volume or species out of range", i);
+  ADEPT_ON_DEVICE(ctx);
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  adept_track *d_in = nullptr, *d_sec = nullptr;
-  adept_step_result* d_out = nullptr;
-  CUDA_TRY(cudaMalloc(&d_in, n * sizeof(adept_track)));
-  CUDA_TRY(cudaMalloc(&d_out, n * sizeof(adept_step_result)));
-  CUDA_TRY(cudaMalloc(&d_sec, 2 * static_cast<size_t>(n) * sizeof(adept_track)));
+  DevBuf<adept_track> d_in, d_sec;
+  DevBuf<adept_step_result> d_out;
+  CUDA_TRY(d_in.alloc(n)); CUDA_TRY(d_out.alloc(n)); CUDA_TRY(d_sec.alloc(2 * static_cast<size_t>(n)));
   CUDA_TRY(cudaMemcpyAsync(d_in, in, n * sizeof(adept_track), cudaMemcpyHostToDevice, st));
   const int grid = std::min((n + kBlock - 1) / kBlock, 65535);
   frozen_kernel<<<grid, kBlock, 0, st>>>(ctx->dev, d_in, d_out, d_sec, n);
@@ -821,7 +920,62 @@ extern "C" int adept_step_frozen(adept_ctx* ctx, int n, const adept_track* in, a
   CUDA_TRY(cudaMemcpyAsync(out, d_out, n * sizeof(adept_step_result), cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaMemcpyAsync(sec, d_sec, 2 * static_cast<size_t>(n) * sizeof(adept_track), cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
-  cudaFree(d_in); cudaFree(d_out); cudaFree(d_sec);
+  return ADEPT_OK;
+}
+
+extern "C" int adept_step_population(adept_ctx* ctx, int slot, int n, const adept_track* in, adept_track* out, size_t out_cap,
+                                     size_t* n_out, void* stream) {
+  const int rc = check_slot(ctx, slot);
+  if (rc != ADEPT_OK) return rc;
+  if (n < 0 || !n_out || (n > 0 && !in) || (out_cap > 0 && !out)) return fail(ADEPT_EINVAL, "null argument");
+  *n_out = 0;
+  for (int i = 0; i < n; ++i)
+    if (in[i].volume >= static_cast<uint32_t>(ctx->n_vol) || in[i].species < 0 || in[i].species > 2 || !(in[i].ekin >= 0.0))
+      return fail(ADEPT_EINVAL, "track %d: volume, species or energy out of range", i);
+  ADEPT_ON_DEVICE(ctx);
+  SlotHost& sh = ctx->slots[slot];
+  if (sh.live || sh.n_pending != sh.n_injected) return fail(ADEPT_ESTATE, "slot %d is not empty", slot);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  CUDA_TRY(cudaMemcpyAsync(sh.pinned, sh.dev.counters, sizeof(SlotCounters), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  if (sh.pinned->live.v != 0) return fail(ADEPT_ESTATE, "slot %d holds %u live tracks", slot, sh.pinned->live.v);
+  if (n == 0) return ADEPT_OK;
+  DevBuf<adept_track> d_in, d_out;
+  CUDA_TRY(d_in.alloc(n));
+  CUDA_TRY(cudaMemcpyAsync(d_in, in, static_cast<size_t>(n) * sizeof(adept_track), cudaMemcpyHostToDevice, st));
+  load_tracks_kernel<<<std::min((n + kBlock - 1) / kBlock, 4096), kBlock, 0, st>>>(ctx->dev, sh.dev, d_in, n);
+  CUDA_TRY(cudaGetLastError());
+  // exactly one population step: the kernels and grids of adept_transport, one step per track and launch
+  DevCtx one = ctx->dev;
+  one.steps_per_launch = 1;
+  const bool timing = ctx->timing_on;
+  ctx->timing_on = false;
+  const int rl = launch_iteration(ctx, sh, st, 0, one);
+  ctx->timing_on = timing;
+  if (rl != ADEPT_OK) return rl;
+  CUDA_TRY(cudaMemcpyAsync(sh.pinned, sh.dev.counters, sizeof(SlotCounters), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  if (sh.pinned->overflow.v) {
+    const int rr = reset_slot_async(ctx, sh, st);
+    if (rr != ADEPT_OK) return rr;
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return fail(ADEPT_EOVERFLOW, "slot %d: track queue overflow in the population step; slot reset", slot);
+  }
+  uint32_t cnt[3];
+  size_t total = 0;
+  for (int sp = 0; sp < 3; ++sp) { cnt[sp] = sh.pinned->count[1][sp].v; total += cnt[sp]; }
+  *n_out = total;
+  if (total > 0) {
+    CUDA_TRY(d_out.alloc(total));
+    gather_tracks_kernel<<<static_cast<int>(std::min<size_t>((total + kBlock - 1) / kBlock, 4096)), kBlock, 0, st>>>(
+        sh.dev, 1, cnt[0], cnt[1], cnt[2], d_out);
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaMemcpyAsync(out, d_out, std::min(total, out_cap) * sizeof(adept_track), cudaMemcpyDeviceToHost, st));
+  }
+  // the slot is empty again: the next population is dropped
+  for (int sp = 0; sp < 3; ++sp) CUDA_TRY(cudaMemsetAsync(&sh.dev.counters->count[1][sp].v, 0, sizeof(uint32_t), st));
+  CUDA_TRY(cudaMemsetAsync(&sh.dev.counters->live.v, 0, sizeof(uint32_t), st));
+  CUDA_TRY(cudaStreamSynchronize(st));
   return ADEPT_OK;
 }
 
@@ -830,12 +984,12 @@ extern "C" int adept_distance_batch(adept_ctx* ctx, int nav, int n, const double
   if (!ctx || n < 0 || (n > 0 && (!pos3 || !dir3 || !volume || !s_max || !out))) return fail(ADEPT_EINVAL, "null argument");
   if (n == 0) return ADEPT_OK;
   for (int i = 0; i < n; ++i) if (volume[i] >= static_cast<uint32_t>(ctx->n_vol)) return fail(ADEPT_EINVAL, "ray %d: volume out of range", i);
+  ADEPT_ON_DEVICE(ctx);
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  double *d_pos, *d_dir, *d_smax, *d_out;
-  uint32_t* d_vol;
-  CUDA_TRY(cudaMalloc(&d_pos, 3 * n * sizeof(double))); CUDA_TRY(cudaMalloc(&d_dir, 3 * n * sizeof(double)));
-  CUDA_TRY(cudaMalloc(&d_smax, n * sizeof(double))); CUDA_TRY(cudaMalloc(&d_out, n * sizeof(double)));
-  CUDA_TRY(cudaMalloc(&d_vol, n * sizeof(uint32_t)));
+  DevBuf<double> d_pos, d_dir, d_smax, d_out;
+  DevBuf<uint32_t> d_vol;
+  CUDA_TRY(d_pos.alloc(3 * static_cast<size_t>(n))); CUDA_TRY(d_dir.alloc(3 * static_cast<size_t>(n)));
+  CUDA_TRY(d_smax.alloc(n)); CUDA_TRY(d_out.alloc(n)); CUDA_TRY(d_vol.alloc(n));
   CUDA_TRY(cudaMemcpyAsync(d_pos, pos3, 3 * n * sizeof(double), cudaMemcpyHostToDevice, st));
   CUDA_TRY(cudaMemcpyAsync(d_dir, dir3, 3 * n * sizeof(double), cudaMemcpyHostToDevice, st));
   CUDA_TRY(cudaMemcpyAsync(d_smax, s_max, n * sizeof(double), cudaMemcpyHostToDevice, st));
@@ -844,7 +998,6 @@ extern "C" int adept_distance_batch(adept_ctx* ctx, int nav, int n, const double
   CUDA_TRY(cudaGetLastError());
   CUDA_TRY(cudaMemcpyAsync(out, d_out, n * sizeof(double), cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
-  cudaFree(d_pos); cudaFree(d_dir); cudaFree(d_smax); cudaFree(d_out); cudaFree(d_vol);
   return ADEPT_OK;
 }
 
@@ -854,6 +1007,7 @@ extern "C" int adept_raycast_batch(adept_ctx* ctx, int nav, int n, const double*
   if (nav != ADEPT_NAV_LOOP && nav != ADEPT_NAV_BVH) return fail(ADEPT_EINVAL, "unknown navigator");
   if (max_crossings < 1) return fail(ADEPT_EINVAL, "max_crossings must be >= 1");
   if (n == 0) return ADEPT_OK;
+  ADEPT_ON_DEVICE(ctx);
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   double *d_pos = nullptr, *d_dir = nullptr, *d_col = nullptr;
   int32_t* d_nx = nullptr;
@@ -886,16 +1040,16 @@ extern "C" int adept_raycast_batch(adept_ctx* ctx, int nav, int n, const double*
 extern "C" int adept_locate_batch(adept_ctx* ctx, int nav, int n, const double* pos3, int64_t* out, void* stream) {
   if (!ctx || n < 0 || (n > 0 && (!pos3 || !out))) return fail(ADEPT_EINVAL, "null argument");
   if (n == 0) return ADEPT_OK;
+  ADEPT_ON_DEVICE(ctx);
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  double* d_pos;
-  long long* d_out;
-  CUDA_TRY(cudaMalloc(&d_pos, 3 * n * sizeof(double))); CUDA_TRY(cudaMalloc(&d_out, n * sizeof(long long)));
+  DevBuf<double> d_pos;
+  DevBuf<long long> d_out;
+  CUDA_TRY(d_pos.alloc(3 * static_cast<size_t>(n))); CUDA_TRY(d_out.alloc(n));
   CUDA_TRY(cudaMemcpyAsync(d_pos, pos3, 3 * n * sizeof(double), cudaMemcpyHostToDevice, st));
   locate_kernel<<<std::min((n + kBlock - 1) / kBlock, 65535), kBlock, 0, st>>>(ctx->dev, nav, n, d_pos, d_out);
   CUDA_TRY(cudaGetLastError());
   CUDA_TRY(cudaMemcpyAsync(out, d_out, n * sizeof(long long), cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
-  cudaFree(d_pos); cudaFree(d_out);
   return ADEPT_OK;
 }
 
@@ -907,25 +1061,24 @@ extern "C" int adept_relocate_batch(adept_ctx* ctx, int nav, int n, const double
     if (from[i] >= static_cast<uint32_t>(ctx->n_vol)) return fail(ADEPT_EINVAL, "point %d: volume out of range", i);
     if (face && (face[i] < -1 || face[i] > 5)) return fail(ADEPT_EINVAL, "point %d: face out of range", i);
   }
+  ADEPT_ON_DEVICE(ctx);
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  double* d_pos;
-  uint32_t* d_from;
-  int32_t* d_face = nullptr;
-  long long* d_out;
-  CUDA_TRY(cudaMalloc(&d_pos, 3 * n * sizeof(double))); CUDA_TRY(cudaMalloc(&d_from, n * sizeof(uint32_t)));
-  CUDA_TRY(cudaMalloc(&d_out, n * sizeof(long long)));
+  DevBuf<double> d_pos;
+  DevBuf<uint32_t> d_from;
+  DevBuf<int32_t> d_face;
+  DevBuf<long long> d_out;
+  CUDA_TRY(d_pos.alloc(3 * static_cast<size_t>(n))); CUDA_TRY(d_from.alloc(n)); CUDA_TRY(d_out.alloc(n));
   CUDA_TRY(cudaMemcpyAsync(d_pos, pos3, 3 * n * sizeof(double), cudaMemcpyHostToDevice, st));
   CUDA_TRY(cudaMemcpyAsync(d_from, from, n * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
   if (face) {
-    CUDA_TRY(cudaMalloc(&d_face, n * sizeof(int32_t)));
+    CUDA_TRY(d_face.alloc(n));
     CUDA_TRY(cudaMemcpyAsync(d_face, face, n * sizeof(int32_t), cudaMemcpyHostToDevice, st));
   }
-  relocate_kernel<<<std::min((n + kBlock - 1) / kBlock, 65535), kBlock, 0, st>>>(ctx->dev, nav, n, d_pos, d_from, d_face, d_out);
+  relocate_kernel<<<std::min((n + kBlock - 1) / kBlock, 65535), kBlock, 0, st>>>(ctx->dev, nav, n, d_pos, d_from,
+                                                                                 face ? d_face.p : nullptr, d_out);
   CUDA_TRY(cudaGetLastError());
   CUDA_TRY(cudaMemcpyAsync(out, d_out, n * sizeof(long long), cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
-  if (d_face) cudaFree(d_face);
-  cudaFree(d_pos); cudaFree(d_from); cudaFree(d_out);
   return ADEPT_OK;
 }
 

@@ -25,9 +25,6 @@ namespace adept {
 #define ADEPT_MINB_C2F 4
 #endif
 
-// generic-proxy writes to the tile must be ordered before the TMA (async proxy) refill of the same buffer
-__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-
 template <int FIELD, bool BVH>
 __global__ void __launch_bounds__(kBlock, FIELD == ADEPT_FIELD_NONE ? ADEPT_MINB_C2 : ADEPT_MINB_C2F)
 charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot, int parity) {
@@ -35,7 +32,8 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
   const bool positron = species == ADEPT_POSITRON;
   const TrackSoA& cur = slot.buf[parity][species];
   SlotCounters* cnt = slot.counters;
-  const uint32_t n = cnt->count[parity][species].v;
+  // (a counter can run past the capacity when its queue overflowed: the stores are guarded, the reads clamped)
+  const uint32_t n = min(cnt->count[parity][species].v, c.capacity);
 
   // destinations: 0 = next buffer of the species, 1..3 = its staging queues, 4 = next gamma buffer (the
   // photons of an annihilation at rest)
@@ -62,6 +60,8 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
   const unsigned lt = (1u << lane) - 1u;
   const int t = threadIdx.x >> lane_shift;                 // this lane's entry of the tile
   const bool mine = (threadIdx.x & ((1u << lane_shift) - 1u)) == 0;
+  const int k_inner = inner_steps(c, n, gridDim.x * kBlock);
+  int counted = 0;   // steps a lane may have added to each field of `packed` since the last flush
   enum { FATE_NONE = 0, FATE_KILLED, FATE_STOPPED, FATE_GO };
 
   if (threadIdx.x == 0) tile_issue_n(pipe.tile[0], cur, static_cast<size_t>(blockIdx.x) * g, g, &pipe.bar[0]);
@@ -72,8 +72,16 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
       tile_issue_n(pipe.tile[phase ^ 1], cur, static_cast<size_t>(tile + gridDim.x) * g, g, &pipe.bar[phase ^ 1]);
     mbar_wait(&pipe.bar[phase], (k >> 1) & 1);
     TrackTile& T = pipe.tile[phase];
+    // A lane steps its track until it leaves the species buffer (interaction, stop, escape, ...) or has taken
+    // k_inner steps (kernels.cuh inner_steps); the warp goes round together because the navigator is
+    // warp-convergent.  The whole post-step state goes back into the lane's tile slot after every step.
+    bool live = false, has_ph = false;
+    int dest = -1;
+    bool cont = mine && tile * g + t < n;
+    if (counted + k_inner > 255) { move_counts_flush(tally, packed); counted = 0; }
+    for (int it = 0;; ++it) {
     const uint32_t vol = T.u[2][t];
-    const bool active = mine && tile * g + t < n && vol != kDeadVolume;
+    const bool active = cont && vol != kDeadVolume;
 
     // ---- phase A: step-start rules, physics step limit (A3), process choice (U1)
     int fate = FATE_NONE, process = 0, mat = 0;
@@ -202,53 +210,67 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
       if (cross) { px += c.eps_push * pdx; py += c.eps_push * pdy; pz += c.eps_push * pdz; }   // G5
     }
     // at-rest annihilation (P8): both photons carry m; below the gamma cut they are deposited (M5)
-    bool has_ph = false;
+    bool ph = false;
     if (ann_rest) {
       if (kMe < mat_scalar(c, mat, S_KCUT)) { edep_cut += kMe; edep_cut += kMe; }
-      else has_ph = true;
+      else ph = true;
     }
 
     // ---- relocation (A5), warp-convergent
     const int nv = nav_relocate<BVH>(c, c.navigator, cross, vol, px, py, pz, face);
 
-    // ---- outcome.  Everything still needed of the track is read from the tile here, before the
-    // reservation barriers: after them thread 0 may already refill this tile buffer.
-    Track post;
-    post.x = px; post.y = py; post.z = pz;
-    post.dx = T.d[3][t]; post.dy = T.d[4][t]; post.dz = T.d[5][t];
-    post.ekin = T.d[6][t]; post.id = T.id[t];
-    post.event = T.u[0][t]; post.step = T.u[1][t] + 1; post.vol = vol; post.species = species;
-    bool live = false;
-    int dest = -1;
+    // ---- outcome; position, step count and volume join the direction and energy in the tile slot
+    bool lv = false;
+    int dst = -1;
     if (active) {
+      uint32_t vol_post = vol;
       packed += 1ull << (8 * MC_STEPS);
       sum_dep += edep_dep; sum_cut += edep_cut;
       if (fate == FATE_KILLED) {
-        atomicAdd(&tally.ledger[3], carried_energy(species, post.ekin));
+        atomicAdd(&tally.ledger[3], carried_energy(species, T.d[6][t]));
         packed += 1ull << (8 * MC_KILLED);
       } else if (fate == FATE_STOPPED) {
         packed += 1ull << (8 * MC_STOPPED);
       } else if (cross) {
         if (nv < 0) {
+          Track post;
+          post.x = px; post.y = py; post.z = pz;
+          post.dx = T.d[3][t]; post.dy = T.d[4][t]; post.dz = T.d[5][t];
+          post.ekin = T.d[6][t]; post.id = T.id[t];
+          post.event = T.u[0][t]; post.step = T.u[1][t] + 1; post.vol = vol; post.species = species;
           atomicAdd(&tally.ledger[2], carried_energy(species, post.ekin));
           record_leak(c, slot, post, species);
           packed += 1ull << (8 * MC_ESCAPED);
         } else {
-          post.vol = static_cast<uint32_t>(nv);
-          live = true; dest = 0;
+          vol_post = static_cast<uint32_t>(nv);
+          lv = true; dst = 0;
           packed += 1ull << (8 * MC_BOUNDARY);
         }
       } else if (flag == 2) {
-        live = true; dest = 0;
+        lv = true; dst = 0;
         packed += 1ull << (8 * MC_TRUNCATED);
       } else if (!lim_disc) {
-        live = true; dest = 0;
+        lv = true; dst = 0;
         packed += 1ull << (8 * MC_LOSS);
       } else {
-        live = true; dest = 1 + stage_queue(process, species) - q0;
+        lv = true; dst = 1 + stage_queue(process, species) - q0;
       }
+      T.d[0][t] = px; T.d[1][t] = py; T.d[2][t] = pz;
+      T.u[1][t] += 1; T.u[2][t] = vol_post;
+      live = lv; dest = dst; has_ph = ph;
     }
     score(slot, vol, edep_dep + edep_cut, active);
+    cont = active && lv && dst == 0 && it + 1 < k_inner;
+    if (!__any_sync(kFull, cont)) break;
+    }   // steps of this lane's track
+    counted += k_inner;
+    // Everything still needed of the track is read from the tile here, before the reservation barriers:
+    // after them thread 0 may already refill this tile buffer.
+    Track post;
+    post.x = T.d[0][t]; post.y = T.d[1][t]; post.z = T.d[2][t];
+    post.dx = T.d[3][t]; post.dy = T.d[4][t]; post.dz = T.d[5][t];
+    post.ekin = T.d[6][t]; post.id = T.id[t];
+    post.event = T.u[0][t]; post.step = T.u[1][t]; post.vol = T.u[2][t]; post.species = species;
     fence_proxy_async_smem();
 
     // ---- reservation and stores (A0)
@@ -296,7 +318,6 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
         cnt->overflow.v = 1;
       }
     }
-    if (k % 255u == 254u) move_counts_flush(tally, packed);
   }
   move_counts_flush(tally, packed);
   {

@@ -123,6 +123,9 @@ __device__ __forceinline__ Track tile_read(const TrackTile& t, int k, int specie
   return r;
 }
 
+// generic-proxy writes to a tile must be ordered before the TMA (async proxy) refill of the same buffer
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
 struct TilePipe {
   TrackTile tile[2];
   uint64_t bar[2];
@@ -175,6 +178,26 @@ __device__ __forceinline__ void block_reserve(BlockReserve<ND>& br, int phase, c
   block_reserve_commit<ND>(br, phase, counter_of);
 #pragma unroll
   for (int d = 0; d < ND; ++d) first[d] = br.wbase[phase][warp][d] + pre[d];
+}
+
+// Steps a lane may take of its own track within one launch of a move kernel (adept_config::steps_per_launch).
+// Automatic choice: one while the species' population fills the lanes of the grid -- a lane that goes on
+// stepping leaves the finished lanes of its warp idle -- and more the emptier the GPU is: below a few
+// thousand tracks a population step is a chain of dependent launches whose cost does not depend on the
+// population, and the tracks that outlive the shower by thousands of steps (e+- spiralling in vacuum, 16
+// chords per step) advance one step per launch triple (PAPER.md:91-99 names these idle gaps).  Random
+// numbers are keyed by (event, track, step), so the result does not depend on the choice.
+#ifndef ADEPT_INNER_MAX
+#define ADEPT_INNER_MAX 32
+#endif
+__device__ __forceinline__ int inner_steps(const DevCtx& c, uint32_t n, uint32_t lanes) {
+  if (c.steps_per_launch > 0) return c.steps_per_launch;
+  if (n >= lanes) return 1;
+  if (n >= lanes / 4) return 2;
+  if (n >= lanes / 16) return 4;
+  if (n >= lanes / 64) return 8;
+  if (n >= lanes / 256) return 16;
+  return ADEPT_INNER_MAX;
 }
 
 // A9: scoring.  Every depositing lane issues one fp64 reduction (RED.ADD.F64, no return value, so the
@@ -310,11 +333,15 @@ __device__ __forceinline__ void move_counts_flush(BlockTally& t, unsigned long l
 // End of one population step: the just-consumed buffers become the next step's output buffers.  Run by
 // the last block of the interaction kernel to finish (ticket counter), so a population step is three
 // launches; every other block has completed its appends (they precede its ticket) when this runs.
-__device__ __forceinline__ void finish_iteration(const DevSlot& slot, int parity) {
+__device__ __forceinline__ void finish_iteration(const DevCtx& c, const DevSlot& slot, int parity) {
   SlotCounters* cnt = slot.counters;
   const int k = threadIdx.x;
   uint32_t before = 0, live = 0, in_sp[3];
-  for (int sp = 0; sp < 3; ++sp) { in_sp[sp] = __ldcg(&cnt->count[parity][sp].v); before += in_sp[sp]; live += __ldcg(&cnt->count[parity ^ 1][sp].v); }
+  for (int sp = 0; sp < 3; ++sp) {   // a counter can run past the capacity when its queue overflowed (the stores are guarded)
+    in_sp[sp] = min(__ldcg(&cnt->count[parity][sp].v), c.capacity);
+    before += in_sp[sp];
+    live += min(__ldcg(&cnt->count[parity ^ 1][sp].v), c.capacity);
+  }
   __syncthreads();
   if (k < 3) cnt->count[parity][k].v = 0;
   else if (k < 3 + kNumStage) cnt->n_stage[k - 3].v = 0;
@@ -354,7 +381,7 @@ interact_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlo
   if (blockIdx.x >= total) {   // no tile for this block (tail of a shower: most blocks); it only takes its ticket
     if (threadIdx.x == 0) is_last = atomicAdd(&cnt->ticket.v, 1u) == gridDim.x - 1;
     __syncthreads();
-    if (is_last) finish_iteration(slot, parity);
+    if (is_last) finish_iteration(c, slot, parity);
     return;
   }
   if (threadIdx.x == 0) {
@@ -456,7 +483,7 @@ interact_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlo
     is_last = atomicAdd(&cnt->ticket.v, 1u) == gridDim.x - 1;
   }
   __syncthreads();
-  if (is_last) finish_iteration(slot, parity);
+  if (is_last) finish_iteration(c, slot, parity);
 }
 
 // Places primaries (G5: volume = Locate(p + eps d)).  pending == nullptr: appends them to the parity-0
@@ -520,6 +547,37 @@ __global__ void __launch_bounds__(kBlock) inject_kernel(const __grid_constant__ 
         store_track(slot.buf[parity][d], j, t);
       }
     }
+  }
+}
+
+// Test hook adept_step_population: scatters tracks, taken as given (volume, step, id), into the parity-0
+// buffers of an empty slot; their carried energy is the ledger's "primary".
+__global__ void __launch_bounds__(kBlock) load_tracks_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot,
+                                                             const adept_track* __restrict__ in, int n) {
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    const adept_track p = in[i];
+    const uint32_t j = atomicAdd(&slot.counters->count[0][p.species].v, 1u);
+    if (j >= c.capacity) { slot.counters->overflow.v = 1; continue; }
+    Track t;
+    t.x = p.pos[0]; t.y = p.pos[1]; t.z = p.pos[2]; t.dx = p.dir[0]; t.dy = p.dir[1]; t.dz = p.dir[2];
+    t.ekin = p.ekin; t.id = p.id; t.event = p.event; t.step = p.step; t.vol = p.volume; t.species = p.species;
+    store_track(slot.buf[0][p.species], j, t);
+    atomicAdd(slot.ledger + 4, carried_energy(p.species, p.ekin));
+    atomicAdd(&slot.counters->live.v, 1u);
+  }
+}
+
+// ... and copies the first n[sp] entries of the three buffers of `parity` to out, species after species.
+__global__ void __launch_bounds__(kBlock) gather_tracks_kernel(const __grid_constant__ DevSlot slot, int parity, uint32_t n0, uint32_t n1,
+                                                               uint32_t n2, adept_track* __restrict__ out) {
+  const uint32_t total = n0 + n1 + n2;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < total; i += gridDim.x * blockDim.x) {
+    const int sp = i < n0 ? 0 : (i < n0 + n1 ? 1 : 2);
+    const uint32_t j = i - (sp == 0 ? 0u : (sp == 1 ? n0 : n0 + n1));
+    const Track t = load_track(slot.buf[parity][sp], j, sp);
+    adept_track& o = out[i];
+    o.pos[0] = t.x; o.pos[1] = t.y; o.pos[2] = t.z; o.dir[0] = t.dx; o.dir[1] = t.dy; o.dir[2] = t.dz;
+    o.ekin = t.ekin; o.id = t.id; o.event = t.event; o.step = t.step; o.volume = t.vol; o.species = sp;
   }
 }
 

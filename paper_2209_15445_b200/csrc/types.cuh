@@ -129,6 +129,7 @@ struct DevCtx {
   double delta_chord, eps_push, alpha_R, rho_R;
   int32_t chord_budget;
   uint32_t seed, max_steps;
+  int32_t steps_per_launch; // adept_config::steps_per_launch (0 = automatic, kernels.cuh inner_steps)
   uint32_t capacity;        // per species per buffer
   uint32_t stage_capacity;  // per interaction queue
   uint32_t leak_capacity;

@@ -41,7 +41,7 @@ def test_binding_structs_match_the_header_layout():
         sizes = [int(x) for x in subprocess.check_output([os.path.join(tmp, "sz")]).split()]
     assert sizes == [C.sizeof(adept.CConfig), C.sizeof(adept.CStats), C.sizeof(adept.CLedger), adept.TRACK.itemsize,
                      adept.RESULT.itemsize, C.sizeof(adept.CGeometry), C.sizeof(adept.CField)]
-    assert C.sizeof(adept.CConfig) == 112 and C.sizeof(adept.CStats) == 184 and C.sizeof(adept.CLedger) == 40
+    assert C.sizeof(adept.CConfig) == 120 and C.sizeof(adept.CStats) == 184 and C.sizeof(adept.CLedger) == 40
     assert adept.TRACK.itemsize == 80 and adept.RESULT.itemsize == 136
     cfg = adept.default_config()
     assert cfg.delta_chord == 1e-3 and cfg.eps_push == 1e-7 and cfg.chord_budget == 16 and cfg.navigator == adept.NAV_BVH

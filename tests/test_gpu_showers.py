@@ -202,53 +202,94 @@ def test_empty_and_error_paths(ob, calo):
         a.enqueue(p)
     assert ei.value.code == adept.EINVAL
     a.close()
-    # queue overflow is reported, not silently dropped
-    a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=64)
-    a.enqueue(primaries.beam(8, 10000.0))
+    # a slot listed twice is refused and leaves nothing marked live
+    a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=1 << 14, n_event_slots=2)
+    s = torch.cuda.current_stream()
     with pytest.raises(adept.AdeptError) as ei:
-        a.transport(0, torch.cuda.current_stream())
-    assert ei.value.code == adept.EOVERFLOW
+        a.transport_many([0, 1, 0], [s, s, s])
+    assert ei.value.code == adept.EINVAL
+    a.enqueue(primaries.beam(2, 50.0))                      # ESTATE if a slot had stayed live
+    a.transport_many([0, 1], [s, torch.cuda.Stream()])
+    assert a.read_scoring(0)[1].primary == 100.0
     a.close()
-    # workspace too small
-    cfg = adept.default_config()
-    ctx = C.c_void_p()
-    ws = torch.empty(1024, dtype=torch.uint8, device="cuda")
-    b = adept.Adept.__new__(adept.Adept)          # build the C structs through a normal context
+    # workspace too small: adept_init refuses it
     a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=64)
     assert a.workspace_bytes > 1024
+    with pytest.raises(adept.AdeptError) as ei:
+        adept.Adept(g, tabs, scal, field.no_field(), track_capacity=64, _workspace_bytes=a.workspace_bytes - 256)
+    assert ei.value.code == adept.ENOMEM
     a.close()
+
+
+def test_queue_overflow_is_reported_and_the_slot_stays_usable(ob, calo):
+    """ADEPT_EOVERFLOW instead of out-of-range reads: a batch that overflows the track buffers by far more than a
+    tile, with the host looking only every 16 population steps; the CUDA context survives, the slot is reset,
+    and a batch that fits then gives the oracle's result.  Same for a staging queue that is too small."""
+    import torch
+    from paper_2209_15445_b200 import adept
+    from paper_2209_15445_b200.inputs import field, primaries
+    g, _, tabs, scal = calo
+    small = primaries.beam(4, 200.0, spread=1.0)
+    o = ob.Oracle(g, tabs, scal, field.no_field())
+    oe, ol, ost = o.run(o.make_tracks(small))
+    for cfg in (dict(track_capacity=4096), dict(track_capacity=1 << 16, stage_capacity=64)):
+        a = adept.Adept(g, tabs, scal, field.no_field(), sync_interval=16, **cfg)
+        for rep in range(2):
+            a.enqueue(primaries.beam(64, 10000.0, spread=1.0))        # peaks at ~3e4 live tracks
+            with pytest.raises(adept.AdeptError) as ei:
+                a.transport(0, torch.cuda.current_stream())
+            assert ei.value.code == adept.EOVERFLOW
+            torch.cuda.synchronize()                                  # no sticky CUDA error
+            a.enqueue(small)
+            a.transport(0, torch.cuda.current_stream())
+            e, led = a.read_scoring(0)
+            assert led.primary == 800.0 and abs(led.total() - led.primary) <= 1e-9 * led.primary
+            np.testing.assert_allclose(e, oe, rtol=1e-9, atol=1e-9)
+        a.reset_slot(0)
+        assert a.read_scoring(0)[0].sum() == 0.0
+        a.close()
 
 
 def test_full_size_config2_properties(ob, calo):
     """Config 2 at the size and launch configuration bench.py times (10 000 x 10 GeV): properties that hold at
-    any size (ledger, conservation) plus the per-layer means against an oracle sample of the same events."""
+    any size (ledger, conservation), and -- random streams being keyed by (event, track, step) -- the first 48
+    events transported again in a second slot of the same context must equal the oracle's exactly: every step,
+    outcome and secondary counter, deposits to 1e-9."""
     import torch
     from paper_2209_15445_b200 import adept
     from paper_2209_15445_b200.inputs import field, primaries
     g, _, tabs, scal = calo
     n = 10000
     prim = primaries.beam(n, 10000.0, spread=1.0)
-    a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=1024 * n, sync_interval=8, time_kernels=1)
+    a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=1024 * n, n_event_slots=2, time_kernels=1)
+    a.set_kernel_timing(False)
     a.enqueue(prim)
     a.transport(0, torch.cuda.current_stream())
     e, led = a.read_scoring(0)
     st = a.stats(0)
-    a.close()
     assert led.primary == n * 10000.0
     assert abs(led.total() - led.primary) <= 1e-9 * led.primary
     assert e[:52].sum() == 0 and np.all(e >= 0)
     assert sum(st.outcomes) == sum(st.steps) and st.outcomes[11] == 0
-    # oracle on the first 48 events: the GPU mean over 10 000 must agree within the sample's statistical error
+    # the oracle on the first 48 events
     o = ob.Oracle(g, tabs, scal, field.no_field())
-    tr = o.make_tracks({k: v[:48] for k, v in prim.items()})
-    o_ev, _ = _oracle_events(o, tr, g.n_volumes)
+    first = {k: v[:48] for k, v in prim.items()}
+    oe, ol, ost = o.run(o.make_tracks(first))
+    a.enqueue(first, slot=1)
+    a.transport(1, torch.cuda.current_stream())
+    e1, led1 = a.read_scoring(1)
+    st1 = a.stats(1)
+    a.close()
+    assert list(st1.steps) == list(ost.steps) and list(st1.outcomes) == list(ost.outcomes)
+    assert list(st1.secondaries) == list(ost.secondaries)
+    np.testing.assert_allclose(e1, oe, rtol=1e-9, atol=1e-9)
+    assert led1.escaped == pytest.approx(ol.escaped, rel=1e-9)
+    # and the 10 000-event means agree with that sample within its statistical error
+    o_ev, _ = _oracle_events(o, o.make_tracks(first), g.n_volumes)
     o_mean, o_err = layer_stats(o_ev)
     gpu_mean = e[52:152].reshape(50, 2).sum(axis=1) / n
     tol = np.maximum(0.005 * o_mean, 3.5 * o_err * np.sqrt(1 + 48 / n))
     assert np.all(np.abs(gpu_mean - o_mean) <= tol)
-    # steps per shower agree with the oracle sample to a few per cent
-    o_steps = 0
-    _, _, ost = o.run(tr)
     assert sum(st.steps) / n == pytest.approx(sum(ost.steps) / 48, rel=0.08)
 
 
