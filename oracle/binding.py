@@ -25,7 +25,7 @@ class Geometry(C.Structure):
 
 
 class Materials(C.Structure):
-    _fields_ = [("n_mat", C.c_int32), ("tables", _dp), ("scalars", _dp)]
+    _fields_ = [("n_mat", C.c_int32), ("tables", _dp), ("scalars", _dp), ("n_elem", _ip), ("elem_bk", _dp), ("pe_cum", _dp)]
 
 
 class Field(C.Structure):
@@ -80,6 +80,7 @@ def _lib():
         "orc_set_recorder": (None, [vp, u32, u32, vp, C.c_size_t]),
         "orc_recorded": (C.c_size_t, [vp]),
         "orc_build_material": (None, [d, d, d, vp, vp]),
+        "orc_build_compound": (None, [i32, vp, vp, vp, d, vp, vp, vp, vp]),
         "orc_sigma_compton": (d, [d]), "orc_pair_shape": (d, [d]), "orc_sigma_photo": (d, [d, d]),
         "orc_brem_shape": (d, [d, d]), "orc_srad_shape": (d, [d, d]), "orc_sigma_moller": (d, [d, d]),
         "orc_sigma_bhabha": (d, [d, d]), "orc_sigma_annihilation": (d, [d]),
@@ -106,14 +107,23 @@ class Oracle:
     """One oracle context: geometry + materials + field + config, copied at construction."""
 
     def __init__(self, geom, tables, scalars, field, delta_chord=1e-3, eps_push=1e-7, alpha_R=0.2, rho_R=0.1,
-                 chord_budget=16, seed=1, max_steps=1000000):
+                 chord_budget=16, seed=1, max_steps=1000000, elements=None):
+        """elements: None (single-element materials) or (n_elem[n_mat], elem_bk[n_mat,4], pe_cum[n_mat,2048,4])."""
         g = Geometry(geom.n_volumes, geom.solid.ctypes.data_as(_ip), geom.dims.ctypes.data_as(_dp),
                      geom.material.ctypes.data_as(_ip), geom.mother.ctypes.data_as(_ip),
                      geom.daughter_begin.ctypes.data_as(_ip), geom.daughter_count.ctypes.data_as(_ip),
                      geom.rot.ctypes.data_as(_dp), geom.trans.ctypes.data_as(_dp))
         tables = np.ascontiguousarray(tables, dtype=np.float64)
         scalars = np.ascontiguousarray(scalars, dtype=np.float64)
-        m = Materials(tables.shape[0], tables.ctypes.data_as(_dp), scalars.ctypes.data_as(_dp))
+        if elements is None:
+            m = Materials(tables.shape[0], tables.ctypes.data_as(_dp), scalars.ctypes.data_as(_dp), None, None, None)
+        else:
+            ne = np.ascontiguousarray(elements[0], dtype=np.int32)
+            bk = np.ascontiguousarray(elements[1], dtype=np.float64)
+            cum = np.ascontiguousarray(elements[2], dtype=np.float64)
+            assert ne.shape == (tables.shape[0],) and bk.shape == (tables.shape[0], 4) and cum.shape == (tables.shape[0], 2048, 4)
+            m = Materials(tables.shape[0], tables.ctypes.data_as(_dp), scalars.ctypes.data_as(_dp), ne.ctypes.data_as(_ip),
+                          bk.ctypes.data_as(_dp), cum.ctypes.data_as(_dp))
         bz = np.ascontiguousarray(field.bz, dtype=np.float64)
         f = Field(field.kind, (C.c_double * 3)(*field.B), field.nr, field.nz, field.r0, field.z0, field.dr,
                   field.dz, bz.ctypes.data_as(_dp))
@@ -220,3 +230,11 @@ def build_material(Z, A, rho):
     scal = np.zeros(8)
     lib.orc_build_material(Z, A, rho, _p(tab), _p(scal))
     return tab, scal
+
+
+def build_compound(Z, A, nu, rho):
+    """-> (tables[12,2048], scalars[8], elem_bk[4], pe_cum[2048,4]) of a compound with nu[i] atoms of (Z[i], A[i])."""
+    Z, A, nu = (np.ascontiguousarray(x, dtype=np.float64) for x in (Z, A, nu))
+    tab, scal, bk, cum = np.zeros((12, 2048)), np.zeros(8), np.zeros(4), np.zeros((2048, 4))
+    lib.orc_build_compound(len(Z), _p(Z), _p(A), _p(nu), rho, _p(tab), _p(scal), _p(bk), _p(cum))
+    return tab, scal, bk, cum

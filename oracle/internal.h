@@ -43,6 +43,9 @@ struct orc_ctx {
   int n_mat = 0;
   std::vector<double> tables;   /* [n_mat][12][2048] */
   std::vector<double> scalars;  /* [n_mat][8] */
+  std::vector<int32_t> n_elem;  /* [n_mat]; empty = single elements only */
+  std::vector<double> elem_bk;  /* [n_mat][4] */
+  std::vector<double> pe_cum;   /* [n_mat][2048][4] */
   orc_field field{};
   std::vector<double> bz;
   orc_config cfg{};

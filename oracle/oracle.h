@@ -52,10 +52,16 @@ typedef struct {
   const double* trans;           /* [n_vol][3] global */
 } orc_geometry;
 
+#define ORC_MAX_ELEMENTS 4
 typedef struct {
   int32_t n_mat;
   const double* tables;  /* [n_mat][12][2048] */
   const double* scalars; /* [n_mat][8]: X0, T_c, k_c, B_K, n_el, vacuum flag, Z, rho */
+  /* Compound materials ("element selector"; DESIGN.md §3 C1-C5).  All three NULL
+     = every material is a single element.  The tables above already hold the sums over the elements. */
+  const int32_t* n_elem; /* [n_mat] number of elements, 1..ORC_MAX_ELEMENTS (vacuum: 1)                         */
+  const double* elem_bk; /* [n_mat][4] K-shell binding energy of each element [MeV]                            */
+  const double* pe_cum;  /* [n_mat][2048][4] cumulative share of elements 0..j in Sigma_photo on the ln T grid */
 } orc_materials;
 
 typedef struct {
@@ -169,6 +175,10 @@ size_t orc_recorded(const orc_ctx*);
 
 /* M1-M6: the oracle's own table builder (long double). tables [12][2048], scalars [8]. */
 void orc_build_material(double Z, double A, double rho, double* tables, double* scalars);
+/* C1-C5: the same for a compound of n <= ORC_MAX_ELEMENTS elements with nu[i] atoms of (Z[i], A[i]) per formula
+   unit; also fills elem_bk[4] and pe_cum[2048][4] (scalars: Z = n_el / n_at, B_K = that of element 0). */
+void orc_build_compound(int n, const double* Z, const double* A, const double* nu, double rho, double* tables,
+                        double* scalars, double* elem_bk, double* pe_cum);
 /* the individual closed forms behind the tables (P1-P8), for the pins */
 double orc_sigma_compton(double k);               /* per electron [cm^2] */
 double orc_pair_shape(double k);                  /* X0 * Sigma_pair     */

@@ -143,10 +143,34 @@ void pair(Final& f, Stream& u) {
   f.out->alive = 0;
 }
 
-/* P3 photoelectric, K shell */
+/* C5 element selector: in a compound the target element of a photoelectric absorption is element j
+   with probability n_j sigma_j(k) / Sigma_photo(k).  The cumulative shares are tabulated on the ln T grid and
+   interpolated like every table (M7); the choice uses U6 of the step's stream (a spare slot of R3): the first
+   j with U6 < c_j(k), else the last element.  Single-element materials draw nothing. */
+int select_element(const orc_ctx* c, int material, const orc_track* parent, double k) {
+  if (c->n_elem.empty() || c->n_elem[material] <= 1) return 0;
+  const int n = c->n_elem[material];
+  const double x = (std::log(k) - c->u0) / c->du;
+  int i = static_cast<int>(std::floor(x));
+  i = std::min(std::max(i, 0), kNGrid - 2);
+  const double fr = x - i;
+  const double* row0 = c->pe_cum.data() + (static_cast<size_t>(material) * kNGrid + i) * ORC_MAX_ELEMENTS;
+  const double* row1 = row0 + ORC_MAX_ELEMENTS;
+  const double u6 = orc_uniform(parent->event, c->cfg.seed, parent->id, parent->step, 6);
+  for (int j = 0; j < n - 1; ++j) {
+    const double cj = row0[j] + fr * (row1[j] - row0[j]);
+    if (u6 < cj) return j;
+  }
+  return n - 1;
+}
+
+/* P3 photoelectric, K shell (of the selected element in a compound) */
 void photo(Final& f, Stream&) {
   orc_track& g = f.out->post;
-  const double k = g.ekin, BK = scalar(f.c, f.material, S_BK);
+  const double k = g.ekin;
+  const int el = select_element(f.c, f.material, f.parent, k);
+  const double BK = f.c->n_elem.empty() ? scalar(f.c, f.material, S_BK)
+                                        : f.c->elem_bk[static_cast<size_t>(f.material) * ORC_MAX_ELEMENTS + el];
   if (k > BK) {
     f.out->edep_cut += BK;
     f.emit(ORC_ELECTRON, g.dir, k - BK, 0);

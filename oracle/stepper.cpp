@@ -37,6 +37,11 @@ extern "C" orc_ctx* orc_create(const orc_geometry* g, const orc_materials* m, co
   c->n_mat = m->n_mat;
   c->tables.assign(m->tables, m->tables + static_cast<size_t>(m->n_mat) * N_TAB * kNGrid);
   c->scalars.assign(m->scalars, m->scalars + static_cast<size_t>(m->n_mat) * N_SCAL);
+  if (m->n_elem && m->elem_bk && m->pe_cum) {
+    c->n_elem.assign(m->n_elem, m->n_elem + m->n_mat);
+    c->elem_bk.assign(m->elem_bk, m->elem_bk + static_cast<size_t>(m->n_mat) * ORC_MAX_ELEMENTS);
+    c->pe_cum.assign(m->pe_cum, m->pe_cum + static_cast<size_t>(m->n_mat) * kNGrid * ORC_MAX_ELEMENTS);
+  }
   c->field = *f;
   if (f->kind == ORC_FIELD_MAP_RZ) c->bz.assign(f->bz, f->bz + static_cast<size_t>(f->nr) * f->nz);
   c->field.bz = nullptr;

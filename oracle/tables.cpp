@@ -18,25 +18,55 @@ typedef long double ld;
 const ld M = 0.51099895L, RE = 2.8179403262e-13L, ALPHA = 1.0L / 137.035999084L, NA = 6.02214076e23L;
 const ld PI = 3.141592653589793238462643383279502884L;
 
+/* A material: one element (M1-M3) or a compound of up to 4 (C1-C3):
+   C1  nu_i atoms of element i per formula unit, molar mass A_mol = sum nu_i A_i; number densities
+       n_i = N_A rho nu_i / A_mol, n_at = sum n_i, n_el = sum n_i Z_i;
+   C2  1/X0 = sum_i 4 alpha r_e^2 n_i [Z_i^2 (L_rad,i - f_c,i) + Z_i L'_rad,i]   (Tsai, additive in the atoms);
+   C3  ln I = sum_i n_i Z_i ln I_i / n_el  (Bragg additivity of the stopping number), plasma energy from the
+       total electron density: hbar omega_p = 28.816 eV sqrt(rho sum nu_i Z_i / A_mol). */
 struct Mat {
-  ld Z, A, rho, n_at, n_el, X0, I, hwp, BK;
+  int n;
+  ld Z[4], A[4], n_i[4], BKi[4];
+  ld rho, n_at, n_el, X0, I, hwp, BK;
 };
 
-Mat make(ld Z, ld A, ld rho) {
-  Mat m{};
-  m.Z = Z; m.A = A; m.rho = rho;
-  m.n_at = NA * rho / A;
-  m.n_el = Z * m.n_at;
+ld tsai_per_atom(ld Z) { /* Z^2 (L_rad - f_c) + Z L'_rad */
   const ld a = ALPHA * Z, a2 = a * a;
   const ld fc = a2 * (1.0L / (1.0L + a2) + 0.20206L - 0.0369L * a2 + 0.0083L * a2 * a2 - 0.002L * a2 * a2 * a2);
   const ld lrad = logl(184.15L * powl(Z, -1.0L / 3.0L));
   const ld lprad = logl(1194.0L * powl(Z, -2.0L / 3.0L));
-  m.X0 = 1.0L / (4.0L * ALPHA * RE * RE * m.n_at * (Z * Z * (lrad - fc) + Z * lprad)); /* M2 Tsai */
-  const ld i_ev = Z < 13.0L ? Z * (12.0L + 7.0L / Z) : Z * (9.76L + 58.8L * powl(Z, -1.19L));  /* M3 */
-  m.I = i_ev * 1.0e-6L;
-  m.hwp = 28.816e-6L * sqrtl(rho * Z / A);
-  m.BK = 13.605693e-6L * (Z - 1.0L) * (Z - 1.0L); /* P3 */
+  return Z * Z * (lrad - fc) + Z * lprad;
+}
+ld mean_excitation(ld Z) { /* M3, MeV */
+  const ld i_ev = Z < 13.0L ? Z * (12.0L + 7.0L / Z) : Z * (9.76L + 58.8L * powl(Z, -1.19L));
+  return i_ev * 1.0e-6L;
+}
+
+Mat make_compound(int n, const ld* Z, const ld* A, const ld* nu, ld rho) {
+  Mat m{};
+  m.n = n; m.rho = rho;
+  ld a_mol = 0.0L, z_mol = 0.0L;
+  for (int i = 0; i < n; ++i) { a_mol += nu[i] * A[i]; z_mol += nu[i] * Z[i]; }
+  ld inv_x0 = 0.0L, lnI = 0.0L;
+  for (int i = 0; i < n; ++i) {
+    m.Z[i] = Z[i]; m.A[i] = A[i];
+    m.n_i[i] = NA * rho * nu[i] / a_mol;
+    m.n_at += m.n_i[i];
+    m.n_el += m.n_i[i] * Z[i];
+    inv_x0 += 4.0L * ALPHA * RE * RE * m.n_i[i] * tsai_per_atom(Z[i]);
+    lnI += m.n_i[i] * Z[i] * logl(mean_excitation(Z[i]));
+    m.BKi[i] = 13.605693e-6L * (Z[i] - 1.0L) * (Z[i] - 1.0L); /* P3 */
+  }
+  m.X0 = 1.0L / inv_x0;
+  m.I = n == 1 ? mean_excitation(Z[0]) : expl(lnI / m.n_el);
+  m.hwp = 28.816e-6L * sqrtl(rho * z_mol / a_mol);
+  m.BK = m.BKi[0];
   return m;
+}
+
+Mat make(ld Z, ld A, ld rho) {
+  const ld one = 1.0L;
+  return make_compound(1, &Z, &A, &one, rho);
 }
 
 /* P1: Klein-Nishina per electron */
@@ -63,6 +93,13 @@ ld pair_shape(ld k) {
 ld sigma_pe(ld k, ld Z) {
   const ld st = 8.0L * PI * RE * RE / 3.0L;
   return 1.25L * 4.0L * sqrtl(2.0L) * powl(ALPHA, 4) * powl(Z, 5) * st * powl(M / k, 3.5L);
+}
+
+/* macroscopic photoelectric cross section: sum over the elements */
+ld Sigma_pe(const Mat& m, ld k) {
+  ld s = 0.0L;
+  for (int i = 0; i < m.n; ++i) s += m.n_i[i] * sigma_pe(k, m.Z[i]);
+  return s;
 }
 
 /* P4: X0 * Sigma_brem and X0 * S_rad */
@@ -138,18 +175,51 @@ extern "C" double orc_s_coll(double T, double Z, double A, double rho, double Tc
   return static_cast<double>(s_coll(T, make(Z, A, rho), Tc, positron != 0));
 }
 
+namespace {
+void build(const Mat* mp, double Zd, double rhod, double* tables, double* scalars);
+}
+
 extern "C" void orc_build_material(double Zd, double Ad, double rhod, double* tables, double* scalars) {
+  if (!(rhod > 0.0)) { build(nullptr, Zd, rhod, tables, scalars); return; }
+  const Mat m = make(Zd, Ad, rhod);
+  build(&m, Zd, rhod, tables, scalars);
+}
+
+/* C1-C5: compound of n elements; elem_bk[4], pe_cum[2048][4] = cumulative share of elements 0..j in Sigma_photo
+   at every grid node (the last used entry is 1; unused entries are 1 as well). */
+extern "C" void orc_build_compound(int n, const double* Z, const double* A, const double* nu, double rho, double* tables,
+                                   double* scalars, double* elem_bk, double* pe_cum) {
+  using namespace orc;
+  ld Zl[4], Al[4], nl[4];
+  for (int i = 0; i < n; ++i) { Zl[i] = Z[i]; Al[i] = A[i]; nl[i] = nu[i]; }
+  const Mat m = make_compound(n, Zl, Al, nl, rho);
+  build(&m, static_cast<double>(m.n_el / m.n_at), rho, tables, scalars);
+  for (int j = 0; j < 4; ++j) elem_bk[j] = j < n ? static_cast<double>(m.BKi[j]) : 0.0;
+  const ld u0 = logl(1.0e-3L), du = (logl(1.0e8L) - logl(1.0e-3L)) / (kNGrid - 1);
+  for (int i = 0; i < kNGrid; ++i) {
+    const ld k = expl(u0 + du * i);
+    const ld tot = Sigma_pe(m, k);
+    ld acc = 0.0L;
+    for (int j = 0; j < 4; ++j) {
+      if (j < n) acc += m.n_i[j] * sigma_pe(k, m.Z[j]);
+      pe_cum[4 * i + j] = j < n - 1 ? static_cast<double>(acc / tot) : 1.0;
+    }
+  }
+}
+
+namespace {
+void build(const Mat* mp, double Zd, double rhod, double* tables, double* scalars) {
   using namespace orc;
   const int N = kNGrid;
   for (int i = 0; i < N_TAB * N; ++i) tables[i] = 0.0;
   for (int i = 0; i < N_SCAL; ++i) scalars[i] = 0.0;
   scalars[S_Z] = Zd; scalars[S_RHO] = rhod;
-  if (!(rhod > 0.0)) { /* M1 vacuum: all Sigma = 0, dE/dx = 0 */
+  if (!mp) { /* M1 vacuum: all Sigma = 0, dE/dx = 0 */
     for (int i = 0; i < N; ++i) tables[T_EM_RANGE * N + i] = tables[T_EP_RANGE * N + i] = 1.0e99;
     scalars[S_X0] = 1.0e99; scalars[S_VACUUM] = 1.0;
     return;
   }
-  const Mat m = make(Zd, Ad, rhod);
+  const Mat& m = *mp;
   const ld u0 = logl(1.0e-3L), du = (logl(1.0e8L) - logl(1.0e-3L)) / (N - 1);
   std::vector<ld> T(N), f(N), R(N), sig(N);
   for (int i = 0; i < N; ++i) T[i] = expl(u0 + du * i);
@@ -169,7 +239,7 @@ extern "C" void orc_build_material(double Zd, double Ad, double rhod, double* ta
     while (j + 1 < N - 1 && R[j + 1] <= cut) ++j;
     tc = expl(u0 + du * j + du * (cut - R[j]) / (R[j + 1] - R[j]));
   }
-  for (int i = 0; i < N; ++i) sig[i] = m.n_el * sigma_kn(T[i]) + pair_shape(T[i]) / m.X0 + m.n_at * sigma_pe(T[i], m.Z);
+  for (int i = 0; i < N; ++i) sig[i] = m.n_el * sigma_kn(T[i]) + pair_shape(T[i]) / m.X0 + Sigma_pe(m, T[i]);
   const ld target = 5.0L / cut;
   ld kc = 1.0e-3L;
   if (sig[0] > target) {
@@ -187,7 +257,7 @@ extern "C" void orc_build_material(double Zd, double Ad, double rhod, double* ta
   for (int i = 0; i < N; ++i) {
     tables[T_G_COMPTON * N + i] = static_cast<double>(m.n_el * sigma_kn(T[i]));
     tables[T_G_PAIR * N + i] = static_cast<double>(pair_shape(T[i]) / m.X0);
-    tables[T_G_PHOTO * N + i] = static_cast<double>(m.n_at * sigma_pe(T[i], m.Z));
+    tables[T_G_PHOTO * N + i] = static_cast<double>(Sigma_pe(m, T[i]));
     const ld br = brem_shape(T[i], kc) / m.X0, sr = srad_shape(T[i], kc) / m.X0;
     tables[T_EM_BREM * N + i] = tables[T_EP_BREM * N + i] = static_cast<double>(br);
     tables[T_EM_IONI * N + i] = static_cast<double>(m.n_el * sigma_moller(T[i], tc));
@@ -205,3 +275,4 @@ extern "C" void orc_build_material(double Zd, double Ad, double rhod, double* ta
   range(S);
   for (int i = 0; i < N; ++i) tables[T_EP_RANGE * N + i] = static_cast<double>(R[i]);
 }
+}  // namespace

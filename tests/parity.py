@@ -117,9 +117,13 @@ def compare_population(pre, out, ores, osec, x0=None, b_max=0.0, dedx=None):
     order).  Tracks are matched by (event, id, step): a survivor of (e, i, s) is (e, i, s + 1), a secondary
     carries the child id the oracle derives from its parent's stream and step 0.  Discrete results -- which
     tracks exist, their species and volume -- must be identical; positions, directions and energies agree to
-    1e-12 of the scale of what enters them, with the same first-order propagation of the observed path
-    difference as compare_steps (|ds| is taken from the positions: a track's end point is its start plus s
-    times a unit vector).  Returns ds per pre-step state (for the deposit tolerances) and the worst errors."""
+    1e-12 of the scale of what enters them, with the same first-order propagation of the path difference as
+    compare_steps.  The population carries no path length, so |ds| is bounded from the positions: the observed
+    end-point difference (a track's end point is its start plus s times a unit vector) plus one unit in the last
+    place of the largest coordinate -- a distance to a boundary is a difference of coordinates of that size and
+    cannot be known better, whoever computes it (the steps of 1e-9 cm right after a boundary, at |x| ~ 150 cm,
+    have |ds| ~ 2e-15 cm = 0.1 ulp(x) and a Highland angle that moves by theta |ds| / (2 s) ~ 1e-9).
+    Returns ds per pre-step state (for the deposit tolerances) and the worst errors."""
     n = len(pre)
     exp_t, exp_parent, exp_kind = [], [], []
     alive = ores["alive"] == 1
@@ -146,6 +150,7 @@ def compare_population(pre, out, ores, osec, x0=None, b_max=0.0, dedx=None):
     dpos = np.linalg.norm(g["pos"] - e["pos"], axis=1)
     ds_pre = np.zeros(n)
     np.maximum.at(ds_pre, parent, dpos)
+    ds_pre += np.spacing(np.abs(pre["pos"]).max(axis=1))
     ds = ds_pre[parent]
     dir_slack = _msc_slack(p, ores[parent], ds, x0[parent]) if x0 is not None else np.zeros(len(e))
     if b_max > 0.0:

@@ -76,7 +76,7 @@ def check_population(a, o, g, scal, fld, pre, ores, osec, slot=0, dedx=None):
     assert not bad.any(), (np.where(bad)[0][:5], edep[bad][:5], want[bad][:5], tol_v[bad][:5])
     # ledger buckets
     tot = tol.sum() + 4e-16 * np.sqrt(len(pre)) * energy_scale(pre).sum()
-    assert led.primary == pytest.approx(energy_scale(pre).sum(), rel=1e-13)
+    assert led.primary == pytest.approx(energy_scale(pre).sum(), rel=1e-11)      # n fp64 atomics in any order
     for name in ("edep_dep", "edep_cut", "escaped", "killed"):
         got = {"edep_dep": led.deposited, "edep_cut": led.below_cut, "escaped": led.escaped, "killed": led.killed}[name]
         assert abs(got - ores[name].sum()) <= tot, (name, got, ores[name].sum())
