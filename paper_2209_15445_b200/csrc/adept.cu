@@ -238,10 +238,12 @@ struct SlotHost {
   unsigned long long launches = 0;
   bool live = false;
   size_t n_pending = 0, n_injected = 0;   // staggered injection: primaries in the pending store / already injected
-  // CUDA graph of one host round (sync_interval population steps), captured once on `cap` and replayed
+  size_t population = 0;                  // live tracks as last seen by the host (enqueue, end of a round)
+  // CUDA graphs of one host round (sync_interval population steps) with the lean [0] and the multi-step [1]
+  // move kernels, captured once on `cap` and replayed
   cudaStream_t cap = nullptr;
-  cudaGraphExec_t gexec = nullptr;
-  bool graph_failed = false;
+  cudaGraphExec_t gexec[2] = {nullptr, nullptr};
+  bool graph_failed[2] = {false, false};
   // optional per-launch timing (config.time_kernels)
   std::vector<cudaEvent_t> tev;      // [sync_interval][kTimed kernels][start, stop]
   int tev_used = 0;
@@ -259,16 +261,17 @@ struct adept_ctx {
   uint32_t* d_bad = nullptr;
   size_t stage_cap = 0;
   int grid_gamma = 0, grid_charged = 0, grid_inter = 0;
-  // move kernels specialised for this context's field kind and for geometries without BVH volumes
+  // move kernels specialised for this context's field kind and for geometries without BVH volumes; [1] = the
+  // variants in which a lane takes several steps of its own track per launch (small populations)
   using Kernel = void (*)(DevCtx, DevSlot, int);
-  Kernel k_move_gamma = nullptr, k_move_charged = nullptr;
+  Kernel k_move_gamma[2] = {nullptr, nullptr}, k_move_charged[2] = {nullptr, nullptr};
   bool timing_on = false;            // per-launch CUDA events active (adept_set_kernel_timing)
 };
 
 namespace {
 void destroy_ctx(adept_ctx* ctx) {
   for (SlotHost& sh : ctx->slots) {
-    if (sh.gexec) cudaGraphExecDestroy(sh.gexec);
+    for (cudaGraphExec_t ge : sh.gexec) if (ge) cudaGraphExecDestroy(ge);
     if (sh.cap) cudaStreamDestroy(sh.cap);
     if (sh.helper) cudaStreamDestroy(sh.helper);
     if (sh.fork) cudaEventDestroy(sh.fork);
@@ -522,7 +525,10 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   d.tab_g = L.tab_g; d.tab_em = L.tab_em; d.tab_ep = L.tab_ep; d.scal = L.scal; d.rhint = L.rhint; d.n_mat = n_mats;
   d.field_kind = f->kind;
   for (int k = 0; k < 3; ++k) d.B[k] = f->B[k];
+  d.Bn = std::sqrt(f->B[0] * f->B[0] + f->B[1] * f->B[1] + f->B[2] * f->B[2]);
+  for (int k = 0; k < 3; ++k) d.bhat[k] = d.Bn > 0.0 ? f->B[k] / d.Bn : 0.0;
   d.nr = f->nr; d.nz = f->nz; d.r0 = f->r0; d.z0 = f->z0; d.dr = f->dr; d.dz = f->dz; d.bz = L.bz;
+  d.inv_dr = f->dr > 0.0 ? 1.0 / f->dr : 0.0; d.inv_dz = f->dz > 0.0 ? 1.0 / f->dz : 0.0;
   d.u0 = std::log(1.0e-3);
   d.du = (std::log(1.0e8) - std::log(1.0e-3)) / (kNGrid - 1);
   d.inv_du = 1.0 / d.du;
@@ -543,18 +549,20 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->device));
   {
     const bool bvh = cfg->navigator == ADEPT_NAV_BVH && !hb.empty();
-    ctx->k_move_gamma = bvh ? gamma_move_kernel<true> : gamma_move_kernel<false>;
-#define ADEPT_CHARGED_KERNEL(F, B) charged_move_kernel<F, B>
+    ctx->k_move_gamma[0] = bvh ? gamma_move_kernel<true, false> : gamma_move_kernel<false, false>;
+    ctx->k_move_gamma[1] = bvh ? gamma_move_kernel<true, true> : gamma_move_kernel<false, true>;
+#define ADEPT_CHARGED_KERNELS(F)                                                                                   \
+  ctx->k_move_charged[0] = bvh ? charged_move_kernel<F, true, false> : charged_move_kernel<F, false, false>;        \
+  ctx->k_move_charged[1] = bvh ? charged_move_kernel<F, true, true> : charged_move_kernel<F, false, true>
     switch (f->kind) {
-      case ADEPT_FIELD_NONE:
-        ctx->k_move_charged = bvh ? ADEPT_CHARGED_KERNEL(ADEPT_FIELD_NONE, true) : ADEPT_CHARGED_KERNEL(ADEPT_FIELD_NONE, false); break;
-      case ADEPT_FIELD_UNIFORM:
-        ctx->k_move_charged = bvh ? ADEPT_CHARGED_KERNEL(ADEPT_FIELD_UNIFORM, true) : ADEPT_CHARGED_KERNEL(ADEPT_FIELD_UNIFORM, false); break;
-      default:
-        ctx->k_move_charged = bvh ? ADEPT_CHARGED_KERNEL(ADEPT_FIELD_MAP_RZ, true) : ADEPT_CHARGED_KERNEL(ADEPT_FIELD_MAP_RZ, false); break;
+      case ADEPT_FIELD_NONE: ADEPT_CHARGED_KERNELS(ADEPT_FIELD_NONE); break;
+      case ADEPT_FIELD_UNIFORM: ADEPT_CHARGED_KERNELS(ADEPT_FIELD_UNIFORM); break;
+      default: ADEPT_CHARGED_KERNELS(ADEPT_FIELD_MAP_RZ); break;
     }
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_g, ctx->k_move_gamma, kBlock, 0));
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_c, ctx->k_move_charged, kBlock, 0));
+#undef ADEPT_CHARGED_KERNELS
+    // one grid for both variants of a kernel (the lean one sets it: it is the one that fills the GPU)
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_g, ctx->k_move_gamma[0], kBlock, 0));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_c, ctx->k_move_charged[0], kBlock, 0));
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_i, interact_kernel, kBlock, 0));
   }
   ctx->grid_gamma = sms * std::max(occ_g, 1);
@@ -612,6 +620,7 @@ int reset_slot_async(adept_ctx* ctx, SlotHost& sh, cudaStream_t st) {
   CUDA_TRY(cudaMemsetAsync(sh.dev.ledger, 0, 8 * sizeof(double), st));
   CUDA_TRY(cudaMemsetAsync(sh.dev.trace_n, 0, sizeof(uint32_t), st));
   sh.n_pending = sh.n_injected = 0;
+  sh.population = 0;
   (void)ctx;
   return ADEPT_OK;
 }
@@ -663,7 +672,7 @@ extern "C" int adept_enqueue_batch(adept_ctx* ctx, int slot, int n, const uint32
     uint32_t bad = 0;
     CUDA_TRY(cudaMemcpy(&bad, ctx->d_bad, sizeof(uint32_t), cudaMemcpyDeviceToHost));
     if (bad) return fail(ADEPT_EINVAL, "%u primaries lie outside the world or have an unknown species", bad);
-    if (stagger) sh.n_pending += m;
+    if (stagger) sh.n_pending += m; else sh.population += m;
     done += m;
   }
   return ADEPT_OK;
@@ -683,7 +692,7 @@ namespace {
 // One population step of a slot: gamma move kernel on the caller's stream, charged move kernel on the
 // helper stream (species kernels on different streams, synchronised with events), then the
 // interaction kernel over what they staged and the buffer swap.
-int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity, const DevCtx& dc) {
+int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity, const DevCtx& dc, int multi) {
   constexpr int kEv = 2 * ADEPT_N_TIMED_KERNELS;
   if (sh.n_injected < sh.n_pending) {   // staggered injection: the next chunk joins the population of this step
     const size_t m = std::min<size_t>(ctx->cfg.inject_chunk, sh.n_pending - sh.n_injected);
@@ -702,10 +711,10 @@ int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity, 
   }
   cudaEvent_t* ev = timed ? &sh.tev[sh.tev_used] : nullptr;
   if (timed) CUDA_TRY(cudaEventRecord(ev[0], st));
-  ctx->k_move_gamma<<<dim3(ctx->grid_gamma, 1), kBlock, 0, st>>>(dc, sh.dev, parity);
+  ctx->k_move_gamma[multi]<<<dim3(ctx->grid_gamma, 1), kBlock, 0, st>>>(dc, sh.dev, parity);
   if (timed) CUDA_TRY(cudaEventRecord(ev[1], st));
   if (timed) CUDA_TRY(cudaEventRecord(ev[2], sc));
-  ctx->k_move_charged<<<dim3(ctx->grid_charged, 2), kBlock, 0, sc>>>(dc, sh.dev, parity);
+  ctx->k_move_charged[multi]<<<dim3(ctx->grid_charged, 2), kBlock, 0, sc>>>(dc, sh.dev, parity);
   if (timed) CUDA_TRY(cudaEventRecord(ev[3], sc));
   if (fork) {
     CUDA_TRY(cudaEventRecord(sh.join, sh.helper));
@@ -723,22 +732,30 @@ int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity, 
 // round.  A small event (config 5: 200 primaries, thousands of nearly empty population steps on each of 16
 // streams) is otherwise bound by the host issuing ~10 API calls per step.  Needs an even sync_interval (every
 // round then starts at parity 0), no per-launch timing and no pending injection; returns false to fall back.
-bool round_graph(adept_ctx* ctx, SlotHost& sh) {
-  if (sh.gexec) return true;
-  if (sh.graph_failed || !ctx->cfg.use_graphs || (ctx->cfg.sync_interval & 1)) return false;
-  if (!sh.cap && cudaStreamCreateWithFlags(&sh.cap, cudaStreamNonBlocking) != cudaSuccess) { sh.graph_failed = true; return false; }
+bool round_graph(adept_ctx* ctx, SlotHost& sh, int multi) {
+  if (sh.gexec[multi]) return true;
+  if (sh.graph_failed[multi] || !ctx->cfg.use_graphs || (ctx->cfg.sync_interval & 1)) return false;
+  if (!sh.cap && cudaStreamCreateWithFlags(&sh.cap, cudaStreamNonBlocking) != cudaSuccess) { sh.graph_failed[multi] = true; return false; }
   const unsigned long long launches = sh.launches;
   cudaGraph_t graph = nullptr;
   bool ok = cudaStreamBeginCapture(sh.cap, cudaStreamCaptureModeRelaxed) == cudaSuccess;
   if (ok) {
-    for (int it = 0; it < ctx->cfg.sync_interval && ok; ++it) ok = launch_iteration(ctx, sh, sh.cap, it & 1, ctx->dev) == ADEPT_OK;
+    for (int it = 0; it < ctx->cfg.sync_interval && ok; ++it) ok = launch_iteration(ctx, sh, sh.cap, it & 1, ctx->dev, multi) == ADEPT_OK;
     ok = (cudaStreamEndCapture(sh.cap, &graph) == cudaSuccess) && ok && graph;
   }
-  if (ok) ok = cudaGraphInstantiate(&sh.gexec, graph, 0) == cudaSuccess;
+  if (ok) ok = cudaGraphInstantiate(&sh.gexec[multi], graph, 0) == cudaSuccess;
   if (graph) cudaGraphDestroy(graph);
   sh.launches = launches;
-  if (!ok) { cudaGetLastError(); sh.gexec = nullptr; sh.graph_failed = true; }
+  if (!ok) { cudaGetLastError(); sh.gexec[multi] = nullptr; sh.graph_failed[multi] = true; }
   return ok;
+}
+
+// Which move kernels the next host round of a slot runs: the multi-step variants once the population the host
+// last saw no longer fills the GPU (their lanes go on stepping their own tracks, kernels.cuh inner_steps).
+// The showers do not depend on the choice; a stale population costs speed only.
+constexpr size_t kMultiBelow = 65536;
+int round_variant(const adept_ctx* ctx, const SlotHost& sh) {
+  return ctx->cfg.steps_per_launch != 1 && sh.population + (sh.n_pending - sh.n_injected) < kMultiBelow ? 1 : 0;
 }
 
 }  // namespace
@@ -766,10 +783,12 @@ extern "C" int adept_transport_many(adept_ctx* ctx, int n_slots, const int* slot
   while (n_live > 0) {
     // slots whose round is a graph: one launch each
     std::vector<char> graphed(n_slots, 0);
+    std::vector<int> variant(n_slots, 0);
     for (int k = 0; k < n_slots; ++k) {
       SlotHost& sh = ctx->slots[slots[k]];
-      if (!sh.live || parity[k] != 0 || ctx->timing_on || sh.n_injected < sh.n_pending || !round_graph(ctx, sh)) continue;
-      CUDA_TRY(cudaGraphLaunch(sh.gexec, static_cast<cudaStream_t>(streams[k])));
+      variant[k] = round_variant(ctx, sh);
+      if (!sh.live || parity[k] != 0 || ctx->timing_on || sh.n_injected < sh.n_pending || !round_graph(ctx, sh, variant[k])) continue;
+      CUDA_TRY(cudaGraphLaunch(sh.gexec[variant[k]], static_cast<cudaStream_t>(streams[k])));
       sh.launches += 3ull * ctx->cfg.sync_interval;
       graphed[k] = 1;
     }
@@ -777,7 +796,7 @@ extern "C" int adept_transport_many(adept_ctx* ctx, int n_slots, const int* slot
       for (int k = 0; k < n_slots; ++k) {
         SlotHost& sh = ctx->slots[slots[k]];
         if (!sh.live || graphed[k]) continue;
-        const int rc = launch_iteration(ctx, sh, static_cast<cudaStream_t>(streams[k]), parity[k], ctx->dev);
+        const int rc = launch_iteration(ctx, sh, static_cast<cudaStream_t>(streams[k]), parity[k], ctx->dev, variant[k]);
         if (rc != ADEPT_OK) return rc;
         parity[k] ^= 1;
       }
@@ -800,6 +819,7 @@ extern "C" int adept_transport_many(adept_ctx* ctx, int n_slots, const int* slot
         }
       sh.tev_used = 0;
       const bool overflow = sh.pinned->overflow.v != 0;
+      sh.population = sh.pinned->live.v;
       if (overflow) {
         // The pass is abandoned: the slot is emptied (tracks, staging queues, scoring, ledger, leaked tracks) so
         // that the caller can enqueue a smaller batch into it.
@@ -811,6 +831,7 @@ extern "C" int adept_transport_many(adept_ctx* ctx, int n_slots, const int* slot
       }
       if ((sh.pinned->live.v == 0 && sh.n_injected == sh.n_pending) || overflow) {
         sh.n_pending = sh.n_injected = 0;
+        sh.population = 0;
         sh.live = false;
         --n_live;
         // counts are all zero: the (empty) slot is at parity 0 for the next enqueue whatever parity[k] is
@@ -946,11 +967,15 @@ extern "C" int adept_step_population(adept_ctx* ctx, int slot, int n, const adep
   load_tracks_kernel<<<std::min((n + kBlock - 1) / kBlock, 4096), kBlock, 0, st>>>(ctx->dev, sh.dev, d_in, n);
   CUDA_TRY(cudaGetLastError());
   // exactly one population step: the kernels and grids of adept_transport, one step per track and launch
+  // (the variant of the move kernels adept_transport would pick for a population of n, held to one step per track)
   DevCtx one = ctx->dev;
   one.steps_per_launch = 1;
+  sh.population = static_cast<size_t>(n);
+  const int variant = round_variant(ctx, sh);
+  sh.population = 0;
   const bool timing = ctx->timing_on;
   ctx->timing_on = false;
-  const int rl = launch_iteration(ctx, sh, st, 0, one);
+  const int rl = launch_iteration(ctx, sh, st, 0, one, variant);
   ctx->timing_on = timing;
   if (rl != ADEPT_OK) return rl;
   CUDA_TRY(cudaMemcpyAsync(sh.pinned, sh.dev.counters, sizeof(SlotCounters), cudaMemcpyDeviceToHost, st));

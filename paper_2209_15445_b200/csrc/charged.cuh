@@ -10,6 +10,8 @@
 // lane's spill space and little is live across the two navigator phases (inlined: calls cost 4-20 %).
 // The discrete process is chosen (U1, same Philox block as U0) before the propagation; the MSC draws
 // (U2, U3) and the at-rest annihilation draws (U4, U5) are regenerated from the key where they are used.
+// As in gamma.cuh there is a lean instantiation (one step per track and launch) and MULTI = true, in which a
+// lane goes on stepping its own track while it stays in its species buffer (kernels.cuh inner_steps).
 #pragma once
 #include "kernels.cuh"
 
@@ -25,63 +27,26 @@ namespace adept {
 #define ADEPT_MINB_C2F 4
 #endif
 
-template <int FIELD, bool BVH>
-__global__ void __launch_bounds__(kBlock, FIELD == ADEPT_FIELD_NONE ? ADEPT_MINB_C2 : ADEPT_MINB_C2F)
-charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot, int parity) {
-  const int species = static_cast<int>(blockIdx.y);   // ADEPT_ELECTRON or ADEPT_POSITRON
-  const bool positron = species == ADEPT_POSITRON;
-  const TrackSoA& cur = slot.buf[parity][species];
-  SlotCounters* cnt = slot.counters;
-  // (a counter can run past the capacity when its queue overflowed: the stores are guarded, the reads clamped)
-  const uint32_t n = min(cnt->count[parity][species].v, c.capacity);
+// One e-/e+ step of the track in tile slot `t`; warp-convergent.  The post-step direction and energy are written
+// into the tile slot (MULTI: position, step count and volume as well, so that the slot is the pre-step state of
+// the lane's next step).  On return (px, py, pz, vol_post) complete the post-step state; `live` and `dest` say
+// where it goes (0 = next buffer of the species, 1.. = staging queue q0 + dest - 1), `has_ph` that two
+// annihilation photons start at the end point.
+struct ChargedLane {
+  double px, py, pz;
+  uint32_t vol_post;
+  bool live, has_ph;
+  int dest;
+};
 
-  // destinations: 0 = next buffer of the species, 1..3 = its staging queues, 4 = next gamma buffer (the
-  // photons of an annihilation at rest)
-  constexpr int ND = 5;
-  const int q0 = positron ? 5 : 3;
-  // Tracks per tile.  A population smaller than the grid's lanes is spread over all blocks and warps
-  // (g tracks per tile, one lane in every 128/g): the warp-cooperative BVH serves the queries of a warp
-  // one after the other, so a few hundred loopers packed into a few warps would take 32 x 16 chord queries
-  // in sequence per step (measured 4 ms per population step on config 4), spread out they run in parallel.
-  uint32_t g = kBlock;
-  while (g > 4 && (n + (g >> 1) - 1) / (g >> 1) <= gridDim.x) g >>= 1;
-  const int lane_shift = __ffs(kBlock / g) - 1;            // every (1 << lane_shift)-th lane takes a track
-  const uint32_t n_tiles = (n + g - 1) / g;
-  if (blockIdx.x >= n_tiles) return;   // no tile for this block
-  __shared__ BlockTally tally;
-  __shared__ BlockReserve<ND> br;
-  __shared__ TilePipe pipe;
-  tally_init(tally);
-  pipe_init(pipe);
-  double sum_dep = 0.0, sum_cut = 0.0;
-  unsigned chords_sum = 0;
-  unsigned long long packed = 0;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const unsigned lt = (1u << lane) - 1u;
-  const int t = threadIdx.x >> lane_shift;                 // this lane's entry of the tile
-  const bool mine = (threadIdx.x & ((1u << lane_shift) - 1u)) == 0;
-  const int k_inner = inner_steps(c, n, gridDim.x * kBlock);
-  int counted = 0;   // steps a lane may have added to each field of `packed` since the last flush
+template <int FIELD, bool BVH, bool MULTI>
+__device__ __forceinline__ void charged_lane(const DevCtx& c, const DevSlot& slot, BlockTally& tally, TrackTile& T, int t, bool in_range,
+                                             int species, int q0, unsigned long long& packed, double& sum_dep, double& sum_cut,
+                                             unsigned& chords_sum, ChargedLane& r) {
   enum { FATE_NONE = 0, FATE_KILLED, FATE_STOPPED, FATE_GO };
-
-  if (threadIdx.x == 0) tile_issue_n(pipe.tile[0], cur, static_cast<size_t>(blockIdx.x) * g, g, &pipe.bar[0]);
-  uint32_t k = 0;
-  for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++k) {
-    const int phase = k & 1;
-    if (threadIdx.x == 0 && tile + gridDim.x < n_tiles)
-      tile_issue_n(pipe.tile[phase ^ 1], cur, static_cast<size_t>(tile + gridDim.x) * g, g, &pipe.bar[phase ^ 1]);
-    mbar_wait(&pipe.bar[phase], (k >> 1) & 1);
-    TrackTile& T = pipe.tile[phase];
-    // A lane steps its track until it leaves the species buffer (interaction, stop, escape, ...) or has taken
-    // k_inner steps (kernels.cuh inner_steps); the warp goes round together because the navigator is
-    // warp-convergent.  The whole post-step state goes back into the lane's tile slot after every step.
-    bool live = false, has_ph = false;
-    int dest = -1;
-    bool cont = mine && tile * g + t < n;
-    if (counted + k_inner > 255) { move_counts_flush(tally, packed); counted = 0; }
-    for (int it = 0;; ++it) {
+  const bool positron = species == ADEPT_POSITRON;
     const uint32_t vol = T.u[2][t];
-    const bool active = cont && vol != kDeadVolume;
+    const bool active = in_range && vol != kDeadVolume;
 
     // ---- phase A: step-start rules, physics step limit (A3), process choice (U1)
     int fate = FATE_NONE, process = 0, mat = 0;
@@ -210,20 +175,20 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
       if (cross) { px += c.eps_push * pdx; py += c.eps_push * pdy; pz += c.eps_push * pdz; }   // G5
     }
     // at-rest annihilation (P8): both photons carry m; below the gamma cut they are deposited (M5)
-    bool ph = false;
+    bool has_ph = false;
     if (ann_rest) {
       if (kMe < mat_scalar(c, mat, S_KCUT)) { edep_cut += kMe; edep_cut += kMe; }
-      else ph = true;
+      else has_ph = true;
     }
 
     // ---- relocation (A5), warp-convergent
     const int nv = nav_relocate<BVH>(c, c.navigator, cross, vol, px, py, pz, face);
 
-    // ---- outcome; position, step count and volume join the direction and energy in the tile slot
-    bool lv = false;
-    int dst = -1;
+    // ---- outcome
+    bool live = false;
+    int dest = -1;
+    uint32_t vol_post = vol;
     if (active) {
-      uint32_t vol_post = vol;
       packed += 1ull << (8 * MC_STEPS);
       sum_dep += edep_dep; sum_cut += edep_cut;
       if (fate == FATE_KILLED) {
@@ -243,34 +208,97 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
           packed += 1ull << (8 * MC_ESCAPED);
         } else {
           vol_post = static_cast<uint32_t>(nv);
-          lv = true; dst = 0;
+          live = true; dest = 0;
           packed += 1ull << (8 * MC_BOUNDARY);
         }
       } else if (flag == 2) {
-        lv = true; dst = 0;
+        live = true; dest = 0;
         packed += 1ull << (8 * MC_TRUNCATED);
       } else if (!lim_disc) {
-        lv = true; dst = 0;
+        live = true; dest = 0;
         packed += 1ull << (8 * MC_LOSS);
       } else {
-        lv = true; dst = 1 + stage_queue(process, species) - q0;
+        live = true; dest = 1 + stage_queue(process, species) - q0;
       }
-      T.d[0][t] = px; T.d[1][t] = py; T.d[2][t] = pz;
-      T.u[1][t] += 1; T.u[2][t] = vol_post;
-      live = lv; dest = dst; has_ph = ph;
+      if (MULTI) {
+        T.d[0][t] = px; T.d[1][t] = py; T.d[2][t] = pz;
+        T.u[1][t] += 1; T.u[2][t] = vol_post;
+      }
+      r.px = px; r.py = py; r.pz = pz; r.vol_post = vol_post; r.live = live; r.dest = dest; r.has_ph = has_ph;
     }
     score(slot, vol, edep_dep + edep_cut, active);
-    cont = active && lv && dst == 0 && it + 1 < k_inner;
-    if (!__any_sync(kFull, cont)) break;
-    }   // steps of this lane's track
-    counted += k_inner;
+}
+
+template <int FIELD, bool BVH, bool MULTI>
+__global__ void __launch_bounds__(kBlock, FIELD == ADEPT_FIELD_NONE ? ADEPT_MINB_C2 : ADEPT_MINB_C2F)
+charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot, int parity) {
+  const int species = static_cast<int>(blockIdx.y);   // ADEPT_ELECTRON or ADEPT_POSITRON
+  const bool positron = species == ADEPT_POSITRON;
+  const TrackSoA& cur = slot.buf[parity][species];
+  SlotCounters* cnt = slot.counters;
+  // (a counter can run past the capacity when its queue overflowed: the stores are guarded, the reads clamped)
+  const uint32_t n = min(cnt->count[parity][species].v, c.capacity);
+
+  // destinations: 0 = next buffer of the species, 1..3 = its staging queues, 4 = next gamma buffer (the
+  // photons of an annihilation at rest)
+  constexpr int ND = 5;
+  const int q0 = positron ? 5 : 3;
+  // Tracks per tile.  A population smaller than the grid's lanes is spread over all blocks and warps
+  // (g tracks per tile, one lane in every 128/g): the warp-cooperative BVH serves the queries of a warp
+  // one after the other, so a few hundred loopers packed into a few warps would take 32 x 16 chord queries
+  // in sequence per step (measured 4 ms per population step on config 4), spread out they run in parallel.
+  uint32_t g = kBlock;
+  while (g > 4 && (n + (g >> 1) - 1) / (g >> 1) <= gridDim.x) g >>= 1;
+  const int lane_shift = __ffs(kBlock / g) - 1;            // every (1 << lane_shift)-th lane takes a track
+  const uint32_t n_tiles = (n + g - 1) / g;
+  if (blockIdx.x >= n_tiles) return;   // no tile for this block
+  __shared__ BlockTally tally;
+  __shared__ BlockReserve<ND> br;
+  __shared__ TilePipe pipe;
+  tally_init(tally);
+  pipe_init(pipe);
+  double sum_dep = 0.0, sum_cut = 0.0;
+  unsigned chords_sum = 0;
+  unsigned long long packed = 0;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned lt = (1u << lane) - 1u;
+  const int t = threadIdx.x >> lane_shift;                 // this lane's entry of the tile
+  const bool mine = (threadIdx.x & ((1u << lane_shift) - 1u)) == 0;
+  const int k_inner = MULTI ? min(inner_steps(c, n, gridDim.x * kBlock), 255) : 1;
+
+  if (threadIdx.x == 0) tile_issue_n(pipe.tile[0], cur, static_cast<size_t>(blockIdx.x) * g, g, &pipe.bar[0]);
+  uint32_t k = 0;
+  for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++k) {
+    const int phase = k & 1;
+    if (threadIdx.x == 0 && tile + gridDim.x < n_tiles)
+      tile_issue_n(pipe.tile[phase ^ 1], cur, static_cast<size_t>(tile + gridDim.x) * g, g, &pipe.bar[phase ^ 1]);
+    mbar_wait(&pipe.bar[phase], (k >> 1) & 1);
+    TrackTile& T = pipe.tile[phase];
+    ChargedLane r;
+    r.px = 0.0; r.py = 0.0; r.pz = 0.0; r.vol_post = 0; r.live = false; r.has_ph = false; r.dest = -1;
+    if (!MULTI) {
+      charged_lane<FIELD, BVH, false>(c, slot, tally, T, t, mine && tile * g + t < n, species, q0, packed, sum_dep, sum_cut, chords_sum, r);
+      if (k % 255u == 254u) move_counts_flush(tally, packed);
+    } else {
+      // A lane steps its track until it leaves the species buffer (interaction, stop, escape, ...) or has taken
+      // k_inner steps; the warp goes round together because the navigator is warp-convergent.
+      bool cont = mine && tile * g + t < n;
+      for (int it = 0;; ++it) {
+        charged_lane<FIELD, BVH, true>(c, slot, tally, T, t, cont, species, q0, packed, sum_dep, sum_cut, chords_sum, r);
+        cont = cont && r.live && r.dest == 0 && it + 1 < k_inner;
+        if (!__any_sync(kFull, cont)) break;
+      }
+      move_counts_flush(tally, packed);
+    }
     // Everything still needed of the track is read from the tile here, before the reservation barriers:
     // after them thread 0 may already refill this tile buffer.
     Track post;
-    post.x = T.d[0][t]; post.y = T.d[1][t]; post.z = T.d[2][t];
+    post.x = r.px; post.y = r.py; post.z = r.pz;
     post.dx = T.d[3][t]; post.dy = T.d[4][t]; post.dz = T.d[5][t];
     post.ekin = T.d[6][t]; post.id = T.id[t];
-    post.event = T.u[0][t]; post.step = T.u[1][t]; post.vol = T.u[2][t]; post.species = species;
+    post.event = T.u[0][t]; post.step = MULTI ? T.u[1][t] : T.u[1][t] + 1; post.vol = r.vol_post; post.species = species;
+    const bool live = r.live, has_ph = r.has_ph;
+    const int dest = r.dest;
     fence_proxy_async_smem();
 
     // ---- reservation and stores (A0)

@@ -20,11 +20,13 @@ __device__ __forceinline__ void field_at(const DevCtx& c, const double p[3], dou
   B[0] = B[1] = B[2] = 0.0;
   if (c.field_kind != ADEPT_FIELD_MAP_RZ) return;
   const double r = sqrt(p[0] * p[0] + p[1] * p[1]);
-  double fr = (r - c.r0) / c.dr, fz = (p[2] - c.z0) / c.dz;
+  // (grid coordinates by multiplication with the inverse spacing: exact for the 1 cm grid of the configs, within
+  // an ulp otherwise, and the interpolant is continuous across cells)
+  double fr = (r - c.r0) * c.inv_dr, fz = (p[2] - c.z0) * c.inv_dz;
   fr = fmin(fmax(fr, 0.0), static_cast<double>(c.nr - 1));
   fz = fmin(fmax(fz, 0.0), static_cast<double>(c.nz - 1));
-  const int ir = min(static_cast<int>(floor(fr)), c.nr - 2);
-  const int iz = min(static_cast<int>(floor(fz)), c.nz - 2);
+  const int ir = min(static_cast<int>(fr), c.nr - 2);
+  const int iz = min(static_cast<int>(fz), c.nz - 2);
   const double a = fr - ir, b = fz - iz;
   const double* m = c.bz + iz * c.nr + ir;
   const double v00 = __ldg(m), v01 = __ldg(m + 1), v10 = __ldg(m + c.nr), v11 = __ldg(m + c.nr + 1);
@@ -33,37 +35,61 @@ __device__ __forceinline__ void field_at(const DevCtx& c, const double p[3], dou
   B[2] = lo + b * (hi - lo);
 }
 
-// F3: exact helix, omega = -q kCB |B| h / p
+// sin and cos of a small angle by their Maclaurin series (|x| <= 0.8: the terms dropped, x^19/19! and x^20/20!,
+// are below 2e-19).  A chord turns the track by omega = sqrt(8 delta / R) about B, half of that is what the helix
+// needs; libdevice's sincos spends most of its ~90 instructions on argument reduction that cannot be needed here.
+__device__ __forceinline__ void sincos_small(double x, double& sn, double& cs) {
+  const double z = x * x;
+  double p = -1.0 / 355687428096000.0;          // -1/17!
+  p = fma(p, z, 1.0 / 1307674368000.0);         //  1/15!
+  p = fma(p, z, -1.0 / 6227020800.0);           // -1/13!
+  p = fma(p, z, 1.0 / 39916800.0);              //  1/11!
+  p = fma(p, z, -1.0 / 362880.0);               // -1/9!
+  p = fma(p, z, 1.0 / 5040.0);                  //  1/7!
+  p = fma(p, z, -1.0 / 120.0);                  // -1/5!
+  p = fma(p, z, 1.0 / 6.0);                     //  1/3!
+  sn = fma(-x * z, p, x);
+  double q = 1.0 / 6402373705728000.0;          //  1/18!
+  q = fma(q, z, -1.0 / 20922789888000.0);       // -1/16!
+  q = fma(q, z, 1.0 / 87178291200.0);           //  1/14!
+  q = fma(q, z, -1.0 / 479001600.0);            // -1/12!
+  q = fma(q, z, 1.0 / 3628800.0);               //  1/10!
+  q = fma(q, z, -1.0 / 40320.0);                // -1/8!
+  q = fma(q, z, 1.0 / 720.0);                   //  1/6!
+  q = fma(q, z, -1.0 / 24.0);                   // -1/4!
+  q = fma(q, z, 0.5);                           //  1/2!
+  cs = fma(-z, q, 1.0);
+}
+
+// F3: exact helix about the unit vector b; kappa = -q kCB |B| / p is the turning angle per unit path length
+// (constant over a step: F1 takes p at the pre-step energy), so omega = kappa h and h / omega = 1 / kappa.
+// sin(omega), cos(omega) and 1 - cos(omega) all come from the half angle.
 // inlined (as rk4): as calls their array arguments lived in local memory (config 3: 251 -> 227 ms per pass)
-__device__ __forceinline__ void helix(const double B[3], int charge, double pmom, double h, const double p[3],
+__device__ __forceinline__ void helix(const double b[3], double kappa, double inv_kappa, double h, const double p[3],
                                       const double d[3], double p1[3], double d1[3]) {
-  const double Bn = sqrt(B[0] * B[0] + B[1] * B[1] + B[2] * B[2]);
-  const double b[3] = {B[0] / Bn, B[1] / Bn, B[2] / Bn};
-  const double omega = -charge * kCB * Bn * h / pmom;
+  const double half = 0.5 * kappa * h;
+  double s2, c2;
+  if (fabs(half) <= 0.8) sincos_small(half, s2, c2);
+  else sincos(half, &s2, &c2);
+  const double so = 2.0 * s2 * c2, omc = 2.0 * s2 * s2, co = 1.0 - omc;
   const double dpar = d[0] * b[0] + d[1] * b[1] + d[2] * b[2];
   const double dl[3] = {dpar * b[0], dpar * b[1], dpar * b[2]};
   const double dt[3] = {d[0] - dl[0], d[1] - dl[1], d[2] - dl[2]};
   double bxd[3];
   cross3(b, dt, bxd);
-  double so, co;
-  sincos(omega, &so, &co);
-  const double sh = sin(0.5 * omega);
-  const double omc = 2.0 * sh * sh;
-  const double hw = h / omega;
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
     d1[i] = dl[i] + dt[i] * co + bxd[i] * so;
-    p1[i] = p[i] + dl[i] * h + hw * (dt[i] * so + bxd[i] * omc);
+    p1[i] = p[i] + dl[i] * h + inv_kappa * (dt[i] * so + bxd[i] * omc);
   }
 }
 
-// F1, F3: one classical RK4 step on (x, d): x' = d, d' = (q kCB / p) d x B(x)
+// F1, F3: one classical RK4 step on (x, d): x' = d, d' = (q kCB / p) d x B(x); B0 = B(p), already known
 __device__ __forceinline__ void rk4(const DevCtx& c, int charge, double pmom, double h, const double p[3],
-                                    const double d[3], double p1[3], double d1[3]) {
+                                    const double d[3], const double B0[3], double p1[3], double d1[3]) {
   const double kap = charge * kCB / pmom;
   double B[3], k1v[3], k2v[3], k3v[3], k4v[3], k2x[3], k3x[3], k4x[3], x[3], v[3], t[3];
-  field_at(c, p, B);
-  cross3(d, B, t);
+  cross3(d, B0, t);
 #pragma unroll
   for (int i = 0; i < 3; ++i) { k1v[i] = kap * t[i]; x[i] = p[i] + 0.5 * h * d[i]; v[i] = d[i] + 0.5 * h * k1v[i]; }
   field_at(c, x, B);
@@ -84,27 +110,38 @@ __device__ __forceinline__ void rk4(const DevCtx& c, int charge, double pmom, do
     d1[i] = d[i] + (h / 6.0) * (k1v[i] + 2.0 * k2v[i] + 2.0 * k3v[i] + k4v[i]);
     n += d1[i] * d1[i];
   }
-  n = sqrt(n);
+  n = rsqrt(n);
 #pragma unroll
-  for (int i = 0; i < 3; ++i) d1[i] /= n;
+  for (int i = 0; i < 3; ++i) d1[i] *= n;
 }
 
 // F2-F4 chord loop.  flag: 0 physics limit reached, 1 boundary (pos = hit point without the push,
 // pushdir = chord direction), 2 truncated (chord budget).  Warp-convergent.
 // FIELD >= 0 fixes the field kind at compile time (no helix / RK4 code where it cannot run); -1 = runtime.
+//
+// What the loop does NOT do per chord (measured: config 3 spent 4.5 us per chord of its spiralling tracks, a
+// chain of ~900 dependent instructions): the constants of a uniform field (|B|, B / |B|, the turning rate kappa)
+// are taken once per step; sines and cosines of the small turning angle come from their series; and the
+// geometry query of a chord is skipped while the track is provably farther from every boundary than the chord is
+// long (nav_safety; SURVEY.md F5 reading A: "safety only decides whether the chord's geometry query can be
+// skipped" -- the outcome of the step is the same, so the oracle has no safety at all).  A safety is computed
+// when a step needs more than one chord, and again when it is used up.
 template <int FIELD = -1, bool BVH = true>
 __device__ __forceinline__ int propagate(const DevCtx& c, int nav, bool active, int charge, double ekin, double pos[3], double dir[3],
                          uint32_t vol, double s_phys, double& s_out, int& chords_out, double pushdir[3], int& face_out) {
   const int field_kind = FIELD >= 0 ? FIELD : c.field_kind;
   const double pmom = sqrt(ekin * (ekin + 2.0 * kMe));
+  const double kappa = field_kind == ADEPT_FIELD_UNIFORM ? -charge * kCB * c.Bn / pmom : 0.0;
+  const double inv_kappa = kappa != 0.0 ? 1.0 / kappa : 0.0;
   double s_done = 0.0;
+  double safe = -1.0;   // clearance known to be left around pos (< 0: not known)
   int chords = 0, flag = 0, face_hit = -1;
   bool running = active;
 #pragma unroll
   for (int i = 0; i < 3; ++i) pushdir[i] = dir[i];
   while (__any_sync(kFull, running)) {
     // --- per-lane: decide the next segment
-    bool query = false, straight = false, last = false;
+    bool query = false, straight = false, last = false, chord = false;
     double h = 0.0, L = 0.0, rest = 0.0;
     double u[3] = {0.0, 0.0, 0.0}, p1[3], d1[3], B[3] = {0.0, 0.0, 0.0};
     if (running) {
@@ -133,56 +170,61 @@ __device__ __forceinline__ int propagate(const DevCtx& c, int nav, bool active, 
           }
           last = h_max >= rest;
           h = last ? rest : h_max;
-          if (field_kind == ADEPT_FIELD_UNIFORM) helix(B, charge, pmom, h, pos, dir, p1, d1);
-          else rk4(c, charge, pmom, h, pos, dir, p1, d1);
+          if (field_kind == ADEPT_FIELD_UNIFORM) helix(c.bhat, kappa, inv_kappa, h, pos, dir, p1, d1);
+          else rk4(c, charge, pmom, h, pos, dir, B, p1, d1);
           const double ch[3] = {p1[0] - pos[0], p1[1] - pos[1], p1[2] - pos[2]};
-          L = sqrt(ch[0] * ch[0] + ch[1] * ch[1] + ch[2] * ch[2]);
-          u[0] = ch[0] / L; u[1] = ch[1] / L; u[2] = ch[2] / L;
-          query = true;
+          const double L2 = ch[0] * ch[0] + ch[1] * ch[1] + ch[2] * ch[2];
+          const double iL = rsqrt(L2);
+          L = L2 * iL;
+          u[0] = ch[0] * iL; u[1] = ch[1] * iL; u[2] = ch[2] * iL;
+          chord = true;
+          // the chord needs no geometry query if it is shorter than the clearance left (a chord's length never
+          // exceeds its arc's, so h bounds it: no dependence on the rounding of L)
+          if (safe < h && !(last && safe < 0.0)) safe = nav_safety(c, vol, pos[0], pos[1], pos[2]);
+          query = !(h < safe);
+          safe = query ? -1.0 : safe - h;
         }
       }
     }
     // --- warp-cooperative geometry query of this segment
     int face;
     const double s_geo = nav_distance<BVH>(c, nav, query, pos[0], pos[1], pos[2], u[0], u[1], u[2], vol, L, face);
-    if (query) {
-      face_hit = face;   // only meaningful when this segment ends on the boundary (flag 1), which ends the loop
-      if (straight) {
-        pushdir[0] = u[0]; pushdir[1] = u[1]; pushdir[2] = u[2];
-        if (s_geo < rest) {
+    if (query) face_hit = face;   // only meaningful when this segment ends on the boundary (flag 1), which ends the loop
+    if (straight) {
+      pushdir[0] = u[0]; pushdir[1] = u[1]; pushdir[2] = u[2];
+      if (s_geo < rest) {
 #pragma unroll
-          for (int i = 0; i < 3; ++i) pos[i] += s_geo * dir[i];
-          s_done += s_geo; flag = 1;
-        } else {
-#pragma unroll
-          for (int i = 0; i < 3; ++i) pos[i] += rest * dir[i];
-          s_done = s_phys; flag = 0;
-        }
-        running = false;
+        for (int i = 0; i < 3; ++i) pos[i] += s_geo * dir[i];
+        s_done += s_geo; flag = 1;
       } else {
-        ++chords;
-        if (s_geo < L) {
-          const double frac = s_geo / L;
-          double dh[3];
-          if (field_kind == ADEPT_FIELD_UNIFORM) {
-            double ph[3];
-            helix(B, charge, pmom, h * frac, pos, dir, ph, dh);
-          } else {
-            double n = 0.0;
 #pragma unroll
-            for (int i = 0; i < 3; ++i) { dh[i] = dir[i] + frac * (d1[i] - dir[i]); n += dh[i] * dh[i]; }
-            n = sqrt(n);
-#pragma unroll
-            for (int i = 0; i < 3; ++i) dh[i] /= n;
-          }
-#pragma unroll
-          for (int i = 0; i < 3; ++i) { pos[i] += s_geo * u[i]; dir[i] = dh[i]; pushdir[i] = u[i]; }
-          s_done += h * frac; flag = 1; running = false;
+        for (int i = 0; i < 3; ++i) pos[i] += rest * dir[i];
+        s_done = s_phys; flag = 0;
+      }
+      running = false;
+    } else if (chord) {
+      ++chords;
+      if (query && s_geo < L) {
+        const double frac = s_geo / L;
+        double dh[3];
+        if (field_kind == ADEPT_FIELD_UNIFORM) {
+          double ph[3];
+          helix(c.bhat, kappa, inv_kappa, h * frac, pos, dir, ph, dh);
         } else {
+          double n = 0.0;
 #pragma unroll
-          for (int i = 0; i < 3; ++i) { pos[i] = p1[i]; dir[i] = d1[i]; }
-          s_done = last ? s_phys : s_done + h;
+          for (int i = 0; i < 3; ++i) { dh[i] = dir[i] + frac * (d1[i] - dir[i]); n += dh[i] * dh[i]; }
+          n = rsqrt(n);
+#pragma unroll
+          for (int i = 0; i < 3; ++i) dh[i] *= n;
         }
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { pos[i] += s_geo * u[i]; dir[i] = dh[i]; pushdir[i] = u[i]; }
+        s_done += h * frac; flag = 1; running = false;
+      } else {
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { pos[i] = p1[i]; dir[i] = d1[i]; }
+        s_done = last ? s_phys : s_done + h;
       }
     }
   }

@@ -9,6 +9,11 @@
 // inlined: as calls they cost 4 % of a config-2 pass).  The discrete process is chosen (U1) before the
 // propagation -- it depends on nothing the propagation computes -- so neither the cross sections nor
 // the Philox state survive phase A.
+//
+// Two instantiations (adept.cu picks one per host round from the slot's population): MULTI = false takes one
+// step per track and launch; MULTI = true lets a lane go on stepping its own track while it stays in the
+// gamma buffer (kernels.cuh inner_steps), with the whole state kept in the lane's tile slot between steps.
+// The loop costs registers (spills at the 5-block cap) and 2-5 % of a full-GPU pass, hence the lean variant.
 #pragma once
 #include "kernels.cuh"
 
@@ -34,19 +39,20 @@ __device__ __forceinline__ void gamma_counts_flush(BlockTally& t, unsigned long 
   packed = 0;
 }
 
-// One gamma step of lane `t` of a tile (phases A-C and the outcome); warp-convergent.  The post-step
-// position, step count and volume go back into the lane's tile slot (a photon's direction and energy do
-// not change in a move), so the slot holds the state to store if `live` (dest 0 = next gamma buffer, 1.. =
-// staging queue of the process) -- or the pre-step state of the lane's next step within this launch
-// (kernels.cuh inner_steps); (has_pe, T_pe) describe the photoelectron.
+// One gamma step of lane `t` of a tile (phases A-C and the outcome); warp-convergent.  On return `post` is
+// the state to store if `live` (dest 0 = next gamma buffer, 1.. = staging queue of the process), and
+// (has_pe, T_pe) describe the photoelectron.  MULTI: the post-step position, step count and volume also go
+// back into the lane's tile slot (a photon's direction and energy do not change in a move), so that the slot
+// is the pre-step state of the lane's next step within this launch.
 struct GammaLane {
+  Track post;
   double edep, T_pe;
   bool active, live, has_pe;
   int dest;
   uint32_t vol;   // pre-step volume (scoring)
 };
 
-template <bool BVH, int N>
+template <bool BVH, bool MULTI, int N>
 __device__ __forceinline__ void gamma_lane(const DevCtx& c, const DevSlot& slot, BlockTally& tally, TrackTileT<N>& T, int t,
                                            bool in_range, unsigned long long& packed, GammaLane& r) {
   constexpr int species = ADEPT_GAMMA;
@@ -106,56 +112,57 @@ __device__ __forceinline__ void gamma_lane(const DevCtx& c, const DevSlot& slot,
     // ---- phase C: relocation (A5)
     const int nv = nav_relocate<BVH>(c, c.navigator, cross, vol, px, py, pz, face);
 
-    // ---- outcome
+    // ---- outcome.  Everything still needed of the track is read from the tile here, before the
+    // reservation barriers: after them thread 0 may already refill this tile buffer.
+    Track post;
+    post.x = px; post.y = py; post.z = pz;
+    post.dx = T.d[3][t]; post.dy = T.d[4][t]; post.dz = T.d[5][t];
+    post.ekin = T.d[6][t]; post.id = T.id[t];
+    post.event = T.u[0][t]; post.step = T.u[1][t] + 1; post.vol = vol; post.species = species;
     double edep = 0.0, T_pe = 0.0;
     bool live = false, has_pe = false;
     int dest = -1;
     if (active) {
-      const double ekin = T.d[6][t];
-      uint32_t vol_post = vol;
       packed += 1ull << (10 * GC_STEPS);
       if (fate == FATE_KILLED) {
-        atomicAdd(&tally.ledger[3], ekin);
+        atomicAdd(&tally.ledger[3], post.ekin);
         packed += 1ull << (10 * GC_KILLED);
       } else if (fate == FATE_STOPPED) {
-        edep = ekin;
+        edep = post.ekin;
         packed += 1ull << (10 * GC_STOPPED);
       } else if (cross) {
         if (nv < 0) {
-          Track post;
-          post.x = px; post.y = py; post.z = pz;
-          post.dx = T.d[3][t]; post.dy = T.d[4][t]; post.dz = T.d[5][t];
-          post.ekin = ekin; post.id = T.id[t];
-          post.event = T.u[0][t]; post.step = T.u[1][t] + 1; post.vol = vol; post.species = species;
-          atomicAdd(&tally.ledger[2], ekin);
+          atomicAdd(&tally.ledger[2], post.ekin);
           record_leak(c, slot, post, species);
           packed += 1ull << (10 * GC_ESCAPED);
         } else {
-          vol_post = static_cast<uint32_t>(nv);
+          post.vol = static_cast<uint32_t>(nv);
           live = true; dest = 0;
           packed += 1ull << (10 * GC_BOUNDARY);
         }
       } else if (process == ADEPT_OUT_PHOTO) {   // P3: no sampling involved, done here rather than staged
         const double BK = mat_scalar(c, mat, S_BK);
-        if (ekin > BK) {
+        if (post.ekin > BK) {
           edep = BK;
-          T_pe = ekin - BK;
+          T_pe = post.ekin - BK;
           if (T_pe < mat_scalar(c, mat, S_TCUT)) edep += T_pe;   // M5: below the production cut
           else has_pe = true;
         } else {
-          edep = ekin;
+          edep = post.ekin;
         }
         packed += 1ull << (10 * GC_PHOTO);
       } else {                                   // Compton / pair: staged for the interaction kernel
         live = true; dest = 1 + process - ADEPT_OUT_COMPTON;
       }
-      T.d[0][t] = px; T.d[1][t] = py; T.d[2][t] = pz;
-      T.u[1][t] += 1; T.u[2][t] = vol_post;
+      if (MULTI) {
+        T.d[0][t] = px; T.d[1][t] = py; T.d[2][t] = pz;
+        T.u[1][t] = post.step; T.u[2][t] = post.vol;
+      }
     }
-    r.edep = edep; r.T_pe = T_pe; r.active = active; r.live = live; r.has_pe = has_pe; r.dest = dest; r.vol = vol;
+    r.post = post; r.edep = edep; r.T_pe = T_pe; r.active = active; r.live = live; r.has_pe = has_pe; r.dest = dest; r.vol = vol;
 }
 
-template <bool BVH>
+template <bool BVH, bool MULTI>
 __global__ void __launch_bounds__(kBlock, ADEPT_MINB_G2)
 gamma_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot, int parity) {
   constexpr int species = ADEPT_GAMMA;
@@ -178,8 +185,7 @@ gamma_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevS
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const unsigned lt = (1u << lane) - 1u;
   const int t = threadIdx.x;
-  const int k_inner = inner_steps(c, n, gridDim.x * kBlock);
-  int counted = 0;   // steps a lane may have added to each field of `packed` since the last flush
+  const int k_inner = MULTI ? min(inner_steps(c, n, gridDim.x * kBlock), 1023) : 1;
 
   const uint32_t n_tiles = (n + kBlock - 1) / kBlock;
   if (t == 0 && blockIdx.x < n_tiles) tile_issue(pipe.tile[0], cur, blockIdx.x, &pipe.bar[0]);
@@ -188,32 +194,33 @@ gamma_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevS
     const int phase = k & 1;
     if (t == 0 && tile + gridDim.x < n_tiles) tile_issue(pipe.tile[phase ^ 1], cur, tile + gridDim.x, &pipe.bar[phase ^ 1]);
     mbar_wait(&pipe.bar[phase], (k >> 1) & 1);
-    TrackTile& T = pipe.tile[phase];
-    // A lane steps its track until it leaves the gamma buffer (interaction, absorption, escape, ...) or has
-    // taken k_inner steps; the warp goes round together because the navigator is warp-convergent.
-    double T_pe = 0.0;
-    bool live = false, has_pe = false;
-    int dest = -1;
-    bool cont = tile * kBlock + t < n;
-    if (counted + k_inner > 1023) { gamma_counts_flush(tally, packed); counted = 0; }
-    for (int it = 0;; ++it) {
-      GammaLane r;
-      gamma_lane<BVH>(c, slot, tally, T, t, cont, packed, r);
+    GammaLane r;
+    if (!MULTI) {
+      gamma_lane<BVH, false>(c, slot, tally, pipe.tile[phase], t, tile * kBlock + t < n, packed, r);
       score(slot, r.vol, r.edep, r.active);
       sum_cut += r.edep;
-      if (r.active) { live = r.live; has_pe = r.has_pe; dest = r.dest; T_pe = r.T_pe; }
-      cont = r.active && r.live && r.dest == 0 && it + 1 < k_inner;
-      if (!__any_sync(kFull, cont)) break;
+      if ((k & 1023u) == 1022u) gamma_counts_flush(tally, packed);
+    } else {
+      // A lane steps its track until it leaves the gamma buffer (interaction, absorption, escape, ...) or has
+      // taken k_inner steps; the warp goes round together because the navigator is warp-convergent.  A lane
+      // that is done keeps the result of its last step in `r`.
+      bool cont = tile * kBlock + t < n;
+      for (int it = 0;; ++it) {
+        GammaLane q;
+        gamma_lane<BVH, true>(c, slot, tally, pipe.tile[phase], t, cont, packed, q);
+        score(slot, q.vol, q.edep, q.active);
+        sum_cut += q.edep;
+        if (q.active || it == 0) r = q;
+        cont = q.active && q.live && q.dest == 0 && it + 1 < k_inner;
+        if (!__any_sync(kFull, cont)) break;
+      }
+      gamma_counts_flush(tally, packed);
+      fence_proxy_async_smem();   // the tile writes (generic proxy) before the TMA refill of this buffer
     }
-    counted += k_inner;
-    // Everything still needed of the track is read from the tile here, before the reservation barriers:
-    // after them thread 0 may already refill this tile buffer.
-    Track post;
-    post.x = T.d[0][t]; post.y = T.d[1][t]; post.z = T.d[2][t];
-    post.dx = T.d[3][t]; post.dy = T.d[4][t]; post.dz = T.d[5][t];
-    post.ekin = T.d[6][t]; post.id = T.id[t];
-    post.event = T.u[0][t]; post.step = T.u[1][t]; post.vol = T.u[2][t]; post.species = species;
-    fence_proxy_async_smem();   // the tile writes of gamma_lane (generic proxy) before the TMA refill of this buffer
+    Track post = r.post;
+    const double T_pe = r.T_pe;
+    const bool live = r.live, has_pe = r.has_pe;
+    const int dest = r.dest;
 
     // ---- reservation and stores (A0)
     uint32_t pre = 0;

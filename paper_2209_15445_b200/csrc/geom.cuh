@@ -341,6 +341,40 @@ __device__ __forceinline__ double nav_distance(const DevCtx& c, int nav, bool ac
   return nav_distance<BVH>(c, nav, active, px, py, pz, dx, dy, dz, vol, s_max, face);
 }
 
+// ---------------------------------------------------------------- safety (reading A)
+// A lower bound on the distance from a point inside volume `vol` (and inside none of its daughters) to the
+// nearest boundary of the volume: its own surface or any daughter.  Only used to decide that a chord of the
+// field propagation shorter than this bound cannot reach a boundary, so that its geometry query can be skipped
+// -- the result of the step is the same with or without it (the oracle has no safety at all).  Conservative by
+// construction: distances to the own surface are exact or under-estimated, a daughter's is bounded by the
+// largest per-axis separation (<= the Euclidean distance); 1e-6 relative and 1e-9 cm are taken off for
+// rounding.  Lane-local.  0 for a volume whose daughters sit in a BVH (no cheap bound).
+__device__ __forceinline__ double solid_safety_in(const DevVolume& v, const double p[3]) {
+  if (v.solid == ADEPT_BOX) return fmin(fmin(v.dims[0] - fabs(p[0]), v.dims[1] - fabs(p[1])), v.dims[2] - fabs(p[2]));
+  const double r = sqrt(p[0] * p[0] + p[1] * p[1]);
+  double s = fmin(v.dims[1] - r, v.dims[2] - fabs(p[2]));
+  if (v.dims[0] > 0.0) s = fmin(s, r - v.dims[0]);
+  return s;
+}
+__device__ __forceinline__ double solid_safety_out(const DevVolume& v, const double p[3]) {
+  if (v.solid == ADEPT_BOX) return fmax(fmax(fabs(p[0]) - v.dims[0], fabs(p[1]) - v.dims[1]), fabs(p[2]) - v.dims[2]);
+  const double r = sqrt(p[0] * p[0] + p[1] * p[1]);
+  return fmax(fmax(r - v.dims[1], v.dims[0] - r), fabs(p[2]) - v.dims[2]);
+}
+__device__ __forceinline__ double nav_safety(const DevCtx& c, uint32_t vol, double px, double py, double pz) {
+  const DevVolume& v = volume(c, vol);
+  if (v.dcount > 0 && v.bvh >= 0) return 0.0;
+  double l[3];
+  to_local(c, vol, v, px, py, pz, l);
+  double s = solid_safety_in(v, l);
+  for (int k = 0; k < v.dcount && s > 0.0; ++k) {
+    const DevVolume& d = volume(c, v.dbegin + k);
+    to_local(c, v.dbegin + k, d, px, py, pz, l);
+    s = fmin(s, solid_safety_out(d, l));
+  }
+  return s * (1.0 - 1.0e-6) - 1.0e-9;
+}
+
 // ---------------------------------------------------------------- G4 Locate
 // From the world down, descend into the first daughter (index order) containing the point.
 // Warp-convergent call; returns -1 outside the world or for inactive lanes.

@@ -122,8 +122,9 @@ struct DevCtx {
   int32_t n_mat;
   int32_t field_kind;
   double B[3];
+  double Bn, bhat[3];       // |B| and B / |B| of a uniform field (adept_init)
   int32_t nr, nz;
-  double r0, z0, dr, dz;
+  double r0, z0, dr, dz, inv_dr, inv_dz;
   const double* bz;
   double u0, inv_du, du;
   double delta_chord, eps_push, alpha_R, rho_R;
