@@ -135,6 +135,7 @@ __device__ __forceinline__ int propagate(const DevCtx& c, int nav, bool active, 
   const double inv_kappa = kappa != 0.0 ? 1.0 / kappa : 0.0;
   double s_done = 0.0;
   double safe = -1.0;   // clearance known to be left around pos (< 0: not known)
+  double h_step = -1.0; // uniform field: the chord length limit of this step (< 0: not yet known)
   int chords = 0, flag = 0, face_hit = -1;
   bool running = active;
 #pragma unroll
@@ -148,41 +149,52 @@ __device__ __forceinline__ int propagate(const DevCtx& c, int nav, bool active, 
       if (s_done >= s_phys) {
         flag = 0; running = false;
       } else {
-        double bperp = 0.0;
-        if (charge != 0 && field_kind != ADEPT_FIELD_NONE) {  // gammas go straight
+        // In a uniform field |d x B| is a constant of the motion, so the radius and the chord limit sqrt(8 delta R)
+        // are those of the step's first chord (the oracle re-evaluates them per chord and finds the same numbers to
+        // rounding).  On a field map they change from chord to chord.
+        double bperp = 0.0, h_max = 0.0;
+        const bool curved = charge != 0 && field_kind != ADEPT_FIELD_NONE;   // gammas go straight
+        if (curved && (field_kind != ADEPT_FIELD_UNIFORM || h_step < 0.0)) {
           field_at(c, pos, B);
           double dxB[3];
           cross3(dir, B, dxB);
           bperp = sqrt(dxB[0] * dxB[0] + dxB[1] * dxB[1] + dxB[2] * dxB[2]);
+          if (bperp != 0.0) {
+            const double Rcurv = pmom / (kCB * bperp);
+            h_max = sqrt(8.0 * c.delta_chord * Rcurv);
+            if (field_kind == ADEPT_FIELD_MAP_RZ) {  // F2': at most 0.5 rad of turn per RK4 chord
+              const double Bn = sqrt(B[0] * B[0] + B[1] * B[1] + B[2] * B[2]);
+              h_max = fmin(h_max, 0.5 * pmom / (kCB * Bn));
+            }
+          }
+          if (field_kind == ADEPT_FIELD_UNIFORM) h_step = h_max;   // 0: the track runs along B
+        } else if (curved) {
+          h_max = h_step;
         }
         rest = s_phys - s_done;
-        if (charge == 0 || bperp == 0.0) {
+        if (!curved || h_max == 0.0) {
           straight = true; query = true; L = rest;
           u[0] = dir[0]; u[1] = dir[1]; u[2] = dir[2];
         } else if (chords >= c.chord_budget) {
           flag = 2; running = false;
         } else {
-          const double Rcurv = pmom / (kCB * bperp);
-          double h_max = sqrt(8.0 * c.delta_chord * Rcurv);
-          if (field_kind == ADEPT_FIELD_MAP_RZ) {  // F2': at most 0.5 rad of turn per RK4 chord
-            const double Bn = sqrt(B[0] * B[0] + B[1] * B[1] + B[2] * B[2]);
-            h_max = fmin(h_max, 0.5 * pmom / (kCB * Bn));
-          }
           last = h_max >= rest;
           h = last ? rest : h_max;
           if (field_kind == ADEPT_FIELD_UNIFORM) helix(c.bhat, kappa, inv_kappa, h, pos, dir, p1, d1);
           else rk4(c, charge, pmom, h, pos, dir, B, p1, d1);
-          const double ch[3] = {p1[0] - pos[0], p1[1] - pos[1], p1[2] - pos[2]};
-          const double L2 = ch[0] * ch[0] + ch[1] * ch[1] + ch[2] * ch[2];
-          const double iL = rsqrt(L2);
-          L = L2 * iL;
-          u[0] = ch[0] * iL; u[1] = ch[1] * iL; u[2] = ch[2] * iL;
           chord = true;
           // the chord needs no geometry query if it is shorter than the clearance left (a chord's length never
-          // exceeds its arc's, so h bounds it: no dependence on the rounding of L)
+          // exceeds its arc's, so h bounds it)
           if (safe < h && !(last && safe < 0.0)) safe = nav_safety(c, vol, pos[0], pos[1], pos[2]);
           query = !(h < safe);
           safe = query ? -1.0 : safe - h;
+          if (query) {   // unit chord vector and length
+            const double ch[3] = {p1[0] - pos[0], p1[1] - pos[1], p1[2] - pos[2]};
+            const double L2 = ch[0] * ch[0] + ch[1] * ch[1] + ch[2] * ch[2];
+            const double iL = rsqrt(L2);
+            L = L2 * iL;
+            u[0] = ch[0] * iL; u[1] = ch[1] * iL; u[2] = ch[2] * iL;
+          }
         }
       }
     }
