@@ -81,6 +81,8 @@ struct HostBvh {
   std::vector<double> prim_box;                // [6][n]
   std::vector<std::vector<double>> node_box;   // per level [6][n_nodes]
   std::vector<int> n_nodes;
+  std::vector<int32_t> nbr, nbr_count;         // [n][kNbrCap], [n]: per-daughter neighbour lists (geom.cuh NavCache)
+  double nbr_reach = 0.0;
 };
 
 // World-frame AABB of a placed solid, padded so that rounding can never make it miss a true hit.
@@ -156,6 +158,51 @@ void mark_isolated(const adept_geometry* g, int m, double margin, std::vector<in
   }
 }
 
+// Per-daughter neighbour lists of volume m (geom.cuh NavCache): for daughter k the siblings that come within `reach`
+// of its solid, itself first.  Conservative: a pair is left out only when the separating-axis test proves two boxes
+// farther apart than `reach`, or the padded world boxes of any two solids are.  Returns the share of daughters
+// whose list fits kNbrCap (the others get count -1).
+double neighbour_lists(const adept_geometry* g, int m, double reach, std::vector<int32_t>& nbr, std::vector<int32_t>& count) {
+  const int b0 = g->daughter_begin[m], n = g->daughter_count[m];
+  std::vector<double> lo(3 * static_cast<size_t>(n)), hi(3 * static_cast<size_t>(n));
+  double mn[3] = {1e300, 1e300, 1e300}, mx[3] = {-1e300, -1e300, -1e300};
+  for (int k = 0; k < n; ++k) {
+    world_aabb(g, b0 + k, &lo[3 * k], &hi[3 * k]);
+    for (int i = 0; i < 3; ++i) { mn[i] = std::min(mn[i], lo[3 * k + i]); mx[i] = std::max(mx[i], hi[3 * k + i]); }
+  }
+  const int ax = (mx[0] - mn[0] >= mx[1] - mn[1] && mx[0] - mn[0] >= mx[2] - mn[2]) ? 0 : (mx[1] - mn[1] >= mx[2] - mn[2] ? 1 : 2);
+  const int a1 = (ax + 1) % 3, a2 = (ax + 2) % 3;
+  std::vector<int> order(n);
+  std::iota(order.begin(), order.end(), 0);
+  std::sort(order.begin(), order.end(), [&](int p, int q) { return lo[3 * p + ax] < lo[3 * q + ax]; });
+  std::vector<std::vector<int32_t>> lists(n);
+  for (int k = 0; k < n; ++k) lists[k].push_back(b0 + k);
+  for (int ii = 0; ii < n; ++ii) {
+    const int p = order[ii];
+    for (int jj = ii + 1; jj < n; ++jj) {
+      const int q = order[jj];
+      if (lo[3 * q + ax] > hi[3 * p + ax] + reach) break;
+      if (lo[3 * q + a1] > hi[3 * p + a1] + reach || lo[3 * p + a1] > hi[3 * q + a1] + reach) continue;
+      if (lo[3 * q + a2] > hi[3 * p + a2] + reach || lo[3 * p + a2] > hi[3 * q + a2] + reach) continue;
+      const bool both_boxes = g->solid[b0 + p] == ADEPT_BOX && g->solid[b0 + q] == ADEPT_BOX;
+      if (both_boxes && boxes_apart(g, b0 + p, b0 + q, reach)) continue;
+      lists[p].push_back(b0 + q);
+      lists[q].push_back(b0 + p);
+    }
+  }
+  nbr.assign(static_cast<size_t>(n) * kNbrCap, -1);
+  count.assign(n, -1);
+  int fit = 0;
+  for (int k = 0; k < n; ++k) {
+    if (static_cast<int>(lists[k].size()) > kNbrCap) continue;
+    std::sort(lists[k].begin() + 1, lists[k].end());
+    std::copy(lists[k].begin(), lists[k].end(), nbr.begin() + static_cast<size_t>(k) * kNbrCap);
+    count[k] = static_cast<int32_t>(lists[k].size());
+    ++fit;
+  }
+  return n ? static_cast<double>(fit) / n : 0.0;
+}
+
 HostBvh build_bvh(const adept_geometry* g, int v) {
   HostBvh b;
   b.volume = v;
@@ -225,6 +272,11 @@ HostBvh build_bvh(const adept_geometry* g, int v) {
     child = &b.node_box.back();
     n_child = nn;
   }
+  // neighbour lists: the largest reach for which (nearly) every daughter's list fits
+  for (double reach : {1.0, 0.5, 0.25, 0.125, 0.0625}) {
+    if (neighbour_lists(g, v, reach, b.nbr, b.nbr_count) >= 0.95) { b.nbr_reach = reach; break; }
+  }
+  if (b.nbr_reach == 0.0) { b.nbr.assign(static_cast<size_t>(n) * kNbrCap, -1); b.nbr_count.assign(n, -1); }
   return b;
 }
 
@@ -328,6 +380,7 @@ int validate(const adept_config* cfg, const adept_geometry* g, int n_mats, const
 struct Layout {
   DevVolume* vol; double* rot; int32_t* nbr; int32_t* rhint; DevBvh* bvh; double *tab_g, *tab_em, *tab_ep, *scal, *bz;
   std::vector<double*> bvh_prim_box; std::vector<int32_t*> bvh_prim_vol; std::vector<std::vector<double*>> bvh_node_box;
+  std::vector<int32_t*> bvh_nbr, bvh_nbr_count;
   adept_track* stage; uint32_t* bad; size_t stage_cap;
   std::vector<DevSlot> slots;
 };
@@ -347,6 +400,8 @@ size_t carve(void* base, const adept_config* cfg, const adept_geometry* g, int n
     const int n = g->daughter_count[bvh_vols[k]];
     L.bvh_prim_box.push_back(cv.take<double>(6 * static_cast<size_t>(n)));
     L.bvh_prim_vol.push_back(cv.take<int32_t>(n));
+    L.bvh_nbr.push_back(cv.take<int32_t>(static_cast<size_t>(n) * kNbrCap));
+    L.bvh_nbr_count.push_back(cv.take<int32_t>(n));
     std::vector<double*> lv;
     int nn = n;
     do { nn = (nn + 31) / 32; lv.push_back(cv.take<double>(6 * static_cast<size_t>(nn))); } while (nn > 32);
@@ -429,6 +484,7 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   std::vector<DevVolume> hv(nv);
   std::vector<DevBvh> hb;
   std::vector<int32_t> isolated(nv, 0);
+  bool any_lists = false;
   for (int v = 0; v < nv; ++v)
     if (g->daughter_count[v] >= kBvhMinDaughters) {
       mark_isolated(g, v, kIsolationMargin, isolated);
@@ -459,6 +515,13 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
       db.prim_vol = L.bvh_prim_vol[k];
       CUDA_TRY(cudaMemcpy(L.bvh_prim_box[k], b.prim_box.data(), b.prim_box.size() * sizeof(double), cudaMemcpyHostToDevice));
       CUDA_TRY(cudaMemcpy(L.bvh_prim_vol[k], b.prim_vol.data(), b.prim_vol.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+      db.nbr = L.bvh_nbr[k]; db.nbr_count = L.bvh_nbr_count[k]; db.nbr_reach = b.nbr_reach;
+      CUDA_TRY(cudaMemcpy(L.bvh_nbr[k], b.nbr.data(), b.nbr.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+      CUDA_TRY(cudaMemcpy(L.bvh_nbr_count[k], b.nbr_count.data(), b.nbr_count.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+      if (std::getenv("ADEPT_VERBOSE"))
+        std::fprintf(stderr, "adept_init: volume %d: neighbour lists with reach %g cm, %d of %d daughters listed\n", v, b.nbr_reach,
+                     static_cast<int>(std::count_if(b.nbr_count.begin(), b.nbr_count.end(), [](int32_t x) { return x >= 0; })), d.dcount);
+      if (b.nbr_reach > 0.0) any_lists = true;
       for (int l = 0; l < db.n_levels; ++l) {
         db.n_nodes[l] = b.n_nodes[l];
         db.node_box[l] = L.bvh_node_box[k][l];
@@ -535,6 +598,7 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   d.delta_chord = cfg->delta_chord; d.eps_push = cfg->eps_push; d.alpha_R = cfg->alpha_R; d.rho_R = cfg->rho_R;
   d.chord_budget = cfg->chord_budget; d.seed = cfg->seed; d.max_steps = cfg->max_steps;
   d.steps_per_launch = cfg->steps_per_launch;
+  d.transit = (any_lists && cfg->navigator == ADEPT_NAV_BVH && cfg->steps_per_launch != 1) ? 1 : 0;
   d.capacity = static_cast<uint32_t>(cfg->track_capacity);
   d.stage_capacity = static_cast<uint32_t>(cfg->stage_capacity ? cfg->stage_capacity : cfg->track_capacity);
   d.leak_capacity = static_cast<uint32_t>(cfg->leak_capacity);
@@ -755,7 +819,9 @@ bool round_graph(adept_ctx* ctx, SlotHost& sh, int multi) {
 // The showers do not depend on the choice; a stale population costs speed only.
 constexpr size_t kMultiBelow = 65536;
 int round_variant(const adept_ctx* ctx, const SlotHost& sh) {
-  return ctx->cfg.steps_per_launch != 1 && sh.population + (sh.n_pending - sh.n_injected) < kMultiBelow ? 1 : 0;
+  if (ctx->cfg.steps_per_launch == 1) return 0;
+  if (ctx->dev.transit) return 1;   // the multi-step variants also take the passage through a vacuum gap in the same launch
+  return sh.population + (sh.n_pending - sh.n_injected) < kMultiBelow ? 1 : 0;
 }
 
 }  // namespace
@@ -970,6 +1036,7 @@ extern "C" int adept_step_population(adept_ctx* ctx, int slot, int n, const adep
   // (the variant of the move kernels adept_transport would pick for a population of n, held to one step per track)
   DevCtx one = ctx->dev;
   one.steps_per_launch = 1;
+  one.transit = 0;
   sh.population = static_cast<size_t>(n);
   const int variant = round_variant(ctx, sh);
   sh.population = 0;

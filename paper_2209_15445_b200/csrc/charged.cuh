@@ -42,7 +42,7 @@ struct ChargedLane {
 template <int FIELD, bool BVH, bool MULTI>
 __device__ __forceinline__ void charged_lane(const DevCtx& c, const DevSlot& slot, BlockTally& tally, TrackTile& T, int t, bool in_range,
                                              int species, int q0, unsigned long long& packed, double& sum_dep, double& sum_cut,
-                                             unsigned& chords_sum, ChargedLane& r) {
+                                             unsigned& chords_sum, ChargedLane& r, NavCache* cache, int32_t* cand) {
   enum { FATE_NONE = 0, FATE_KILLED, FATE_STOPPED, FATE_GO };
   const bool positron = species == ADEPT_POSITRON;
     const uint32_t vol = T.u[2][t];
@@ -108,7 +108,7 @@ __device__ __forceinline__ void charged_lane(const DevCtx& c, const DevSlot& slo
       const double dx = T.d[3][t], dy = T.d[4][t], dz = T.d[5][t];
       const bool query = go && !(0.0 >= s_phys);
       int f;
-      const double s_geo = nav_distance<BVH>(c, c.navigator, query, px, py, pz, dx, dy, dz, vol, s_phys, f);
+      const double s_geo = nav_distance<BVH>(c, c.navigator, query, px, py, pz, dx, dy, dz, vol, s_phys, f, cache, cand);
       if (query) {
         if (s_geo < s_phys) { px += s_geo * dx; py += s_geo * dy; pz += s_geo * dz; s = s_geo; flag = 1; face = f; }
         else { px += s_phys * dx; py += s_phys * dy; pz += s_phys * dz; s = s_phys; }
@@ -117,7 +117,8 @@ __device__ __forceinline__ void charged_lane(const DevCtx& c, const DevSlot& slo
     } else {
       double pos[3] = {px, py, pz}, dir[3] = {T.d[3][t], T.d[4][t], T.d[5][t]}, pushdir[3];
       int chords = 0;
-      flag = propagate<FIELD, BVH>(c, c.navigator, go, positron ? +1 : -1, T.d[6][t], pos, dir, vol, s_phys, s, chords, pushdir, face);
+      flag = propagate<FIELD, BVH>(c, c.navigator, go, positron ? +1 : -1, T.d[6][t], pos, dir, vol, s_phys, s, chords, pushdir, face,
+                                   cache, cand);
       px = pos[0]; py = pos[1]; pz = pos[2];
       pdx = pushdir[0]; pdy = pushdir[1]; pdz = pushdir[2];
       if (go) { T.d[3][t] = dir[0]; T.d[4][t] = dir[1]; T.d[5][t] = dir[2]; chords_sum += chords; }
@@ -210,6 +211,7 @@ __device__ __forceinline__ void charged_lane(const DevCtx& c, const DevSlot& slo
           vol_post = static_cast<uint32_t>(nv);
           live = true; dest = 0;
           packed += 1ull << (8 * MC_BOUNDARY);
+          if (MULTI && BVH && cache) nav_cache_left_daughter(c, *cache, vol, nv, px, py, pz);
         }
       } else if (flag == 2) {
         live = true; dest = 0;
@@ -248,13 +250,20 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
   // one after the other, so a few hundred loopers packed into a few warps would take 32 x 16 chord queries
   // in sequence per step (measured 4 ms per population step on config 4), spread out they run in parallel.
   uint32_t g = kBlock;
-  while (g > 4 && (n + (g >> 1) - 1) / (g >> 1) <= gridDim.x) g >>= 1;
+  while (g > 4 && (n + (g >> 1) - 1) / (g >> 1) <= gridDim.x / 2) g >>= 1;   // (half the grid: the other species runs beside)
   const int lane_shift = __ffs(kBlock / g) - 1;            // every (1 << lane_shift)-th lane takes a track
   const uint32_t n_tiles = (n + g - 1) / g;
   if (blockIdx.x >= n_tiles) return;   // no tile for this block
   __shared__ BlockTally tally;
   __shared__ BlockReserve<ND> br;
   __shared__ TilePipe pipe;
+  // candidate lists of the chord queries in a BVH volume (geom.cuh NavCache): one per lane, kept across the
+  // tiles and steps of the launch
+  constexpr bool kLists = BVH;
+  __shared__ int32_t cand_lists[kLists ? kBlock * kCandCap : 1];
+  NavCache nav_cache;
+  nav_cache_reset(nav_cache);
+  NavCache* const cache = kLists ? &nav_cache : nullptr;
   tally_init(tally);
   pipe_init(pipe);
   double sum_dep = 0.0, sum_cut = 0.0;
@@ -264,7 +273,11 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
   const unsigned lt = (1u << lane) - 1u;
   const int t = threadIdx.x >> lane_shift;                 // this lane's entry of the tile
   const bool mine = (threadIdx.x & ((1u << lane_shift) - 1u)) == 0;
-  const int k_inner = MULTI ? min(inner_steps(c, n, gridDim.x * kBlock), 255) : 1;
+  int k_inner = MULTI ? min(inner_steps(c, n, gridDim.x * kBlock), 255) : 1;
+  // full GPU, BVH geometry: only the passage through the gap a track has just entered from a daughter is taken in
+  // the same launch (geom.cuh NavCache)
+  const bool transit_only = MULTI && BVH && k_inner == 1 && c.transit;
+  if (transit_only) k_inner = 2;
 
   if (threadIdx.x == 0) tile_issue_n(pipe.tile[0], cur, static_cast<size_t>(blockIdx.x) * g, g, &pipe.bar[0]);
   uint32_t k = 0;
@@ -277,15 +290,17 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
     ChargedLane r;
     r.px = 0.0; r.py = 0.0; r.pz = 0.0; r.vol_post = 0; r.live = false; r.has_ph = false; r.dest = -1;
     if (!MULTI) {
-      charged_lane<FIELD, BVH, false>(c, slot, tally, T, t, mine && tile * g + t < n, species, q0, packed, sum_dep, sum_cut, chords_sum, r);
+      charged_lane<FIELD, BVH, false>(c, slot, tally, T, t, mine && tile * g + t < n, species, q0, packed, sum_dep, sum_cut, chords_sum, r,
+                                      cache, cand_lists);
       if (k % 255u == 254u) move_counts_flush(tally, packed);
     } else {
       // A lane steps its track until it leaves the species buffer (interaction, stop, escape, ...) or has taken
       // k_inner steps; the warp goes round together because the navigator is warp-convergent.
       bool cont = mine && tile * g + t < n;
       for (int it = 0;; ++it) {
-        charged_lane<FIELD, BVH, true>(c, slot, tally, T, t, cont, species, q0, packed, sum_dep, sum_cut, chords_sum, r);
+        charged_lane<FIELD, BVH, true>(c, slot, tally, T, t, cont, species, q0, packed, sum_dep, sum_cut, chords_sum, r, cache, cand_lists);
         cont = cont && r.live && r.dest == 0 && it + 1 < k_inner;
+        if (transit_only) cont = cont && nav_cache.reach > 0.0 && nav_cache.vol == r.vol_post;
         if (!__any_sync(kFull, cont)) break;
       }
       move_counts_flush(tally, packed);

@@ -128,7 +128,8 @@ __device__ __forceinline__ void rk4(const DevCtx& c, int charge, double pmom, do
 // when a step needs more than one chord, and again when it is used up.
 template <int FIELD = -1, bool BVH = true>
 __device__ __forceinline__ int propagate(const DevCtx& c, int nav, bool active, int charge, double ekin, double pos[3], double dir[3],
-                         uint32_t vol, double s_phys, double& s_out, int& chords_out, double pushdir[3], int& face_out) {
+                         uint32_t vol, double s_phys, double& s_out, int& chords_out, double pushdir[3], int& face_out,
+                         NavCache* cache = nullptr, int32_t* cand = nullptr) {
   const int field_kind = FIELD >= 0 ? FIELD : c.field_kind;
   const double pmom = sqrt(ekin * (ekin + 2.0 * kMe));
   const double kappa = field_kind == ADEPT_FIELD_UNIFORM ? -charge * kCB * c.Bn / pmom : 0.0;
@@ -188,6 +189,7 @@ __device__ __forceinline__ int propagate(const DevCtx& c, int nav, bool active, 
           if (safe < h && !(last && safe < 0.0)) safe = nav_safety(c, vol, pos[0], pos[1], pos[2]);
           query = !(h < safe);
           safe = query ? -1.0 : safe - h;
+          if (cache && query && !last && cache->queries < 1) cache->queries = 1;   // a step of several chords: list at once
           if (query) {   // unit chord vector and length
             const double ch[3] = {p1[0] - pos[0], p1[1] - pos[1], p1[2] - pos[2]};
             const double L2 = ch[0] * ch[0] + ch[1] * ch[1] + ch[2] * ch[2];
@@ -200,7 +202,7 @@ __device__ __forceinline__ int propagate(const DevCtx& c, int nav, bool active, 
     }
     // --- warp-cooperative geometry query of this segment
     int face;
-    const double s_geo = nav_distance<BVH>(c, nav, query, pos[0], pos[1], pos[2], u[0], u[1], u[2], vol, L, face);
+    const double s_geo = nav_distance<BVH>(c, nav, query, pos[0], pos[1], pos[2], u[0], u[1], u[2], vol, L, face, cache, cand);
     if (query) face_hit = face;   // only meaningful when this segment ends on the boundary (flag 1), which ends the loop
     if (straight) {
       pushdir[0] = u[0]; pushdir[1] = u[1]; pushdir[2] = u[2];

@@ -54,7 +54,7 @@ struct GammaLane {
 
 template <bool BVH, bool MULTI, int N>
 __device__ __forceinline__ void gamma_lane(const DevCtx& c, const DevSlot& slot, BlockTally& tally, TrackTileT<N>& T, int t,
-                                           bool in_range, unsigned long long& packed, GammaLane& r) {
+                                           bool in_range, unsigned long long& packed, GammaLane& r, NavCache* cache = nullptr) {
   constexpr int species = ADEPT_GAMMA;
   enum { FATE_NONE = 0, FATE_KILLED, FATE_STOPPED, FATE_GO };
     const uint32_t vol = T.u[2][t];
@@ -101,7 +101,7 @@ __device__ __forceinline__ void gamma_lane(const DevCtx& c, const DevSlot& slot,
     int face = -1;
     {
       const double dx = T.d[3][t], dy = T.d[4][t], dz = T.d[5][t];
-      const double s_geo = nav_distance<BVH>(c, c.navigator, go, px, py, pz, dx, dy, dz, vol, s_phys, face);
+      const double s_geo = nav_distance<BVH>(c, c.navigator, go, px, py, pz, dx, dy, dz, vol, s_phys, face, cache);
       if (go) {
         cross = s_geo < s_phys;
         const double s = cross ? s_geo : s_phys;
@@ -139,6 +139,7 @@ __device__ __forceinline__ void gamma_lane(const DevCtx& c, const DevSlot& slot,
           post.vol = static_cast<uint32_t>(nv);
           live = true; dest = 0;
           packed += 1ull << (10 * GC_BOUNDARY);
+          if (MULTI && BVH && cache) nav_cache_left_daughter(c, *cache, vol, nv, px, py, pz);
         }
       } else if (process == ADEPT_OUT_PHOTO) {   // P3: no sampling involved, done here rather than staged
         const double BK = mat_scalar(c, mat, S_BK);
@@ -185,7 +186,14 @@ gamma_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevS
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const unsigned lt = (1u << lane) - 1u;
   const int t = threadIdx.x;
-  const int k_inner = MULTI ? min(inner_steps(c, n, gridDim.x * kBlock), 1023) : 1;
+  int k_inner = MULTI ? min(inner_steps(c, n, gridDim.x * kBlock), 1023) : 1;
+  // full GPU, BVH geometry: only the passage through the gap a track has just entered from a daughter is taken in
+  // the same launch (geom.cuh NavCache: the daughter's neighbour list answers its query without a traversal)
+  const bool transit_only = MULTI && BVH && k_inner == 1 && c.transit;
+  if (transit_only) k_inner = 2;
+  NavCache nav_cache;
+  nav_cache_reset(nav_cache);
+  NavCache* const cache = (MULTI && BVH) ? &nav_cache : nullptr;
 
   const uint32_t n_tiles = (n + kBlock - 1) / kBlock;
   if (t == 0 && blockIdx.x < n_tiles) tile_issue(pipe.tile[0], cur, blockIdx.x, &pipe.bar[0]);
@@ -207,11 +215,12 @@ gamma_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevS
       bool cont = tile * kBlock + t < n;
       for (int it = 0;; ++it) {
         GammaLane q;
-        gamma_lane<BVH, true>(c, slot, tally, pipe.tile[phase], t, cont, packed, q);
+        gamma_lane<BVH, true>(c, slot, tally, pipe.tile[phase], t, cont, packed, q, cache);
         score(slot, q.vol, q.edep, q.active);
         sum_cut += q.edep;
         if (q.active || it == 0) r = q;
         cont = q.active && q.live && q.dest == 0 && it + 1 < k_inner;
+        if (transit_only) cont = cont && nav_cache.reach > 0.0 && nav_cache.vol == q.post.vol;
         if (!__any_sync(kFull, cont)) break;
       }
       gamma_counts_flush(tally, packed);

@@ -154,6 +154,26 @@ __device__ __forceinline__ double entry_distance(const DevCtx& c, int vol, doubl
   return solid_entry(v, lp, ld);
 }
 
+// Entry distance into daughter `vol` for a segment of length s_max: the exact entry_distance when that is <= s_max,
+// else any value > s_max.  For a box the segment's extent along each local axis is compared with the slab first
+// (no division): a segment that stays clear of a slab by more than rounding cannot enter the box.
+__device__ __forceinline__ double entry_distance_within(const DevCtx& c, int vol, double px, double py, double pz, double dx,
+                                                        double dy, double dz, double s_max) {
+  const DevVolume& v = volume(c, vol);
+  double lp[3], ld[3];
+  to_local(c, vol, v, px, py, pz, lp);
+  dir_to_local(c, vol, v, dx, dy, dz, ld);
+  if (v.solid == ADEPT_BOX && s_max < 1.0e30) {
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      const double a = lp[i], b = lp[i] + s_max * ld[i];
+      const double pad = 1.0e-9 * (fabs(a) + fabs(b) + v.dims[i]);
+      if (fmin(a, b) > v.dims[i] + pad || fmax(a, b) < -v.dims[i] - pad) return ADEPT_INF;
+    }
+  }
+  return solid_entry(v, lp, ld);
+}
+
 // ---------------------------------------------------------------- warp-cooperative BVH
 __device__ __forceinline__ double warp_min(double v) {
 #pragma unroll
@@ -277,6 +297,107 @@ __device__ __forceinline__ int bvh_point(const DevCtx& c, const DevBvh& b, doubl
   return found == 0x7fffffff ? -1 : found;
 }
 
+// ---------------------------------------------------------------- candidate lists
+// Most queries in a BVH volume are asked from a place whose surroundings are already known.  A NavCache says:
+// "every daughter of `vol` that comes within `reach` of the point q0 is in `list`".  A segment from p of length
+// s can then only enter listed daughters if |p - q0| + s <= reach, so the query is a lane-local loop of exact
+// entry tests over the list -- no traversal, no warp cooperation -- and because the minimum is taken over a
+// superset of the daughters the traversal would test exactly, by the same entry_distance, the result is
+// bit-identical.  For a longer ray the list is tried first: a hit closer than reach - |p - q0| is final, else the
+// traversal starts from that bound.  Two sources of lists:
+//  * per daughter, built once by adept_init (DevBvh::nbr): the siblings within DevBvh::nbr_reach of the daughter's
+//    solid (and the daughter itself).  A track that has just left daughter A into the mother is within the push
+//    distance of A, so the list of A serves with reach = nbr_reach - margin around its exit point.  This is the
+//    crystal -> gap -> crystal passage, i.e. nearly every query of a shower in a barrel of crystals.
+//  * per lane, built on the spot by the warp (bvh_candidates) around a track that keeps asking from within a small
+//    ball: 16 chords per step, step after step, of the e+- that spiral in the gaps (profiles/r1e_configs34.md:
+//    82 % of the instructions of such a step were traversals).
+constexpr int kCandCap = 8;             // entries of a lane-built list (a gap corner touches 4 crystals)
+constexpr double kCandRadius = 0.25;    // [cm] radius of the ball a lane-built list covers
+constexpr int kNbrCap = 12;             // entries of a per-daughter list
+struct NavCache {
+  double qx, qy, qz, reach;             // see above (reach <= 0: no list)
+  const int32_t* list;
+  uint32_t vol;                         // the BVH volume the list belongs to
+  int count, queries;                   // entries; traversals made in `vol` since the last list
+};
+__device__ __forceinline__ void nav_cache_reset(NavCache& k) {
+  k.qx = k.qy = k.qz = 0.0; k.reach = -1.0; k.list = nullptr; k.vol = kDeadVolume; k.count = 0; k.queries = 0;
+}
+
+// A track has crossed from volume `from` into `into` at (x, y, z): if `from` is a daughter of the BVH volume `into`
+// with a neighbour list, that list serves the next queries.
+__device__ __forceinline__ void nav_cache_left_daughter(const DevCtx& c, NavCache& k, uint32_t from, int into, double x, double y, double z) {
+  if (into < 0) return;
+  const DevVolume& m = volume(c, into);
+  if (m.bvh < 0 || volume(c, from).mother != into) return;
+  const DevBvh& b = c.bvh[m.bvh];
+  if (b.nbr_reach <= 0.0) return;
+  const int d = static_cast<int>(from) - m.dbegin;
+  const int n = __ldg(b.nbr_count + d);
+  if (n < 0) return;
+  k.qx = x; k.qy = y; k.qz = z;
+  k.reach = b.nbr_reach - 1.0e-5;        // the exit point is within the push distance (and rounding) of `from`
+  k.list = b.nbr + static_cast<size_t>(d) * kNbrCap;
+  k.vol = static_cast<uint32_t>(into); k.count = n; k.queries = 0;
+}
+
+// All arguments warp-uniform; list = the requesting lane's kCandCap entries in shared memory.
+// Returns the number of daughters within rho of (px, py, pz), or -1 if they do not fit the list.
+__device__ __forceinline__ int bvh_candidates(const DevCtx& c, const DevBvh& b, double px, double py, double pz, double rho,
+                                              int32_t* list) {
+  const int lane = threadIdx.x & 31;
+  const unsigned lt = (1u << lane) - 1u;
+  const double pad = rho * (1.0 + 1.0e-9) + 1.0e-12;
+  const auto near_box = [&](const double* __restrict__ box, int stride, int i, bool valid) {
+    if (!valid) return false;
+    return px >= __ldg(box + i) - pad && py >= __ldg(box + stride + i) - pad && pz >= __ldg(box + 2 * stride + i) - pad &&
+           px <= __ldg(box + 3 * stride + i) + pad && py <= __ldg(box + 4 * stride + i) + pad && pz <= __ldg(box + 5 * stride + i) + pad;
+  };
+  const int top = b.n_levels - 1;
+  unsigned mask[kBvhMaxLevels];
+  int first[kBvhMaxLevels];
+  int level = top, count = 0;
+  first[top] = 0;
+  mask[top] = __ballot_sync(kFull, near_box(b.node_box[top], b.n_nodes[top], lane, lane < b.n_nodes[top]));
+  for (;;) {
+    if (mask[level] == 0) {
+      if (level == top) break;
+      ++level;
+      continue;
+    }
+    const int ch = __ffs(mask[level]) - 1;
+    mask[level] &= mask[level] - 1;
+    const int base = (first[level] + ch) << 5;
+    const int i = base + lane;
+    if (level == 0) {
+      bool ok = false;
+      int pv = -1;
+      if (near_box(b.prim_box, b.n_prims, i, i < b.n_prims)) {
+        pv = __ldg(b.prim_vol + i);
+        const DevVolume& v = volume(c, pv);
+        ok = true;
+        if (v.solid == ADEPT_BOX) {   // the oriented box itself, inflated
+          double l[3];
+          to_local(c, pv, v, px, py, pz, l);
+          ok = fabs(l[0]) <= v.dims[0] + pad && fabs(l[1]) <= v.dims[1] + pad && fabs(l[2]) <= v.dims[2] + pad;
+        }
+      }
+      const unsigned m = __ballot_sync(kFull, ok);
+      const int at = count + __popc(m & lt);
+      if (ok && at < kCandCap) list[at] = pv;
+      count += __popc(m);
+    } else {
+      const int n = b.n_nodes[level - 1];
+      first[level - 1] = base;
+      mask[level - 1] = __ballot_sync(kFull, near_box(b.node_box[level - 1], n, i, i < n));
+      --level;
+    }
+  }
+  __syncwarp();
+  return count <= kCandCap ? count : -1;
+}
+
 // ---------------------------------------------------------------- G3 distance to boundary
 // min(exit distance of the own solid, entry distance of every daughter), capped at s_max.
 // Warp-convergent call; lanes with active == false return s_max.
@@ -288,9 +409,13 @@ __device__ __forceinline__ int bvh_point(const DevCtx& c, const DevBvh& b, doubl
 // Inlined into the step kernels (3.7 % of a config-2 pass, 5 % of a config-4 pass, 20 % of the ray-cast over
 // calls: no argument moves, and the compiler schedules the box test into the surrounding phase), and so are
 // the cooperative traversals bvh_ray / bvh_point (another 5 % of a config-4 pass).
+// `cache` (BVH only, warp-uniformly null or not): the lane's candidate list (see above); `cand` (may be null): the
+// block's shared-memory room for lane-built lists -- with it, a lane that traverses twice in a row in the same
+// volume gets a list around its current point.
 template <bool BVH>
 __device__ __forceinline__ double nav_distance_body(const DevCtx& c, int nav, bool active, double px, double py, double pz, double dx,
-                               double dy, double dz, uint32_t vol, double s_max, int& face) {
+                               double dy, double dz, uint32_t vol, double s_max, int& face, NavCache* cache = nullptr,
+                               int32_t* cand = nullptr) {
   const int lane = threadIdx.x & 31;
   double s = s_max;
   bool need = false;
@@ -317,6 +442,17 @@ __device__ __forceinline__ double nav_distance_body(const DevCtx& c, int nav, bo
     }
   }
   if (!BVH) return s;
+  if (cache) {   // the lane's candidate list first (lane-local): final if the segment cannot leave its reach
+    if (need && cache->reach > 0.0 && cache->vol == vol) {
+      for (int j = 0; j < cache->count; ++j) {
+        const int pv = cache->list[j];
+        const double e = entry_distance_within(c, pv, px, py, pz, dx, dy, dz, s);
+        if (e <= s) { face = e < s ? -2 - pv : -1; s = e; }   // (a tie between two daughters: no hint, as in bvh_ray)
+      }
+      const double ox = px - cache->qx, oy = py - cache->qy, oz = pz - cache->qz;
+      if (sqrt(ox * ox + oy * oy + oz * oz) + s <= cache->reach * (1.0 - 1.0e-9)) need = false;
+    }
+  }
   unsigned m = __ballot_sync(kFull, need);
   while (m) {
     const int src = __ffs(m) - 1;
@@ -327,12 +463,35 @@ __device__ __forceinline__ double nav_distance_body(const DevCtx& c, int nav, bo
                              __shfl_sync(kFull, dy, src), __shfl_sync(kFull, dz, src), __shfl_sync(kFull, s, src), hit);
     if (lane == src && r < s) { s = r; face = hit >= 0 ? -2 - hit : -1; }
   }
+  if (cache) {   // a lane that keeps traversing in the same volume gets a list of its own around where it is
+    bool build = false;
+    if (need && cand) {
+      if (cache->vol != vol) { cache->vol = vol; cache->queries = 0; cache->reach = -1.0; }
+      build = ++cache->queries >= 2;
+    }
+    unsigned mb = __ballot_sync(kFull, build);
+    while (mb) {
+      const int src = __ffs(mb) - 1;
+      mb &= mb - 1;
+      int32_t* mine = cand + kCandCap * ((threadIdx.x & ~31) + src);
+      const int n = bvh_candidates(c, c.bvh[__shfl_sync(kFull, bvh, src)], __shfl_sync(kFull, px, src), __shfl_sync(kFull, py, src),
+                                   __shfl_sync(kFull, pz, src), kCandRadius, mine);
+      if (lane == src) {
+        cache->qx = px; cache->qy = py; cache->qz = pz;
+        cache->reach = n >= 0 ? kCandRadius : -1.0;
+        cache->list = mine;
+        cache->count = n >= 0 ? n : 0;
+        cache->queries = 0;
+      }
+    }
+  }
   return s;
 }
 template <bool BVH = true>
 __device__ __forceinline__ double nav_distance(const DevCtx& c, int nav, bool active, double px, double py, double pz, double dx,
-                                               double dy, double dz, uint32_t vol, double s_max, int& face) {
-  return nav_distance_body<BVH>(c, nav, active, px, py, pz, dx, dy, dz, vol, s_max, face);
+                                               double dy, double dz, uint32_t vol, double s_max, int& face, NavCache* cache = nullptr,
+                                               int32_t* cand = nullptr) {
+  return nav_distance_body<BVH>(c, nav, active, px, py, pz, dx, dy, dz, vol, s_max, face, cache, cand);
 }
 template <bool BVH = true>
 __device__ __forceinline__ double nav_distance(const DevCtx& c, int nav, bool active, double px, double py, double pz, double dx,

@@ -683,9 +683,12 @@ __global__ void __launch_bounds__(kBlock) raycast_kernel(const __grid_constant__
     bool alive = a && vol >= 0;
     double col = 0.0;
     int nx = alive ? 0 : -1;
+    NavCache cache;
+    nav_cache_reset(cache);
     while (__any_sync(kFull, alive)) {
       int face;
-      const double s = nav_distance(c, nav, alive, px, py, pz, dx, dy, dz, alive ? static_cast<uint32_t>(vol) : 0u, ADEPT_INF, face);
+      const double s = nav_distance(c, nav, alive, px, py, pz, dx, dy, dz, alive ? static_cast<uint32_t>(vol) : 0u, ADEPT_INF, face,
+                                    &cache);
       if (alive) {
         col += s * mat_scalar(c, volume(c, vol).material, S_RHO);
         px += s * dx; py += s * dy; pz += s * dz;
@@ -694,6 +697,7 @@ __global__ void __launch_bounds__(kBlock) raycast_kernel(const __grid_constant__
       const int nv = nav_relocate(c, nav, alive, alive ? static_cast<uint32_t>(vol) : 0u, px, py, pz, face);
       if (alive) {
         ++nx;
+        if (nav == ADEPT_NAV_BVH) nav_cache_left_daughter(c, cache, static_cast<uint32_t>(vol), nv, px, py, pz);
         vol = nv;
         if (nv < 0 || nx >= max_crossings) alive = false;
       }

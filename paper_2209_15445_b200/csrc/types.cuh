@@ -53,6 +53,11 @@ struct DevBvh {
   const double* prim_box;            // [6][n_prims]
   const int32_t* prim_vol;           // [n_prims] touchable id
   const double* node_box[kBvhMaxLevels];  // [6][n_nodes[L]]
+  // per-daughter neighbour lists (geom.cuh NavCache): for daughter d (index relative to the volume's first
+  // daughter) the touchable ids of the siblings within nbr_reach of its solid, itself included
+  const int32_t* nbr;                // [n_prims][kNbrCap]
+  const int32_t* nbr_count;          // [n_prims] entries, -1 = the list did not fit
+  double nbr_reach;                  // [cm], <= 0: no lists
 };
 
 // One species' track buffer, structure of arrays (76 B per track).
@@ -131,6 +136,8 @@ struct DevCtx {
   int32_t chord_budget;
   uint32_t seed, max_steps;
   int32_t steps_per_launch; // adept_config::steps_per_launch (0 = automatic, kernels.cuh inner_steps)
+  int32_t transit;          // 1: BVH volumes have per-daughter neighbour lists: a track that leaves a daughter into such a
+                            // (vacuum) mother takes the step across the gap in the same launch, whatever the population
   uint32_t capacity;        // per species per buffer
   uint32_t stage_capacity;  // per interaction queue
   uint32_t leak_capacity;
