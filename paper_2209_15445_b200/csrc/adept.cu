@@ -592,6 +592,7 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   for (int k = 0; k < 3; ++k) d.bhat[k] = d.Bn > 0.0 ? f->B[k] / d.Bn : 0.0;
   d.nr = f->nr; d.nz = f->nz; d.r0 = f->r0; d.z0 = f->z0; d.dr = f->dr; d.dz = f->dz; d.bz = L.bz;
   d.inv_dr = f->dr > 0.0 ? 1.0 / f->dr : 0.0; d.inv_dz = f->dz > 0.0 ? 1.0 / f->dz : 0.0;
+  d.fr_max = f->nr - 1; d.fz_max = f->nz - 1;
   d.u0 = std::log(1.0e-3);
   d.du = (std::log(1.0e8) - std::log(1.0e-3)) / (kNGrid - 1);
   d.inv_du = 1.0 / d.du;

@@ -23,8 +23,8 @@ __device__ __forceinline__ void field_at(const DevCtx& c, const double p[3], dou
   // (grid coordinates by multiplication with the inverse spacing: exact for the 1 cm grid of the configs, within
   // an ulp otherwise, and the interpolant is continuous across cells)
   double fr = (r - c.r0) * c.inv_dr, fz = (p[2] - c.z0) * c.inv_dz;
-  fr = fmin(fmax(fr, 0.0), static_cast<double>(c.nr - 1));
-  fz = fmin(fmax(fz, 0.0), static_cast<double>(c.nz - 1));
+  fr = fmin(fmax(fr, 0.0), c.fr_max);
+  fz = fmin(fmax(fz, 0.0), c.fz_max);
   const int ir = min(static_cast<int>(fr), c.nr - 2);
   const int iz = min(static_cast<int>(fz), c.nz - 2);
   const double a = fr - ir, b = fz - iz;
@@ -135,7 +135,8 @@ __device__ __forceinline__ int propagate(const DevCtx& c, int nav, bool active, 
   const double kappa = field_kind == ADEPT_FIELD_UNIFORM ? -charge * kCB * c.Bn / pmom : 0.0;
   const double inv_kappa = kappa != 0.0 ? 1.0 / kappa : 0.0;
   double s_done = 0.0;
-  double safe = -1.0;   // clearance known to be left around pos (< 0: not known)
+  double safe = -1.0;   // clearance known to be left around pos (< 0: not known) ...
+  bool own_only = false; // ... to the volume's own surface only (its daughters sit in a BVH)
   double h_step = -1.0; // uniform field: the chord length limit of this step (< 0: not yet known)
   int chords = 0, flag = 0, face_hit = -1;
   bool running = active;
@@ -143,7 +144,7 @@ __device__ __forceinline__ int propagate(const DevCtx& c, int nav, bool active, 
   for (int i = 0; i < 3; ++i) pushdir[i] = dir[i];
   while (__any_sync(kFull, running)) {
     // --- per-lane: decide the next segment
-    bool query = false, straight = false, last = false, chord = false;
+    bool query = false, straight = false, last = false, chord = false, skip_own = false;
     double h = 0.0, L = 0.0, rest = 0.0;
     double u[3] = {0.0, 0.0, 0.0}, p1[3], d1[3], B[3] = {0.0, 0.0, 0.0};
     if (running) {
@@ -186,9 +187,11 @@ __device__ __forceinline__ int propagate(const DevCtx& c, int nav, bool active, 
           chord = true;
           // the chord needs no geometry query if it is shorter than the clearance left (a chord's length never
           // exceeds its arc's, so h bounds it)
-          if (safe < h && !(last && safe < 0.0)) safe = nav_safety(c, vol, pos[0], pos[1], pos[2]);
-          query = !(h < safe);
-          safe = query ? -1.0 : safe - h;
+          if (safe < h && !(last && safe < 0.0)) safe = nav_safety(c, vol, pos[0], pos[1], pos[2], own_only);
+          const bool clear = h < safe;
+          query = !clear || own_only;      // (own_only: the daughters still have to be asked, the own solid not)
+          skip_own = clear;
+          safe = clear ? safe - h : -1.0;
           if (cache && query && !last && cache->queries < 1) cache->queries = 1;   // a step of several chords: list at once
           if (query) {   // unit chord vector and length
             const double ch[3] = {p1[0] - pos[0], p1[1] - pos[1], p1[2] - pos[2]};
@@ -202,7 +205,7 @@ __device__ __forceinline__ int propagate(const DevCtx& c, int nav, bool active, 
     }
     // --- warp-cooperative geometry query of this segment
     int face;
-    const double s_geo = nav_distance<BVH>(c, nav, query, pos[0], pos[1], pos[2], u[0], u[1], u[2], vol, L, face, cache, cand);
+    const double s_geo = nav_distance<BVH>(c, nav, query, pos[0], pos[1], pos[2], u[0], u[1], u[2], vol, L, face, cache, cand, skip_own);
     if (query) face_hit = face;   // only meaningful when this segment ends on the boundary (flag 1), which ends the loop
     if (straight) {
       pushdir[0] = u[0]; pushdir[1] = u[1]; pushdir[2] = u[2];

@@ -415,7 +415,7 @@ __device__ __forceinline__ int bvh_candidates(const DevCtx& c, const DevBvh& b, 
 template <bool BVH>
 __device__ __forceinline__ double nav_distance_body(const DevCtx& c, int nav, bool active, double px, double py, double pz, double dx,
                                double dy, double dz, uint32_t vol, double s_max, int& face, NavCache* cache = nullptr,
-                               int32_t* cand = nullptr) {
+                               int32_t* cand = nullptr, bool skip_own = false) {
   const int lane = threadIdx.x & 31;
   double s = s_max;
   bool need = false;
@@ -423,12 +423,14 @@ __device__ __forceinline__ double nav_distance_body(const DevCtx& c, int nav, bo
   face = -1;
   if (active) {
     const DevVolume& v = volume(c, vol);
-    double lp[3], ld[3];
-    to_local(c, vol, v, px, py, pz, lp);
-    dir_to_local(c, vol, v, dx, dy, dz, ld);
-    int f;
-    const double s_exit = solid_exit(v, lp, ld, f);
-    if (s_exit < s_max) { s = s_exit; face = f; }
+    if (!skip_own) {   // (skip_own: the caller knows the segment ends before the volume's own surface, nav_safety)
+      double lp[3], ld[3];
+      to_local(c, vol, v, px, py, pz, lp);
+      dir_to_local(c, vol, v, dx, dy, dz, ld);
+      int f;
+      const double s_exit = solid_exit(v, lp, ld, f);
+      if (s_exit < s_max) { s = s_exit; face = f; }
+    }
     if (v.dcount > 0) {
       if (BVH && nav == ADEPT_NAV_BVH && v.bvh >= 0) {
         need = true;
@@ -490,8 +492,8 @@ __device__ __forceinline__ double nav_distance_body(const DevCtx& c, int nav, bo
 template <bool BVH = true>
 __device__ __forceinline__ double nav_distance(const DevCtx& c, int nav, bool active, double px, double py, double pz, double dx,
                                                double dy, double dz, uint32_t vol, double s_max, int& face, NavCache* cache = nullptr,
-                                               int32_t* cand = nullptr) {
-  return nav_distance_body<BVH>(c, nav, active, px, py, pz, dx, dy, dz, vol, s_max, face, cache, cand);
+                                               int32_t* cand = nullptr, bool skip_own = false) {
+  return nav_distance_body<BVH>(c, nav, active, px, py, pz, dx, dy, dz, vol, s_max, face, cache, cand, skip_own);
 }
 template <bool BVH = true>
 __device__ __forceinline__ double nav_distance(const DevCtx& c, int nav, bool active, double px, double py, double pz, double dx,
@@ -507,7 +509,8 @@ __device__ __forceinline__ double nav_distance(const DevCtx& c, int nav, bool ac
 // -- the result of the step is the same with or without it (the oracle has no safety at all).  Conservative by
 // construction: distances to the own surface are exact or under-estimated, a daughter's is bounded by the
 // largest per-axis separation (<= the Euclidean distance); 1e-6 relative and 1e-9 cm are taken off for
-// rounding.  Lane-local.  0 for a volume whose daughters sit in a BVH (no cheap bound).
+// rounding.  Lane-local.  For a volume whose daughters sit in a BVH there is no cheap bound on them: `own_only` is
+// set and the value bounds the distance to the volume's own surface only (the query then skips the own solid).
 __device__ __forceinline__ double solid_safety_in(const DevVolume& v, const double p[3]) {
   if (v.solid == ADEPT_BOX) return fmin(fmin(v.dims[0] - fabs(p[0]), v.dims[1] - fabs(p[1])), v.dims[2] - fabs(p[2]));
   const double r = sqrt(p[0] * p[0] + p[1] * p[1]);
@@ -520,13 +523,13 @@ __device__ __forceinline__ double solid_safety_out(const DevVolume& v, const dou
   const double r = sqrt(p[0] * p[0] + p[1] * p[1]);
   return fmax(fmax(r - v.dims[1], v.dims[0] - r), fabs(p[2]) - v.dims[2]);
 }
-__device__ __forceinline__ double nav_safety(const DevCtx& c, uint32_t vol, double px, double py, double pz) {
+__device__ __forceinline__ double nav_safety(const DevCtx& c, uint32_t vol, double px, double py, double pz, bool& own_only) {
   const DevVolume& v = volume(c, vol);
-  if (v.dcount > 0 && v.bvh >= 0) return 0.0;
   double l[3];
   to_local(c, vol, v, px, py, pz, l);
   double s = solid_safety_in(v, l);
-  for (int k = 0; k < v.dcount && s > 0.0; ++k) {
+  own_only = v.dcount > 0 && v.bvh >= 0;
+  for (int k = 0; !own_only && k < v.dcount && s > 0.0; ++k) {
     const DevVolume& d = volume(c, v.dbegin + k);
     to_local(c, v.dbegin + k, d, px, py, pz, l);
     s = fmin(s, solid_safety_out(d, l));

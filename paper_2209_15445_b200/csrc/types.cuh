@@ -129,7 +129,7 @@ struct DevCtx {
   double B[3];
   double Bn, bhat[3];       // |B| and B / |B| of a uniform field (adept_init)
   int32_t nr, nz;
-  double r0, z0, dr, dz, inv_dr, inv_dz;
+  double r0, z0, dr, dz, inv_dr, inv_dz, fr_max, fz_max;   // (fr_max = nr - 1, fz_max = nz - 1 as doubles)
   const double* bz;
   double u0, inv_du, du;
   double delta_chord, eps_push, alpha_R, rho_R;
