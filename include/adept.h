@@ -83,8 +83,17 @@ typedef struct {
  * e+ {brem, Bhabha, annihilation, dE/dx, range}.  Macroscopic cross sections in 1/cm. */
 #define ADEPT_N_TABLES 12
 #define ADEPT_N_GRID 2048
+#define ADEPT_MAX_ELEMENTS 4
 typedef struct {
   const double* data; /* [n_materials][12][2048] */
+  /* Compound materials ("element selector"; DESIGN.md §3 C1-C5).  The tables above
+   * hold the sums over the elements of each material.  Where the final state depends on the target element -- the
+   * K-shell binding energy of a photoelectric absorption -- the element is sampled with uniform U6 of the step
+   * against the cumulative shares below, interpolated in ln T like every table.  All three NULL: every material
+   * is a single element (the binding energy is adept_material::B_K, nothing is drawn). */
+  const int32_t* n_elem; /* [n_materials]          elements of the material, 1..ADEPT_MAX_ELEMENTS              */
+  const double* elem_bk; /* [n_materials][4]       K-shell binding energy of each element [MeV]                 */
+  const double* pe_cum;  /* [n_materials][2048][4] share of elements 0..j in Sigma_photo at each grid node      */
 } adept_tables;
 
 /* Magnetic field.  MAP_RZ: B = (0, 0, bz(r, z)), bilinear, clamped outside. */

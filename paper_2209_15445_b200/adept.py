@@ -32,7 +32,7 @@ class CGeometry(C.Structure):
 
 
 class CTables(C.Structure):
-    _fields_ = [("data", _dp)]
+    _fields_ = [("data", _dp), ("n_elem", _ip), ("elem_bk", _dp), ("pe_cum", _dp)]
 
 
 class CField(C.Structure):
@@ -150,8 +150,9 @@ class Adept:
     """One library context.  `geom`, `field` come from paper_2209_15445_b200.inputs; `scalars` is
     (n_mat, 8) and `tables` (n_mat, 12, 2048) as built by inputs.materials.build_material_set."""
 
-    def __init__(self, geom, tables, scalars, field, device="cuda:0", _workspace_bytes=None, **config):
-        """_workspace_bytes (tests): size of the workspace handed to adept_init instead of adept_workspace_bytes()."""
+    def __init__(self, geom, tables, scalars, field, device="cuda:0", _workspace_bytes=None, elements=None, **config):
+        """elements: None, or (n_elem, elem_bk, pe_cum) from inputs.materials.element_tables for compound materials.
+        _workspace_bytes (tests): size of the workspace handed to adept_init instead of adept_workspace_bytes()."""
         import torch
         self._torch = torch
         self.device = torch.device(device)
@@ -165,7 +166,16 @@ class Adept:
                       geom.material.ctypes.data_as(_ip), geom.mother.ctypes.data_as(_ip),
                       geom.daughter_begin.ctypes.data_as(_ip), geom.daughter_count.ctypes.data_as(_ip),
                       geom.rot.ctypes.data_as(_dp), geom.trans.ctypes.data_as(_dp))
-        t = CTables(self._keep[1].ctypes.data_as(_dp))
+        if elements is None:
+            t = CTables(self._keep[1].ctypes.data_as(_dp), None, None, None)
+        else:
+            el = [np.ascontiguousarray(elements[0], dtype=np.int32), np.ascontiguousarray(elements[1], dtype=np.float64),
+                  np.ascontiguousarray(elements[2], dtype=np.float64)]
+            n_mat_ = self._keep[2].shape[0]
+            assert el[0].shape == (n_mat_,) and el[1].shape == (n_mat_, 4) and el[2].shape == (n_mat_, 2048, 4)
+            self._keep += el
+            t = CTables(self._keep[1].ctypes.data_as(_dp), el[0].ctypes.data_as(_ip), el[1].ctypes.data_as(_dp),
+                        el[2].ctypes.data_as(_dp))
         f = CField(field.kind, (C.c_double * 3)(*field.B), field.nr, field.nz, field.r0, field.z0, field.dr,
                    field.dz, self._keep[3].ctypes.data_as(_dp))
         n_mat = self._keep[2].shape[0]

@@ -379,6 +379,7 @@ int validate(const adept_config* cfg, const adept_geometry* g, int n_mats, const
 
 struct Layout {
   DevVolume* vol; double* rot; int32_t* nbr; int32_t* rhint; DevBvh* bvh; double *tab_g, *tab_em, *tab_ep, *scal, *bz;
+  int32_t* n_elem; double *elem_bk, *pe_cum;
   std::vector<double*> bvh_prim_box; std::vector<int32_t*> bvh_prim_vol; std::vector<std::vector<double*>> bvh_node_box;
   std::vector<int32_t*> bvh_nbr, bvh_nbr_count;
   adept_track* stage; uint32_t* bad; size_t stage_cap;
@@ -413,6 +414,9 @@ size_t carve(void* base, const adept_config* cfg, const adept_geometry* g, int n
   L.tab_ep = cv.take<double>(static_cast<size_t>(n_mats) * kNGrid * kRowEp);
   L.scal = cv.take<double>(static_cast<size_t>(n_mats) * N_SCAL);
   L.rhint = cv.take<int32_t>(static_cast<size_t>(n_mats) * 2 * kHintStride);
+  L.n_elem = cv.take<int32_t>(n_mats);
+  L.elem_bk = cv.take<double>(static_cast<size_t>(n_mats) * ADEPT_MAX_ELEMENTS);
+  L.pe_cum = cv.take<double>(static_cast<size_t>(n_mats) * kNGrid * ADEPT_MAX_ELEMENTS);
   L.bz = cv.take<double>(f->kind == ADEPT_FIELD_MAP_RZ ? static_cast<size_t>(f->nr) * f->nz : 1);
   L.stage_cap = std::min<size_t>(cfg->track_capacity, 1u << 20);
   L.stage = cv.take<adept_track>(L.stage_cap);
@@ -576,6 +580,17 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   }
   if (f->kind == ADEPT_FIELD_MAP_RZ)
     CUDA_TRY(cudaMemcpy(L.bz, f->bz, static_cast<size_t>(f->nr) * f->nz * sizeof(double), cudaMemcpyHostToDevice));
+  // element selector of compound materials (all three arrays or none)
+  const bool compounds = tables->n_elem && tables->elem_bk && tables->pe_cum;
+  if (!compounds && (tables->n_elem || tables->elem_bk || tables->pe_cum))
+    return fail(ADEPT_EINVAL, "adept_tables: n_elem, elem_bk and pe_cum must be given together");
+  if (compounds) {
+    for (int m = 0; m < n_mats; ++m)
+      if (tables->n_elem[m] < 1 || tables->n_elem[m] > ADEPT_MAX_ELEMENTS) return fail(ADEPT_EINVAL, "material %d: n_elem out of range", m);
+    CUDA_TRY(cudaMemcpy(L.n_elem, tables->n_elem, static_cast<size_t>(n_mats) * sizeof(int32_t), cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaMemcpy(L.elem_bk, tables->elem_bk, static_cast<size_t>(n_mats) * ADEPT_MAX_ELEMENTS * sizeof(double), cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaMemcpy(L.pe_cum, tables->pe_cum, static_cast<size_t>(n_mats) * kNGrid * ADEPT_MAX_ELEMENTS * sizeof(double), cudaMemcpyHostToDevice));
+  }
 
   adept_ctx* ctx = new (std::nothrow) adept_ctx;
   if (!ctx) return fail(ADEPT_ENOMEM, "host allocation failed");
@@ -586,6 +601,7 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   DevCtx& d = ctx->dev;
   d.vol = L.vol; d.rot = L.rot; d.nbr = L.nbr; d.n_vol = nv; d.bvh = L.bvh; d.navigator = cfg->navigator;
   d.tab_g = L.tab_g; d.tab_em = L.tab_em; d.tab_ep = L.tab_ep; d.scal = L.scal; d.rhint = L.rhint; d.n_mat = n_mats;
+  d.n_elem = compounds ? L.n_elem : nullptr; d.elem_bk = L.elem_bk; d.pe_cum = L.pe_cum;
   d.field_kind = f->kind;
   for (int k = 0; k < 3; ++k) d.B[k] = f->B[k];
   d.Bn = std::sqrt(f->B[0] * f->B[0] + f->B[1] * f->B[1] + f->B[2] * f->B[2]);

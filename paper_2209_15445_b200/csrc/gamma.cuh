@@ -142,7 +142,7 @@ __device__ __forceinline__ void gamma_lane(const DevCtx& c, const DevSlot& slot,
           if (MULTI && BVH && cache) nav_cache_left_daughter(c, *cache, vol, nv, px, py, pz);
         }
       } else if (process == ADEPT_OUT_PHOTO) {   // P3: no sampling involved, done here rather than staged
-        const double BK = mat_scalar(c, mat, S_BK);
+        const double BK = photo_binding(c, mat, post.ekin, post.event, post.id, post.step - 1);
         if (post.ekin > BK) {
           edep = BK;
           T_pe = post.ekin - BK;

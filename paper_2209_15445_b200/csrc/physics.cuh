@@ -101,6 +101,26 @@ __device__ __forceinline__ void emit(const DevCtx& c, int mat, StepOut& o, int s
   o.n_sec += 1;
 }
 
+// C5 element selector: the K-shell binding energy of the element a photon of energy k is absorbed on.
+// In a compound that is element j with probability n_j sigma_j(k) / Sigma_photo(k): U6 of the step's stream (a
+// spare slot of R3) against the cumulative shares, which are tabulated on the grid and interpolated like every
+// table (M7); the first j with U6 < c_j, else the last element.  A single-element material draws nothing.
+__device__ __forceinline__ double photo_binding(const DevCtx& c, int mat, double k, uint32_t event, uint64_t id, uint32_t step) {
+  const int n = c.n_elem ? __ldg(c.n_elem + mat) : 1;
+  if (n <= 1) return mat_scalar(c, mat, S_BK);
+  const GridPos gp = grid_pos(c, k);
+  const double* tab = c.pe_cum + (static_cast<size_t>(mat) * kNGrid + gp.i) * 4;
+  const Row4 r0 = load_row4(tab), r1 = load_row4(tab + 4);
+  Stream u;
+  u.init(event, c.seed, id, step);
+  const double u6 = u.uniform(6);
+  int j = n - 1;
+#pragma unroll
+  for (int e = 2; e >= 0; --e)
+    if (e < n - 1 && u6 < lerp_col(r0, r1, e, gp.f)) j = e;
+  return __ldg(c.elem_bk + mat * 4 + j);
+}
+
 // ---- P1 Klein-Nishina Compton
 __device__ __forceinline__ void compton(const DevCtx& c, int mat, StepOut& o, Stream& u) {
   Track& g = o.post;
@@ -161,10 +181,10 @@ __device__ __forceinline__ void pair_production(const DevCtx& c, int mat, StepOu
   o.alive = 0;
 }
 
-// ---- P3 photoelectric, K shell
-__device__ void photoelectric(const DevCtx& c, int mat, StepOut& o) {
+// ---- P3 photoelectric, K shell; `step` = the step the absorption happens in (its stream selects the element)
+__device__ void photoelectric(const DevCtx& c, int mat, StepOut& o, uint32_t step) {
   Track& g = o.post;
-  const double k = g.ekin, BK = mat_scalar(c, mat, S_BK);
+  const double k = g.ekin, BK = photo_binding(c, mat, k, g.event, g.id, step);
   if (k > BK) {
     o.edep_cut += BK;
     const double d0[3] = {g.dx, g.dy, g.dz};
@@ -307,7 +327,7 @@ __device__ __forceinline__ void run_process(const DevCtx& c, int process, int sp
   switch (process) {
     case ADEPT_OUT_COMPTON: compton(c, mat, o, u); break;
     case ADEPT_OUT_PAIR: pair_production(c, mat, o, u); break;
-    case ADEPT_OUT_PHOTO: photoelectric(c, mat, o); break;
+    case ADEPT_OUT_PHOTO: photoelectric(c, mat, o, u.c2); break;
     case ADEPT_OUT_BREM: open = bremsstrahlung(c, mat, o, u); break;
     case ADEPT_OUT_IONI: open = species == ADEPT_ELECTRON ? moller(c, mat, o, u) : bhabha(c, mat, o, u); break;
     case ADEPT_OUT_ANNI: annihilation(c, mat, o, u); break;

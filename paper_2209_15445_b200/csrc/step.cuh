@@ -167,7 +167,7 @@ __device__ int step_move(const DevCtx& c, int nav, bool active, const Track& in,
     if (u1 * stot < x0) process = ADEPT_OUT_COMPTON;
     else if (u1 * stot < x0 + x1) process = ADEPT_OUT_PAIR;
     if (process == ADEPT_OUT_PHOTO) {  // no sampling involved: done here rather than staged (12 % of all steps)
-      photoelectric(c, mat, o);
+      photoelectric(c, mat, o, in.step);
       o.outcome = ADEPT_OUT_PHOTO;
       return NEXT_NONE;
     }

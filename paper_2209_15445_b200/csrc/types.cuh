@@ -124,6 +124,9 @@ struct DevCtx {
   const double* tab_ep;     // [n_mat][2048][kRowEp]
   const double* scal;       // [n_mat][N_SCAL]
   const int32_t* rhint;     // [n_mat][2 (e-, e+)][kHintStride] inverse-range search hints (physics.cuh)
+  const int32_t* n_elem;    // [n_mat] elements per material, nullptr = single elements only (physics.cuh photo_binding)
+  const double* elem_bk;    // [n_mat][4] K-shell binding energy per element
+  const double* pe_cum;     // [n_mat][2048][4] cumulative shares of the elements in the photoelectric cross section
   int32_t n_mat;
   int32_t field_kind;
   double B[3];

@@ -74,11 +74,12 @@ def calorimeter(n_layers=50, t_abs=0.23, t_gap=0.57):
     return _finish(solid, dims, material, mother, rot, trans, ["vacuum", "Pb", "LAr"], "calorimeter")
 
 
-def barrel(n_eta=170, n_phi=360, n_shells=10):
+def barrel(n_eta=170, n_phi=360, n_shells=10, crystal="PbWO4"):
     """Configs 4-5 (BASELINE.json:configs[3]; SURVEY.md §8(d) cfg 4).
 
     Volumes: 0 world tube, 1..10 Si shells, 11 ECAL mother tube, 12 + i*n_phi + j crystal (row i, col j).
-    Materials: 0 vacuum, 1 Si, 2 PbWO4 (effective Z=73).
+    Materials: 0 vacuum, 1 Si, 2 `crystal`: "PbWO4" (the effective element Z=73 of BASELINE.json:configs[3]) or
+    "PbWO4_true" (the compound Pb + W + 4 O).
     """
     solid, dims, material, mother, trans, rot = [], [], [], [], [], []
     eye = np.eye(3)
@@ -108,4 +109,4 @@ def barrel(n_eta=170, n_phi=360, n_shells=10):
             R = np.stack([xh, yh, a], axis=1)            # columns = local axes
             add(BOX, (1.1, 1.1, 11.5), 2, mom, front + 11.5 * a, R)
     return _finish(solid, dims, material, mother, np.stack(rot), trans,
-                   ["vacuum", "Si", "PbWO4"], "barrel")
+                   ["vacuum", "Si", crystal], "barrel")

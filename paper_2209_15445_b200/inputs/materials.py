@@ -33,9 +33,13 @@ class Material:
     X0: float = math.inf        # [cm]
     I: float = 0.0              # [MeV]
     hwp: float = 0.0            # plasma energy [MeV]
-    B_K: float = 0.0            # K-shell binding [MeV]
+    B_K: float = 0.0            # K-shell binding [MeV] (compound: of its first element)
     e_cut: float = 0.0          # T_c [MeV]
     g_cut: float = 0.0          # k_c [MeV]
+    # compounds (DESIGN.md §3 C1-C5): per element (Z, A, atoms per formula unit), number density, B_K
+    elements: tuple = ()
+    n_i: tuple = ()
+    B_K_i: tuple = ()
 
     @property
     def vacuum(self):
@@ -43,7 +47,7 @@ class Material:
 
 
 def make_material(name, Z, A, rho):
-    """M1-M3: densities, Tsai radiation length, mean excitation energy, plasma energy, B_K."""
+    """M1-M3: densities, Tsai radiation length, mean excitation energy, plasma energy, B_K (one element)."""
     mat = Material(name, float(Z), float(A), float(rho))
     if mat.vacuum:
         return mat
@@ -63,9 +67,47 @@ def make_material(name, Z, A, rho):
     return mat
 
 
-# the materials BASELINE.json:configs names (A_eff of the PbWO4 stand-in: SURVEY.md M1)
+def _tsai_per_atom(Z):
+    a2 = (ALPHA * Z) ** 2
+    f_c = a2 * (1.0 / (1.0 + a2) + 0.20206 - 0.0369 * a2 + 0.0083 * a2 ** 2 - 0.002 * a2 ** 3)
+    return Z * Z * (math.log(184.15 * Z ** (-1.0 / 3.0)) - f_c) + Z * math.log(1194.0 * Z ** (-2.0 / 3.0))
+
+
+def _mean_excitation(Z):
+    return (Z * (12.0 + 7.0 / Z) if Z < 13 else Z * (9.76 + 58.8 * Z ** (-1.19))) * 1.0e-6
+
+
+def make_compound(name, elements, rho):
+    """C1-C3: a compound of (Z, A, atoms per formula unit) triples.  Number densities n_i = N_A rho nu_i / A_mol;
+    1/X0 additive over the atoms (Tsai); ln I = sum n_i Z_i ln I_i / n_el (Bragg); plasma energy from the total
+    electron density."""
+    elements = tuple((float(z), float(a), float(nu)) for z, a, nu in elements)
+    a_mol = sum(nu * a for _, a, nu in elements)
+    z_mol = sum(nu * z for z, _, nu in elements)
+    mat = Material(name, z_mol / sum(nu for _, _, nu in elements), a_mol, float(rho), elements=elements)
+    mat.n_i = tuple(N_AVOGADRO * rho * nu / a_mol for _, _, nu in elements)
+    mat.n_at = sum(mat.n_i)
+    mat.n_el = sum(n * z for n, (z, _, _) in zip(mat.n_i, elements))
+    mat.X0 = 1.0 / sum(4.0 * ALPHA * R_E ** 2 * n * _tsai_per_atom(z) for n, (z, _, _) in zip(mat.n_i, elements))
+    mat.I = math.exp(sum(n * z * math.log(_mean_excitation(z)) for n, (z, _, _) in zip(mat.n_i, elements)) / mat.n_el)
+    mat.hwp = 28.816e-6 * math.sqrt(rho * z_mol / a_mol)
+    mat.B_K_i = tuple(RYDBERG_EV * 1.0e-6 * (z - 1.0) ** 2 for z, _, _ in elements)
+    mat.B_K = mat.B_K_i[0]
+    return mat
+
+
+def photo_macro(mat, k):
+    """Macroscopic photoelectric cross section [1/cm]: sum over the elements of a compound."""
+    if mat.elements:
+        return sum(n * sigma_photo_atom(k, z) for n, (z, _, _) in zip(mat.n_i, mat.elements))
+    return mat.n_at * sigma_photo_atom(k, mat.Z)
+
+
+# the materials BASELINE.json:configs names (A_eff of the PbWO4 stand-in: SURVEY.md M1); "PbWO4_true" is the real
+# compound (PAPER.md:61), Pb + W + 4 O
 def standard_materials():
     return {
+        "PbWO4_true": make_compound("PbWO4_true", [(82.0, 207.2, 1), (74.0, 183.84, 1), (8.0, 15.999, 4)], 8.28),
         "vacuum": make_material("vacuum", 0.0, 0.0, 0.0),
         "Pb": make_material("Pb", 82.0, 207.2, 11.35),
         "LAr": make_material("LAr", 18.0, 39.95, 1.396),
@@ -210,7 +252,7 @@ def compute_cuts(mat):
         j = int(np.searchsorted(R, PRODUCTION_CUT_CM, side="right")) - 1
         e_cut = math.exp(_interp_crossing_lnT(U0 + DU * j, R[j], R[j + 1], PRODUCTION_CUT_CM))
     # gamma: falling low-energy branch where 5 / Sigma_tot = cut
-    sig = mat.n_el * sigma_compton(T) + pair_shape(T) / mat.X0 + mat.n_at * sigma_photo_atom(T, mat.Z)
+    sig = mat.n_el * sigma_compton(T) + pair_shape(T) / mat.X0 + photo_macro(mat, T)
     target = 5.0 / PRODUCTION_CUT_CM
     if sig[0] <= target:
         g_cut = T_GRID_MIN
@@ -231,7 +273,7 @@ def build_tables(mat):
     T = energy_grid()
     tab[TAB_G_COMPTON] = mat.n_el * sigma_compton(T)
     tab[TAB_G_PAIR] = pair_shape(T) / mat.X0
-    tab[TAB_G_PHOTO] = mat.n_at * sigma_photo_atom(T, mat.Z)
+    tab[TAB_G_PHOTO] = photo_macro(mat, T)
     brem = brem_shape(T, mat.g_cut) / mat.X0
     srad = srad_shape(T, mat.g_cut) / mat.X0
     tab[TAB_EM_BREM] = brem
@@ -253,6 +295,33 @@ def material_scalars(mat):
     """Per-material scalar block of the C ABI: X0, T_c, k_c, B_K, n_el, vacuum flag, Z, rho."""
     return np.array([mat.X0 if not mat.vacuum else 1.0e99, mat.e_cut, mat.g_cut, mat.B_K, mat.n_el,
                      1.0 if mat.vacuum else 0.0, mat.Z, mat.rho], dtype=np.float64)
+
+
+MAX_ELEMENTS = 4
+
+
+def element_tables(mats):
+    """C5, the element selector's inputs (adept_tables.n_elem / elem_bk / pe_cum): per material the number of
+    elements, their K-shell binding energies, and on the ln T grid the cumulative share of elements 0..j in the
+    photoelectric cross section (1 from the last element on).  None if every material is a single element."""
+    if not any(len(m.elements) > 1 for m in mats):
+        return None
+    n_elem = np.ones(len(mats), dtype=np.int32)
+    bk = np.zeros((len(mats), MAX_ELEMENTS))
+    cum = np.ones((len(mats), N_GRID, MAX_ELEMENTS))
+    T = energy_grid()
+    for i, m in enumerate(mats):
+        if not m.elements:
+            bk[i, 0] = m.B_K
+            continue
+        n = len(m.elements)
+        assert n <= MAX_ELEMENTS
+        n_elem[i] = n
+        bk[i, :n] = m.B_K_i
+        part = np.stack([ni * sigma_photo_atom(T, z) for ni, (z, _, _) in zip(m.n_i, m.elements)], axis=1)
+        share = np.cumsum(part, axis=1) / part.sum(axis=1, keepdims=True)
+        cum[i, :, :n - 1] = share[:, :n - 1]
+    return n_elem, np.ascontiguousarray(bk), np.ascontiguousarray(cum)
 
 
 def build_material_set(names):

@@ -31,6 +31,15 @@ def barrel_patch():
 
 
 @pytest.fixture(scope="session")
+def barrel_patch_compound():
+    """The same patch with crystals of the real compound PbWO4 (Pb + W + 4 O) and its element-selector tables."""
+    from paper_2209_15445_b200.inputs import geometry, materials
+    g = geometry.barrel(n_eta=12, n_phi=12, crystal="PbWO4_true")
+    mats, tabs, scal = materials.build_material_set(g.material_names)
+    return g, mats, tabs, scal, materials.element_tables(mats)
+
+
+@pytest.fixture(scope="session")
 def barrel_full():
     from paper_2209_15445_b200.inputs import geometry, materials
     g = geometry.barrel()

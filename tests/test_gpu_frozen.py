@@ -119,15 +119,15 @@ def check_per_track_deposits(a, g, scal, fld, pre, ores, osec, dedx, n_chunks=48
     return checked
 
 
-def _run_case(ob, geom_set, fld, prim, per_species, stride, **cfg):
+def _run_case(ob, geom_set, fld, prim, per_species, stride, elements=None, **cfg):
     from paper_2209_15445_b200 import adept
-    g, _, tabs, scal = geom_set
-    o = ob.Oracle(g, tabs, scal, fld)
+    g, _, tabs, scal = geom_set[:4]
+    o = ob.Oracle(g, tabs, scal, fld, elements=elements)
     pre = _states(o, prim, per_species, stride)
     counts = np.bincount(pre["species"], minlength=3)
     ores, osec = o.step(pre)
     dedx = _dedx(o, g, scal, pre)
-    a = adept.Adept(g, tabs, scal, fld, track_capacity=1 << 18, leak_capacity=1 << 18, **cfg)
+    a = adept.Adept(g, tabs, scal, fld, track_capacity=1 << 18, leak_capacity=1 << 18, elements=elements, **cfg)
     worst_p = check_population(a, o, g, scal, fld, pre, ores, osec, dedx=dedx)
     # a small batch takes the sparse-tile path of the charged kernel (a few tracks per block)
     few = np.concatenate([np.where(pre["species"] == sp)[0][:700] for sp in range(3)])
@@ -163,6 +163,26 @@ def test_barrel_patch_frozen_steps(ob, barrel_patch):
     counts, worst_p, worst_g, ores, n_single = _run_case(ob, barrel_patch, field.solenoid_map(), prim, 40000, 1)
     assert np.all(counts >= 20000), counts
     assert 8 in set(np.unique(ores["outcome"]).tolist())             # truncated (chord budget) steps occur
+    print("worst scaled errors: population", worst_p, "generic", worst_g)
+
+
+def test_compound_crystals_frozen_steps(ob, barrel_patch_compound):
+    """the crystal patch in the real compound PbWO4 = Pb + W + 4 O, whose
+    photoelectric absorptions pick their target element (and its K-shell binding energy) with uniform U6."""
+    from paper_2209_15445_b200.inputs import field, primaries
+    g, mats, tabs, scal, elements = barrel_patch_compound
+    prim = primaries.barrel_events(1, 40, 1e3, 2e4, mode="cfg5")
+    d = np.array([np.cos(0.1), np.sin(0.1), 0.01])
+    prim["dir"][:] = d / np.linalg.norm(d)
+    counts, worst_p, worst_g, ores, n_single = _run_case(ob, barrel_patch_compound, field.solenoid_map(), prim, 40000, 1,
+                                                         elements=elements)
+    assert np.all(counts >= 20000), counts
+    pe = ores["outcome"] == 3
+    assert pe.sum() > 2000
+    # both heavy elements were chosen: deposits of the two K-shell binding energies occur among the absorptions
+    bk = elements[1][2]
+    dep = ores["edep_cut"][pe]
+    assert np.isclose(dep, bk[0], rtol=1e-12).sum() > 100 and np.isclose(dep, bk[1], rtol=1e-12).sum() > 50
     print("worst scaled errors: population", worst_p, "generic", worst_g)
 
 

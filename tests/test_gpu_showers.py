@@ -180,6 +180,37 @@ def test_config5_concurrent_events_on_streams(ob, barrel_patch, navigator):
     a.close()
 
 
+def test_compound_crystals_showers(ob, barrel_patch_compound):
+    """showers in crystals of the real compound PbWO4 with the element selector; identical random
+    streams, so every counter and every per-volume deposit equals the oracle's."""
+    import torch
+    from paper_2209_15445_b200 import adept
+    from paper_2209_15445_b200.inputs import field, primaries
+    g, mats, tabs, scal, elements = barrel_patch_compound
+    fld = field.solenoid_map()
+    prim = primaries.barrel_events(6, 6, 200.0, 3e3, mode="cfg5")
+    rng = np.random.default_rng(7)
+    phi, z = rng.uniform(0.03, 0.17, 36), rng.uniform(-0.08, 0.08, 36)
+    d = np.stack([np.cos(phi), np.sin(phi), z], axis=1)
+    prim["dir"][:] = d / np.linalg.norm(d, axis=1, keepdims=True)
+    o = ob.Oracle(g, tabs, scal, fld, elements=elements)
+    oe, ol, ost = o.run(o.make_tracks(prim))
+    # without the element tables the result differs: the selector is really in the path
+    oe1, _, ost1 = ob.Oracle(g, tabs, scal, fld).run(o.make_tracks(prim))
+    assert list(ost1.outcomes) != list(ost.outcomes) or not np.allclose(oe1, oe, rtol=1e-9, atol=1e-9)
+    a = adept.Adept(g, tabs, scal, fld, track_capacity=1 << 17, elements=elements)
+    a.enqueue(prim)
+    a.transport(0, torch.cuda.current_stream())
+    e, led = a.read_scoring(0)
+    st = a.stats(0)
+    a.close()
+    assert abs(led.total() - led.primary) <= 1e-9 * led.primary
+    assert list(st.steps) == list(ost.steps) and list(st.outcomes) == list(ost.outcomes)
+    assert list(st.secondaries) == list(ost.secondaries)
+    np.testing.assert_allclose(e, oe, rtol=1e-9, atol=1e-9)
+    assert led.escaped == pytest.approx(ol.escaped, rel=1e-9, abs=1e-9)
+
+
 def test_empty_and_error_paths(ob, calo):
     import ctypes as C
     import torch
