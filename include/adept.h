@@ -39,7 +39,9 @@ enum {
 enum { ADEPT_ELECTRON = 0, ADEPT_POSITRON = 1, ADEPT_GAMMA = 2 };
 enum { ADEPT_BOX = 0, ADEPT_TUBE = 1 };
 enum { ADEPT_FIELD_NONE = 0, ADEPT_FIELD_UNIFORM = 1, ADEPT_FIELD_MAP_RZ = 2 };
-enum { ADEPT_NAV_LOOP = 0, ADEPT_NAV_BVH = 1 };
+enum { ADEPT_NAV_LOOP = 0, ADEPT_NAV_BVH = 1,
+       /* single-precision geometry: solids, transforms and BVH boxes in fp32; ray-cast validator only */
+       ADEPT_NAV_LOOP_F32 = 2, ADEPT_NAV_BVH_F32 = 3 };
 
 /* Outcome of one step. */
 enum {
@@ -253,7 +255,10 @@ int adept_get_iteration_trace(adept_ctx*, int event_slot, uint64_t* t_ns, uint32
  * vector dir3[i] is marched boundary by boundary -- distance to boundary, push, relocation: the calls of a photon
  * step -- until it leaves the world or has crossed max_crossings boundaries.  column[i] = sum of path length x
  * density [g/cm^2], crossings[i] = boundaries crossed (-1 if the ray starts outside the world).  Host arrays in
- * and out; *device_ms (may be NULL) = CUDA-event time of the kernel.  The navigator is chosen here. */
+ * and out; *device_ms (may be NULL) = CUDA-event time of the kernel.  The navigator is chosen here.
+ * ADEPT_NAV_LOOP_F32 / ADEPT_NAV_BVH_F32 march the same rays through the single-precision copy of the geometry
+ * (all geometry types in fp32; validated by comparing the pictures): positions,
+ * distances and the column density are fp32, the boundary push is 1e-3 cm (float spacing at 300 cm is 3e-5 cm). */
 int adept_raycast_batch(adept_ctx*, int navigator, int n, const double* pos3, const double* dir3, int max_crossings,
                         double* column, int32_t* crossings, double* device_ms, void* cuda_stream);
 

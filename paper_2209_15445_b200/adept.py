@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("ADEPT_B200_LIB", os.path.join(HERE, "libadept_b200.so"))
 
 OK, EINVAL, ENOMEM, EOVERFLOW, ECUDA, ESTATE = 0, -1, -2, -3, -4, -5
-NAV_LOOP, NAV_BVH = 0, 1
+NAV_LOOP, NAV_BVH, NAV_LOOP_F32, NAV_BVH_F32 = 0, 1, 2, 3
 OUTCOMES = ["boundary", "compton", "pair", "photo", "brem", "ioni", "anni", "stopped", "truncated", "loss",
             "escaped", "killed", "closed"]
 

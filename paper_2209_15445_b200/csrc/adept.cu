@@ -360,6 +360,8 @@ int validate(const adept_config* cfg, const adept_geometry* g, int n_mats, const
   if (cfg->track_capacity < 32 || cfg->track_capacity > 0x3fffffffu) return fail(ADEPT_EINVAL, "track_capacity out of range");
   if (cfg->stage_capacity != 0 && (cfg->stage_capacity < 32 || cfg->stage_capacity > 0x3fffffffu)) return fail(ADEPT_EINVAL, "stage_capacity out of range");
   if (cfg->chord_budget < 1 || cfg->sync_interval < 1) return fail(ADEPT_EINVAL, "chord_budget / sync_interval must be >= 1");
+  if (cfg->navigator != ADEPT_NAV_LOOP && cfg->navigator != ADEPT_NAV_BVH)
+    return fail(ADEPT_EINVAL, "transport runs on the fp64 navigators (ADEPT_NAV_LOOP or ADEPT_NAV_BVH)");
   if (cfg->steps_per_launch < 0 || cfg->steps_per_launch > 4096) return fail(ADEPT_EINVAL, "steps_per_launch out of range");
   if (g->mother[0] != -1) return fail(ADEPT_EINVAL, "volume 0 must be the world");
   for (int v = 0; v < g->n_volumes; ++v) {
@@ -380,6 +382,7 @@ int validate(const adept_config* cfg, const adept_geometry* g, int n_mats, const
 struct Layout {
   DevVolume* vol; double* rot; int32_t* nbr; int32_t* rhint; DevBvh* bvh; double *tab_g, *tab_em, *tab_ep, *scal, *bz;
   int32_t* n_elem; double *elem_bk, *pe_cum;
+  VolT<float>* vol32; float* rot32; BvhT<float>* bvh32; std::vector<float*> bvh32_prim_box; std::vector<std::vector<float*>> bvh32_node_box;
   std::vector<double*> bvh_prim_box; std::vector<int32_t*> bvh_prim_vol; std::vector<std::vector<double*>> bvh_node_box;
   std::vector<int32_t*> bvh_nbr, bvh_nbr_count;
   adept_track* stage; uint32_t* bad; size_t stage_cap;
@@ -397,6 +400,9 @@ size_t carve(void* base, const adept_config* cfg, const adept_geometry* g, int n
   std::vector<int> bvh_vols;
   for (int v = 0; v < g->n_volumes; ++v) if (g->daughter_count[v] >= kBvhMinDaughters) bvh_vols.push_back(v);
   L.bvh = cv.take<DevBvh>(std::max<size_t>(bvh_vols.size(), 1));
+  L.vol32 = cv.take<VolT<float>>(g->n_volumes);
+  L.rot32 = cv.take<float>(9 * static_cast<size_t>(g->n_volumes));
+  L.bvh32 = cv.take<BvhT<float>>(std::max<size_t>(bvh_vols.size(), 1));
   for (size_t k = 0; k < bvh_vols.size(); ++k) {
     const int n = g->daughter_count[bvh_vols[k]];
     L.bvh_prim_box.push_back(cv.take<double>(6 * static_cast<size_t>(n)));
@@ -404,9 +410,16 @@ size_t carve(void* base, const adept_config* cfg, const adept_geometry* g, int n
     L.bvh_nbr.push_back(cv.take<int32_t>(static_cast<size_t>(n) * kNbrCap));
     L.bvh_nbr_count.push_back(cv.take<int32_t>(n));
     std::vector<double*> lv;
+    std::vector<float*> lv32;
+    L.bvh32_prim_box.push_back(cv.take<float>(6 * static_cast<size_t>(n)));
     int nn = n;
-    do { nn = (nn + 31) / 32; lv.push_back(cv.take<double>(6 * static_cast<size_t>(nn))); } while (nn > 32);
+    do {
+      nn = (nn + 31) / 32;
+      lv.push_back(cv.take<double>(6 * static_cast<size_t>(nn)));
+      lv32.push_back(cv.take<float>(6 * static_cast<size_t>(nn)));
+    } while (nn > 32);
     L.bvh_node_box.push_back(lv);
+    L.bvh32_node_box.push_back(lv32);
   }
   (void)bvhs;
   L.tab_g = cv.take<double>(static_cast<size_t>(n_mats) * kNGrid * kRowG);
@@ -487,6 +500,7 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   const int nv = g->n_volumes;
   std::vector<DevVolume> hv(nv);
   std::vector<DevBvh> hb;
+  std::vector<BvhT<float>> hb32;
   std::vector<int32_t> isolated(nv, 0);
   bool any_lists = false;
   for (int v = 0; v < nv; ++v)
@@ -531,6 +545,31 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
         db.node_box[l] = L.bvh_node_box[k][l];
         CUDA_TRY(cudaMemcpy(L.bvh_node_box[k][l], b.node_box[l].data(), b.node_box[l].size() * sizeof(double), cudaMemcpyHostToDevice));
       }
+      // single-precision copy: boxes rounded outwards (a float box must not be smaller than the fp32 solid inside it)
+      auto outward = [](const std::vector<double>& box) {
+        std::vector<float> f(box.size());
+        const size_t third = box.size() / 2;      // [lo.xyz | hi.xyz]
+        for (size_t i = 0; i < box.size(); ++i) {
+          const double pad = 1.0e-4 + 4.0e-7 * std::fabs(box[i]);
+          f[i] = static_cast<float>(i < third ? box[i] - pad : box[i] + pad);
+        }
+        return f;
+      };
+      BvhT<float> db32{};
+      db32.n_prims = db.n_prims; db32.n_levels = db.n_levels; db32.prim_vol = db.prim_vol;
+      db32.nbr = db.nbr; db32.nbr_count = db.nbr_count; db32.nbr_reach = 0.0;
+      db32.prim_box = L.bvh32_prim_box[k];
+      {
+        const std::vector<float> f = outward(b.prim_box);
+        CUDA_TRY(cudaMemcpy(L.bvh32_prim_box[k], f.data(), f.size() * sizeof(float), cudaMemcpyHostToDevice));
+      }
+      for (int l = 0; l < db.n_levels; ++l) {
+        db32.n_nodes[l] = b.n_nodes[l];
+        db32.node_box[l] = L.bvh32_node_box[k][l];
+        const std::vector<float> f = outward(b.node_box[l]);
+        CUDA_TRY(cudaMemcpy(L.bvh32_node_box[k][l], f.data(), f.size() * sizeof(float), cudaMemcpyHostToDevice));
+      }
+      hb32.push_back(db32);
       d.bvh = static_cast<int>(k);
       hb.push_back(db);
     }
@@ -538,6 +577,20 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   CUDA_TRY(cudaMemcpy(L.vol, hv.data(), hv.size() * sizeof(DevVolume), cudaMemcpyHostToDevice));
   CUDA_TRY(cudaMemcpy(L.rot, g->rot, 9 * static_cast<size_t>(nv) * sizeof(double), cudaMemcpyHostToDevice));
   if (!hb.empty()) CUDA_TRY(cudaMemcpy(L.bvh, hb.data(), hb.size() * sizeof(DevBvh), cudaMemcpyHostToDevice));
+  {  // the geometry in single precision
+    std::vector<VolT<float>> hv32(nv);
+    std::vector<float> rot32(9 * static_cast<size_t>(nv));
+    for (int v = 0; v < nv; ++v) {
+      VolT<float>& f = hv32[v];
+      for (int k = 0; k < 3; ++k) { f.t[k] = static_cast<float>(hv[v].t[k]); f.dims[k] = static_cast<float>(hv[v].dims[k]); }
+      f.solid = hv[v].solid; f.material = hv[v].material; f.dbegin = hv[v].dbegin; f.dcount = hv[v].dcount;
+      f.bvh = hv[v].bvh; f.identity = hv[v].identity; f.mother = hv[v].mother; f.isolated = hv[v].isolated;
+      for (int k = 0; k < 9; ++k) rot32[9 * static_cast<size_t>(v) + k] = static_cast<float>(g->rot[9 * static_cast<size_t>(v) + k]);
+    }
+    CUDA_TRY(cudaMemcpy(L.vol32, hv32.data(), hv32.size() * sizeof(VolT<float>), cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaMemcpy(L.rot32, rot32.data(), rot32.size() * sizeof(float), cudaMemcpyHostToDevice));
+    if (!hb32.empty()) CUDA_TRY(cudaMemcpy(L.bvh32, hb32.data(), hb32.size() * sizeof(BvhT<float>), cudaMemcpyHostToDevice));
+  }
 
   // ---- interleaved table slices (one node = one row)
   {
@@ -600,6 +653,7 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   ctx->n_vol = nv; ctx->n_mat = n_mats;
   DevCtx& d = ctx->dev;
   d.vol = L.vol; d.rot = L.rot; d.nbr = L.nbr; d.n_vol = nv; d.bvh = L.bvh; d.navigator = cfg->navigator;
+  d.vol32 = L.vol32; d.rot32 = L.rot32; d.bvh32 = L.bvh32;
   d.tab_g = L.tab_g; d.tab_em = L.tab_em; d.tab_ep = L.tab_ep; d.scal = L.scal; d.rhint = L.rhint; d.n_mat = n_mats;
   d.n_elem = compounds ? L.n_elem : nullptr; d.elem_bk = L.elem_bk; d.pe_cum = L.pe_cum;
   d.field_kind = f->kind;
@@ -1113,7 +1167,7 @@ extern "C" int adept_distance_batch(adept_ctx* ctx, int nav, int n, const double
 extern "C" int adept_raycast_batch(adept_ctx* ctx, int nav, int n, const double* pos3, const double* dir3, int max_crossings,
                                    double* column, int32_t* crossings, double* device_ms, void* stream) {
   if (!ctx || n < 0 || (n > 0 && (!pos3 || !dir3 || !column || !crossings))) return fail(ADEPT_EINVAL, "null argument");
-  if (nav != ADEPT_NAV_LOOP && nav != ADEPT_NAV_BVH) return fail(ADEPT_EINVAL, "unknown navigator");
+  if (nav < ADEPT_NAV_LOOP || nav > ADEPT_NAV_BVH_F32) return fail(ADEPT_EINVAL, "unknown navigator");
   if (max_crossings < 1) return fail(ADEPT_EINVAL, "max_crossings must be >= 1");
   if (n == 0) return ADEPT_OK;
   ADEPT_ON_DEVICE(ctx);
@@ -1131,7 +1185,11 @@ extern "C" int adept_raycast_batch(adept_ctx* ctx, int nav, int n, const double*
     if (cudaMemcpyAsync(d_pos, pos3, nb, cudaMemcpyHostToDevice, st) != cudaSuccess ||
         cudaMemcpyAsync(d_dir, dir3, nb, cudaMemcpyHostToDevice, st) != cudaSuccess) { rc = fail(ADEPT_ECUDA, "ray-cast upload"); break; }
     cudaEventRecord(e0, st);
-    raycast_kernel<<<std::min((n + kBlock - 1) / kBlock, 65535), kBlock, 0, st>>>(ctx->dev, nav, n, d_pos, d_dir, max_crossings, d_col, d_nx);
+    const int grid = std::min((n + kBlock - 1) / kBlock, 65535);
+    if (nav >= ADEPT_NAV_LOOP_F32)   // ADEPT_NAV_LOOP_F32 -> loop, ADEPT_NAV_BVH_F32 -> BVH, on the fp32 geometry
+      raycast_kernel<float><<<grid, kBlock, 0, st>>>(ctx->dev, nav - ADEPT_NAV_LOOP_F32, n, d_pos, d_dir, max_crossings, d_col, d_nx);
+    else
+      raycast_kernel<double><<<grid, kBlock, 0, st>>>(ctx->dev, nav, n, d_pos, d_dir, max_crossings, d_col, d_nx);
     cudaEventRecord(e1, st);
     if (cudaMemcpyAsync(column, d_col, static_cast<size_t>(n) * sizeof(double), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
         cudaMemcpyAsync(crossings, d_nx, static_cast<size_t>(n) * sizeof(int32_t), cudaMemcpyDeviceToHost, st) != cudaSuccess ||

@@ -4,27 +4,54 @@
 // other by the whole warp (each lane tests one child box / one primitive), which turns the paper's
 // "quasi-random memory access + divergence" bottleneck into coalesced, uniform work.
 #pragma once
+#include <type_traits>
+
 #include "types.cuh"
 
 namespace adept {
 
 __device__ __forceinline__ const DevVolume& volume(const DevCtx& c, int v) { return c.vol[v]; }
 
+// The navigator is written once for the precision R of the geometry it reads: double -- the transport path, all
+// state fp64 (BASELINE.json:north_star) -- or float, the single-precision geometry mode of PAPER.md:41 (every solid,
+// transform and BVH box in fp32), which the ray-cast validator can be pointed at.
+template <typename R> struct Geo;
+template <> struct Geo<double> {
+  static __device__ __forceinline__ const VolT<double>& vol(const DevCtx& c, int v) { return c.vol[v]; }
+  static __device__ __forceinline__ const double* rot(const DevCtx& c) { return c.rot; }
+  static __device__ __forceinline__ const BvhT<double>& bvh(const DevCtx& c, int i) { return c.bvh[i]; }
+  static __device__ __forceinline__ double inf() { return ADEPT_INF; }
+};
+template <> struct Geo<float> {
+  static __device__ __forceinline__ const VolT<float>& vol(const DevCtx& c, int v) { return c.vol32[v]; }
+  static __device__ __forceinline__ const float* rot(const DevCtx& c) { return c.rot32; }
+  static __device__ __forceinline__ const BvhT<float>& bvh(const DevCtx& c, int i) { return c.bvh32[i]; }
+  static __device__ __forceinline__ float inf() { return __int_as_float(0x7f800000); }
+};
+__device__ __forceinline__ double r_abs(double x) { return fabs(x); }
+__device__ __forceinline__ float r_abs(float x) { return fabsf(x); }
+__device__ __forceinline__ double r_sqrt(double x) { return sqrt(x); }
+__device__ __forceinline__ float r_sqrt(float x) { return sqrtf(x); }
+__device__ __forceinline__ double r_min(double a, double b) { return fmin(a, b); }
+__device__ __forceinline__ float r_min(float a, float b) { return fminf(a, b); }
+__device__ __forceinline__ double r_max(double a, double b) { return fmax(a, b); }
+__device__ __forceinline__ float r_max(float a, float b) { return fmaxf(a, b); }
+
 // local = R^T (global - t); R (row-major, local axes as columns) is only read for rotated placements
-__device__ __forceinline__ void to_local(const DevCtx& c, int vi, const DevVolume& v, double gx, double gy, double gz,
-                                         double l[3]) {
-  const double q0 = gx - v.t[0], q1 = gy - v.t[1], q2 = gz - v.t[2];
+template <typename R>
+__device__ __forceinline__ void to_local(const DevCtx& c, int vi, const VolT<R>& v, R gx, R gy, R gz, R l[3]) {
+  const R q0 = gx - v.t[0], q1 = gy - v.t[1], q2 = gz - v.t[2];
   if (v.identity) { l[0] = q0; l[1] = q1; l[2] = q2; return; }
-  const double* __restrict__ R = c.rot + 9 * static_cast<size_t>(vi);
+  const R* __restrict__ M = Geo<R>::rot(c) + 9 * static_cast<size_t>(vi);
 #pragma unroll
-  for (int i = 0; i < 3; ++i) l[i] = __ldg(R + i) * q0 + __ldg(R + 3 + i) * q1 + __ldg(R + 6 + i) * q2;
+  for (int i = 0; i < 3; ++i) l[i] = __ldg(M + i) * q0 + __ldg(M + 3 + i) * q1 + __ldg(M + 6 + i) * q2;
 }
-__device__ __forceinline__ void dir_to_local(const DevCtx& c, int vi, const DevVolume& v, double gx, double gy, double gz,
-                                             double l[3]) {
+template <typename R>
+__device__ __forceinline__ void dir_to_local(const DevCtx& c, int vi, const VolT<R>& v, R gx, R gy, R gz, R l[3]) {
   if (v.identity) { l[0] = gx; l[1] = gy; l[2] = gz; return; }
-  const double* __restrict__ R = c.rot + 9 * static_cast<size_t>(vi);
+  const R* __restrict__ M = Geo<R>::rot(c) + 9 * static_cast<size_t>(vi);
 #pragma unroll
-  for (int i = 0; i < 3; ++i) l[i] = __ldg(R + i) * gx + __ldg(R + 3 + i) * gy + __ldg(R + 6 + i) * gz;
+  for (int i = 0; i < 3; ++i) l[i] = __ldg(M + i) * gx + __ldg(M + 3 + i) * gy + __ldg(M + 6 + i) * gz;
 }
 
 // global = t + R local (inverse of to_local)
@@ -36,119 +63,127 @@ __device__ __forceinline__ void to_global(const DevCtx& c, int vi, const DevVolu
 }
 
 // ---------------------------------------------------------------- G1 solids
-__device__ __forceinline__ bool inside_solid(int solid, const double h[3], const double p[3]) {
-  if (solid == ADEPT_BOX) return fabs(p[0]) <= h[0] && fabs(p[1]) <= h[1] && fabs(p[2]) <= h[2];
-  const double r2 = p[0] * p[0] + p[1] * p[1];
-  return r2 >= h[0] * h[0] && r2 <= h[1] * h[1] && fabs(p[2]) <= h[2];
+template <typename R>
+__device__ __forceinline__ bool inside_solid(int solid, const R h[3], const R p[3]) {
+  if (solid == ADEPT_BOX) return r_abs(p[0]) <= h[0] && r_abs(p[1]) <= h[1] && r_abs(p[2]) <= h[2];
+  const R r2 = p[0] * p[0] + p[1] * p[1];
+  return r2 >= h[0] * h[0] && r2 <= h[1] * h[1] && r_abs(p[2]) <= h[2];
 }
 
 // min_i (sgn(d_i) h_i - p_i) / d_i over d_i != 0.  The three quotients n_i / |d_i| are compared by
 // cross-multiplication and only the smallest is divided (one division instead of three; when two are
 // within rounding of each other either is the minimum to 1 ulp).
 // `face` receives the exit face, 2 * axis + (d[axis] > 0), or -1.
-__device__ __forceinline__ double box_exit(const double h[3], const double p[3], const double d[3], int& face) {
-  double num = 1.0, den = 0.0;   // +inf as 1/0
+template <typename R>
+__device__ __forceinline__ R box_exit(const R h[3], const R p[3], const R d[3], int& face) {
+  R num = R(1), den = R(0);   // +inf as 1/0
   face = -1;
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
-    const double ad = fabs(d[i]);
-    const double ni = h[i] - (d[i] > 0.0 ? p[i] : -p[i]);   // distance to the exit plane along the axis
-    if (ad != 0.0 && ni * den <= num * ad) { num = ni; den = ad; face = 2 * i + (d[i] > 0.0 ? 1 : 0); }
+    const R ad = r_abs(d[i]);
+    const R ni = h[i] - (d[i] > R(0) ? p[i] : -p[i]);   // distance to the exit plane along the axis
+    if (ad != R(0) && ni * den <= num * ad) { num = ni; den = ad; face = 2 * i + (d[i] > R(0) ? 1 : 0); }
   }
-  return den != 0.0 ? fmax(num / den, 0.0) : ADEPT_INF;
+  return den != R(0) ? r_max(num / den, R(0)) : Geo<R>::inf();
 }
 
-__device__ __forceinline__ double box_entry(const double h[3], const double p[3], const double d[3]) {
-  double tn = -ADEPT_INF, tf = ADEPT_INF;
+template <typename R>
+__device__ __forceinline__ R box_entry(const R h[3], const R p[3], const R d[3]) {
+  R tn = -Geo<R>::inf(), tf = Geo<R>::inf();
   bool miss = false;
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
-    if (d[i] != 0.0) {
-      const double t1 = (-h[i] - p[i]) / d[i];
-      const double t2 = (h[i] - p[i]) / d[i];
-      tn = fmax(tn, fmin(t1, t2));
-      tf = fmin(tf, fmax(t1, t2));
-    } else if (fabs(p[i]) > h[i]) {
+    if (d[i] != R(0)) {
+      const R t1 = (-h[i] - p[i]) / d[i];
+      const R t2 = (h[i] - p[i]) / d[i];
+      tn = r_max(tn, r_min(t1, t2));
+      tf = r_min(tf, r_max(t1, t2));
+    } else if (r_abs(p[i]) > h[i]) {
       miss = true;
     }
   }
-  if (!miss && tn <= tf && tf > 0.0) return fmax(tn, 0.0);
-  return ADEPT_INF;
+  if (!miss && tn <= tf && tf > R(0)) return r_max(tn, R(0));
+  return Geo<R>::inf();
 }
 
-__device__ __forceinline__ double tube_exit(const double h[3], const double p[3], const double d[3]) {
-  double t = ADEPT_INF;
-  if (d[2] != 0.0) t = ((d[2] > 0.0 ? h[2] : -h[2]) - p[2]) / d[2];
-  const double A = d[0] * d[0] + d[1] * d[1];
-  if (A > 0.0) {
-    const double B = p[0] * d[0] + p[1] * d[1];
-    const double r2 = p[0] * p[0] + p[1] * p[1];
-    const double Co = r2 - h[1] * h[1];
-    const double disc_o = B * B - A * Co;
-    t = fmin(t, (-B + sqrt(fmax(disc_o, 0.0))) / A);
-    if (h[0] > 0.0 && B < 0.0) {
-      const double Ci = r2 - h[0] * h[0];
-      const double disc_i = B * B - A * Ci;
-      if (disc_i > 0.0) t = fmin(t, (-B - sqrt(disc_i)) / A);
+template <typename R>
+__device__ __forceinline__ R tube_exit(const R h[3], const R p[3], const R d[3]) {
+  R t = Geo<R>::inf();
+  if (d[2] != R(0)) t = ((d[2] > R(0) ? h[2] : -h[2]) - p[2]) / d[2];
+  const R A = d[0] * d[0] + d[1] * d[1];
+  if (A > R(0)) {
+    const R B = p[0] * d[0] + p[1] * d[1];
+    const R r2 = p[0] * p[0] + p[1] * p[1];
+    const R Co = r2 - h[1] * h[1];
+    const R disc_o = B * B - A * Co;
+    t = r_min(t, (-B + r_sqrt(r_max(disc_o, R(0)))) / A);
+    if (h[0] > R(0) && B < R(0)) {
+      const R Ci = r2 - h[0] * h[0];
+      const R disc_i = B * B - A * Ci;
+      if (disc_i > R(0)) t = r_min(t, (-B - r_sqrt(disc_i)) / A);
     }
   }
-  return fmax(t, 0.0);
+  return r_max(t, R(0));
 }
 
-__device__ __forceinline__ double tube_entry(const double h[3], const double p[3], const double d[3]) {
-  if (inside_solid(ADEPT_TUBE, h, p)) return 0.0;
-  double best = ADEPT_INF;
-  const double r2 = p[0] * p[0] + p[1] * p[1];
-  const double rmin2 = h[0] * h[0], rmax2 = h[1] * h[1];
-  if (fabs(p[2]) > h[2] && p[2] * d[2] < 0.0) {  // (a) end caps
-    const double t = (fabs(p[2]) - h[2]) / fabs(d[2]);
-    const double x = p[0] + t * d[0], y = p[1] + t * d[1];
-    const double q2 = x * x + y * y;
-    if (q2 >= rmin2 && q2 <= rmax2) best = fmin(best, t);
+template <typename R>
+__device__ __forceinline__ R tube_entry(const R h[3], const R p[3], const R d[3]) {
+  if (inside_solid(ADEPT_TUBE, h, p)) return R(0);
+  R best = Geo<R>::inf();
+  const R r2 = p[0] * p[0] + p[1] * p[1];
+  const R rmin2 = h[0] * h[0], rmax2 = h[1] * h[1];
+  if (r_abs(p[2]) > h[2] && p[2] * d[2] < R(0)) {  // (a) end caps
+    const R t = (r_abs(p[2]) - h[2]) / r_abs(d[2]);
+    const R x = p[0] + t * d[0], y = p[1] + t * d[1];
+    const R q2 = x * x + y * y;
+    if (q2 >= rmin2 && q2 <= rmax2) best = r_min(best, t);
   }
-  const double A = d[0] * d[0] + d[1] * d[1];
-  if (A > 0.0) {
-    const double B = p[0] * d[0] + p[1] * d[1];
-    const double Co = r2 - rmax2;
-    if (Co > 0.0 && B < 0.0) {  // (b) outer cylinder from outside
-      const double disc = B * B - A * Co;
-      if (disc > 0.0) {
-        const double t = (-B - sqrt(disc)) / A;
-        if (t >= 0.0 && fabs(p[2] + t * d[2]) <= h[2]) best = fmin(best, t);
+  const R A = d[0] * d[0] + d[1] * d[1];
+  if (A > R(0)) {
+    const R B = p[0] * d[0] + p[1] * d[1];
+    const R Co = r2 - rmax2;
+    if (Co > R(0) && B < R(0)) {  // (b) outer cylinder from outside
+      const R disc = B * B - A * Co;
+      if (disc > R(0)) {
+        const R t = (-B - r_sqrt(disc)) / A;
+        if (t >= R(0) && r_abs(p[2] + t * d[2]) <= h[2]) best = r_min(best, t);
       }
     }
-    if (h[0] > 0.0) {  // (c) inner cylinder, far root: leaving the hole into the solid
-      const double Ci = r2 - rmin2;
-      const double disc = B * B - A * Ci;
-      if (disc > 0.0) {
-        const double t = (-B + sqrt(disc)) / A;
-        if (t > 0.0 && fabs(p[2] + t * d[2]) <= h[2]) best = fmin(best, t);
+    if (h[0] > R(0)) {  // (c) inner cylinder, far root: leaving the hole into the solid
+      const R Ci = r2 - rmin2;
+      const R disc = B * B - A * Ci;
+      if (disc > R(0)) {
+        const R t = (-B + r_sqrt(disc)) / A;
+        if (t > R(0) && r_abs(p[2] + t * d[2]) <= h[2]) best = r_min(best, t);
       }
     }
   }
   return best;
 }
 
-__device__ __forceinline__ double solid_exit(const DevVolume& v, const double p[3], const double d[3], int& face) {
+template <typename R>
+__device__ __forceinline__ R solid_exit(const VolT<R>& v, const R p[3], const R d[3], int& face) {
   if (v.solid == ADEPT_BOX) return box_exit(v.dims, p, d, face);
   face = -1;
   return tube_exit(v.dims, p, d);
 }
-__device__ __forceinline__ double solid_entry(const DevVolume& v, const double p[3], const double d[3]) {
+template <typename R>
+__device__ __forceinline__ R solid_entry(const VolT<R>& v, const R p[3], const R d[3]) {
   return v.solid == ADEPT_BOX ? box_entry(v.dims, p, d) : tube_entry(v.dims, p, d);
 }
 
-__device__ __forceinline__ bool inside_volume(const DevCtx& c, int vol, double x, double y, double z) {
-  const DevVolume& v = volume(c, vol);
-  double l[3];
+template <typename R>
+__device__ __forceinline__ bool inside_volume(const DevCtx& c, int vol, R x, R y, R z) {
+  const VolT<R>& v = Geo<R>::vol(c, vol);
+  R l[3];
   to_local(c, vol, v, x, y, z, l);
   return inside_solid(v.solid, v.dims, l);
 }
 
-__device__ __forceinline__ double entry_distance(const DevCtx& c, int vol, double px, double py, double pz,
-                                                 double dx, double dy, double dz) {
-  const DevVolume& v = volume(c, vol);
-  double lp[3], ld[3];
+template <typename R>
+__device__ __forceinline__ R entry_distance(const DevCtx& c, int vol, R px, R py, R pz, R dx, R dy, R dz) {
+  const VolT<R>& v = Geo<R>::vol(c, vol);
+  R lp[3], ld[3];
   to_local(c, vol, v, px, py, pz, lp);
   dir_to_local(c, vol, v, dx, dy, dz, ld);
   return solid_entry(v, lp, ld);
@@ -180,6 +215,11 @@ __device__ __forceinline__ double warp_min(double v) {
   for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(kFull, v, o));
   return v;
 }
+__device__ __forceinline__ float warp_min(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(kFull, v, o));
+  return v;
+}
 __device__ __forceinline__ int warp_min_int(int v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v = min(v, __shfl_xor_sync(kFull, v, o));
@@ -187,22 +227,23 @@ __device__ __forceinline__ int warp_min_int(int v) {
 }
 
 // lane tests box `i` (< n valid) of a SoA box array of stride `stride` against the ray; returns hit
-__device__ __forceinline__ bool ray_box(const double* __restrict__ box, int stride, int i, bool valid, double px,
-                                        double py, double pz, double ix, double iy, double iz, double best) {
+template <typename R>
+__device__ __forceinline__ bool ray_box(const R* __restrict__ box, int stride, int i, bool valid, R px, R py, R pz, R ix, R iy, R iz,
+                                        R best) {
   if (!valid) return false;
-  const double lx = __ldg(box + i), ly = __ldg(box + stride + i), lz = __ldg(box + 2 * stride + i);
-  const double hx = __ldg(box + 3 * stride + i), hy = __ldg(box + 4 * stride + i), hz = __ldg(box + 5 * stride + i);
-  const double ax = (lx - px) * ix, bx = (hx - px) * ix;
-  const double ay = (ly - py) * iy, by = (hy - py) * iy;
-  const double az = (lz - pz) * iz, bz = (hz - pz) * iz;
+  const R lx = __ldg(box + i), ly = __ldg(box + stride + i), lz = __ldg(box + 2 * stride + i);
+  const R hx = __ldg(box + 3 * stride + i), hy = __ldg(box + 4 * stride + i), hz = __ldg(box + 5 * stride + i);
+  const R ax = (lx - px) * ix, bx = (hx - px) * ix;
+  const R ay = (ly - py) * iy, by = (hy - py) * iy;
+  const R az = (lz - pz) * iz, bz = (hz - pz) * iz;
   // fmin/fmax drop NaN operands (0 * inf when the ray is parallel to a slab and starts on its plane)
-  const double tn = fmax(fmax(fmin(ax, bx), fmin(ay, by)), fmin(az, bz));
-  const double tf = fmin(fmin(fmax(ax, bx), fmax(ay, by)), fmax(az, bz));
-  return tn <= tf && tf >= 0.0 && tn < best;
+  const R tn = r_max(r_max(r_min(ax, bx), r_min(ay, by)), r_min(az, bz));
+  const R tf = r_min(r_min(r_max(ax, bx), r_max(ay, by)), r_max(az, bz));
+  return tn <= tf && tf >= R(0) && tn < best;
 }
 
-__device__ __forceinline__ bool point_box(const double* __restrict__ box, int stride, int i, bool valid, double px,
-                                          double py, double pz) {
+template <typename R>
+__device__ __forceinline__ bool point_box(const R* __restrict__ box, int stride, int i, bool valid, R px, R py, R pz) {
   if (!valid) return false;
   return px >= __ldg(box + i) && py >= __ldg(box + stride + i) && pz >= __ldg(box + 2 * stride + i) &&
          px <= __ldg(box + 3 * stride + i) && py <= __ldg(box + 4 * stride + i) && pz <= __ldg(box + 5 * stride + i);
@@ -212,11 +253,11 @@ __device__ __forceinline__ bool point_box(const double* __restrict__ box, int st
 // state is a short stack of one 32-bit child mask per level, shared by the warp.
 // `hit` (warp-uniform, out): touchable id of the daughter that gave the returned minimum, -1 if none did
 // or two daughters tie.
-__device__ __forceinline__ double bvh_ray(const DevCtx& c, const DevBvh& b, double px, double py, double pz, double dx, double dy,
-                          double dz, double best, int& hit) {
+template <typename R>
+__device__ __forceinline__ R bvh_ray(const DevCtx& c, const BvhT<R>& b, R px, R py, R pz, R dx, R dy, R dz, R best, int& hit) {
   hit = -1;
   const int lane = threadIdx.x & 31;
-  const double ix = 1.0 / dx, iy = 1.0 / dy, iz = 1.0 / dz;
+  const R ix = R(1) / dx, iy = R(1) / dy, iz = R(1) / dz;
   const int top = b.n_levels - 1;
   unsigned mask[kBvhMaxLevels];
   int first[kBvhMaxLevels];
@@ -236,13 +277,13 @@ __device__ __forceinline__ double bvh_ray(const DevCtx& c, const DevBvh& b, doub
     const int base = node << 5;
     if (level == 0) {
       const int i = base + lane;
-      double t = ADEPT_INF;
+      R t = Geo<R>::inf();
       int pv = -1;
       if (ray_box(b.prim_box, b.n_prims, i, i < b.n_prims, px, py, pz, ix, iy, iz, best)) {
         pv = __ldg(b.prim_vol + i);
-        t = entry_distance(c, pv, px, py, pz, dx, dy, dz);
+        t = entry_distance<R>(c, pv, px, py, pz, dx, dy, dz);
       }
-      const double m = warp_min(t);
+      const R m = warp_min(t);
       if (m < best) {
         best = m;
         const unsigned w = __ballot_sync(kFull, t == m);
@@ -261,7 +302,8 @@ __device__ __forceinline__ double bvh_ray(const DevCtx& c, const DevBvh& b, doub
 }
 
 // All arguments warp-uniform.  Lowest touchable id among the daughters containing the point, or -1.
-__device__ __forceinline__ int bvh_point(const DevCtx& c, const DevBvh& b, double px, double py, double pz) {
+template <typename R>
+__device__ __forceinline__ int bvh_point(const DevCtx& c, const BvhT<R>& b, R px, R py, R pz) {
   const int lane = threadIdx.x & 31;
   const int top = b.n_levels - 1;
   unsigned mask[kBvhMaxLevels];
@@ -284,7 +326,7 @@ __device__ __forceinline__ int bvh_point(const DevCtx& c, const DevBvh& b, doubl
       int hit = 0x7fffffff;
       if (point_box(b.prim_box, b.n_prims, i, i < b.n_prims, px, py, pz)) {
         const int v = __ldg(b.prim_vol + i);
-        if (inside_volume(c, v, px, py, pz)) hit = v;
+        if (inside_volume<R>(c, v, px, py, pz)) hit = v;
       }
       found = min(found, warp_min_int(hit));
     } else {
@@ -412,23 +454,23 @@ __device__ __forceinline__ int bvh_candidates(const DevCtx& c, const DevBvh& b, 
 // `cache` (BVH only, warp-uniformly null or not): the lane's candidate list (see above); `cand` (may be null): the
 // block's shared-memory room for lane-built lists -- with it, a lane that traverses twice in a row in the same
 // volume gets a list around its current point.
-template <bool BVH>
-__device__ __forceinline__ double nav_distance_body(const DevCtx& c, int nav, bool active, double px, double py, double pz, double dx,
-                               double dy, double dz, uint32_t vol, double s_max, int& face, NavCache* cache = nullptr,
-                               int32_t* cand = nullptr, bool skip_own = false) {
+template <bool BVH, typename R>
+__device__ __forceinline__ R nav_distance_body(const DevCtx& c, int nav, bool active, R px, R py, R pz, R dx, R dy, R dz, uint32_t vol,
+                                               R s_max, int& face, NavCache* cache = nullptr, int32_t* cand = nullptr,
+                                               bool skip_own = false) {
   const int lane = threadIdx.x & 31;
-  double s = s_max;
+  R s = s_max;
   bool need = false;
   int bvh = -1;
   face = -1;
   if (active) {
-    const DevVolume& v = volume(c, vol);
+    const VolT<R>& v = Geo<R>::vol(c, vol);
     if (!skip_own) {   // (skip_own: the caller knows the segment ends before the volume's own surface, nav_safety)
-      double lp[3], ld[3];
+      R lp[3], ld[3];
       to_local(c, vol, v, px, py, pz, lp);
       dir_to_local(c, vol, v, dx, dy, dz, ld);
       int f;
-      const double s_exit = solid_exit(v, lp, ld, f);
+      const R s_exit = solid_exit(v, lp, ld, f);
       if (s_exit < s_max) { s = s_exit; face = f; }
     }
     if (v.dcount > 0) {
@@ -437,14 +479,14 @@ __device__ __forceinline__ double nav_distance_body(const DevCtx& c, int nav, bo
         bvh = v.bvh;
       } else {
         for (int k = 0; k < v.dcount; ++k) {
-          const double e = entry_distance(c, v.dbegin + k, px, py, pz, dx, dy, dz);
+          const R e = entry_distance<R>(c, v.dbegin + k, px, py, pz, dx, dy, dz);
           if (e <= s) { face = e < s ? -2 - (v.dbegin + k) : -1; s = e; }
         }
       }
     }
   }
   if (!BVH) return s;
-  if (cache) {   // the lane's candidate list first (lane-local): final if the segment cannot leave its reach
+  if constexpr (std::is_same<R, double>::value) if (cache) {   // the lane's candidate list first (lane-local): final if the segment cannot leave its reach
     if (need && cache->reach > 0.0 && cache->vol == vol) {
       for (int j = 0; j < cache->count; ++j) {
         const int pv = cache->list[j];
@@ -460,12 +502,12 @@ __device__ __forceinline__ double nav_distance_body(const DevCtx& c, int nav, bo
     const int src = __ffs(m) - 1;
     m &= m - 1;
     int hit;
-    const double r = bvh_ray(c, c.bvh[__shfl_sync(kFull, bvh, src)], __shfl_sync(kFull, px, src),
-                             __shfl_sync(kFull, py, src), __shfl_sync(kFull, pz, src), __shfl_sync(kFull, dx, src),
-                             __shfl_sync(kFull, dy, src), __shfl_sync(kFull, dz, src), __shfl_sync(kFull, s, src), hit);
+    const R r = bvh_ray<R>(c, Geo<R>::bvh(c, __shfl_sync(kFull, bvh, src)), __shfl_sync(kFull, px, src),
+                           __shfl_sync(kFull, py, src), __shfl_sync(kFull, pz, src), __shfl_sync(kFull, dx, src),
+                           __shfl_sync(kFull, dy, src), __shfl_sync(kFull, dz, src), __shfl_sync(kFull, s, src), hit);
     if (lane == src && r < s) { s = r; face = hit >= 0 ? -2 - hit : -1; }
   }
-  if (cache) {   // a lane that keeps traversing in the same volume gets a list of its own around where it is
+  if constexpr (std::is_same<R, double>::value) if (cache) {   // a lane that keeps traversing in the same volume gets a list of its own around where it is
     bool build = false;
     if (need && cand) {
       if (cache->vol != vol) { cache->vol = vol; cache->queries = 0; cache->reach = -1.0; }
@@ -489,17 +531,16 @@ __device__ __forceinline__ double nav_distance_body(const DevCtx& c, int nav, bo
   }
   return s;
 }
-template <bool BVH = true>
-__device__ __forceinline__ double nav_distance(const DevCtx& c, int nav, bool active, double px, double py, double pz, double dx,
-                                               double dy, double dz, uint32_t vol, double s_max, int& face, NavCache* cache = nullptr,
-                                               int32_t* cand = nullptr, bool skip_own = false) {
-  return nav_distance_body<BVH>(c, nav, active, px, py, pz, dx, dy, dz, vol, s_max, face, cache, cand, skip_own);
+template <bool BVH = true, typename R = double>
+__device__ __forceinline__ R nav_distance(const DevCtx& c, int nav, bool active, R px, R py, R pz, R dx, R dy, R dz, uint32_t vol, R s_max,
+                                          int& face, NavCache* cache = nullptr, int32_t* cand = nullptr, bool skip_own = false) {
+  return nav_distance_body<BVH, R>(c, nav, active, px, py, pz, dx, dy, dz, vol, s_max, face, cache, cand, skip_own);
 }
 template <bool BVH = true>
 __device__ __forceinline__ double nav_distance(const DevCtx& c, int nav, bool active, double px, double py, double pz, double dx,
                                                double dy, double dz, uint32_t vol, double s_max) {
   int face;
-  return nav_distance<BVH>(c, nav, active, px, py, pz, dx, dy, dz, vol, s_max, face);
+  return nav_distance<BVH, double>(c, nav, active, px, py, pz, dx, dy, dz, vol, s_max, face);
 }
 
 // ---------------------------------------------------------------- safety (reading A)
@@ -540,21 +581,21 @@ __device__ __forceinline__ double nav_safety(const DevCtx& c, uint32_t vol, doub
 // ---------------------------------------------------------------- G4 Locate
 // From the world down, descend into the first daughter (index order) containing the point.
 // Warp-convergent call; returns -1 outside the world or for inactive lanes.
-template <bool BVH = true>
-__device__ __noinline__ int nav_locate(const DevCtx& c, int nav, bool active, double qx, double qy, double qz) {
+template <bool BVH = true, typename R = double>
+__device__ __noinline__ int nav_locate(const DevCtx& c, int nav, bool active, R qx, R qy, R qz) {
   const int lane = threadIdx.x & 31;
   int cur = -1;
   bool desc = false;
-  if (active && inside_volume(c, 0, qx, qy, qz)) {
+  if (active && inside_volume<R>(c, 0, qx, qy, qz)) {
     cur = 0;
     desc = true;
   }
   if (!BVH) {  // lane-local descent, no warp cooperation needed
     while (desc) {
-      const DevVolume& v = volume(c, cur);
+      const VolT<R>& v = Geo<R>::vol(c, cur);
       int next = -1;
       for (int k = 0; k < v.dcount; ++k) {
-        if (inside_volume(c, v.dbegin + k, qx, qy, qz)) { next = v.dbegin + k; break; }
+        if (inside_volume<R>(c, v.dbegin + k, qx, qy, qz)) { next = v.dbegin + k; break; }
       }
       if (next < 0) desc = false; else cur = next;
     }
@@ -564,7 +605,7 @@ __device__ __noinline__ int nav_locate(const DevCtx& c, int nav, bool active, do
     bool need = false;
     int bvh = -1;
     if (desc) {
-      const DevVolume& v = volume(c, cur);
+      const VolT<R>& v = Geo<R>::vol(c, cur);
       if (v.dcount == 0) {
         desc = false;
       } else if (nav == ADEPT_NAV_BVH && v.bvh >= 0) {
@@ -573,7 +614,7 @@ __device__ __noinline__ int nav_locate(const DevCtx& c, int nav, bool active, do
       } else {
         int next = -1;
         for (int k = 0; k < v.dcount; ++k) {
-          if (inside_volume(c, v.dbegin + k, qx, qy, qz)) { next = v.dbegin + k; break; }
+          if (inside_volume<R>(c, v.dbegin + k, qx, qy, qz)) { next = v.dbegin + k; break; }
         }
         if (next < 0) desc = false; else cur = next;
       }
@@ -582,8 +623,8 @@ __device__ __noinline__ int nav_locate(const DevCtx& c, int nav, bool active, do
     while (m) {
       const int src = __ffs(m) - 1;
       m &= m - 1;
-      const int r = bvh_point(c, c.bvh[__shfl_sync(kFull, bvh, src)], __shfl_sync(kFull, qx, src),
-                              __shfl_sync(kFull, qy, src), __shfl_sync(kFull, qz, src));
+      const int r = bvh_point<R>(c, Geo<R>::bvh(c, __shfl_sync(kFull, bvh, src)), __shfl_sync(kFull, qx, src),
+                                 __shfl_sync(kFull, qy, src), __shfl_sync(kFull, qz, src));
       if (lane == src) {
         if (r < 0) desc = false; else cur = r;
       }
@@ -606,14 +647,13 @@ __device__ __noinline__ int nav_locate(const DevCtx& c, int nav, bool active, do
 // face <= -2: the daughter -2 - face the step ended on.  Either way that one candidate is tested first; if the pushed point is inside it, the descent
 // starts there -- the deepest volume containing q is unique, so the answer is the same as the climb's --
 // and in a stack of slabs a crossing costs one containment test instead of four or five dependent ones.
-template <bool BVH>
-__device__ __forceinline__ int nav_relocate_body(const DevCtx& c, int nav, bool active, uint32_t vol_old, double qx, double qy,
-                                                 double qz, int face) {
+template <bool BVH, typename R>
+__device__ __forceinline__ int nav_relocate_body(const DevCtx& c, int nav, bool active, uint32_t vol_old, R qx, R qy, R qz, int face) {
   int cur = -1, prev = -1;
   bool desc = false, done = false;
   if (active) {
     const int cand = face >= 0 ? __ldg(c.nbr + 6 * static_cast<size_t>(vol_old) + face) : (face <= -2 ? -2 - face : -1);
-    if (cand >= 0 && inside_volume(c, cand, qx, qy, qz)) {
+    if (cand >= 0 && inside_volume<R>(c, cand, qx, qy, qz)) {
       cur = cand;
       // Out of an ISOLATED daughter (adept_init: a box with no sibling within kIsolationMargin of it) into
       // its mother: a point outside the box but within margin / 2 of it along every local axis is nearer
@@ -621,18 +661,18 @@ __device__ __forceinline__ int nav_relocate_body(const DevCtx& c, int nav, bool 
       // descent, i.e. no BVH point query per crystal-to-gap crossing.  Checked here, not assumed, so the
       // result is Locate(q) for any q and any hint.
       if (face >= 0) {
-        const DevVolume& vo = volume(c, vol_old);
+        const VolT<R>& vo = Geo<R>::vol(c, vol_old);
         if (vo.isolated && vo.mother == cand) {
-          double l[3];
+          R l[3];
           to_local(c, vol_old, vo, qx, qy, qz, l);
-          const double a0 = fabs(l[0]) - vo.dims[0], a1 = fabs(l[1]) - vo.dims[1], a2 = fabs(l[2]) - vo.dims[2];
-          const double out = fmax(a0, fmax(a1, a2));      // > 0: outside the box; <= margin / 2: within reach of no sibling
-          done = out > 0.0 && out <= 0.5 * kIsolationMargin;
+          const R a0 = r_abs(l[0]) - vo.dims[0], a1 = r_abs(l[1]) - vo.dims[1], a2 = r_abs(l[2]) - vo.dims[2];
+          const R out = r_max(a0, r_max(a1, a2));      // > 0: outside the box; <= margin / 2: within reach of no sibling
+          done = out > R(0) && out <= R(0.5 * kIsolationMargin);
         }
       }
     } else {
       cur = static_cast<int>(vol_old);
-      while (cur >= 0 && !inside_volume(c, cur, qx, qy, qz)) { prev = cur; cur = volume(c, cur).mother; }
+      while (cur >= 0 && !inside_volume<R>(c, cur, qx, qy, qz)) { prev = cur; cur = Geo<R>::vol(c, cur).mother; }
     }
     desc = cur >= 0 && !done;
   }
@@ -641,7 +681,7 @@ __device__ __forceinline__ int nav_relocate_body(const DevCtx& c, int nav, bool 
     bool need = false;
     int bvh = -1;
     if (desc) {
-      const DevVolume& v = volume(c, cur);
+      const VolT<R>& v = Geo<R>::vol(c, cur);
       if (v.dcount == 0) {
         desc = false;
       } else if (BVH && nav == ADEPT_NAV_BVH && v.bvh >= 0) {
@@ -651,13 +691,13 @@ __device__ __forceinline__ int nav_relocate_body(const DevCtx& c, int nav, bool 
         int next = -1;
         if (prev >= 0) {  // came up from daughter `prev` (q is outside it): try its neighbours first
           const int k0 = prev - v.dbegin;
-          if (k0 + 1 < v.dcount && inside_volume(c, prev + 1, qx, qy, qz)) next = prev + 1;
-          else if (k0 >= 1 && inside_volume(c, prev - 1, qx, qy, qz)) next = prev - 1;
+          if (k0 + 1 < v.dcount && inside_volume<R>(c, prev + 1, qx, qy, qz)) next = prev + 1;
+          else if (k0 >= 1 && inside_volume<R>(c, prev - 1, qx, qy, qz)) next = prev - 1;
         }
         for (int k = 0; next < 0 && k < v.dcount; ++k) {
           const int d = v.dbegin + k;
           if (prev >= 0 && (d == prev || d == prev + 1 || d == prev - 1)) continue;
-          if (inside_volume(c, d, qx, qy, qz)) next = d;
+          if (inside_volume<R>(c, d, qx, qy, qz)) next = d;
         }
         if (next < 0) desc = false; else cur = next;
         prev = -1;
@@ -669,8 +709,8 @@ __device__ __forceinline__ int nav_relocate_body(const DevCtx& c, int nav, bool 
       while (m) {
         const int src = __ffs(m) - 1;
         m &= m - 1;
-        const int r = bvh_point(c, c.bvh[__shfl_sync(kFull, bvh, src)], __shfl_sync(kFull, qx, src),
-                                __shfl_sync(kFull, qy, src), __shfl_sync(kFull, qz, src));
+        const int r = bvh_point<R>(c, Geo<R>::bvh(c, __shfl_sync(kFull, bvh, src)), __shfl_sync(kFull, qx, src),
+                                   __shfl_sync(kFull, qy, src), __shfl_sync(kFull, qz, src));
         if (lane == src) {
           if (r < 0) desc = false; else cur = r;
           prev = -1;
@@ -680,10 +720,9 @@ __device__ __forceinline__ int nav_relocate_body(const DevCtx& c, int nav, bool 
   }
   return cur;
 }
-template <bool BVH = true>
-__device__ __forceinline__ int nav_relocate(const DevCtx& c, int nav, bool active, uint32_t vol_old, double qx, double qy, double qz,
-                                            int face = -1) {
-  return nav_relocate_body<BVH>(c, nav, active, vol_old, qx, qy, qz, face);
+template <bool BVH = true, typename R = double>
+__device__ __forceinline__ int nav_relocate(const DevCtx& c, int nav, bool active, uint32_t vol_old, R qx, R qy, R qz, int face = -1) {
+  return nav_relocate_body<BVH, R>(c, nav, active, vol_old, qx, qy, qz, face);
 }
 
 }  // namespace adept

@@ -670,39 +670,43 @@ __global__ void __launch_bounds__(kBlock) locate_kernel(const __grid_constant__ 
 // dir[i] and is marched boundary by boundary -- distance to boundary (A4), push, relocation (A5), exactly the
 // calls a photon step makes -- until it leaves the world or has crossed max_crossings boundaries.
 // column[i] = sum of path x density [g/cm^2], crossings[i] = boundaries crossed (-1: start outside the world).
+// R = double: the transport path's navigator.  R = float: the single-precision geometry mode.
+template <typename R>
 __global__ void __launch_bounds__(kBlock) raycast_kernel(const __grid_constant__ DevCtx c, int nav, int n, const double* __restrict__ pos,
                                                          const double* __restrict__ dir, int max_crossings, double* __restrict__ column,
                                                          int32_t* __restrict__ crossings) {
+  constexpr bool kDouble = std::is_same<R, double>::value;
+  const R eps = kDouble ? static_cast<R>(c.eps_push) : static_cast<R>(kPushF32);
   const int n_round = (n + 31) & ~31;
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += gridDim.x * blockDim.x) {
     const bool a = i < n;
     const int k = a ? i : 0;
-    double px = pos[3 * k], py = pos[3 * k + 1], pz = pos[3 * k + 2];
-    const double dx = dir[3 * k], dy = dir[3 * k + 1], dz = dir[3 * k + 2];
-    int vol = nav_locate(c, nav, a, px, py, pz);
+    R px = static_cast<R>(pos[3 * k]), py = static_cast<R>(pos[3 * k + 1]), pz = static_cast<R>(pos[3 * k + 2]);
+    const R dx = static_cast<R>(dir[3 * k]), dy = static_cast<R>(dir[3 * k + 1]), dz = static_cast<R>(dir[3 * k + 2]);
+    int vol = nav_locate<true, R>(c, nav, a, px, py, pz);
     bool alive = a && vol >= 0;
-    double col = 0.0;
+    R col = R(0);
     int nx = alive ? 0 : -1;
     NavCache cache;
     nav_cache_reset(cache);
     while (__any_sync(kFull, alive)) {
       int face;
-      const double s = nav_distance(c, nav, alive, px, py, pz, dx, dy, dz, alive ? static_cast<uint32_t>(vol) : 0u, ADEPT_INF, face,
-                                    &cache);
+      const R s = nav_distance<true, R>(c, nav, alive, px, py, pz, dx, dy, dz, alive ? static_cast<uint32_t>(vol) : 0u, Geo<R>::inf(), face,
+                                        kDouble ? &cache : nullptr);
       if (alive) {
-        col += s * mat_scalar(c, volume(c, vol).material, S_RHO);
+        col += s * static_cast<R>(mat_scalar(c, Geo<R>::vol(c, vol).material, S_RHO));
         px += s * dx; py += s * dy; pz += s * dz;
-        px += c.eps_push * dx; py += c.eps_push * dy; pz += c.eps_push * dz;
+        px += eps * dx; py += eps * dy; pz += eps * dz;
       }
-      const int nv = nav_relocate(c, nav, alive, alive ? static_cast<uint32_t>(vol) : 0u, px, py, pz, face);
+      const int nv = nav_relocate<true, R>(c, nav, alive, alive ? static_cast<uint32_t>(vol) : 0u, px, py, pz, face);
       if (alive) {
         ++nx;
-        if (nav == ADEPT_NAV_BVH) nav_cache_left_daughter(c, cache, static_cast<uint32_t>(vol), nv, px, py, pz);
+        if constexpr (kDouble) { if (nav == ADEPT_NAV_BVH) nav_cache_left_daughter(c, cache, static_cast<uint32_t>(vol), nv, px, py, pz); }
         vol = nv;
         if (nv < 0 || nx >= max_crossings) alive = false;
       }
     }
-    if (a) { column[i] = col; crossings[i] = nx; }
+    if (a) { column[i] = static_cast<double>(col); crossings[i] = nx; }
   }
 }
 

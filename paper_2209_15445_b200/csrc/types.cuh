@@ -14,7 +14,8 @@ constexpr double kTmin = 1.0e-3;     // 1 keV
 constexpr int kNGrid = ADEPT_N_GRID;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr uint32_t kDeadVolume = 0xffffffffu;
-constexpr double kIsolationMargin = 1.0e-4;  // [cm] see DevVolume::isolated (1000 x the default boundary push)
+constexpr double kIsolationMargin = 4.0e-3;  // [cm] see DevVolume::isolated (twice the single-precision push of the ray-cast and its rounding)
+constexpr float kPushF32 = 1.0e-3f;          // [cm] boundary push of the single-precision ray-cast (float spacing at 300 cm is 3e-5 cm)
 
 #define ADEPT_INF (__longlong_as_double(0x7ff0000000000000LL))
 
@@ -29,9 +30,10 @@ constexpr int kRowG = 4, kRowEm = 4, kRowEp = 8;
 
 // Hot part of a touchable (80 B); the 3x3 rotation lives in DevCtx::rot and is only read for rotated
 // placements, so the 152 volumes of the calorimeter stay L1-resident (12 KB).
-struct __align__(16) DevVolume {
-  double t[3];
-  double dims[3];
+template <typename R>
+struct __align__(16) VolT {
+  R t[3];
+  R dims[3];
   int32_t solid;
   int32_t material;
   int32_t dbegin;
@@ -41,24 +43,27 @@ struct __align__(16) DevVolume {
   int32_t mother;    // -1 for the world
   int32_t isolated;  // 1: a box with no sibling within kIsolationMargin (adept_init), see nav_relocate
 };
+using DevVolume = VolT<double>;
 
 // Implicit complete 32-ary BVH over the daughters of one volume, in the world frame.
 // Primitives are sorted along a Morton curve; node k of level L covers nodes [32k, 32k+32) of level L-1
 // (level 0 covers primitives).  Boxes are stored SoA: lo.x, lo.y, lo.z, hi.x, hi.y, hi.z.
 constexpr int kBvhMaxLevels = 5;
-struct DevBvh {
+template <typename R>
+struct BvhT {
   int32_t n_prims;
   int32_t n_levels;                  // number of node levels (>= 1)
   int32_t n_nodes[kBvhMaxLevels];    // nodes per level
-  const double* prim_box;            // [6][n_prims]
+  const R* prim_box;                 // [6][n_prims]
   const int32_t* prim_vol;           // [n_prims] touchable id
-  const double* node_box[kBvhMaxLevels];  // [6][n_nodes[L]]
+  const R* node_box[kBvhMaxLevels];  // [6][n_nodes[L]]
   // per-daughter neighbour lists (geom.cuh NavCache): for daughter d (index relative to the volume's first
   // daughter) the touchable ids of the siblings within nbr_reach of its solid, itself included
   const int32_t* nbr;                // [n_prims][kNbrCap]
   const int32_t* nbr_count;          // [n_prims] entries, -1 = the list did not fit
   double nbr_reach;                  // [cm], <= 0: no lists
 };
+using DevBvh = BvhT<double>;
 
 // One species' track buffer, structure of arrays (76 B per track).
 struct TrackSoA {
@@ -118,6 +123,11 @@ struct DevCtx {
   const int32_t* nbr;       // [n_vol][6] relocation hints: volume beyond each box face, -1 = none (geom.cuh nav_relocate)
   int32_t n_vol;
   const DevBvh* bvh;
+  // the same geometry in single precision (the ray-cast validator's ADEPT_NAV_*_F32 modes): boxes of
+  // the BVH rounded outwards
+  const VolT<float>* vol32;
+  const float* rot32;
+  const BvhT<float>* bvh32;
   int32_t navigator;
   const double* tab_g;      // [n_mat][2048][kRowG]
   const double* tab_em;     // [n_mat][2048][kRowEm]

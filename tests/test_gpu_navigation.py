@@ -185,3 +185,52 @@ def test_raycast_validator(ob, barrel_patch, barrel_full, tmp_path):
     data = out.read_bytes()
     assert data.startswith(b"P6\n96 40\n255\n") and len(data) == len(b"P6\n96 40\n255\n") + 3 * w * h
     a.close()
+
+
+def test_single_precision_geometry_raycast(ob, barrel_patch, barrel_full):
+    """the single-precision geometry mode (every solid, transform and BVH box in
+    fp32) validated the paper's way, by comparing its ray-cast picture with the double-precision one, and against the
+    oracle's march.  fp32 positions at r ~ 150 cm resolve 1.5e-5 cm and the fp32 march pushes 1e-3 cm past every
+    boundary, so per crossing a path length is off by at most the push plus a few spacings: the column density agrees
+    within crossings x (1e-3 + 2e-4) cm x the largest density, and the crossing count is the same except on rays
+    that graze an edge within that distance."""
+    from paper_2209_15445_b200 import adept, raycast
+    from paper_2209_15445_b200.inputs import field
+    rho_max = 8.28
+    # patch: against the oracle's fp64 march
+    g, _, tabs, scal = barrel_patch
+    o = ob.Oracle(g, tabs, scal, field.no_field())
+    a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=1 << 10)
+    rng = np.random.default_rng(12)
+    phi, eta = rng.uniform(-0.02, 0.23, 300), rng.uniform(-0.12, 0.12, 300)
+    th = 2.0 * np.arctan(np.exp(-eta))
+    d = np.stack([np.sin(th) * np.cos(phi), np.sin(th) * np.sin(phi), np.cos(th)], axis=1)
+    pos = np.zeros_like(d)
+    ocol, onx = _oracle_raycast(o, scal, g, pos, d)
+    for nav in (adept.NAV_BVH_F32, adept.NAV_LOOP_F32):
+        col, nx, _ = a.raycast(pos, d, nav)
+        same = nx == onx
+        assert same.mean() > 0.97, same.mean()
+        tol = (np.maximum(nx, onx) + 1) * 1.2e-3 * rho_max
+        assert np.all(np.abs(col - ocol)[same] <= tol[same]), np.abs(col - ocol)[same].max()
+    cb, nb, _ = a.raycast(pos, d, adept.NAV_BVH_F32)
+    cl, nl, _ = a.raycast(pos, d, adept.NAV_LOOP_F32)
+    assert np.array_equal(nb, nl) and np.array_equal(cb, cl)      # the fp32 BVH culls, the fp32 solids decide
+    a.close()
+    # full barrel: fp32 picture against the fp64 picture, pixel for pixel
+    g, _, tabs, scal = barrel_full
+    a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=1 << 10)
+    w, h = 256, 96
+    p, d = raycast.barrel_rays(w, h)
+    c64, n64, ms64 = a.raycast(p, d, adept.NAV_BVH)
+    c32, n32, ms32 = a.raycast(p, d, adept.NAV_BVH_F32)
+    same = n64 == n32
+    assert same.mean() > 0.98, same.mean()
+    tol = (n64 + 1) * 1.2e-3 * rho_max
+    assert np.all(np.abs(c32 - c64)[same] <= tol[same])
+    assert np.abs(c32 - c64)[same].max() > 0.0                    # it really is another arithmetic
+    # pictures agree to a grey level almost everywhere (a differing pixel is a ray down an edge of a crystal)
+    top = c64.max()
+    assert (np.abs(c32 - c64) > top / 255.0).mean() < 0.02
+    print(f"ray-cast {w}x{h}: fp64 {ms64:.2f} ms, fp32 {ms32:.2f} ms, ratio {ms64 / ms32:.2f}; same crossings {same.mean():.4f}")
+    a.close()
