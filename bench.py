@@ -29,15 +29,20 @@ BYTES_PER_STEP = 160      # 76 B track read + 76 B survivor write + 8 B scoring 
 BYTES_PER_SECONDARY = 76
 E_PRIMARY = 10000.0
 KERNELS = ("gamma_move_kernel", "charged_move_kernel", "interact_kernel")
-# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of each kernel at the peak
-# population of a config-2 pass, and the tracks that launch processed, from the `ncu --set full` capture
-# summarised in profiles/r1f_summary.md.  Reported as roofline.traffic (bytes of that one launch) beside the
-# algorithmic bytes of the same launch (tracks x 160 B).
-NCU_TRAFFIC = {   # bytes of DRAM traffic, tracks processed, kernel time [us] of the captured launch (population step 64)
-    "gamma_move_kernel": {"dram_bytes": 516.2e6, "tracks": 3986758, "time_us": 195.0},
-    "charged_move_kernel": {"dram_bytes": 203.8e6, "tracks": 1698340, "time_us": 167.6},
-    "interact_kernel": {"dram_bytes": 188.7e6, "tracks": None, "time_us": 102.6},
-}
+# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of each kernel at the peak population of a
+# config-2 pass and the tracks that launch processed come from the `ncu --set full` capture recorded in this file
+# (written from the .ncu-rep together with the commit of the build that was profiled; profiles/r2_summary.md).
+# Reported as roofline.traffic (bytes of that one launch) beside the algorithmic bytes of the same launch; null when
+# the file is missing.
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r2_traffic.json")
+
+
+def ncu_traffic():
+    try:
+        with open(TRAFFIC_FILE) as f:
+            return json.load(f)
+    except (OSError, ValueError):
+        return None
 
 
 def parse():
@@ -317,6 +322,7 @@ def run_ours(args):
             pass
         peak = float(peaks.get("hbm_gbs", 6650.0))
         peak_src = "MEASURED_PEAKS.json hbm_gbs (of measured)" if "hbm_gbs" in peaks else "6650 GB/s (of fallback)"
+        traffic = ncu_traffic() if args.config == 2 else None
         # algorithmic HBM bytes of the timed passes per kernel: a move kernel reads 76 B and
         # writes 76 B per track step and scores 8 B; the interaction kernel reads the staged track, writes
         # the parent back and writes 76 B per secondary
@@ -345,9 +351,12 @@ def run_ours(args):
             "clocks": clk,
             "roofline": {"bound": "hbm", "kernel": KERNELS[dom],
                          "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": NCU_TRAFFIC[KERNELS[dom]]["dram_bytes"],
-                         "traffic_launch": dict(NCU_TRAFFIC[KERNELS[dom]], source="ncu --set full, profiles/r1f_summary.md",
-                                                algorithmic_bytes=(NCU_TRAFFIC[KERNELS[dom]]["tracks"] or 0) * BYTES_PER_STEP),
+                         "traffic": traffic["kernels"][KERNELS[dom]]["dram_bytes"] if traffic else None,
+                         "traffic_launch": (dict(traffic["kernels"][KERNELS[dom]], source=traffic.get("source"), commit=traffic.get("commit"),
+                                                 algorithmic_bytes=(traffic["kernels"][KERNELS[dom]].get("tracks") or 0) * BYTES_PER_STEP)
+                                            if traffic else None),
+                         "limiter": "instruction latency: dependent fp64 chains and scattered L2 reads at 30-36 % resident warps; "
+                                    "neither HBM (DRAM 15-32 % busy) nor the fp64 pipe (16-25 %) is near its limit (profiles/)",
                          "peak_source": peak_src, "launches": int(kn[dom]), "avg_launch_ms": float(kms[dom] / max(kn[dom], 1)),
                          "algorithmic_bytes_per_step": BYTES_PER_STEP, "per_kernel": per_kernel,
                          "timing": f"CUDA events around every launch in {n_pass} instrumented passes after the timed region "
@@ -362,8 +371,11 @@ def run_ours(args):
         }
         if world == 1 and not args.no_cpu_baseline and not args.profile:
             ob = oracle_throughput(args, args.cpu_events_per_core)
+            one = oracle_throughput(args, 48, cores=1)       # SURVEY.md §8(d) "oracle timing (i)": one thread
             line["cpu_baseline"] = {"value": ob["steps_per_s"], "unit": "steps/s", "cores": ob["cores"], "kind": "oracle",
-                                    "sample": ob["sample"], "showers_per_s": ob["showers_per_s"]}
+                                    "sample": ob["sample"], "showers_per_s": ob["showers_per_s"],
+                                    "value_1core": one["steps_per_s"], "sample_1core": one["sample"],
+                                    "same_workload": args.config != 4}
         print(json.dumps(line))
     a.close()
     if dist is not None:

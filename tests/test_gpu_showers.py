@@ -180,6 +180,87 @@ def test_config5_concurrent_events_on_streams(ob, barrel_patch, navigator):
     a.close()
 
 
+def _full_barrel_run_worker(job):
+    tracks, max_steps = job
+    from oracle import binding as ob
+    from paper_2209_15445_b200.inputs import field, geometry, materials
+    g = geometry.barrel()
+    _, tabs, scal = materials.build_material_set(g.material_names)
+    o = ob.Oracle(g, tabs, scal, field.solenoid_map(), max_steps=max_steps)
+    edep, led, st = o.run(tracks)
+    nz = np.nonzero(edep)[0]
+    return nz, edep[nz], (led.deposited, led.below_cut, led.escaped, led.killed, led.primary), list(st.steps), list(st.outcomes)
+
+
+def test_config5_full_barrel_200_primaries(ob, barrel_full):
+    """BASELINE.json:configs[4] at its stated structure: 16 events x 200 primaries (e-, e+, gamma 2:1:2) on 16 CUDA
+    streams in the FULL barrel (61 200 crystals, BVH, solenoid map), per-event hits copied back per event.  The
+    energies are lowered to 20-200 MeV log-uniform and the step cap to 300 so that the loop-navigator oracle (3 ms
+    per step in a gap between crystals) finishes two whole events in a process pool: events 0 and 1 are compared
+    with the oracle crystal by crystal, the other 14 by their ledgers and against a second, sequential transport
+    of the same event (random streams are keyed by event, track and step, so the schedule must not matter)."""
+    import multiprocessing as mp
+    import os
+    import torch
+    from paper_2209_15445_b200 import adept
+    from paper_2209_15445_b200.inputs import field, primaries
+    g, _, tabs, scal = barrel_full
+    n_ev, n_per, max_steps = 16, 200, 300
+    prim = primaries.barrel_events(n_ev, n_per, 20.0, 200.0, mode="cfg5")
+    o = ob.Oracle(g, tabs, scal, field.solenoid_map(), max_steps=max_steps)
+    a = adept.Adept(g, tabs, scal, field.solenoid_map(), track_capacity=1 << 16, n_event_slots=n_ev + 1, max_steps=max_steps)
+    streams = [torch.cuda.Stream() for _ in range(n_ev)]
+    sel = [prim["event"] == e for e in range(n_ev)]
+    for e in range(n_ev):
+        a.enqueue_primaries(e, e, prim["species"][sel[e]], prim["pos"][sel[e]], prim["dir"][sel[e]], prim["ekin"][sel[e]])
+    a.transport_many(list(range(n_ev)), streams)
+    hits, leds, stats = [], [], []
+    for e in range(n_ev):
+        h, led = a.read_scoring(e, streams[e])
+        hits.append(h); leds.append(led); stats.append(a.stats(e))
+        assert abs(led.total() - led.primary) <= 1e-9 * led.primary
+        assert led.primary == pytest.approx((prim["ekin"][sel[e]] + np.where(prim["species"][sel[e]] == 1, 2 * M, 0)).sum(), rel=1e-12)
+    assert sum(h[12:].sum() for h in hits) > 0 and sum(l.killed for l in leds) > 0    # crystals hit; curlers reached the cap
+    # events 2..15: the same event alone, sequentially, in the spare slot
+    for e in range(2, n_ev):
+        a.enqueue_primaries(n_ev, e, prim["species"][sel[e]], prim["pos"][sel[e]], prim["dir"][sel[e]], prim["ekin"][sel[e]])
+        st0 = a.stats(n_ev)
+        a.transport(n_ev, torch.cuda.current_stream())
+        h, led = a.read_scoring(n_ev)
+        st1 = a.stats(n_ev)
+        np.testing.assert_allclose(h, hits[e], rtol=1e-9, atol=1e-10)
+        assert [st1.steps[k] - st0.steps[k] for k in range(3)] == list(stats[e].steps)
+        assert [st1.outcomes[k] - st0.outcomes[k] for k in range(13)] == list(stats[e].outcomes)
+        assert led.killed == pytest.approx(leds[e].killed, rel=1e-9, abs=1e-9)
+    a.close()
+    # events 0 and 1 against the oracle: the primaries of each spread over half of a process pool (deposits add)
+    n_proc = min(os.cpu_count() or 2, 16)
+    per_ev = max(n_proc // 2, 1)
+    jobs, owner = [], []
+    for e in (0, 1):
+        tr = o.make_tracks({k: v[sel[e]] for k, v in prim.items()})
+        tr["id"] = np.arange(len(tr))
+        for i in range(per_ev):
+            jobs.append((tr[i::per_ev].copy(), max_steps)); owner.append(e)
+    with mp.get_context("spawn").Pool(len(jobs)) as pool:
+        parts = pool.map(_full_barrel_run_worker, jobs)
+    for e in (0, 1):
+        want, led = np.zeros(g.n_volumes), np.zeros(5)
+        steps, outcomes = np.zeros(3, dtype=np.int64), np.zeros(13, dtype=np.int64)
+        for (nz, val, l, st, oc), ev in zip(parts, owner):
+            if ev != e:
+                continue
+            want[nz] += val
+            led += np.array(l)
+            steps += np.array(st, dtype=np.int64)
+            outcomes += np.array(oc, dtype=np.int64)
+        assert list(stats[e].steps) == steps.tolist() and list(stats[e].outcomes) == outcomes.tolist()
+        np.testing.assert_allclose(hits[e], want, rtol=1e-8, atol=1e-9)
+        assert leds[e].escaped == pytest.approx(led[2], rel=1e-9, abs=1e-9)
+        assert leds[e].killed == pytest.approx(led[3], rel=1e-9, abs=1e-9)
+        assert (want[12:] > 0).sum() > 20
+
+
 def test_compound_crystals_showers(ob, barrel_patch_compound):
     """showers in crystals of the real compound PbWO4 with the element selector; identical random
     streams, so every counter and every per-volume deposit equals the oracle's."""

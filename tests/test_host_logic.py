@@ -45,7 +45,9 @@ def test_bench_workloads_and_sharding():
     assert "max_steps=4096" in b.workload_name(a) and "61200" in b.workload_name(a)
     # ranks own disjoint, consecutive event ranges: Philox streams are keyed by event id
     assert [b.shard_first_event(r, 10000) for r in range(4)] == [0, 10000, 20000, 30000]
-    assert b.BYTES_PER_STEP == 76 + 76 + 8 and set(b.NCU_TRAFFIC) == set(b.KERNELS)
+    assert b.BYTES_PER_STEP == 76 + 76 + 8
+    t = b.ncu_traffic()
+    assert t is None or (set(t["kernels"]) == set(b.KERNELS) and t.get("commit"))
     g, tabs, scal, fld, prim = b.workload(argparse.Namespace(config=2, events=7, field=0.0), first_event=3)
     assert list(prim["event"]) == list(range(3, 10)) and (prim["ekin"] == 10000.0).all() and g.n_volumes == 152
 
