@@ -34,13 +34,28 @@ KERNELS = ("gamma_move_kernel", "charged_move_kernel", "interact_kernel")
 # (written from the .ncu-rep together with the commit of the build that was profiled; profiles/r2_summary.md).
 # Reported as roofline.traffic (bytes of that one launch) beside the algorithmic bytes of the same launch; null when
 # the file is missing.
-TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r2_traffic.json")
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r2_traffic.csv")
 
 
 def ncu_traffic():
+    """{"commit", "source", "kernels": {name: {"dram_bytes", "dram_read", "dram_write", "duration_us", "tracks"}}} or None."""
     try:
+        out = {"source": "profiles/r2_traffic.csv (ncu --set full, one launch per kernel at the peak population step; profiles/r2_summary.md)",
+               "commit": None, "kernels": {}}
         with open(TRAFFIC_FILE) as f:
-            return json.load(f)
+            for line in f:
+                line = line.strip()
+                if line.startswith("#"):
+                    for tok in line[1:].split():
+                        if tok.startswith("commit="):
+                            out["commit"] = tok[7:]
+                    continue
+                if not line or line.startswith("kernel,"):
+                    continue
+                name, rd, wr, us, tracks = line.split(",")
+                out["kernels"][name] = {"dram_bytes": int(rd) + int(wr), "dram_read": int(rd), "dram_write": int(wr),
+                                        "duration_us": float(us), "tracks": int(tracks) if tracks else None}
+        return out if all(k in out["kernels"] for k in KERNELS) else None
     except (OSError, ValueError):
         return None
 
@@ -67,6 +82,8 @@ def parse():
                     help="experiments only: no per-kernel CUDA events (the roofline object is then empty)")
     ap.add_argument("--profile", action="store_true",
                     help="for runs under ncu: take --warmup literally (the timed numbers of such a run are not bench values)")
+    ap.add_argument("--trace-out", default="",
+                    help="write the iteration trace (device time and population of every population step) of the last timed pass to this JSON file")
     ap.add_argument("--cpu-events-per-core", type=int, default=96)
     a = ap.parse_args()
     if a.config == 3 and a.field == 0.0:
@@ -220,6 +237,26 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+# ----------------------------------------------------------------------------- iteration trace
+def write_trace(path, trace, pass_ms, workload):
+    """Per population step: device time since the previous step's end [us] and the e-, e+, gamma tracks that entered it
+    (adept_get_iteration_trace), plus the time spent in steps of each population decade."""
+    t_ns, pop = trace
+    if len(t_ns) == 0:
+        return
+    dt = np.diff(t_ns.astype(np.int64), prepend=t_ns[0]) * 1e-3      # us; the first step's own duration is not known
+    tot = pop.sum(axis=1)
+    buckets = {}
+    for lo, hi in ((0, 1e2), (1e2, 1e3), (1e3, 1e4), (1e4, 1e5), (1e5, 1e6), (1e6, 1e12)):
+        m = (tot >= lo) & (tot < hi)
+        buckets[f"{int(lo)}-{int(hi)}"] = {"steps": int(m.sum()), "ms": float(dt[m].sum() * 1e-3), "tracks": int(tot[m].sum())}
+    k = int(np.argmax(tot))
+    with open(path, "w") as f:
+        json.dump({"workload": workload, "pass_ms": pass_ms, "population_steps": int(len(t_ns)), "by_population": buckets,
+                   "peak_step": {"index": k, "e-": int(pop[k, 0]), "e+": int(pop[k, 1]), "gamma": int(pop[k, 2])},
+                   "dt_us": [round(float(x), 2) for x in dt], "population": pop.tolist()}, f)
+
+
 # ----------------------------------------------------------------------------- GPU arm
 def run_ours(args):
     import torch
@@ -281,13 +318,17 @@ def run_ours(args):
     barrier()
     t_wall0 = time.perf_counter()
     dev_ms, wall_s = [], []
-    for _ in range(args.steps):
+    for k in range(args.steps):
+        if args.trace_out and k == args.steps - 1:
+            a.iteration_trace(0)         # empties the trace: what is read after the loop is the last pass alone
         ms, w = one_pass()
         dev_ms.append(ms)
         wall_s.append(w)
     barrier()
     t_wall = time.perf_counter() - t_wall0
     st = a.stats(0)
+    if args.trace_out and rank == 0:
+        write_trace(args.trace_out, a.iteration_trace(0), dev_ms[-1], workload_name(args))
 
     # Instrumented passes of the same workload, for the roofline object only: CUDA events around every
     # launch, kernels one after the other on the stream (adept.h: adept_set_kernel_timing).  The events
