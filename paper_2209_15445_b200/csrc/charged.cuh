@@ -42,9 +42,10 @@ struct ChargedLane {
 template <int FIELD, bool BVH, bool MULTI>
 __device__ __forceinline__ void charged_lane(const DevCtx& c, const DevSlot& slot, BlockTally& tally, TrackTile& T, int t, bool in_range,
                                              int species, int q0, unsigned long long& packed, double& sum_dep, double& sum_cut,
-                                             unsigned& chords_sum, ChargedLane& r, NavCache* cache, int32_t* cand) {
+                                             unsigned& chords_sum, ChargedLane& r, NavCache* cache, int32_t* cand, int wide_shift = 0) {
   enum { FATE_NONE = 0, FATE_KILLED, FATE_STOPPED, FATE_GO };
   const bool positron = species == ADEPT_POSITRON;
+    if (MULTI && wide_shift) __syncwarp();   // the slot as the group's first lane left it after the previous step
     const uint32_t vol = T.u[2][t];
     const bool active = in_range && vol != kDeadVolume;
 
@@ -117,6 +118,15 @@ __device__ __forceinline__ void charged_lane(const DevCtx& c, const DevSlot& slo
     } else {
       double pos[3] = {px, py, pz}, dir[3] = {T.d[3][t], T.d[4][t], T.d[5][t]}, pushdir[3];
       int chords = 0;
+      if (MULTI && wide_shift) {
+        // sparse tiles: the 2^wide_shift lanes that share tile slot t take the chord loop of its track together
+        // (field.cuh propagate_wide); only the first of them has run phase A
+        const double ekin = T.d[6][t];
+        __syncwarp();   // every lane of the group has read the slot before its first lane writes the post-step state into it
+        const int g0 = (threadIdx.x & 31) & ~((1 << wide_shift) - 1);
+        flag = propagate_wide<FIELD, BVH>(c, c.navigator, wide_shift, __shfl_sync(kFull, go, g0), positron ? +1 : -1, ekin, pos, dir, vol,
+                                          __shfl_sync(kFull, s_phys, g0), s, chords, pushdir, face, cache, cand);
+      } else
       flag = propagate<FIELD, BVH>(c, c.navigator, go, positron ? +1 : -1, T.d[6][t], pos, dir, vol, s_phys, s, chords, pushdir, face,
                                    cache, cand);
       px = pos[0]; py = pos[1]; pz = pos[2];
@@ -250,7 +260,7 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
   // one after the other, so a few hundred loopers packed into a few warps would take 32 x 16 chord queries
   // in sequence per step (measured 4 ms per population step on config 4), spread out they run in parallel.
   uint32_t g = kBlock;
-  while (g > 4 && (n + (g >> 1) - 1) / (g >> 1) <= gridDim.x / 2) g >>= 1;   // (half the grid: the other species runs beside)
+  while (g > kBlock / 32 && (n + (g >> 1) - 1) / (g >> 1) <= gridDim.x / 2) g >>= 1;   // (half the grid: the other species runs beside; at most a warp per track)
   const int lane_shift = __ffs(kBlock / g) - 1;            // every (1 << lane_shift)-th lane takes a track
   const uint32_t n_tiles = (n + g - 1) / g;
   if (blockIdx.x >= n_tiles) return;   // no tile for this block
@@ -273,6 +283,8 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
   const unsigned lt = (1u << lane) - 1u;
   const int t = threadIdx.x >> lane_shift;                 // this lane's entry of the tile
   const bool mine = (threadIdx.x & ((1u << lane_shift) - 1u)) == 0;
+  // eight or more lanes per track: they take its chord loop together (field.cuh propagate_wide)
+  const int wide_shift = (MULTI && FIELD != ADEPT_FIELD_NONE && lane_shift >= 3) ? lane_shift : 0;
   int k_inner = MULTI ? min(inner_steps(c, n, gridDim.x * kBlock), 255) : 1;
   // full GPU, BVH geometry: only the passage through the gap a track has just entered from a daughter is taken in
   // the same launch (geom.cuh NavCache)
@@ -298,7 +310,8 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
       // k_inner steps; the warp goes round together because the navigator is warp-convergent.
       bool cont = mine && tile * g + t < n;
       for (int it = 0;; ++it) {
-        charged_lane<FIELD, BVH, true>(c, slot, tally, T, t, cont, species, q0, packed, sum_dep, sum_cut, chords_sum, r, cache, cand_lists);
+        charged_lane<FIELD, BVH, true>(c, slot, tally, T, t, cont, species, q0, packed, sum_dep, sum_cut, chords_sum, r, cache, cand_lists,
+                                       wide_shift);
         cont = cont && r.live && r.dest == 0 && it + 1 < k_inner;
         if (transit_only) cont = cont && nav_cache.reach > 0.0 && nav_cache.vol == r.vol_post;
         if (!__any_sync(kFull, cont)) break;

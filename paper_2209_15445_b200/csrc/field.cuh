@@ -251,4 +251,199 @@ __device__ __forceinline__ int propagate(const DevCtx& c, int nav, bool active, 
   return flag;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Wide form of the chord loop, for populations so small that a track has W = 8, 16 or 32 lanes of its warp to
+// itself (charged.cuh: sparse tiles).  The tracks that outlive a shower by thousands of steps -- e+- spiralling
+// in vacuum, 16 chords per step -- are one serial chain of chords each, and in the loop above every link of
+// that chain is an integration step AND a geometry query (in a gap between crystals ~1 000 dependent
+// instructions over the candidate list; profiles/r2_summary.md).  Only the integration is inherently serial:
+// chord k+1 starts where chord k ends, whether or not chord k was tested yet.  So the lanes of the group
+// integrate up to W chords ahead (all lanes redundantly, in lockstep; lane j keeps chord j), then lane j asks
+// the geometry about chord j, and the first chord that ends on a boundary -- exactly the one the sequential
+// loop would have stopped at -- decides the step; what was integrated beyond it is dropped.  Every chord and
+// every query is computed by the same arithmetic as in propagate(), so the result is bit-identical.
+// All lanes of a group pass the same track; `cache` is the group's candidate list (kept identical in its lanes).
+template <int FIELD, bool BVH>
+__device__ __forceinline__ int propagate_wide(const DevCtx& c, int nav, int shift, bool active, int charge, double ekin, double pos[3],
+                                              double dir[3], uint32_t vol, double s_phys, double& s_out, int& chords_out,
+                                              double pushdir[3], int& face_out, NavCache* cache, int32_t* cand) {
+  constexpr int field_kind = FIELD;
+  const int lane = threadIdx.x & 31;
+  const int W = 1 << shift, li = lane & (W - 1), g0 = lane & ~(W - 1);
+  const unsigned gmask = (W == 32 ? kFull : ((1u << W) - 1u)) << g0;
+  const double pmom = sqrt(ekin * (ekin + 2.0 * kMe));
+  const double kappa = field_kind == ADEPT_FIELD_UNIFORM ? -charge * kCB * c.Bn / pmom : 0.0;
+  const double inv_kappa = kappa != 0.0 ? 1.0 / kappa : 0.0;
+  const bool curved = charge != 0 && field_kind != ADEPT_FIELD_NONE;
+  double s_done = 0.0, h_step = -1.0;
+  int chords = 0, flag = 0, face_hit = -1;
+  bool running = active;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) pushdir[i] = dir[i];
+  if (BVH && cache) {   // the list of the group's first lane (the lane that runs the rest of the step) is the group's
+    cache->qx = __shfl_sync(kFull, cache->qx, g0); cache->qy = __shfl_sync(kFull, cache->qy, g0);
+    cache->qz = __shfl_sync(kFull, cache->qz, g0); cache->reach = __shfl_sync(kFull, cache->reach, g0);
+    cache->list = reinterpret_cast<const int32_t*>(__shfl_sync(kFull, reinterpret_cast<unsigned long long>(cache->list), g0));
+    cache->vol = __shfl_sync(kFull, cache->vol, g0); cache->count = __shfl_sync(kFull, cache->count, g0);
+    cache->queries = 0;
+  }
+  while (__any_sync(kFull, running)) {
+    // ---- integrate up to W segments ahead; lane li keeps segment li
+    double p[3] = {pos[0], pos[1], pos[2]}, d[3] = {dir[0], dir[1], dir[2]};
+    double P[3] = {0.0, 0.0, 0.0}, D[3] = {0.0, 0.0, 0.0}, D1[3] = {0.0, 0.0, 0.0}, U[3] = {0.0, 0.0, 0.0};
+    double L = 0.0, H = 0.0, Sb = 0.0, reach_end = 0.0;   // reach_end: path from the round's start to the end of my segment
+    int kind = 0;                                          // my segment: 0 none, 1 chord, 2 straight
+    double sd = s_done, cum = 0.0;
+    int ch = chords, nseg = 0, end = -1;                   // end: -1 round full, 0 physics limit, 2 chord budget
+    bool integ = running;
+    for (int j = 0; j < W; ++j) {
+      if (!__any_sync(kFull, integ)) break;
+      if (!integ) continue;
+      if (sd >= s_phys) { end = 0; integ = false; continue; }
+      double B[3] = {0.0, 0.0, 0.0}, h_max = 0.0;
+      if (curved && (field_kind != ADEPT_FIELD_UNIFORM || h_step < 0.0)) {
+        field_at(c, p, B);
+        double dxB[3];
+        cross3(d, B, dxB);
+        const double bperp = sqrt(dxB[0] * dxB[0] + dxB[1] * dxB[1] + dxB[2] * dxB[2]);
+        if (bperp != 0.0) {
+          const double Rcurv = pmom / (kCB * bperp);
+          h_max = sqrt(8.0 * c.delta_chord * Rcurv);
+          if (field_kind == ADEPT_FIELD_MAP_RZ) {
+            const double Bn = sqrt(B[0] * B[0] + B[1] * B[1] + B[2] * B[2]);
+            h_max = fmin(h_max, 0.5 * pmom / (kCB * Bn));
+          }
+        }
+        if (field_kind == ADEPT_FIELD_UNIFORM) h_step = h_max;
+      } else if (curved) {
+        h_max = h_step;
+      }
+      const double rest = s_phys - sd;
+      if (!curved || h_max == 0.0) {          // straight to the physics limit: the last segment
+        if (li == j) {
+          kind = 2; L = rest; Sb = sd; reach_end = cum + rest;
+#pragma unroll
+          for (int i = 0; i < 3; ++i) { P[i] = p[i]; D[i] = d[i]; U[i] = d[i]; }
+        }
+#pragma unroll
+        for (int i = 0; i < 3; ++i) p[i] += rest * d[i];
+        sd = s_phys; nseg = j + 1; end = 0; integ = false;
+      } else if (ch >= c.chord_budget) {
+        end = 2; integ = false;
+      } else {
+        const bool last = h_max >= rest;
+        const double h = last ? rest : h_max;
+        double p1[3], d1[3];
+        if (field_kind == ADEPT_FIELD_UNIFORM) helix(c.bhat, kappa, inv_kappa, h, p, d, p1, d1);
+        else rk4(c, charge, pmom, h, p, d, B, p1, d1);
+        if (li == j) {
+          kind = 1; H = h; Sb = sd; reach_end = cum + h;
+          const double cv[3] = {p1[0] - p[0], p1[1] - p[1], p1[2] - p[2]};
+          const double L2 = cv[0] * cv[0] + cv[1] * cv[1] + cv[2] * cv[2];
+          const double iL = rsqrt(L2);
+          L = L2 * iL;
+#pragma unroll
+          for (int i = 0; i < 3; ++i) { P[i] = p[i]; D[i] = d[i]; D1[i] = d1[i]; U[i] = cv[i] * iL; }
+        }
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { p[i] = p1[i]; d[i] = d1[i]; }
+        sd = last ? s_phys : sd + h;
+        cum += h; ++ch; nseg = j + 1;
+        if (last) { end = 0; integ = false; }
+      }
+    }
+    // ---- which segments need a geometry query (nav_safety, as in propagate(): one clearance around the round's start)
+    double safe = -1.0;
+    bool own_only = false;
+    if (running && nseg > 1) safe = nav_safety(c, vol, pos[0], pos[1], pos[2], own_only);
+    const bool clear = kind == 1 && reach_end < safe;
+    const bool query = running && (kind == 2 || (kind == 1 && (!clear || own_only)));
+    // ---- the group's candidate list (geom.cuh NavCache): rebuilt around the middle of the round when two or more of
+    // its segments are not covered by the list the group has
+    if (BVH && cache && cand) {
+      bool uncovered = false;
+      if (query && nav == ADEPT_NAV_BVH) {
+        const DevVolume& v = volume(c, vol);
+        if (v.dcount > 0 && v.bvh >= 0) {
+          uncovered = true;
+          if (cache->reach > 0.0 && cache->vol == vol) {
+            const double ox = P[0] - cache->qx, oy = P[1] - cache->qy, oz = P[2] - cache->qz;
+            uncovered = !(sqrt(ox * ox + oy * oy + oz * oz) + L <= cache->reach * (1.0 - 1.0e-9));
+          }
+        }
+      }
+      const unsigned um = __ballot_sync(kFull, uncovered) & gmask;
+      unsigned mb = __ballot_sync(kFull, li == 0 && __popc(um) >= 2);
+      const double mx = 0.5 * (pos[0] + p[0]), my = 0.5 * (pos[1] + p[1]), mz = 0.5 * (pos[2] + p[2]);
+      const int bvh = (__popc(um) >= 2) ? volume(c, vol).bvh : 0;
+      while (mb) {
+        const int src = __ffs(mb) - 1;
+        mb &= mb - 1;
+        int32_t* list = cand + kCandCap * ((threadIdx.x & ~31) + src);
+        const int n = bvh_candidates(c, c.bvh[__shfl_sync(kFull, bvh, src)], __shfl_sync(kFull, mx, src), __shfl_sync(kFull, my, src),
+                                     __shfl_sync(kFull, mz, src), kCandRadius, list);
+        if (g0 == src) {
+          cache->qx = mx; cache->qy = my; cache->qz = mz;
+          cache->reach = n >= 0 ? kCandRadius : -1.0;
+          cache->list = list;
+          cache->count = n >= 0 ? n : 0;
+          cache->vol = vol; cache->queries = 0;
+        }
+      }
+    }
+    int face;
+    const double s_geo = nav_distance<BVH>(c, nav, query, P[0], P[1], P[2], U[0], U[1], U[2], vol, L, face, cache, nullptr, clear);
+    const unsigned hm = __ballot_sync(kFull, query && s_geo < L) & gmask;
+    // the first segment of the group that ends on a boundary decides (its lane computes the end state; the shuffles
+    // are unconditional because the groups of a warp differ)
+    const int src = hm ? __ffs(hm) - 1 : lane;
+    double r[10] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    int rf = -1, rc = 0;
+    if (hm && lane == src) {
+      double dh[3] = {D[0], D[1], D[2]};
+      double s_end = Sb + s_geo;
+      if (kind == 1) {
+        const double frac = s_geo / L;
+        if (field_kind == ADEPT_FIELD_UNIFORM) {
+          double ph[3];
+          helix(c.bhat, kappa, inv_kappa, H * frac, P, D, ph, dh);
+        } else {
+          double n = 0.0;
+#pragma unroll
+          for (int i = 0; i < 3; ++i) { dh[i] = D[i] + frac * (D1[i] - D[i]); n += dh[i] * dh[i]; }
+          n = rsqrt(n);
+#pragma unroll
+          for (int i = 0; i < 3; ++i) dh[i] *= n;
+        }
+        s_end = Sb + H * frac;
+      }
+      // (a straight segment advances along the direction itself, a chord along its unit vector; U is either)
+#pragma unroll
+      for (int i = 0; i < 3; ++i) { r[i] = P[i] + s_geo * U[i]; r[3 + i] = dh[i]; r[6 + i] = U[i]; }
+      r[9] = s_end;
+      rf = face;
+      rc = chords + li + (kind == 1 ? 1 : 0);
+    }
+#pragma unroll
+    for (int i = 0; i < 10; ++i) r[i] = __shfl_sync(kFull, r[i], src);
+    rf = __shfl_sync(kFull, rf, src);
+    rc = __shfl_sync(kFull, rc, src);
+    if (hm) {    // (only groups that are running have queries)
+#pragma unroll
+      for (int i = 0; i < 3; ++i) { pos[i] = r[i]; dir[i] = r[3 + i]; pushdir[i] = r[6 + i]; }
+      s_done = r[9]; face_hit = rf; chords = rc;
+      flag = 1; running = false;
+    } else if (running) {
+#pragma unroll
+      for (int i = 0; i < 3; ++i) { pos[i] = p[i]; dir[i] = d[i]; }
+      s_done = sd; chords = ch;
+      if (end >= 0) { flag = end; running = false; }
+    }
+  }
+  s_out = s_done;
+  chords_out = chords;
+  face_out = flag == 1 ? face_hit : -1;
+  return flag;
+}
+
 }  // namespace adept
