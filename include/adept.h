@@ -292,8 +292,9 @@ int adept_buffer_destroy(adept_buffer*);
 int adept_step_population(adept_ctx*, int event_slot, int n, const adept_track* in, adept_track* out, size_t out_cap,
                           size_t* n_out, void* cuda_stream);
 
-/* Test hook of the generic per-lane step (csrc/step.cuh), the form the persistent tail kernel runs: exactly one
- * step for each of n tracks, results in input order; secondaries[2*i + k]. */
+/* Test hook of the generic per-lane step (csrc/step.cuh: move and interaction chained in one lane, any species): exactly
+ * one step for each of n tracks, results in input order; secondaries[2*i + k].  Transport does not run this form; it is
+ * kept as a second, structurally different arm of the frozen-step parity tests (the first is adept_step_population). */
 int adept_step_frozen(adept_ctx*, int n, const adept_track* in, adept_step_result* out,
                       adept_track* secondaries, void* cuda_stream);
 

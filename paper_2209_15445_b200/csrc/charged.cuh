@@ -260,7 +260,7 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
   // one after the other, so a few hundred loopers packed into a few warps would take 32 x 16 chord queries
   // in sequence per step (measured 4 ms per population step on config 4), spread out they run in parallel.
   uint32_t g = kBlock;
-  while (g > kBlock / 32 && (n + (g >> 1) - 1) / (g >> 1) <= gridDim.x / 2) g >>= 1;   // (half the grid: the other species runs beside; at most a warp per track)
+  while (g > (kBlock / 32 > 4 ? kBlock / 32 : 4) && (n + (g >> 1) - 1) / (g >> 1) <= gridDim.x / 2) g >>= 1;   // (half the grid: the other species runs beside; at most a warp per track)
   const int lane_shift = __ffs(kBlock / g) - 1;            // every (1 << lane_shift)-th lane takes a track
   const uint32_t n_tiles = (n + g - 1) / g;
   if (blockIdx.x >= n_tiles) return;   // no tile for this block

@@ -259,13 +259,14 @@ __device__ __forceinline__ void tally_flush(BlockTally& t, const DevSlot& slot, 
     if (cut != 0.0) atomicAdd(&t.ledger[1], cut);
   }
   __syncthreads();
-  const int k = threadIdx.x;
-  if (k < 4) { if (t.ledger[k] != 0.0) atomicAdd(slot.ledger + k, t.ledger[k]); }
-  else if (k == 4) { if (t.steps) atomicAdd(&slot.stats->steps[species], static_cast<unsigned long long>(t.steps)); }
-  else if (k == 5) { if (t.chords) atomicAdd(&slot.stats->chords, t.chords); }
-  else if (k < 6 + 3) { if (t.secondaries[k - 6]) atomicAdd(&slot.stats->secondaries[k - 6], static_cast<unsigned long long>(t.secondaries[k - 6])); }
-  else if (k >= 32 && k < 32 + ADEPT_N_OUTCOMES) {
-    if (t.outcomes[k - 32]) atomicAdd(&slot.stats->outcomes[k - 32], static_cast<unsigned long long>(t.outcomes[k - 32]));
+  for (int k = threadIdx.x; k < 32 + ADEPT_N_OUTCOMES; k += kBlock) {   // (one pass for blocks of 64 threads and more)
+    if (k < 4) { if (t.ledger[k] != 0.0) atomicAdd(slot.ledger + k, t.ledger[k]); }
+    else if (k == 4) { if (t.steps) atomicAdd(&slot.stats->steps[species], static_cast<unsigned long long>(t.steps)); }
+    else if (k == 5) { if (t.chords) atomicAdd(&slot.stats->chords, t.chords); }
+    else if (k < 6 + 3) { if (t.secondaries[k - 6]) atomicAdd(&slot.stats->secondaries[k - 6], static_cast<unsigned long long>(t.secondaries[k - 6])); }
+    else if (k >= 32) {
+      if (t.outcomes[k - 32]) atomicAdd(&slot.stats->outcomes[k - 32], static_cast<unsigned long long>(t.outcomes[k - 32]));
+    }
   }
 }
 
