@@ -66,9 +66,10 @@ def parse():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4, 5],
-                    help="BASELINE.json config: 2 (default, the bench line), 3 (same + 1 T field), 4 (barrel, BVH, field map; extra), "
-                         "5 (16 barrel events on 16 streams; extra, 1 GPU)")
+    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5],
+                    help="BASELINE.json config: 2 (default, the bench line), 1 (256 x 1 GeV, the small case), 3 (config 2 + 1 T field), "
+                         "4 (barrel, BVH, field map), 5 (16 barrel events on 16 streams, 1 GPU); all but 2 are extras for BASELINE.md")
+    ap.add_argument("--species", default="e-", choices=["e-", "gamma"], help="primary of configs 1-3 (config 3 has a second run with gammas)")
     ap.add_argument("--events", type=int, default=0, help="events per batch (0 = 10000 for configs 2-3, 100 x 50 primaries for config 4)")
     ap.add_argument("--field", type=float, default=0.0, help="uniform Bz in tesla for configs 2-3 (config 3 sets 1.0)")
     ap.add_argument("--max-steps", type=int, default=0, help="looper cut S4 (0 = 1e6 for configs 2-3, 4096 for config 4)")
@@ -88,18 +89,23 @@ def parse():
     a = ap.parse_args()
     if a.config == 3 and a.field == 0.0:
         a.field = 1.0
-    a.events = a.events or (100 if a.config == 4 else (16 if a.config == 5 else 10000))
+    a.events = a.events or (100 if a.config == 4 else (16 if a.config == 5 else (256 if a.config == 1 else 10000)))
+    a.e_primary = 1000.0 if a.config == 1 else E_PRIMARY
+    a.spread = 0.0 if a.config == 1 else 1.0
     a.max_steps = a.max_steps or (4096 if a.config in (4, 5) else 1000000)
     return a
 
 
 def workload_name(args):
+    species = getattr(args, "species", "e-")
     if args.config == 4:
         return (f"config4: barrel of 61200 PbWO4 crystals + 10 Si shells, BVH navigation, solenoid field map (RK4), "
                 f"{args.events} events x 50 e-/gamma of 1-100 GeV, looper cut max_steps={args.max_steps}")
+    if args.config == 1:
+        return f"config1: {args.events} x 1 GeV {species} from the front face centre of the 50-layer Pb/LAr calorimeter, no field, 0.7 mm cuts"
     if args.field != 0.0:
-        return f"config3: {args.events} x 10 GeV e- in the 50-layer Pb/LAr calorimeter, uniform {args.field} T field, 0.7 mm cuts"
-    return f"config2: {args.events} x 10 GeV e- in the 50-layer Pb/LAr calorimeter, no field, 0.7 mm cuts"
+        return f"config3: {args.events} x 10 GeV {species} in the 50-layer Pb/LAr calorimeter, uniform {args.field} T field, 0.7 mm cuts"
+    return f"config2: {args.events} x 10 GeV {species} in the 50-layer Pb/LAr calorimeter, no field, 0.7 mm cuts"
 
 
 def shard_first_event(rank, events_per_rank):
@@ -129,14 +135,15 @@ def workload(args, first_event=0):
     else:
         g = geometry.calorimeter()
         fld = field.uniform_field(0, 0, args.field) if args.field != 0.0 else field.no_field()
-        prim = primaries.beam(args.events, E_PRIMARY, spread=1.0, seed=1, first_event=first_event)
+        prim = primaries.beam(args.events, getattr(args, "e_primary", E_PRIMARY), species=2 if getattr(args, "species", "e-") == "gamma" else 0,
+                              spread=getattr(args, "spread", 1.0), seed=1, first_event=first_event)
     mats, tabs, scal = materials.build_material_set(g.material_names)
     return g, tabs, scal, fld, prim
 
 
 # ----------------------------------------------------------------------------- CPU oracle legs
 def _oracle_worker(job):
-    config, first_event, n_events, field_bz, max_steps = job
+    config, first_event, n_events, field_bz, max_steps, e_primary, species, spread = job
     from oracle import binding as ob
     from paper_2209_15445_b200.inputs import field, geometry, materials, primaries
     if config == 4:     # the loop navigator over 61 212 volumes: low-energy primaries of the same generator
@@ -146,7 +153,7 @@ def _oracle_worker(job):
     else:
         g = geometry.calorimeter()
         fld = field.uniform_field(0, 0, field_bz) if field_bz != 0.0 else field.no_field()
-        prim = primaries.beam(n_events, E_PRIMARY, spread=1.0, seed=1, first_event=first_event)
+        prim = primaries.beam(n_events, e_primary, species=species, spread=spread, seed=1, first_event=first_event)
     _, tabs, scal = materials.build_material_set(g.material_names)
     o = ob.Oracle(g, tabs, scal, fld, max_steps=max_steps)
     tr = o.make_tracks(prim)
@@ -163,17 +170,21 @@ def oracle_throughput(args, events_per_core, cores=None):
     cores = cores or os.cpu_count() or 1
     if args.config == 4:
         events_per_core = 1
-    jobs = [(args.config, c * events_per_core, events_per_core, args.field, args.max_steps) for c in range(cores)]
+    sp = 2 if args.species == "gamma" else 0
+    if args.config == 1:
+        events_per_core = max(1, min(events_per_core, args.events // cores))       # the whole config is 256 showers
+    jobs = [(args.config, c * events_per_core, events_per_core, args.field, args.max_steps, args.e_primary, sp, args.spread)
+            for c in range(cores)]
     ctx = mp.get_context("spawn")
     with ctx.Pool(cores) as pool:
-        pool.map(_oracle_worker, [(2, 0, 1, 0.0, args.max_steps)] * cores)        # start-up (imports, build) untimed
+        pool.map(_oracle_worker, [(2, 0, 1, 0.0, args.max_steps, 1000.0, 0, 0.0)] * cores)        # start-up (imports, build) untimed
         t0 = time.perf_counter()
         res = pool.map(_oracle_worker, jobs)
         wall = time.perf_counter() - t0
     steps = sum(r[0] for r in res)
     sample = (f"{cores} events of 2 e-/gamma primaries of 0.2-2 GeV from config 4's generator in the full barrel (one oracle "
               f"process per core; the loop navigator makes full-energy events take minutes)" if args.config == 4 else
-              f"{cores * events_per_core} of the workload's 10 GeV e- showers ({events_per_core} consecutive events per core, "
+              f"{cores * events_per_core} of the workload's {args.e_primary / 1000:g} GeV {args.species} showers ({events_per_core} consecutive events per core, "
               f"one oracle process per core)")
     return {"steps": steps, "wall_s": wall, "steps_per_s": steps / wall, "showers_per_s": cores * events_per_core / wall,
             "cores": cores, "sample": sample, "events": cores * events_per_core}
@@ -412,7 +423,7 @@ def run_ours(args):
         }
         if world == 1 and not args.no_cpu_baseline and not args.profile:
             ob = oracle_throughput(args, args.cpu_events_per_core)
-            one = oracle_throughput(args, 48, cores=1)       # SURVEY.md §8(d) "oracle timing (i)": one thread
+            one = oracle_throughput(args, 16 if args.config == 1 else 48, cores=1)       # SURVEY.md §8(d) "oracle timing (i)": one thread
             line["cpu_baseline"] = {"value": ob["steps_per_s"], "unit": "steps/s", "cores": ob["cores"], "kind": "oracle",
                                     "sample": ob["sample"], "showers_per_s": ob["showers_per_s"],
                                     "value_1core": one["steps_per_s"], "sample_1core": one["sample"],

@@ -43,6 +43,12 @@ def test_bench_workloads_and_sharding():
     assert "uniform 1.0 T" in b.workload_name(a)
     a = argparse.Namespace(config=4, events=100, field=0.0, max_steps=4096)
     assert "max_steps=4096" in b.workload_name(a) and "61200" in b.workload_name(a)
+    a = argparse.Namespace(config=3, events=10000, field=1.0, max_steps=1000000, species="gamma")
+    assert "10 GeV gamma" in b.workload_name(a)
+    a = argparse.Namespace(config=1, events=256, field=0.0, max_steps=1000000, species="e-", e_primary=1000.0, spread=0.0)
+    assert b.workload_name(a).startswith("config1: 256 x 1 GeV e-")
+    _, _, _, _, p1 = b.workload(a)
+    assert len(p1["ekin"]) == 256 and (p1["ekin"] == 1000.0).all() and not p1["pos"].any()
     # ranks own disjoint, consecutive event ranges: Philox streams are keyed by event id
     assert [b.shard_first_event(r, 10000) for r in range(4)] == [0, 10000, 20000, 30000]
     assert b.BYTES_PER_STEP == 76 + 76 + 8
