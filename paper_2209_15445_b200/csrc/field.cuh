@@ -358,10 +358,13 @@ __device__ __forceinline__ int propagate_wide(const DevCtx& c, int nav, int shif
     if (running && nseg > 1) safe = nav_safety(c, vol, pos[0], pos[1], pos[2], own_only);
     const bool clear = kind == 1 && reach_end < safe;
     const bool query = running && (kind == 2 || (kind == 1 && (!clear || own_only)));
-    // ---- the group's candidate list (geom.cuh NavCache): rebuilt around the middle of the round when two or more of
-    // its segments are not covered by the list the group has
+    // ---- the group's candidate list (geom.cuh NavCache): when two or more of the round's segments are not covered by
+    // the list the group has, a new one is built around the middle of the round, its ball just large enough for all
+    // of them (up to kCandRadiusMax)
     if (BVH && cache && cand) {
       bool uncovered = false;
+      const double mx = 0.5 * (pos[0] + p[0]), my = 0.5 * (pos[1] + p[1]), mz = 0.5 * (pos[2] + p[2]);
+      double need_r = 0.0;
       if (query && nav == ADEPT_NAV_BVH) {
         const DevVolume& v = volume(c, vol);
         if (v.dcount > 0 && v.bvh >= 0) {
@@ -370,21 +373,29 @@ __device__ __forceinline__ int propagate_wide(const DevCtx& c, int nav, int shif
             const double ox = P[0] - cache->qx, oy = P[1] - cache->qy, oz = P[2] - cache->qz;
             uncovered = !(sqrt(ox * ox + oy * oy + oz * oz) + L <= cache->reach * (1.0 - 1.0e-9));
           }
+          const double ox = P[0] - mx, oy = P[1] - my, oz = P[2] - mz;
+          need_r = sqrt(ox * ox + oy * oy + oz * oz) + L;
         }
       }
       const unsigned um = __ballot_sync(kFull, uncovered) & gmask;
-      unsigned mb = __ballot_sync(kFull, li == 0 && __popc(um) >= 2);
-      const double mx = 0.5 * (pos[0] + p[0]), my = 0.5 * (pos[1] + p[1]), mz = 0.5 * (pos[2] + p[2]);
-      const int bvh = (__popc(um) >= 2) ? volume(c, vol).bvh : 0;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {   // largest need of the group (groups are aligned runs of W lanes)
+        const double other = __shfl_xor_sync(kFull, need_r, o);
+        if (o < W) need_r = fmax(need_r, other);
+      }
+      const double rho = fmax(kCandRadius, need_r * (1.0 + 1.0e-6) + 1.0e-9);
+      const bool rebuild = __popc(um) >= 2 && rho <= kCandRadiusMax;
+      unsigned mb = __ballot_sync(kFull, li == 0 && rebuild);
+      const int bvh = rebuild ? volume(c, vol).bvh : 0;
       while (mb) {
         const int src = __ffs(mb) - 1;
         mb &= mb - 1;
         int32_t* list = cand + kCandCap * ((threadIdx.x & ~31) + src);
         const int n = bvh_candidates(c, c.bvh[__shfl_sync(kFull, bvh, src)], __shfl_sync(kFull, mx, src), __shfl_sync(kFull, my, src),
-                                     __shfl_sync(kFull, mz, src), kCandRadius, list);
+                                     __shfl_sync(kFull, mz, src), __shfl_sync(kFull, rho, src), list);
         if (g0 == src) {
           cache->qx = mx; cache->qy = my; cache->qz = mz;
-          cache->reach = n >= 0 ? kCandRadius : -1.0;
+          cache->reach = n >= 0 ? rho : -1.0;
           cache->list = list;
           cache->count = n >= 0 ? n : 0;
           cache->vol = vol; cache->queries = 0;

@@ -355,7 +355,10 @@ __device__ __forceinline__ int bvh_point(const DevCtx& c, const BvhT<R>& b, R px
 //    ball: 16 chords per step, step after step, of the e+- that spiral in the gaps (profiles/r1e_configs34.md:
 //    82 % of the instructions of such a step were traversals).
 constexpr int kCandCap = 8;             // entries of a lane-built list (a gap corner touches 4 crystals)
-constexpr double kCandRadius = 0.25;    // [cm] radius of the ball a lane-built list covers
+constexpr double kCandRadius = 0.25;    // [cm] least radius of the ball a lane-built list covers ...
+constexpr double kCandRadiusMax = 1.0;  // ... and the largest: the ball is sized to serve the next few segments of the track that asks
+                                        // (four times the segment that triggered it; a list whose ball the very next chord leaves is
+                                        // pure cost -- profiles/r2_summary.md: 18 % of the samples of a config-4 launch were such builds)
 constexpr int kNbrCap = 12;             // entries of a per-daughter list
 struct NavCache {
   double qx, qy, qz, reach;             // see above (reach <= 0: no list)
@@ -509,7 +512,8 @@ __device__ __forceinline__ R nav_distance_body(const DevCtx& c, int nav, bool ac
   }
   if constexpr (std::is_same<R, double>::value) if (cache) {   // a lane that keeps traversing in the same volume gets a list of its own around where it is
     bool build = false;
-    if (need && cand) {
+    const double rho = fmax(kCandRadius, 4.0 * static_cast<double>(s_max));
+    if (need && cand && rho <= kCandRadiusMax) {   // (a longer segment would leave any ball that still fits a list)
       if (cache->vol != vol) { cache->vol = vol; cache->queries = 0; cache->reach = -1.0; }
       build = ++cache->queries >= 2;
     }
@@ -519,10 +523,10 @@ __device__ __forceinline__ R nav_distance_body(const DevCtx& c, int nav, bool ac
       mb &= mb - 1;
       int32_t* mine = cand + kCandCap * ((threadIdx.x & ~31) + src);
       const int n = bvh_candidates(c, c.bvh[__shfl_sync(kFull, bvh, src)], __shfl_sync(kFull, px, src), __shfl_sync(kFull, py, src),
-                                   __shfl_sync(kFull, pz, src), kCandRadius, mine);
+                                   __shfl_sync(kFull, pz, src), __shfl_sync(kFull, rho, src), mine);
       if (lane == src) {
         cache->qx = px; cache->qy = py; cache->qz = pz;
-        cache->reach = n >= 0 ? kCandRadius : -1.0;
+        cache->reach = n >= 0 ? rho : -1.0;
         cache->list = mine;
         cache->count = n >= 0 ? n : 0;
         cache->queries = 0;

@@ -3,7 +3,10 @@ barrel (or a y-z picture of the calorimeter) taken with the transport path's own
 the BVH navigator and once with the loop over all daughters; the two pictures must be identical, pixel for
 pixel.  Headless: the picture goes to a PPM file.
 
-  python -m paper_2209_15445_b200.raycast [--geometry barrel|calorimeter] [--size 1024x512] [--out picture.ppm] [--skip-loop]
+  python -m paper_2209_15445_b200.raycast [--geometry barrel|calorimeter] [--size 1024x512] [--out picture.ppm] [--skip-loop] [--fp32]
+
+--fp32 also takes the picture through the single-precision copy of the geometry and reports how it differs from
+the fp64 picture and the ratio of the two ray rates.
 """
 import argparse
 import time
@@ -49,6 +52,7 @@ def main():
     ap.add_argument("--size", default="1024x512")
     ap.add_argument("--out", default="")
     ap.add_argument("--skip-loop", action="store_true", help="BVH picture only (the loop navigator tests 61 200 crystals per step)")
+    ap.add_argument("--fp32", action="store_true", help="also the single-precision geometry mode (BVH navigator)")
     args = ap.parse_args()
     from . import adept
     w, h = (int(x) for x in args.size.split("x"))
@@ -56,17 +60,25 @@ def main():
     _, tabs, scal = materials.build_material_set(g.material_names)
     pos, d = barrel_rays(w, h) if args.geometry == "barrel" else calorimeter_rays(w, h)
     a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=1 << 10)
-    res = {}
-    for name, nav in (("bvh", adept.NAV_BVH), ("loop", adept.NAV_LOOP)):
-        if nav == adept.NAV_LOOP and args.skip_loop:
+    res, rate = {}, {}
+    for name, nav in (("bvh", adept.NAV_BVH), ("loop", adept.NAV_LOOP), ("bvh_fp32", adept.NAV_BVH_F32)):
+        if (nav == adept.NAV_LOOP and args.skip_loop) or (nav == adept.NAV_BVH_F32 and not args.fp32):
             continue
         a.raycast(pos[:1024], d[:1024], nav)          # warm-up
         t0 = time.perf_counter()
         col, nx, ms = a.raycast(pos, d, nav)
         res[name] = (col, nx)
+        rate[name] = len(col) / ms * 1e3
         print(f"{name}: {len(col)} rays, {int(nx.sum())} boundary crossings, kernel {ms:.2f} ms = {len(col) / ms * 1e3:.3e} rays/s, "
               f"{nx.sum() / ms * 1e3:.3e} crossings/s (host call {1e3 * (time.perf_counter() - t0):.1f} ms)")
-    if len(res) == 2:
+    if "bvh_fp32" in res:
+        c64, n64 = res["bvh"]
+        c32, n32 = res["bvh_fp32"]
+        same_nx = n32 == n64
+        rel = np.abs(c32[same_nx] - c64[same_nx]) / np.maximum(c64[same_nx], 1e-30)
+        print(f"fp32 vs fp64 picture: {100.0 * same_nx.mean():.3f} % of the rays cross the same number of boundaries; column density of those "
+              f"differs by at most {rel.max():.2e} relative; fp32 / fp64 ray rate {rate['bvh_fp32'] / rate['bvh']:.2f}")
+    if "loop" in res:
         same = np.array_equal(res["bvh"][1], res["loop"][1]) and np.array_equal(res["bvh"][0], res["loop"][0])
         print("BVH picture == loop picture, bit for bit:", same)
     if args.out:
