@@ -489,8 +489,9 @@ __device__ __forceinline__ R nav_distance_body(const DevCtx& c, int nav, bool ac
     }
   }
   if (!BVH) return s;
-  if constexpr (std::is_same<R, double>::value) if (cache) {   // the lane's candidate list first (lane-local): final if the segment cannot leave its reach
-    if (need && cache->reach > 0.0 && cache->vol == vol) {
+  if constexpr (std::is_same<R, double>::value) if (cache) {
+    // the lane's candidate list first (lane-local): final if the segment cannot leave its reach
+    const auto ask_list = [&]() {
       for (int j = 0; j < cache->count; ++j) {
         const int pv = cache->list[j];
         const double e = entry_distance_within(c, pv, px, py, pz, dx, dy, dz, s);
@@ -498,24 +499,18 @@ __device__ __forceinline__ R nav_distance_body(const DevCtx& c, int nav, bool ac
       }
       const double ox = px - cache->qx, oy = py - cache->qy, oz = pz - cache->qz;
       if (sqrt(ox * ox + oy * oy + oz * oz) + s <= cache->reach * (1.0 - 1.0e-9)) need = false;
-    }
-  }
-  unsigned m = __ballot_sync(kFull, need);
-  while (m) {
-    const int src = __ffs(m) - 1;
-    m &= m - 1;
-    int hit;
-    const R r = bvh_ray<R>(c, Geo<R>::bvh(c, __shfl_sync(kFull, bvh, src)), __shfl_sync(kFull, px, src),
-                           __shfl_sync(kFull, py, src), __shfl_sync(kFull, pz, src), __shfl_sync(kFull, dx, src),
-                           __shfl_sync(kFull, dy, src), __shfl_sync(kFull, dz, src), __shfl_sync(kFull, s, src), hit);
-    if (lane == src && r < s) { s = r; face = hit >= 0 ? -2 - hit : -1; }
-  }
-  if constexpr (std::is_same<R, double>::value) if (cache) {   // a lane that keeps traversing in the same volume gets a list of its own around where it is
+    };
+    if (need && cache->reach > 0.0 && cache->vol == vol) ask_list();
+    // A lane that keeps asking in the same volume -- its list has just run out, or this is its second uncovered
+    // query there -- gets a list of its own around where it is, built by the warp (one cooperative walk, the price
+    // of one traversal) BEFORE the query is answered, so that the list answers it and the next few: a ball of four
+    // segment lengths.  (A longer segment would leave any ball that still fits a list; a first query in a volume
+    // is a traversal: most tracks only pass through.)
     bool build = false;
     const double rho = fmax(kCandRadius, 4.0 * static_cast<double>(s_max));
-    if (need && cand && rho <= kCandRadiusMax) {   // (a longer segment would leave any ball that still fits a list)
+    if (need && cand && rho <= kCandRadiusMax) {
       if (cache->vol != vol) { cache->vol = vol; cache->queries = 0; cache->reach = -1.0; }
-      build = ++cache->queries >= 2;
+      build = cache->reach > 0.0 || ++cache->queries >= 2;
     }
     unsigned mb = __ballot_sync(kFull, build);
     while (mb) {
@@ -529,9 +524,20 @@ __device__ __forceinline__ R nav_distance_body(const DevCtx& c, int nav, bool ac
         cache->reach = n >= 0 ? rho : -1.0;
         cache->list = mine;
         cache->count = n >= 0 ? n : 0;
-        cache->queries = 0;
+        cache->queries = n >= 0 ? 0 : -6;  // (did not fit: traverse now, and the next seven times)
       }
     }
+    if (build && cache->reach > 0.0) ask_list();
+  }
+  unsigned m = __ballot_sync(kFull, need);
+  while (m) {
+    const int src = __ffs(m) - 1;
+    m &= m - 1;
+    int hit;
+    const R r = bvh_ray<R>(c, Geo<R>::bvh(c, __shfl_sync(kFull, bvh, src)), __shfl_sync(kFull, px, src),
+                           __shfl_sync(kFull, py, src), __shfl_sync(kFull, pz, src), __shfl_sync(kFull, dx, src),
+                           __shfl_sync(kFull, dy, src), __shfl_sync(kFull, dz, src), __shfl_sync(kFull, s, src), hit);
+    if (lane == src && r < s) { s = r; face = hit >= 0 ? -2 - hit : -1; }
   }
   return s;
 }
