@@ -14,11 +14,14 @@ __device__ __forceinline__ void cross3(const double a[3], const double b[3], dou
   c[2] = a[0] * b[1] - a[1] * b[0];
 }
 
-// F6: B = (0, 0, bz(r, z)), bilinear, clamped outside the grid
+// F6: B = (0, 0, bz(r, z)), bilinear, clamped outside the grid.  FIELD >= 0: the field kind, known at compile time
+// (no test of it per evaluation: four evaluations per RK4 chord); -1: read from the context.
+template <int FIELD = -1>
 __device__ __forceinline__ void field_at(const DevCtx& c, const double p[3], double B[3]) {
-  if (c.field_kind == ADEPT_FIELD_UNIFORM) { B[0] = c.B[0]; B[1] = c.B[1]; B[2] = c.B[2]; return; }
+  const int kind = FIELD >= 0 ? FIELD : c.field_kind;
+  if (kind == ADEPT_FIELD_UNIFORM) { B[0] = c.B[0]; B[1] = c.B[1]; B[2] = c.B[2]; return; }
   B[0] = B[1] = B[2] = 0.0;
-  if (c.field_kind != ADEPT_FIELD_MAP_RZ) return;
+  if (kind != ADEPT_FIELD_MAP_RZ) return;
   const double r = sqrt(p[0] * p[0] + p[1] * p[1]);
   // (grid coordinates by multiplication with the inverse spacing: exact for the 1 cm grid of the configs, within
   // an ulp otherwise, and the interpolant is continuous across cells)
@@ -85,6 +88,7 @@ __device__ __forceinline__ void helix(const double b[3], double kappa, double in
 }
 
 // F1, F3: one classical RK4 step on (x, d): x' = d, d' = (q kCB / p) d x B(x); B0 = B(p), already known
+template <int FIELD = -1>
 __device__ __forceinline__ void rk4(const DevCtx& c, int charge, double pmom, double h, const double p[3],
                                     const double d[3], const double B0[3], double p1[3], double d1[3]) {
   const double kap = charge * kCB / pmom;
@@ -92,15 +96,15 @@ __device__ __forceinline__ void rk4(const DevCtx& c, int charge, double pmom, do
   cross3(d, B0, t);
 #pragma unroll
   for (int i = 0; i < 3; ++i) { k1v[i] = kap * t[i]; x[i] = p[i] + 0.5 * h * d[i]; v[i] = d[i] + 0.5 * h * k1v[i]; }
-  field_at(c, x, B);
+  field_at<FIELD>(c, x, B);
   cross3(v, B, t);
 #pragma unroll
   for (int i = 0; i < 3; ++i) { k2x[i] = v[i]; k2v[i] = kap * t[i]; x[i] = p[i] + 0.5 * h * k2x[i]; v[i] = d[i] + 0.5 * h * k2v[i]; }
-  field_at(c, x, B);
+  field_at<FIELD>(c, x, B);
   cross3(v, B, t);
 #pragma unroll
   for (int i = 0; i < 3; ++i) { k3x[i] = v[i]; k3v[i] = kap * t[i]; x[i] = p[i] + h * k3x[i]; v[i] = d[i] + h * k3v[i]; }
-  field_at(c, x, B);
+  field_at<FIELD>(c, x, B);
   cross3(v, B, t);
   double n = 0.0;
 #pragma unroll
@@ -157,7 +161,7 @@ __device__ __forceinline__ int propagate(const DevCtx& c, int nav, bool active, 
         double bperp = 0.0, h_max = 0.0;
         const bool curved = charge != 0 && field_kind != ADEPT_FIELD_NONE;   // gammas go straight
         if (curved && (field_kind != ADEPT_FIELD_UNIFORM || h_step < 0.0)) {
-          field_at(c, pos, B);
+          field_at<FIELD>(c, pos, B);
           double dxB[3];
           cross3(dir, B, dxB);
           bperp = sqrt(dxB[0] * dxB[0] + dxB[1] * dxB[1] + dxB[2] * dxB[2]);
@@ -183,7 +187,7 @@ __device__ __forceinline__ int propagate(const DevCtx& c, int nav, bool active, 
           last = h_max >= rest;
           h = last ? rest : h_max;
           if (field_kind == ADEPT_FIELD_UNIFORM) helix(c.bhat, kappa, inv_kappa, h, pos, dir, p1, d1);
-          else rk4(c, charge, pmom, h, pos, dir, B, p1, d1);
+          else rk4<FIELD>(c, charge, pmom, h, pos, dir, B, p1, d1);
           chord = true;
           // the chord needs no geometry query if it is shorter than the clearance left (a chord's length never
           // exceeds its arc's, so h bounds it)
@@ -302,7 +306,7 @@ __device__ __forceinline__ int propagate_wide(const DevCtx& c, int nav, int shif
       if (sd >= s_phys) { end = 0; integ = false; continue; }
       double B[3] = {0.0, 0.0, 0.0}, h_max = 0.0;
       if (curved && (field_kind != ADEPT_FIELD_UNIFORM || h_step < 0.0)) {
-        field_at(c, p, B);
+        field_at<FIELD>(c, p, B);
         double dxB[3];
         cross3(d, B, dxB);
         const double bperp = sqrt(dxB[0] * dxB[0] + dxB[1] * dxB[1] + dxB[2] * dxB[2]);
@@ -335,7 +339,7 @@ __device__ __forceinline__ int propagate_wide(const DevCtx& c, int nav, int shif
         const double h = last ? rest : h_max;
         double p1[3], d1[3];
         if (field_kind == ADEPT_FIELD_UNIFORM) helix(c.bhat, kappa, inv_kappa, h, p, d, p1, d1);
-        else rk4(c, charge, pmom, h, p, d, B, p1, d1);
+        else rk4<FIELD>(c, charge, pmom, h, p, d, B, p1, d1);
         if (li == j) {
           kind = 1; H = h; Sb = sd; reach_end = cum + h;
           const double cv[3] = {p1[0] - p[0], p1[1] - p[1], p1[2] - p[2]};

@@ -354,10 +354,20 @@ __device__ __forceinline__ int bvh_point(const DevCtx& c, const BvhT<R>& b, R px
 //  * per lane, built on the spot by the warp (bvh_candidates) around a track that keeps asking from within a small
 //    ball: 16 chords per step, step after step, of the e+- that spiral in the gaps (profiles/r1e_configs34.md:
 //    82 % of the instructions of such a step were traversals).
-constexpr int kCandCap = 8;             // entries of a lane-built list (a gap corner touches 4 crystals)
+#ifndef ADEPT_CAND_CAP
+#define ADEPT_CAND_CAP 12
+#endif
+#ifndef ADEPT_CAND_MULT
+#define ADEPT_CAND_MULT 8.0
+#endif
+#ifndef ADEPT_CAND_RMAX
+#define ADEPT_CAND_RMAX 2.0
+#endif
+constexpr int kCandCap = ADEPT_CAND_CAP;             // entries of a lane-built list (a gap corner touches 4 crystals)
+// (measured on configs 4 / 5, profiles/r2_summary.md: cap 8, ball 4 segments <= 1 cm: 1130 ms / 21.7 events/s; 12, 8, 2 cm: 1084 / 22.6)
 constexpr double kCandRadius = 0.25;    // [cm] least radius of the ball a lane-built list covers ...
-constexpr double kCandRadiusMax = 1.0;  // ... and the largest: the ball is sized to serve the next few segments of the track that asks
-                                        // (four times the segment that triggered it; a list whose ball the very next chord leaves is
+constexpr double kCandRadiusMax = ADEPT_CAND_RMAX;  // ... and the largest: the ball is sized to serve the next few segments of the track that asks
+                                        // (ADEPT_CAND_MULT times the segment that triggered it; a list whose ball the very next chord leaves is
                                         // pure cost -- profiles/r2_summary.md: 18 % of the samples of a config-4 launch were such builds)
 constexpr int kNbrCap = 12;             // entries of a per-daughter list
 struct NavCache {
@@ -503,11 +513,11 @@ __device__ __forceinline__ R nav_distance_body(const DevCtx& c, int nav, bool ac
     if (need && cache->reach > 0.0 && cache->vol == vol) ask_list();
     // A lane that keeps asking in the same volume -- its list has just run out, or this is its second uncovered
     // query there -- gets a list of its own around where it is, built by the warp (one cooperative walk, the price
-    // of one traversal) BEFORE the query is answered, so that the list answers it and the next few: a ball of four
-    // segment lengths.  (A longer segment would leave any ball that still fits a list; a first query in a volume
+    // of one traversal) BEFORE the query is answered, so that the list answers it and the next few: a ball of
+    // ADEPT_CAND_MULT segment lengths.  (A longer segment would leave any ball that still fits a list; a first query in a volume
     // is a traversal: most tracks only pass through.)
     bool build = false;
-    const double rho = fmax(kCandRadius, 4.0 * static_cast<double>(s_max));
+    const double rho = fmax(kCandRadius, ADEPT_CAND_MULT * static_cast<double>(s_max));
     if (need && cand && rho <= kCandRadiusMax) {
       if (cache->vol != vol) { cache->vol = vol; cache->queries = 0; cache->reach = -1.0; }
       build = cache->reach > 0.0 || ++cache->queries >= 2;
