@@ -264,8 +264,11 @@ __device__ __forceinline__ int propagate(const DevCtx& c, int nav, bool active, 
 // chord k+1 starts where chord k ends, whether or not chord k was tested yet.  So the lanes of the group
 // integrate up to W chords ahead (all lanes redundantly, in lockstep; lane j keeps chord j), then lane j asks
 // the geometry about chord j, and the first chord that ends on a boundary -- exactly the one the sequential
-// loop would have stopped at -- decides the step; what was integrated beyond it is dropped.  Every chord and
-// every query is computed by the same arithmetic as in propagate(), so the result is bit-identical.
+// loop would have stopped at -- decides the step; what was integrated beyond it is dropped.  On a field map every
+// chord and every query is computed by the same arithmetic as in propagate(), so the result is bit-identical.  In a
+// uniform field not even the integration is serial: the helix is exact for any arc length, so lane j evaluates the
+// end of chord j directly from the start of the round (same chord lengths, accumulated by the same additions; end
+// points equal to those of the chord-by-chord composition to rounding).
 // All lanes of a group pass the same track; `cache` is the group's candidate list (kept identical in its lanes).
 template <int FIELD, bool BVH>
 __device__ __forceinline__ int propagate_wide(const DevCtx& c, int nav, int shift, bool active, int charge, double ekin, double pos[3],
@@ -329,31 +332,70 @@ __device__ __forceinline__ int propagate_wide(const DevCtx& c, int nav, int shif
 #pragma unroll
           for (int i = 0; i < 3; ++i) { P[i] = p[i]; D[i] = d[i]; U[i] = d[i]; }
         }
+        if (field_kind != ADEPT_FIELD_UNIFORM) {
 #pragma unroll
-        for (int i = 0; i < 3; ++i) p[i] += rest * d[i];
+          for (int i = 0; i < 3; ++i) p[i] += rest * d[i];
+        }
         sd = s_phys; nseg = j + 1; end = 0; integ = false;
       } else if (ch >= c.chord_budget) {
         end = 2; integ = false;
       } else {
         const bool last = h_max >= rest;
         const double h = last ? rest : h_max;
-        double p1[3], d1[3];
-        if (field_kind == ADEPT_FIELD_UNIFORM) helix(c.bhat, kappa, inv_kappa, h, p, d, p1, d1);
-        else rk4<FIELD>(c, charge, pmom, h, p, d, B, p1, d1);
-        if (li == j) {
-          kind = 1; H = h; Sb = sd; reach_end = cum + h;
-          const double cv[3] = {p1[0] - p[0], p1[1] - p[1], p1[2] - p[2]};
-          const double L2 = cv[0] * cv[0] + cv[1] * cv[1] + cv[2] * cv[2];
-          const double iL = rsqrt(L2);
-          L = L2 * iL;
+        if (field_kind == ADEPT_FIELD_UNIFORM) {
+          // the helix is known in closed form: only the arc lengths are accumulated here (by the same additions as in
+          // the sequential loop); every lane evaluates its own chord's end point after the loop, all at once
+          if (li == j) { kind = 1; H = h; Sb = sd; reach_end = cum + h; }
+        } else {
+          double p1[3], d1[3];
+          rk4<FIELD>(c, charge, pmom, h, p, d, B, p1, d1);
+          if (li == j) {
+            kind = 1; H = h; Sb = sd; reach_end = cum + h;
+            const double cv[3] = {p1[0] - p[0], p1[1] - p[1], p1[2] - p[2]};
+            const double L2 = cv[0] * cv[0] + cv[1] * cv[1] + cv[2] * cv[2];
+            const double iL = rsqrt(L2);
+            L = L2 * iL;
 #pragma unroll
-          for (int i = 0; i < 3; ++i) { P[i] = p[i]; D[i] = d[i]; D1[i] = d1[i]; U[i] = cv[i] * iL; }
+            for (int i = 0; i < 3; ++i) { P[i] = p[i]; D[i] = d[i]; D1[i] = d1[i]; U[i] = cv[i] * iL; }
+          }
+#pragma unroll
+          for (int i = 0; i < 3; ++i) { p[i] = p1[i]; d[i] = d1[i]; }
         }
-#pragma unroll
-        for (int i = 0; i < 3; ++i) { p[i] = p1[i]; d[i] = d1[i]; }
         sd = last ? s_phys : sd + h;
         cum += h; ++ch; nseg = j + 1;
         if (last) { end = 0; integ = false; }
+      }
+    }
+    if (field_kind == ADEPT_FIELD_UNIFORM) {
+      // Exact helix: lane li evaluates the end of chord li from the round's start, arc length = the accumulated
+      // chord lengths (F3 holds for any arc; the sequential loop composes the same rotation chord by chord, so
+      // the two agree to rounding, not bit for bit); a segment starts where the previous lane's chord ends.
+      double E[3] = {pos[0], pos[1], pos[2]}, F[3] = {dir[0], dir[1], dir[2]};
+      if (kind == 1) helix(c.bhat, kappa, inv_kappa, reach_end, pos, dir, E, F);
+      double Ep[3], Fp[3];
+#pragma unroll
+      for (int i = 0; i < 3; ++i) { Ep[i] = __shfl_up_sync(kFull, E[i], 1); Fp[i] = __shfl_up_sync(kFull, F[i], 1); }
+      if (li == 0) {
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { Ep[i] = pos[i]; Fp[i] = dir[i]; }
+      }
+      if (kind == 1) {
+        const double cv[3] = {E[0] - Ep[0], E[1] - Ep[1], E[2] - Ep[2]};
+        const double L2 = cv[0] * cv[0] + cv[1] * cv[1] + cv[2] * cv[2];
+        const double iL = rsqrt(L2);
+        L = L2 * iL;
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { P[i] = Ep[i]; D[i] = Fp[i]; D1[i] = F[i]; U[i] = cv[i] * iL; }
+      } else if (kind == 2) {   // the straight last segment (a track along B) starts at the end of the chords before it
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { P[i] = Ep[i]; D[i] = Fp[i]; U[i] = Fp[i]; E[i] = Ep[i] + L * Fp[i]; F[i] = Fp[i]; }
+      }
+      // the state after the round's last segment, for every lane of the group
+      const int src = g0 + (nseg > 0 ? nseg - 1 : 0);
+#pragma unroll
+      for (int i = 0; i < 3; ++i) {
+        const double e = __shfl_sync(kFull, E[i], src), f = __shfl_sync(kFull, F[i], src);
+        if (nseg > 0) { p[i] = e; d[i] = f; }
       }
     }
     // ---- which segments need a geometry query (nav_safety, as in propagate(): one clearance around the round's start)
