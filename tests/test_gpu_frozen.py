@@ -129,9 +129,11 @@ def _run_case(ob, geom_set, fld, prim, per_species, stride, elements=None, **cfg
     dedx = _dedx(o, g, scal, pre)
     a = adept.Adept(g, tabs, scal, fld, track_capacity=1 << 18, leak_capacity=1 << 18, elements=elements, **cfg)
     worst_p = check_population(a, o, g, scal, fld, pre, ores, osec, dedx=dedx)
-    # a small batch takes the sparse-tile path of the charged kernel (a few tracks per block)
-    few = np.concatenate([np.where(pre["species"] == sp)[0][:700] for sp in range(3)])
-    check_population(a, o, g, scal, fld, pre[few], ores[few], osec[few], dedx=dedx[few])
+    # small batches take the sparse-tile path of the charged kernel: 32, 16 and 8 lanes per track, i.e. in a field the
+    # wide chord loop with one and with two rounds of chords per step (csrc/field.cuh propagate_wide)
+    for m in (700, 2000, 4000):
+        few = np.concatenate([np.where(pre["species"] == sp)[0][:m] for sp in range(3)])
+        check_population(a, o, g, scal, fld, pre[few], ores[few], osec[few], dedx=dedx[few])
     n_single = check_per_track_deposits(a, g, scal, fld, pre, ores, osec, dedx)
     worst_g = check_generic(a, g, scal, fld, pre, ores, osec, dedx)
     a.close()
