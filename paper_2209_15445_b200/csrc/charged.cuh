@@ -259,8 +259,12 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
   // (g tracks per tile, one lane in every 128/g): the warp-cooperative BVH serves the queries of a warp
   // one after the other, so a few hundred loopers packed into a few warps would take 32 x 16 chord queries
   // in sequence per step (measured 4 ms per population step on config 4), spread out they run in parallel.
+  // (the two species share the resident blocks: the tiles of both together must fit one wave; at most a warp per track)
+  // (without a field the other species is taken to be as numerous: nothing hangs on it there, and the kernel that fills
+  // the GPU on the bench configuration reads one counter less)
+  const uint32_t n_other = FIELD == ADEPT_FIELD_NONE ? n : min(cnt->count[parity][species ^ 1].v, c.capacity);   // e- = 0, e+ = 1
   uint32_t g = kBlock;
-  while (g > (kBlock / 32 > 4 ? kBlock / 32 : 4) && (n + (g >> 1) - 1) / (g >> 1) <= gridDim.x / 2) g >>= 1;   // (half the grid: the other species runs beside; at most a warp per track)
+  while (g > (kBlock / 32 > 4 ? kBlock / 32 : 4) && (n + (g >> 1) - 1) / (g >> 1) + (n_other + (g >> 1) - 1) / (g >> 1) <= gridDim.x) g >>= 1;
   const int lane_shift = __ffs(kBlock / g) - 1;            // every (1 << lane_shift)-th lane takes a track
   const uint32_t n_tiles = (n + g - 1) / g;
   if (blockIdx.x >= n_tiles) return;   // no tile for this block
