@@ -19,8 +19,13 @@
 
 namespace adept {
 
+// resident blocks per SM asked of the compiler (measured, profiles/r2_summary.md): without a BVH 6 (80 registers, a few
+// bytes of spill; config-2 pass 35.65 -> 35.17 ms over 5 blocks; 7 and 8 blocks: 36.3, 38.2); with the traversal code 5 (96)
 #ifndef ADEPT_MINB_G2
-#define ADEPT_MINB_G2 5
+#define ADEPT_MINB_G2 6
+#endif
+#ifndef ADEPT_MINB_G2B
+#define ADEPT_MINB_G2B 5
 #endif
 
 // per-thread outcome counters, 10 bits per field, folded into the block tally every 1023 tiles
@@ -164,7 +169,7 @@ __device__ __forceinline__ void gamma_lane(const DevCtx& c, const DevSlot& slot,
 }
 
 template <bool BVH, bool MULTI>
-__global__ void __launch_bounds__(kBlock, ADEPT_MINB_G2)
+__global__ void __launch_bounds__(kBlock, BVH ? ADEPT_MINB_G2B : ADEPT_MINB_G2)
 gamma_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot, int parity) {
   constexpr int species = ADEPT_GAMMA;
   const TrackSoA& cur = slot.buf[parity][species];
