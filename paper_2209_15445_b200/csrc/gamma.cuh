@@ -78,19 +78,23 @@ __device__ __forceinline__ void gamma_lane(const DevCtx& c, const DevSlot& slot,
       } else {
         fate = FATE_GO;
         mat = volume(c, vol).material;
-        {  // the rows of a vacuum are zero (adept_init), so no material flag has to be read first
+        {  // the rows of a vacuum are zero (adept_init), so no material flag has to be read first.
+          // Order: the two dependent loads of this phase (material of the volume, then the table rows) are each
+          // followed by arithmetic that does not need them -- the grid position and the Philox block, then -ln U0
+          // -- so that their latency is covered by the lane's own work (a photon in vacuum computes them in vain).
           const GridPos gp = grid_pos(c, T0);
+          Stream u;
+          u.init(T.u[0][t], c.seed, T.id[t], step);
+          const double u0 = u.uniform(0), u1 = u.uniform(1);
           const double* tab = c.tab_g + (static_cast<size_t>(mat) * kNGrid + gp.i) * kRowG;
           const Row4 r0 = load_row4(tab), r1 = load_row4(tab + kRowG);
+          const double nlu0 = -log_pos(u0);
           const double x0 = lerp_col(r0, r1, 0, gp.f);                                 // Compton
           const double x1 = T0 > 2.0 * kMe ? lerp_col(r0, r1, 1, gp.f) : 0.0;          // pair, exact threshold (P2)
           const double se = lerp_col(r0, r1, 2, gp.f);                                 // photoelectric
           const double stot = x0 + x1 + se;
           if (stot > 0.0) {
-            Stream u;
-            u.init(T.u[0][t], c.seed, T.id[t], step);
-            s_phys = div_pos(-log_pos(u.uniform(0)), stot);
-            const double u1 = u.uniform(1);
+            s_phys = div_pos(nlu0, stot);
             process = ADEPT_OUT_PHOTO;
             if (u1 * stot < x0) process = ADEPT_OUT_COMPTON;
             else if (u1 * stot < x0 + x1) process = ADEPT_OUT_PAIR;
