@@ -412,7 +412,9 @@ def run_ours(args):
                          "peak_source": peak_src, "launches": int(kn[dom]), "avg_launch_ms": float(kms[dom] / max(kn[dom], 1)),
                          "algorithmic_bytes_per_step": BYTES_PER_STEP, "per_kernel": per_kernel,
                          "timing": f"CUDA events around every launch in {n_pass} instrumented passes after the timed region "
-                                   f"(kernels run one after the other; {np.mean(ims) if ims else 0:.2f} ms per instrumented pass)",
+                                   f"(kernels run one after the other; {np.mean(ims) if ims else 0:.2f} ms per instrumented pass)"
+                                   + ("; in the timed passes the gamma and e+- move kernels are the blocks of ONE launch (move_kernel: "
+                                      "no field, no BVH), the instrumented passes launch the same code as two kernels" if args.config in (1, 2) and args.field == 0.0 else ""),
                          "note": "latency/divergence bound fp64 Monte Carlo: see DESIGN.md \u00a75 and profiles/"},
             "iterations_per_step": (st.iterations - st0.iterations) / args.steps,
             "track_steps_per_species_per_step": {"e-": steps_sp[0] / n_pass, "e+": steps_sp[1] / n_pass, "gamma": steps_sp[2] / n_pass},

@@ -317,6 +317,7 @@ struct adept_ctx {
   // variants in which a lane takes several steps of its own track per launch (small populations)
   using Kernel = void (*)(DevCtx, DevSlot, int);
   Kernel k_move_gamma[2] = {nullptr, nullptr}, k_move_charged[2] = {nullptr, nullptr};
+  Kernel k_move_merged[2] = {nullptr, nullptr};   // one launch for all three species (charged.cuh move_kernel), or null
   bool timing_on = false;            // per-launch CUDA events active (adept_set_kernel_timing)
 };
 
@@ -702,6 +703,11 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   }
   ctx->grid_gamma = sms * std::max(occ_g, 1);
   ctx->grid_charged = sms * std::max(occ_c, 1);
+  if (f->kind == ADEPT_FIELD_NONE && !(cfg->navigator == ADEPT_NAV_BVH && !hb.empty()) && cfg->concurrent_species != 0 &&
+      ctx->grid_gamma == ctx->grid_charged) {
+    ctx->k_move_merged[0] = move_kernel<false>;
+    ctx->k_move_merged[1] = move_kernel<true>;
+  }
   ctx->grid_inter = sms * std::max(occ_i, 1);
 
   ctx->slots.resize(cfg->n_event_slots);
@@ -838,6 +844,12 @@ int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity, 
   }
   const bool timed = ctx->timing_on && !sh.tev.empty() && sh.tev_used + kEv <= static_cast<int>(sh.tev.size());
   // a timed pass runs the kernels one after the other, so that an event pair brackets one kernel alone
+  if (ctx->k_move_merged[multi] && !ctx->timing_on) {   // all three species in one launch
+    ctx->k_move_merged[multi]<<<dim3(ctx->grid_gamma, 3), kBlock, 0, st>>>(dc, sh.dev, parity);
+    interact_kernel<<<ctx->grid_inter, kBlock, 0, st>>>(dc, sh.dev, parity);
+    sh.launches += 2;
+    return ADEPT_OK;
+  }
   const bool fork = ctx->cfg.concurrent_species != 0 && !ctx->timing_on;
   cudaStream_t sc = fork ? sh.helper : st;   // stream of the charged move kernel
   if (fork) {

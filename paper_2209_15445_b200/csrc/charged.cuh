@@ -242,9 +242,8 @@ __device__ __forceinline__ void charged_lane(const DevCtx& c, const DevSlot& slo
 }
 
 template <int FIELD, bool BVH, bool MULTI>
-__global__ void __launch_bounds__(kBlock, FIELD == ADEPT_FIELD_NONE ? ADEPT_MINB_C2 : ADEPT_MINB_C2F)
-charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot, int parity) {
-  const int species = static_cast<int>(blockIdx.y);   // ADEPT_ELECTRON or ADEPT_POSITRON
+__device__ __forceinline__ void charged_move_body(const DevCtx& c, const DevSlot& slot, int parity, int species, BlockTally& tally,
+                                                  BlockReserve<5>& br, TilePipe& pipe, int32_t* cand_lists) {
   const bool positron = species == ADEPT_POSITRON;
   const TrackSoA& cur = slot.buf[parity][species];
   SlotCounters* cnt = slot.counters;
@@ -268,13 +267,9 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
   const int lane_shift = __ffs(kBlock / g) - 1;            // every (1 << lane_shift)-th lane takes a track
   const uint32_t n_tiles = (n + g - 1) / g;
   if (blockIdx.x >= n_tiles) return;   // no tile for this block
-  __shared__ BlockTally tally;
-  __shared__ BlockReserve<ND> br;
-  __shared__ TilePipe pipe;
   // candidate lists of the chord queries in a BVH volume (geom.cuh NavCache): one per lane, kept across the
   // tiles and steps of the launch
   constexpr bool kLists = BVH;
-  __shared__ int32_t cand_lists[kLists ? kBlock * kCandCap : 1];
   NavCache nav_cache;
   nav_cache_reset(nav_cache);
   NavCache* const cache = kLists ? &nav_cache : nullptr;
@@ -385,6 +380,30 @@ charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ De
     if (lane == 0 && ch) atomicAdd(&tally.chords, ch);
   }
   tally_flush(tally, slot, species, sum_dep, sum_cut);
+}
+
+template <int FIELD, bool BVH, bool MULTI>
+__global__ void __launch_bounds__(kBlock, FIELD == ADEPT_FIELD_NONE ? ADEPT_MINB_C2 : ADEPT_MINB_C2F)
+charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot, int parity) {
+  __shared__ BlockTally tally;
+  __shared__ BlockReserve<5> br;
+  __shared__ TilePipe pipe;
+  __shared__ int32_t cand_lists[BVH ? kBlock * kCandCap : 1];
+  charged_move_body<FIELD, BVH, MULTI>(c, slot, parity, static_cast<int>(blockIdx.y) /* e- or e+ */, tally, br, pipe, cand_lists);
+}
+
+// Without a field and without a BVH the photon and the e+- kernel need the same registers (80) and the same shared
+// memory, so one launch serves all three species of a population step: blockIdx.y = 0 photons (the longest, scheduled
+// first), 1 electrons, 2 positrons.  One launch and no fork/join between two streams per population step; the
+// per-kernel timing mode and the other field kinds keep the two kernels.
+template <bool MULTI>
+__global__ void __launch_bounds__(kBlock, ADEPT_MINB_C2)
+move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot, int parity) {
+  __shared__ BlockTally tally;
+  __shared__ BlockReserve<5> br;
+  __shared__ TilePipe pipe;
+  if (blockIdx.y == 0) gamma_move_body<false, MULTI>(c, slot, parity, tally, br, pipe);
+  else charged_move_body<ADEPT_FIELD_NONE, false, MULTI>(c, slot, parity, static_cast<int>(blockIdx.y) - 1, tally, br, pipe, nullptr);
 }
 
 }  // namespace adept

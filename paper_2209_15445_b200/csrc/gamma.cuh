@@ -172,9 +172,11 @@ __device__ __forceinline__ void gamma_lane(const DevCtx& c, const DevSlot& slot,
     r.post = post; r.edep = edep; r.T_pe = T_pe; r.active = active; r.live = live; r.has_pe = has_pe; r.dest = dest; r.vol = vol;
 }
 
+// (the body of the kernel, so that the merged move kernel of charged.cuh can run it in the blocks it gives to photons; the
+// block's shared memory comes from the kernel)
 template <bool BVH, bool MULTI>
-__global__ void __launch_bounds__(kBlock, BVH ? ADEPT_MINB_G2B : ADEPT_MINB_G2)
-gamma_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot, int parity) {
+__device__ __forceinline__ void gamma_move_body(const DevCtx& c, const DevSlot& slot, int parity, BlockTally& tally, BlockReserve<5>& br,
+                                                TilePipe& pipe) {
   constexpr int species = ADEPT_GAMMA;
   const TrackSoA& cur = slot.buf[parity][species];
   SlotCounters* cnt = slot.counters;
@@ -185,9 +187,6 @@ gamma_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevS
   // electron buffer (photoelectrons)
   constexpr int ND = 5;
   if (blockIdx.x >= (n + kBlock - 1) / kBlock) return;   // no tile for this block (tail of a shower: most blocks)
-  __shared__ BlockTally tally;
-  __shared__ BlockReserve<ND> br;
-  __shared__ TilePipe pipe;
   tally_init(tally);
   pipe_init(pipe);
   double sum_cut = 0.0;
@@ -277,6 +276,15 @@ gamma_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevS
   }
   gamma_counts_flush(tally, packed);
   tally_flush(tally, slot, species, 0.0, sum_cut);
+}
+
+template <bool BVH, bool MULTI>
+__global__ void __launch_bounds__(kBlock, BVH ? ADEPT_MINB_G2B : ADEPT_MINB_G2)
+gamma_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot, int parity) {
+  __shared__ BlockTally tally;
+  __shared__ BlockReserve<5> br;
+  __shared__ TilePipe pipe;
+  gamma_move_body<BVH, MULTI>(c, slot, parity, tally, br, pipe);
 }
 
 }  // namespace adept
