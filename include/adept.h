@@ -237,7 +237,10 @@ int adept_get_stats(adept_ctx*, int event_slot, adept_stats* out);
  * a population step run one after the other on the caller's stream, so every event pair brackets one
  * kernel alone; the events themselves cost ~5 us of stream time per launch.  adept_set_kernel_timing
  * switches the events off (0) and on (1) between passes of a context created with time_kernels = 1, so
- * that a benchmark can time untimed passes and instrumented passes of the same context. */
+ * that a benchmark can time untimed passes and instrumented passes of the same context.
+ * A context without a field and without a BVH volume (and with config.concurrent_species != 0) runs the gamma and
+ * the charged move kernel as the blocks of ONE launch; [0] is then that merged kernel and [1] stays empty (0 ms, 0
+ * launches): create the context with concurrent_species = 0 to time the two kernels by themselves. */
 int adept_set_kernel_timing(adept_ctx*, int on);
 #define ADEPT_N_TIMED_KERNELS 3
 int adept_get_kernel_times(adept_ctx*, int event_slot, double ms[ADEPT_N_TIMED_KERNELS],

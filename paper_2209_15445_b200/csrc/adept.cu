@@ -844,9 +844,13 @@ int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity, 
   }
   const bool timed = ctx->timing_on && !sh.tev.empty() && sh.tev_used + kEv <= static_cast<int>(sh.tev.size());
   // a timed pass runs the kernels one after the other, so that an event pair brackets one kernel alone
-  if (ctx->k_move_merged[multi] && !ctx->timing_on) {   // all three species in one launch
+  if (ctx->k_move_merged[multi]) {   // all three species in one launch (timed as kernel [0]; [1] stays empty)
+    cudaEvent_t* ev = timed ? &sh.tev[sh.tev_used] : nullptr;
+    if (timed) CUDA_TRY(cudaEventRecord(ev[0], st));
     ctx->k_move_merged[multi]<<<dim3(ctx->grid_gamma, 3), kBlock, 0, st>>>(dc, sh.dev, parity);
+    if (timed) { CUDA_TRY(cudaEventRecord(ev[1], st)); CUDA_TRY(cudaEventRecord(ev[4], st)); }
     interact_kernel<<<ctx->grid_inter, kBlock, 0, st>>>(dc, sh.dev, parity);
+    if (timed) { CUDA_TRY(cudaEventRecord(ev[5], st)); sh.tev_used += kEv; }
     sh.launches += 2;
     return ADEPT_OK;
   }
@@ -961,6 +965,7 @@ extern "C" int adept_transport_many(adept_ctx* ctx, int n_slots, const int* slot
       CUDA_TRY(cudaStreamSynchronize(st));
       for (int e = 0; e + 2 * ADEPT_N_TIMED_KERNELS <= sh.tev_used; e += 2 * ADEPT_N_TIMED_KERNELS)
         for (int kk = 0; kk < ADEPT_N_TIMED_KERNELS; ++kk) {
+          if (kk == 1 && ctx->k_move_merged[0]) continue;   // the merged move kernel is kernel [0]
           float ms = 0.f;
           CUDA_TRY(cudaEventElapsedTime(&ms, sh.tev[e + 2 * kk], sh.tev[e + 2 * kk + 1]));
           sh.kernel_ms[kk] += ms;

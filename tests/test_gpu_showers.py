@@ -500,7 +500,7 @@ def test_measurement_modes_do_not_change_the_showers(ob, calo):
     prim = primaries.beam(40, 400.0, spread=1.0)
     prim["species"][1::2] = 2
     ref = None
-    for conc, timed in ((1, 0), (0, 0), (1, 1)):
+    for conc, timed in ((1, 0), (0, 0), (1, 1), (0, 1)):
         a = adept.Adept(g, tabs, scal, field.no_field(), track_capacity=1 << 16, concurrent_species=conc, time_kernels=timed)
         if not timed:
             with pytest.raises(adept.AdeptError):
@@ -516,8 +516,12 @@ def test_measurement_modes_do_not_change_the_showers(ob, calo):
         assert len(a.iteration_trace()[0]) == 0     # reading clears
         if timed:
             ms, n = a.kernel_times(0)
-            assert (n == st.iterations).all() or (n >= st.iterations).all()
-            assert (ms > 0).all()
+            # no field, no BVH: with concurrent species the gamma and the e+- kernel are the blocks of one launch, timed
+            # as kernel [0] while [1] stays empty (adept.h); with concurrent_species = 0 all three are launched and timed
+            used = [0, 2] if conc else [0, 1, 2]
+            assert (n[used] >= st.iterations).all() and (ms[used] > 0).all()
+            if conc:
+                assert n[1] == 0 and ms[1] == 0
             a.set_kernel_timing(False)
             a.enqueue(prim)
             a.transport(0, torch.cuda.current_stream())
