@@ -942,7 +942,7 @@ extern "C" int adept_transport_many(adept_ctx* ctx, int n_slots, const int* slot
       variant[k] = round_variant(ctx, sh);
       if (!sh.live || parity[k] != 0 || ctx->timing_on || sh.n_injected < sh.n_pending || !round_graph(ctx, sh, variant[k])) continue;
       CUDA_TRY(cudaGraphLaunch(sh.gexec[variant[k]], static_cast<cudaStream_t>(streams[k])));
-      sh.launches += 3ull * ctx->cfg.sync_interval;
+      sh.launches += (ctx->k_move_merged[variant[k]] ? 2ull : 3ull) * ctx->cfg.sync_interval;   // kernels of the replayed round
       graphed[k] = 1;
     }
     for (int it = 0; it < ctx->cfg.sync_interval; ++it)
