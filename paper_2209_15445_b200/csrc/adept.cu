@@ -7,6 +7,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <numeric>
+#include <thread>
 #include <vector>
 
 #include "kernels.cuh"
@@ -933,64 +934,88 @@ extern "C" int adept_transport_many(adept_ctx* ctx, int n_slots, const int* slot
   }
   std::vector<int> parity(n_slots, 0);
   int n_live = n_slots, rc_final = ADEPT_OK;
-  while (n_live > 0) {
-    // slots whose round is a graph: one launch each
-    std::vector<char> graphed(n_slots, 0);
-    std::vector<int> variant(n_slots, 0);
-    for (int k = 0; k < n_slots; ++k) {
-      SlotHost& sh = ctx->slots[slots[k]];
-      variant[k] = round_variant(ctx, sh);
-      if (!sh.live || parity[k] != 0 || ctx->timing_on || sh.n_injected < sh.n_pending || !round_graph(ctx, sh, variant[k])) continue;
-      CUDA_TRY(cudaGraphLaunch(sh.gexec[variant[k]], static_cast<cudaStream_t>(streams[k])));
-      sh.launches += (ctx->k_move_merged[variant[k]] ? 2ull : 3ull) * ctx->cfg.sync_interval;   // kernels of the replayed round
-      graphed[k] = 1;
-    }
-    for (int it = 0; it < ctx->cfg.sync_interval; ++it)
-      for (int k = 0; k < n_slots; ++k) {
-        SlotHost& sh = ctx->slots[slots[k]];
-        if (!sh.live || graphed[k]) continue;
-        const int rc = launch_iteration(ctx, sh, static_cast<cudaStream_t>(streams[k]), parity[k], ctx->dev, variant[k]);
+  // One host round of slot k: sync_interval population steps (one graph launch where possible) and the copy of its
+  // counters, all on the slot's stream.
+  const auto issue_round = [&](int k) -> int {
+    SlotHost& sh = ctx->slots[slots[k]];
+    cudaStream_t st = static_cast<cudaStream_t>(streams[k]);
+    const int variant = round_variant(ctx, sh);
+    if (parity[k] == 0 && !ctx->timing_on && sh.n_injected == sh.n_pending && round_graph(ctx, sh, variant)) {
+      CUDA_TRY(cudaGraphLaunch(sh.gexec[variant], st));
+      sh.launches += (ctx->k_move_merged[variant] ? 2ull : 3ull) * ctx->cfg.sync_interval;   // kernels of the replayed round
+    } else {
+      for (int it = 0; it < ctx->cfg.sync_interval; ++it) {
+        const int rc = launch_iteration(ctx, sh, st, parity[k], ctx->dev, variant);
         if (rc != ADEPT_OK) return rc;
         parity[k] ^= 1;
       }
-    for (int k = 0; k < n_slots; ++k) {
-      SlotHost& sh = ctx->slots[slots[k]];
-      if (sh.live) CUDA_TRY(cudaMemcpyAsync(sh.pinned, sh.dev.counters, sizeof(SlotCounters), cudaMemcpyDeviceToHost,
-                                            static_cast<cudaStream_t>(streams[k])));
     }
+    CUDA_TRY(cudaMemcpyAsync(sh.pinned, sh.dev.counters, sizeof(SlotCounters), cudaMemcpyDeviceToHost, st));
+    return ADEPT_OK;
+  };
+  // What the round of slot k left behind (its stream is idle): kernel times, overflow, population; *done = the slot is empty.
+  const auto finish_round = [&](int k, bool* done) -> int {
+    SlotHost& sh = ctx->slots[slots[k]];
+    cudaStream_t st = static_cast<cudaStream_t>(streams[k]);
+    for (int e = 0; e + 2 * ADEPT_N_TIMED_KERNELS <= sh.tev_used; e += 2 * ADEPT_N_TIMED_KERNELS)
+      for (int kk = 0; kk < ADEPT_N_TIMED_KERNELS; ++kk) {
+        if (kk == 1 && ctx->k_move_merged[0]) continue;   // the merged move kernel is kernel [0]
+        float ms = 0.f;
+        CUDA_TRY(cudaEventElapsedTime(&ms, sh.tev[e + 2 * kk], sh.tev[e + 2 * kk + 1]));
+        sh.kernel_ms[kk] += ms;
+        sh.kernel_launches[kk] += 1;
+      }
+    sh.tev_used = 0;
+    const bool overflow = sh.pinned->overflow.v != 0;
+    sh.population = sh.pinned->live.v;
+    if (overflow) {
+      // The pass is abandoned: the slot is emptied (tracks, staging queues, scoring, ledger, leaked tracks) so
+      // that the caller can enqueue a smaller batch into it.
+      rc_final = fail(ADEPT_EOVERFLOW, "slot %d: track queue overflow (capacity %llu per species, %llu per staging queue); slot reset",
+                      slots[k], static_cast<unsigned long long>(ctx->dev.capacity), static_cast<unsigned long long>(ctx->dev.stage_capacity));
+      const int rr = reset_slot_async(ctx, sh, st);
+      if (rr != ADEPT_OK) return rr;
+      CUDA_TRY(cudaStreamSynchronize(st));
+    }
+    *done = (sh.pinned->live.v == 0 && sh.n_injected == sh.n_pending) || overflow;
+    if (*done) {
+      sh.n_pending = sh.n_injected = 0;
+      sh.population = 0;
+      sh.live = false;
+      --n_live;
+      // counts are all zero: the (empty) slot is at parity 0 for the next enqueue whatever parity[k] is
+    }
+    return ADEPT_OK;
+  };
+  // Every slot advances at its own pace: its next round is issued as soon as its own round has finished, not when the
+  // slowest slot's has (config 5: the rounds of 16 events last from a fraction of a millisecond to tens of them).
+  for (int k = 0; k < n_slots; ++k) {
+    const int rc = issue_round(k);
+    if (rc != ADEPT_OK) return rc;
+  }
+  while (n_live > 0) {
+    bool progressed = false;
     for (int k = 0; k < n_slots; ++k) {
       SlotHost& sh = ctx->slots[slots[k]];
       if (!sh.live) continue;
       cudaStream_t st = static_cast<cudaStream_t>(streams[k]);
-      CUDA_TRY(cudaStreamSynchronize(st));
-      for (int e = 0; e + 2 * ADEPT_N_TIMED_KERNELS <= sh.tev_used; e += 2 * ADEPT_N_TIMED_KERNELS)
-        for (int kk = 0; kk < ADEPT_N_TIMED_KERNELS; ++kk) {
-          if (kk == 1 && ctx->k_move_merged[0]) continue;   // the merged move kernel is kernel [0]
-          float ms = 0.f;
-          CUDA_TRY(cudaEventElapsedTime(&ms, sh.tev[e + 2 * kk], sh.tev[e + 2 * kk + 1]));
-          sh.kernel_ms[kk] += ms;
-          sh.kernel_launches[kk] += 1;
-        }
-      sh.tev_used = 0;
-      const bool overflow = sh.pinned->overflow.v != 0;
-      sh.population = sh.pinned->live.v;
-      if (overflow) {
-        // The pass is abandoned: the slot is emptied (tracks, staging queues, scoring, ledger, leaked tracks) so
-        // that the caller can enqueue a smaller batch into it.
-        rc_final = fail(ADEPT_EOVERFLOW, "slot %d: track queue overflow (capacity %llu per species, %llu per staging queue); slot reset",
-                        slots[k], static_cast<unsigned long long>(ctx->dev.capacity), static_cast<unsigned long long>(ctx->dev.stage_capacity));
-        const int rr = reset_slot_async(ctx, sh, st);
-        if (rr != ADEPT_OK) return rr;
-        CUDA_TRY(cudaStreamSynchronize(st));
+      if (n_live == 1) {
+        CUDA_TRY(cudaStreamSynchronize(st));      // a single slot left: wait for it, no polling
+      } else {
+        const cudaError_t q = cudaStreamQuery(st);
+        if (q == cudaErrorNotReady) continue;
+        CUDA_TRY(q);
       }
-      if ((sh.pinned->live.v == 0 && sh.n_injected == sh.n_pending) || overflow) {
-        sh.n_pending = sh.n_injected = 0;
-        sh.population = 0;
-        sh.live = false;
-        --n_live;
-        // counts are all zero: the (empty) slot is at parity 0 for the next enqueue whatever parity[k] is
+      bool done = false;
+      int rc = finish_round(k, &done);
+      if (rc != ADEPT_OK) return rc;
+      if (!done) {
+        rc = issue_round(k);
+        if (rc != ADEPT_OK) return rc;
       }
+      progressed = true;
     }
+    if (!progressed) std::this_thread::yield();
   }
   CUDA_TRY(cudaGetLastError());
   if (rc_final != ADEPT_OK) fail(rc_final, "a slot's track queue overflowed (track_capacity %llu, stage_capacity %llu); the slot was reset",
