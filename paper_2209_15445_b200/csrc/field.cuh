@@ -64,6 +64,11 @@ __device__ __forceinline__ void sincos_small(double x, double& sn, double& cs) {
   cs = fma(-z, q, 1.0);
 }
 
+// sin and cos of an angle too large for the series: libdevice's routine, out of line (the chord loop is the hottest code
+// of the field kernels and misses the instruction cache as it is; a chord turns the track by more than 1.6 rad only
+// below ~3 keV at 3.8 T)
+__device__ __noinline__ void sincos_large(double x, double* sn, double* cs) { sincos(x, sn, cs); }
+
 // F3: exact helix about the unit vector b; kappa = -q kCB |B| / p is the turning angle per unit path length
 // (constant over a step: F1 takes p at the pre-step energy), so omega = kappa h and h / omega = 1 / kappa.
 // sin(omega), cos(omega) and 1 - cos(omega) all come from the half angle.
@@ -73,7 +78,7 @@ __device__ __forceinline__ void helix(const double b[3], double kappa, double in
   const double half = 0.5 * kappa * h;
   double s2, c2;
   if (fabs(half) <= 0.8) sincos_small(half, s2, c2);
-  else sincos(half, &s2, &c2);
+  else sincos_large(half, &s2, &c2);
   const double so = 2.0 * s2 * c2, omc = 2.0 * s2 * s2, co = 1.0 - omc;
   const double dpar = d[0] * b[0] + d[1] * b[1] + d[2] * b[2];
   const double dl[3] = {dpar * b[0], dpar * b[1], dpar * b[2]};
@@ -85,6 +90,22 @@ __device__ __forceinline__ void helix(const double b[3], double kappa, double in
     d1[i] = dl[i] + dt[i] * co + bxd[i] * so;
     p1[i] = p[i] + dl[i] * h + inv_kappa * (dt[i] * so + bxd[i] * omc);
   }
+}
+
+// ... and its direction alone (the tangent at a boundary hit): the same arithmetic as helix() for d1
+__device__ __forceinline__ void helix_dir(const double b[3], double kappa, double h, const double d[3], double d1[3]) {
+  const double half = 0.5 * kappa * h;
+  double s2, c2;
+  if (fabs(half) <= 0.8) sincos_small(half, s2, c2);
+  else sincos_large(half, &s2, &c2);
+  const double so = 2.0 * s2 * c2, omc = 2.0 * s2 * s2, co = 1.0 - omc;
+  const double dpar = d[0] * b[0] + d[1] * b[1] + d[2] * b[2];
+  const double dl[3] = {dpar * b[0], dpar * b[1], dpar * b[2]};
+  const double dt[3] = {d[0] - dl[0], d[1] - dl[1], d[2] - dl[2]};
+  double bxd[3];
+  cross3(b, dt, bxd);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) d1[i] = dl[i] + dt[i] * co + bxd[i] * so;
 }
 
 // F1, F3: one classical RK4 step on (x, d): x' = d, d' = (q kCB / p) d x B(x); B0 = B(p), already known
@@ -229,8 +250,7 @@ __device__ __forceinline__ int propagate(const DevCtx& c, int nav, bool active, 
         const double frac = s_geo / L;
         double dh[3];
         if (field_kind == ADEPT_FIELD_UNIFORM) {
-          double ph[3];
-          helix(c.bhat, kappa, inv_kappa, h * frac, pos, dir, ph, dh);
+          helix_dir(c.bhat, kappa, h * frac, dir, dh);
         } else {
           double n = 0.0;
 #pragma unroll
@@ -462,8 +482,7 @@ __device__ __forceinline__ int propagate_wide(const DevCtx& c, int nav, int shif
       if (kind == 1) {
         const double frac = s_geo / L;
         if (field_kind == ADEPT_FIELD_UNIFORM) {
-          double ph[3];
-          helix(c.bhat, kappa, inv_kappa, H * frac, P, D, ph, dh);
+          helix_dir(c.bhat, kappa, H * frac, D, dh);
         } else {
           double n = 0.0;
 #pragma unroll
