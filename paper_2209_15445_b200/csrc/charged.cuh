@@ -284,7 +284,7 @@ __device__ __forceinline__ void charged_move_body(const DevCtx& c, const DevSlot
   const bool mine = (threadIdx.x & ((1u << lane_shift) - 1u)) == 0;
   // eight or more lanes per track: they take its chord loop together (field.cuh propagate_wide)
   const int wide_shift = (MULTI && FIELD != ADEPT_FIELD_NONE && lane_shift >= 3) ? lane_shift : 0;
-  int k_inner = MULTI ? min(inner_steps(c, n, gridDim.x * kBlock), 255) : 1;
+  int k_inner = MULTI ? min(inner_steps(c, n, gridDim.x * kBlock, FIELD == ADEPT_FIELD_NONE ? ADEPT_INNER_MAX_STRAIGHT : ADEPT_INNER_MAX), 255) : 1;
   // full GPU, BVH geometry: only the passage through the gap a track has just entered from a daughter is taken in
   // the same launch (geom.cuh NavCache)
   const bool transit_only = MULTI && BVH && k_inner == 1 && c.transit;

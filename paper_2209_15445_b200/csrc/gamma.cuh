@@ -194,7 +194,7 @@ __device__ __forceinline__ void gamma_move_body(const DevCtx& c, const DevSlot& 
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const unsigned lt = (1u << lane) - 1u;
   const int t = threadIdx.x;
-  int k_inner = MULTI ? min(inner_steps(c, n, gridDim.x * kBlock), 1023) : 1;
+  int k_inner = MULTI ? min(inner_steps(c, n, gridDim.x * kBlock, ADEPT_INNER_MAX_STRAIGHT), 1023) : 1;
   // full GPU, BVH geometry: only the passage through the gap a track has just entered from a daughter is taken in
   // the same launch (geom.cuh NavCache: the daughter's neighbour list answers its query without a traversal)
   const bool transit_only = MULTI && BVH && k_inner == 1 && c.transit;

@@ -190,14 +190,23 @@ __device__ __forceinline__ void block_reserve(BlockReserve<ND>& br, int phase, c
 #ifndef ADEPT_INNER_MAX
 #define ADEPT_INNER_MAX 32
 #endif
-__device__ __forceinline__ int inner_steps(const DevCtx& c, uint32_t n, uint32_t lanes) {
+// Photons and field-free e+- do not loop: their long-lived tracks are few steps from an interaction, and a lane that
+// holds on to its track keeps the secondaries of the others waiting.  Measured (profiles/r2_summary.md): at most 3
+// steps per launch for them, config 1 4.42 -> 3.10 ms, config 2 34.19 -> 33.78 ms per pass (2: 3.19 / 33.73;
+// 4: 3.32 / 33.88; 8: 3.98 / 34.06); e+- in a field keep ADEPT_INNER_MAX.
+#ifndef ADEPT_INNER_MAX_STRAIGHT
+#define ADEPT_INNER_MAX_STRAIGHT 3
+#endif
+// `cap`: ADEPT_INNER_MAX for e+- in a field (the loopers), ADEPT_INNER_MAX_STRAIGHT for photons and field-free e+-
+__device__ __forceinline__ int inner_steps(const DevCtx& c, uint32_t n, uint32_t lanes, int cap = ADEPT_INNER_MAX) {
   if (c.steps_per_launch > 0) return c.steps_per_launch;
-  if (n >= lanes) return 1;
-  if (n >= lanes / 4) return 2;
-  if (n >= lanes / 16) return 4;
-  if (n >= lanes / 64) return 8;
-  if (n >= lanes / 256) return 16;
-  return ADEPT_INNER_MAX;
+  int k = ADEPT_INNER_MAX;
+  if (n >= lanes) k = 1;
+  else if (n >= lanes / 4) k = 2;
+  else if (n >= lanes / 16) k = 4;
+  else if (n >= lanes / 64) k = 8;
+  else if (n >= lanes / 256) k = 16;
+  return min(k, cap);
 }
 
 // A9: scoring.  Every depositing lane issues one fp64 reduction (RED.ADD.F64, no return value, so the
