@@ -265,6 +265,23 @@ int adept_get_iteration_trace(adept_ctx*, int event_slot, uint64_t* t_ns, uint32
 int adept_raycast_batch(adept_ctx*, int navigator, int n, const double* pos3, const double* dir3, int max_crossings,
                         double* column, int32_t* crossings, double* device_ms, void* cuda_stream);
 
+/* adept_raycast_batch for callers that must not allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same kernel, the same arguments but device_ms (timing it would take two
+ * events created per call), the same results bit for bit.  The device copies of the rays and of the results live
+ * in one file-scope `static __device__` array of ADEPT_STATIC_MAX_RAYS x 60 B = 3.75 MiB instead of cudaMalloc'ed
+ * buffers; every GPU that loads the library holds that array until the process exits.  The call makes no
+ * cudaMalloc, cudaFree, event or stream creation, or other allocating runtime call: two memsets (the results
+ * start at zero: the array keeps what the previous call left in it), two uploads, the kernel, two downloads and a
+ * synchronisation of cuda_stream.  The array's device address is asked of the runtime once per device
+ * (cudaGetSymbolAddress, with the context's device current), on that device's first call.
+ * n > ADEPT_STATIC_MAX_RAYS: ADEPT_EINVAL, nothing is launched (split the batch, or call adept_raycast_batch).
+ * All calls on a device share the one array, whatever their context or stream: calls that overlap on the GPU
+ * (two host threads, or two contexts on two streams) race on it and return garbage; the caller serialises them.
+ * Calls one after the other on one host thread are safe (each ends with cuda_stream synchronised). */
+#define ADEPT_STATIC_MAX_RAYS 65536
+int adept_raycast_batch_static(adept_ctx*, int navigator, int n, const double* pos3, const double* dir3, int max_crossings,
+                               double* column, int32_t* crossings, void* cuda_stream);
+
 /* ---- Hybrid-workflow boundary.  The host simulation hands over, one at
  * a time, the tracks that enter the GPU region; they are buffered on the host until `threshold` of them
  * trigger synchronous transport of the batch in `event_slot` on `cuda_stream`; adept_buffer_flush transports

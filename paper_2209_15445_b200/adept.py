@@ -14,6 +14,7 @@ LIB_PATH = os.environ.get("ADEPT_B200_LIB", os.path.join(HERE, "libadept_b200.so
 
 OK, EINVAL, ENOMEM, EOVERFLOW, ECUDA, ESTATE = 0, -1, -2, -3, -4, -5
 NAV_LOOP, NAV_BVH, NAV_LOOP_F32, NAV_BVH_F32 = 0, 1, 2, 3
+STATIC_MAX_RAYS = 65536  # ADEPT_STATIC_MAX_RAYS: most rays of one raycast_static call
 OUTCOMES = ["boundary", "compton", "pair", "photo", "brem", "ioni", "anni", "stopped", "truncated", "loss",
             "escaped", "killed", "closed"]
 
@@ -68,7 +69,7 @@ INTERACTION_OUTCOMES = (1, 2, 4, 5, 6, 12)
 EXPORTS = ["adept_last_error", "adept_default_config", "adept_workspace_bytes", "adept_init",
            "adept_enqueue_primaries", "adept_enqueue_batch", "adept_transport", "adept_transport_many",
            "adept_read_scoring", "adept_read_leaked", "adept_get_stats", "adept_get_kernel_times", "adept_set_kernel_timing", "adept_get_iteration_trace",
-           "adept_raycast_batch", "adept_buffer_create", "adept_buffer_add", "adept_buffer_flush", "adept_buffer_pending", "adept_buffer_take",
+           "adept_raycast_batch", "adept_raycast_batch_static", "adept_buffer_create", "adept_buffer_add", "adept_buffer_flush", "adept_buffer_pending", "adept_buffer_take",
            "adept_buffer_destroy", "adept_step_frozen", "adept_step_population", "adept_reset_slot",
            "adept_distance_batch", "adept_locate_batch", "adept_relocate_batch", "adept_shutdown"]
 
@@ -103,6 +104,7 @@ def load_library():
     lib.adept_relocate_batch.argtypes = [vp, i, i, vp, vp, vp, vp, vp]
     lib.adept_shutdown.argtypes = [vp]
     lib.adept_raycast_batch.argtypes = [vp, i, i, vp, vp, i, vp, vp, C.POINTER(C.c_double), vp]
+    lib.adept_raycast_batch_static.argtypes = [vp, i, i, vp, vp, i, vp, vp, vp]
     lib.adept_buffer_create.argtypes = [C.POINTER(vp), vp, i, sz, vp]
     lib.adept_buffer_add.argtypes = [vp, C.c_uint32, C.c_uint64, i, vp, vp, C.c_double]
     lib.adept_buffer_flush.argtypes = [vp]
@@ -270,6 +272,19 @@ class Adept:
             _check(lib.adept_raycast_batch(self.ctx, navigator, n, _ptr(p), _ptr(d), max_crossings, _ptr(col), _ptr(nx),
                                            C.byref(ms), _stream_ptr(stream)))
         return col, nx, ms.value
+
+    def raycast_static(self, pos, direc, navigator=NAV_BVH, max_crossings=100000, stream=None):
+        """raycast() through adept_raycast_batch_static: no device allocation, at most STATIC_MAX_RAYS rays, and
+        calls that overlap on one GPU race on the library's static scratch array (include/adept.h)."""
+        p = np.ascontiguousarray(pos, dtype=np.float64)
+        d = np.ascontiguousarray(direc, dtype=np.float64)
+        n = p.shape[0]
+        col = np.zeros(n)
+        nx = np.zeros(n, dtype=np.int32)
+        with self._torch.cuda.device(self.device):
+            _check(lib.adept_raycast_batch_static(self.ctx, navigator, n, _ptr(p), _ptr(d), max_crossings, _ptr(col), _ptr(nx),
+                                                  _stream_ptr(stream)))
+        return col, nx
 
     def iteration_trace(self, slot=0, cap=4096):
         """(t_ns[n], population[n, 3]) of the population steps since the last call (device %globaltimer;

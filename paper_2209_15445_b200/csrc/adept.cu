@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <numeric>
 #include <thread>
 #include <vector>
@@ -1244,6 +1245,79 @@ extern "C" int adept_raycast_batch(adept_ctx* ctx, int nav, int n, const double*
   if (e0) cudaEventDestroy(e0);
   if (e1) cudaEventDestroy(e1);
   return rc;
+}
+
+// ---- adept_raycast_batch without an allocation (include/adept.h adept_raycast_batch_static) ----
+// The ray-cast kernel reads ray origins and directions and writes column densities and crossing counts in device
+// memory; adept_raycast_batch takes those four buffers from cudaMalloc, this variant from one file-scope array.
+// Every GPU that loads the library holds the array (3.75 MiB) until the process exits.  In host code the name
+// g_static_scratch is a stand-in for the symbol, not a device address: kernels are given what
+// cudaGetSymbolAddress returned on their device.
+constexpr size_t kStaticMaxRays = ADEPT_STATIC_MAX_RAYS;
+constexpr size_t kStaticPos = 0;                                                // [n][3] doubles
+constexpr size_t kStaticDir = kStaticPos + kStaticMaxRays * 3 * sizeof(double); // [n][3] doubles
+constexpr size_t kStaticCol = kStaticDir + kStaticMaxRays * 3 * sizeof(double); // [n] doubles
+constexpr size_t kStaticNx = kStaticCol + kStaticMaxRays * sizeof(double);      // [n] int32
+constexpr size_t kStaticBytes = kStaticNx + kStaticMaxRays * sizeof(int32_t);
+static_assert(kStaticDir % 256 == 0 && kStaticCol % 256 == 0 && kStaticNx % 256 == 0, "sub-buffers keep the array's alignment");
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticBytes];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mutex;
+unsigned char* g_static_addr[kStaticMaxDevices] = {};  // device address of g_static_scratch, per device ordinal
+
+// Address of g_static_scratch on `device`, which the caller has made current: asked of the runtime once per device.
+int static_scratch(int device, unsigned char** out) {
+  if (device < 0 || device >= kStaticMaxDevices) return fail(ADEPT_EINVAL, "device %d: the static scratch serves devices 0..%d", device, kStaticMaxDevices - 1);
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  if (!g_static_addr[device]) {
+    unsigned char* ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress((void**)&ptr, g_static_scratch);
+    if (e != cudaSuccess || !ptr) return fail(ADEPT_ECUDA, "cudaGetSymbolAddress(g_static_scratch) on device %d: %s", device, cudaGetErrorString(e));
+    g_static_addr[device] = ptr;
+  }
+  *out = g_static_addr[device];
+  return ADEPT_OK;
+}
+
+}  // namespace
+
+extern "C" int adept_raycast_batch_static(adept_ctx* ctx, int nav, int n, const double* pos3, const double* dir3, int max_crossings,
+                                          double* column, int32_t* crossings, void* stream) {
+  if (!ctx || n < 0 || (n > 0 && (!pos3 || !dir3 || !column || !crossings))) return fail(ADEPT_EINVAL, "null argument");
+  if (nav < ADEPT_NAV_LOOP || nav > ADEPT_NAV_BVH_F32) return fail(ADEPT_EINVAL, "unknown navigator");
+  if (max_crossings < 1) return fail(ADEPT_EINVAL, "max_crossings must be >= 1");
+  if (static_cast<size_t>(n) > kStaticMaxRays)
+    return fail(ADEPT_EINVAL, "adept_raycast_batch_static: %d rays exceed ADEPT_STATIC_MAX_RAYS = %d (the static scratch array); "
+                "split the batch or call adept_raycast_batch", n, ADEPT_STATIC_MAX_RAYS);
+  if (n == 0) return ADEPT_OK;
+  ADEPT_ON_DEVICE(ctx);
+  unsigned char* base = nullptr;
+  const int rc = static_scratch(ctx->device, &base);
+  if (rc != ADEPT_OK) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  double* d_pos = reinterpret_cast<double*>(base + kStaticPos);
+  double* d_dir = reinterpret_cast<double*>(base + kStaticDir);
+  double* d_col = reinterpret_cast<double*>(base + kStaticCol);
+  int32_t* d_nx = reinterpret_cast<int32_t*>(base + kStaticNx);
+  const size_t nb = static_cast<size_t>(n) * 3 * sizeof(double);
+  // the array keeps the last call's contents: the results start at zero, the inputs are overwritten
+  CUDA_TRY(cudaMemsetAsync(d_col, 0, static_cast<size_t>(n) * sizeof(double), st));
+  CUDA_TRY(cudaMemsetAsync(d_nx, 0, static_cast<size_t>(n) * sizeof(int32_t), st));
+  CUDA_TRY(cudaMemcpyAsync(d_pos, pos3, nb, cudaMemcpyHostToDevice, st));
+  CUDA_TRY(cudaMemcpyAsync(d_dir, dir3, nb, cudaMemcpyHostToDevice, st));
+  const int grid = std::min((n + kBlock - 1) / kBlock, 65535);
+  if (nav >= ADEPT_NAV_LOOP_F32)
+    raycast_kernel<float><<<grid, kBlock, 0, st>>>(ctx->dev, nav - ADEPT_NAV_LOOP_F32, n, d_pos, d_dir, max_crossings, d_col, d_nx);
+  else
+    raycast_kernel<double><<<grid, kBlock, 0, st>>>(ctx->dev, nav, n, d_pos, d_dir, max_crossings, d_col, d_nx);
+  CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(cudaMemcpyAsync(column, d_col, static_cast<size_t>(n) * sizeof(double), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaMemcpyAsync(crossings, d_nx, static_cast<size_t>(n) * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  return ADEPT_OK;
 }
 
 extern "C" int adept_locate_batch(adept_ctx* ctx, int nav, int n, const double* pos3, int64_t* out, void* stream) {
