@@ -56,7 +56,9 @@ def test_bench_workloads_and_sharding():
     assert t is None or (set(b.KERNELS) <= set(t["kernels"]) <= set(b.KERNELS) | {"move_kernel"} and t.get("commit"))
     if t is not None:      # the merged move kernel: its own row, or the sum of its two bodies
         m = b.traffic_of(t, "move_kernel")
-        assert m["tracks"] == t["kernels"]["gamma_move_kernel"]["tracks"] + t["kernels"]["charged_move_kernel"]["tracks"]
+        # captures of launches at the peak of a pass (the file names the population step of each): within 1 % of each other
+        bodies = t["kernels"]["gamma_move_kernel"]["tracks"] + t["kernels"]["charged_move_kernel"]["tracks"]
+        assert abs(m["tracks"] - bodies) <= 0.01 * bodies
         assert m["dram_bytes"] == m["dram_read"] + m["dram_write"] > t["kernels"]["gamma_move_kernel"]["dram_bytes"]
     g, tabs, scal, fld, prim = b.workload(argparse.Namespace(config=2, events=7, field=0.0), first_event=3)
     assert list(prim["event"]) == list(range(3, 10)) and (prim["ekin"] == 10000.0).all() and g.n_volumes == 152
