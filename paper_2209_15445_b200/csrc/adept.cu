@@ -296,8 +296,8 @@ struct SlotHost {
   // CUDA graphs of one host round (sync_interval population steps) with the lean [0] and the multi-step [1]
   // move kernels, captured once on `cap` and replayed
   cudaStream_t cap = nullptr;
-  cudaGraphExec_t gexec[2] = {nullptr, nullptr};
-  bool graph_failed[2] = {false, false};
+  cudaGraphExec_t gexec[3] = {nullptr, nullptr, nullptr};   // per kernel variant (round_variant)
+  bool graph_failed[3] = {false, false, false};
   // optional per-launch timing (config.time_kernels)
   std::vector<cudaEvent_t> tev;      // [sync_interval][kTimed kernels][start, stop]
   int tev_used = 0;
@@ -314,12 +314,13 @@ struct adept_ctx {
   adept_track* d_stage = nullptr;    // staging area for primaries (inside the workspace)
   uint32_t* d_bad = nullptr;
   size_t stage_cap = 0;
-  int grid_gamma = 0, grid_charged = 0, grid_inter = 0;
+  int grid_gamma = 0, grid_charged = 0, grid_charged_low = 0, grid_inter = 0;
   // move kernels specialised for this context's field kind and for geometries without BVH volumes; [1] = the
-  // variants in which a lane takes several steps of its own track per launch (small populations)
+  // variants in which a lane takes several steps of its own track per launch (small populations); [2] = [1] with
+  // the e+- kernel compiled for two resident blocks per SM (BVH geometry in a field only, else null: charged.cuh)
   using Kernel = void (*)(DevCtx, DevSlot, int);
-  Kernel k_move_gamma[2] = {nullptr, nullptr}, k_move_charged[2] = {nullptr, nullptr};
-  Kernel k_move_merged[2] = {nullptr, nullptr};   // one launch for all three species (charged.cuh move_kernel), or null
+  Kernel k_move_gamma[3] = {nullptr, nullptr, nullptr}, k_move_charged[3] = {nullptr, nullptr, nullptr};
+  Kernel k_move_merged[3] = {nullptr, nullptr, nullptr};   // one launch for all three species (charged.cuh move_kernel), or null
   bool timing_on = false;            // per-launch CUDA events active (adept_set_kernel_timing)
 };
 
@@ -694,10 +695,22 @@ extern "C" int adept_init(adept_ctx** out, const adept_geometry* g, const adept_
   ctx->k_move_charged[1] = bvh ? charged_move_kernel<F, true, true> : charged_move_kernel<F, false, true>
     switch (f->kind) {
       case ADEPT_FIELD_NONE: ADEPT_CHARGED_KERNELS(ADEPT_FIELD_NONE); break;
-      case ADEPT_FIELD_UNIFORM: ADEPT_CHARGED_KERNELS(ADEPT_FIELD_UNIFORM); break;
-      default: ADEPT_CHARGED_KERNELS(ADEPT_FIELD_MAP_RZ); break;
+      case ADEPT_FIELD_UNIFORM:
+        ADEPT_CHARGED_KERNELS(ADEPT_FIELD_UNIFORM);
+        if (bvh) ctx->k_move_charged[2] = charged_move_kernel<ADEPT_FIELD_UNIFORM, true, true, true>;
+        break;
+      default:
+        ADEPT_CHARGED_KERNELS(ADEPT_FIELD_MAP_RZ);
+        if (bvh) ctx->k_move_charged[2] = charged_move_kernel<ADEPT_FIELD_MAP_RZ, true, true, true>;
+        break;
     }
 #undef ADEPT_CHARGED_KERNELS
+    if (ctx->k_move_charged[2]) {
+      int occ_low = 1;
+      ctx->k_move_gamma[2] = ctx->k_move_gamma[1];
+      CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_low, ctx->k_move_charged[2], kBlock, 0));
+      ctx->grid_charged_low = sms * std::max(occ_low, 1);
+    }
     // one grid for both variants of a kernel (the lean one sets it: it is the one that fills the GPU)
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_g, ctx->k_move_gamma[0], kBlock, 0));
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_c, ctx->k_move_charged[0], kBlock, 0));
@@ -867,7 +880,7 @@ int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity, 
   ctx->k_move_gamma[multi]<<<dim3(ctx->grid_gamma, 1), kBlock, 0, st>>>(dc, sh.dev, parity);
   if (timed) CUDA_TRY(cudaEventRecord(ev[1], st));
   if (timed) CUDA_TRY(cudaEventRecord(ev[2], sc));
-  ctx->k_move_charged[multi]<<<dim3(ctx->grid_charged, 2), kBlock, 0, sc>>>(dc, sh.dev, parity);
+  ctx->k_move_charged[multi]<<<dim3(multi == 2 ? ctx->grid_charged_low : ctx->grid_charged, 2), kBlock, 0, sc>>>(dc, sh.dev, parity);
   if (timed) CUDA_TRY(cudaEventRecord(ev[3], sc));
   if (fork) {
     CUDA_TRY(cudaEventRecord(sh.join, sh.helper));
@@ -907,10 +920,17 @@ bool round_graph(adept_ctx* ctx, SlotHost& sh, int multi) {
 // last saw no longer fills the GPU (their lanes go on stepping their own tracks, kernels.cuh inner_steps).
 // The showers do not depend on the choice; a stale population costs speed only.
 constexpr size_t kMultiBelow = 65536;
+// BVH geometry in a field: below this population a launch lasts as long as its longest chain of chords and traversals,
+// and the e+- kernel without register spills (two resident blocks per SM) is the faster one (charged.cuh)
+#ifndef ADEPT_LOWOCC_BELOW
+#define ADEPT_LOWOCC_BELOW 262144
+#endif
 int round_variant(const adept_ctx* ctx, const SlotHost& sh) {
   if (ctx->cfg.steps_per_launch == 1) return 0;
+  const size_t population = sh.population + (sh.n_pending - sh.n_injected);
+  if (ctx->k_move_charged[2] && population < static_cast<size_t>(ADEPT_LOWOCC_BELOW)) return 2;
   if (ctx->dev.transit) return 1;   // the multi-step variants also take the passage through a vacuum gap in the same launch
-  return sh.population + (sh.n_pending - sh.n_injected) < kMultiBelow ? 1 : 0;
+  return population < kMultiBelow ? 1 : 0;
 }
 
 }  // namespace

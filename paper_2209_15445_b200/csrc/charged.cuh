@@ -26,6 +26,17 @@ namespace adept {
 #ifndef ADEPT_MINB_C2F
 #define ADEPT_MINB_C2F 4
 #endif
+// field + BVH (configs 4-5): 3 blocks (168 registers) for the populations that fill the GPU, and a second
+// instantiation with 2 (255 registers, no spills) for the small ones (LOWOCC below).  Measured, config 4 ms per pass /
+// config 5 events/s: 4 blocks everywhere 1 012 / 25.9; 3: 980 / 28.6; 2: 972 / 33.1 (with 16 steps per launch);
+// 3 and 2 below 262 144 tracks: 904 / 32.3 (below 65 536: 908 / 32.0, below 16 384: 900 / 29.9), all with 8 steps
+// per launch (kernels.cuh ADEPT_INNER_MAX_BVH)
+#ifndef ADEPT_MINB_C2FB
+#define ADEPT_MINB_C2FB 3
+#endif
+#ifndef ADEPT_MINB_LOW
+#define ADEPT_MINB_LOW 2
+#endif
 
 // One e-/e+ step of the track in tile slot `t`; warp-convergent.  The post-step direction and energy are written
 // into the tile slot (MULTI: position, step count and volume as well, so that the slot is the pre-step state of
@@ -284,7 +295,7 @@ __device__ __forceinline__ void charged_move_body(const DevCtx& c, const DevSlot
   const bool mine = (threadIdx.x & ((1u << lane_shift) - 1u)) == 0;
   // eight or more lanes per track: they take its chord loop together (field.cuh propagate_wide)
   const int wide_shift = (MULTI && FIELD != ADEPT_FIELD_NONE && lane_shift >= 3) ? lane_shift : 0;
-  int k_inner = MULTI ? min(inner_steps(c, n, gridDim.x * kBlock, FIELD == ADEPT_FIELD_NONE ? ADEPT_INNER_MAX_STRAIGHT : ADEPT_INNER_MAX), 255) : 1;
+  int k_inner = MULTI ? min(inner_steps(c, n, gridDim.x * kBlock, FIELD == ADEPT_FIELD_NONE ? ADEPT_INNER_MAX_STRAIGHT : BVH ? ADEPT_INNER_MAX_BVH : ADEPT_INNER_MAX), 255) : 1;
   // full GPU, BVH geometry: only the passage through the gap a track has just entered from a daughter is taken in
   // the same launch (geom.cuh NavCache)
   const bool transit_only = MULTI && BVH && k_inner == 1 && c.transit;
@@ -382,8 +393,12 @@ __device__ __forceinline__ void charged_move_body(const DevCtx& c, const DevSlot
   tally_flush(tally, slot, species, sum_dep, sum_cut);
 }
 
-template <int FIELD, bool BVH, bool MULTI>
-__global__ void __launch_bounds__(kBlock, FIELD == ADEPT_FIELD_NONE ? ADEPT_MINB_C2 : ADEPT_MINB_C2F)
+// LOWOCC: the same kernel compiled for ADEPT_MINB_LOW resident blocks per SM (255 registers, no spills), which the host
+// launches while the population is small (adept.cu round_variant).  BVH geometry in a field only: there a launch of
+// a small population lasts as long as its longest chain of chords and traversals, and the spills of the
+// 128-register form are on that chain.
+template <int FIELD, bool BVH, bool MULTI, bool LOWOCC = false>
+__global__ void __launch_bounds__(kBlock, FIELD == ADEPT_FIELD_NONE ? ADEPT_MINB_C2 : LOWOCC ? ADEPT_MINB_LOW : BVH ? ADEPT_MINB_C2FB : ADEPT_MINB_C2F)
 charged_move_kernel(const __grid_constant__ DevCtx c, const __grid_constant__ DevSlot slot, int parity) {
   __shared__ BlockTally tally;
   __shared__ BlockReserve<5> br;

@@ -20,12 +20,13 @@
 namespace adept {
 
 // resident blocks per SM asked of the compiler (measured, profiles/r2_summary.md): without a BVH 6 (80 registers, a few
-// bytes of spill; config-2 pass 35.65 -> 35.17 ms over 5 blocks; 7 and 8 blocks: 36.3, 38.2); with the traversal code 5 (96)
+// bytes of spill; config-2 pass 35.65 -> 35.17 ms over 5 blocks; 7 and 8 blocks: 36.3, 38.2); with the traversal code 4 (128 registers; the gamma kernel of a config-4 pass 134.9 -> 124.0 ms over 5 blocks,
+// config 5 32.3 -> 32.9 events/s; 3 blocks: 147.5 ms)
 #ifndef ADEPT_MINB_G2
 #define ADEPT_MINB_G2 6
 #endif
 #ifndef ADEPT_MINB_G2B
-#define ADEPT_MINB_G2B 5
+#define ADEPT_MINB_G2B 4
 #endif
 
 // per-thread outcome counters, 10 bits per field, folded into the block tally every 1023 tiles

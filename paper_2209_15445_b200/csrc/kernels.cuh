@@ -190,6 +190,13 @@ __device__ __forceinline__ void block_reserve(BlockReserve<ND>& br, int phase, c
 #ifndef ADEPT_INNER_MAX
 #define ADEPT_INNER_MAX 32
 #endif
+// e+- in a field and a BVH geometry (configs 4-5), where a looper's step is 16 chords with a traversal each and the
+// showers of the other primaries go on beside it: config 4 ms per pass / config 5 events/s (3 resident blocks) with
+// 32: 980 / 28.6, 16: 937 / 28.7, 12: 918 / 28.4, 8: 897 / 28.1; with the two-block variant for small populations
+// (charged.cuh LOWOCC) 8: 905 / 32.3, 6: 890 / 31.7, 4: 884 / 30.8
+#ifndef ADEPT_INNER_MAX_BVH
+#define ADEPT_INNER_MAX_BVH 8
+#endif
 // Photons and field-free e+- do not loop: their long-lived tracks are few steps from an interaction, and a lane that
 // holds on to its track keeps the secondaries of the others waiting.  Measured (profiles/r2_summary.md): at most 3
 // steps per launch for them, config 1 4.42 -> 3.10 ms, config 2 34.19 -> 33.78 ms per pass (2: 3.19 / 33.73;
