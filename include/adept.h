@@ -139,6 +139,12 @@ typedef struct {
   int32_t use_graphs;      /* 1 (default): a host round of sync_interval population steps is replayed as one CUDA
                               graph per slot (needs an even sync_interval; off while per-launch timing is on or
                               primaries wait for injection); 0: every kernel is launched individually           */
+  int32_t low_occupancy_below; /* BVH geometry in a field only: the e+- move kernel exists in two builds of the same
+                              source, for three resident blocks per SM and for two (255 registers, no spills: faster
+                              where a launch lasts as long as its longest chain of chords and traversals).  A host round
+                              whose population, as the host last saw it, is below this number of tracks launches the
+                              second: 0 (default) = 262 144, < 0 = never.  The two builds agree to rounding, not bit
+                              for bit (the compiler contracts them differently)                                   */
 } adept_config;
 
 typedef struct {

@@ -47,7 +47,7 @@ class CConfig(C.Structure):
                 ("n_event_slots", C.c_int32), ("sync_interval", C.c_int32), ("track_capacity", C.c_uint64),
                 ("leak_capacity", C.c_uint64), ("stage_capacity", C.c_uint64), ("time_kernels", C.c_int32),
                 ("inject_chunk", C.c_uint64), ("pending_capacity", C.c_uint64), ("concurrent_species", C.c_int32), ("steps_per_launch", C.c_int32),
-                ("use_graphs", C.c_int32)]
+                ("use_graphs", C.c_int32), ("low_occupancy_below", C.c_int32)]
 
 
 class CLedger(C.Structure):

@@ -351,6 +351,7 @@ extern "C" void adept_default_config(adept_config* c) {
   c->concurrent_species = 1;
   c->steps_per_launch = 0;
   c->use_graphs = 1;
+  c->low_occupancy_below = 0;
 }
 
 namespace {
@@ -928,7 +929,8 @@ constexpr size_t kMultiBelow = 65536;
 int round_variant(const adept_ctx* ctx, const SlotHost& sh) {
   if (ctx->cfg.steps_per_launch == 1) return 0;
   const size_t population = sh.population + (sh.n_pending - sh.n_injected);
-  if (ctx->k_move_charged[2] && population < static_cast<size_t>(ADEPT_LOWOCC_BELOW)) return 2;
+  const int below = ctx->cfg.low_occupancy_below == 0 ? ADEPT_LOWOCC_BELOW : ctx->cfg.low_occupancy_below;
+  if (ctx->k_move_charged[2] && below > 0 && population < static_cast<size_t>(below)) return 2;
   if (ctx->dev.transit) return 1;   // the multi-step variants also take the passage through a vacuum gap in the same launch
   return population < kMultiBelow ? 1 : 0;
 }

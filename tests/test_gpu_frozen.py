@@ -245,7 +245,12 @@ def test_full_barrel_sampled_frozen_steps(ob, barrel_full):
     check_population(a, o, g, scal, fld, pre[few], ores[few], osec[few], dedx=dedx[few])
     worst_g = check_generic(a, g, scal, fld, pre, ores, osec, dedx)
     a.close()
-    print("worst scaled errors: population", worst_p, "generic", worst_g)
+    # 6e4 tracks are below config.low_occupancy_below: the steps above ran the two-block build of the e+- kernel.
+    # The same states through the three-block build, which transport launches for the populations that fill the GPU:
+    a = adept.Adept(g, tabs, scal, fld, track_capacity=1 << 17, leak_capacity=1 << 17, low_occupancy_below=-1)
+    worst_p3 = check_population(a, o, g, scal, fld, pre, ores, osec, dedx=dedx)
+    a.close()
+    print("worst scaled errors: population", worst_p, "three-block build", worst_p3, "generic", worst_g)
 
 
 def test_degenerate_states(ob, calo):

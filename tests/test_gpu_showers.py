@@ -112,31 +112,35 @@ def test_config4_full_barrel_showers(ob, barrel_full):
         o_led.append(led_e)
         o_steps += np.array(list(st_e.steps), dtype=np.int64)
         o_outcomes = np.array(list(st_e.outcomes), dtype=np.int64) + (0 if o_outcomes is None else o_outcomes)
-    a = adept.Adept(g, tabs, scal, fld, track_capacity=1 << 16, n_event_slots=n_ev + 1, sync_interval=8)
-    same = 0
-    for e in range(n_ev):
-        sel = prim["event"] == e
-        a.enqueue_primaries(e, e, prim["species"][sel], prim["pos"][sel], prim["dir"][sel], prim["ekin"][sel])
-        a.transport(e, torch.cuda.current_stream())
-        hits, led = a.read_scoring(e)
-        assert abs(led.total() - led.primary) <= 1e-9 * led.primary
-        assert led.primary == pytest.approx(o_led[e].primary, rel=1e-14)
-        if np.allclose(hits, o_ev[e], rtol=1e-8, atol=1e-8):
-            same += 1
-            assert led.escaped == pytest.approx(o_led[e].escaped, rel=1e-9, abs=1e-9)
-        else:    # a threshold flip: the shower legitimately diverges, totals stay statistically close
-            assert hits.sum() == pytest.approx(o_ev[e].sum(), rel=0.05)
-    assert same >= n_ev - 1
-    # all events in one population: counts of every outcome equal the oracle's
-    a.enqueue(prim, slot=n_ev)
-    a.transport(n_ev, torch.cuda.current_stream())
-    hits, led = a.read_scoring(n_ev)
-    st = a.stats(n_ev)
-    a.close()
-    if same == n_ev:
-        assert list(st.steps) == list(o_steps) and list(st.outcomes) == list(o_outcomes)
-        np.testing.assert_allclose(hits, o_ev.sum(axis=0), rtol=1e-8, atol=1e-8)
-    assert st.chords > 0 and hits[12:].sum() > 0          # RK4 chords ran, crystals were hit
+    # both builds of the e+- kernel of a BVH geometry in a field (include/adept.h low_occupancy_below): the one for small
+    # populations (default here) and the one transport launches when the population fills the GPU
+    for below in (0, -1):
+        a = adept.Adept(g, tabs, scal, fld, track_capacity=1 << 16, n_event_slots=n_ev + 1, sync_interval=8,
+                        low_occupancy_below=below)
+        same = 0
+        for e in range(n_ev):
+            sel = prim["event"] == e
+            a.enqueue_primaries(e, e, prim["species"][sel], prim["pos"][sel], prim["dir"][sel], prim["ekin"][sel])
+            a.transport(e, torch.cuda.current_stream())
+            hits, led = a.read_scoring(e)
+            assert abs(led.total() - led.primary) <= 1e-9 * led.primary
+            assert led.primary == pytest.approx(o_led[e].primary, rel=1e-14)
+            if np.allclose(hits, o_ev[e], rtol=1e-8, atol=1e-8):
+                same += 1
+                assert led.escaped == pytest.approx(o_led[e].escaped, rel=1e-9, abs=1e-9)
+            else:    # a threshold flip: the shower legitimately diverges, totals stay statistically close
+                assert hits.sum() == pytest.approx(o_ev[e].sum(), rel=0.05)
+        assert same >= n_ev - 1
+        # all events in one population: counts of every outcome equal the oracle's
+        a.enqueue(prim, slot=n_ev)
+        a.transport(n_ev, torch.cuda.current_stream())
+        hits, led = a.read_scoring(n_ev)
+        st = a.stats(n_ev)
+        a.close()
+        if same == n_ev:
+            assert list(st.steps) == list(o_steps) and list(st.outcomes) == list(o_outcomes)
+            np.testing.assert_allclose(hits, o_ev.sum(axis=0), rtol=1e-8, atol=1e-8)
+        assert st.chords > 0 and hits[12:].sum() > 0          # RK4 chords ran, crystals were hit
 
 
 @pytest.mark.parametrize("navigator", [1, 0])
