@@ -296,8 +296,8 @@ struct SlotHost {
   // CUDA graphs of one host round (sync_interval population steps) with the lean [0] and the multi-step [1]
   // move kernels, captured once on `cap` and replayed
   cudaStream_t cap = nullptr;
-  cudaGraphExec_t gexec[3] = {nullptr, nullptr, nullptr};   // per kernel variant (round_variant)
-  bool graph_failed[3] = {false, false, false};
+  cudaGraphExec_t gexec[6] = {};   // per kernel variant (round_variant)
+  bool graph_failed[6] = {};
   // optional per-launch timing (config.time_kernels)
   std::vector<cudaEvent_t> tev;      // [sync_interval][kTimed kernels][start, stop]
   int tev_used = 0;
@@ -846,10 +846,18 @@ extern "C" int adept_enqueue_primaries(adept_ctx* ctx, int slot, uint32_t event_
 
 namespace {
 
+// waves of sparse tiles of a BVH field kernel whose slot has the GPU to itself (round_variant)
+#ifndef ADEPT_SPARSE_WAVES_ALONE
+#define ADEPT_SPARSE_WAVES_ALONE 4
+#endif
+
 // One population step of a slot: gamma move kernel on the caller's stream, charged move kernel on the
 // helper stream (species kernels on different streams, synchronised with events), then the
 // interaction kernel over what they staged and the buffer swap.
-int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity, const DevCtx& dc, int multi) {
+int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity, const DevCtx& dc_in, int variant) {
+  const int multi = variant % 3;   // kernels; variant >= 3: the slot has the GPU to itself (round_variant)
+  DevCtx dc = dc_in;
+  dc.sparse_waves = variant >= 3 ? ADEPT_SPARSE_WAVES_ALONE : 1;
   constexpr int kEv = 2 * ADEPT_N_TIMED_KERNELS;
   if (sh.n_injected < sh.n_pending) {   // staggered injection: the next chunk joins the population of this step
     const size_t m = std::min<size_t>(ctx->cfg.inject_chunk, sh.n_pending - sh.n_injected);
@@ -899,7 +907,7 @@ int launch_iteration(adept_ctx* ctx, SlotHost& sh, cudaStream_t st, int parity, 
 // round.  A small event (config 5: 200 primaries, thousands of nearly empty population steps on each of 16
 // streams) is otherwise bound by the host issuing ~10 API calls per step.  Needs an even sync_interval (every
 // round then starts at parity 0), no per-launch timing and no pending injection; returns false to fall back.
-bool round_graph(adept_ctx* ctx, SlotHost& sh, int multi) {
+bool round_graph(adept_ctx* ctx, SlotHost& sh, int multi /* variant index 0..5 */) {
   if (sh.gexec[multi]) return true;
   if (sh.graph_failed[multi] || !ctx->cfg.use_graphs || (ctx->cfg.sync_interval & 1)) return false;
   if (!sh.cap && cudaStreamCreateWithFlags(&sh.cap, cudaStreamNonBlocking) != cudaSuccess) { sh.graph_failed[multi] = true; return false; }
@@ -926,7 +934,12 @@ constexpr size_t kMultiBelow = 65536;
 #ifndef ADEPT_LOWOCC_BELOW
 #define ADEPT_LOWOCC_BELOW 262144
 #endif
-int round_variant(const adept_ctx* ctx, const SlotHost& sh) {
+// + 3 (`alone`): the call transports one or two slots, so this slot's kernels have the GPU (nearly) to themselves: a BVH
+// field kernel may then spread a small e+- population over several waves of sparse tiles and still take the chord loop
+// with several lanes per track (charged.cuh; config 4 863 -> 820 ms per pass with 4 waves, 832 with 2; with sixteen slots
+// side by side it costs: config 5 33.0 -> 27.5 events/s, which is why it hangs on the number of slots)
+int round_variant(const adept_ctx* ctx, const SlotHost& sh, bool alone = false) {
+  if (alone && ctx->k_move_charged[2]) return 3 + round_variant(ctx, sh, false);
   if (ctx->cfg.steps_per_launch == 1) return 0;
   const size_t population = sh.population + (sh.n_pending - sh.n_injected);
   const int below = ctx->cfg.low_occupancy_below == 0 ? ADEPT_LOWOCC_BELOW : ctx->cfg.low_occupancy_below;
@@ -962,10 +975,10 @@ extern "C" int adept_transport_many(adept_ctx* ctx, int n_slots, const int* slot
   const auto issue_round = [&](int k) -> int {
     SlotHost& sh = ctx->slots[slots[k]];
     cudaStream_t st = static_cast<cudaStream_t>(streams[k]);
-    const int variant = round_variant(ctx, sh);
+    const int variant = round_variant(ctx, sh, n_slots <= 2);
     if (parity[k] == 0 && !ctx->timing_on && sh.n_injected == sh.n_pending && round_graph(ctx, sh, variant)) {
       CUDA_TRY(cudaGraphLaunch(sh.gexec[variant], st));
-      sh.launches += (ctx->k_move_merged[variant] ? 2ull : 3ull) * ctx->cfg.sync_interval;   // kernels of the replayed round
+      sh.launches += (ctx->k_move_merged[variant % 3] ? 2ull : 3ull) * ctx->cfg.sync_interval;   // kernels of the replayed round
     } else {
       for (int it = 0; it < ctx->cfg.sync_interval; ++it) {
         const int rc = launch_iteration(ctx, sh, st, parity[k], ctx->dev, variant);

@@ -23,6 +23,10 @@ namespace adept {
 #ifndef ADEPT_MINB_C2
 #define ADEPT_MINB_C2 6
 #endif
+// fewest lanes per track (as a shift) that take the chord loop in its wide form (field.cuh propagate_wide)
+#ifndef ADEPT_WIDE_MIN_SHIFT
+#define ADEPT_WIDE_MIN_SHIFT 2
+#endif
 #ifndef ADEPT_MINB_C2F
 #define ADEPT_MINB_C2F 4
 #endif
@@ -269,12 +273,13 @@ __device__ __forceinline__ void charged_move_body(const DevCtx& c, const DevSlot
   // (g tracks per tile, one lane in every 128/g): the warp-cooperative BVH serves the queries of a warp
   // one after the other, so a few hundred loopers packed into a few warps would take 32 x 16 chord queries
   // in sequence per step (measured 4 ms per population step on config 4), spread out they run in parallel.
-  // (the two species share the resident blocks: the tiles of both together must fit one wave; at most a warp per track)
+  // (the two species share the resident blocks: the tiles of both together must fit one wave -- DevCtx::sparse_waves of
+  // them in a BVH geometry in a field when the slot has the GPU to itself, adept.cu --; at most a warp per track)
   // (without a field the other species is taken to be as numerous: nothing hangs on it there, and the kernel that fills
   // the GPU on the bench configuration reads one counter less)
   const uint32_t n_other = FIELD == ADEPT_FIELD_NONE ? n : min(cnt->count[parity][species ^ 1].v, c.capacity);   // e- = 0, e+ = 1
   uint32_t g = kBlock;
-  while (g > (kBlock / 32 > 4 ? kBlock / 32 : 4) && (n + (g >> 1) - 1) / (g >> 1) + (n_other + (g >> 1) - 1) / (g >> 1) <= gridDim.x) g >>= 1;
+  while (g > (kBlock / 32 > 4 ? kBlock / 32 : 4) && (n + (g >> 1) - 1) / (g >> 1) + (n_other + (g >> 1) - 1) / (g >> 1) <= gridDim.x * ((FIELD == ADEPT_FIELD_NONE || !BVH) ? 1u : static_cast<uint32_t>(c.sparse_waves))) g >>= 1;
   const int lane_shift = __ffs(kBlock / g) - 1;            // every (1 << lane_shift)-th lane takes a track
   const uint32_t n_tiles = (n + g - 1) / g;
   if (blockIdx.x >= n_tiles) return;   // no tile for this block
@@ -294,7 +299,7 @@ __device__ __forceinline__ void charged_move_body(const DevCtx& c, const DevSlot
   const int t = threadIdx.x >> lane_shift;                 // this lane's entry of the tile
   const bool mine = (threadIdx.x & ((1u << lane_shift) - 1u)) == 0;
   // eight or more lanes per track: they take its chord loop together (field.cuh propagate_wide)
-  const int wide_shift = (MULTI && FIELD != ADEPT_FIELD_NONE && lane_shift >= 3) ? lane_shift : 0;
+  const int wide_shift = (MULTI && FIELD != ADEPT_FIELD_NONE && lane_shift >= ADEPT_WIDE_MIN_SHIFT) ? lane_shift : 0;
   int k_inner = MULTI ? min(inner_steps(c, n, gridDim.x * kBlock, FIELD == ADEPT_FIELD_NONE ? ADEPT_INNER_MAX_STRAIGHT : BVH ? ADEPT_INNER_MAX_BVH : ADEPT_INNER_MAX), 255) : 1;
   // full GPU, BVH geometry: only the passage through the gap a track has just entered from a daughter is taken in
   // the same launch (geom.cuh NavCache)

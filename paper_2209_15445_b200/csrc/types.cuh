@@ -149,6 +149,7 @@ struct DevCtx {
   int32_t chord_budget;
   uint32_t seed, max_steps;
   int32_t steps_per_launch; // adept_config::steps_per_launch (0 = automatic, kernels.cuh inner_steps)
+  int32_t sparse_waves;     // charged.cuh: waves of sparse tiles a BVH field kernel may take (1, or more when the slot has the GPU to itself)
   int32_t transit;          // 1: BVH volumes have per-daughter neighbour lists: a track that leaves a daughter into such a
                             // (vacuum) mother takes the step across the gap in the same launch, whatever the population
   uint32_t capacity;        // per species per buffer
